@@ -1,0 +1,273 @@
+"""Pins for the oracle's plan application (parameters, page table, paged KV) and the linear reference:
+hand-worked golden images, the plain definitions ("new shard == slice of the unsharded tensor",
+"KV_ref readable at its new place") checked through numpy N-d indexing rather than the oracle's own
+offset arithmetic, and the textbook triple loop."""
+import numpy as np
+import pytest
+
+from oracle import linear as OL
+from oracle import planning as OP
+from oracle import state as OS
+from tests import harness as H
+from workloads import get_config
+
+
+# ------------------------------------------------------------------------------------------ golden slab
+def load_slab_golden(golden_dir):
+    g = {"geom": {}, "before": {}, "after": {}, "shard": [], "host": None}
+    for line in open(f"{golden_dir}/slab_tiny.txt"):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = line.split()
+        if w[0] == "geom":
+            g["geom"][int(w[1])] = (int(w[2]), int(w[3]))
+        elif w[0] == "host":
+            g["host"] = (int(w[1]), w[2])
+        elif w[0] in ("before", "after"):
+            g[w[0]][int(w[1])] = w[2]
+        elif w[0] == "shard":
+            g["shard"].append((int(w[1]), int(w[2]), int(w[3]), w[4]))
+    return g
+
+
+def expand(label: str, unit_bytes: int) -> np.ndarray:
+    return np.repeat(np.frombuffer(label.encode(), dtype=np.uint8), unit_bytes).copy()
+
+
+@pytest.mark.parametrize("unit_bytes", [1, 16, 48])
+def test_golden_slab_image(golden_dir, unit_bytes):
+    g = load_slab_golden(golden_dir)
+    old = [(0, 0, 4, 1), (1, 4, 6, 0), (2, 6, 9, 1), (3, 9, 12, 1)]
+    tasks, new = OP.cmm_plan(old, 3)
+    snap = {r: expand(s, unit_bytes) for r, s in g["before"].items()}
+    host0, host = g["host"]
+    out, stats = OS.apply_params(tasks, snap, g["geom"], unit_bytes, expand(host, unit_bytes), host0)
+    for r, s in g["after"].items():
+        assert out[r].tobytes() == expand(s, unit_bytes).tobytes(), f"rank {r}"
+    for (r, b, e, s) in g["shard"]:
+        a, c = g["geom"][r]
+        assert OS.read_units(out[r], a, c, unit_bytes, b, e).tobytes() == expand(s, unit_bytes).tobytes()
+    assert stats == {"d2d_bytes": unit_bytes, "h2d_bytes": 2 * unit_bytes, "kept_bytes": 9 * unit_bytes}
+    # snapshot semantics: the inputs were not modified
+    for r, s in g["before"].items():
+        assert snap[r].tobytes() == expand(s, unit_bytes).tobytes()
+
+
+def test_slot_addressing():
+    assert [OS.slot(u, 6, 4) for u in (6, 7, 8, 4, 5)] == [0, 1, 2, 2, 3]      # golden's r2
+    assert [OS.slot(u, 9, 4) for u in (9, 10, 11, 8)] == [0, 1, 2, 3]           # golden's r3
+    L = OS._lib()
+    for u in range(-20, 40):
+        for anchor in (0, 3, 17):
+            for cap in (1, 4, 7):
+                assert L.oracle_slot(u, anchor, cap) == OS.slot(u, anchor, cap) == ((u - anchor) % cap + cap) % cap
+
+
+# ------------------------------------------------------------------------------------------ plain definition, params
+def check_plain_definition(world, step_idx, out):
+    st = world.steps[step_idx]
+    for sp in world.specs:
+        W = world.unsharded[sp.name].reshape(sp.total_units, sp.unit_bytes)
+        for (r, b, e, _) in st.new[sp.klass]:
+            anchor, cap = world.geom[sp.name][r]
+            S = out[sp.name][r].reshape(cap, sp.unit_bytes)
+            idx = [(u - anchor) % cap for u in range(b, e)]
+            assert len(set(idx)) == len(idx)
+            assert np.array_equal(S[idx], W[b:e]), f"{sp.name} rank {r}: new shard != unsharded slice"
+
+
+def check_untouched(world, step_idx, before, out):
+    st = world.steps[step_idx]
+    for sp in world.specs:
+        for r, a in out[sp.name].items():
+            anchor, cap = world.geom[sp.name][r]
+            written = set()
+            for (k, src, dst, b, e) in st.tasks[sp.klass]:
+                if dst == r and k != OP.KEEP:
+                    written |= {(u - anchor) % cap for u in range(b, e)}
+            S0 = before[sp.name][r].reshape(cap, sp.unit_bytes)
+            S1 = a.reshape(cap, sp.unit_bytes)
+            keep = [s for s in range(cap) if s not in written]
+            assert np.array_equal(S0[keep], S1[keep]), f"{sp.name} rank {r}: bytes outside the plan changed"
+
+
+@pytest.mark.parametrize("mode", ["span", "tight", "full"])
+@pytest.mark.parametrize("policy", ["floor", "ceil_first"])
+@pytest.mark.parametrize("dead", [0, 1, 2, 3])
+def test_config1_params_plain_definition(mode, policy, dead):
+    cfg = get_config("1")
+    world = H.build_param_world(cfg, mode=mode, new_policy=policy, failed=(dead,))
+    out, stats = H.oracle_reshard_params(world, 0)
+    check_plain_definition(world, 0, out)
+    check_untouched(world, 0, world.slabs, out)
+    total = sum(sp.total_units * sp.unit_bytes for sp in world.specs)
+    assert stats["d2d_bytes"] + stats["h2d_bytes"] + stats["kept_bytes"] == total
+
+
+def test_config1_byte_counts_match_survey():
+    """FFN per tensor keep 435 / P2P 69 / reload 184 units of 512 B; heads: reload
+    group 2 -> rank 3, no P2P."""
+    world = H.build_param_world(get_config("1"))
+    _, stats = H.oracle_reshard_params(world, 0)
+    ffn_d2d = 3 * 69 * 512
+    ffn_h2d = 3 * 184 * 512
+    head_h2d = 32768 + 16384 + 16384 + 32768      # wq, wk, wv, wo_t: one KV group each
+    assert stats["d2d_bytes"] == ffn_d2d
+    assert stats["h2d_bytes"] == ffn_h2d + head_h2d
+
+
+def test_sequential_reshards_tiny():
+    """Config-5a style chain on the tiny shape: 4 -> 3 -> 2, each plan from the previous layout."""
+    cfg = get_config("1")
+    for mode in ("span", "tight"):
+        world = H.build_param_world(cfg, mode=mode, failed=(2, 0))
+        cur = world.slabs
+        for i in range(2):
+            out, _ = H.oracle_reshard_params(world, i, cur)
+            check_plain_definition(world, i, out)
+            cur = out
+
+
+# ------------------------------------------------------------------------------------------ page table
+def load_pt_golden(golden_dir):
+    d = {"cases": []}
+    row = lambda s: [[int(x) for x in r.split()] for r in s.split("|")]
+    for line in open(f"{golden_dir}/page_table.txt"):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = line.split(None, 1)
+        if w[0] in ("block_size",):
+            d[w[0]] = int(w[1])
+        elif w[0] in ("seq_lens", "last_use"):
+            d[w[0]] = [int(x) for x in w[1].split()]
+        elif w[0] == "table":
+            d["table"] = np.array(row(w[1]), dtype=np.int32)
+        elif w[0] == "case":
+            budget, ev, tab = [x.strip() for x in w[1].split(":")]
+            ev = [] if ev.split()[1] == "-" else [int(x) for x in ev.split()[1:]]
+            d["cases"].append((int(budget), ev, np.array(row(tab), dtype=np.int32)))
+    return d
+
+
+def test_page_table_golden(golden_dir):
+    d = load_pt_golden(golden_dir)
+    assert len(d["cases"]) == 4
+    for budget, ev, tab in d["cases"]:
+        new, evicted, pairs = OS.page_table_rewrite(d["table"], d["seq_lens"], d["last_use"], d["block_size"], budget)
+        assert evicted == ev, budget
+        assert np.array_equal(new, tab), budget
+
+
+def test_page_table_properties():
+    rng = np.random.default_rng(5)
+    for _ in range(200):
+        n_seqs = int(rng.integers(1, 7))
+        bs = int(rng.choice([1, 4, 16]))
+        lens = rng.integers(0, 6 * bs, n_seqs)
+        from workloads.gen import make_page_table
+        table, lens, last_use, n_blocks = make_page_table(n_seqs, lens, bs, 1.5, int(rng.integers(1 << 30)))
+        per = [-(-int(x) // bs) for x in lens]
+        budget = int(rng.integers(0, n_blocks + 1))
+        new, evicted, pairs = OS.page_table_rewrite(table, lens, last_use, bs, budget)
+        surv = [s for s in range(n_seqs) if s not in evicted]
+        ids = [int(new[s, i]) for s in surv for i in range(per[s])]
+        assert len(set(ids)) == len(ids) and all(0 <= b < budget for b in ids)          # injective, in budget
+        assert sum(per[s] for s in surv) <= budget
+        # LRU order: every evicted sequence is colder than every surviving non-empty sequence
+        for v in evicted:
+            for s in surv:
+                if per[s]:
+                    assert (last_use[v], v) < (last_use[s], s)
+        # minimal eviction: putting the last evicted one back would exceed the budget
+        if evicted:
+            assert sum(per[s] for s in surv) + per[evicted[-1]] > budget
+        # blocks already below the budget never move
+        for (s, i, bo, bn) in pairs:
+            assert (bn == bo) if bo < budget else (bn < budget)
+        for s in evicted:
+            assert (new[s] == -1).all()
+
+
+# ------------------------------------------------------------------------------------------ KV plain definition
+def check_kv_plain_definition(world, st, out, new_table, evicted):
+    g, cfg = world.g, world.cfg
+    owner = {}
+    for (r, b, e, _) in st.new["head"]:
+        for h in range(b, e):
+            owner[h] = r
+    n = 0
+    for s in range(cfg.kv.n_seqs):
+        if s in evicted:
+            continue
+        for t in range(int(world.seq_lens[s])):
+            b = int(new_table[s, t // g.block_size])
+            for l in range(g.n_layers):
+                for c in range(2):
+                    for h in range(cfg.model.n_kv_heads):
+                        r = owner[h]
+                        got = H.kv_get(world, out[r], l, c, b, t % g.block_size, (h - world.anchors[r]) % g.head_cap)
+                        assert np.array_equal(got, world.kv_ref[s, t, l, c, h]), (s, t, l, c, h)
+                        n += 1
+    return n
+
+
+@pytest.mark.parametrize("layout", [0, 1])
+@pytest.mark.parametrize("dead", [0, 1, 2, 3])
+@pytest.mark.parametrize("budget", [None, 12])
+def test_config1_kv_plain_definition(layout, dead, budget):
+    """Config 1 KV: 2 seqs x 128 tokens, block 16 (20-block pool); budget 12 of 20 -> one eviction + relocations."""
+    cfg = get_config("1")
+    world = H.build_kv_world(cfg, layout=layout, failed=(dead,))
+    st = world.steps[0]
+    bud = world.g.n_blocks if budget is None else budget
+    new_table, evicted, pairs = OS.page_table_rewrite(world.table, world.seq_lens, world.last_use,
+                                                      world.g.block_size, bud)
+    if budget is None:
+        assert evicted == [] and np.array_equal(new_table, world.table)
+    else:
+        assert len(evicted) == 1 and any(bo != bn for (_, _, bo, bn) in pairs)
+    snap = {r: p for r, p in world.pools.items() if r != dead}
+    out, stats = OS.apply_kv(st.tasks["head"], snap, world.anchors, world.g, world.host_backup,
+                             world.host_heads, world.host_head0, pairs)
+    n = check_kv_plain_definition(world, st, out, new_table, evicted)
+    assert n > 0
+    # nothing outside live destination blocks changed
+    touched_blocks = {bn for (_, _, _, bn) in pairs}
+    for r in out:
+        v0, v1 = H.kv_view(world, snap[r]), H.kv_view(world, out[r])
+        for b in range(world.g.n_blocks):
+            if b not in touched_blocks:
+                assert np.array_equal(v0[:, :, b], v1[:, :, b])
+
+
+def test_kv_ragged_lengths_and_head_major():
+    cfg = get_config("1")
+    world = H.build_kv_world(cfg, layout=1, seq_lens=[37, 128])
+    st = world.steps[0]
+    new_table, evicted, pairs = OS.page_table_rewrite(world.table, world.seq_lens, world.last_use,
+                                                      world.g.block_size, world.g.n_blocks)
+    snap = {r: p for r, p in world.pools.items() if r != st.dead}
+    out, _ = OS.apply_kv(st.tasks["head"], snap, world.anchors, world.g, world.host_backup,
+                         world.host_heads, world.host_head0, pairs)
+    check_kv_plain_definition(world, st, out, new_table, evicted)
+
+
+# ------------------------------------------------------------------------------------------ linear reference
+def test_linear_ref_is_the_textbook_definition():
+    rng = np.random.default_rng(1)
+    x = rng.standard_normal((3, 17))
+    w = rng.standard_normal((5, 17))
+    np.testing.assert_allclose(OL.linear_ref(x, w), OL.linear_triple_loop(x, w), rtol=1e-12, atol=1e-12)
+    # a transposed operand or a dropped term fails:
+    assert OL.linear_ref(x, w).shape == (3, 5)
+    e = np.eye(4)
+    assert np.array_equal(OL.linear_ref(e, np.arange(16.0).reshape(4, 4)), np.arange(16.0).reshape(4, 4).T)
+
+
+def test_decode16_exact():
+    import torch
+    for name, dt in (("bf16", torch.bfloat16), ("fp16", torch.float16)):
+        t = torch.tensor([0.0, 1.0, -2.5, 0.02, 65504.0 if name == "fp16" else 3.0e38, 1e-3], dtype=dt)
+        got = OL.decode16(t.view(torch.uint8).numpy(), name)
+        assert np.array_equal(got, t.to(torch.float64).numpy())
+    assert OL.max_rel_err(np.array([1.0, 2.0]), np.array([1.0, 2.01])) == pytest.approx(0.01 / 2.01)
