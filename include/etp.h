@@ -1,0 +1,216 @@
+/* etp.h — C ABI of the B200-native Elastic-TP reshard library (libetp.so).
+ *
+ * The hot path of AnchorTP's state-preserving recovery (arxiv 2511.11617; citations are PAPER.md:line):
+ * apply a Continuous Minimal Migration (CMM) plan — rewrite model parameters and a paged KV cache from an
+ * N-rank unequal-width Elastic-TP layout into an M-rank one, moving only the intervals the plan says move,
+ * with the host reload of the failed rank's bytes pipelined beside the device copies.
+ * Every simulated TP rank is a separate allocation on ONE GPU; P2P is an intra-HBM copy.
+ *
+ * Conventions
+ *  - plain C, no exceptions or aborts cross this boundary; every call returns etp_status (0 = OK) and
+ *    etp_last_error() returns a thread-local message for the last failure on the calling thread.
+ *  - the CALLER owns every data buffer (device slabs, KV pools, host image, page table, X/Y); pointers are raw
+ *    (torch.Tensor.data_ptr()) and streams are raw cudaStream_t (torch.cuda.Stream.cuda_stream), passed as void*.
+ *    "device" / "host" / "pinned host" is stated per argument.
+ *  - the LIBRARY owns plan objects, descriptor arenas (pinned + device), the staging ring and its events; they
+ *    live in an etp_ctx / etp_plan and are freed by the matching _destroy / _free.
+ *  - device calls are ASYNCHRONOUS: work is enqueued on the given streams and is complete when the caller has
+ *    synchronised BOTH streams.  Data buffers must stay valid until then.  A ctx may be used from one host
+ *    thread at a time.
+ *  - all byte sizes are int64_t; every base pointer and unit_bytes must be a multiple of 16 (else
+ *    ETP_ERR_ALIGNMENT).  Rank ids are 0-based (Fig. 3 of the paper is 1-based).
+ *  - there is no CPU fallback: without a CUDA device every device call fails with ETP_ERR_CUDA.
+ */
+#ifndef ETP_H_
+#define ETP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    ETP_OK = 0,
+    ETP_ERR_INVALID_ARG = 1,
+    ETP_ERR_ALIGNMENT = 2,
+    ETP_ERR_CAPACITY = 3,     /* a new shard does not fit its slab (width > cap_units) / output array too small */
+    ETP_ERR_NO_SOURCE = 4,    /* a RELOAD task but no host image / backup covering it */
+    ETP_ERR_UNSUPPORTED = 5,  /* fewer units than shards; cyclic write-after-read hazard; bad dtype */
+    ETP_ERR_CUDA = 6,
+    ETP_ERR_NOMEM = 7
+} etp_status;
+
+typedef struct etp_ctx etp_ctx;
+typedef struct etp_plan etp_plan;
+
+/* ------------------------------------------------------------------------------------------------ context */
+
+/* Create a context on CUDA device `device`.  `staging_bytes` (>= 0; 0 = default 256 MiB) sizes the device staging
+ * ring used by the KV reload pipeline (pinned host -> staging by DMA, staging -> head-strided fragments by the
+ * copy kernel).  Fails with ETP_ERR_CUDA if the device is missing or is not compute capability 10.x. */
+etp_status etp_ctx_create(int device, int64_t staging_bytes, etp_ctx** out);
+void etp_ctx_destroy(etp_ctx* ctx);
+const char* etp_last_error(void);
+/* library version string, e.g. "etp 0.1 sm_100a" (static storage) */
+const char* etp_version(void);
+
+typedef enum {
+    ETP_OPT_SKIP_D2D = 0,        /* 1: do not launch the device-copy kernel (time pipeline (b) alone)            */
+    ETP_OPT_SKIP_RELOAD = 1,     /* 1: do not issue reloads (time kernel (a) alone)                              */
+    ETP_OPT_TMA_MIN_BYTES = 2,   /* contiguous intervals >= this go to the cp.async.bulk path (default 32768);
+                                    INT64_MAX disables the TMA path, 0 sends everything 16-B aligned to it       */
+    ETP_OPT_LDG_STEALS_BULK = 3, /* 1 (default): vector-copy warps also drain the bulk queue when theirs is empty */
+    ETP_OPT_RELOAD_CHUNK_BYTES = 4, /* max bytes per cudaMemcpyAsync of the reload pipeline (default 64 MiB)     */
+    ETP_OPT_KV_RELOAD_MODE = 5,  /* 0 (default): DMA to staging ring + scatter kernel; 1: zero-copy gather kernel
+                                    reading pinned host memory directly                                          */
+    ETP_OPT_GRID_CTAS = 6,       /* persistent grid size; 0 (default) = number of SMs                            */
+    ETP_OPT__COUNT
+} etp_option;
+etp_status etp_ctx_set_option(etp_ctx* ctx, etp_option key, int64_t value);
+etp_status etp_ctx_get_option(const etp_ctx* ctx, etp_option key, int64_t* value);
+
+/* ------------------------------------------------------------------------------------------------ S1 partition
+ * "some GPUs hold shard size floor(S/g_t) while others hold ceil(S/g_t)"; Algorithm 1 l.2-5
+ * (PAPER.md:107-110): s_j = floor((j-1)H/M), e_j = floor(jH/M); Fig. 3 (:144): 1024 over 3 -> 0/341/682/1024. */
+typedef enum {
+    ETP_SPLIT_FLOOR_BOUNDARY = 0, /* bounds[j] = floor(j*S/M)  (the paper's formula; wide shards last) */
+    ETP_SPLIT_CEIL_FIRST = 1      /* first S mod M shards get ceil(S/M)  (BASELINE.json config 2: heads 3/3/2) */
+} etp_split_policy;
+typedef enum { ETP_GRAN_HEAD = 0, ETP_GRAN_FFN = 1, ETP_GRAN_EXPERT = 2, ETP_GRAN_VOCAB = 3 } etp_granularity; /* label only */
+
+/* Host-only.  Writes parts+1 non-decreasing bounds, bounds[0] = 0, bounds[parts] = total_units, into bounds_out
+ * (host, caller-owned, parts+1 entries).  align_units >= 1: every interior bound is a multiple of it.
+ * ETP_ERR_UNSUPPORTED if ceil(total_units/align_units) < parts (replication is out of scope). */
+etp_status etp_partition(etp_granularity g, int64_t total_units, int32_t parts, etp_split_policy policy,
+                         int64_t align_units, int64_t* bounds_out);
+
+/* ------------------------------------------------------------------------------------------------ S2 CMM plan
+ * Algorithm 1: Require {(gpu_i, s_i, e_i, alive_i)}, target GPU count M;
+ * Ensure {(gpu_j, sources_j)}.  Intersections with surviving sources become Transfer tasks (Keep when the
+ * source is the owner itself, Fig. 3 "keeps"); uncovered gaps become Reload tasks. */
+typedef struct { int32_t rank; int32_t alive; int64_t begin, end; } etp_shard;   /* (gpu_i, alive_i, s_i, e_i) */
+typedef enum { ETP_KEEP = 0, ETP_TRANSFER = 1, ETP_RELOAD = 2 } etp_task_kind;
+typedef struct { int32_t kind; int32_t src_rank /* -1 for RELOAD */; int32_t dst_rank; int32_t reserved;
+                 int64_t begin, end; } etp_task;
+typedef struct { int64_t total_units, keep_units, transfer_units, reload_units,
+                 reload_lower_bound /* Eq. 1 */, n_tasks; } etp_plan_stats;
+typedef enum { ETP_PLAN_CMM = 0, ETP_PLAN_GREEDY = 1, ETP_PLAN_FULL_RELOAD = 2 } etp_plan_mode;
+
+/* Host-only.  old_layout: n_old entries (host), distinct rank ids, arbitrary intervals.  target_bounds: M+1 bounds
+ * tiling [0,H), H = max end over ALL entries, or NULL for the floor formula.  Target j is owned by the j-th alive
+ * rank in ascending rank id; M must be in 1..#alive.  Tasks are sorted by (dst_rank, begin).  *out is owned by the
+ * library: release with etp_plan_free. */
+etp_status etp_cmm_plan(const etp_shard* old_layout, int32_t n_old, const int64_t* target_bounds, int32_t M,
+                        etp_plan** out);
+/* same with the comparison planners of PAPER.md:204 / Table II (Greedy: no P2P for gaps; Full Reload: no reuse) */
+etp_status etp_plan_create(etp_plan_mode mode, const etp_shard* old_layout, int32_t n_old,
+                           const int64_t* target_bounds, int32_t M, etp_plan** out);
+/* copies up to cap tasks into out (host); *n_out = total number of tasks (call with cap = 0 to size) */
+etp_status etp_plan_tasks(const etp_plan* plan, etp_task* out, int64_t cap, int64_t* n_out);
+/* writes the M new shards (host, M entries), alive = 1 */
+etp_status etp_plan_new_layout(const etp_plan* plan, etp_shard* out, int32_t cap, int32_t* n_out);
+etp_status etp_plan_get_stats(const etp_plan* plan, etp_plan_stats* out);
+void etp_plan_free(etp_plan* plan);
+
+/* ------------------------------------------------------------------------------------------------ S3-S5 parameters
+ * PAPER.md:96 "parameter re-assignment/reloading primitive"; :164-166 pre-allocation, overlap of reloads with P2P.
+ *
+ * Layout contract (L1-L7): a sharded tensor is [total_units][unit_bytes], each unit contiguous.  Rank r keeps
+ * unit u at  slabs[r].base + ((u - anchor_unit) mod cap_units) * unit_bytes ; kept units never change address, a shard
+ * may wrap.  Sources are read with SNAPSHOT semantics (as if every read happened before every write); when a write
+ * would land on bytes another task still has to read, the library orders the copies in hazard phases.
+ * Only bytes of TRANSFER and RELOAD tasks are written; everything else in a slab is left untouched. */
+typedef struct { void* base /* device, 16-B aligned; NULL for a dead rank */; int64_t cap_units; int64_t anchor_unit; } etp_slab;
+typedef struct {
+    int64_t total_units, unit_bytes;
+    const etp_slab* slabs;      /* host array indexed by rank id, n_ranks entries                                   */
+    int32_t n_ranks;
+    int32_t plan_index;         /* which of `plans` drives this tensor (one plan per granularity class)             */
+    const void* host_image;     /* reload source, addressed by global unit: host_image + (u - host_unit0)*unit_bytes.
+                                   PINNED HOST memory (copied by DMA on the reload stream) or DEVICE memory (then
+                                   reloads are lowered into the device-copy kernel).  NULL only if no RELOAD task.  */
+    int64_t host_unit0, host_units;
+} etp_tensor;
+typedef struct {
+    int64_t d2d_bytes;          /* bytes moved device-to-device by TRANSFER tasks (and same-rank KV relocations)   */
+    int64_t h2d_bytes;          /* bytes reloaded from pinned host memory                                          */
+    int64_t reload_dev_bytes;   /* bytes reloaded from a device-resident image (moved by the copy kernel)          */
+    int64_t kept_bytes;         /* bytes of KEEP tasks (never touched)                                             */
+    int64_t n_jobs, n_units;    /* descriptors uploaded / work-queue units                                         */
+    int64_t n_memcpys;          /* cudaMemcpyAsync calls issued by the reload pipeline                             */
+    int32_t n_phases;           /* hazard phases (1 = hazard-free)                                                 */
+    int32_t n_kernel_launches;  /* launches of this library's kernels                                              */
+    double lower_ms;            /* host time spent lowering + enqueueing                                           */
+} etp_reshard_report;
+
+/* tensors: host array.  plans: host array of n_plans plan handles.  copy_stream / reload_stream: cudaStream_t of the
+ * ctx device (may be the same stream; NULL = legacy default stream).  report: host, may be NULL. */
+etp_status etp_reshard_params(etp_ctx* ctx, const etp_tensor* tensors, int32_t n_tensors,
+                              const etp_plan* const* plans, int32_t n_plans,
+                              void* copy_stream, void* reload_stream, etp_reshard_report* report);
+
+/* ------------------------------------------------------------------------------------------------ S3-S6 paged KV
+ * PAPER.md:96 "the KV cache is localized by attention head-groups per token block ... KV-cache operators that support
+ * variable-length shards"; :166 "the runtime KV cache and parameters share the same planning and task generation";
+ * :86 LRU eviction when KV demand exceeds the budget. */
+typedef enum { ETP_KV_TOKEN_MAJOR = 0 /* [block][token][slot][dim] */, ETP_KV_HEAD_MAJOR = 1 /* [block][slot][token][dim] */ } etp_kv_layout;
+typedef struct {
+    int32_t n_layers, n_blocks, block_size, head_cap /* slots per token */, head_dim, elem_bytes;
+    int32_t layout;             /* etp_kv_layout                                                                    */
+    int32_t n_ranks;
+    void* const* pools;         /* host array [n_ranks] of device pointers (NULL for a dead rank);
+                                   pool[r] = [layer][K|V][n_blocks][...layout...], head h at slot (h - head_anchor[r]) mod head_cap */
+    const int64_t* head_anchor; /* host array [n_ranks]                                                             */
+    const void* host_backup;    /* the dead rank's pool compacted to host_heads slots (slot = h - host_head0), same
+                                   layout, indexed by the OLD physical block id.  Pinned host or device memory; NULL =>
+                                   reload heads are left untouched and every live sequence is reported evicted.     */
+    int32_t host_heads; int64_t host_head0;
+} etp_kv_geometry;
+typedef struct {
+    int32_t n_seqs, max_blocks;
+    int32_t* block_table;       /* host [n_seqs][max_blocks], in/out, -1 = none                                     */
+    const int32_t* seq_lens;    /* host [n_seqs]                                                                    */
+    const int64_t* last_use;    /* host [n_seqs], larger = more recent                                              */
+} etp_page_table;
+
+/* Host-only page-table rule (K5): (i) while live blocks > budget evict the sequence with the smallest last_use
+ * (tie: smaller index), its row becomes -1; (ii) every surviving block with id >= budget moves, in ascending (seq, logical
+ * index), to the smallest id < budget not used by a surviving block.  pairs_out (host, may be NULL, cap entries of
+ * {old id, new id}) receives every surviving live block.  evicted_out: host [n_seqs]. */
+etp_status etp_page_table_rewrite(etp_page_table* pt, int32_t block_size, int32_t new_block_budget,
+                                  int32_t* evicted_out, int32_t* n_evicted,
+                                  int32_t* pairs_out, int64_t pairs_cap, int64_t* n_pairs);
+
+/* Rewrites the page table (above), then moves KV-head slices of every surviving live block according to head_plan
+ * (unit = KV head): TRANSFER heads between pools, RELOAD heads from the backup, KEEP heads only when their block was
+ * relocated.  Free blocks are never copied. */
+etp_status etp_reshard_kv(etp_ctx* ctx, const etp_kv_geometry* geom, etp_page_table* pt, const etp_plan* head_plan,
+                          int32_t new_block_budget, int32_t* evicted_seqs_out, int32_t* n_evicted,
+                          void* copy_stream, void* reload_stream, etp_reshard_report* report);
+
+/* ------------------------------------------------------------------------------------------------ S7 shard linear
+ * unequal-width sharding for linear layers.  Computes, on the sharded weight as it sits in the
+ * slabs, Y[tokens][out_features] = X[tokens][in_features] · W^T with fp32 accumulation and one rounding to 16 bit:
+ *   ETP_COL_PARALLEL: the weight is cut along out-features; w is stored [out][in]; rank r produces its columns of Y.
+ *   ETP_ROW_PARALLEL: the weight is cut along in-features; w is stored transposed [in][out]; the rank partial sums
+ *                     are accumulated in one fp32 accumulator in ascending unit order (no second pass).
+ * w->unit_bytes = features_per_unit * (row length) * 2.  x, y: device, 16-B aligned, row-major, same dtype as w. */
+typedef enum { ETP_COL_PARALLEL = 0, ETP_ROW_PARALLEL = 1 } etp_linear_mode;
+typedef enum { ETP_BF16 = 0, ETP_FP16 = 1 } etp_dtype;
+etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype,
+                            const void* x, int64_t tokens, int64_t in_features, int64_t out_features,
+                            const etp_tensor* w, const etp_shard* layout, int32_t n_shards,
+                            int64_t features_per_unit, void* y, void* stream);
+
+/* ------------------------------------------------------------------------------------------------ microbenchmark entry
+ * Copies n arbitrary intervals with the same persistent kernel (config 5b).  host_descs: host array; src/dst: device,
+ * 16-B aligned; bytes: multiple of 16.  Destinations must be mutually disjoint and disjoint from every source. */
+typedef struct { const void* src; void* dst; int64_t bytes; } etp_interval;
+etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_descs, int64_t n, void* stream,
+                              etp_reshard_report* report);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ETP_H_ */
