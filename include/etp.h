@@ -60,11 +60,13 @@ typedef enum {
     ETP_OPT_SKIP_RELOAD = 1,     /* 1: do not issue reloads (time kernel (a) alone)                              */
     ETP_OPT_TMA_MIN_BYTES = 2,   /* contiguous intervals >= this go to the cp.async.bulk path (default 32768);
                                     INT64_MAX disables the TMA path, 0 sends everything 16-B aligned to it       */
-    ETP_OPT_LDG_STEALS_BULK = 3, /* 1 (default): vector-copy warps also drain the bulk queue when theirs is empty */
+    ETP_OPT_LDG_STEALS_BULK = 3, /* 1 (default 0): vector-copy warps also drain the bulk queue when theirs is empty */
     ETP_OPT_RELOAD_CHUNK_BYTES = 4, /* max bytes per cudaMemcpyAsync of the reload pipeline (default 64 MiB)     */
-    ETP_OPT_KV_RELOAD_MODE = 5,  /* 0 (default): DMA to staging ring + scatter kernel; 1: zero-copy gather kernel
-                                    reading pinned host memory directly                                          */
+    ETP_OPT_KV_RELOAD_MODE = 5,  /* 0 (default): zero-copy gather - the copy kernel reads the pinned backup over the
+                                    host link and writes the head-strided fragments in place; 1: DMA of whole
+                                    (layer, K|V) planes to the staging ring + scatter by the copy kernel           */
     ETP_OPT_GRID_CTAS = 6,       /* persistent grid size; 0 (default) = number of SMs                            */
+    ETP_OPT_GATHER_CTAS = 7,     /* CTAs of the zero-copy gather launch on the reload stream (default 16)        */
     ETP_OPT__COUNT
 } etp_option;
 etp_status etp_ctx_set_option(etp_ctx* ctx, etp_option key, int64_t value);

@@ -1,0 +1,328 @@
+"""Thin ctypes binding of libetp.so (include/etp.h).  Argument marshalling only — every step of the hot path runs
+inside the library.  Names follow the C ABI.  There is no CPU fallback: if the library is missing or no sm_100 device
+is present, the device calls raise EtpError."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, List, Optional, Sequence, Tuple
+
+from . import _build
+
+i32, i64, vp = C.c_int32, C.c_int64, C.c_void_p
+
+ETP_OK = 0
+STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALIGNMENT", 3: "CAPACITY", 4: "NO_SOURCE", 5: "UNSUPPORTED", 6: "CUDA", 7: "NOMEM"}
+KEEP, TRANSFER, RELOAD = 0, 1, 2
+SPLIT = {"floor": 0, "ceil_first": 1}
+GRAN = {"head": 0, "ffn": 1, "expert": 2, "vocab": 3}
+PLAN_CMM, PLAN_GREEDY, PLAN_FULL_RELOAD = 0, 1, 2
+COL_PARALLEL, ROW_PARALLEL = 0, 1
+DTYPE = {"bf16": 0, "fp16": 1}
+KV_TOKEN_MAJOR, KV_HEAD_MAJOR = 0, 1
+(OPT_SKIP_D2D, OPT_SKIP_RELOAD, OPT_TMA_MIN_BYTES, OPT_LDG_STEALS_BULK, OPT_RELOAD_CHUNK_BYTES, OPT_KV_RELOAD_MODE,
+ OPT_GRID_CTAS, OPT_GATHER_CTAS) = range(8)
+
+
+class EtpError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"ETP_ERR_{STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class etp_shard(C.Structure):
+    _fields_ = [("rank", i32), ("alive", i32), ("begin", i64), ("end", i64)]
+
+
+class etp_task(C.Structure):
+    _fields_ = [("kind", i32), ("src_rank", i32), ("dst_rank", i32), ("reserved", i32), ("begin", i64), ("end", i64)]
+
+
+class etp_plan_stats(C.Structure):
+    _fields_ = [(n, i64) for n in ("total_units", "keep_units", "transfer_units", "reload_units", "reload_lower_bound", "n_tasks")]
+
+
+class etp_slab(C.Structure):
+    _fields_ = [("base", vp), ("cap_units", i64), ("anchor_unit", i64)]
+
+
+class etp_tensor(C.Structure):
+    _fields_ = [("total_units", i64), ("unit_bytes", i64), ("slabs", C.POINTER(etp_slab)), ("n_ranks", i32), ("plan_index", i32),
+                ("host_image", vp), ("host_unit0", i64), ("host_units", i64)]
+
+
+class etp_reshard_report(C.Structure):
+    _fields_ = [("d2d_bytes", i64), ("h2d_bytes", i64), ("reload_dev_bytes", i64), ("kept_bytes", i64), ("n_jobs", i64), ("n_units", i64),
+                ("n_memcpys", i64), ("n_phases", i32), ("n_kernel_launches", i32), ("lower_ms", C.c_double)]
+
+    def as_dict(self) -> Dict[str, float]:
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class etp_kv_geometry(C.Structure):
+    _fields_ = [("n_layers", i32), ("n_blocks", i32), ("block_size", i32), ("head_cap", i32), ("head_dim", i32), ("elem_bytes", i32),
+                ("layout", i32), ("n_ranks", i32), ("pools", C.POINTER(vp)), ("head_anchor", C.POINTER(i64)),
+                ("host_backup", vp), ("host_heads", i32), ("host_head0", i64)]
+
+
+class etp_page_table(C.Structure):
+    _fields_ = [("n_seqs", i32), ("max_blocks", i32), ("block_table", C.POINTER(i32)), ("seq_lens", C.POINTER(i32)),
+                ("last_use", C.POINTER(i64))]
+
+
+class etp_interval(C.Structure):
+    _fields_ = [("src", vp), ("dst", vp), ("bytes", i64)]
+
+
+EXPORTS = ["etp_ctx_create", "etp_ctx_destroy", "etp_last_error", "etp_version", "etp_ctx_set_option", "etp_ctx_get_option",
+           "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_tasks", "etp_plan_new_layout", "etp_plan_get_stats",
+           "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
+           "etp_copy_intervals"]
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads (building first if stale) libetp.so.  Fails loudly if it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        so = _build.build()
+        L = C.CDLL(so)
+        L.etp_last_error.restype = C.c_char_p
+        L.etp_version.restype = C.c_char_p
+        L.etp_ctx_create.argtypes = [C.c_int, i64, C.POINTER(vp)]
+        L.etp_ctx_destroy.argtypes = [vp]
+        L.etp_ctx_destroy.restype = None
+        L.etp_ctx_set_option.argtypes = [vp, C.c_int, i64]
+        L.etp_ctx_get_option.argtypes = [vp, C.c_int, C.POINTER(i64)]
+        L.etp_partition.argtypes = [C.c_int, i64, i32, C.c_int, i64, C.POINTER(i64)]
+        L.etp_cmm_plan.argtypes = [C.POINTER(etp_shard), i32, C.POINTER(i64), i32, C.POINTER(vp)]
+        L.etp_plan_create.argtypes = [C.c_int, C.POINTER(etp_shard), i32, C.POINTER(i64), i32, C.POINTER(vp)]
+        L.etp_plan_tasks.argtypes = [vp, C.POINTER(etp_task), i64, C.POINTER(i64)]
+        L.etp_plan_new_layout.argtypes = [vp, C.POINTER(etp_shard), i32, C.POINTER(i32)]
+        L.etp_plan_get_stats.argtypes = [vp, C.POINTER(etp_plan_stats)]
+        L.etp_plan_free.argtypes = [vp]
+        L.etp_plan_free.restype = None
+        L.etp_reshard_params.argtypes = [vp, C.POINTER(etp_tensor), i32, C.POINTER(vp), i32, vp, vp, C.POINTER(etp_reshard_report)]
+        L.etp_page_table_rewrite.argtypes = [C.POINTER(etp_page_table), i32, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), i64,
+                                             C.POINTER(i64)]
+        L.etp_reshard_kv.argtypes = [vp, C.POINTER(etp_kv_geometry), C.POINTER(etp_page_table), vp, i32, C.POINTER(i32), C.POINTER(i32),
+                                     vp, vp, C.POINTER(etp_reshard_report)]
+        L.etp_shard_linear.argtypes = [vp, C.c_int, C.c_int, vp, i64, i64, i64, C.POINTER(etp_tensor), C.POINTER(etp_shard), i32, i64,
+                                       vp, vp]
+        L.etp_copy_intervals.argtypes = [vp, C.POINTER(etp_interval), i64, vp, C.POINTER(etp_reshard_report)]
+        _lib = L
+    return _lib
+
+
+def _check(status: int) -> None:
+    if status != ETP_OK:
+        raise EtpError(status, lib().etp_last_error().decode())
+
+
+def etp_version() -> str:
+    return lib().etp_version().decode()
+
+
+# ------------------------------------------------------------------------------------------------ S1 / S2 (host)
+def etp_partition(total_units: int, parts: int, policy: str = "floor", align_units: int = 1, granularity: str = "ffn") -> List[int]:
+    out = (i64 * (parts + 1 if parts >= 0 else 1))()
+    _check(lib().etp_partition(GRAN[granularity], total_units, parts, SPLIT[policy], align_units, out))
+    return list(out)
+
+
+Shard = Tuple[int, int, int, int]  # (rank, begin, end, alive) — the tuple order used by the tests' harness
+
+
+def _shards(layout: Sequence[Shard]):
+    arr = (etp_shard * max(len(layout), 1))()
+    for k, (r, b, e, a) in enumerate(layout):
+        arr[k] = etp_shard(int(r), int(a), int(b), int(e))
+    return arr
+
+
+class Plan:
+    """Owns an etp_plan handle."""
+
+    def __init__(self, handle: int):
+        self.handle = vp(handle)
+
+    def __del__(self):
+        if getattr(self, "handle", None) and _lib is not None:
+            _lib.etp_plan_free(self.handle)
+            self.handle = None
+
+    def tasks(self) -> List[Tuple[int, int, int, int, int]]:
+        n = i64()
+        _check(lib().etp_plan_tasks(self.handle, None, 0, C.byref(n)))
+        arr = (etp_task * max(n.value, 1))()
+        _check(lib().etp_plan_tasks(self.handle, arr, n.value, C.byref(n)))
+        return [(t.kind, t.src_rank, t.dst_rank, t.begin, t.end) for t in arr[: n.value]]
+
+    def new_layout(self) -> List[Shard]:
+        n = i32()
+        _check(lib().etp_plan_new_layout(self.handle, None, 0, C.byref(n)))
+        arr = (etp_shard * max(n.value, 1))()
+        _check(lib().etp_plan_new_layout(self.handle, arr, n.value, C.byref(n)))
+        return [(s.rank, s.begin, s.end, s.alive) for s in arr[: n.value]]
+
+    def stats(self) -> Dict[str, int]:
+        st = etp_plan_stats()
+        _check(lib().etp_plan_get_stats(self.handle, C.byref(st)))
+        return {n: getattr(st, n) for n, _ in st._fields_}
+
+
+def etp_plan_create(mode: int, old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None) -> Plan:
+    h = vp()
+    tb = None
+    if target_bounds is not None:
+        tb = (i64 * len(target_bounds))(*[int(x) for x in target_bounds])
+    _check(lib().etp_plan_create(mode, _shards(old_layout), len(old_layout), tb, M, C.byref(h)))
+    return Plan(h.value)
+
+
+def etp_cmm_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None) -> Plan:
+    h = vp()
+    tb = None
+    if target_bounds is not None:
+        tb = (i64 * len(target_bounds))(*[int(x) for x in target_bounds])
+    _check(lib().etp_cmm_plan(_shards(old_layout), len(old_layout), tb, M, C.byref(h)))
+    return Plan(h.value)
+
+
+def etp_page_table_rewrite(table, seq_lens, last_use, block_size: int, budget: int):
+    """table: numpy int32 [n_seqs][max_blocks] (modified in place).  Returns (evicted list, pairs [(old, new)])."""
+    import numpy as np
+    assert table.dtype == np.int32 and table.flags["C_CONTIGUOUS"]
+    sl = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    lu = np.ascontiguousarray(last_use, dtype=np.int64)
+    n_seqs, max_blocks = table.shape
+    pt = etp_page_table(n_seqs, max_blocks, table.ctypes.data_as(C.POINTER(i32)), sl.ctypes.data_as(C.POINTER(i32)),
+                        lu.ctypes.data_as(C.POINTER(i64)))
+    cap = int(((sl.astype(np.int64) + block_size - 1) // block_size).sum()) if block_size > 0 else 0
+    pairs = np.zeros((max(cap, 1), 2), dtype=np.int32)
+    ev = np.zeros(max(n_seqs, 1), dtype=np.int32)
+    n_ev, n_pairs = i32(), i64()
+    _check(lib().etp_page_table_rewrite(C.byref(pt), block_size, budget, ev.ctypes.data_as(C.POINTER(i32)), C.byref(n_ev),
+                                        pairs.ctypes.data_as(C.POINTER(i32)), cap, C.byref(n_pairs)))
+    return [int(v) for v in ev[: n_ev.value]], [(int(a), int(b)) for a, b in pairs[: n_pairs.value]]
+
+
+# ------------------------------------------------------------------------------------------------ device calls
+class Context:
+    """Owns an etp_ctx (descriptor arenas, staging ring, events) on one CUDA device."""
+
+    def __init__(self, device: int = 0, staging_bytes: int = 0):
+        h = vp()
+        _check(lib().etp_ctx_create(device, staging_bytes, C.byref(h)))
+        self.handle = h
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lib().etp_ctx_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, key: int, value: int) -> None:
+        _check(lib().etp_ctx_set_option(self.handle, key, value))
+
+    def get_option(self, key: int) -> int:
+        v = i64()
+        _check(lib().etp_ctx_get_option(self.handle, key, C.byref(v)))
+        return v.value
+
+
+class TensorDesc:
+    """Python-side description of one sharded tensor: slabs = {rank: (device ptr, cap_units, anchor_unit)}."""
+
+    def __init__(self, total_units: int, unit_bytes: int, slabs: Dict[int, Tuple[int, int, int]], n_ranks: int, plan_index: int,
+                 host_image: int = 0, host_unit0: int = 0, host_units: int = 0):
+        self.total_units, self.unit_bytes, self.slabs, self.n_ranks = total_units, unit_bytes, slabs, n_ranks
+        self.plan_index, self.host_image, self.host_unit0, self.host_units = plan_index, host_image, host_unit0, host_units
+
+
+def _marshal_tensors(tensors: Sequence[TensorDesc]):
+    arr = (etp_tensor * max(len(tensors), 1))()
+    keep = []
+    for k, t in enumerate(tensors):
+        sl = (etp_slab * max(t.n_ranks, 1))()
+        for r in range(t.n_ranks):
+            base, cap, anchor = t.slabs.get(r, (0, 0, 0))
+            sl[r] = etp_slab(base or None, cap, anchor)
+        keep.append(sl)
+        arr[k] = etp_tensor(t.total_units, t.unit_bytes, sl, t.n_ranks, t.plan_index, t.host_image or None, t.host_unit0, t.host_units)
+    return arr, keep
+
+
+def etp_reshard_params(ctx: Context, tensors: Sequence[TensorDesc], plans: Sequence[Plan], copy_stream: int = 0,
+                       reload_stream: int = 0) -> Dict[str, float]:
+    arr, keep = _marshal_tensors(tensors)
+    ph = (vp * max(len(plans), 1))(*[p.handle for p in plans])
+    rep = etp_reshard_report()
+    _check(lib().etp_reshard_params(ctx.handle, arr, len(tensors), ph, len(plans), copy_stream or None, reload_stream or None, C.byref(rep)))
+    del keep
+    return rep.as_dict()
+
+
+class PreparedParams:
+    """Pre-marshalled arguments of etp_reshard_params, so that a timed loop pays only the C call."""
+
+    def __init__(self, tensors: Sequence[TensorDesc], plans: Sequence[Plan]):
+        self.arr, self._keep = _marshal_tensors(tensors)
+        self.n = len(tensors)
+        self.plans = list(plans)
+        self.ph = (vp * max(len(plans), 1))(*[p.handle for p in plans])
+
+    def run(self, ctx: Context, copy_stream: int = 0, reload_stream: int = 0) -> Dict[str, float]:
+        rep = etp_reshard_report()
+        _check(lib().etp_reshard_params(ctx.handle, self.arr, self.n, self.ph, len(self.plans), copy_stream or None, reload_stream or None,
+                                        C.byref(rep)))
+        return rep.as_dict()
+
+
+def etp_reshard_kv(ctx: Context, *, n_layers: int, n_blocks: int, block_size: int, head_cap: int, head_dim: int, elem_bytes: int,
+                   layout: int, pools: Dict[int, int], head_anchor: Dict[int, int], n_ranks: int, table, seq_lens, last_use,
+                   head_plan: Plan, new_block_budget: int, host_backup: int = 0, host_heads: int = 0, host_head0: int = 0,
+                   copy_stream: int = 0, reload_stream: int = 0):
+    """table: numpy int32 [n_seqs][max_blocks], rewritten in place.  Returns (evicted seq ids, report dict)."""
+    import numpy as np
+    assert table.dtype == np.int32 and table.flags["C_CONTIGUOUS"]
+    sl = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    lu = np.ascontiguousarray(last_use, dtype=np.int64)
+    pool_arr = (vp * n_ranks)(*[(pools.get(r) or None) for r in range(n_ranks)])
+    anchor_arr = (i64 * n_ranks)(*[int(head_anchor.get(r, 0)) for r in range(n_ranks)])
+    g = etp_kv_geometry(n_layers, n_blocks, block_size, head_cap, head_dim, elem_bytes, layout, n_ranks, pool_arr, anchor_arr,
+                        host_backup or None, host_heads, host_head0)
+    n_seqs, max_blocks = table.shape
+    pt = etp_page_table(n_seqs, max_blocks, table.ctypes.data_as(C.POINTER(i32)), sl.ctypes.data_as(C.POINTER(i32)),
+                        lu.ctypes.data_as(C.POINTER(i64)))
+    ev = np.zeros(max(n_seqs, 1), dtype=np.int32)
+    n_ev = i32()
+    rep = etp_reshard_report()
+    _check(lib().etp_reshard_kv(ctx.handle, C.byref(g), C.byref(pt), head_plan.handle, new_block_budget, ev.ctypes.data_as(C.POINTER(i32)),
+                                C.byref(n_ev), copy_stream or None, reload_stream or None, C.byref(rep)))
+    return [int(v) for v in ev[: n_ev.value]], rep.as_dict()
+
+
+def etp_shard_linear(ctx: Context, mode: int, dtype: str, x_ptr: int, tokens: int, in_features: int, out_features: int,
+                     w: TensorDesc, layout: Sequence[Shard], features_per_unit: int, y_ptr: int, stream: int = 0) -> None:
+    arr, keep = _marshal_tensors([w])
+    _check(lib().etp_shard_linear(ctx.handle, mode, DTYPE[dtype], x_ptr, tokens, in_features, out_features, arr, _shards(layout),
+                                  len(layout), features_per_unit, y_ptr, stream or None))
+    del keep
+
+
+def etp_copy_intervals(ctx: Context, src_ptrs, dst_ptrs, sizes, stream: int = 0) -> Dict[str, float]:
+    """src_ptrs / dst_ptrs / sizes: numpy int64 arrays of absolute device addresses and byte counts."""
+    import numpy as np
+    n = len(sizes)
+    rec = np.empty((n, 3), dtype=np.int64)
+    rec[:, 0], rec[:, 1], rec[:, 2] = src_ptrs, dst_ptrs, sizes
+    rep = etp_reshard_report()
+    _check(lib().etp_copy_intervals(ctx.handle, rec.ctypes.data_as(C.POINTER(etp_interval)), n, stream or None, C.byref(rep)))
+    return rep.as_dict()

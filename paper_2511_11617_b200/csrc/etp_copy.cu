@@ -1,0 +1,234 @@
+#include "etp_copy.cuh"
+
+namespace etp {
+namespace {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t"
+        "}" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+// global -> shared, completion counted in bytes on an mbarrier
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, uint64_t src_gmem, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem),
+                 "l"(src_gmem), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+// shared -> global, completion tracked by the thread's bulk async-group
+__device__ __forceinline__ void bulk_s2g(uint64_t dst_gmem, uint32_t src_smem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(src_smem), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+__device__ __forceinline__ uint4 ld_stream(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream(void* p, const uint4& v) {
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------- bulk (TMA) driver
+// One thread.  Chunks (<= kStageBytes) of successive jobs flow through the ring; `loaded - stored <= kLookahead`.
+__device__ void tma_driver(const CopyArgs& a, uint8_t* ring, uint64_t* full_bar, uint64_t* s_dst, uint32_t* s_bytes) {
+    uint32_t loaded = 0, stored = 0;
+    uint64_t cur_src = 0, cur_dst = 0, cur_left = 0;
+    bool exhausted = a.n_bulk == 0;
+    for (;;) {
+        bool progressed = false;
+        if (!exhausted) {
+            if (cur_left == 0) {
+                const unsigned int idx = atomicAdd(&a.counters[0], 1u);
+                if (idx < a.n_bulk) {
+                    const uint4 lo = __ldg(reinterpret_cast<const uint4*>(a.bulk + idx));
+                    const uint2 hi = __ldg(reinterpret_cast<const uint2*>(a.bulk + idx) + 2);
+                    cur_src = (uint64_t)lo.x | ((uint64_t)lo.y << 32);
+                    cur_dst = (uint64_t)lo.z | ((uint64_t)lo.w << 32);
+                    cur_left = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
+                } else {
+                    exhausted = true;
+                }
+            }
+            if (cur_left != 0) {
+                const uint32_t n = cur_left > (uint64_t)kStageBytes ? (uint32_t)kStageBytes : (uint32_t)cur_left;
+                const uint32_t st = loaded % kStages;
+                // the stage was last used by chunk loaded-kStages; its store is one of the committed groups and at most
+                // kStages-1-kLookahead younger groups may still be reading shared memory
+                if (loaded >= (uint32_t)kStages) bulk_wait_read<kStages - 1 - kLookahead>();
+                const uint32_t bar = smem_u32(&full_bar[st]);
+                mbar_arrive_expect_tx(bar, n);
+                bulk_g2s(smem_u32(ring + (size_t)st * kStageBytes), cur_src, n, bar);
+                s_dst[st] = cur_dst;
+                s_bytes[st] = n;
+                cur_src += n;
+                cur_dst += n;
+                cur_left -= n;
+                ++loaded;
+                progressed = true;
+            }
+        }
+        if (stored < loaded && (loaded - stored > (uint32_t)kLookahead || exhausted)) {
+            const uint32_t st = stored % kStages;
+            mbar_wait(smem_u32(&full_bar[st]), (stored / kStages) & 1u);
+            bulk_s2g(s_dst[st], smem_u32(ring + (size_t)st * kStageBytes), s_bytes[st]);
+            bulk_commit();
+            ++stored;
+            progressed = true;
+        }
+        if (!progressed) break;
+    }
+    bulk_wait_all();
+}
+
+// ---------------------------------------------------------------------------------------------- vector-copy warps
+constexpr int kUnroll = 8;
+
+__device__ __forceinline__ void copy_linear(const char* __restrict__ src, char* __restrict__ dst, uint32_t n_vec, int lane) {
+    uint32_t v = lane;
+    for (; v + 32 * (kUnroll - 1) < n_vec; v += 32 * kUnroll) {
+        uint4 buf[kUnroll];
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) buf[u] = ld_stream(src + (size_t)(v + 32 * u) * 16);
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) st_stream(dst + (size_t)(v + 32 * u) * 16, buf[u]);
+    }
+    for (; v < n_vec; v += 32) st_stream(dst + (size_t)v * 16, ld_stream(src + (size_t)v * 16));
+}
+
+__device__ __forceinline__ void frag_offsets(const FragJob& j, uint32_t v, uint32_t vs, uint32_t gs, uint32_t vpr, int64_t* so, int64_t* d_o) {
+    uint32_t row, col;
+    if (vs != 0xFFu) {
+        row = v >> vs;
+        col = v & (vpr - 1);
+    } else {
+        row = v / vpr;
+        col = v - row * vpr;
+    }
+    uint32_t grp, r;
+    if (gs != 0xFFu) {
+        grp = row >> gs;
+        r = row & (j.rows_per_group - 1);
+    } else {
+        grp = row / j.rows_per_group;
+        r = row - grp * j.rows_per_group;
+    }
+    *so = (int64_t)grp * j.s_grp + (int64_t)r * j.s_row + (int64_t)col * 16;
+    *d_o = (int64_t)grp * j.d_grp + (int64_t)r * j.d_row + (int64_t)col * 16;
+}
+
+__device__ void copy_frag_job(const FragJob& j, int lane) {
+    const char* src = reinterpret_cast<const char*>(j.src);
+    char* dst = reinterpret_cast<char*>(j.dst);
+    if (j.n_rows == 1) {
+        copy_linear(src, dst, j.row_bytes >> 4, lane);
+        return;
+    }
+    const uint32_t vs = j.vec_shift & 0xFFu, gs = (j.vec_shift >> 8) & 0xFFu;
+    const uint32_t vpr = j.row_bytes >> 4;
+    const uint32_t total = j.n_rows * vpr;
+    uint32_t v = lane;
+    for (; v + 32 * (kUnroll - 1) < total; v += 32 * kUnroll) {
+        uint4 buf[kUnroll];
+        int64_t d_o[kUnroll];
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) {
+            int64_t so;
+            frag_offsets(j, v + 32 * u, vs, gs, vpr, &so, &d_o[u]);
+            buf[u] = ld_stream(src + so);
+        }
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) st_stream(dst + d_o[u], buf[u]);
+    }
+    for (; v < total; v += 32) {
+        int64_t so, d_o;
+        frag_offsets(j, v, vs, gs, vpr, &so, &d_o);
+        st_stream(dst + d_o, ld_stream(src + so));
+    }
+}
+
+__device__ void vector_warp(const CopyArgs& a, int lane) {
+    for (;;) {
+        unsigned int idx = 0;
+        if (lane == 0) idx = atomicAdd(&a.counters[1], 1u);
+        idx = __shfl_sync(0xffffffffu, idx, 0);
+        if (idx >= a.n_frag) break;
+        FragJob j;
+        const uint4* p = reinterpret_cast<const uint4*>(a.frag + idx);
+        uint4 q0 = __ldg(p), q1 = __ldg(p + 1), q2 = __ldg(p + 2), q3 = __ldg(p + 3);
+        j.src = (uint64_t)q0.x | ((uint64_t)q0.y << 32);
+        j.dst = (uint64_t)q0.z | ((uint64_t)q0.w << 32);
+        j.row_bytes = q1.x; j.n_rows = q1.y; j.rows_per_group = q1.z; j.vec_shift = q1.w;
+        j.s_row = (int64_t)((uint64_t)q2.x | ((uint64_t)q2.y << 32));
+        j.d_row = (int64_t)((uint64_t)q2.z | ((uint64_t)q2.w << 32));
+        j.s_grp = (int64_t)((uint64_t)q3.x | ((uint64_t)q3.y << 32));
+        j.d_grp = (int64_t)((uint64_t)q3.z | ((uint64_t)q3.w << 32));
+        copy_frag_job(j, lane);
+    }
+    if (a.flags & 1u) {
+        // drain the bulk queue too (one job per warp at a time)
+        for (;;) {
+            unsigned int idx = 0;
+            if (lane == 0) idx = atomicAdd(&a.counters[0], 1u);
+            idx = __shfl_sync(0xffffffffu, idx, 0);
+            if (idx >= a.n_bulk) break;
+            const uint4 lo = __ldg(reinterpret_cast<const uint4*>(a.bulk + idx));
+            const uint2 hi = __ldg(reinterpret_cast<const uint2*>(a.bulk + idx) + 2);
+            const char* src = reinterpret_cast<const char*>((uint64_t)lo.x | ((uint64_t)lo.y << 32));
+            char* dst = reinterpret_cast<char*>((uint64_t)lo.z | ((uint64_t)lo.w << 32));
+            const uint64_t bytes = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
+            copy_linear(src, dst, (uint32_t)(bytes >> 4), lane);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kCopyThreads, 1) etp_interval_copy_kernel(const CopyArgs a) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* ring = smem;
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + (size_t)kStages * kStageBytes);
+    uint64_t* s_dst = full_bar + kStages;
+    uint32_t* s_bytes = reinterpret_cast<uint32_t*>(s_dst + kStages);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp == 0) {
+        if (lane == 0) {
+            for (int s = 0; s < kStages; ++s) mbar_init(smem_u32(&full_bar[s]), 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            tma_driver(a, ring, full_bar, s_dst, s_bytes);
+        }
+    } else {
+        vector_warp(a, lane);
+    }
+}
+
+}  // namespace
+
+cudaError_t configure_copy_kernel() {
+    return cudaFuncSetAttribute(etp_interval_copy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCopySmemBytes);
+}
+
+void launch_copy_kernel(const CopyArgs& a, int grid, cudaStream_t stream) {
+    etp_interval_copy_kernel<<<grid, kCopyThreads, kCopySmemBytes, stream>>>(a);
+}
+
+}  // namespace etp

@@ -1,0 +1,354 @@
+// Context, options and the executor: uploads descriptors, launches kernel (a) per hazard phase on the copy stream and
+// runs the reload pipeline (b) on the reload stream.  PAPER.md:162-166: "issuing host-to-device reloads alongside GPU P2P
+// transfers, allowing the P2P portions to be hidden beneath the PCIe-bound reload time".
+#include <algorithm>
+#include <chrono>
+#include <cstring>
+
+#include "etp_copy.cuh"
+
+using namespace etp;
+
+namespace {
+constexpr int kArenaSlots = 2;
+constexpr int kCounterSlots = 256;   // pairs of work-queue heads available to one call
+
+struct ArenaSlot {
+    void* h = nullptr;
+    void* d = nullptr;
+    int64_t bytes = 0;
+    cudaEvent_t done_copy = nullptr, done_reload = nullptr;
+    bool busy = false;
+};
+struct CtxExtra {
+    ArenaSlot slot[kArenaSlots];
+    int next = 0;
+    cudaEvent_t uploaded = nullptr;
+};
+CtxExtra* extra(etp_ctx* c) { return reinterpret_cast<CtxExtra*>(c->impl); }
+
+double now_ms() {
+    return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count();
+}
+}  // namespace
+
+extern "C" etp_status etp_ctx_create(int device, int64_t staging_bytes, etp_ctx** out) {
+    if (!out) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_ctx_create: out is NULL");
+    *out = nullptr;
+    if (staging_bytes < 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_ctx_create: staging_bytes < 0");
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) {
+        cudaGetLastError();
+        ETP_FAIL(ETP_ERR_CUDA, "etp_ctx_create: CUDA device %d not available (%d devices); there is no CPU fallback", device, n_dev);
+    }
+    cudaDeviceProp prop;
+    ETP_CUDA_OK(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) ETP_FAIL(ETP_ERR_CUDA, "etp_ctx_create: device %d is sm_%d%d; this library is built for sm_100a only", device, prop.major, prop.minor);
+    ETP_CUDA_OK(cudaSetDevice(device));
+    etp_ctx* c = new (std::nothrow) etp_ctx();
+    if (!c) ETP_FAIL(ETP_ERR_NOMEM, "etp_ctx_create: out of memory");
+    c->device = device;
+    c->n_sms = prop.multiProcessorCount;
+    std::memset(c->opts, 0, sizeof(c->opts));
+    c->opts[ETP_OPT_TMA_MIN_BYTES] = 32768;
+    c->opts[ETP_OPT_LDG_STEALS_BULK] = 0;
+    c->opts[ETP_OPT_RELOAD_CHUNK_BYTES] = 64 << 20;
+    c->opts[ETP_OPT_KV_RELOAD_MODE] = 0;
+    c->opts[ETP_OPT_GRID_CTAS] = 0;
+    c->opts[ETP_OPT_GATHER_CTAS] = 16;
+    c->staging_bytes = staging_bytes ? staging_bytes : (int64_t(256) << 20);
+    CtxExtra* x = new (std::nothrow) CtxExtra();
+    if (!x) { delete c; ETP_FAIL(ETP_ERR_NOMEM, "etp_ctx_create: out of memory"); }
+    c->impl = x;
+    cudaError_t e = cudaMalloc(&c->d_counters, sizeof(unsigned int) * 2 * kCounterSlots);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&x->uploaded, cudaEventDisableTiming);
+    for (int i = 0; i < kArenaSlots && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&x->slot[i].done_copy, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&x->slot[i].done_reload, cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = configure_copy_kernel();
+    if (e != cudaSuccess) {
+        set_error("etp_ctx_create: %s", cudaGetErrorString(e));
+        etp_ctx_destroy(c);
+        return ETP_ERR_CUDA;
+    }
+    c->n_counter_slots = kCounterSlots;
+    *out = c;
+    return ETP_OK;
+}
+
+extern "C" void etp_ctx_destroy(etp_ctx* c) {
+    if (!c) return;
+    cudaSetDevice(c->device);
+    cudaDeviceSynchronize();
+    CtxExtra* x = extra(c);
+    if (x) {
+        for (int i = 0; i < kArenaSlots; ++i) {
+            if (x->slot[i].h) cudaFreeHost(x->slot[i].h);
+            if (x->slot[i].d) cudaFree(x->slot[i].d);
+            if (x->slot[i].done_copy) cudaEventDestroy(x->slot[i].done_copy);
+            if (x->slot[i].done_reload) cudaEventDestroy(x->slot[i].done_reload);
+        }
+        if (x->uploaded) cudaEventDestroy(x->uploaded);
+        delete x;
+    }
+    for (cudaEvent_t e : c->events) cudaEventDestroy(e);
+    if (c->d_counters) cudaFree(c->d_counters);
+    if (c->d_staging) cudaFree(c->d_staging);
+    cudaGetLastError();
+    delete c;
+}
+
+extern "C" etp_status etp_ctx_set_option(etp_ctx* c, etp_option key, int64_t value) {
+    if (!c || key < 0 || key >= ETP_OPT__COUNT) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_ctx_set_option: bad ctx/key");
+    if (value < 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_ctx_set_option: negative value");
+    if (key == ETP_OPT_TMA_MIN_BYTES && value < 16) value = 16;
+    if (key == ETP_OPT_RELOAD_CHUNK_BYTES && value < 4096) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_ctx_set_option: reload chunk < 4096");
+    c->opts[key] = value;
+    return ETP_OK;
+}
+
+extern "C" etp_status etp_ctx_get_option(const etp_ctx* c, etp_option key, int64_t* value) {
+    if (!c || !value || key < 0 || key >= ETP_OPT__COUNT) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_ctx_get_option: bad ctx/key");
+    *value = c->opts[key];
+    return ETP_OK;
+}
+
+namespace etp {
+
+static etp_status ensure_event(etp_ctx* c, size_t i) {
+    while (c->events.size() <= i) {
+        cudaEvent_t e;
+        ETP_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        c->events.push_back(e);
+    }
+    return ETP_OK;
+}
+
+etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload_stream_v, etp_reshard_report* report) {
+    const double t0 = now_ms();
+    cudaStream_t cs = (cudaStream_t)copy_stream_v, rs = (cudaStream_t)reload_stream_v;
+    ETP_CUDA_OK(cudaSetDevice(c->device));
+    CtxExtra* x = extra(c);
+    const bool skip_d2d = c->opts[ETP_OPT_SKIP_D2D] != 0, skip_reload = c->opts[ETP_OPT_SKIP_RELOAD] != 0;
+    const size_t n_ph = std::max(w->phases.size(), w->host_gather.size());
+    w->phases.resize(n_ph);
+    w->host_gather.resize(n_ph);
+
+    // ---- descriptor arena layout: [phase p bulk | phase p frag | gather p frag] ...
+    int64_t total = 0, n_jobs = 0;
+    auto pad = [](int64_t b) { return (b + 255) & ~int64_t(255); };
+    std::vector<int64_t> off_bulk(n_ph), off_frag(n_ph), off_gather(n_ph);
+    int launches_needed = 0;
+    for (size_t p = 0; p < n_ph; ++p) {
+        off_bulk[p] = total;   total += pad((int64_t)w->phases[p].bulk.size() * sizeof(BulkJob));
+        off_frag[p] = total;   total += pad((int64_t)w->phases[p].frag.size() * sizeof(FragJob));
+        off_gather[p] = total; total += pad((int64_t)w->host_gather[p].frag.size() * sizeof(FragJob));
+        n_jobs += (int64_t)(w->phases[p].bulk.size() + w->phases[p].frag.size() + w->host_gather[p].frag.size());
+        launches_needed += (!w->phases[p].empty()) + (!w->host_gather[p].frag.empty());
+        if (w->phases[p].bulk.size() >= 0xFFFFFFF0ull || w->phases[p].frag.size() >= 0xFFFFFFF0ull || w->host_gather[p].frag.size() >= 0xFFFFFFF0ull)
+            ETP_FAIL(ETP_ERR_CAPACITY, "too many jobs in one phase");
+    }
+    if (launches_needed > c->n_counter_slots) ETP_FAIL(ETP_ERR_CAPACITY, "plan needs %d launches > %d", launches_needed, c->n_counter_slots);
+
+    char* d_base = nullptr;
+    ArenaSlot* slot = nullptr;
+    if (total > 0) {
+        slot = &x->slot[x->next];
+        x->next = (x->next + 1) % kArenaSlots;
+        if (slot->busy) {  // the call that used this slot two calls ago must have consumed its descriptors
+            ETP_CUDA_OK(cudaEventSynchronize(slot->done_copy));
+            ETP_CUDA_OK(cudaEventSynchronize(slot->done_reload));
+            slot->busy = false;
+        }
+        if (slot->bytes < total) {
+            if (slot->h) cudaFreeHost(slot->h);
+            if (slot->d) cudaFree(slot->d);
+            slot->h = slot->d = nullptr;
+            slot->bytes = 0;
+            const int64_t want = std::max<int64_t>(total + total / 4, 1 << 20);
+            ETP_CUDA_OK(cudaMallocHost(&slot->h, want));
+            ETP_CUDA_OK(cudaMalloc(&slot->d, want));
+            slot->bytes = want;
+        }
+        char* h = (char*)slot->h;
+        for (size_t p = 0; p < n_ph; ++p) {
+            if (!w->phases[p].bulk.empty()) std::memcpy(h + off_bulk[p], w->phases[p].bulk.data(), w->phases[p].bulk.size() * sizeof(BulkJob));
+            if (!w->phases[p].frag.empty()) std::memcpy(h + off_frag[p], w->phases[p].frag.data(), w->phases[p].frag.size() * sizeof(FragJob));
+            if (!w->host_gather[p].frag.empty()) std::memcpy(h + off_gather[p], w->host_gather[p].frag.data(), w->host_gather[p].frag.size() * sizeof(FragJob));
+        }
+        d_base = (char*)slot->d;
+        ETP_CUDA_OK(cudaMemsetAsync(c->d_counters, 0, sizeof(unsigned int) * 2 * launches_needed, cs));
+        ETP_CUDA_OK(cudaMemcpyAsync(d_base, h, total, cudaMemcpyHostToDevice, cs));
+        ETP_CUDA_OK(cudaEventRecord(x->uploaded, cs));
+    }
+
+    // which phases must publish an event for the reload stream
+    std::vector<char> need_event(n_ph + 1, 0);
+    if (!skip_reload) {
+        for (const DmaCopy& d : w->dma)
+            if (d.phase > 0) need_event[d.phase - 1] = 1;
+        for (size_t p = 1; p < n_ph; ++p)
+            if (!w->host_gather[p].frag.empty()) need_event[p - 1] = 1;
+    }
+
+    const int grid = c->opts[ETP_OPT_GRID_CTAS] > 0 ? (int)c->opts[ETP_OPT_GRID_CTAS] : c->n_sms;
+    int counter_slot = 0, launches = 0;
+    // ---- kernel (a) on the copy stream, one launch per hazard phase
+    for (size_t p = 0; p < n_ph; ++p) {
+        const JobList& jl = w->phases[p];
+        if (!jl.empty() && !skip_d2d) {
+            CopyArgs a;
+            a.bulk = (const BulkJob*)(d_base + off_bulk[p]);
+            a.frag = (const FragJob*)(d_base + off_frag[p]);
+            a.n_bulk = (unsigned)jl.bulk.size();
+            a.n_frag = (unsigned)jl.frag.size();
+            a.counters = c->d_counters + 2 * counter_slot;
+            a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
+            launch_copy_kernel(a, grid, cs);
+            ETP_CUDA_OK(cudaGetLastError());
+            ++launches;
+        }
+        if (!jl.empty()) ++counter_slot;
+        if (need_event[p]) {
+            ETP_TRY(ensure_event(c, p));
+            ETP_CUDA_OK(cudaEventRecord(c->events[p], cs));
+        }
+    }
+
+    // ---- pipeline (b) on the reload stream
+    int64_t n_memcpys = 0;
+    if (!skip_reload) {
+        const int64_t chunk = c->opts[ETP_OPT_RELOAD_CHUNK_BYTES];
+        // DMAs in phase order so that a late-phase wait does not hold back hazard-free reloads
+        std::stable_sort(w->dma.begin(), w->dma.end(), [](const DmaCopy& a, const DmaCopy& b) { return a.phase < b.phase; });
+        bool gather_waited_upload = false;
+        size_t di = 0;
+        for (size_t p = 0; p < n_ph; ++p) {
+            bool has_work = !w->host_gather[p].frag.empty();
+            for (size_t k = di; k < w->dma.size() && !has_work; ++k) has_work = w->dma[k].phase == (int32_t)p;
+            if (p > 0 && has_work && cs != rs) ETP_CUDA_OK(cudaStreamWaitEvent(rs, c->events[p - 1], 0));
+            for (; di < w->dma.size() && w->dma[di].phase == (int32_t)p; ++di) {
+                const DmaCopy& d = w->dma[di];
+                for (int64_t o = 0; o < d.bytes; o += chunk) {
+                    const int64_t n = std::min(chunk, d.bytes - o);
+                    ETP_CUDA_OK(cudaMemcpyAsync((char*)d.dst + o, (const char*)d.src + o, n, cudaMemcpyHostToDevice, rs));
+                    ++n_memcpys;
+                }
+            }
+            const JobList& gl = w->host_gather[p];
+            if (!gl.frag.empty()) {
+                if (!gather_waited_upload && cs != rs) {
+                    ETP_CUDA_OK(cudaStreamWaitEvent(rs, x->uploaded, 0));
+                    gather_waited_upload = true;
+                }
+                CopyArgs a;
+                a.bulk = nullptr;
+                a.frag = (const FragJob*)(d_base + off_gather[p]);
+                a.n_bulk = 0;
+                a.n_frag = (unsigned)gl.frag.size();
+                a.counters = c->d_counters + 2 * counter_slot;
+                a.flags = 0;
+                const int ggrid = (int)std::max<int64_t>(1, std::min<int64_t>(c->opts[ETP_OPT_GATHER_CTAS], c->n_sms));
+                launch_copy_kernel(a, ggrid, rs);
+                ETP_CUDA_OK(cudaGetLastError());
+                ++launches;
+                ++counter_slot;
+            }
+        }
+    }
+    if (slot) {
+        ETP_CUDA_OK(cudaEventRecord(slot->done_copy, cs));
+        ETP_CUDA_OK(cudaEventRecord(slot->done_reload, rs));
+        slot->busy = true;
+    }
+    c->launches = launches;
+    w->rep.n_jobs = n_jobs;
+    w->rep.n_memcpys = n_memcpys;
+    w->rep.n_kernel_launches = launches;
+    w->rep.lower_ms += now_ms() - t0;
+    if (report) *report = w->rep;
+    return ETP_OK;
+}
+
+}  // namespace etp
+
+// ------------------------------------------------------------------------------------------------ C ABI device calls
+extern "C" etp_status etp_reshard_params(etp_ctx* ctx, const etp_tensor* tensors, int32_t n_tensors,
+                                         const etp_plan* const* plans, int32_t n_plans, void* copy_stream,
+                                         void* reload_stream, etp_reshard_report* report) {
+    if (!ctx) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_params: ctx is NULL");
+    const double t0 = now_ms();
+    ETP_CUDA_OK(cudaSetDevice(ctx->device));
+    LoweredWork w;
+    ETP_TRY(lower_params(ctx, tensors, n_tensors, plans, n_plans, &w));
+    w.rep.lower_ms = now_ms() - t0;
+    return execute(ctx, &w, copy_stream, reload_stream, report);
+}
+
+extern "C" etp_status etp_reshard_kv(etp_ctx* ctx, const etp_kv_geometry* geom, etp_page_table* pt,
+                                     const etp_plan* head_plan, int32_t new_block_budget, int32_t* evicted_seqs_out,
+                                     int32_t* n_evicted, void* copy_stream, void* reload_stream,
+                                     etp_reshard_report* report) {
+    if (!ctx || !geom || !pt || !head_plan || !n_evicted) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: NULL argument");
+    const double t0 = now_ms();
+    ETP_CUDA_OK(cudaSetDevice(ctx->device));
+    if (new_block_budget < 0 || new_block_budget > geom->n_blocks)
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: budget %d outside [0, n_blocks=%d]", new_block_budget, geom->n_blocks);
+    if (head_plan->total_units < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: empty head plan");
+    // validate before touching the caller's table
+    int64_t max_pairs = 0;
+    for (int32_t s = 0; s < pt->n_seqs; ++s) {
+        if (!pt->seq_lens) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: seq_lens is NULL");
+        max_pairs += (pt->seq_lens[s] + geom->block_size - 1) / std::max(geom->block_size, 1);
+    }
+    for (int32_t s = 0; s < pt->n_seqs; ++s)
+        for (int32_t i = 0; i < (pt->seq_lens[s] + geom->block_size - 1) / geom->block_size && i < pt->max_blocks; ++i) {
+            const int32_t b = pt->block_table[(int64_t)s * pt->max_blocks + i];
+            if (b >= geom->n_blocks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: block id %d >= n_blocks %d", b, geom->n_blocks);
+        }
+    std::vector<int32_t> pairs((size_t)std::max<int64_t>(max_pairs, 1) * 2);
+    std::vector<int32_t> ev((size_t)std::max(pt->n_seqs, 1));
+    int64_t n_pairs = 0;
+    int32_t n_ev = 0;
+    ETP_TRY(etp_page_table_rewrite(pt, geom->block_size, new_block_budget, ev.data(), &n_ev, pairs.data(), max_pairs, &n_pairs));
+    bool needs_backup = false;
+    for (const etp_task& t : head_plan->tasks) needs_backup = needs_backup || (t.kind == ETP_RELOAD && t.begin < t.end);
+    if (needs_backup && !geom->host_backup) {
+        // reading K4: without a backup the reloaded heads stay missing; every surviving sequence is reported too
+        std::vector<char> gone((size_t)std::max(pt->n_seqs, 1), 0);
+        for (int32_t i = 0; i < n_ev; ++i) gone[ev[i]] = 1;
+        for (int32_t s = 0; s < pt->n_seqs; ++s)
+            if (!gone[s] && pt->seq_lens[s] > 0) ev[n_ev++] = s;
+    }
+    *n_evicted = n_ev;
+    if (evicted_seqs_out)
+        for (int32_t i = 0; i < n_ev; ++i) evicted_seqs_out[i] = ev[i];
+    LoweredWork w;
+    ETP_TRY(lower_kv(ctx, geom, head_plan, pairs.data(), n_pairs, &w));
+    w.rep.lower_ms = now_ms() - t0;
+    return execute(ctx, &w, copy_stream, reload_stream, report);
+}
+
+extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_descs, int64_t n, void* stream,
+                                         etp_reshard_report* report) {
+    if (!ctx || n < 0 || (n > 0 && !host_descs)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: bad arguments");
+    const double t0 = now_ms();
+    LoweredWork w;
+    w.phases.resize(1);
+    w.phases[0].bulk.reserve((size_t)n);
+    for (int64_t i = 0; i < n; ++i) {
+        const etp_interval& d = host_descs[i];
+        if (d.bytes < 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has negative size", (long long)i);
+        if (d.bytes == 0) continue;
+        if (!d.src || !d.dst) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has a NULL pointer", (long long)i);
+        if (((uintptr_t)d.src | (uintptr_t)d.dst | (uint64_t)d.bytes) & 15)
+            ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_copy_intervals: interval %lld is not 16-byte aligned", (long long)i);
+        push_contiguous(ctx, &w.phases[0], d.src, d.dst, d.bytes);
+        w.rep.d2d_bytes += d.bytes;
+        w.rep.n_units += 1;
+    }
+    w.rep.n_phases = 1;
+    w.rep.lower_ms = now_ms() - t0;
+    return execute(ctx, &w, stream, stream, report);
+}

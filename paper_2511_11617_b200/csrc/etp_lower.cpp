@@ -1,0 +1,378 @@
+// S3 — lowering a CMM plan onto concrete memory: unit intervals x (tensor, src slab, dst slab) -> byte descriptors of the
+// copy kernel and DMA requests of the reload pipeline, with write-after-read hazard phases.
+// PAPER.md:164 ("a single pass pre-allocates all destination buffers"), :178 (Transfer / Reload tasks on interval
+// boundaries, range reads of only the needed byte intervals); layout contract: DESIGN.md readings L1-L7, K1-K6.
+#include <algorithm>
+#include <cstring>
+
+#include "etp_internal.h"
+
+namespace etp {
+
+MemKind classify_pointer(const void* p) {
+    cudaPointerAttributes a;
+    std::memset(&a, 0, sizeof(a));
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return MEM_HOST_PAGEABLE;
+    }
+    if (a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged) return MEM_DEVICE;
+    if (a.type == cudaMemoryTypeHost) return MEM_HOST_PINNED;
+    return MEM_HOST_PAGEABLE;
+}
+
+static inline uint32_t log2_exact(uint64_t v) {  // 0xFF when v is not a power of two
+    if (v == 0 || (v & (v - 1))) return 0xFFu;
+    uint32_t s = 0;
+    while ((uint64_t(1) << s) < v) ++s;
+    return s;
+}
+
+static inline FragJob make_frag(const void* src, void* dst, uint32_t row_bytes, uint32_t n_rows, uint32_t rows_per_group,
+                                int64_t s_row, int64_t d_row, int64_t s_grp, int64_t d_grp) {
+    FragJob j;
+    j.src = (uint64_t)(uintptr_t)src;
+    j.dst = (uint64_t)(uintptr_t)dst;
+    j.row_bytes = row_bytes;
+    j.n_rows = n_rows;
+    j.rows_per_group = rows_per_group;
+    j.vec_shift = log2_exact(row_bytes >> 4) | (log2_exact(rows_per_group) << 8);
+    j.s_row = s_row;
+    j.d_row = d_row;
+    j.s_grp = s_grp;
+    j.d_grp = d_grp;
+    return j;
+}
+
+// One contiguous interval -> work-queue jobs.  Large intervals go to the cp.async.bulk queue in pieces of kBulkJobMax
+// (so that 148 SMs balance even on a single 130 MB embedding interval); small ones to the vector-copy queue.
+void push_contiguous(const etp_ctx* ctx, JobList* jl, const void* src, void* dst, int64_t bytes) {
+    const int64_t tma_min = ctx->opts[ETP_OPT_TMA_MIN_BYTES];
+    const char* s = (const char*)src;
+    char* d = (char*)dst;
+    jl->bytes += bytes;
+    if (bytes >= tma_min) {
+        while (bytes > 0) {
+            // avoid a tiny last piece: split the tail evenly once it is below two jobs
+            int64_t n = bytes > 2 * kBulkJobMax ? kBulkJobMax : (bytes > kBulkJobMax ? ((bytes / 2 + 15) & ~int64_t(15)) : bytes);
+            jl->bulk.push_back({(uint64_t)(uintptr_t)s, (uint64_t)(uintptr_t)d, (uint64_t)n, 0});
+            s += n; d += n; bytes -= n;
+        }
+    } else {
+        while (bytes > 0) {
+            const int64_t n = std::min<int64_t>(bytes, kFragJobTarget);
+            jl->frag.push_back(make_frag(s, d, (uint32_t)n, 1, 1, 0, 0, 0, 0));
+            s += n; d += n; bytes -= n;
+        }
+    }
+}
+
+namespace {
+inline int64_t pmod(int64_t a, int64_t m) {
+    int64_t r = a % m;
+    return r < 0 ? r + m : r;
+}
+
+struct SlotRun {
+    int64_t first_unit, count, src_slot, dst_slot;
+};
+
+// Split units [b,e) into runs over which both the source slot and the destination slot advance without wrapping.
+// src_cap == 0 means "no slot addressing on the source side" (host image).
+void slot_runs(int64_t b, int64_t e, int64_t src_anchor, int64_t src_cap, int64_t dst_anchor, int64_t dst_cap,
+               std::vector<SlotRun>* out) {
+    out->clear();
+    int64_t u = b;
+    while (u < e) {
+        int64_t n = e - u;
+        int64_t ss = 0, ds = pmod(u - dst_anchor, dst_cap);
+        n = std::min(n, dst_cap - ds);
+        if (src_cap > 0) {
+            ss = pmod(u - src_anchor, src_cap);
+            n = std::min(n, src_cap - ss);
+        }
+        out->push_back({u, n, ss, ds});
+        u += n;
+    }
+}
+
+struct Range {
+    int32_t rank;
+    int64_t b, e;  // slots
+};
+inline bool hits(const Range& a, const Range& b) { return a.rank == b.rank && a.b < b.e && b.b < a.e; }
+
+// Hazard phases (reading L4): task k must run after every task j that READS bytes k OVERWRITES.
+// phase(k) = 0 if nothing reads what k writes, else 1 + max phase of those readers.  A cycle is unsupported.
+etp_status assign_phases(const std::vector<std::vector<Range>>& reads, const std::vector<std::vector<Range>>& writes,
+                         std::vector<int32_t>* phase) {
+    const size_t n = reads.size();
+    phase->assign(n, 0);
+    for (size_t round = 0; round <= n; ++round) {
+        bool changed = false;
+        for (size_t k = 0; k < n; ++k)
+            for (size_t j = 0; j < n; ++j) {
+                if (j == k) continue;
+                bool dep = false;
+                for (const Range& w : writes[k])
+                    for (const Range& r : reads[j]) dep = dep || hits(w, r);
+                if (dep && (*phase)[k] < (*phase)[j] + 1) {
+                    (*phase)[k] = (*phase)[j] + 1;
+                    changed = true;
+                }
+            }
+        if (!changed) return ETP_OK;
+    }
+    ETP_FAIL(ETP_ERR_UNSUPPORTED, "cyclic write-after-read hazard between tasks (needs a bounce buffer)");
+}
+
+JobList& phase_list(std::vector<JobList>& v, int32_t p) {
+    if ((int32_t)v.size() <= p) v.resize(p + 1);
+    return v[p];
+}
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ parameters
+etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n_tensors, const etp_plan* const* plans,
+                        int32_t n_plans, LoweredWork* out) {
+    if (n_tensors < 0 || n_plans < 0 || (n_tensors > 0 && (!tensors || !plans)))
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_params: NULL tensors/plans");
+    std::vector<SlotRun> runs;
+    int32_t max_phase = 0;
+    for (int32_t t = 0; t < n_tensors; ++t) {
+        const etp_tensor& T = tensors[t];
+        if (T.plan_index < 0 || T.plan_index >= n_plans || !plans[T.plan_index])
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "tensor %d: plan_index %d out of range", t, T.plan_index);
+        const etp_plan& P = *plans[T.plan_index];
+        if (T.unit_bytes <= 0 || T.total_units != P.total_units)
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "tensor %d: total_units %lld does not match its plan (%lld) or unit_bytes <= 0", t,
+                     (long long)T.total_units, (long long)P.total_units);
+        if (T.unit_bytes % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "tensor %d: unit_bytes %lld is not a multiple of 16", t, (long long)T.unit_bytes);
+        if (!T.slabs || T.n_ranks < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "tensor %d: no slabs", t);
+        auto slab_of = [&](int32_t rank) -> const etp_slab* {
+            return (rank >= 0 && rank < T.n_ranks) ? &T.slabs[rank] : nullptr;
+        };
+        // capacity: every new shard must fit its slab
+        for (const etp_shard& s : P.new_layout) {
+            const etp_slab* sl = slab_of(s.rank);
+            if (!sl || (s.end > s.begin && !sl->base)) ETP_FAIL(ETP_ERR_INVALID_ARG, "tensor %d: no slab for rank %d", t, s.rank);
+            if (sl->cap_units < 1 || s.end - s.begin > sl->cap_units)
+                ETP_FAIL(ETP_ERR_CAPACITY, "tensor %d rank %d: new shard of %lld units does not fit cap_units %lld", t, s.rank,
+                         (long long)(s.end - s.begin), (long long)sl->cap_units);
+            if ((uintptr_t)sl->base % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "tensor %d rank %d: slab base not 16-byte aligned", t, s.rank);
+        }
+        MemKind image_kind = MEM_HOST_PAGEABLE;
+        bool image_checked = false;
+
+        // read / write slot ranges per task for the hazard analysis
+        const size_t nt = P.tasks.size();
+        std::vector<std::vector<Range>> reads(nt), writes(nt);
+        for (size_t k = 0; k < nt; ++k) {
+            const etp_task& K = P.tasks[k];
+            if (K.kind == ETP_KEEP || K.begin >= K.end) continue;
+            const etp_slab* D = slab_of(K.dst_rank);
+            const etp_slab* S = K.kind == ETP_TRANSFER ? slab_of(K.src_rank) : nullptr;
+            if (K.kind == ETP_TRANSFER) {
+                if (!S || !S->base || S->cap_units < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "tensor %d: no slab for source rank %d", t, K.src_rank);
+                if ((uintptr_t)S->base % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "tensor %d rank %d: slab base not 16-byte aligned", t, K.src_rank);
+                if (K.end - K.begin > S->cap_units) ETP_FAIL(ETP_ERR_CAPACITY, "tensor %d: transfer wider than the source slab", t);
+            }
+            slot_runs(K.begin, K.end, S ? S->anchor_unit : 0, S ? S->cap_units : 0, D->anchor_unit, D->cap_units, &runs);
+            for (const SlotRun& r : runs) {
+                writes[k].push_back({K.dst_rank, r.dst_slot, r.dst_slot + r.count});
+                if (S) reads[k].push_back({K.src_rank, r.src_slot, r.src_slot + r.count});
+            }
+        }
+        std::vector<int32_t> phase;
+        ETP_TRY(assign_phases(reads, writes, &phase));
+
+        for (size_t k = 0; k < nt; ++k) {
+            const etp_task& K = P.tasks[k];
+            const int64_t bytes = (K.end - K.begin) * T.unit_bytes;
+            if (K.kind == ETP_KEEP) {
+                out->rep.kept_bytes += bytes;
+                continue;
+            }
+            if (K.begin >= K.end) continue;
+            max_phase = std::max(max_phase, phase[k]);
+            const etp_slab* D = slab_of(K.dst_rank);
+            if (K.kind == ETP_TRANSFER) {
+                const etp_slab* S = slab_of(K.src_rank);
+                slot_runs(K.begin, K.end, S->anchor_unit, S->cap_units, D->anchor_unit, D->cap_units, &runs);
+                for (const SlotRun& r : runs) {
+                    push_contiguous(ctx, &phase_list(out->phases, phase[k]), (const char*)S->base + r.src_slot * T.unit_bytes,
+                                    (char*)D->base + r.dst_slot * T.unit_bytes, r.count * T.unit_bytes);
+                    out->rep.n_units += 1;
+                }
+                out->rep.d2d_bytes += bytes;
+            } else {  // RELOAD
+                if (!T.host_image || K.begin < T.host_unit0 || K.end > T.host_unit0 + T.host_units)
+                    ETP_FAIL(ETP_ERR_NO_SOURCE, "tensor %d: RELOAD [%lld,%lld) not covered by the host image", t,
+                             (long long)K.begin, (long long)K.end);
+                if ((uintptr_t)T.host_image % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "tensor %d: host image not 16-byte aligned", t);
+                if (!image_checked) {
+                    image_kind = classify_pointer(T.host_image);
+                    image_checked = true;
+                }
+                slot_runs(K.begin, K.end, 0, 0, D->anchor_unit, D->cap_units, &runs);
+                for (const SlotRun& r : runs) {
+                    const char* src = (const char*)T.host_image + (r.first_unit - T.host_unit0) * T.unit_bytes;
+                    char* dst = (char*)D->base + r.dst_slot * T.unit_bytes;
+                    if (image_kind == MEM_DEVICE) {
+                        push_contiguous(ctx, &phase_list(out->phases, phase[k]), src, dst, r.count * T.unit_bytes);
+                    } else {
+                        out->dma.push_back({src, dst, r.count * T.unit_bytes, phase[k]});
+                    }
+                    out->rep.n_units += 1;
+                }
+                if (image_kind == MEM_DEVICE) out->rep.reload_dev_bytes += bytes;
+                else out->rep.h2d_bytes += bytes;
+            }
+        }
+    }
+    out->rep.n_phases = std::max<int32_t>(out->rep.n_phases, max_phase + 1);
+    return ETP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ paged KV
+namespace {
+struct PoolShape {
+    int64_t plane, block, row, slot;  // byte strides: (layer,K|V) plane, block, token row (token-major) and head slot
+};
+PoolShape pool_shape(const etp_kv_geometry& g, int64_t heads) {
+    const int64_t frag = (int64_t)g.head_dim * g.elem_bytes;
+    PoolShape s;
+    s.block = (int64_t)g.block_size * heads * frag;
+    s.plane = (int64_t)g.n_blocks * s.block;
+    if (g.layout == ETP_KV_TOKEN_MAJOR) {
+        s.row = heads * frag;  // [token][slot][dim]
+        s.slot = frag;
+    } else {
+        s.row = frag;  // [slot][token][dim]
+        s.slot = (int64_t)g.block_size * frag;
+    }
+    return s;
+}
+}  // namespace
+
+etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* gp, const etp_plan* head_plan, const int32_t* pairs,
+                    int64_t n_pairs, LoweredWork* out) {
+    const etp_kv_geometry& g = *gp;
+    const etp_plan& P = *head_plan;
+    if (g.n_layers < 1 || g.n_blocks < 1 || g.block_size < 1 || g.head_cap < 1 || g.head_dim < 1 || g.elem_bytes < 1 || g.n_ranks < 1 ||
+        !g.pools || !g.head_anchor)
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: bad geometry");
+    if (g.layout != ETP_KV_TOKEN_MAJOR && g.layout != ETP_KV_HEAD_MAJOR) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: unknown layout");
+    const int64_t frag = (int64_t)g.head_dim * g.elem_bytes;
+    if (frag % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_reshard_kv: fragment of %lld bytes is not a multiple of 16", (long long)frag);
+    for (const etp_shard& s : P.new_layout) {
+        if (s.rank < 0 || s.rank >= g.n_ranks || (s.end > s.begin && !g.pools[s.rank]))
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: no pool for rank %d", s.rank);
+        if (s.end - s.begin > g.head_cap)
+            ETP_FAIL(ETP_ERR_CAPACITY, "etp_reshard_kv: rank %d gets %lld heads > head_cap %d", s.rank, (long long)(s.end - s.begin), g.head_cap);
+        if ((uintptr_t)g.pools[s.rank] % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_reshard_kv: pool of rank %d not 16-byte aligned", s.rank);
+    }
+    const PoolShape dev = pool_shape(g, g.head_cap);
+    const PoolShape bak = pool_shape(g, g.host_heads > 0 ? g.host_heads : 1);
+    const int64_t n_planes = 2 * (int64_t)g.n_layers;
+    MemKind backup_kind = g.host_backup ? classify_pointer(g.host_backup) : MEM_DEVICE;
+    if (g.host_backup && backup_kind == MEM_HOST_PAGEABLE)
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: host_backup must be pinned host or device memory");
+
+    // hazard analysis at (rank, slot) granularity; relocations of kept heads only touch free blocks -> phase 0
+    const size_t nt = P.tasks.size();
+    std::vector<std::vector<Range>> reads(nt), writes(nt);
+    std::vector<SlotRun> runs;
+    for (size_t k = 0; k < nt; ++k) {
+        const etp_task& K = P.tasks[k];
+        if (K.kind == ETP_KEEP || K.begin >= K.end) continue;
+        if (K.kind == ETP_TRANSFER && (K.src_rank < 0 || K.src_rank >= g.n_ranks || !g.pools[K.src_rank]))
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: no pool for source rank %d", K.src_rank);
+        const bool dev_src = K.kind == ETP_TRANSFER;
+        slot_runs(K.begin, K.end, dev_src ? g.head_anchor[K.src_rank] : 0, dev_src ? g.head_cap : 0, g.head_anchor[K.dst_rank], g.head_cap, &runs);
+        for (const SlotRun& r : runs) {
+            writes[k].push_back({K.dst_rank, r.dst_slot, r.dst_slot + r.count});
+            if (dev_src) reads[k].push_back({K.src_rank, r.src_slot, r.src_slot + r.count});
+        }
+    }
+    std::vector<int32_t> phase;
+    ETP_TRY(assign_phases(reads, writes, &phase));
+    int32_t max_phase = 0;
+
+    for (size_t k = 0; k < nt; ++k) {
+        const etp_task& K = P.tasks[k];
+        if (K.begin >= K.end) continue;
+        const int64_t live_bytes = (K.end - K.begin) * frag * g.block_size * n_planes * n_pairs;
+        const char* src_base;
+        const PoolShape* ss;
+        std::vector<JobList>* dest = &out->phases;
+        int64_t* counter;
+        if (K.kind == ETP_KEEP) {
+            src_base = (const char*)g.pools[K.dst_rank];
+            ss = &dev;
+            slot_runs(K.begin, K.end, g.head_anchor[K.dst_rank], g.head_cap, g.head_anchor[K.dst_rank], g.head_cap, &runs);
+            counter = &out->rep.d2d_bytes;
+        } else if (K.kind == ETP_TRANSFER) {
+            src_base = (const char*)g.pools[K.src_rank];
+            ss = &dev;
+            slot_runs(K.begin, K.end, g.head_anchor[K.src_rank], g.head_cap, g.head_anchor[K.dst_rank], g.head_cap, &runs);
+            counter = &out->rep.d2d_bytes;
+        } else {
+            if (!g.host_backup) continue;  // reading K4: fragments left untouched; the caller reports the sequences
+            if (K.begin < g.host_head0 || K.end > g.host_head0 + g.host_heads)
+                ETP_FAIL(ETP_ERR_NO_SOURCE, "etp_reshard_kv: RELOAD heads [%lld,%lld) not covered by the backup", (long long)K.begin, (long long)K.end);
+            if ((uintptr_t)g.host_backup % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_reshard_kv: host_backup not 16-byte aligned");
+            src_base = (const char*)g.host_backup;
+            ss = &bak;
+            slot_runs(K.begin, K.end, 0, 0, g.head_anchor[K.dst_rank], g.head_cap, &runs);
+            for (SlotRun& r : runs) r.src_slot = r.first_unit - g.host_head0;
+            if (backup_kind == MEM_DEVICE) {
+                counter = &out->rep.reload_dev_bytes;
+            } else {
+                counter = &out->rep.h2d_bytes;
+                dest = &out->host_gather;
+            }
+        }
+        const int32_t ph = K.kind == ETP_KEEP ? 0 : phase[k];
+        int64_t moved = 0;
+        char* dst_base = (char*)g.pools[K.dst_rank];
+        for (const SlotRun& r : runs) {
+            uint32_t row_bytes, rows_per_plane;
+            int64_t s_row, d_row;
+            if (g.layout == ETP_KV_TOKEN_MAJOR) {  // block_size rows of (run of heads) per plane
+                row_bytes = (uint32_t)(r.count * frag);
+                rows_per_plane = (uint32_t)g.block_size;
+                s_row = ss->row;
+                d_row = dev.row;
+            } else {  // one contiguous run of block_size * heads fragments per plane
+                row_bytes = (uint32_t)(r.count * g.block_size * frag);
+                rows_per_plane = 1;
+                s_row = d_row = 0;
+            }
+            const int64_t plane_bytes = (int64_t)row_bytes * rows_per_plane;
+            const int64_t planes_per_job = std::max<int64_t>(1, kFragJobTarget / plane_bytes);
+            for (int64_t p = 0; p < n_pairs; ++p) {
+                const int64_t bo = pairs[2 * p], bn = pairs[2 * p + 1];
+                if (K.kind == ETP_KEEP && bo == bn) continue;
+                JobList& jl = phase_list(*dest, ph);
+                for (int64_t pl = 0; pl < n_planes; pl += planes_per_job) {
+                    const int64_t np = std::min(planes_per_job, n_planes - pl);
+                    const char* s = src_base + pl * ss->plane + bo * ss->block + r.src_slot * ss->slot;
+                    char* d = dst_base + pl * dev.plane + bn * dev.block + r.dst_slot * dev.slot;
+                    jl.frag.push_back(make_frag(s, d, row_bytes, (uint32_t)(np * rows_per_plane), rows_per_plane, s_row, d_row, ss->plane, dev.plane));
+                    jl.bytes += np * plane_bytes;
+                    moved += np * plane_bytes;
+                }
+                out->rep.n_units += 1;
+            }
+        }
+        *counter += moved;
+        if (K.kind == ETP_KEEP) out->rep.kept_bytes += live_bytes - moved;
+        if (moved) max_phase = std::max(max_phase, ph);
+    }
+    out->rep.n_phases = std::max<int32_t>(out->rep.n_phases, max_phase + 1);
+    (void)ctx;
+    return ETP_OK;
+}
+
+}  // namespace etp
