@@ -1,0 +1,305 @@
+"""Parity proper: the CUDA path (through the C ABI) against the CPU oracle, byte for byte.
+
+Whole slabs / whole pools are compared (not only the new shards), so a byte written outside the plan fails
+(reading L6), and every device buffer sits between guard bands."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2511_11617_b200 as etp
+from oracle import state as OS
+from tests import harness as H
+from tests.gpu_util import DevBuf, LibSide, Streams, make_plans, pinned
+from workloads import get_config
+from workloads.configs import FFN, HEAD, VOCAB, Config, KVShape, ModelShape, Scenario
+from workloads.gen import microbench_intervals
+
+pytestmark = pytest.mark.gpu
+
+# a shape whose transfers span several 256-KiB bulk jobs and 32-KiB ring stages with ragged tails
+MID = Config(1, "mid", ModelShape("mid-dense", 2, 1024, 16, 8, 64, ffn=2731, vocab=5003, dtype="bf16"),
+             KVShape(3, 1000), Scenario(4, (1,), old_widths={FFN: (700, 650, 720, 661)}), tokens=4)
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = etp.Context(0)
+    yield c
+    c.close()
+
+
+def upload_param_world(world, image="pinned"):
+    bufs, descs, images = {}, {}, {}
+    for sp in world.specs:
+        bufs[sp.name] = {r: DevBuf(a) for r, a in world.slabs[sp.name].items()}
+        if image == "pinned":
+            images[sp.name] = pinned(world.unsharded[sp.name])
+        else:
+            images[sp.name] = torch.from_numpy(world.unsharded[sp.name]).cuda()
+    return bufs, images
+
+
+def tensor_descs(world, bufs, images, step, class_index):
+    n_ranks = max(r for (r, _, _, _) in world.steps[0].old[world.specs[0].klass]) + 1
+    out = []
+    for sp in world.specs:
+        slabs = {}
+        for r, b in bufs[sp.name].items():
+            if r == step.dead:
+                continue
+            anchor, cap = world.geom[sp.name][r]
+            slabs[r] = (b.ptr, cap, anchor)
+        out.append(etp.TensorDesc(sp.total_units, sp.unit_bytes, slabs, n_ranks, class_index[sp.klass],
+                                  images[sp.name].data_ptr(), 0, sp.total_units))
+    return out
+
+
+def run_param_step(ctx, world, bufs, images, step_idx, streams):
+    step = world.steps[step_idx]
+    plans = make_plans(step)
+    klasses = sorted(plans)
+    class_index = {k: i for i, k in enumerate(klasses)}
+    descs = tensor_descs(world, bufs, images, step, class_index)
+    rep = etp.etp_reshard_params(ctx, descs, [plans[k] for k in klasses], streams.copy.cuda_stream, streams.reload.cuda_stream)
+    streams.sync()
+    return rep
+
+
+def compare_params(world, bufs, expect, dead_ranks):
+    for sp in world.specs:
+        for r, b in bufs[sp.name].items():
+            assert b.guards_intact(), f"{sp.name} rank {r}: guard band overwritten"
+            if r in dead_ranks:
+                continue
+            got = b.payload()
+            assert got.tobytes() == expect[sp.name][r].tobytes(), f"{sp.name} rank {r}: slab differs from the oracle image"
+
+
+@pytest.mark.parametrize("mode", ["span", "tight", "full"])
+@pytest.mark.parametrize("policy", ["floor", "ceil_first"])
+@pytest.mark.parametrize("dead", [0, 1, 2, 3])
+def test_config1_params_bit_exact(ctx, mode, policy, dead):
+    cfg = get_config("1")
+    world = H.build_param_world(cfg, side=LibSide, mode=mode, new_policy=policy, failed=(dead,))
+    expect, stats = H.oracle_reshard_params(world, 0)
+    bufs, images = upload_param_world(world)
+    rep = run_param_step(ctx, world, bufs, images, 0, Streams())
+    compare_params(world, bufs, expect, {dead})
+    assert rep["d2d_bytes"] == stats["d2d_bytes"] and rep["h2d_bytes"] == stats["h2d_bytes"]
+    assert rep["kept_bytes"] == stats["kept_bytes"]
+    assert rep["n_kernel_launches"] >= (1 if stats["d2d_bytes"] else 0)
+    if mode != "tight":
+        assert rep["n_phases"] == 1
+
+
+@pytest.mark.parametrize("image", ["pinned", "device"])
+@pytest.mark.parametrize("tma_min", [None, 16, 1 << 62])
+def test_mid_params_bit_exact_every_copy_path(ctx, image, tma_min):
+    """Multi-tile sizes with ragged tails; TMA-only, vector-only and mixed routing of the same plan."""
+    world = H.build_param_world(MID, side=LibSide, mode="span")
+    expect, stats = H.oracle_reshard_params(world, 0)
+    bufs, images = upload_param_world(world, image)
+    default = ctx.get_option(etp.OPT_TMA_MIN_BYTES)
+    try:
+        if tma_min is not None:
+            ctx.set_option(etp.OPT_TMA_MIN_BYTES, tma_min)
+        rep = run_param_step(ctx, world, bufs, images, 0, Streams())
+    finally:
+        ctx.set_option(etp.OPT_TMA_MIN_BYTES, default)
+    compare_params(world, bufs, expect, {1})
+    assert rep["d2d_bytes"] == stats["d2d_bytes"]
+    assert rep["h2d_bytes"] + rep["reload_dev_bytes"] == stats["h2d_bytes"]
+
+
+@pytest.mark.parametrize("mode", ["span", "tight"])
+def test_sequential_failures_bit_exact(ctx, mode):
+    """Config-5a style chain (PAPER.md:206 k -> k-1 switches) on the mid shape: 4 -> 3 -> 2, in place."""
+    world = H.build_param_world(MID, side=LibSide, mode=mode, failed=(2, 0))
+    bufs, images = upload_param_world(world)
+    cur, dead = world.slabs, set()
+    streams = Streams()
+    for i in range(2):
+        expect, _ = H.oracle_reshard_params(world, i, cur)
+        rep = run_param_step(ctx, world, bufs, images, i, streams)
+        dead.add(world.steps[i].dead)
+        compare_params(world, bufs, expect, dead)
+        cur = expect
+        if mode == "tight":
+            assert rep["n_phases"] >= 1
+
+
+def test_same_stream_and_skip_options(ctx):
+    world = H.build_param_world(MID, side=LibSide, mode="span")
+    expect, stats = H.oracle_reshard_params(world, 0)
+    bufs, images = upload_param_world(world)
+    s = Streams()
+    s.reload = s.copy                       # one stream for both legs
+    run_param_step(ctx, world, bufs, images, 0, s)
+    compare_params(world, bufs, expect, {1})
+    # SKIP_D2D + SKIP_RELOAD touch nothing
+    bufs2, images2 = upload_param_world(world)
+    ctx.set_option(etp.OPT_SKIP_D2D, 1)
+    ctx.set_option(etp.OPT_SKIP_RELOAD, 1)
+    try:
+        run_param_step(ctx, world, bufs2, images2, 0, Streams())
+    finally:
+        ctx.set_option(etp.OPT_SKIP_D2D, 0)
+        ctx.set_option(etp.OPT_SKIP_RELOAD, 0)
+    compare_params(world, bufs2, world.slabs, {1})
+
+
+def test_param_errors(ctx):
+    world = H.build_param_world(get_config("1"), side=LibSide, mode="span")
+    bufs, images = upload_param_world(world)
+    step = world.steps[0]
+    plans = make_plans(step)
+    klasses = sorted(plans)
+    ci = {k: i for i, k in enumerate(klasses)}
+    descs = tensor_descs(world, bufs, images, step, ci)
+    pl = [plans[k] for k in klasses]
+    s = Streams()
+    bad = tensor_descs(world, bufs, images, step, ci)
+    bad[0].host_image = 0
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_reshard_params(ctx, bad, pl, s.copy.cuda_stream, s.reload.cuda_stream)
+    assert e.value.status == 4              # NO_SOURCE
+    bad = tensor_descs(world, bufs, images, step, ci)
+    r0 = min(bad[4].slabs)
+    p, cap, a = bad[4].slabs[r0]
+    bad[4].slabs[r0] = (p + 8, cap, a)
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_reshard_params(ctx, bad, pl, s.copy.cuda_stream, s.reload.cuda_stream)
+    assert e.value.status == 2              # ALIGNMENT
+    bad = tensor_descs(world, bufs, images, step, ci)
+    for r in bad[4].slabs:
+        p, cap, a = bad[4].slabs[r]
+        bad[4].slabs[r] = (p, 3, a)
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_reshard_params(ctx, bad, pl, s.copy.cuda_stream, s.reload.cuda_stream)
+    assert e.value.status == 3              # CAPACITY
+    s.sync()
+    compare_params(world, bufs, world.slabs, {step.dead})     # failed calls wrote nothing
+    del descs
+
+
+# ------------------------------------------------------------------------------------------------ KV
+def run_kv(ctx, world, budget, backup="pinned", head_cap=None):
+    st = world.steps[0]
+    g = world.g
+    new_table, evicted, pairs = OS.page_table_rewrite(world.table, world.seq_lens, world.last_use, g.block_size, budget)
+    snap = {r: p for r, p in world.pools.items() if r != st.dead}
+    hb = world.host_backup if backup else None
+    expect, stats = OS.apply_kv(st.tasks["head"], snap, world.anchors, g, hb, world.host_heads, world.host_head0, pairs)
+    bufs = {r: DevBuf(p) for r, p in snap.items()}
+    if backup == "pinned":
+        img = pinned(world.host_backup)
+    elif backup == "device":
+        img = torch.from_numpy(world.host_backup).cuda()
+    else:
+        img = None
+    plan = make_plans(st)["head"]
+    n_ranks = max(world.pools) + 1
+    table = world.table.copy()
+    s = Streams()
+    ev, rep = etp.etp_reshard_kv(ctx, n_layers=g.n_layers, n_blocks=g.n_blocks, block_size=g.block_size, head_cap=g.head_cap,
+                                 head_dim=g.head_dim, elem_bytes=g.elem_bytes, layout=g.layout,
+                                 pools={r: b.ptr for r, b in bufs.items()}, head_anchor=world.anchors, n_ranks=n_ranks,
+                                 table=table, seq_lens=world.seq_lens, last_use=world.last_use, head_plan=plan,
+                                 new_block_budget=budget, host_backup=img.data_ptr() if img is not None else 0,
+                                 host_heads=world.host_heads, host_head0=world.host_head0,
+                                 copy_stream=s.copy.cuda_stream, reload_stream=s.reload.cuda_stream)
+    s.sync()
+    assert np.array_equal(table, new_table)
+    for r, b in bufs.items():
+        assert b.guards_intact()
+        assert b.payload().tobytes() == expect[r].tobytes(), f"pool of rank {r} differs from the oracle image"
+    return ev, evicted, rep, stats
+
+
+@pytest.mark.parametrize("layout", [0, 1])
+@pytest.mark.parametrize("dead", [0, 1, 2, 3])
+@pytest.mark.parametrize("budget", [None, 12])
+def test_config1_kv_bit_exact(ctx, layout, dead, budget):
+    world = H.build_kv_world(get_config("1"), side=LibSide, layout=layout, failed=(dead,))
+    bud = world.g.n_blocks if budget is None else budget
+    ev, evicted, rep, stats = run_kv(ctx, world, bud)
+    assert ev == evicted
+    assert rep["d2d_bytes"] == stats["d2d_bytes"] and rep["h2d_bytes"] == stats["h2d_bytes"]
+
+
+@pytest.mark.parametrize("layout", [0, 1])
+@pytest.mark.parametrize("backup", ["pinned", "device"])
+@pytest.mark.parametrize("policy", ["floor", "ceil_first"])
+def test_mid_kv_bit_exact(ctx, layout, backup, policy):
+    """Ragged sequence lengths (a 1-block sequence, a partial last block), 8 KV heads 4 -> 3, head_cap with slack."""
+    cfg = dataclasses.replace(MID, model=dataclasses.replace(MID.model, n_layers=2))
+    world = H.build_kv_world(cfg, side=LibSide, layout=layout, new_policy=policy, seq_lens=[300, 7, 1000], head_cap=4)
+    ev, evicted, rep, stats = run_kv(ctx, world, world.g.n_blocks, backup)
+    assert ev == evicted == []
+    assert rep["d2d_bytes"] == stats["d2d_bytes"]
+    assert rep["h2d_bytes"] + rep["reload_dev_bytes"] == stats["h2d_bytes"]
+
+
+def test_kv_budget_shrink_and_no_backup(ctx):
+    cfg = dataclasses.replace(MID, model=dataclasses.replace(MID.model, n_layers=1))
+    world = H.build_kv_world(cfg, side=LibSide, layout=0, seq_lens=[300, 7, 1000], head_cap=4)
+    live = int(((world.seq_lens + 15) // 16).sum())
+    ev, evicted, rep, stats = run_kv(ctx, world, live - 10)
+    assert ev == evicted and len(ev) >= 1
+    # reading K4: no backup -> reload heads untouched, every live sequence reported
+    ev, evicted, rep, stats = run_kv(ctx, world, world.g.n_blocks, backup=None)
+    assert sorted(ev) == [0, 1, 2] and rep["h2d_bytes"] == 0
+
+
+def test_kv_staged_reload_mode(ctx):
+    cfg = dataclasses.replace(MID, model=dataclasses.replace(MID.model, n_layers=2))
+    world = H.build_kv_world(cfg, side=LibSide, layout=0, seq_lens=[300, 7, 1000], head_cap=4)
+    ctx.set_option(etp.OPT_KV_RELOAD_MODE, 1)
+    try:
+        run_kv(ctx, world, world.g.n_blocks, "pinned")
+    finally:
+        ctx.set_option(etp.OPT_KV_RELOAD_MODE, 0)
+
+
+# ------------------------------------------------------------------------------------------------ interval copy (5b)
+@pytest.mark.parametrize("n,hi", [(0, 1 << 20), (1, 1 << 20), (300, 4 << 20), (20000, 8 << 10)])
+@pytest.mark.parametrize("tma_min", [None, 16, 1 << 62])
+def test_copy_intervals_bit_exact(ctx, n, hi, tma_min):
+    """Config 5b recipe at a size the host reproduces in seconds: log-uniform sizes from 16 B, random 16-B aligned
+    offsets, overlapping sources, disjoint destinations with random gaps (gaps must keep their old bytes)."""
+    src_arena = 64 << 20
+    if n:
+        so, do, sz, dst_arena = microbench_intervals(n, 16, hi, 1234 + n, src_arena, max_total=256 << 20)
+    else:
+        so = do = sz = np.zeros(0, dtype=np.int64)
+        dst_arena = 1024
+    rng = np.random.default_rng(5)
+    src = rng.integers(0, 256, src_arena, dtype=np.uint8)
+    dst0 = rng.integers(0, 256, dst_arena, dtype=np.uint8)
+    expect = dst0.copy()
+    for a, b, m in zip(so, do, sz):
+        expect[b:b + m] = src[a:a + m]
+    S, D = DevBuf(src), DevBuf(dst0)
+    default = ctx.get_option(etp.OPT_TMA_MIN_BYTES)
+    stream = torch.cuda.Stream()
+    try:
+        if tma_min is not None:
+            ctx.set_option(etp.OPT_TMA_MIN_BYTES, tma_min)
+        rep = etp.etp_copy_intervals(ctx, so + S.ptr, do + D.ptr, sz, stream.cuda_stream)
+    finally:
+        ctx.set_option(etp.OPT_TMA_MIN_BYTES, default)
+    stream.synchronize()
+    assert D.guards_intact() and S.guards_intact()
+    assert D.payload().tobytes() == expect.tobytes()
+    assert rep["d2d_bytes"] == int(sz.sum())
+    assert S.payload().tobytes() == src.tobytes()
+
+
+def test_copy_intervals_errors(ctx):
+    S, D = DevBuf(np.zeros(4096, np.uint8)), DevBuf(np.zeros(4096, np.uint8))
+    for so, do, sz, status in [(8, 0, 16, 2), (0, 0, 24, 2), (0, 0, -16, 1)]:
+        with pytest.raises(etp.EtpError) as e:
+            etp.etp_copy_intervals(ctx, np.array([S.ptr + so]), np.array([D.ptr + do]), np.array([sz]))
+        assert e.value.status == status

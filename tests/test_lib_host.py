@@ -1,0 +1,211 @@
+"""Host logic of libetp.so against the oracle (no GPU needed): the library loads and exports every symbol
+include/etp.h declares; etp_partition / etp_cmm_plan / etp_plan_create / etp_page_table_rewrite agree with the
+oracle exactly (the plan is unique under the readings of DESIGN.md, so task lists are compared verbatim);
+status codes of the error paths."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2511_11617_b200 as etp
+from oracle import planning as OP
+from oracle import state as OS
+from tests import harness as H
+from workloads import get_config
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def header_symbols():
+    src = open(os.path.join(ROOT, "include", "etp.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(etp_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    L = etp.lib()
+    syms = header_symbols()
+    assert set(syms) == set(etp.EXPORTS), (syms, etp.EXPORTS)
+    for s in syms:
+        assert getattr(L, s) is not None
+    assert "sm_100a" in etp.etp_version()
+
+
+def test_binding_does_not_import_oracle():
+    for f in os.listdir(os.path.join(ROOT, "paper_2511_11617_b200")):
+        if f.endswith(".py"):
+            txt = open(os.path.join(ROOT, "paper_2511_11617_b200", f)).read()
+            assert "oracle" not in txt.replace("``oracle/``", ""), f
+    for f in os.listdir(os.path.join(ROOT, "paper_2511_11617_b200", "csrc")):
+        assert "oracle" not in open(os.path.join(ROOT, "paper_2511_11617_b200", "csrc", f)).read(), f
+
+
+def test_fig3_through_the_c_abi(golden_dir):
+    """PAPER.md:144 (Fig. 3): 1024 rows, 4 -> 3, GPU:2 (rank 1) fails."""
+    assert etp.etp_partition(1024, 3) == [0, 341, 682, 1024]
+    old = [(0, 0, 256, 1), (1, 256, 512, 0), (2, 512, 768, 1), (3, 768, 1024, 1)]
+    p = etp.etp_cmm_plan(old, 3)
+    K, T, R = etp.KEEP, etp.TRANSFER, etp.RELOAD
+    assert p.tasks() == [(K, 0, 0, 0, 256), (R, -1, 0, 256, 341), (R, -1, 2, 341, 512), (K, 2, 2, 512, 682),
+                         (T, 2, 3, 682, 768), (K, 3, 3, 768, 1024)]
+    st = p.stats()
+    assert (st["keep_units"], st["transfer_units"], st["reload_units"], st["reload_lower_bound"]) == (682, 86, 256, 256)
+    assert p.new_layout() == [(0, 0, 341, 1), (2, 341, 682, 1), (3, 682, 1024, 1)]
+
+
+@pytest.mark.parametrize("policy", ["floor", "ceil_first"])
+def test_partition_matches_oracle(policy):
+    rng = np.random.default_rng(7)
+    for _ in range(400):
+        M = int(rng.integers(1, 17))
+        S = int(rng.integers(M, 200000))
+        a = int(rng.choice([1, 1, 1, 2, 8, 128]))
+        if -(-S // a) < M:
+            continue
+        assert etp.etp_partition(S, M, policy, a) == OP.partition(S, M, policy, a)
+    for S in (8, 17408, 14336, 128, 151936, 128256, 688, 4):
+        for M in (1, 2, 3, 4):
+            assert etp.etp_partition(S, M, policy) == OP.partition(S, M, policy)
+
+
+def random_layout(rng, max_n=8, max_h=3000):
+    n = int(rng.integers(2, max_n + 1))
+    H_ = int(rng.integers(n, max_h))
+    cuts = sorted(rng.choice(np.arange(1, H_), size=n - 1, replace=False).tolist()) if n > 1 else []
+    b = [0] + cuts + [H_]
+    n_dead = int(rng.integers(0, min(3, n - 1) + 1))
+    dead = set(rng.choice(n, size=n_dead, replace=False).tolist())
+    ranks = sorted(rng.choice(np.arange(0, 2 * n), size=n, replace=False).tolist())
+    return [(int(ranks[i]), b[i], b[i + 1], 0 if i in dead else 1) for i in range(n)]
+
+
+def test_cmm_plan_matches_oracle_random():
+    rng = np.random.default_rng(11)
+    for it in range(400):
+        old = random_layout(rng)
+        n_alive = sum(a for (_, _, _, a) in old)
+        M = int(rng.integers(1, n_alive + 1))
+        Ht = max(e for (_, _, e, _) in old)
+        tb = None
+        if it % 3 and Ht >= M:
+            tb = OP.partition(Ht, M, "ceil_first" if it % 2 else "floor")
+        tasks, new = OP.cmm_plan(old, M, tb)
+        p = etp.etp_cmm_plan(old, M, tb)
+        assert p.tasks() == tasks
+        assert p.new_layout() == new
+        st, ref = p.stats(), OP.plan_stats(tasks)
+        for k in ref:
+            assert st[k] == ref[k]
+        assert st["reload_lower_bound"] == OP.eq1_reload_lower_bound(old, [b for (_, b, _, _) in new] + [Ht])
+        assert st["reload_units"] == st["reload_lower_bound"]          # Eq. 1 attained
+
+
+def test_comparison_planners_match_oracle():
+    """PAPER.md:204 / Table II: Greedy (no P2P for gaps) and Full Reload (no reuse)."""
+    rng = np.random.default_rng(13)
+    for _ in range(100):
+        old = random_layout(rng)
+        M = sum(a for (_, _, _, a) in old)
+        g_tasks, _ = OP.greedy_plan(old, M)
+        f_tasks, _ = OP.full_reload_plan(old, M)
+        pg = etp.etp_plan_create(etp.PLAN_GREEDY, old, M)
+        pf = etp.etp_plan_create(etp.PLAN_FULL_RELOAD, old, M)
+        assert OP._merge_adjacent(pg.tasks()) == g_tasks
+        assert pf.tasks() == f_tasks
+        pc = etp.etp_cmm_plan(old, M)
+        assert pc.stats()["reload_units"] <= pg.stats()["reload_units"] <= pf.stats()["reload_units"]
+
+
+def test_replicated_sources_reading_c7():
+    old = [(0, 0, 6, 1), (1, 4, 10, 1), (2, 8, 12, 0)]
+    tasks, new = OP.cmm_plan(old, 2)
+    p = etp.etp_cmm_plan(old, 2)
+    assert p.tasks() == tasks and p.new_layout() == new
+
+
+def test_scenario_plans_of_every_config_match():
+    class LibSide:
+        @staticmethod
+        def partition(Hh, M, policy="floor", align=1):
+            return etp.etp_partition(Hh, M, policy, align)
+
+        @staticmethod
+        def plan(old, M, tb=None):
+            p = etp.etp_cmm_plan(old, M, tb)
+            return p.tasks(), p.new_layout()
+
+    for key in ("1", "2", "2b", "3", "4", "5a"):
+        cfg = get_config(key)
+        a = H.plan_scenario(cfg, H.OracleSide)
+        b = H.plan_scenario(cfg, LibSide)
+        assert len(a) == len(b)
+        for sa, sb in zip(a, b):
+            assert sa.tasks == sb.tasks and sa.new == sb.new, key
+
+
+def test_page_table_rewrite_matches_oracle():
+    rng = np.random.default_rng(17)
+    for _ in range(200):
+        n_seqs = int(rng.integers(1, 9))
+        bs = int(rng.choice([1, 4, 16]))
+        lens = rng.integers(0, 9 * bs, n_seqs).astype(np.int32)
+        per = (lens + bs - 1) // bs
+        live = int(per.sum())
+        n_blocks = live + int(rng.integers(0, 6))
+        ids = rng.permutation(max(n_blocks, 1))[:live]
+        mb = max(int(per.max()), 1)
+        table = np.full((n_seqs, mb), -1, dtype=np.int32)
+        k = 0
+        for s in range(n_seqs):
+            table[s, : per[s]] = ids[k : k + per[s]]
+            k += per[s]
+        last_use = rng.integers(0, 5, n_seqs).astype(np.int64)        # ties on purpose
+        budget = int(rng.integers(0, n_blocks + 1))
+        ref_table, ref_ev, ref_pairs = OS.page_table_rewrite(table, lens, last_use, bs, budget)
+        t = table.copy()
+        ev, pairs = etp.etp_page_table_rewrite(t, lens, last_use, bs, budget)
+        assert ev == ref_ev
+        assert np.array_equal(t, ref_table)
+        assert pairs == [(bo, bn) for (_, _, bo, bn) in ref_pairs]
+
+
+def test_page_table_golden_through_the_c_abi(golden_dir):
+    from tests.test_oracle_state import load_pt_golden
+    g = load_pt_golden(golden_dir)
+    for budget, evicted, tab in g["cases"]:
+        t = np.array(g["table"], dtype=np.int32)
+        ev, pairs = etp.etp_page_table_rewrite(t, g["seq_lens"], g["last_use"], g["block_size"], budget)
+        assert ev == evicted, budget
+        assert np.array_equal(t, tab), budget
+
+
+def test_error_statuses():
+    E = etp.EtpError
+    with pytest.raises(E) as e:
+        etp.etp_partition(4, 5)
+    assert e.value.status == 5                      # UNSUPPORTED: fewer units than shards (reading P4)
+    with pytest.raises(E) as e:
+        etp.etp_partition(10, 0)
+    assert e.value.status == 1
+    with pytest.raises(E) as e:
+        etp.etp_cmm_plan([(0, 0, 4, 1), (1, 4, 8, 0)], 2)      # M > #alive (reading C6)
+    assert e.value.status == 1
+    with pytest.raises(E) as e:
+        etp.etp_cmm_plan([(0, 0, 4, 1), (0, 4, 8, 1)], 1)      # duplicate rank id
+    assert e.value.status == 1
+    with pytest.raises(E) as e:
+        etp.etp_cmm_plan([(0, 0, 4, 1), (1, 4, 8, 1)], 2, [0, 5, 7])   # bounds do not tile [0,H)
+    assert e.value.status == 1
+    # an empty interval is a joining rank (reading C6)
+    p = etp.etp_cmm_plan([(0, 0, 8, 1), (1, 8, 8, 1)], 2)
+    assert p.tasks() == OP.cmm_plan([(0, 0, 8, 1), (1, 8, 8, 1)], 2)[0]
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(etp.EtpError) as e:
+        etp.Context(0)
+    assert e.value.status == 6                      # ETP_ERR_CUDA
