@@ -131,7 +131,8 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
     ETP_CUDA_OK(cudaSetDevice(c->device));
     CtxExtra* x = extra(c);
     const bool skip_d2d = c->opts[ETP_OPT_SKIP_D2D] != 0, skip_reload = c->opts[ETP_OPT_SKIP_RELOAD] != 0;
-    const size_t n_ph = std::max(w->phases.size(), w->host_gather.size());
+    size_t n_ph = std::max(w->phases.size(), w->host_gather.size());
+    for (const DmaCopy& d : w->dma) n_ph = std::max(n_ph, (size_t)d.phase + 1);   // a reload may be the last phase
     w->phases.resize(n_ph);
     w->host_gather.resize(n_ph);
 

@@ -63,6 +63,15 @@ _IH_MEAN = 4 * 65535 / 2.0
 _IH_STD = math.sqrt(4 * (65536.0 ** 2 - 1) / 12.0)
 
 
+def normal16_at(idx: torch.Tensor, seed: int, stream: int, std: float, dtype: torch.dtype) -> torch.Tensor:
+    """Value of the 16-bit N(0, std) stream at arbitrary int64 element indices (any shape)."""
+    scale = np.float32(std / _IH_STD)
+    h = hash64(idx, seed, stream)
+    s = (h & 0xFFFF) + (_lsr(h, 16) & 0xFFFF) + (_lsr(h, 32) & 0xFFFF) + (_lsr(h, 48) & 0xFFFF)
+    v = (s.to(torch.float32) - np.float32(_IH_MEAN)) * float(scale)
+    return v.to(dtype)
+
+
 def fill_normal16(seed: int, stream: int, elem_offset: int, n: int, std: float, dtype: torch.dtype,
                   device="cpu", out: torch.Tensor | None = None) -> torch.Tensor:
     """16-bit float tensor, approximately N(0, std): sum of the four 16-bit fields of hash64(index)
@@ -70,15 +79,27 @@ def fill_normal16(seed: int, stream: int, elem_offset: int, n: int, std: float, 
     assert dtype in (torch.float16, torch.bfloat16)
     if out is None:
         out = torch.empty(n, dtype=dtype, device=device)
-    scale = np.float32(std / _IH_STD)
     for a in range(0, n, _CHUNK):
         b = min(n, a + _CHUNK)
         idx = torch.arange(elem_offset + a, elem_offset + b, dtype=torch.int64, device=out.device)
-        h = hash64(idx, seed, stream)
-        s = (h & 0xFFFF) + (_lsr(h, 16) & 0xFFFF) + (_lsr(h, 32) & 0xFFFF) + (_lsr(h, 48) & 0xFFFF)
-        v = (s.to(torch.float32) - np.float32(_IH_MEAN)) * float(scale)
-        out[a:b] = v.to(dtype)
+        out[a:b] = normal16_at(idx, seed, stream, std, dtype)
     return out
+
+
+def fill_kv_pool(pool: torch.Tensor, rows: int, heads_in_pool: int, dim: int, slot0: int, head0: int, n: int,
+                 n_kv_heads: int, seed: int, stream: int, dtype: torch.dtype, row_chunk: int = 1 << 16) -> None:
+    """Paged-KV content that is a pure function of (row, head, d): element d of KV head ``h`` at pool row ``row``
+    (row = flattened (layer, K|V, block, token)) has the value of stream index (row * n_kv_heads + h) * dim + d,
+    N(0,1).  Writes heads head0..head0+n-1 into slots slot0..slot0+n-1 of ``pool`` viewed as
+    [rows][heads_in_pool][dim] (token-major layout); every other slot is left as it is."""
+    v = pool.view(dtype).view(rows, heads_in_pool, dim)
+    d = torch.arange(dim, dtype=torch.int64, device=pool.device)
+    hh = torch.arange(head0, head0 + n, dtype=torch.int64, device=pool.device)
+    for a in range(0, rows, row_chunk):
+        b = min(rows, a + row_chunk)
+        r = torch.arange(a, b, dtype=torch.int64, device=pool.device)
+        idx = ((r[:, None, None] * n_kv_heads + hh[None, :, None]) * dim) + d[None, None, :]
+        v[a:b, slot0:slot0 + n, :] = normal16_at(idx, seed, stream, 1.0, dtype)
 
 
 def torch_dtype(name: str) -> torch.dtype:
