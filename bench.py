@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""bench.py — one "step" = one pass of the whole hot path (partition, CMM plan, lowering, device
+interval copy, host reload, page-table rewrite) over the full model state of one BASELINE.json config, through the C ABI.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+Metric (BASELINE.json): moved-bytes GB/s of the reshard (+ full-state reshard ms).
+  value      inputs resident in HBM: the failed rank's image / KV backup are device tensors, so every moved byte goes
+             through the interval-copy kernel.  GB/s = (TRANSFER + RELOAD bytes) / step time.
+  e2e        the same call with the reload sources in PINNED HOST memory: chunked cudaMemcpyAsync + zero-copy KV gather on
+             the reload stream overlapped with the copy kernel; host->device bytes are inside the timed region.
+  roofline   interval-copy kernel: 2 * bytes it moved / its device time (CUDA events recorded by the library on the
+             launching stream), against MEASURED_PEAKS.json hbm_gbs.
+  cpu_baseline / --impl reference: the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+Multi-GPU: "replicas only" — every rank reshards its own replica, no collective on the data path.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "etp_reshard_moved_bytes_throughput"
+UNIT = "GB/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="2")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--layers", type=int, default=0, help="debug: fewer layers (marks the result as reduced)")
+    ap.add_argument("--seqs", type=int, default=0, help="debug: fewer sequences (marks the result as reduced)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget-s", type=float, default=15.0, help="CPU seconds of oracle work in the cpu_baseline leg")
+    ap.add_argument("--ref-layers", type=int, default=2, help="--impl reference: layers in the per-step sample")
+    return ap.parse_args()
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx, self.p = gpu_index, None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                                       "-i", str(self.idx)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+            out, _ = self.p.communicate()
+        sm, smax, reasons = [], 0.0, set()
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                smax = max(smax, float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        # under load = the upper half of the samples (the sampler also sees the idle host-lowering gaps)
+        load = sm[len(sm) // 2:] if sm else []
+        med = load[len(load) // 2] if load else None
+        return {"sm_mhz": med, "sm_max_mhz": smax or None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ================================================================================================ the oracle legs
+def oracle_sample_worlds(cfg, n_layers, device):
+    """Inputs of the oracle legs: parameters of `n_layers` layers (no embedding) + the KV planes of ONE layer for every
+    sequence, as host arrays.  Seeded generators only; partition / plan / placement by the oracle."""
+    from tests import harness as H
+    from workloads.configs import scaled
+    pw = H.build_param_world(scaled(cfg, n_layers=n_layers, vocab=0), mode="span", device=device)
+    kw = H.build_kv_world(scaled(cfg, n_layers=1, vocab=0), device=device)
+    return pw, kw
+
+
+def oracle_pass(pw, kw):
+    """One pass of the oracle over the sample: S1 + S2 (oracle planner), S4/S5 element by element, S6.
+    Returns (moved bytes, seconds)."""
+    from oracle import state as OS
+    from tests import harness as H
+    t0 = time.perf_counter()
+    moved = 0
+    steps = H.plan_scenario(pw.cfg, H.OracleSide)          # S1 + S2 again, as a step does
+    pw2 = H.ParamWorld(pw.cfg, pw.specs, steps, pw.geom, pw.unsharded, pw.slabs)
+    _, st = H.oracle_reshard_params(pw2, 0)
+    moved += st["d2d_bytes"] + st["h2d_bytes"]
+    ksteps = H.plan_scenario(kw.cfg, H.OracleSide)
+    g = kw.g
+    _, evicted, pairs = OS.page_table_rewrite(kw.table, kw.seq_lens, kw.last_use, g.block_size, g.n_blocks)
+    snap = {r: p for r, p in kw.pools.items() if r != ksteps[0].dead}
+    _, st = OS.apply_kv(ksteps[0].tasks["head"], snap, kw.anchors, g, kw.host_backup, kw.host_heads, kw.host_head0, pairs)
+    moved += st["d2d_bytes"] + st["h2d_bytes"]
+    return moved, time.perf_counter() - t0
+
+
+def cpu_baseline_leg(cfg, device, budget_s):
+    """The oracle as it stands on a bounded sample (~budget_s of CPU work): layer samples of 2 parameter layers + 1 KV
+    layer, repeated on fresh layer data until the budget is used."""
+    n_layers = 2
+    pw, kw = oracle_sample_worlds(cfg, n_layers, device)
+    moved = secs = 0.0
+    passes = 0
+    while secs < budget_s and passes < 64:
+        m, s = oracle_pass(pw, kw)
+        moved += m
+        secs += s
+        passes += 1
+    return {"value": moved / secs / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"{passes} passes over parameters of {n_layers} layers (no embedding) + KV planes of 1 layer x "
+                      f"{cfg.kv.n_seqs} seqs x {cfg.kv.seq_len} tok of config {cfg.key}; {moved / 1e9:.2f} GB moved in {secs:.1f} s",
+            "seconds": secs}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle timed on the host cores, same metric / config; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import torch
+    from workloads import get_config
+    cfg = get_config(args.config)
+    device = "cuda:0" if torch.cuda.is_available() else "cpu"
+    n_layers = args.ref_layers
+    pw, kw = oracle_sample_worlds(cfg, n_layers, device)
+    for _ in range(args.warmup):
+        oracle_pass(pw, kw)
+    moved = secs = 0.0
+    for _ in range(args.steps):
+        m, s = oracle_pass(pw, kw)
+        moved += m
+        secs += s
+    val = moved / secs / 1e9
+    sample = (f"per step: parameters of {n_layers} layers (no embedding) + KV planes of 1 layer x {cfg.kv.n_seqs} seqs x "
+              f"{cfg.kv.seq_len} tok of config {cfg.key}; {moved / args.steps / 1e9:.3f} GB moved per step")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+            "config": {"workload": f"config {cfg.key}: {cfg.note}", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ================================================================================================ the CUDA path
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    import paper_2511_11617_b200 as etp
+    from paper_2511_11617_b200.state import ModelState
+    from workloads import get_config
+    from workloads.configs import scaled
+
+    cfg = get_config(args.config)
+    reduced = bool(args.layers or args.seqs)
+    if reduced:
+        cfg = scaled(cfg, n_layers=args.layers or None, n_seqs=args.seqs or None)
+    hbm_peak, peak_src = load_peaks()
+
+    t_build = time.perf_counter()
+    state = ModelState(cfg, device=dev, image="both")
+    t_build = time.perf_counter() - t_build
+    ctx = etp.Context(local_rank)
+    ctx.set_option(etp.OPT_TIME_KERNELS, 1)
+    cs, rs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def one_step(image):
+        """One pass S1-S6.  Returns (device ms from first enqueue to both streams done, reports)."""
+        e0, e1, er = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event()
+        e0.record(cs)
+        rep = state.reshard(ctx, 0, image, cs.cuda_stream, rs.cuda_stream, replan=True)
+        er.record(rs)
+        cs.wait_event(er)
+        e1.record(cs)
+        e1.synchronize()
+        return e0.elapsed_time(e1), rep
+
+    def timed(image, K, W):
+        for _ in range(W):
+            one_step(image)
+        barrier()
+        tot_ms, moved, launches = 0.0, 0, 0
+        h2d = 0
+        rep = None
+        for _ in range(K):
+            ms, rep = one_step(image)
+            tot_ms += ms
+            for r in (rep["params"], rep["kv"]):
+                if r:
+                    moved += r["d2d_bytes"] + r["h2d_bytes"] + r["reload_dev_bytes"]
+                    h2d += r["h2d_bytes"]
+                    launches += r["n_kernel_launches"]
+        barrier()
+        if world > 1:
+            t = torch.tensor([tot_ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            tot_ms = float(t.item())
+        return tot_ms, moved, h2d, launches, rep
+
+    def kernel_leg(image, K):
+        """Device time of the interval-copy kernel, params call and KV call separately (events on the copy stream)."""
+        kms, kbytes, kl = 0.0, 0, 0
+        st = state.steps[0]
+        for _ in range(K):
+            if state.specs:
+                r = state.prepared(0, image).run(ctx, [st.plans[k] for k in state.klasses], cs.cuda_stream, rs.cuda_stream)
+                ms, n = ctx.kernel_time()
+                torch.cuda.synchronize(dev)
+                kms += ms
+                kl += n
+                kbytes += r["d2d_bytes"] + (r["reload_dev_bytes"] if image == "device" else 0)
+            if state.kv is not None:
+                saved, state.specs = state.specs, []
+                try:
+                    rep = state.reshard(ctx, 0, image, cs.cuda_stream, rs.cuda_stream, replan=False)
+                finally:
+                    state.specs = saved
+                ms, n = ctx.kernel_time()
+                torch.cuda.synchronize(dev)
+                kms += ms
+                kl += n
+                r = rep["kv"]
+                kbytes += r["d2d_bytes"] + (r["reload_dev_bytes"] if image == "device" else 0)
+        return kms, kbytes, kl
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    K, W = args.steps, max(args.warmup, 0)
+    tot_ms, moved, _, launches, rep = timed("device", K, W)
+    kms, kbytes, kl = kernel_leg("device", K)
+    e_ms, e_moved, e_h2d, e_launches, e_rep = timed("pinned", K, W)
+    # kernel (a) alone on the TRANSFER bytes only (reload skipped): the north_star's "moved bytes vs HBM peak" figure
+    ctx.set_option(etp.OPT_SKIP_RELOAD, 1)
+    try:
+        for _ in range(W):
+            kernel_leg("pinned", 1)
+        d_kms, d_bytes, d_kl = kernel_leg("pinned", K)
+    finally:
+        ctx.set_option(etp.OPT_SKIP_RELOAD, 0)
+    clocks = sampler.stop() if rank == 0 else None
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    value = moved * world / (tot_ms * 1e-3) / 1e9
+    e2e = e_moved * world / (e_ms * 1e-3) / 1e9
+    achieved = 2.0 * kbytes / (kms * 1e-3) / 1e9 if kms > 0 else 0.0
+    rp, rk = rep["params"] or {}, rep["kv"] or {}
+    ep, ek = e_rep["params"] or {}, e_rep["kv"] or {}
+    sb = state.state_bytes()
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": tot_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
+        "data": "synthetic",
+        "config": {"workload": f"config {cfg.key}: {cfg.note}" + (" [REDUCED: debug run, not a bench value]" if reduced else ""),
+                   "state_GB": round((sb["param_bytes"] + sb["kv_live_bytes"]) / 1e9, 2),
+                   "moved_GB_per_step": round(moved / K / 1e9, 3),
+                   "l2": "inputs larger than L2 (every step re-reads and re-writes GBs; plans are hazard-free so a step is idempotent in place)",
+                   "replicas": world, "step": "S1 partition + S2 CMM plan + S3 lowering + S4 copy + S5 reload + S6 page table, synchronised per step"},
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": e_h2d // K, "d2h_bytes_per_step": 0,
+                "ms_per_step": e_ms / K, "h2d_GBps": e_h2d / (e_ms * 1e-3) / 1e9,
+                "note": "reload sources in pinned host memory; result stays on the device (the page table is host-side)"},
+        "gpu_launches": launches + kl + e_launches + d_kl,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+                     "traffic": None, "kernel": "etp_interval_copy_kernel", "peak_source": peak_src,
+                     "bytes_per_launch": 2.0 * kbytes / max(kl, 1), "ms_per_launch": kms / max(kl, 1), "launches": kl,
+                     "d2d_only": {"moved_bytes": d_bytes // max(K, 1), "ms": d_kms / max(K, 1),
+                                  "moved_GBps": d_bytes / (d_kms * 1e-3) / 1e9 if d_kms > 0 else None,
+                                  "hbm_frac": 2.0 * d_bytes / (d_kms * 1e-3) / 1e9 / hbm_peak if d_kms > 0 else None}},
+        "clocks": clocks,
+        "detail": {"build_s": round(t_build, 1),
+                   "device_image": {"params": rp, "kv": rk}, "pinned_image": {"params": ep, "kv": ek}},
+    }
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline_leg(get_config(args.config), str(dev), args.cpu_budget_s)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))

@@ -67,10 +67,16 @@ typedef enum {
                                     (layer, K|V) planes to the staging ring + scatter by the copy kernel           */
     ETP_OPT_GRID_CTAS = 6,       /* persistent grid size; 0 (default) = number of SMs                            */
     ETP_OPT_GATHER_CTAS = 7,     /* CTAs of the zero-copy gather launch on the reload stream (default 16)        */
+    ETP_OPT_TIME_KERNELS = 8,    /* 1 (default 0): bracket every launch of the copy kernel on the copy stream with CUDA
+                                    events (on that stream) so that etp_ctx_kernel_time can report device durations   */
     ETP_OPT__COUNT
 } etp_option;
 etp_status etp_ctx_set_option(etp_ctx* ctx, etp_option key, int64_t value);
 etp_status etp_ctx_get_option(const etp_ctx* ctx, etp_option key, int64_t* value);
+/* With ETP_OPT_TIME_KERNELS = 1: blocks until the copy-stream kernels of the LAST device call have finished and writes
+ * the sum of their device durations (CUDA events recorded on the launching stream, milliseconds) and their count.
+ * ms_out / n_out: host.  Without the option (or before any call) both are 0. */
+etp_status etp_ctx_kernel_time(etp_ctx* ctx, double* ms_out, int32_t* n_out);
 
 /* ------------------------------------------------------------------------------------------------ S1 partition
  * "some GPUs hold shard size floor(S/g_t) while others hold ceil(S/g_t)"; Algorithm 1 l.2-5
@@ -113,6 +119,11 @@ etp_status etp_plan_tasks(const etp_plan* plan, etp_task* out, int64_t cap, int6
 /* writes the M new shards (host, M entries), alive = 1 */
 etp_status etp_plan_new_layout(const etp_plan* plan, etp_shard* out, int32_t cap, int32_t* n_out);
 etp_status etp_plan_get_stats(const etp_plan* plan, etp_plan_stats* out);
+/* PAPER.md:164 "a single pass pre-allocates all destination buffers": the union span of `rank`'s old and new interval
+ * under this plan, [*first_unit, *first_unit + *span_units).  A slab with cap_units >= span_units (any anchor) holds both
+ * without wrap-around collisions, so the plan lowers to a single hazard phase (L4/L5).  A rank that holds
+ * nothing before and after gives span 0.  ETP_ERR_INVALID_ARG if the rank is in neither layout. */
+etp_status etp_plan_slab_span(const etp_plan* plan, int32_t rank, int64_t* first_unit, int64_t* span_units);
 void etp_plan_free(etp_plan* plan);
 
 /* ------------------------------------------------------------------------------------------------ S3-S5 parameters

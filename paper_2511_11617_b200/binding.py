@@ -21,7 +21,7 @@ COL_PARALLEL, ROW_PARALLEL = 0, 1
 DTYPE = {"bf16": 0, "fp16": 1}
 KV_TOKEN_MAJOR, KV_HEAD_MAJOR = 0, 1
 (OPT_SKIP_D2D, OPT_SKIP_RELOAD, OPT_TMA_MIN_BYTES, OPT_LDG_STEALS_BULK, OPT_RELOAD_CHUNK_BYTES, OPT_KV_RELOAD_MODE,
- OPT_GRID_CTAS, OPT_GATHER_CTAS) = range(8)
+ OPT_GRID_CTAS, OPT_GATHER_CTAS, OPT_TIME_KERNELS) = range(9)
 
 
 class EtpError(RuntimeError):
@@ -75,8 +75,8 @@ class etp_interval(C.Structure):
 
 
 EXPORTS = ["etp_ctx_create", "etp_ctx_destroy", "etp_last_error", "etp_version", "etp_ctx_set_option", "etp_ctx_get_option",
-           "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_tasks", "etp_plan_new_layout", "etp_plan_get_stats",
-           "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
+           "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_tasks", "etp_plan_new_layout",
+           "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
            "etp_copy_intervals"]
 
 _lib = None
@@ -95,6 +95,8 @@ def lib() -> C.CDLL:
         L.etp_ctx_destroy.restype = None
         L.etp_ctx_set_option.argtypes = [vp, C.c_int, i64]
         L.etp_ctx_get_option.argtypes = [vp, C.c_int, C.POINTER(i64)]
+        L.etp_ctx_kernel_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i32)]
+        L.etp_plan_slab_span.argtypes = [vp, i32, C.POINTER(i64), C.POINTER(i64)]
         L.etp_partition.argtypes = [C.c_int, i64, i32, C.c_int, i64, C.POINTER(i64)]
         L.etp_cmm_plan.argtypes = [C.POINTER(etp_shard), i32, C.POINTER(i64), i32, C.POINTER(vp)]
         L.etp_plan_create.argtypes = [C.c_int, C.POINTER(etp_shard), i32, C.POINTER(i64), i32, C.POINTER(vp)]
@@ -166,6 +168,12 @@ class Plan:
         _check(lib().etp_plan_new_layout(self.handle, arr, n.value, C.byref(n)))
         return [(s.rank, s.begin, s.end, s.alive) for s in arr[: n.value]]
 
+    def slab_span(self, rank: int) -> Tuple[int, int]:
+        """(first_unit, span_units) of the union of the rank's old and new interval."""
+        a, n = i64(), i64()
+        _check(lib().etp_plan_slab_span(self.handle, rank, C.byref(a), C.byref(n)))
+        return a.value, n.value
+
     def stats(self) -> Dict[str, int]:
         st = etp_plan_stats()
         _check(lib().etp_plan_get_stats(self.handle, C.byref(st)))
@@ -236,6 +244,12 @@ class Context:
         _check(lib().etp_ctx_get_option(self.handle, key, C.byref(v)))
         return v.value
 
+    def kernel_time(self) -> Tuple[float, int]:
+        """(ms, launches) of the copy-stream kernels of the last device call (needs OPT_TIME_KERNELS = 1)."""
+        ms, n = C.c_double(), i32()
+        _check(lib().etp_ctx_kernel_time(self.handle, C.byref(ms), C.byref(n)))
+        return ms.value, n.value
+
 
 class TensorDesc:
     """Python-side description of one sharded tensor: slabs = {rank: (device ptr, cap_units, anchor_unit)}."""
@@ -270,17 +284,16 @@ def etp_reshard_params(ctx: Context, tensors: Sequence[TensorDesc], plans: Seque
 
 
 class PreparedParams:
-    """Pre-marshalled arguments of etp_reshard_params, so that a timed loop pays only the C call."""
+    """Pre-marshalled tensor array of etp_reshard_params, so that a timed loop pays only the C call."""
 
-    def __init__(self, tensors: Sequence[TensorDesc], plans: Sequence[Plan]):
+    def __init__(self, tensors: Sequence[TensorDesc]):
         self.arr, self._keep = _marshal_tensors(tensors)
         self.n = len(tensors)
-        self.plans = list(plans)
-        self.ph = (vp * max(len(plans), 1))(*[p.handle for p in plans])
 
-    def run(self, ctx: Context, copy_stream: int = 0, reload_stream: int = 0) -> Dict[str, float]:
+    def run(self, ctx: Context, plans: Sequence[Plan], copy_stream: int = 0, reload_stream: int = 0) -> Dict[str, float]:
+        ph = (vp * max(len(plans), 1))(*[p.handle for p in plans])
         rep = etp_reshard_report()
-        _check(lib().etp_reshard_params(ctx.handle, self.arr, self.n, self.ph, len(self.plans), copy_stream or None, reload_stream or None,
+        _check(lib().etp_reshard_params(ctx.handle, self.arr, self.n, ph, len(plans), copy_stream or None, reload_stream or None,
                                         C.byref(rep)))
         return rep.as_dict()
 

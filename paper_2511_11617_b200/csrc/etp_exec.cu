@@ -93,6 +93,7 @@ extern "C" void etp_ctx_destroy(etp_ctx* c) {
         delete x;
     }
     for (cudaEvent_t e : c->events) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->tev) cudaEventDestroy(e);
     if (c->d_counters) cudaFree(c->d_counters);
     if (c->d_staging) cudaFree(c->d_staging);
     cudaGetLastError();
@@ -111,6 +112,20 @@ extern "C" etp_status etp_ctx_set_option(etp_ctx* c, etp_option key, int64_t val
 extern "C" etp_status etp_ctx_get_option(const etp_ctx* c, etp_option key, int64_t* value) {
     if (!c || !value || key < 0 || key >= ETP_OPT__COUNT) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_ctx_get_option: bad ctx/key");
     *value = c->opts[key];
+    return ETP_OK;
+}
+
+extern "C" etp_status etp_ctx_kernel_time(etp_ctx* c, double* ms_out, int32_t* n_out) {
+    if (!c || !ms_out || !n_out) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_ctx_kernel_time: NULL argument");
+    double ms = 0;
+    for (int32_t i = 0; i < c->n_timed; ++i) {
+        float t = 0;
+        ETP_CUDA_OK(cudaEventSynchronize(c->tev[2 * i + 1]));
+        ETP_CUDA_OK(cudaEventElapsedTime(&t, c->tev[2 * i], c->tev[2 * i + 1]));
+        ms += t;
+    }
+    *ms_out = ms;
+    *n_out = c->n_timed;
     return ETP_OK;
 }
 
@@ -195,6 +210,8 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
 
     const int grid = c->opts[ETP_OPT_GRID_CTAS] > 0 ? (int)c->opts[ETP_OPT_GRID_CTAS] : c->n_sms;
     int counter_slot = 0, launches = 0;
+    const bool timed = c->opts[ETP_OPT_TIME_KERNELS] != 0;
+    c->n_timed = 0;
     // ---- kernel (a) on the copy stream, one launch per hazard phase
     for (size_t p = 0; p < n_ph; ++p) {
         const JobList& jl = w->phases[p];
@@ -206,8 +223,20 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
             a.n_frag = (unsigned)jl.frag.size();
             a.counters = c->d_counters + 2 * counter_slot;
             a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
+            if (timed) {
+                while ((int)c->tev.size() < 2 * (c->n_timed + 1)) {
+                    cudaEvent_t e;
+                    ETP_CUDA_OK(cudaEventCreate(&e));
+                    c->tev.push_back(e);
+                }
+                ETP_CUDA_OK(cudaEventRecord(c->tev[2 * c->n_timed], cs));
+            }
             launch_copy_kernel(a, grid, cs);
             ETP_CUDA_OK(cudaGetLastError());
+            if (timed) {
+                ETP_CUDA_OK(cudaEventRecord(c->tev[2 * c->n_timed + 1], cs));
+                ++c->n_timed;
+            }
             ++launches;
         }
         if (!jl.empty()) ++counter_slot;

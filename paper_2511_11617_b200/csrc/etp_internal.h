@@ -99,6 +99,8 @@ struct etp_ctx {
     int64_t staging_bytes = 0;
     std::vector<cudaEvent_t> events;    // hazard-phase events
     int32_t launches = 0;               // kernels launched by the last call
+    std::vector<cudaEvent_t> tev;       // timing events (pairs) around copy-stream launches, ETP_OPT_TIME_KERNELS
+    int32_t n_timed = 0;                // pairs recorded by the last call
 };
 
 namespace etp {

@@ -204,6 +204,26 @@ extern "C" etp_status etp_plan_get_stats(const etp_plan* plan, etp_plan_stats* o
     return ETP_OK;
 }
 
+extern "C" etp_status etp_plan_slab_span(const etp_plan* plan, int32_t rank, int64_t* first_unit, int64_t* span_units) {
+    if (!plan || !first_unit || !span_units) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_slab_span: NULL argument");
+    bool found = false, any = false;
+    int64_t lo = 0, hi = 0;
+    auto take = [&](const etp_shard& s) {
+        if (s.rank != rank) return;
+        found = true;
+        if (s.begin >= s.end) return;
+        lo = any ? std::min(lo, s.begin) : s.begin;
+        hi = any ? std::max(hi, s.end) : s.end;
+        any = true;
+    };
+    for (const etp_shard& s : plan->old_layout) take(s);
+    for (const etp_shard& s : plan->new_layout) take(s);
+    if (!found) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_slab_span: rank %d is in neither layout", rank);
+    *first_unit = lo;
+    *span_units = hi - lo;
+    return ETP_OK;
+}
+
 extern "C" void etp_plan_free(etp_plan* plan) { delete plan; }
 
 // ------------------------------------------------------------------------------------------------ S6 page table

@@ -103,9 +103,9 @@ class ParamWorld:
     slabs: Dict[str, Dict[int, np.ndarray]]              # tensor name -> rank -> uint8 [cap*unit_bytes]
 
 
-def build_param_world(cfg: Config, side=OracleSide, mode="span", new_policy=None, failed=None) -> ParamWorld:
-    """Small configs only: unsharded tensors ~N(0, std) in the config dtype, slabs pre-filled with seeded
-    garbage, then the old shard placed unit by unit."""
+def build_param_world(cfg: Config, side=OracleSide, mode="span", new_policy=None, failed=None, device="cpu") -> ParamWorld:
+    """Unsharded tensors ~N(0, std) in the config dtype, slabs pre-filled with seeded garbage, then the old shard
+    placed unit by unit.  ``device`` only says where the seeded generator runs (same bytes on CPU and CUDA)."""
     seed = seed_for(cfg)
     specs = tensor_inventory(cfg)
     steps = plan_scenario(cfg, side, new_policy, failed)
@@ -115,14 +115,14 @@ def build_param_world(cfg: Config, side=OracleSide, mode="span", new_policy=None
         g = slab_geometry(steps, sp.klass, mode)
         geom[sp.name] = g
         n_el = sp.total_units * sp.unit_bytes // cfg.model.elem_bytes
-        w = as_u8(fill_normal16(seed, sp.stream, 0, n_el, cfg.model.init_std, dt)).copy()
+        w = as_u8(fill_normal16(seed, sp.stream, 0, n_el, cfg.model.init_std, dt, device=device)).copy()
         unsharded[sp.name] = w
         slabs[sp.name] = {}
         for (r, s, e, _) in steps[0].old[sp.klass]:
             anchor, cap = g[r]
             nb = cap * sp.unit_bytes
             nb8 = (nb + 7) // 8 * 8
-            slab = as_u8(fill_bytes(seed, 10_000 + sp.stream * 16 + r, 0, nb8))[:nb].copy()
+            slab = as_u8(fill_bytes(seed, 10_000 + sp.stream * 16 + r, 0, nb8, device=device))[:nb].copy()
             OS.place_units(slab, anchor, cap, sp.unit_bytes, s, e, w)
             slabs[sp.name][r] = slab
     return ParamWorld(cfg, specs, steps, geom, unsharded, slabs)
@@ -161,9 +161,10 @@ class KVWorld:
 
 
 def build_kv_world(cfg: Config, side=OracleSide, head_cap: Optional[int] = None, layout: int = 0,
-                   new_policy=None, failed=None, seq_lens=None) -> KVWorld:
-    """Small configs only.  KV_ref values ~N(0,1); every rank's pool is seeded garbage with the rank's old
-    heads of every live block written in (through numpy N-d indexing, not the oracle's offset arithmetic)."""
+                   new_policy=None, failed=None, seq_lens=None, device="cpu") -> KVWorld:
+    """KV_ref values ~N(0,1); every rank's pool is seeded garbage with the rank's old heads of every live block
+    written in (through numpy N-d indexing, not the oracle's offset arithmetic).  ``device`` only says where the
+    seeded generator runs."""
     seed = seed_for(cfg) + 500
     m, kv = cfg.model, cfg.kv
     steps = plan_scenario(cfg, side, new_policy, failed)
@@ -176,7 +177,7 @@ def build_kv_world(cfg: Config, side=OracleSide, head_cap: Optional[int] = None,
     dt = torch_dtype(m.dtype)
     max_len = int(max(seq_lens)) if len(seq_lens) else 0
     n_ref = kv.n_seqs * max_len * m.n_layers * 2 * m.n_kv_heads * m.head_dim
-    kv_ref = as_u8(fill_normal16(seed, 1, 0, n_ref, 1.0, dt)).copy().reshape(
+    kv_ref = as_u8(fill_normal16(seed, 1, 0, n_ref, 1.0, dt, device=device)).copy().reshape(
         kv.n_seqs, max_len, m.n_layers, 2, m.n_kv_heads, g.frag_bytes)
     anchors = {r: s for (r, s, e, _) in steps[0].old["head"]}
     pools = {}
@@ -186,24 +187,22 @@ def build_kv_world(cfg: Config, side=OracleSide, head_cap: Optional[int] = None,
             return pool.reshape(m.n_layers, 2, n_blocks, kv.block_size, heads, g.frag_bytes)
         return pool.reshape(m.n_layers, 2, n_blocks, heads, kv.block_size, g.frag_bytes)
 
-    def put(v, l, c, b, t, slot_, frag):
+    def put(v, b, t, slot_, frags):          # frags: [layer][K|V][frag_bytes] of one (token, head)
         if layout == 0:
-            v[l, c, b, t, slot_] = frag
+            v[:, :, b, t, slot_] = frags
         else:
-            v[l, c, b, slot_, t] = frag
+            v[:, :, b, slot_, t] = frags
 
     dead0 = steps[0].dead
     for (r, s, e, _) in steps[0].old["head"]:
         nb = g.pool_bytes()
-        pool = as_u8(fill_bytes(seed, 100 + r, 0, (nb + 7) // 8 * 8))[:nb].copy()
+        pool = as_u8(fill_bytes(seed, 100 + r, 0, (nb + 7) // 8 * 8, device=device))[:nb].copy()
         v = view(pool, head_cap)
         for sq in range(kv.n_seqs):
             for t in range(int(seq_lens[sq])):
                 b = int(table[sq, t // kv.block_size])
                 for h in range(s, e):
-                    for l in range(m.n_layers):
-                        for c in range(2):
-                            put(v, l, c, b, t % kv.block_size, (h - anchors[r]) % head_cap, kv_ref[sq, t, l, c, h])
+                    put(v, b, t % kv.block_size, (h - anchors[r]) % head_cap, kv_ref[sq, t, :, :, h])
         pools[r] = pool
     # host backup = the first dead rank's pool, compacted to its own heads (reading K4)
     ds, de = [(s, e) for (r, s, e, _) in steps[0].old["head"] if r == dead0][0]
@@ -211,7 +210,7 @@ def build_kv_world(cfg: Config, side=OracleSide, head_cap: Optional[int] = None,
     host = None
     if hh > 0:
         nb = g.pool_bytes(hh)
-        host = as_u8(fill_bytes(seed, 99, 0, (nb + 7) // 8 * 8))[:nb].copy()
+        host = as_u8(fill_bytes(seed, 99, 0, (nb + 7) // 8 * 8, device=device))[:nb].copy()
         hv = view(host, hh)
         dv = view(pools[dead0], head_cap)
         for h in range(ds, de):

@@ -167,10 +167,12 @@ MICROBENCH_LO = 256
 
 
 def scaled(cfg: Config, n_layers: Optional[int] = None, n_seqs: Optional[int] = None,
-           seq_len: Optional[int] = None) -> Config:
-    """Same shape with fewer layers / sequences (bounded samples of a workload)."""
+           seq_len: Optional[int] = None, vocab: Optional[int] = None) -> Config:
+    """Same shape with fewer layers / sequences / no embedding (bounded samples of a workload)."""
     import dataclasses
     m = cfg.model if n_layers is None else dataclasses.replace(cfg.model, n_layers=n_layers)
+    if vocab is not None:
+        m = dataclasses.replace(m, vocab=vocab)
     kv = cfg.kv
     if n_seqs is not None or seq_len is not None:
         kv = dataclasses.replace(kv, n_seqs=n_seqs or kv.n_seqs, seq_len=seq_len or kv.seq_len)
