@@ -253,44 +253,49 @@ def run_ours(args):
         return tot_ms, moved, h2d, launches, rep
 
     def kernel_leg(image, K):
-        """Device time of the interval-copy kernel, params call and KV call separately (events on the copy stream)."""
-        kms, kbytes, kl = 0.0, 0, 0
+        """Device time of the interval-copy kernel (events recorded by the library on the copy stream), parameter call
+        and KV call separately.  Returns {"params"|"kv": [ms, bytes moved by the kernel, launches]}."""
+        acc = {"params": [0.0, 0, 0], "kv": [0.0, 0, 0]}
         st = state.steps[0]
+
+        def take(key, r):
+            ms, n = ctx.kernel_time()
+            torch.cuda.synchronize(dev)
+            acc[key][0] += ms
+            acc[key][1] += r["d2d_bytes"] + (r["reload_dev_bytes"] if image == "device" else 0)
+            acc[key][2] += n
+
         for _ in range(K):
             if state.specs:
-                r = state.prepared(0, image).run(ctx, [st.plans[k] for k in state.klasses], cs.cuda_stream, rs.cuda_stream)
-                ms, n = ctx.kernel_time()
-                torch.cuda.synchronize(dev)
-                kms += ms
-                kl += n
-                kbytes += r["d2d_bytes"] + (r["reload_dev_bytes"] if image == "device" else 0)
+                take("params", state.prepared(0, image).run(ctx, [st.plans[k] for k in state.klasses], cs.cuda_stream, rs.cuda_stream))
             if state.kv is not None:
                 saved, state.specs = state.specs, []
                 try:
                     rep = state.reshard(ctx, 0, image, cs.cuda_stream, rs.cuda_stream, replan=False)
                 finally:
                     state.specs = saved
-                ms, n = ctx.kernel_time()
-                torch.cuda.synchronize(dev)
-                kms += ms
-                kl += n
-                r = rep["kv"]
-                kbytes += r["d2d_bytes"] + (r["reload_dev_bytes"] if image == "device" else 0)
-        return kms, kbytes, kl
+                take("kv", rep["kv"])
+        return acc
+
+    def gbps(ms_bytes):
+        ms, nbytes = ms_bytes[0], ms_bytes[1]
+        return nbytes / (ms * 1e-3) / 1e9 if ms > 0 else None
 
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
     K, W = args.steps, max(args.warmup, 0)
     tot_ms, moved, _, launches, rep = timed("device", K, W)
-    kms, kbytes, kl = kernel_leg("device", K)
+    kacc = kernel_leg("device", K)
+    kms, kbytes, kl = (sum(kacc[k][i] for k in kacc) for i in range(3))
     e_ms, e_moved, e_h2d, e_launches, e_rep = timed("pinned", K, W)
     # kernel (a) alone on the TRANSFER bytes only (reload skipped): the north_star's "moved bytes vs HBM peak" figure
     ctx.set_option(etp.OPT_SKIP_RELOAD, 1)
     try:
         for _ in range(W):
             kernel_leg("pinned", 1)
-        d_kms, d_bytes, d_kl = kernel_leg("pinned", K)
+        dacc = kernel_leg("pinned", K)
+        d_kms, d_bytes, d_kl = (sum(dacc[k][i] for k in dacc) for i in range(3))
     finally:
         ctx.set_option(etp.OPT_SKIP_RELOAD, 0)
     clocks = sampler.stop() if rank == 0 else None
@@ -327,6 +332,8 @@ def run_ours(args):
                                   "hbm_frac": 2.0 * d_bytes / (d_kms * 1e-3) / 1e9 / hbm_peak if d_kms > 0 else None}},
         "clocks": clocks,
         "detail": {"build_s": round(t_build, 1),
+                   "kernel_moved_GBps": {"params_call": gbps(kacc["params"]), "kv_call": gbps(kacc["kv"]),
+                                         "params_ms": kacc["params"][0] / K, "kv_ms": kacc["kv"][0] / K},
                    "device_image": {"params": rp, "kv": rk}, "pinned_image": {"params": ep, "kv": ek}},
     }
     if not args.no_cpu_baseline and world == 1:

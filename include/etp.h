@@ -150,7 +150,7 @@ typedef struct {
     int64_t h2d_bytes;          /* bytes reloaded from pinned host memory                                          */
     int64_t reload_dev_bytes;   /* bytes reloaded from a device-resident image (moved by the copy kernel)          */
     int64_t kept_bytes;         /* bytes of KEEP tasks (never touched)                                             */
-    int64_t n_jobs, n_units;    /* descriptors uploaded / work-queue units                                         */
+    int64_t n_jobs, n_units;    /* segment descriptors uploaded / work items the kernels derived from them         */
     int64_t n_memcpys;          /* cudaMemcpyAsync calls issued by the reload pipeline                             */
     int32_t n_phases;           /* hazard phases (1 = hazard-free)                                                 */
     int32_t n_kernel_launches;  /* launches of this library's kernels                                              */

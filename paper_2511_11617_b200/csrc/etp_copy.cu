@@ -49,23 +49,31 @@ __device__ __forceinline__ void st_stream(void* p, const uint4& v) {
     asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// work item idx of the bulk queue -> (src, dst, bytes): piece (idx - first_item) of its segment
+__device__ __forceinline__ void load_bulk_item(const CopyArgs& a, unsigned int idx, uint64_t* src, uint64_t* dst, uint64_t* bytes) {
+    const BulkSeg* sg = a.bulk + __ldg(a.bulk_items + idx);
+    const uint4 lo = __ldg(reinterpret_cast<const uint4*>(sg));
+    const uint4 hi = __ldg(reinterpret_cast<const uint4*>(sg) + 1);
+    const uint64_t total = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
+    const uint64_t off = (uint64_t)(idx - hi.z) * (uint64_t)kBulkItem;
+    *src = ((uint64_t)lo.x | ((uint64_t)lo.y << 32)) + off;
+    *dst = ((uint64_t)lo.z | ((uint64_t)lo.w << 32)) + off;
+    *bytes = total - off < (uint64_t)kBulkItem ? total - off : (uint64_t)kBulkItem;
+}
+
 // ---------------------------------------------------------------------------------------------- bulk (TMA) driver
 // One thread.  Chunks (<= kStageBytes) of successive jobs flow through the ring; `loaded - stored <= kLookahead`.
 __device__ void tma_driver(const CopyArgs& a, uint8_t* ring, uint64_t* full_bar, uint64_t* s_dst, uint32_t* s_bytes) {
     uint32_t loaded = 0, stored = 0;
     uint64_t cur_src = 0, cur_dst = 0, cur_left = 0;
-    bool exhausted = a.n_bulk == 0;
+    bool exhausted = a.n_bulk_items == 0;
     for (;;) {
         bool progressed = false;
         if (!exhausted) {
             if (cur_left == 0) {
                 const unsigned int idx = atomicAdd(&a.counters[0], 1u);
-                if (idx < a.n_bulk) {
-                    const uint4 lo = __ldg(reinterpret_cast<const uint4*>(a.bulk + idx));
-                    const uint2 hi = __ldg(reinterpret_cast<const uint2*>(a.bulk + idx) + 2);
-                    cur_src = (uint64_t)lo.x | ((uint64_t)lo.y << 32);
-                    cur_dst = (uint64_t)lo.z | ((uint64_t)lo.w << 32);
-                    cur_left = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
+                if (idx < a.n_bulk_items) {
+                    load_bulk_item(a, idx, &cur_src, &cur_dst, &cur_left);
                 } else {
                     exhausted = true;
                 }
@@ -116,9 +124,17 @@ __device__ __forceinline__ void copy_linear(const char* __restrict__ src, char* 
     for (; v < n_vec; v += 32) st_stream(dst + (size_t)v * 16, ld_stream(src + (size_t)v * 16));
 }
 
-__device__ __forceinline__ void frag_offsets(const FragJob& j, uint32_t v, uint32_t vs, uint32_t gs, uint32_t vpr, int64_t* so, int64_t* d_o) {
+// a strided set of rows seen by one warp: row i sits at base + (i / rows_per_group) * grp + (i % rows_per_group) * row
+struct RowSet {
+    const char* src;
+    char* dst;
+    uint32_t row_bytes, n_rows, rows_per_group;
+    int64_t s_row, d_row, s_grp, d_grp;
+};
+
+__device__ __forceinline__ void row_offsets(const RowSet& j, uint32_t v, int vs, int gs, uint32_t vpr, int64_t* so, int64_t* d_o) {
     uint32_t row, col;
-    if (vs != 0xFFu) {
+    if (vs >= 0) {
         row = v >> vs;
         col = v & (vpr - 1);
     } else {
@@ -126,7 +142,7 @@ __device__ __forceinline__ void frag_offsets(const FragJob& j, uint32_t v, uint3
         col = v - row * vpr;
     }
     uint32_t grp, r;
-    if (gs != 0xFFu) {
+    if (gs >= 0) {
         grp = row >> gs;
         r = row & (j.rows_per_group - 1);
     } else {
@@ -137,15 +153,11 @@ __device__ __forceinline__ void frag_offsets(const FragJob& j, uint32_t v, uint3
     *d_o = (int64_t)grp * j.d_grp + (int64_t)r * j.d_row + (int64_t)col * 16;
 }
 
-__device__ void copy_frag_job(const FragJob& j, int lane) {
-    const char* src = reinterpret_cast<const char*>(j.src);
-    char* dst = reinterpret_cast<char*>(j.dst);
-    if (j.n_rows == 1) {
-        copy_linear(src, dst, j.row_bytes >> 4, lane);
-        return;
-    }
-    const uint32_t vs = j.vec_shift & 0xFFu, gs = (j.vec_shift >> 8) & 0xFFu;
+__device__ __forceinline__ int log2_exact(uint32_t v) { return (v & (v - 1)) ? -1 : 31 - __clz(v); }
+
+__device__ void copy_rows(const RowSet& j, int lane) {
     const uint32_t vpr = j.row_bytes >> 4;
+    const int vs = log2_exact(vpr), gs = log2_exact(j.rows_per_group);
     const uint32_t total = j.n_rows * vpr;
     uint32_t v = lane;
     for (; v + 32 * (kUnroll - 1) < total; v += 32 * kUnroll) {
@@ -154,17 +166,52 @@ __device__ void copy_frag_job(const FragJob& j, int lane) {
 #pragma unroll
         for (int u = 0; u < kUnroll; ++u) {
             int64_t so;
-            frag_offsets(j, v + 32 * u, vs, gs, vpr, &so, &d_o[u]);
-            buf[u] = ld_stream(src + so);
+            row_offsets(j, v + 32 * u, vs, gs, vpr, &so, &d_o[u]);
+            buf[u] = ld_stream(j.src + so);
         }
 #pragma unroll
-        for (int u = 0; u < kUnroll; ++u) st_stream(dst + d_o[u], buf[u]);
+        for (int u = 0; u < kUnroll; ++u) st_stream(j.dst + d_o[u], buf[u]);
     }
     for (; v < total; v += 32) {
         int64_t so, d_o;
-        frag_offsets(j, v, vs, gs, vpr, &so, &d_o);
-        st_stream(dst + d_o, ld_stream(src + so));
+        row_offsets(j, v, vs, gs, vpr, &so, &d_o);
+        st_stream(j.dst + d_o, ld_stream(j.src + so));
     }
+}
+
+__device__ __forceinline__ uint64_t u64_of(uint32_t lo, uint32_t hi) { return (uint64_t)lo | ((uint64_t)hi << 32); }
+
+// work item idx of the vector queue: look up its segment, derive the item's addresses, copy it
+__device__ void copy_vec_item(const CopyArgs& a, unsigned int idx, int lane) {
+    const uint4* p = reinterpret_cast<const uint4*>(a.vec + __ldg(a.vec_items + idx));
+    const uint4 q0 = __ldg(p), q1 = __ldg(p + 1);
+    const char* src = reinterpret_cast<const char*>(u64_of(q0.x, q0.y));
+    char* dst = reinterpret_cast<char*>(u64_of(q0.z, q0.w));
+    const uint32_t k = idx - q1.y;   // item within the segment
+    if (q1.x == VEC_LINEAR) {
+        const uint4 q4 = __ldg(p + 4);
+        const uint64_t total = u64_of(q4.x, q4.y), off = (uint64_t)k * (uint64_t)kVecItem;
+        const uint64_t n = total - off < (uint64_t)kVecItem ? total - off : (uint64_t)kVecItem;
+        copy_linear(src + off, dst + off, (uint32_t)(n >> 4), lane);
+        return;
+    }
+    const uint4 q2 = __ldg(p + 2), q3 = __ldg(p + 3), q4 = __ldg(p + 4), q5 = __ldg(p + 5);
+    const uint32_t planes_per_item = q2.x, n_planes = q2.y, items_per_pair = q2.z, pairs_first = q2.w;
+    const uint32_t pr = k / items_per_pair, grp = k - pr * items_per_pair;
+    const uint32_t pl0 = grp * planes_per_item;
+    const uint32_t np = n_planes - pl0 < planes_per_item ? n_planes - pl0 : planes_per_item;
+    const int2 ids = __ldg(a.pairs + pairs_first + pr);
+    RowSet j;
+    j.row_bytes = q1.z;
+    j.rows_per_group = q1.w;
+    j.n_rows = np * q1.w;
+    j.s_row = (int64_t)u64_of(q3.x, q3.y);
+    j.d_row = (int64_t)u64_of(q3.z, q3.w);
+    j.s_grp = (int64_t)u64_of(q4.x, q4.y);
+    j.d_grp = (int64_t)u64_of(q4.z, q4.w);
+    j.src = src + (int64_t)pl0 * j.s_grp + (int64_t)ids.x * (int64_t)u64_of(q5.x, q5.y);
+    j.dst = dst + (int64_t)pl0 * j.d_grp + (int64_t)ids.y * (int64_t)u64_of(q5.z, q5.w);
+    copy_rows(j, lane);
 }
 
 __device__ void vector_warp(const CopyArgs& a, int lane) {
@@ -172,32 +219,19 @@ __device__ void vector_warp(const CopyArgs& a, int lane) {
         unsigned int idx = 0;
         if (lane == 0) idx = atomicAdd(&a.counters[1], 1u);
         idx = __shfl_sync(0xffffffffu, idx, 0);
-        if (idx >= a.n_frag) break;
-        FragJob j;
-        const uint4* p = reinterpret_cast<const uint4*>(a.frag + idx);
-        uint4 q0 = __ldg(p), q1 = __ldg(p + 1), q2 = __ldg(p + 2), q3 = __ldg(p + 3);
-        j.src = (uint64_t)q0.x | ((uint64_t)q0.y << 32);
-        j.dst = (uint64_t)q0.z | ((uint64_t)q0.w << 32);
-        j.row_bytes = q1.x; j.n_rows = q1.y; j.rows_per_group = q1.z; j.vec_shift = q1.w;
-        j.s_row = (int64_t)((uint64_t)q2.x | ((uint64_t)q2.y << 32));
-        j.d_row = (int64_t)((uint64_t)q2.z | ((uint64_t)q2.w << 32));
-        j.s_grp = (int64_t)((uint64_t)q3.x | ((uint64_t)q3.y << 32));
-        j.d_grp = (int64_t)((uint64_t)q3.z | ((uint64_t)q3.w << 32));
-        copy_frag_job(j, lane);
+        if (idx >= a.n_vec_items) break;
+        copy_vec_item(a, idx, lane);
     }
     if (a.flags & 1u) {
-        // drain the bulk queue too (one job per warp at a time)
+        // drain the bulk queue too (one item per warp at a time)
         for (;;) {
             unsigned int idx = 0;
             if (lane == 0) idx = atomicAdd(&a.counters[0], 1u);
             idx = __shfl_sync(0xffffffffu, idx, 0);
-            if (idx >= a.n_bulk) break;
-            const uint4 lo = __ldg(reinterpret_cast<const uint4*>(a.bulk + idx));
-            const uint2 hi = __ldg(reinterpret_cast<const uint2*>(a.bulk + idx) + 2);
-            const char* src = reinterpret_cast<const char*>((uint64_t)lo.x | ((uint64_t)lo.y << 32));
-            char* dst = reinterpret_cast<char*>((uint64_t)lo.z | ((uint64_t)lo.w << 32));
-            const uint64_t bytes = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
-            copy_linear(src, dst, (uint32_t)(bytes >> 4), lane);
+            if (idx >= a.n_bulk_items) break;
+            uint64_t src, dst, bytes;
+            load_bulk_item(a, idx, &src, &dst, &bytes);
+            copy_linear(reinterpret_cast<const char*>(src), reinterpret_cast<char*>(dst), (uint32_t)(bytes >> 4), lane);
         }
     }
 }

@@ -1,12 +1,13 @@
 // Kernel (a): persistent, descriptor-driven interval copy for sm_100a.
 // PAPER.md:96 / :146 (parameter re-assignment primitive, KV operators for variable-length shards), :166 (P2P transfers
-// run beside the reloads).  One CTA per SM; two work queues with atomic heads:
-//   * BULK queue  - contiguous intervals of up to 256 KiB.  Warp 0's elected thread drives a ring of shared-memory
+// run beside the reloads).  One CTA per SM; two work queues with atomic heads; the queues hold WORK ITEMS that the kernel
+// derives from O(#intervals) segment descriptors through an item table (etp_internal.h):
+//   * BULK queue  - 256-KiB pieces of contiguous intervals.  Warp 0's elected thread drives a ring of shared-memory
 //                   stages: cp.async.bulk global->shared (mbarrier complete_tx), then cp.async.bulk shared->global
 //                   (bulk_group), kLookahead loads in flight, stores drained with wait_group.read.
-//   * FRAG queue  - two-level strided rows (head-strided KV fragments) and small intervals.  Each of the other warps
-//                   claims one job at a time and moves it with 16-byte ld.global.nc / st.global, 8 vectors in flight
-//                   per lane, consecutive lanes on consecutive 16-byte words of a row (coalesced).
+//   * VEC queue   - ~32-KiB items: pieces of small intervals, or the head-strided KV fragments of one (live block, plane
+//                   group).  Each of the other warps claims one item at a time and moves it with 16-byte ld.global.nc /
+//                   st.global, 8 vectors in flight per lane, consecutive lanes on consecutive 16-byte words of a row.
 #pragma once
 #include "etp_internal.h"
 
@@ -19,11 +20,14 @@ constexpr int kLookahead = 3;                 // bulk loads in flight ahead of t
 constexpr int kCopySmemBytes = kStages * kStageBytes + 1024;
 
 struct CopyArgs {
-    const BulkJob* bulk;
-    const FragJob* frag;
-    unsigned int n_bulk, n_frag;
-    unsigned int* counters;   // [0] bulk head, [1] frag head (zeroed before launch)
-    unsigned int flags;       // bit 0: vector warps also drain the bulk queue when the frag queue is empty
+    const BulkSeg* bulk;
+    const VecSeg* vec;
+    const uint32_t* bulk_items;   // segment index of every bulk work item
+    const uint32_t* vec_items;    // segment index of every vector work item
+    const int2* pairs;            // {old block id, new block id} lists of the VEC_PAGED segments
+    unsigned int n_bulk_items, n_vec_items;
+    unsigned int* counters;       // [0] bulk head, [1] vec head (zeroed before launch)
+    unsigned int flags;           // bit 0: vector warps also drain the bulk queue when theirs is empty
 };
 
 void launch_copy_kernel(const CopyArgs& a, int grid, cudaStream_t stream);

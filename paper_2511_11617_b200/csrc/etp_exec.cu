@@ -151,25 +151,42 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
     w->phases.resize(n_ph);
     w->host_gather.resize(n_ph);
 
-    // ---- descriptor arena layout: [phase p bulk | phase p frag | gather p frag] ...
-    int64_t total = 0, n_jobs = 0;
+    // ---- descriptor arena layout: pairs | per phase: bulk segs, bulk items, vec segs, vec items, gather segs, gather items
+    int64_t total = 0, n_jobs = 0, n_items = 0;
     auto pad = [](int64_t b) { return (b + 255) & ~int64_t(255); };
-    std::vector<int64_t> off_bulk(n_ph), off_frag(n_ph), off_gather(n_ph);
+    struct Off { int64_t bulk, bulk_items, vec, vec_items, gat, gat_items; };
+    std::vector<Off> off(n_ph);
+    const int64_t off_pairs = 0;
+    total += pad((int64_t)w->pairs.size() * sizeof(int32_t));
     int launches_needed = 0;
     for (size_t p = 0; p < n_ph; ++p) {
-        off_bulk[p] = total;   total += pad((int64_t)w->phases[p].bulk.size() * sizeof(BulkJob));
-        off_frag[p] = total;   total += pad((int64_t)w->phases[p].frag.size() * sizeof(FragJob));
-        off_gather[p] = total; total += pad((int64_t)w->host_gather[p].frag.size() * sizeof(FragJob));
-        n_jobs += (int64_t)(w->phases[p].bulk.size() + w->phases[p].frag.size() + w->host_gather[p].frag.size());
-        launches_needed += (!w->phases[p].empty()) + (!w->host_gather[p].frag.empty());
-        if (w->phases[p].bulk.size() >= 0xFFFFFFF0ull || w->phases[p].frag.size() >= 0xFFFFFFF0ull || w->host_gather[p].frag.size() >= 0xFFFFFFF0ull)
-            ETP_FAIL(ETP_ERR_CAPACITY, "too many jobs in one phase");
+        const JobList &jl = w->phases[p], &gl = w->host_gather[p];
+        off[p].bulk = total;        total += pad((int64_t)jl.bulk.size() * sizeof(BulkSeg));
+        off[p].bulk_items = total;  total += pad((int64_t)jl.n_bulk_items * sizeof(uint32_t));
+        off[p].vec = total;         total += pad((int64_t)jl.vec.size() * sizeof(VecSeg));
+        off[p].vec_items = total;   total += pad((int64_t)jl.n_vec_items * sizeof(uint32_t));
+        off[p].gat = total;         total += pad((int64_t)gl.vec.size() * sizeof(VecSeg));
+        off[p].gat_items = total;   total += pad((int64_t)gl.n_vec_items * sizeof(uint32_t));
+        n_jobs += (int64_t)(jl.bulk.size() + jl.vec.size() + gl.vec.size());
+        n_items += (int64_t)jl.n_bulk_items + jl.n_vec_items + gl.n_vec_items;
+        launches_needed += (!jl.empty()) + (!gl.vec.empty());
+        if (jl.bulk.size() >= 0xFFFFFFF0ull || jl.vec.size() >= 0xFFFFFFF0ull || gl.vec.size() >= 0xFFFFFFF0ull)
+            ETP_FAIL(ETP_ERR_CAPACITY, "too many segments in one phase");
     }
     if (launches_needed > c->n_counter_slots) ETP_FAIL(ETP_ERR_CAPACITY, "plan needs %d launches > %d", launches_needed, c->n_counter_slots);
 
+    // item table: the segment index of every work item, one fill per segment
+    auto fill_items = [](uint32_t* items, uint32_t n_items_total, const uint32_t* firsts, size_t n_segs, size_t stride) {
+        for (size_t i = 0; i < n_segs; ++i) {
+            const uint32_t b = *(const uint32_t*)((const char*)firsts + i * stride);
+            const uint32_t e = i + 1 < n_segs ? *(const uint32_t*)((const char*)firsts + (i + 1) * stride) : n_items_total;
+            std::fill(items + b, items + e, (uint32_t)i);
+        }
+    };
+
     char* d_base = nullptr;
     ArenaSlot* slot = nullptr;
-    if (total > 0) {
+    if (n_jobs > 0) {
         slot = &x->slot[x->next];
         x->next = (x->next + 1) % kArenaSlots;
         if (slot->busy) {  // the call that used this slot two calls ago must have consumed its descriptors
@@ -188,10 +205,21 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
             slot->bytes = want;
         }
         char* h = (char*)slot->h;
+        if (!w->pairs.empty()) std::memcpy(h + off_pairs, w->pairs.data(), w->pairs.size() * sizeof(int32_t));
         for (size_t p = 0; p < n_ph; ++p) {
-            if (!w->phases[p].bulk.empty()) std::memcpy(h + off_bulk[p], w->phases[p].bulk.data(), w->phases[p].bulk.size() * sizeof(BulkJob));
-            if (!w->phases[p].frag.empty()) std::memcpy(h + off_frag[p], w->phases[p].frag.data(), w->phases[p].frag.size() * sizeof(FragJob));
-            if (!w->host_gather[p].frag.empty()) std::memcpy(h + off_gather[p], w->host_gather[p].frag.data(), w->host_gather[p].frag.size() * sizeof(FragJob));
+            const JobList &jl = w->phases[p], &gl = w->host_gather[p];
+            if (!jl.bulk.empty()) {
+                std::memcpy(h + off[p].bulk, jl.bulk.data(), jl.bulk.size() * sizeof(BulkSeg));
+                fill_items((uint32_t*)(h + off[p].bulk_items), jl.n_bulk_items, &jl.bulk[0].first_item, jl.bulk.size(), sizeof(BulkSeg));
+            }
+            if (!jl.vec.empty()) {
+                std::memcpy(h + off[p].vec, jl.vec.data(), jl.vec.size() * sizeof(VecSeg));
+                fill_items((uint32_t*)(h + off[p].vec_items), jl.n_vec_items, &jl.vec[0].first_item, jl.vec.size(), sizeof(VecSeg));
+            }
+            if (!gl.vec.empty()) {
+                std::memcpy(h + off[p].gat, gl.vec.data(), gl.vec.size() * sizeof(VecSeg));
+                fill_items((uint32_t*)(h + off[p].gat_items), gl.n_vec_items, &gl.vec[0].first_item, gl.vec.size(), sizeof(VecSeg));
+            }
         }
         d_base = (char*)slot->d;
         ETP_CUDA_OK(cudaMemsetAsync(c->d_counters, 0, sizeof(unsigned int) * 2 * launches_needed, cs));
@@ -205,7 +233,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
         for (const DmaCopy& d : w->dma)
             if (d.phase > 0) need_event[d.phase - 1] = 1;
         for (size_t p = 1; p < n_ph; ++p)
-            if (!w->host_gather[p].frag.empty()) need_event[p - 1] = 1;
+            if (!w->host_gather[p].vec.empty()) need_event[p - 1] = 1;
     }
 
     const int grid = c->opts[ETP_OPT_GRID_CTAS] > 0 ? (int)c->opts[ETP_OPT_GRID_CTAS] : c->n_sms;
@@ -217,10 +245,13 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
         const JobList& jl = w->phases[p];
         if (!jl.empty() && !skip_d2d) {
             CopyArgs a;
-            a.bulk = (const BulkJob*)(d_base + off_bulk[p]);
-            a.frag = (const FragJob*)(d_base + off_frag[p]);
-            a.n_bulk = (unsigned)jl.bulk.size();
-            a.n_frag = (unsigned)jl.frag.size();
+            a.bulk = (const BulkSeg*)(d_base + off[p].bulk);
+            a.vec = (const VecSeg*)(d_base + off[p].vec);
+            a.bulk_items = (const uint32_t*)(d_base + off[p].bulk_items);
+            a.vec_items = (const uint32_t*)(d_base + off[p].vec_items);
+            a.pairs = (const int2*)(d_base + off_pairs);
+            a.n_bulk_items = jl.n_bulk_items;
+            a.n_vec_items = jl.n_vec_items;
             a.counters = c->d_counters + 2 * counter_slot;
             a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
             if (timed) {
@@ -255,7 +286,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
         bool gather_waited_upload = false;
         size_t di = 0;
         for (size_t p = 0; p < n_ph; ++p) {
-            bool has_work = !w->host_gather[p].frag.empty();
+            bool has_work = !w->host_gather[p].vec.empty();
             for (size_t k = di; k < w->dma.size() && !has_work; ++k) has_work = w->dma[k].phase == (int32_t)p;
             if (p > 0 && has_work && cs != rs) ETP_CUDA_OK(cudaStreamWaitEvent(rs, c->events[p - 1], 0));
             for (; di < w->dma.size() && w->dma[di].phase == (int32_t)p; ++di) {
@@ -267,16 +298,19 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
                 }
             }
             const JobList& gl = w->host_gather[p];
-            if (!gl.frag.empty()) {
+            if (!gl.vec.empty()) {
                 if (!gather_waited_upload && cs != rs) {
                     ETP_CUDA_OK(cudaStreamWaitEvent(rs, x->uploaded, 0));
                     gather_waited_upload = true;
                 }
                 CopyArgs a;
                 a.bulk = nullptr;
-                a.frag = (const FragJob*)(d_base + off_gather[p]);
-                a.n_bulk = 0;
-                a.n_frag = (unsigned)gl.frag.size();
+                a.bulk_items = nullptr;
+                a.vec = (const VecSeg*)(d_base + off[p].gat);
+                a.vec_items = (const uint32_t*)(d_base + off[p].gat_items);
+                a.pairs = (const int2*)(d_base + off_pairs);
+                a.n_bulk_items = 0;
+                a.n_vec_items = gl.n_vec_items;
                 a.counters = c->d_counters + 2 * counter_slot;
                 a.flags = 0;
                 const int ggrid = (int)std::max<int64_t>(1, std::min<int64_t>(c->opts[ETP_OPT_GATHER_CTAS], c->n_sms));
@@ -294,6 +328,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
     }
     c->launches = launches;
     w->rep.n_jobs = n_jobs;
+    w->rep.n_units = n_items;
     w->rep.n_memcpys = n_memcpys;
     w->rep.n_kernel_launches = launches;
     w->rep.lower_ms += now_ms() - t0;
@@ -366,7 +401,6 @@ extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_
     const double t0 = now_ms();
     LoweredWork w;
     w.phases.resize(1);
-    w.phases[0].bulk.reserve((size_t)n);
     for (int64_t i = 0; i < n; ++i) {
         const etp_interval& d = host_descs[i];
         if (d.bytes < 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has negative size", (long long)i);
@@ -376,7 +410,6 @@ extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_
             ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_copy_intervals: interval %lld is not 16-byte aligned", (long long)i);
         push_contiguous(ctx, &w.phases[0], d.src, d.dst, d.bytes);
         w.rep.d2d_bytes += d.bytes;
-        w.rep.n_units += 1;
     }
     w.rep.n_phases = 1;
     w.rep.lower_ms = now_ms() - t0;

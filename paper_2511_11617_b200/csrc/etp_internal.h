@@ -32,37 +32,49 @@ void set_error(const char* fmt, ...) __attribute__((format(printf, 1, 2)));
     } while (0)
 
 // ---- device work descriptors of the interval-copy kernel (kernel (a))
-// A BULK job is one contiguous interval of at most kBulkJobMax bytes; it is moved global -> shared -> global with
-// cp.async.bulk by the CTA's TMA thread.  32 B = one sector.
-struct BulkJob {
+// The host uploads O(#intervals) SEGMENT descriptors; the kernel expands them into fixed-size WORK ITEMS.  The k-th item
+// of a queue is looked up through an item table (uint32 segment index per item, filled on the host with one fill_n per
+// segment), so a claim costs one atomicAdd + two dependent loads and the host never touches per-block / per-chunk state.
+//
+// A BULK segment is one contiguous interval; its items are pieces of kBulkItem bytes moved global -> shared -> global
+// with cp.async.bulk by the CTA's TMA thread.  32 B = one sector.
+struct BulkSeg {
     uint64_t src, dst;
-    uint64_t bytes;   // multiple of 16
-    uint64_t pad;
+    uint64_t bytes;        // multiple of 16
+    uint32_t first_item;   // index of this segment's first item in the bulk queue
+    uint32_t pad;
 };
-// A FRAG job is a two-level strided set of rows, each `row_bytes` contiguous (a KV (token, head-run) fragment, or a
-// small contiguous interval when n_rows == 1).  Row i sits at  base + (i / rows_per_group) * grp_stride
-// + (i % rows_per_group) * row_stride.  Moved by one warp with 16-byte vector loads/stores.  64 B.
-struct FragJob {
+// A VEC segment is moved by the vector-copy warps with 16-byte loads/stores, one item per warp at a time.
+//   kind VEC_LINEAR: a contiguous interval below the TMA threshold; item k = bytes [k*kVecItem, (k+1)*kVecItem).
+//   kind VEC_PAGED : head-strided KV fragments of every live block.  Item k = (pair p = k / items_per_pair, plane group
+//                    g = k % items_per_pair): planes [g*planes_per_item, ...) of (layer, K|V); within a plane
+//                    rows_per_plane rows of row_bytes contiguous bytes.  Block ids come from pairs[pairs_first + p]
+//                    = {old id, new id}:  src = src + plane*s_plane + old*s_block + row*s_row (dst likewise).
+struct VecSeg {
     uint64_t src, dst;
+    uint32_t kind, first_item;
     uint32_t row_bytes;        // multiple of 16
-    uint32_t n_rows;
-    uint32_t rows_per_group;   // >= 1
-    uint32_t vec_shift;        // log2(row_bytes / 16) if row_bytes/16 is a power of two, else 0xFFFFFFFF
-    int64_t s_row, d_row;      // byte strides between rows of a group
-    int64_t s_grp, d_grp;      // byte strides between groups
+    uint32_t rows_per_plane;   // >= 1
+    uint32_t planes_per_item, n_planes;
+    uint32_t items_per_pair, pairs_first;
+    int64_t s_row, d_row;      // byte strides between rows of a plane
+    int64_t s_plane, d_plane;  // byte strides between planes   (VEC_LINEAR: s_plane = total bytes of the interval)
+    int64_t s_block, d_block;  // byte strides between blocks
 };
-static_assert(sizeof(BulkJob) == 32, "BulkJob layout");
-static_assert(sizeof(FragJob) == 64, "FragJob layout");
+enum { VEC_LINEAR = 0, VEC_PAGED = 1 };
+static_assert(sizeof(BulkSeg) == 32, "BulkSeg layout");
+static_assert(sizeof(VecSeg) == 96, "VecSeg layout");
 
-constexpr int64_t kBulkJobMax = 256 << 10;   // bytes per bulk job (work-queue granularity)
-constexpr int64_t kFragJobTarget = 32 << 10; // target bytes per frag job
+constexpr int64_t kBulkItem = 256 << 10;   // bytes per bulk work item (work-queue granularity)
+constexpr int64_t kVecItem = 32 << 10;     // bytes per vector work item (target for paged items)
 
-// One launch of the copy kernel = the jobs of one hazard phase.
+// One launch of the copy kernel = the segments of one hazard phase.
 struct JobList {
-    std::vector<BulkJob> bulk;
-    std::vector<FragJob> frag;
+    std::vector<BulkSeg> bulk;
+    std::vector<VecSeg> vec;
+    uint32_t n_bulk_items = 0, n_vec_items = 0;
     int64_t bytes = 0;
-    bool empty() const { return bulk.empty() && frag.empty(); }
+    bool empty() const { return bulk.empty() && vec.empty(); }
 };
 
 // A pinned-host -> device DMA of the reload pipeline (pipeline (b)).
@@ -106,9 +118,10 @@ struct etp_ctx {
 namespace etp {
 // lowering (host): etp_lower.cpp
 struct LoweredWork {
-    std::vector<JobList> phases;       // device-copy jobs per hazard phase (copy stream)
-    std::vector<JobList> host_gather;  // frag jobs whose source is pinned host memory (zero-copy gather, reload stream), per phase
+    std::vector<JobList> phases;       // device-copy segments per hazard phase (copy stream)
+    std::vector<JobList> host_gather;  // segments whose source is pinned host memory (zero-copy gather, reload stream), per phase
     std::vector<DmaCopy> dma;          // pinned host -> device DMAs (reload stream)
+    std::vector<int32_t> pairs;        // {old block id, new block id} lists referenced by VEC_PAGED segments
     etp_reshard_report rep{};
 };
 etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n_tensors, const etp_plan* const* plans,

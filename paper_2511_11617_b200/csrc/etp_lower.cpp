@@ -21,49 +21,24 @@ MemKind classify_pointer(const void* p) {
     return MEM_HOST_PAGEABLE;
 }
 
-static inline uint32_t log2_exact(uint64_t v) {  // 0xFF when v is not a power of two
-    if (v == 0 || (v & (v - 1))) return 0xFFu;
-    uint32_t s = 0;
-    while ((uint64_t(1) << s) < v) ++s;
-    return s;
-}
-
-static inline FragJob make_frag(const void* src, void* dst, uint32_t row_bytes, uint32_t n_rows, uint32_t rows_per_group,
-                                int64_t s_row, int64_t d_row, int64_t s_grp, int64_t d_grp) {
-    FragJob j;
-    j.src = (uint64_t)(uintptr_t)src;
-    j.dst = (uint64_t)(uintptr_t)dst;
-    j.row_bytes = row_bytes;
-    j.n_rows = n_rows;
-    j.rows_per_group = rows_per_group;
-    j.vec_shift = log2_exact(row_bytes >> 4) | (log2_exact(rows_per_group) << 8);
-    j.s_row = s_row;
-    j.d_row = d_row;
-    j.s_grp = s_grp;
-    j.d_grp = d_grp;
-    return j;
-}
-
-// One contiguous interval -> work-queue jobs.  Large intervals go to the cp.async.bulk queue in pieces of kBulkJobMax
-// (so that 148 SMs balance even on a single 130 MB embedding interval); small ones to the vector-copy queue.
+// One contiguous interval -> one segment.  Large intervals go to the cp.async.bulk queue, where the kernel cuts them into
+// kBulkItem pieces (so that 148 SMs balance even on a single 130 MB embedding interval); small ones to the vector queue.
 void push_contiguous(const etp_ctx* ctx, JobList* jl, const void* src, void* dst, int64_t bytes) {
+    if (bytes <= 0) return;
     const int64_t tma_min = ctx->opts[ETP_OPT_TMA_MIN_BYTES];
-    const char* s = (const char*)src;
-    char* d = (char*)dst;
     jl->bytes += bytes;
     if (bytes >= tma_min) {
-        while (bytes > 0) {
-            // avoid a tiny last piece: split the tail evenly once it is below two jobs
-            int64_t n = bytes > 2 * kBulkJobMax ? kBulkJobMax : (bytes > kBulkJobMax ? ((bytes / 2 + 15) & ~int64_t(15)) : bytes);
-            jl->bulk.push_back({(uint64_t)(uintptr_t)s, (uint64_t)(uintptr_t)d, (uint64_t)n, 0});
-            s += n; d += n; bytes -= n;
-        }
+        jl->bulk.push_back({(uint64_t)(uintptr_t)src, (uint64_t)(uintptr_t)dst, (uint64_t)bytes, jl->n_bulk_items, 0});
+        jl->n_bulk_items += (uint32_t)((bytes + kBulkItem - 1) / kBulkItem);
     } else {
-        while (bytes > 0) {
-            const int64_t n = std::min<int64_t>(bytes, kFragJobTarget);
-            jl->frag.push_back(make_frag(s, d, (uint32_t)n, 1, 1, 0, 0, 0, 0));
-            s += n; d += n; bytes -= n;
-        }
+        VecSeg v{};
+        v.src = (uint64_t)(uintptr_t)src;
+        v.dst = (uint64_t)(uintptr_t)dst;
+        v.kind = VEC_LINEAR;
+        v.first_item = jl->n_vec_items;
+        v.s_plane = bytes;
+        jl->vec.push_back(v);
+        jl->n_vec_items += (uint32_t)((bytes + kVecItem - 1) / kVecItem);
     }
 }
 
@@ -202,7 +177,6 @@ etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n
                 for (const SlotRun& r : runs) {
                     push_contiguous(ctx, &phase_list(out->phases, phase[k]), (const char*)S->base + r.src_slot * T.unit_bytes,
                                     (char*)D->base + r.dst_slot * T.unit_bytes, r.count * T.unit_bytes);
-                    out->rep.n_units += 1;
                 }
                 out->rep.d2d_bytes += bytes;
             } else {  // RELOAD
@@ -223,7 +197,6 @@ etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n
                     } else {
                         out->dma.push_back({src, dst, r.count * T.unit_bytes, phase[k]});
                     }
-                    out->rep.n_units += 1;
                 }
                 if (image_kind == MEM_DEVICE) out->rep.reload_dev_bytes += bytes;
                 else out->rep.h2d_bytes += bytes;
@@ -299,6 +272,16 @@ etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* gp, const etp_pla
     ETP_TRY(assign_phases(reads, writes, &phase));
     int32_t max_phase = 0;
 
+    // pair lists on the device: [0, n_pairs) every surviving live block, [n_pairs, n_pairs + n_reloc) the relocated ones
+    out->pairs.assign(pairs, pairs + 2 * n_pairs);
+    int64_t n_reloc = 0;
+    for (int64_t p = 0; p < n_pairs; ++p)
+        if (pairs[2 * p] != pairs[2 * p + 1]) {
+            out->pairs.push_back(pairs[2 * p]);
+            out->pairs.push_back(pairs[2 * p + 1]);
+            ++n_reloc;
+        }
+
     for (size_t k = 0; k < nt; ++k) {
         const etp_task& K = P.tasks[k];
         if (K.begin >= K.end) continue;
@@ -336,35 +319,44 @@ etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* gp, const etp_pla
         const int32_t ph = K.kind == ETP_KEEP ? 0 : phase[k];
         int64_t moved = 0;
         char* dst_base = (char*)g.pools[K.dst_rank];
+        // KEEP heads move only inside relocated blocks; every other task touches every surviving live block
+        const int64_t np_task = K.kind == ETP_KEEP ? n_reloc : n_pairs;
+        const uint32_t pairs_first = K.kind == ETP_KEEP ? (uint32_t)n_pairs : 0u;
+        if (np_task == 0) {
+            if (K.kind == ETP_KEEP) out->rep.kept_bytes += live_bytes;
+            continue;
+        }
         for (const SlotRun& r : runs) {
-            uint32_t row_bytes, rows_per_plane;
-            int64_t s_row, d_row;
+            VecSeg v{};
+            v.kind = VEC_PAGED;
             if (g.layout == ETP_KV_TOKEN_MAJOR) {  // block_size rows of (run of heads) per plane
-                row_bytes = (uint32_t)(r.count * frag);
-                rows_per_plane = (uint32_t)g.block_size;
-                s_row = ss->row;
-                d_row = dev.row;
+                v.row_bytes = (uint32_t)(r.count * frag);
+                v.rows_per_plane = (uint32_t)g.block_size;
+                v.s_row = ss->row;
+                v.d_row = dev.row;
             } else {  // one contiguous run of block_size * heads fragments per plane
-                row_bytes = (uint32_t)(r.count * g.block_size * frag);
-                rows_per_plane = 1;
-                s_row = d_row = 0;
+                v.row_bytes = (uint32_t)(r.count * g.block_size * frag);
+                v.rows_per_plane = 1;
             }
-            const int64_t plane_bytes = (int64_t)row_bytes * rows_per_plane;
-            const int64_t planes_per_job = std::max<int64_t>(1, kFragJobTarget / plane_bytes);
-            for (int64_t p = 0; p < n_pairs; ++p) {
-                const int64_t bo = pairs[2 * p], bn = pairs[2 * p + 1];
-                if (K.kind == ETP_KEEP && bo == bn) continue;
-                JobList& jl = phase_list(*dest, ph);
-                for (int64_t pl = 0; pl < n_planes; pl += planes_per_job) {
-                    const int64_t np = std::min(planes_per_job, n_planes - pl);
-                    const char* s = src_base + pl * ss->plane + bo * ss->block + r.src_slot * ss->slot;
-                    char* d = dst_base + pl * dev.plane + bn * dev.block + r.dst_slot * dev.slot;
-                    jl.frag.push_back(make_frag(s, d, row_bytes, (uint32_t)(np * rows_per_plane), rows_per_plane, s_row, d_row, ss->plane, dev.plane));
-                    jl.bytes += np * plane_bytes;
-                    moved += np * plane_bytes;
-                }
-                out->rep.n_units += 1;
-            }
+            const int64_t plane_bytes = (int64_t)v.row_bytes * v.rows_per_plane;
+            v.planes_per_item = (uint32_t)std::min<int64_t>(n_planes, std::max<int64_t>(1, kVecItem / plane_bytes));
+            v.n_planes = (uint32_t)n_planes;
+            v.items_per_pair = (uint32_t)((n_planes + v.planes_per_item - 1) / v.planes_per_item);
+            v.pairs_first = pairs_first;
+            v.src = (uint64_t)(uintptr_t)(src_base + r.src_slot * ss->slot);
+            v.dst = (uint64_t)(uintptr_t)(dst_base + r.dst_slot * dev.slot);
+            v.s_plane = ss->plane;
+            v.d_plane = dev.plane;
+            v.s_block = ss->block;
+            v.d_block = dev.block;
+            JobList& jl = phase_list(*dest, ph);
+            const int64_t items = np_task * v.items_per_pair;
+            if (items + jl.n_vec_items >= 0xFFFFFFF0ll) ETP_FAIL(ETP_ERR_CAPACITY, "etp_reshard_kv: too many work items in one phase");
+            v.first_item = jl.n_vec_items;
+            jl.n_vec_items += (uint32_t)items;
+            jl.vec.push_back(v);
+            jl.bytes += np_task * n_planes * plane_bytes;
+            moved += np_task * n_planes * plane_bytes;
         }
         *counter += moved;
         if (K.kind == ETP_KEEP) out->rep.kept_bytes += live_bytes - moved;
