@@ -55,6 +55,24 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic_per_launch():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel (a), from the committed `ncu --set full` capture
+    (profiles/r1_copy_kernel_full.csv: one parameter launch + one KV launch of this workload), or None."""
+    p = os.path.join(ROOT, "profiles", "r1_copy_kernel_full.csv")
+    try:
+        rows = {}
+        with open(p) as f:
+            for line in f:
+                c = line.rstrip("\n").split(",")
+                rows[c[0]] = c
+        rd, wr = rows["dram__bytes_read.sum"], rows["dram__bytes_write.sum"]
+        assert rd[1] == "Gbyte" and wr[1] == "Gbyte"
+        # columns 2 and 3 = the parameter launch and the KV launch of one step
+        return (float(rd[2]) + float(wr[2]) + float(rd[3]) + float(wr[3])) * 1e9 / 2.0
+    except Exception:
+        return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region (B200_PROFILING.md)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -325,7 +343,8 @@ def run_ours(args):
                 "note": "reload sources in pinned host memory; result stays on the device (the page table is host-side)"},
         "gpu_launches": launches + kl + e_launches + d_kl,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-                     "traffic": None, "kernel": "etp_interval_copy_kernel", "peak_source": peak_src,
+                     "traffic": None if reduced or cfg.key != "2" else ncu_traffic_per_launch(),
+                     "kernel": "etp_interval_copy_kernel", "peak_source": peak_src,
                      "bytes_per_launch": 2.0 * kbytes / max(kl, 1), "ms_per_launch": kms / max(kl, 1), "launches": kl,
                      "d2d_only": {"moved_bytes": d_bytes // max(K, 1), "ms": d_kms / max(K, 1),
                                   "moved_GBps": d_bytes / (d_kms * 1e-3) / 1e9 if d_kms > 0 else None,
