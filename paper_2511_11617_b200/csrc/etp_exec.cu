@@ -96,6 +96,8 @@ extern "C" void etp_ctx_destroy(etp_ctx* c) {
     for (cudaEvent_t e : c->tev) cudaEventDestroy(e);
     if (c->d_counters) cudaFree(c->d_counters);
     if (c->d_staging) cudaFree(c->d_staging);
+    if (c->lin_ws) cudaFree(c->lin_ws);
+    if (c->lin_tickets) cudaFree(c->lin_tickets);
     cudaGetLastError();
     delete c;
 }

@@ -113,6 +113,10 @@ struct etp_ctx {
     int32_t launches = 0;               // kernels launched by the last call
     std::vector<cudaEvent_t> tev;       // timing events (pairs) around copy-stream launches, ETP_OPT_TIME_KERNELS
     int32_t n_timed = 0;                // pairs recorded by the last call
+    void* lin_ws = nullptr;             // split-K workspace of etp_shard_linear (fp32 partial tiles), grown on demand
+    int64_t lin_ws_bytes = 0;
+    unsigned int* lin_tickets = nullptr; // per-tile arrival tickets of the split-K reduction (zero between launches)
+    int64_t lin_tickets_n = 0;
 };
 
 namespace etp {

@@ -1,7 +1,558 @@
+// Kernel (c): unequal-width column/row-parallel shard linear on the 5th-gen tensor cores (tcgen05 + TMEM, fed by TMA).
+// PAPER.md:45 ("unequal-width partitioning ... for attention and linear layers"), :92-94 (shard widths floor/ceil of S/g_t).
+//
+//   Y[tokens][out] = X[tokens][in] . W^T        fp32 accumulation, one round-to-nearest-even cast to 16 bit (G2)
+//
+// computed on the weight exactly as it sits in the simulated ranks' slabs after a reshard (slot-addressed, L3):
+//   ETP_COL_PARALLEL  W is cut along out-features, stored [out][in]; a rank's shard is <= 2 contiguous row runs.
+//   ETP_ROW_PARALLEL  W is cut along in-features, stored transposed [in][out]; the rank partial sums are accumulated in
+//                     ONE TMEM accumulator by walking the K loop over the ranks' runs in ascending unit order.
+//
+// Mapping onto the MMA (the roles of the operands are swapped so the wide weight dimension fills the 128 MMA rows and the
+// token count - 4 in config 1 - only costs MMA columns):
+//   D[m = out feature (128 TMEM lanes)][n = token (BN fp32 columns)] += A[m][k] . B[n][k]
+//   A = weight tile: K-major for column-parallel (rows of W), MN-major for row-parallel (rows of W^T are K, out is contiguous)
+//   B = X tile [BN tokens][64 k], always K-major.
+// Ragged shard edges never need a special path: every run has its own TMA tensor map, so rows past the end of a run are
+// zero-filled by the TMA unit (out-of-bounds fill) and the epilogue masks them.
+//
+// CTA = 6 warps: warp 0 TMA producer, warp 1 MMA issuer (+ TMEM allocation), warps 2-5 epilogue (tcgen05.ld -> 16-bit
+// stores, or fp32 split-K partials + ticketed last-arriver reduction in fixed split order, so results are deterministic).
+// Persistent grid, static round-robin over (m tile, token tile, k split) items; two TMEM accumulator stages so the epilogue
+// of item i overlaps the MMAs of item i+1.
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
 #include "etp_internal.h"
+
+using namespace etp;
+
+namespace {
+
+constexpr int kBM = 128;          // out features per tile = UMMA_M
+constexpr int kBK = 64;           // K elements per pipeline stage: 128 bytes = one 128B-swizzle atom
+constexpr int kUmmaK = 16;        // K per tcgen05.mma for 16-bit inputs
+constexpr int kMaxRuns = 16;      // <= 2 contiguous runs per rank, 8 ranks
+constexpr int kLinThreads = 192;  // 6 warps
+constexpr int kABytes = kBM * kBK * 2;
+constexpr int kSmemBudget = 200 << 10;
+
+struct Run {          // one contiguous slot range of a rank's shard, runs sorted by global feature
+    int64_t feat0;    // first global feature of the run (out-feature: column-parallel, in-feature: row-parallel)
+    int32_t n_feat;   // features in the run
+    int32_t first;    // column-parallel: index of the run's first m tile; row-parallel: of its first K chunk entry
+};
+
+struct alignas(64) LinearParams {
+    CUtensorMap map_x;
+    CUtensorMap map_w[kMaxRuns];
+    Run runs[kMaxRuns];
+    int32_t n_runs, mode, dtype;
+    int32_t tokens, in_features, out_features;
+    int32_t n_m_tiles, n_n_tiles, n_splits, n_chunks;   // n_chunks: K chunks of kBK per output tile
+    void* y;
+    float* partials;          // split-K workspace [(tile * n_splits + split)][BN][128]
+    unsigned int* tickets;    // one per output tile, zero between launches (the last arriver resets its ticket)
+    int32_t debug;
+};
+
+// ------------------------------------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t"
+        "}" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int32_t c0, int32_t c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+            smem_u32(smem_dst)),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+        : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tc_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor (tcgen05 "smem descriptor"): start address, leading / stride byte offsets (all >> 4),
+// descriptor version 1 (Blackwell) at bit 46, layout type SWIZZLE_128B (= 2) at bits 61-63.
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    return uint64_t((saddr & 0x3FFFFu) >> 4) | (uint64_t(lbo_bytes >> 4) << 16) | (uint64_t(sbo_bytes >> 4) << 32) |
+           (uint64_t(1) << 46) | (uint64_t(2) << 61);
+}
+// Instruction descriptor of kind::f16: D = fp32 (bits 4-5 = 1), A/B format (0 = fp16, 1 = bf16) at bits 7-9 / 10-12,
+// A/B major (0 = K, 1 = MN) at bits 15 / 16, N >> 3 at bits 17-22, M >> 4 at bits 24-28.
+__host__ __device__ constexpr uint32_t make_idesc(uint32_t fmt, uint32_t a_mn_major, uint32_t n) {
+    return (1u << 4) | (fmt << 7) | (fmt << 10) | (a_mn_major << 15) | ((n >> 3) << 17) | ((uint32_t(kBM) >> 4) << 24);
+}
+
+template <int BN>
+struct Cfg {
+    static constexpr int kBBytes = BN * kBK * 2;
+    static constexpr int kStageBytes = kABytes + kBBytes;
+    static constexpr int kStages = (kSmemBudget / kStageBytes) > 12 ? 12 : (kSmemBudget / kStageBytes);
+    static constexpr int kTmemCols = (2 * BN) < 32 ? 32 : 2 * BN;   // two accumulator stages; a power of two >= 32
+    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+};
+
+struct Item {
+    int m, n, split, tile, c0, c1;
+};
+__device__ __forceinline__ Item decode_item(const LinearParams& p, int item) {
+    Item it;
+    it.split = item % p.n_splits;
+    it.tile = item / p.n_splits;
+    it.n = it.tile % p.n_n_tiles;
+    it.m = it.tile / p.n_n_tiles;
+    it.c0 = int(int64_t(it.split) * p.n_chunks / p.n_splits);
+    it.c1 = int(int64_t(it.split + 1) * p.n_chunks / p.n_splits);
+    return it;
+}
+__device__ __forceinline__ int find_run(const LinearParams& p, int key) {   // last run with first <= key
+    int r = 0;
+    while (r + 1 < p.n_runs && p.runs[r + 1].first <= key) ++r;
+    return r;
+}
+template <typename T>
+__device__ __forceinline__ T cvt16(float v);
+template <>
+__device__ __forceinline__ __nv_bfloat16 cvt16<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
+template <>
+__device__ __forceinline__ __half cvt16<__half>(float v) { return __float2half_rn(v); }
+
+// ------------------------------------------------------------------------------------------------ the kernel
+template <int BN, typename OutT>
+__global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const __grid_constant__ LinearParams p) {
+    using C = Cfg<BN>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 128B swizzle atoms need 1024-B alignment
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + C::kStages * C::kStageBytes);
+    uint64_t* empty_bar = full_bar + C::kStages;
+    uint64_t* tmem_full = empty_bar + C::kStages;
+    uint64_t* tmem_empty = tmem_full + 2;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+    uint32_t* last_flag = tmem_ptr + 1;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_items = p.n_m_tiles * p.n_n_tiles * p.n_splits;
+    const bool row_par = p.mode == ETP_ROW_PARALLEL;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < C::kStages; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], 1);
+        }
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&tmem_full[s], 1);
+            mbar_init(&tmem_empty[s], 4);   // one arrival per epilogue warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {   // whole warp: allocate the TMEM columns of the two accumulator stages
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_ptr)), "r"(uint32_t(C::kTmemCols))
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+
+    if (warp == 0) {
+        // ===================================================================== TMA producer (one elected lane)
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+                const Item it = decode_item(p, item);
+                const int t0 = it.n * BN;
+                int r = row_par ? 0 : find_run(p, it.m);
+                const int row = row_par ? 0 : (it.m - p.runs[r].first) * kBM;
+                for (int c = it.c0; c < it.c1; ++c) {
+                    uint8_t* sa = smem + stage * C::kStageBytes;
+                    uint8_t* sb = sa + kABytes;
+                    mbar_wait(&empty_bar[stage], phase ^ 1);
+                    mbar_expect_tx(&full_bar[stage], C::kStageBytes);
+                    if (!row_par) {
+                        tma_load_2d(sa, &p.map_w[r], &full_bar[stage], c * kBK, row);
+                        tma_load_2d(sb, &p.map_x, &full_bar[stage], c * kBK, t0);
+                    } else {
+                        while (r + 1 < p.n_runs && p.runs[r + 1].first <= c) ++r;
+                        // K chunks are aligned to multiples of 64 GLOBAL in-features (TMA needs 16-byte aligned box starts in X);
+                        // a chunk that straddles two runs is issued once per run, the rows outside the run (negative or past
+                        // its end) being zero-filled by TMA.
+                        const int feat0 = int(p.runs[r].feat0);
+                        const int xk = (feat0 / kBK + (c - p.runs[r].first)) * kBK;
+                        const int kin = xk - feat0;
+                        tma_load_2d(sa, &p.map_w[r], &full_bar[stage], it.m * kBM, kin);              // out features m0 .. m0+63
+                        tma_load_2d(sa + kABytes / 2, &p.map_w[r], &full_bar[stage], it.m * kBM + 64, kin);   // m0+64 .. m0+127
+                        tma_load_2d(sb, &p.map_x, &full_bar[stage], xk, t0);
+                    }
+                    if (++stage == C::kStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 1) {
+        // ===================================================================== MMA issuer (one elected lane)
+        if (lane == 0) {
+            const bool a_mn = row_par && !(p.debug & 1);
+            const uint32_t idesc = make_idesc(p.dtype == ETP_BF16 ? 1u : 0u, a_mn ? 1u : 0u, uint32_t(BN));
+            // A, K-major  : rows of 128 B, 8-row groups 1024 B apart (SBO); LBO unused with 128B swizzle; +32 B per UMMA_K.
+            // A, MN-major : k rows of 128 B (64 out features), 8-k groups 1024 B apart (SBO), the second 64 out features
+            //               8192 B further (LBO); +16 k rows = 2048 B per UMMA_K.
+            const uint32_t a_lbo = a_mn ? uint32_t(kABytes / 2) : 16u;
+            const uint32_t a_kstep = a_mn ? (uint32_t(kUmmaK) * 128u) >> 4 : (uint32_t(kUmmaK) * 2u) >> 4;
+            int stage = 0;
+            uint32_t phase = 0;
+            int local = 0;
+            for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++local) {
+                const Item it = decode_item(p, item);
+                const int as = local & 1;
+                const uint32_t aph = (local >> 1) & 1;
+                mbar_wait(&tmem_empty[as], aph ^ 1);   // the epilogue has drained this accumulator stage
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + uint32_t(as * BN);
+                for (int c = it.c0; c < it.c1; ++c) {
+                    uint8_t* sa = smem + stage * C::kStageBytes;
+                    mbar_wait(&full_bar[stage], phase);
+                    tc_fence_after();
+                    const uint64_t a_desc = make_smem_desc(smem_u32(sa), a_lbo, 1024);
+                    const uint64_t b_desc = make_smem_desc(smem_u32(sa + kABytes), 16, 1024);
+#pragma unroll
+                    for (int k = 0; k < kBK / kUmmaK; ++k)
+                        if (!(p.debug & 2)) tc_mma(d_tmem, a_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > it.c0 || k > 0) ? 1u : 0u);
+                    tc_commit(&empty_bar[stage]);   // frees the smem stage once these MMAs have read it
+                    if (++stage == C::kStages) { stage = 0; phase ^= 1; }
+                }
+                tc_commit(&tmem_full[as]);          // accumulator complete -> epilogue
+            }
+        }
+        __syncwarp();
+    } else {
+        // ===================================================================== epilogue warps 2..5
+        const int q = warp & 3;                 // a warp may only touch TMEM lanes 32*(warp % 4) .. +31
+        const int m_local = q * 32 + lane;
+        OutT* y = reinterpret_cast<OutT*>(p.y);
+        int local = 0;
+        for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++local) {
+            const Item it = decode_item(p, item);
+            const int as = local & 1;
+            const uint32_t aph = (local >> 1) & 1;
+            const int t0 = it.n * BN;
+            const int n_tok = min(BN, p.tokens - t0);
+            int64_t gm0;
+            int valid;
+            if (!row_par) {
+                const int r = find_run(p, it.m);
+                const int row = (it.m - p.runs[r].first) * kBM;
+                gm0 = p.runs[r].feat0 + row;
+                valid = min(kBM, p.runs[r].n_feat - row);
+            } else {
+                gm0 = int64_t(it.m) * kBM;
+                valid = min(kBM, p.out_features - it.m * kBM);
+            }
+            mbar_wait(&tmem_full[as], aph);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + uint32_t(as * BN) + (uint32_t(q * 32) << 16);
+            float* ws = p.partials + (size_t(it.tile) * p.n_splits + it.split) * size_t(BN) * kBM;
+            for (int c16 = 0; c16 < n_tok; c16 += 16) {
+                uint32_t v[16];
+                tc_ld16(taddr + uint32_t(c16), v);
+                tc_ld_wait();
+                if (p.n_splits == 1) {
+                    if (m_local < valid) {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)
+                            if (c16 + j < n_tok) y[size_t(t0 + c16 + j) * p.out_features + gm0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j)
+                        if (c16 + j < n_tok) ws[(c16 + j) * kBM + m_local] = __uint_as_float(v[j]);
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&tmem_empty[as]);
+            if (p.n_splits > 1) {
+                // split-K: the last split to arrive at this tile sums the fp32 partials in split order 0..S-1 (deterministic)
+                __threadfence();
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (threadIdx.x == 64) *last_flag = (atomicAdd(&p.tickets[it.tile], 1u) == uint32_t(p.n_splits - 1)) ? 1u : 0u;
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (*last_flag) {
+                    __threadfence();
+                    const float* w0 = p.partials + size_t(it.tile) * p.n_splits * size_t(BN) * kBM;
+                    if (m_local < valid) {
+                        for (int j = 0; j < n_tok; ++j) {
+                            float acc = 0.f;
+                            for (int s = 0; s < p.n_splits; ++s) acc += __ldcg(w0 + (size_t(s) * BN + j) * kBM + m_local);
+                            y[size_t(t0 + j) * p.out_features + gm0 + m_local] = cvt16<OutT>(acc);
+                        }
+                    }
+                    if (threadIdx.x == 64) p.tickets[it.tile] = 0;
+                }
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+            }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        __syncwarp();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(uint32_t(C::kTmemCols)) : "memory");
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            p = nullptr;
+        }
+        return reinterpret_cast<EncodeTiledFn>(p);
+    }();
+    return fn;
+}
+
+// 2-D row-major 16-bit tensor [rows][cols] at `base`, box {box_cols (= 64 elements = 128 B), box_rows}, 128B swizzle,
+// out-of-bounds elements read as zero.
+etp_status encode_2d(CUtensorMap* map, etp_dtype dtype, const void* base, int64_t rows, int64_t cols, int64_t pitch_elems,
+                     int box_cols, int box_rows) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) ETP_FAIL(ETP_ERR_CUDA, "etp_shard_linear: cuTensorMapEncodeTiled is not available from the driver");
+    cuuint64_t dims[2] = {cuuint64_t(cols), cuuint64_t(rows)};
+    cuuint64_t strides[1] = {cuuint64_t(pitch_elems) * 2};
+    cuuint32_t box[2] = {cuuint32_t(box_cols), cuuint32_t(box_rows)};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(map, dtype == ETP_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
+                    const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS)
+        ETP_FAIL(ETP_ERR_CUDA, "etp_shard_linear: cuTensorMapEncodeTiled failed (%d) for [%lld][%lld] pitch %lld box {%d,%d}", int(r),
+                 (long long)rows, (long long)cols, (long long)pitch_elems, box_cols, box_rows);
+    return ETP_OK;
+}
+
+// Number of K splits: a function of the nominal shapes only (never of the shard layout), so a column-parallel output is
+// bit-identical before and after a reshard (G3).  Splitting only pays when few output tiles exist (small T).
+int choose_splits(int64_t nominal_tiles, int nominal_chunks, int n_sms, int bn) {
+    if (bn > 64 || nominal_chunks < 2) return 1;
+    int best = 1;
+    int64_t best_cost = INT64_MAX;
+    for (int s = 1; s <= std::min(nominal_chunks, 16); ++s) {
+        const int64_t waves = (nominal_tiles * s + n_sms - 1) / n_sms;
+        const int64_t cost = waves * ((nominal_chunks + s - 1) / s + 6) + (s > 1 ? 2 : 0);
+        if (cost < best_cost) { best_cost = cost; best = s; }
+    }
+    return best;
+}
+
+template <int BN>
+etp_status launch_linear(const LinearParams& p, int grid, cudaStream_t stream) {
+    using C = Cfg<BN>;
+    cudaError_t e;
+    if (p.dtype == ETP_BF16) {
+        auto k = etp_shard_linear_kernel<BN, __nv_bfloat16>;
+        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes));
+        k<<<grid, kLinThreads, C::kSmemBytes, stream>>>(p);
+    } else {
+        auto k = etp_shard_linear_kernel<BN, __half>;
+        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes));
+        k<<<grid, kLinThreads, C::kSmemBytes, stream>>>(p);
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) ETP_FAIL(ETP_ERR_CUDA, "etp_shard_linear: launch failed: %s", cudaGetErrorString(e));
+    return ETP_OK;
+}
+
+}  // namespace
+
 extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x, int64_t tokens,
-                                       int64_t in_features, int64_t out_features, const etp_tensor* w,
-                                       const etp_shard* layout, int32_t n_shards, int64_t features_per_unit, void* y,
-                                       void* stream) {
-    ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: not built yet");
+                                       int64_t in_features, int64_t out_features, const etp_tensor* w, const etp_shard* layout,
+                                       int32_t n_shards, int64_t features_per_unit, void* y, void* stream) {
+    if (!ctx || !w || !layout || !w->slabs) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: NULL argument");
+    if (mode != ETP_COL_PARALLEL && mode != ETP_ROW_PARALLEL) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: bad mode %d", int(mode));
+    if (dtype != ETP_BF16 && dtype != ETP_FP16) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: dtype %d is not bf16/fp16", int(dtype));
+    if (tokens < 0 || in_features <= 0 || out_features <= 0 || features_per_unit <= 0 || n_shards <= 0)
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: non-positive size");
+    if (tokens >= (int64_t(1) << 31) || in_features >= (int64_t(1) << 31) || out_features >= (int64_t(1) << 31))
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: sizes must be below 2^31");
+    const bool row_par = mode == ETP_ROW_PARALLEL;
+    const int64_t sharded = row_par ? in_features : out_features;   // the dimension the weight is cut along
+    const int64_t row_len = row_par ? out_features : in_features;   // contiguous elements per feature row of the stored weight
+    if (w->total_units * features_per_unit != sharded)
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: total_units %lld x features_per_unit %lld != sharded dimension %lld",
+                 (long long)w->total_units, (long long)features_per_unit, (long long)sharded);
+    if (w->unit_bytes != features_per_unit * row_len * 2)
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: unit_bytes %lld != features_per_unit x row length x 2 = %lld",
+                 (long long)w->unit_bytes, (long long)(features_per_unit * row_len * 2));
+    if ((in_features * 2) % 16 || (row_len * 2) % 16)
+        ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: row pitches must be multiples of 16 bytes (in %lld, stored row %lld elements)",
+                 (long long)in_features, (long long)row_len);
+    if (tokens == 0) return ETP_OK;
+    if (!x || !y) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: x / y is NULL");
+    if ((reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(y)) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: x / y not 16-byte aligned");
+
+    // ---- the shards in ascending unit order must tile [0, total_units)
+    std::vector<etp_shard> sh;
+    for (int i = 0; i < n_shards; ++i)
+        if (layout[i].alive && layout[i].end > layout[i].begin) sh.push_back(layout[i]);
+    std::sort(sh.begin(), sh.end(), [](const etp_shard& a, const etp_shard& b) { return a.begin < b.begin; });
+    int64_t cursor = 0;
+    for (const etp_shard& s : sh) {
+        if (s.begin != cursor) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: layout does not tile [0,%lld): gap or overlap at unit %lld", (long long)w->total_units, (long long)cursor);
+        cursor = s.end;
+    }
+    if (cursor != w->total_units) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: layout covers %lld of %lld units", (long long)cursor, (long long)w->total_units);
+
+    // ---- contiguous runs of every shard inside its slot-addressed slab (L3)
+    LinearParams p;
+    std::memset(&p, 0, sizeof(p));
+    const void* run_addr[kMaxRuns];
+    int n_runs = 0;
+    for (const etp_shard& s : sh) {
+        if (s.rank < 0 || s.rank >= w->n_ranks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d outside the tensor's %d slabs", s.rank, w->n_ranks);
+        const etp_slab& sl = w->slabs[s.rank];
+        if (!sl.base) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d has no slab", s.rank);
+        if (reinterpret_cast<uintptr_t>(sl.base) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: slab of rank %d not 16-byte aligned", s.rank);
+        const int64_t width = s.end - s.begin;
+        if (sl.cap_units <= 0 || width > sl.cap_units) ETP_FAIL(ETP_ERR_CAPACITY, "etp_shard_linear: shard of rank %d (%lld units) exceeds its slab (%lld)", s.rank, (long long)width, (long long)sl.cap_units);
+        int64_t slot0 = (s.begin - sl.anchor_unit) % sl.cap_units;
+        if (slot0 < 0) slot0 += sl.cap_units;
+        const int64_t len1 = std::min(width, sl.cap_units - slot0);
+        const int64_t piece_b[2] = {s.begin, s.begin + len1};
+        const int64_t piece_n[2] = {len1, width - len1};
+        const int64_t piece_slot[2] = {slot0, 0};
+        for (int k = 0; k < 2; ++k) {
+            if (piece_n[k] == 0) continue;
+            if (n_runs == kMaxRuns) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: more than %d contiguous runs", kMaxRuns);
+            if (piece_n[k] * features_per_unit >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: run too long");
+            p.runs[n_runs].feat0 = piece_b[k] * features_per_unit;
+            p.runs[n_runs].n_feat = int32_t(piece_n[k] * features_per_unit);
+            run_addr[n_runs] = static_cast<const char*>(sl.base) + piece_slot[k] * w->unit_bytes;
+            ++n_runs;
+        }
+    }
+
+    // ---- tiling
+    const int bn = tokens <= 16 ? 16 : (tokens <= 64 ? 64 : 256);
+    p.n_runs = n_runs;
+    p.mode = mode;
+    p.dtype = dtype;
+    p.tokens = int32_t(tokens);
+    p.in_features = int32_t(in_features);
+    p.out_features = int32_t(out_features);
+    p.n_n_tiles = int32_t((tokens + bn - 1) / bn);
+    p.y = y;
+    int32_t acc = 0;
+    for (int r = 0; r < n_runs; ++r) {
+        p.runs[r].first = acc;
+        if (row_par) acc += int32_t((p.runs[r].feat0 + p.runs[r].n_feat + kBK - 1) / kBK - p.runs[r].feat0 / kBK);   // 64-aligned global K chunks it touches
+        else acc += (p.runs[r].n_feat + kBM - 1) / kBM;
+    }
+    if (row_par) {
+        p.n_chunks = acc;
+        p.n_m_tiles = int32_t((out_features + kBM - 1) / kBM);
+    } else {
+        p.n_m_tiles = acc;
+        p.n_chunks = int32_t((in_features + kBK - 1) / kBK);
+    }
+    const int64_t nominal_tiles = ((out_features + kBM - 1) / kBM) * p.n_n_tiles;
+    p.n_splits = std::min(choose_splits(nominal_tiles, int((in_features + kBK - 1) / kBK), ctx->n_sms, bn), p.n_chunks);
+    const int64_t n_tiles = int64_t(p.n_m_tiles) * p.n_n_tiles;
+    const int64_t n_items = n_tiles * p.n_splits;
+    if (n_items >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: too many work items");
+
+    ETP_CUDA_OK(cudaSetDevice(ctx->device));
+    if (p.n_splits > 1) {   // split-K workspace, owned by the ctx and grown on demand (calls on one ctx must not overlap in time)
+        const int64_t need = n_tiles * p.n_splits * bn * kBM * int64_t(sizeof(float));
+        if (need > ctx->lin_ws_bytes) {
+            if (ctx->lin_ws) ETP_CUDA_OK(cudaFree(ctx->lin_ws));
+            ctx->lin_ws = nullptr;
+            ctx->lin_ws_bytes = 0;
+            ETP_CUDA_OK(cudaMalloc(&ctx->lin_ws, size_t(need)));
+            ctx->lin_ws_bytes = need;
+        }
+        if (n_tiles > ctx->lin_tickets_n) {
+            if (ctx->lin_tickets) ETP_CUDA_OK(cudaFree(ctx->lin_tickets));
+            ctx->lin_tickets = nullptr;
+            ctx->lin_tickets_n = 0;
+            const int64_t n = std::max<int64_t>(n_tiles, 4096);
+            ETP_CUDA_OK(cudaMalloc(&ctx->lin_tickets, size_t(n) * sizeof(unsigned int)));
+            ETP_CUDA_OK(cudaMemset(ctx->lin_tickets, 0, size_t(n) * sizeof(unsigned int)));
+            ETP_CUDA_OK(cudaDeviceSynchronize());
+            ctx->lin_tickets_n = n;
+        }
+        p.partials = static_cast<float*>(ctx->lin_ws);
+        p.tickets = ctx->lin_tickets;
+    }
+
+    // ---- tensor maps: X [tokens][in]; one map per run so that TMA zero-fills everything past a run's end
+    ETP_TRY(encode_2d(&p.map_x, dtype, x, tokens, in_features, in_features, kBK, bn));
+    for (int r = 0; r < n_runs; ++r) {
+        if (row_par) ETP_TRY(encode_2d(&p.map_w[r], dtype, run_addr[r], p.runs[r].n_feat, out_features, out_features, 64, kBK));
+        else ETP_TRY(encode_2d(&p.map_w[r], dtype, run_addr[r], p.runs[r].n_feat, in_features, in_features, kBK, kBM));
+    }
+
+    if (const char* dbg = getenv("ETP_LINEAR_DEBUG")) p.debug = atoi(dbg);
+    const int grid = int(std::min<int64_t>(n_items, ctx->n_sms));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    ctx->launches = 1;
+    if (bn == 16) return launch_linear<16>(p, grid, st);
+    if (bn == 64) return launch_linear<64>(p, grid, st);
+    return launch_linear<256>(p, grid, st);
 }

@@ -1,0 +1,211 @@
+"""Parity of kernel (c) etp_shard_linear (tcgen05/TMEM/TMA) against the oracle's UNSHARDED fp64 linear reference.
+
+north_star: "the shard-linear outputs must match an unsharded fp32 reference within max relative error 5e-3"; reading G1
+(DESIGN.md): max|y - ref| / max|ref| over the whole output.  The weight is handed to the kernel exactly as a reshard leaves
+it: slot-addressed slabs (wrapped shards included), unequal widths, slack slots full of NaN bit patterns so that a read
+outside a shard poisons the output."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2511_11617_b200 as etp
+from oracle import linear as OL
+from oracle import state as OS
+from tests import harness as H
+from tests.gpu_util import DevBuf, LibSide, Streams, make_plans
+from workloads import get_config
+from workloads.gen import as_u8, fill_normal16, torch_dtype
+
+pytestmark = pytest.mark.gpu
+
+TOL = 5e-3          # north_star
+SEED = 25111617
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = etp.Context(0)
+    yield c
+    c.close()
+
+
+def widths_to_layout(widths, ranks=None):
+    ranks = list(range(len(widths))) if ranks is None else ranks
+    out, b = [], 0
+    for r, w in zip(ranks, widths):
+        out.append((r, b, b + w, 1))
+        b += w
+    return out
+
+
+def shard_into_slabs(w_u8, unit_bytes, layout, geom):
+    """slabs[r]: cap*unit_bytes bytes of 0xFF (16-bit NaN patterns) with the rank's units placed by the slot rule."""
+    slabs = {}
+    for (r, b, e, alive) in layout:
+        anchor, cap = geom[r]
+        slab = np.full(cap * unit_bytes, 0xFF, dtype=np.uint8)
+        OS.place_units(slab, anchor, cap, unit_bytes, b, e, w_u8)
+        slabs[r] = slab
+    return slabs
+
+
+def run_linear(ctx, mode, dtype, x_u8, T, K, N, w_desc, layout, fpu, stream=0):
+    xb = DevBuf(x_u8)
+    yb = DevBuf(np.full(T * N * 2, 0xEE, dtype=np.uint8))
+    etp.etp_shard_linear(ctx, mode, dtype, xb.ptr, T, K, N, w_desc, layout, fpu, yb.ptr, stream)
+    torch.cuda.synchronize()
+    assert xb.guards_intact() and yb.guards_intact()
+    return yb.payload()
+
+
+def reference(dtype, x_u8, w_u8, T, K, N, transposed):
+    x = OL.decode16(x_u8, dtype).reshape(T, K)
+    w = OL.decode16(w_u8, dtype)
+    w = w.reshape(K, N).T if transposed else w.reshape(N, K)
+    return OL.linear_ref(x, w)
+
+
+def check(y_u8, ref, dtype, T, N):
+    y = OL.decode16(y_u8, dtype).reshape(T, N)
+    assert np.isfinite(y).all(), "non-finite output: the kernel read outside a shard or left outputs unwritten"
+    err = OL.max_rel_err(y, ref)
+    assert err <= TOL, f"max relative error {err:.3e} > {TOL}"
+    # sharper, derived from the arithmetic: fp32 accumulation + ONE rounding to 16 bit.  bf16 keeps 8 significant bits
+    # (spacing 2^-7 relative, so round-to-nearest errs by at most 2^-8), fp16 keeps 11 (at most 2^-11).
+    half_ulp = 2.0 ** -8 if dtype == "bf16" else 2.0 ** -11
+    assert err <= half_ulp + 1e-4, f"max relative error {err:.3e} exceeds one 16-bit rounding"
+    return err
+
+
+CASES = [
+    # mode, dtype, T, in, out, fpu, widths (units), geometry mode
+    ("col", "bf16", 4, 256, 512, 1, (171, 171, 170), "tight"),
+    ("col", "fp16", 4, 256, 256, 32, (3, 3, 2), "wrap"),
+    ("col", "bf16", 4, 200, 1000, 1, (333, 334, 333), "wrap"),             # K tail (200 = 3 chunks + 8), ragged m tiles
+    ("row", "bf16", 4, 688, 256, 1, (229, 229, 230), "tight"),             # config-1 down_t: K runs with tails
+    ("row", "fp16", 4, 256, 256, 64, (1, 1, 2), "wrap"),                   # config-1 wo_t
+    ("row", "bf16", 4, 1000, 200, 1, (100, 500, 400), "wrap"),             # out not a multiple of 64 / 128
+    ("col", "bf16", 33, 512, 640, 1, (200, 240, 200), "wrap"),             # BN = 64
+    ("row", "bf16", 50, 520, 384, 1, (260, 260), "tight"),
+    ("col", "bf16", 100, 1000, 777, 1, (111, 222, 333, 111), "wrap"),      # BN = 256, ragged token tile
+    ("row", "fp16", 300, 1000, 776, 1, (111, 222, 333, 334), "wrap"),      # two token tiles
+    ("col", "bf16", 4, 5120, 5120, 640, (3, 3, 2), "tight"),               # Qwen3-14B wq, 4 tokens: split-K path
+    ("row", "bf16", 4, 5120, 5120, 640, (3, 3, 2), "tight"),               # Qwen3-14B wo_t
+    ("col", "bf16", 512, 2048, 2304, 1, (768, 769, 767), "wrap"),          # several items per CTA (accumulator stages)
+    ("row", "bf16", 512, 2307 + 5, 2048, 1, (770, 771, 771), "wrap"),
+]
+
+
+@pytest.mark.parametrize("mode,dtype,T,K,N,fpu,widths,gmode", CASES)
+def test_shard_linear_matches_unsharded_reference(ctx, mode, dtype, T, K, N, fpu, widths, gmode):
+    transposed = mode == "row"
+    sharded = K if transposed else N
+    units = sharded // fpu
+    assert units * fpu == sharded and sum(widths) == units
+    row_len = N if transposed else K
+    unit_bytes = fpu * row_len * 2
+    dt = torch_dtype(dtype)
+    std = 0.02
+    w_u8 = as_u8(fill_normal16(SEED, 700 + T, 0, K * N, std, dt)).copy()
+    x_u8 = as_u8(fill_normal16(SEED, 701 + T, 0, T * K, 1.0, dt)).copy()
+    layout = widths_to_layout(widths)
+    geom = {}
+    for (r, b, e, _) in layout:
+        if gmode == "tight":
+            geom[r] = (b, e - b)                         # anchor = first unit, cap = width: no wrap
+        else:
+            cap = (e - b) + 1 + r
+            geom[r] = (b - (cap - (e - b) // 2) % cap, cap)   # the shard starts mid-slab and wraps
+    slabs = shard_into_slabs(w_u8, unit_bytes, layout, geom)
+    bufs = {r: DevBuf(a) for r, a in slabs.items()}
+    desc = etp.TensorDesc(units, unit_bytes, {r: (bufs[r].ptr, geom[r][1], geom[r][0]) for r in bufs}, len(widths), 0)
+    y_u8 = run_linear(ctx, etp.ROW_PARALLEL if transposed else etp.COL_PARALLEL, dtype, x_u8, T, K, N, desc, layout, fpu)
+    ref = reference(dtype, x_u8, w_u8, T, K, N, transposed)
+    check(y_u8, ref, dtype, T, N)
+    assert all(b.guards_intact() for b in bufs.values())
+    for r, b in bufs.items():
+        assert np.array_equal(b.payload(), slabs[r]), "the weight slabs are read-only for the linear"
+
+
+def test_column_parallel_is_bitwise_independent_of_the_split(ctx):
+    """Reading G3: the K order of a column-parallel output does not depend on how out-features are cut."""
+    T, K, N = 4, 1024, 1536
+    dt = torch_dtype("bf16")
+    w_u8 = as_u8(fill_normal16(SEED, 720, 0, K * N, 0.02, dt)).copy()
+    x_u8 = as_u8(fill_normal16(SEED, 721, 0, T * K, 1.0, dt)).copy()
+    outs = []
+    for widths in ((384, 384, 384, 384), (512, 512, 512), (1536,), (100, 1000, 436)):
+        layout = widths_to_layout(widths)
+        geom = {r: (b, e - b) for (r, b, e, _) in layout}
+        slabs = shard_into_slabs(w_u8, K * 2, layout, geom)
+        bufs = {r: DevBuf(a) for r, a in slabs.items()}
+        desc = etp.TensorDesc(N, K * 2, {r: (bufs[r].ptr, geom[r][1], geom[r][0]) for r in bufs}, len(widths), 0)
+        outs.append(run_linear(ctx, etp.COL_PARALLEL, "bf16", x_u8, T, K, N, desc, layout, 1))
+    for o in outs[1:]:
+        assert np.array_equal(o, outs[0])
+
+
+def linear_checks_for_world(ctx, world, bufs, layouts_by_class, tokens, dead=None):
+    """Every sharded linear of the world on `layouts_by_class` against the unsharded reference.  Returns {name: y bytes}."""
+    cfg = world.cfg
+    dtype = cfg.model.dtype
+    dt = torch_dtype(dtype)
+    outs = {}
+    n_ranks = max(r for (r, _, _, _) in world.steps[0].old[world.specs[0].klass]) + 1
+    for sp in world.specs:
+        if sp.name in ("embed",):
+            continue                                   # a lookup table, not a linear
+        sharded = sp.total_units * sp.features_per_unit
+        K, N = (sharded, sp.row_elems) if sp.transposed else (sp.row_elems, sharded)
+        x_u8 = as_u8(fill_normal16(H.seed_for(cfg), 5000 + sp.stream, 0, tokens * K, 1.0, dt)).copy()
+        # before the failure every rank still holds its shard (the plan input marks the failing rank alive = 0)
+        layout = [(r, b, e, 1) for (r, b, e, a) in layouts_by_class[sp.klass] if (a or dead is None) and r != dead]
+        slabs = {r: (bufs[sp.name][r].ptr, world.geom[sp.name][r][1], world.geom[sp.name][r][0]) for (r, _, _, _) in layout}
+        desc = etp.TensorDesc(sp.total_units, sp.unit_bytes, slabs, n_ranks, 0)
+        y = run_linear(ctx, etp.ROW_PARALLEL if sp.transposed else etp.COL_PARALLEL, dtype, x_u8, tokens, K, N, desc, layout,
+                       sp.features_per_unit)
+        ref = reference(dtype, x_u8, world.unsharded[sp.name], tokens, K, N, sp.transposed)
+        check(y, ref, dtype, tokens, N)
+        outs[sp.name] = y
+    return outs
+
+
+@pytest.mark.parametrize("mode", ["tight", "span"])
+def test_config1_layer_outputs_survive_the_reshard(ctx, mode):
+    """Config 1 (BASELINE.json configs[0]): 4 unequal ranks, rank 2 fails, reshard to 3, "shard-linear check on a batch of
+    4 tokens": every linear computes the unsharded layer output before AND after the reshard; column-parallel bitwise equal."""
+    from tests import test_gpu_reshard as TR
+    cfg = get_config("1")
+    world = H.build_param_world(cfg, side=LibSide, mode=mode)
+    bufs, images = TR.upload_param_world(world)
+    step = world.steps[0]
+    before = linear_checks_for_world(ctx, world, bufs, step.old, cfg.tokens)
+    TR.run_param_step(ctx, world, bufs, images, 0, Streams())
+    after = linear_checks_for_world(ctx, world, bufs, step.new, cfg.tokens, dead=step.dead)
+    for sp in world.specs:
+        if sp.name in before and not sp.transposed:
+            assert np.array_equal(before[sp.name], after[sp.name]), sp.name
+
+
+def test_shard_linear_argument_errors(ctx):
+    T, K, N = 4, 64, 128
+    w = DevBuf(np.zeros(N * K * 2, dtype=np.uint8))
+    x = DevBuf(np.zeros(T * K * 2, dtype=np.uint8))
+    y = DevBuf(np.zeros(T * N * 2, dtype=np.uint8))
+    desc = etp.TensorDesc(N, K * 2, {0: (w.ptr, N, 0)}, 1, 0)
+    ok = [(0, 0, N, 1)]
+    etp.etp_shard_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, T, K, N, desc, ok, 1, y.ptr)
+    torch.cuda.synchronize()
+    with pytest.raises(etp.EtpError) as e:   # layout with a gap
+        etp.etp_shard_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, T, K, N, desc, [(0, 0, N - 1, 1)], 1, y.ptr)
+    assert e.value.status == 1
+    with pytest.raises(etp.EtpError) as e:   # unit_bytes inconsistent with the shapes
+        etp.etp_shard_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, T, K + 8, N, desc, ok, 1, y.ptr)
+    assert e.value.status == 1
+    with pytest.raises(etp.EtpError) as e:   # misaligned x
+        etp.etp_shard_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr + 2, T, K, N, desc, ok, 1, y.ptr)
+    assert e.value.status == 2
+    with pytest.raises(etp.EtpError) as e:   # shard wider than its slab
+        d2 = etp.TensorDesc(N, K * 2, {0: (w.ptr, N - 1, 0)}, 1, 0)
+        etp.etp_shard_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, T, K, N, d2, ok, 1, y.ptr)
+    assert e.value.status == 3
