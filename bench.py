@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--layers", type=int, default=0, help="debug: fewer layers (marks the result as reduced)")
     ap.add_argument("--seqs", type=int, default=0, help="debug: fewer sequences (marks the result as reduced)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-linear", action="store_true", help="skip the S7 (shard linear) leg")
+    ap.add_argument("--linear-only", action="store_true", help="only the S7 leg, on parameters alone (for ncu captures of kernel (c))")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0, help="CPU seconds of oracle work in the cpu_baseline leg")
     ap.add_argument("--ref-layers", type=int, default=2, help="--impl reference: layers in the per-step sample")
     return ap.parse_args()
@@ -198,6 +200,61 @@ def run_reference(args):
     return 0
 
 
+# ================================================================================================ S7 leg
+def shard_linear_leg(state, ctx, dev, hbm_peak, tokens_list=(4, 4096)):
+    """Kernel (c) on the RESHARDED state of the config (new unequal-width layout, slot-addressed slabs): every sharded
+    linear of a layer, cycling over the layers so every call streams weights that are not in L2 (a layer's tensor is
+    re-read only after the 39 others), with a 256-MiB READ (a sum: leaves L2 full of clean lines, so no write-back
+    competes with the timed kernel) before each call, which also lets the host run ahead so that the events bracket the
+    kernel only.  T = 4 is weight
+    streaming (HBM bound: GB/s of algorithmic bytes 2KN + 2T(K+N)); T = 4096 is tensor bound (TFLOP/s of 2TKN)."""
+    import torch
+    from workloads.gen import fill_normal16
+    m = state.cfg.model
+    kinds = sorted({sp.name.split(".", 1)[1] for sp in state.specs if sp.layer >= 0})
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    tf_burst = tf_sust = None
+    if os.path.exists(peaks_path):
+        with open(peaks_path) as f:
+            d = json.load(f)
+        tf_burst, tf_sust = d.get("bf16_tflops"), d.get("bf16_tflops_sustained")
+    st = torch.cuda.Stream(dev)
+    flush = torch.zeros(64 << 20, dtype=torch.int32, device=dev)
+    out = {"layout": {k: [e - b for (_, b, e, _) in v] for k, v in state.steps[0].new.items()}, "launches": 0}
+    for T in tokens_list:
+        per, tot_ms, tot_flop, tot_bytes = {}, 0.0, 0.0, 0.0
+        for kind in kinds:
+            calls = [state.linear(f"l{l}.{kind}", 0, after=True) for l in range(m.n_layers)]
+            K, N = calls[0].K, calls[0].N
+            x = fill_normal16(state.seed, 9000 + T, 0, T * K, 1.0, state.dt, device=dev)
+            y = torch.empty(T * N, dtype=state.dt, device=dev)
+            evs = []
+            with torch.cuda.stream(st):
+                for i, c in enumerate(calls[-3:] + calls):         # 3 warm-up calls (on the layers timed last)
+                    flush.sum()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(st)
+                    c.run(ctx, x.data_ptr(), T, y.data_ptr(), st.cuda_stream)
+                    e1.record(st)
+                    evs.append((e0, e1))
+            st.synchronize()
+            ms = sorted(a.elapsed_time(b) for a, b in evs[3:])
+            med = ms[len(ms) // 2]
+            flop, byts = 2.0 * T * K * N, 2.0 * K * N + 2.0 * T * (K + N)
+            per[kind] = {"K": K, "N": N, "us": round(med * 1e3, 2), "TFLOPs": round(flop / med / 1e9, 1), "GBps": round(byts / med / 1e6, 1)}
+            tot_ms, tot_flop, tot_bytes = tot_ms + med, tot_flop + flop, tot_bytes + byts
+            out["launches"] += len(evs)
+        agg = {"layer_us": round(tot_ms * 1e3, 1), "TFLOPs": tot_flop / tot_ms / 1e9, "GBps": tot_bytes / tot_ms / 1e6, "per_linear": per}
+        if T <= 64:
+            agg["roofline"] = {"bound": "hbm", "achieved": agg["GBps"], "peak": hbm_peak, "unit": "GB/s", "frac": agg["GBps"] / hbm_peak}
+        elif tf_burst:
+            agg["roofline"] = {"bound": "tensor", "achieved": agg["TFLOPs"], "peak": tf_burst, "unit": "TFLOP/s",
+                               "frac": agg["TFLOPs"] / tf_burst, "peak_kind": "bf16 burst (kernel timed alone)",
+                               "frac_of_sustained": agg["TFLOPs"] / tf_sust if tf_sust else None}
+        out[f"T{T}"] = agg
+    return out
+
+
 # ================================================================================================ the CUDA path
 def run_ours(args):
     import torch
@@ -225,11 +282,19 @@ def run_ours(args):
     hbm_peak, peak_src = load_peaks()
 
     t_build = time.perf_counter()
-    state = ModelState(cfg, device=dev, image="both")
+    state = ModelState(cfg, device=dev, image="device" if args.linear_only else "both", with_kv=not args.linear_only)
     t_build = time.perf_counter() - t_build
     ctx = etp.Context(local_rank)
     ctx.set_option(etp.OPT_TIME_KERNELS, 1)
     cs, rs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+
+    if args.linear_only:
+        state.reshard(ctx, 0, "device", cs.cuda_stream, rs.cuda_stream, replan=True)   # the linears run on the NEW layout
+        torch.cuda.synchronize(dev)
+        lin = shard_linear_leg(state, ctx, dev, hbm_peak)
+        if rank == 0:
+            print(json.dumps({"shard_linear": lin, "config": {"workload": f"config {cfg.key}", "reduced": reduced}}))
+        return 0
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -316,6 +381,9 @@ def run_ours(args):
         d_kms, d_bytes, d_kl = (sum(dacc[k][i] for k in dacc) for i in range(3))
     finally:
         ctx.set_option(etp.OPT_SKIP_RELOAD, 0)
+    lin = None
+    if state.specs and cfg.model.ffn and not args.no_linear:
+        lin = shard_linear_leg(state, ctx, dev, hbm_peak)
     clocks = sampler.stop() if rank == 0 else None
 
     if rank != 0:
@@ -341,7 +409,8 @@ def run_ours(args):
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": e_h2d // K, "d2h_bytes_per_step": 0,
                 "ms_per_step": e_ms / K, "h2d_GBps": e_h2d / (e_ms * 1e-3) / 1e9,
                 "note": "reload sources in pinned host memory; result stays on the device (the page table is host-side)"},
-        "gpu_launches": launches + kl + e_launches + d_kl,
+        "gpu_launches": launches + kl + e_launches + d_kl + (lin["launches"] if lin else 0),
+        "shard_linear": lin,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
                      "traffic": None if reduced or cfg.key != "2" else ncu_traffic_per_launch(),
                      "kernel": "etp_interval_copy_kernel", "peak_source": peak_src,

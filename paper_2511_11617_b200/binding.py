@@ -330,6 +330,21 @@ def etp_shard_linear(ctx: Context, mode: int, dtype: str, x_ptr: int, tokens: in
     del keep
 
 
+class PreparedLinear:
+    """Pre-marshalled arguments of one etp_shard_linear call (weight descriptor + layout), so that a timed loop pays only
+    the C call."""
+
+    def __init__(self, mode: int, dtype: str, in_features: int, out_features: int, w: TensorDesc, layout: Sequence[Shard],
+                 features_per_unit: int):
+        self.mode, self.dtype, self.K, self.N, self.fpu = mode, DTYPE[dtype], in_features, out_features, features_per_unit
+        self.arr, self._keep = _marshal_tensors([w])
+        self.layout, self.n = _shards(layout), len(layout)
+
+    def run(self, ctx: Context, x_ptr: int, tokens: int, y_ptr: int, stream: int = 0) -> None:
+        _check(lib().etp_shard_linear(ctx.handle, self.mode, self.dtype, x_ptr, tokens, self.K, self.N, self.arr, self.layout,
+                                      self.n, self.fpu, y_ptr, stream or None))
+
+
 def etp_copy_intervals(ctx: Context, src_ptrs, dst_ptrs, sizes, stream: int = 0) -> Dict[str, float]:
     """src_ptrs / dst_ptrs / sizes: numpy int64 arrays of absolute device addresses and byte counts."""
     import numpy as np

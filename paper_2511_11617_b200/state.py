@@ -280,6 +280,26 @@ class ModelState:
                 copy_stream=copy_stream, reload_stream=reload_stream)
         return {"params": rep_p, "kv": rep_k, "evicted": evicted, "table": new_table, "plans": plans}
 
+    # ------------------------------------------------------------------ S7: the layer outputs on the sharded state
+    def linear(self, name: str, step_idx: int, after: bool = True) -> "B.PreparedLinear":
+        """etp_shard_linear arguments for tensor ``name`` as it sits in the slabs before (``after=False``: every old rank
+        still holds its shard) or after the reshard of step ``step_idx``."""
+        key = (name, step_idx, after)
+        if key not in self._prepared:
+            sp = next(s for s in self.specs if s.name == name)
+            st = self.steps[step_idx]
+            layout = list(st.new[sp.klass]) if after else [(r, s, e, 1) for (r, s, e, _) in st.old[sp.klass]]
+            slabs = {}
+            for (r, _, _, _) in layout:
+                anchor, cap = self.geom[sp.klass][r]
+                slabs[r] = (self.slabs[name][r].data_ptr(), cap, anchor)
+            sharded = sp.total_units * sp.features_per_unit
+            K, N = (sharded, sp.row_elems) if sp.transposed else (sp.row_elems, sharded)
+            desc = B.TensorDesc(sp.total_units, sp.unit_bytes, slabs, self.n_ranks, 0)
+            self._prepared[key] = B.PreparedLinear(B.ROW_PARALLEL if sp.transposed else B.COL_PARALLEL, self.cfg.model.dtype,
+                                                   K, N, desc, layout, sp.features_per_unit)
+        return self._prepared[key]
+
     def state_bytes(self) -> Dict[str, int]:
         p = sum(sp.total_units * sp.unit_bytes for sp in self.specs)
         k = 0

@@ -209,3 +209,14 @@ def test_shard_linear_argument_errors(ctx):
         d2 = etp.TensorDesc(N, K * 2, {0: (w.ptr, N - 1, 0)}, 1, 0)
         etp.etp_shard_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, T, K, N, d2, ok, 1, y.ptr)
     assert e.value.status == 3
+
+
+def smoke_shard_linear(ctx):
+    """Used by __graft_entry__.smoke(): config 1's layer on the resharded state, 4 tokens, against the oracle reference."""
+    from tests import test_gpu_reshard as TR
+    cfg = get_config("1")
+    world = H.build_param_world(cfg, side=LibSide, mode="tight")
+    bufs, images = TR.upload_param_world(world)
+    TR.run_param_step(ctx, world, bufs, images, 0, Streams())
+    outs = linear_checks_for_world(ctx, world, bufs, world.steps[0].new, cfg.tokens, dead=world.steps[0].dead)
+    print(f"smoke shard_linear OK: {len(outs)} linears of config 1 on the resharded layout within {TOL} of the unsharded reference")
