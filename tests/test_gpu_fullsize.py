@@ -1,0 +1,320 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (ModelState, two streams, single-phase
+slabs, device-resident and pinned reload sources).
+
+Two kinds of check per config:
+  * the plain definition over the WHOLE state, evaluated on the device from the seeded generator (every byte of the
+    unsharded tensors / KV reference is a pure function of its index, workloads/gen.py): every unit of every new shard ==
+    the unsharded tensor's unit; every slot outside the new shards still holds what it held before; every (layer, K|V, live
+    block, token, new head) fragment == the reference fragment.  These hold at any size.
+  * the CPU oracle (oracle/state.py, element by element) on sampled layers: their slabs / pool planes are copied to the
+    host before the reshard, the oracle applies the plan, and the result is compared byte for byte with what the GPU left.
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_2511_11617_b200 as etp
+from oracle import planning as OP
+from oracle import state as OS
+from paper_2511_11617_b200.state import ModelState
+from workloads import get_config
+from workloads.configs import scaled
+from workloads.gen import fill_bytes, fill_kv_pool, fill_normal16
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = etp.Context(0)
+    yield c
+    c.close()
+
+
+def slot_runs(begin, end, anchor, cap):
+    """[(first unit, n units, first slot)] of units [begin, end) in a slot-addressed slab (test-side restatement of L3)."""
+    out, u = [], begin
+    while u < end:
+        s = (u - anchor) % cap
+        n = min(end - u, cap - s)
+        out.append((u, n, s))
+        u += n
+    return out
+
+
+def holdings(state, klass, upto_step):
+    """rank -> list of (unit interval) the rank's slab holds VALID data for after steps [0, upto_step) — new shard — plus
+    the stale units it held before and that were not overwritten.  Returned as {rank: {slot: unit}} would be O(units); we
+    return interval lists instead: (valid [(b, e)], stale candidates in order of age [(b, e), ...])."""
+    first = state.initial_layouts()[klass]
+    hist = {r: [(s, e)] for (r, s, e, _) in first}
+    for i in range(upto_step):
+        for (r, s, e, _) in state.steps[i].new[klass]:
+            hist[r].append((s, e))
+    return hist
+
+
+def expected_slab(state, sp, r, upto_step, garbage):
+    """Device tensor: what rank r's slab of tensor sp must hold after steps [0, upto_step): start from the initial image
+    (garbage or zeros + the initial shard), then overlay each later shard the rank owned, oldest first; a newer unit
+    landing on a slot replaces the older one (the slot rule makes the address a function of the unit alone)."""
+    anchor, cap = state.geom[sp.klass][r]
+    eb = state.cfg.model.elem_bytes
+    epu = sp.unit_bytes // eb
+    nb = cap * sp.unit_bytes
+    if garbage:
+        exp = fill_bytes(state.seed, 10_000 + sp.stream * 16 + r, 0, (nb + 7) // 8 * 8, device=state.device)[:nb].clone()
+    else:
+        exp = torch.zeros(nb, dtype=torch.uint8, device=state.device)
+    for (b, e) in holdings(state, sp.klass, upto_step)[r]:
+        for (u, n, s) in slot_runs(b, e, anchor, cap):
+            fill_normal16(state.seed, sp.stream, u * epu, n * epu, state.cfg.model.init_std, state.dt,
+                          out=exp[s * sp.unit_bytes:(s + n) * sp.unit_bytes].view(state.dt))
+    return exp
+
+
+def check_params_whole_state(state, upto_step, garbage):
+    dead = {st.dead for st in state.steps[:upto_step]}
+    n = 0
+    for sp in state.specs:
+        for r, slab in state.slabs[sp.name].items():
+            if r in dead:
+                continue
+            exp = expected_slab(state, sp, r, upto_step, garbage)
+            if not torch.equal(slab, exp):
+                bad = torch.nonzero(slab != exp)[:4].flatten().tolist()
+                raise AssertionError(f"{sp.name} rank {r}: slab differs from the plain definition at bytes {bad}")
+            n += slab.numel()
+            del exp
+    return n
+
+
+def snapshot_layer_params(state, layer):
+    """Host copies of every slab of `layer`'s tensors (pre-reshard image for the oracle)."""
+    return {sp.name: {r: t.cpu().numpy().copy() for r, t in state.slabs[sp.name].items()} for sp in state.specs if sp.layer == layer}
+
+
+def oracle_layer_params(state, step_idx, snap):
+    """oracle/state.apply_params on the snapshot of one layer; returns {name: {rank: expected slab bytes}}."""
+    st = state.steps[step_idx]
+    out = {}
+    for sp in state.specs:
+        if sp.name not in snap:
+            continue
+        M = len(st.new[sp.klass])
+        tasks = OP.cmm_plan([tuple(s) for s in st.old[sp.klass]], M, OP.partition(sp.total_units, M, state.cfg.scenario.new_policy))[0]
+        lo, hi = state.reload_range[sp.klass]
+        epu = sp.unit_bytes // state.cfg.model.elem_bytes
+        img = None
+        if hi > lo:
+            img = fill_normal16(state.seed, sp.stream, lo * epu, (hi - lo) * epu, state.cfg.model.init_std, state.dt,
+                                device=state.device).view(torch.uint8).cpu().numpy()
+        alive = {r: a for r, a in snap[sp.name].items() if r != st.dead}
+        exp, _ = OS.apply_params(tasks, alive, state.geom[sp.klass], sp.unit_bytes, img, lo)
+        out[sp.name] = exp
+    return out
+
+
+def compare_layer_params(state, expect):
+    for name, per_rank in expect.items():
+        for r, e in per_rank.items():
+            got = state.slabs[name][r].cpu().numpy()
+            assert np.array_equal(got, e), f"{name} rank {r}: GPU slab != oracle image"
+
+
+# ------------------------------------------------------------------------------------------------ paged KV
+def kv_dims(state):
+    m, kv = state.cfg.model, state.kv
+    return m.n_layers * 2, kv["n_blocks"], state.cfg.kv.block_size, kv["head_cap"], kv["frag"]
+
+
+def live_block_ids(state):
+    t = state.kv["table"]
+    return torch.from_numpy(np.unique(t[t >= 0]).astype(np.int64)).to(state.device)
+
+
+def expected_pool(state, r, upto_step, garbage):
+    """What rank r's pool must hold after steps [0, upto_step) with an identity page table: the initial image (its old
+    heads in EVERY block, as ModelState fills them), then, step by step, the heads of its new shard in the LIVE blocks only
+    (free blocks are never copied, reading K6)."""
+    planes, n_blocks, bs, cap, frag = kv_dims(state)
+    m = state.cfg.model
+    seed = state.seed + 500
+    rows = planes * n_blocks * bs
+    nb = rows * cap * frag
+    first = {rr: (s, e) for (rr, s, e, _) in state.initial_layouts()["head"]}
+    anchor = state.kv["anchors"][r]
+    if garbage:
+        exp = fill_bytes(seed, 100 + r, 0, (nb + 7) // 8 * 8, device=state.device)[:nb].clone()
+    else:
+        exp = torch.zeros(nb, dtype=torch.uint8, device=state.device)
+    s, e = first[r]
+    if e > s:
+        fill_kv_pool(exp, rows, cap, m.head_dim, 0, s, e - s, m.n_kv_heads, seed, 1, state.dt)
+    live = live_block_ids(state)
+    ev = exp.view(planes, n_blocks, bs, cap, frag)
+    held = set(range(s, e))
+    for i in range(upto_step):
+        new = [(b, e2) for (rr, b, e2, _) in state.steps[i].new["head"] if rr == r]
+        for (b, e2) in new:
+            for h in range(b, e2):
+                if h in held:
+                    continue                                   # KEEP: never touched
+                one = torch.empty(rows * frag, dtype=torch.uint8, device=state.device)
+                fill_kv_pool(one, rows, 1, m.head_dim, 0, h, 1, m.n_kv_heads, seed, 1, state.dt)
+                ov = one.view(planes, n_blocks, bs, frag)
+                ev[:, live, :, (h - anchor) % cap, :] = ov[:, live]
+                del one, ov
+            held = set(range(b, e2))
+    return exp
+
+
+def check_kv_whole_state(state, upto_step, garbage):
+    dead = {st.dead for st in state.steps[:upto_step]}
+    n = 0
+    for r, pool in state.kv["pools"].items():
+        if r in dead:
+            continue
+        exp = expected_pool(state, r, upto_step, garbage)
+        if not torch.equal(pool, exp):
+            bad = torch.nonzero(pool != exp)[:4].flatten().tolist()
+            raise AssertionError(f"KV pool of rank {r} differs from the plain definition at bytes {bad}")
+        n += pool.numel()
+        del exp
+    return n
+
+
+def layer_slice(state, t, layer, heads):
+    planes, n_blocks, bs, cap, frag = kv_dims(state)
+    per_layer = 2 * n_blocks * bs * heads * frag
+    return t[layer * per_layer:(layer + 1) * per_layer]
+
+
+def snapshot_layer_kv(state, layer):
+    cap = state.kv["head_cap"]
+    return {r: layer_slice(state, p, layer, cap).cpu().numpy().copy() for r, p in state.kv["pools"].items()}
+
+
+def oracle_layer_kv(state, step_idx, layer, snap, image):
+    st = state.steps[step_idx]
+    m, kv = state.cfg.model, state.kv
+    planes, n_blocks, bs, cap, frag = kv_dims(state)
+    g1 = OS.KVGeom(1, n_blocks, bs, cap, m.head_dim, m.elem_bytes, 0)
+    sc = state.cfg.scenario
+    H = m.n_kv_heads
+    tasks = OP.cmm_plan([tuple(s) for s in st.old["head"]], len(st.new["head"]), OP.partition(H, len(st.new["head"]), sc.new_policy))[0]
+    _, evicted, pairs = OS.page_table_rewrite(kv["table"], kv["seq_lens"], kv["last_use"], bs, n_blocks)
+    assert not evicted
+    per_kind, hh, ds = kv["backup"][step_idx]
+    backup = layer_slice(state, per_kind[image], layer, hh).cpu().numpy() if hh > 0 else None
+    alive = {r: a for r, a in snap.items() if r != st.dead and any(rr == r for (rr, _, _, _) in st.old["head"])}
+    exp, stats = OS.apply_kv(tasks, alive, kv["anchors"], g1, backup, hh, ds, pairs)
+    return exp, stats
+
+
+def compare_layer_kv(state, layer, expect):
+    cap = state.kv["head_cap"]
+    for r, e in expect.items():
+        got = layer_slice(state, state.kv["pools"][r], layer, cap).cpu().numpy()
+        assert np.array_equal(got, e), f"KV pool of rank {r}, layer {layer}: GPU planes != oracle image"
+
+
+# ------------------------------------------------------------------------------------------------ S7 on sampled outputs
+def check_linear_sampled(ctx, state, step_idx, layer, tokens, n_tok=12, n_feat=24):
+    """etp_shard_linear on the resharded slabs of one layer at `tokens` tokens; n_tok x n_feat sampled outputs per linear are
+    recomputed in fp64 from the generator's values of the UNSHARDED weight rows (oracle/linear.py) - max rel err <= 5e-3."""
+    from oracle import linear as OL
+    from workloads.gen import as_u8, normal16_at
+    dtn = state.cfg.model.dtype
+    rng = np.random.default_rng(1234 + layer)
+    worst = 0.0
+    for sp in state.specs:
+        if sp.layer != layer:
+            continue
+        lin = state.linear(sp.name, step_idx, after=True)
+        K, N = lin.K, lin.N
+        x = fill_normal16(state.seed, 9100 + sp.stream, 0, tokens * K, 1.0, state.dt, device=state.device)
+        y = torch.full((tokens * N,), float("nan"), dtype=state.dt, device=state.device)
+        lin.run(ctx, x.data_ptr(), tokens, y.data_ptr(), 0)
+        torch.cuda.synchronize()
+        assert torch.isfinite(y.float()).all(), f"{sp.name}: unwritten or poisoned outputs"
+        ts = np.unique(np.concatenate([[0, tokens - 1], rng.integers(0, tokens, n_tok)]))
+        ns = np.unique(np.concatenate([[0, N - 1], rng.integers(0, N, n_feat)]))
+        xs = OL.decode16(as_u8(x.view(tokens, K)[torch.from_numpy(ts).to(state.device)]), dtn).reshape(len(ts), K)
+        k = torch.arange(K, dtype=torch.int64, device=state.device)
+        nn = torch.from_numpy(ns).to(state.device)
+        idx = (k[None, :] * N + nn[:, None]) if sp.transposed else (nn[:, None] * K + k[None, :])     # element index in the unsharded tensor
+        ws = OL.decode16(as_u8(normal16_at(idx, state.seed, sp.stream, state.cfg.model.init_std, state.dt)), dtn).reshape(len(ns), K)
+        ref = OL.linear_ref(xs, ws)
+        got = OL.decode16(as_u8(y.view(tokens, N)[torch.from_numpy(ts).to(state.device)][:, nn]), dtn).reshape(len(ts), len(ns))
+        err = OL.max_rel_err(got, ref)
+        assert err <= 5e-3, f"{sp.name} T={tokens}: max relative error {err:.3e} on sampled outputs"
+        worst = max(worst, err)
+    return worst
+
+
+# ------------------------------------------------------------------------------------------------ the tests
+def run_full_config(ctx, key, image, linear_tokens=(), garbage=True, shrink=None):
+    cfg = get_config(key)
+    if shrink:
+        cfg = scaled(cfg, **shrink)
+    state = ModelState(cfg, device="cuda:0", image=image, slack_garbage=garbage)
+    cs, rs = torch.cuda.Stream(), torch.cuda.Stream()
+    m = cfg.model
+    for i, st in enumerate(state.steps):
+        layer = (7 * i + 3) % m.n_layers
+        sample_layers = [layer] + ([-1] if (m.vocab and i == 0) else [])
+        snaps = {L: snapshot_layer_params(state, L) for L in sample_layers}
+        ksnap = snapshot_layer_kv(state, layer)
+        rep = state.reshard(ctx, i, image, cs.cuda_stream, rs.cuda_stream, replan=True)
+        cs.synchronize()
+        rs.synchronize()
+        assert rep["params"]["n_phases"] == 1 and not rep["evicted"]
+        # the oracle on the sampled layers
+        for L in sample_layers:
+            compare_layer_params(state, oracle_layer_params(state, i, snaps[L]))
+        kexp, kstats = oracle_layer_kv(state, i, layer, ksnap, image)
+        compare_layer_kv(state, layer, kexp)
+        assert (rep["kv"]["d2d_bytes"], rep["kv"]["h2d_bytes"] + rep["kv"]["reload_dev_bytes"]) == \
+               (kstats["d2d_bytes"] * m.n_layers, kstats["h2d_bytes"] * m.n_layers)
+        # byte accounting of the parameters from the oracle's plan
+        d2d = h2d = 0
+        for sp in state.specs:
+            M = len(st.new[sp.klass])
+            tasks = OP.cmm_plan([tuple(s) for s in st.old[sp.klass]], M, OP.partition(sp.total_units, M, cfg.scenario.new_policy))[0]
+            ps = OP.plan_stats(tasks)
+            d2d += ps["transfer_units"] * sp.unit_bytes
+            h2d += ps["reload_units"] * sp.unit_bytes
+        assert rep["params"]["d2d_bytes"] == d2d and rep["params"]["h2d_bytes"] + rep["params"]["reload_dev_bytes"] == h2d
+        # the plain definition over the whole state
+        check_params_whole_state(state, i + 1, garbage)
+        check_kv_whole_state(state, i + 1, garbage)
+        for T in linear_tokens:
+            check_linear_sampled(ctx, state, i, layer, T)
+    return state
+
+
+@pytest.mark.parametrize("image", ["device", "pinned"])
+def test_config2_full_state(ctx, image):
+    """BASELINE.json configs[1]: Qwen3-14B shape, 4 -> 3 after rank 1 fails, heads 3/3/2 - the bench workload."""
+    run_full_config(ctx, "2", image, linear_tokens=(4, 4096) if image == "device" else ())
+
+
+def test_config2b_full_state_floor_policy(ctx):
+    """same workload under the paper's floor-boundary policy (heads 2/3/3): one KV head and its weights move D2D."""
+    run_full_config(ctx, "2b", "pinned", linear_tokens=(4,))
+
+
+def test_config3_full_state(ctx):
+    """configs[2]: Llama-3-8B shape, 8 -> 7 after rank 5 fails, unequal old FFN widths."""
+    run_full_config(ctx, "3", "pinned", linear_tokens=(4,))
+
+
+def test_config4_full_state_moe(ctx):
+    """configs[3]: Qwen3-30B-A3B shape (24 layers), 4 -> 3, experts repartitioned unequally (42/43/43)."""
+    run_full_config(ctx, "4", "pinned")
+
+
+def test_config5a_sequential_failures_full_state(ctx):
+    """configs[4] (a): Llama-3-8B shape, 8 -> 7 -> 6 -> 5, each reshard planned from the previous layout."""
+    run_full_config(ctx, "5a", "pinned", linear_tokens=(4,))
