@@ -41,6 +41,7 @@ def parse_args():
     ap.add_argument("--layers", type=int, default=0, help="debug: fewer layers (marks the result as reduced)")
     ap.add_argument("--seqs", type=int, default=0, help="debug: fewer sequences (marks the result as reduced)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--microbench", action="store_true", help="config 5b: copy-kernel microbenchmark over synthetic plans")
     ap.add_argument("--no-linear", action="store_true", help="skip the S7 (shard linear) leg")
     ap.add_argument("--linear-only", action="store_true", help="only the S7 leg, on parameters alone (for ncu captures of kernel (c))")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0, help="CPU seconds of oracle work in the cpu_baseline leg")
@@ -255,6 +256,74 @@ def shard_linear_leg(state, ctx, dev, hbm_peak, tokens_list=(4, 4096)):
     return out
 
 
+# ================================================================================================ config 5b
+def run_microbench(args):
+    """Config 5b: the interval-copy kernel over synthetic plans - n in 10^2..10^6 intervals, sizes log-uniform from 256 B to
+    the per-n clip of workloads/configs.py (R-5b), random 16-B aligned sources in a 32-GiB arena, disjoint
+    destinations with random gaps - plus fixed-size buckets.  One JSON line; sampled intervals are verified against the source."""
+    import numpy as np
+    import torch
+    import paper_2511_11617_b200 as etp
+    from workloads.configs import MICROBENCH_HI, MICROBENCH_LO
+    from workloads.gen import SEED0, fill_bytes, microbench_intervals
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    hbm_peak, peak_src = load_peaks()
+    ctx = etp.Context(0)
+    ctx.set_option(etp.OPT_TIME_KERNELS, 1)
+    st = torch.cuda.Stream(dev)
+    src_arena = 32 << 30
+    src = fill_bytes(SEED0 + 5000, 1, 0, src_arena, device=dev)
+    rng = np.random.default_rng(7)
+    torch.cuda.synchronize(dev)          # the source fill ran on torch's stream; the copies run on `st`
+
+    def run_plan(so, do, sz, dst_arena, iters=5):
+        dst = torch.empty(dst_arena + 256, dtype=torch.uint8, device=dev)
+        sp, dp = so + src.data_ptr(), do + dst.data_ptr()
+        kms, cms = [], []
+        for it in range(2 + iters):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            rep = etp.etp_copy_intervals(ctx, sp, dp, sz, st.cuda_stream)
+            e1.record(st)
+            e1.synchronize()
+            ms, _ = ctx.kernel_time()
+            if it >= 2:
+                kms.append(ms)
+                cms.append(e0.elapsed_time(e1))
+        n = len(sz)
+        pick = np.unique(np.concatenate([[int(np.argmax(sz)), int(np.argmin(sz))], rng.integers(0, n, 62)]))
+        for i in pick:
+            a, b, m = int(so[i]), int(do[i]), int(sz[i])
+            assert torch.equal(dst[b:b + m], src[a:a + m]), f"interval {i} differs from its source"
+        del dst
+        kms.sort(), cms.sort()
+        tot = int(sz.sum())
+        k, c = kms[len(kms) // 2], cms[len(cms) // 2]
+        return {"n": n, "total_GiB": round(tot / 2 ** 30, 3), "kernel_ms": round(k, 4), "moved_GBps": round(tot / k / 1e6, 1),
+                "hbm_frac": round(2.0 * tot / k / 1e6 / hbm_peak, 4), "call_ms": round(c, 3), "call_GBps": round(tot / c / 1e6, 1),
+                "segments": rep["n_jobs"], "work_items": rep["n_units"], "lower_ms": round(rep["lower_ms"], 3)}
+
+    sweep, buckets = [], []
+    for n in (100, 1000, 10_000, 100_000, 1_000_000):
+        so, do, sz, arena = microbench_intervals(n, MICROBENCH_LO, MICROBENCH_HI[n], SEED0 + 5000 + n, src_arena)
+        r = run_plan(so, do, sz, arena)
+        r["size_hi"] = MICROBENCH_HI[n]
+        sweep.append(r)
+    for size, n in ((256, 1 << 18), (4096, 1 << 18), (65536, 1 << 16), (1 << 20, 1 << 13), (16 << 20, 512)):
+        sz = np.full(n, size, dtype=np.int64)
+        so = rng.integers(0, (src_arena - size) // 16, n).astype(np.int64) * 16
+        do = np.arange(n, dtype=np.int64) * (size + 16)
+        r = run_plan(so, do, sz, int(do[-1] + size))
+        r["size"] = size
+        buckets.append(r)
+    print(json.dumps({"microbench": "config 5b: etp_copy_intervals", "peak": hbm_peak, "peak_source": peak_src,
+                      "hbm_frac": "2 x moved bytes / kernel time / peak; call_* include descriptor lowering + upload",
+                      "by_n": sweep, "by_size": buckets}))
+    ctx.close()
+    return 0
+
+
 # ================================================================================================ the CUDA path
 def run_ours(args):
     import torch
@@ -434,4 +503,6 @@ def run_ours(args):
 
 if __name__ == "__main__":
     a = parse_args()
+    if a.microbench:
+        sys.exit(run_microbench(a))
     sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))
