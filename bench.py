@@ -324,6 +324,23 @@ def run_microbench(args):
     return 0
 
 
+# ================================================================================================ multi-rank plumbing
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """Replicas only: every rank times its own replica; the job's time is the MAX over ranks."""
+    if world <= 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gbps(bytes_per_rank: float, world: int, ms: float) -> float:
+    """value = the units ALL ranks processed / the max-over-ranks time (weak scaling: per-GPU work is fixed)."""
+    return bytes_per_rank * world / (ms * 1e-3) / 1e9
+
+
 # ================================================================================================ the CUDA path
 def run_ours(args):
     import torch
@@ -398,10 +415,7 @@ def run_ours(args):
                     h2d += r["h2d_bytes"]
                     launches += r["n_kernel_launches"]
         barrier()
-        if world > 1:
-            t = torch.tensor([tot_ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            tot_ms = float(t.item())
+        tot_ms = max_over_ranks(tot_ms, world, dev)
         return tot_ms, moved, h2d, launches, rep
 
     def kernel_leg(image, K):
@@ -460,8 +474,8 @@ def run_ours(args):
             dist.destroy_process_group()
         return 0
 
-    value = moved * world / (tot_ms * 1e-3) / 1e9
-    e2e = e_moved * world / (e_ms * 1e-3) / 1e9
+    value = whole_job_gbps(moved, world, tot_ms)
+    e2e = whole_job_gbps(e_moved, world, e_ms)
     achieved = 2.0 * kbytes / (kms * 1e-3) / 1e9 if kms > 0 else 0.0
     rp, rk = rep["params"] or {}, rep["kv"] or {}
     ep, ek = e_rep["params"] or {}, e_rep["kv"] or {}

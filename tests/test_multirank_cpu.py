@@ -1,0 +1,63 @@
+"""The N > 1 path of bench.py on CPU (gloo, world_size 2).  The hot path does not shard ("replicas only"):
+every rank reshards its own replica, there is no data-path collective, and the only cross-rank step is the max-over-ranks
+of the device times; `value` = bytes of ALL ranks / that time.  `--impl reference` runs on rank 0 alone."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import bench
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        ms = bench.max_over_ranks(10.0 + 5.0 * rank, world, torch.device("cpu"))     # rank 1 is the slow replica
+        out[rank] = (ms, bench.whole_job_gbps(3e9, world, ms))
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_max_over_ranks_and_whole_job_value_gloo_world2():
+    world, port = 2, 29500 + os.getpid() % 2000
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker, args=(world, port, out), nprocs=world, join=True)
+        res = dict(out)
+    assert res[0] == res[1]                                  # every rank sees the same aggregate
+    ms, gbps = res[0]
+    assert ms == 15.0                                        # the MAX over ranks, not the mean or rank 0's
+    assert gbps == pytest.approx(2 * 3e9 / 15e-3 / 1e9)      # bytes of all ranks / max time
+
+
+def _run_reference(rank):
+    env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", LOCAL_RANK=str(rank), CUDA_VISIBLE_DEVICES="")
+    return subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1", "--gpus", "2",
+                           "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=600)
+
+
+def test_reference_arm_runs_on_rank0_only():
+    r1 = _run_reference(1)
+    assert r1.returncode == 0 and r1.stdout.strip() == ""   # other ranks exit 0 without work
+    r0 = _run_reference(0)
+    assert r0.returncode == 0, r0.stderr[-2000:]
+    line = json.loads(r0.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+    assert line["gpu_launches"] == 0 and line["higher_is_better"] is True
+
+
+def test_ours_fails_loudly_without_a_gpu():
+    env = dict(os.environ, CUDA_VISIBLE_DEVICES="")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--warmup", "0"], env=env,
+                       capture_output=True, text=True, timeout=600)
+    assert r.returncode != 0 and "no CPU fallback" in (r.stderr + r.stdout)
