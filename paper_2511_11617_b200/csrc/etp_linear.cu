@@ -25,7 +25,6 @@
 #include <cuda_fp16.h>
 
 #include <algorithm>
-#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -59,7 +58,6 @@ struct alignas(64) LinearParams {
     void* y;
     float* partials;          // split-K workspace [(tile * n_splits + split)][BN][128]
     unsigned int* tickets;    // one per output tile, zero between launches (the last arriver resets its ticket)
-    int32_t debug;
 };
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
@@ -240,7 +238,7 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
     } else if (warp == 1) {
         // ===================================================================== MMA issuer (one elected lane)
         if (lane == 0) {
-            const bool a_mn = row_par && !(p.debug & 1);
+            const bool a_mn = row_par;
             const uint32_t idesc = make_idesc(p.dtype == ETP_BF16 ? 1u : 0u, a_mn ? 1u : 0u, uint32_t(BN));
             // A, K-major  : rows of 128 B, 8-row groups 1024 B apart (SBO); LBO unused with 128B swizzle; +32 B per UMMA_K.
             // A, MN-major : k rows of 128 B (64 out features), 8-k groups 1024 B apart (SBO), the second 64 out features
@@ -265,7 +263,7 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
                     const uint64_t b_desc = make_smem_desc(smem_u32(sa + kABytes), 16, 1024);
 #pragma unroll
                     for (int k = 0; k < kBK / kUmmaK; ++k)
-                        if (!(p.debug & 2)) tc_mma(d_tmem, a_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > it.c0 || k > 0) ? 1u : 0u);
+                        tc_mma(d_tmem, a_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > it.c0 || k > 0) ? 1u : 0u);
                     tc_commit(&empty_bar[stage]);   // frees the smem stage once these MMAs have read it
                     if (++stage == C::kStages) { stage = 0; phase ^= 1; }
                 }
@@ -548,7 +546,6 @@ extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_d
         else ETP_TRY(encode_2d(&p.map_w[r], dtype, run_addr[r], p.runs[r].n_feat, in_features, in_features, kBK, kBM));
     }
 
-    if (const char* dbg = getenv("ETP_LINEAR_DEBUG")) p.debug = atoi(dbg);
     const int grid = int(std::min<int64_t>(n_items, ctx->n_sms));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     ctx->launches = 1;
