@@ -214,13 +214,66 @@ __device__ void copy_vec_item(const CopyArgs& a, unsigned int idx, int lane) {
     copy_rows(j, lane);
 }
 
+// One batch of small contiguous intervals: 32 descriptors per round, one per lane.  Their lengths (in
+// 16-byte words) are prefix-summed across the warp, then the warp walks the concatenated words with consecutive lanes on
+// consecutive words; the interval of word w is the largest j with excl[j] <= w, found by a 5-step shuffle search, and its
+// addresses come from lane j (pre-biased by -excl[j]*16 so that address = base + w*16).
+__device__ void copy_small_batch(const CopyArgs& a, unsigned int k, int lane) {
+    const uint32_t s0 = __ldg(a.small_first + k), s1 = __ldg(a.small_first + k + 1);
+    for (uint32_t s = s0; s < s1; s += 32) {
+        uint64_t sb = 0, db = 0;
+        uint32_t nv = 0;
+        if (s + lane < s1) {
+            const uint4* p = reinterpret_cast<const uint4*>(a.small + s + lane);
+            const uint4 q0 = __ldg(p), q1 = __ldg(p + 1);
+            sb = u64_of(q0.x, q0.y);
+            db = u64_of(q0.z, q0.w);
+            nv = q1.x >> 4;
+        }
+        uint32_t incl = nv;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        const uint32_t excl = incl - nv;
+        const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
+        sb -= (uint64_t)excl * 16;
+        db -= (uint64_t)excl * 16;
+        for (uint32_t w0 = 0; w0 < total; w0 += 32 * kUnroll) {   // uniform trip count: every lane joins the shuffles
+            uint4 buf[kUnroll];
+            uint64_t da[kUnroll];
+#pragma unroll
+            for (int u = 0; u < kUnroll; ++u) {
+                const uint32_t w = w0 + 32 * u + lane;
+                int j = 0;
+#pragma unroll
+                for (int step = 16; step >= 1; step >>= 1) {
+                    const uint32_t e = __shfl_sync(0xffffffffu, excl, j + step);
+                    if (e <= w) j += step;
+                }
+                const uint64_t sj = __shfl_sync(0xffffffffu, sb, j);
+                da[u] = __shfl_sync(0xffffffffu, db, j) + (uint64_t)w * 16;
+                if (w < total) buf[u] = ld_stream(reinterpret_cast<const char*>(sj + (uint64_t)w * 16));
+            }
+#pragma unroll
+            for (int u = 0; u < kUnroll; ++u)
+                if (w0 + 32 * u + lane < total) st_stream(reinterpret_cast<char*>(da[u]), buf[u]);
+        }
+    }
+}
+
 __device__ void vector_warp(const CopyArgs& a, int lane) {
+    const unsigned int n_items = a.n_vec_items + a.n_small_batches;
     for (;;) {
         unsigned int idx = 0;
         if (lane == 0) idx = atomicAdd(&a.counters[1], 1u);
         idx = __shfl_sync(0xffffffffu, idx, 0);
-        if (idx >= a.n_vec_items) break;
-        copy_vec_item(a, idx, lane);
+        if (idx >= n_items) break;
+        if (idx < a.n_vec_items)
+            copy_vec_item(a, idx, lane);
+        else
+            copy_small_batch(a, idx - a.n_vec_items, lane);
     }
     if (a.flags & 1u) {
         // drain the bulk queue too (one item per warp at a time)

@@ -8,6 +8,8 @@
 //   * VEC queue   - ~32-KiB items: pieces of small intervals, or the head-strided KV fragments of one (live block, plane
 //                   group).  Each of the other warps claims one item at a time and moves it with 16-byte ld.global.nc /
 //                   st.global, 8 vectors in flight per lane, consecutive lanes on consecutive 16-byte words of a row.
+//                   Intervals of <= 32 KiB are batched (<= 128 per item): the warp loads 32 descriptors at once, scans
+//                   their lengths and walks the concatenated 16-byte words, finding each word's interval by a shuffle search.
 #pragma once
 #include "etp_internal.h"
 
@@ -25,7 +27,9 @@ struct CopyArgs {
     const uint32_t* bulk_items;   // segment index of every bulk work item
     const uint32_t* vec_items;    // segment index of every vector work item
     const int2* pairs;            // {old block id, new block id} lists of the VEC_PAGED segments
-    unsigned int n_bulk_items, n_vec_items;
+    const SmallSeg* small;        // small contiguous intervals, batched: vector-queue items n_vec_items .. + n_small_batches
+    const uint32_t* small_first;  // n_small_batches + 1 entries
+    unsigned int n_bulk_items, n_vec_items, n_small_batches;
     unsigned int* counters;       // [0] bulk head, [1] vec head (zeroed before launch)
     unsigned int flags;           // bit 0: vector warps also drain the bulk queue when theirs is empty
 };

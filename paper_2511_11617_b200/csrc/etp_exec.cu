@@ -153,10 +153,11 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
     w->phases.resize(n_ph);
     w->host_gather.resize(n_ph);
 
-    // ---- descriptor arena layout: pairs | per phase: bulk segs, bulk items, vec segs, vec items, gather segs, gather items
+    // ---- descriptor arena layout: pairs | per phase: bulk segs, bulk items, vec segs, vec items, small segs, batch starts,
+    //      gather segs, gather items
     int64_t total = 0, n_jobs = 0, n_items = 0;
     auto pad = [](int64_t b) { return (b + 255) & ~int64_t(255); };
-    struct Off { int64_t bulk, bulk_items, vec, vec_items, gat, gat_items; };
+    struct Off { int64_t bulk, bulk_items, vec, vec_items, small, small_first, gat, gat_items; };
     std::vector<Off> off(n_ph);
     const int64_t off_pairs = 0;
     total += pad((int64_t)w->pairs.size() * sizeof(int32_t));
@@ -167,12 +168,15 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
         off[p].bulk_items = total;  total += pad((int64_t)jl.n_bulk_items * sizeof(uint32_t));
         off[p].vec = total;         total += pad((int64_t)jl.vec.size() * sizeof(VecSeg));
         off[p].vec_items = total;   total += pad((int64_t)jl.n_vec_items * sizeof(uint32_t));
+        off[p].small = total;       total += pad((int64_t)jl.small.size() * sizeof(SmallSeg));
+        off[p].small_first = total; total += pad((int64_t)(jl.small_first.size() + 1) * sizeof(uint32_t));
         off[p].gat = total;         total += pad((int64_t)gl.vec.size() * sizeof(VecSeg));
         off[p].gat_items = total;   total += pad((int64_t)gl.n_vec_items * sizeof(uint32_t));
-        n_jobs += (int64_t)(jl.bulk.size() + jl.vec.size() + gl.vec.size());
-        n_items += (int64_t)jl.n_bulk_items + jl.n_vec_items + gl.n_vec_items;
+        n_jobs += (int64_t)(jl.bulk.size() + jl.vec.size() + jl.small.size() + gl.vec.size());
+        n_items += (int64_t)jl.n_bulk_items + jl.n_vec_items + (int64_t)jl.small_first.size() + gl.n_vec_items;
         launches_needed += (!jl.empty()) + (!gl.vec.empty());
-        if (jl.bulk.size() >= 0xFFFFFFF0ull || jl.vec.size() >= 0xFFFFFFF0ull || gl.vec.size() >= 0xFFFFFFF0ull)
+        if (jl.bulk.size() >= 0xFFFFFFF0ull || jl.vec.size() >= 0xFFFFFFF0ull || jl.small.size() >= 0xFFFFFFF0ull ||
+            gl.vec.size() >= 0xFFFFFFF0ull || (uint64_t)jl.n_vec_items + jl.small_first.size() >= 0xFFFFFFF0ull)
             ETP_FAIL(ETP_ERR_CAPACITY, "too many segments in one phase");
     }
     if (launches_needed > c->n_counter_slots) ETP_FAIL(ETP_ERR_CAPACITY, "plan needs %d launches > %d", launches_needed, c->n_counter_slots);
@@ -218,6 +222,12 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
                 std::memcpy(h + off[p].vec, jl.vec.data(), jl.vec.size() * sizeof(VecSeg));
                 fill_items((uint32_t*)(h + off[p].vec_items), jl.n_vec_items, &jl.vec[0].first_item, jl.vec.size(), sizeof(VecSeg));
             }
+            if (!jl.small.empty()) {
+                std::memcpy(h + off[p].small, jl.small.data(), jl.small.size() * sizeof(SmallSeg));
+                uint32_t* f = (uint32_t*)(h + off[p].small_first);
+                std::memcpy(f, jl.small_first.data(), jl.small_first.size() * sizeof(uint32_t));
+                f[jl.small_first.size()] = (uint32_t)jl.small.size();
+            }
             if (!gl.vec.empty()) {
                 std::memcpy(h + off[p].gat, gl.vec.data(), gl.vec.size() * sizeof(VecSeg));
                 fill_items((uint32_t*)(h + off[p].gat_items), gl.n_vec_items, &gl.vec[0].first_item, gl.vec.size(), sizeof(VecSeg));
@@ -254,6 +264,9 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
             a.pairs = (const int2*)(d_base + off_pairs);
             a.n_bulk_items = jl.n_bulk_items;
             a.n_vec_items = jl.n_vec_items;
+            a.small = (const SmallSeg*)(d_base + off[p].small);
+            a.small_first = (const uint32_t*)(d_base + off[p].small_first);
+            a.n_small_batches = (unsigned int)jl.small_first.size();
             a.counters = c->d_counters + 2 * counter_slot;
             a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
             if (timed) {
@@ -312,6 +325,9 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
                 a.vec_items = (const uint32_t*)(d_base + off[p].gat_items);
                 a.pairs = (const int2*)(d_base + off_pairs);
                 a.n_bulk_items = 0;
+                a.small = nullptr;
+                a.small_first = nullptr;
+                a.n_small_batches = 0;
                 a.n_vec_items = gl.n_vec_items;
                 a.counters = c->d_counters + 2 * counter_slot;
                 a.flags = 0;
@@ -403,6 +419,7 @@ extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_
     const double t0 = now_ms();
     LoweredWork w;
     w.phases.resize(1);
+    w.phases[0].small.reserve((size_t)n);
     for (int64_t i = 0; i < n; ++i) {
         const etp_interval& d = host_descs[i];
         if (d.bytes < 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has negative size", (long long)i);

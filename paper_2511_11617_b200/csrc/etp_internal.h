@@ -62,6 +62,18 @@ struct VecSeg {
     int64_t s_block, d_block;  // byte strides between blocks
 };
 enum { VEC_LINEAR = 0, VEC_PAGED = 1 };
+// A SMALL segment is a contiguous interval of at most kVecItem bytes (below the TMA threshold).  Consecutive small segments
+// are grouped on the host into BATCHES (<= kSmallBatchSegs segments, ~kVecItem bytes); one batch is one work item of the
+// vector queue (indices n_vec_items .. n_vec_items + n_small_batches - 1), so that a queue claim moves tens of KiB even when
+// every interval is 256 bytes.  32 B = one sector; batch k covers segments [small_first[k], small_first[k+1]).
+struct SmallSeg {
+    uint64_t src, dst;
+    uint32_t bytes;        // multiple of 16, <= kVecItem
+    uint32_t pad0;
+    uint64_t pad1;
+};
+static_assert(sizeof(SmallSeg) == 32, "SmallSeg layout");
+constexpr int kSmallBatchSegs = 128;
 static_assert(sizeof(BulkSeg) == 32, "BulkSeg layout");
 static_assert(sizeof(VecSeg) == 96, "VecSeg layout");
 
@@ -72,9 +84,12 @@ constexpr int64_t kVecItem = 32 << 10;     // bytes per vector work item (target
 struct JobList {
     std::vector<BulkSeg> bulk;
     std::vector<VecSeg> vec;
+    std::vector<SmallSeg> small;
+    std::vector<uint32_t> small_first;   // first segment of every batch
+    int64_t open_batch_bytes = 0;        // bytes in the last (still open) batch
     uint32_t n_bulk_items = 0, n_vec_items = 0;
     int64_t bytes = 0;
-    bool empty() const { return bulk.empty() && vec.empty(); }
+    bool empty() const { return bulk.empty() && vec.empty() && small.empty(); }
 };
 
 // A pinned-host -> device DMA of the reload pipeline (pipeline (b)).

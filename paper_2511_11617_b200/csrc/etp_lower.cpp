@@ -30,6 +30,15 @@ void push_contiguous(const etp_ctx* ctx, JobList* jl, const void* src, void* dst
     if (bytes >= tma_min) {
         jl->bulk.push_back({(uint64_t)(uintptr_t)src, (uint64_t)(uintptr_t)dst, (uint64_t)bytes, jl->n_bulk_items, 0});
         jl->n_bulk_items += (uint32_t)((bytes + kBulkItem - 1) / kBulkItem);
+    } else if (bytes <= kVecItem) {
+        const bool open = !jl->small_first.empty() && jl->small.size() - jl->small_first.back() < (size_t)kSmallBatchSegs &&
+                          jl->open_batch_bytes + bytes <= kVecItem;
+        if (!open) {
+            jl->small_first.push_back((uint32_t)jl->small.size());
+            jl->open_batch_bytes = 0;
+        }
+        jl->small.push_back({(uint64_t)(uintptr_t)src, (uint64_t)(uintptr_t)dst, (uint32_t)bytes, 0, 0});
+        jl->open_batch_bytes += bytes;
     } else {
         VecSeg v{};
         v.src = (uint64_t)(uintptr_t)src;

@@ -297,6 +297,31 @@ def test_copy_intervals_bit_exact(ctx, n, hi, tma_min):
     assert S.payload().tobytes() == src.tobytes()
 
 
+@pytest.mark.parametrize("size,n", [(16, 5000), (256, 4099), (4096, 777), (32768, 65)])
+def test_copy_intervals_small_batches(ctx, size, n):
+    """The descriptor-bound corner of config 5b: every interval the same small size, so every vector work item is a
+    batch of up to 128 intervals (or 32 KiB) walked with the shuffle search; ragged last batch, last round and last word."""
+    rng = np.random.default_rng(size + n)
+    src_arena = 8 << 20
+    src = rng.integers(0, 256, src_arena, dtype=np.uint8)
+    so = rng.integers(0, (src_arena - size) // 16, n).astype(np.int64) * 16
+    gaps = rng.integers(0, 4, n).astype(np.int64) * 16
+    do_sorted = np.cumsum(gaps + size) - size
+    do = do_sorted[rng.permutation(n)]
+    sz = np.full(n, size, dtype=np.int64)
+    dst0 = rng.integers(0, 256, int(do_sorted[-1] + size + 64), dtype=np.uint8)
+    expect = dst0.copy()
+    for a, b in zip(so, do):
+        expect[b:b + size] = src[a:a + size]
+    S, D = DevBuf(src), DevBuf(dst0)
+    stream = torch.cuda.Stream()
+    rep = etp.etp_copy_intervals(ctx, so + S.ptr, do + D.ptr, sz, stream.cuda_stream)
+    stream.synchronize()
+    assert D.guards_intact() and S.guards_intact()
+    assert D.payload().tobytes() == expect.tobytes()
+    assert rep["d2d_bytes"] == n * size
+
+
 def test_copy_intervals_errors(ctx):
     S, D = DevBuf(np.zeros(4096, np.uint8)), DevBuf(np.zeros(4096, np.uint8))
     for so, do, sz, status in [(8, 0, 16, 2), (0, 0, 24, 2), (0, 0, -16, 1)]:
