@@ -43,3 +43,43 @@ def max_rel_err(y: np.ndarray, ref: np.ndarray) -> float:
     d = float(np.max(np.abs(np.asarray(y, dtype=np.float64) - ref)))
     m = float(np.max(np.abs(ref)))
     return d / m if m > 0 else d
+
+
+# ---------------------------------------------------------------------------------------------- MoE layer (config 4)
+# SURVEY.md 8(c) reading G5 / DESIGN.md G5; PAPER.md:172-174 (MoE experts are the unit of the expert-granularity plan).
+# Router logits -> softmax over all experts -> top-k (tie -> lower expert index) -> weights renormalised to sum 1;
+# y[t] = sum over the k chosen experts e of w[t,e] * down_e( silu(gate_e x[t]) * (up_e x[t]) ).  Plain loops, fp64.
+def moe_route(logits: np.ndarray, top_k: int):
+    """logits [T][E] -> (experts [T][top_k] int64 in descending probability, weights [T][top_k] fp64 summing to 1)."""
+    logits = np.asarray(logits, dtype=np.float64)
+    T, E = logits.shape
+    idx = np.zeros((T, top_k), dtype=np.int64)
+    wts = np.zeros((T, top_k), dtype=np.float64)
+    for t in range(T):
+        z = np.exp(logits[t] - logits[t].max())
+        p = z / z.sum()
+        order = sorted(range(E), key=lambda e: (-p[e], e))[:top_k]
+        s = sum(p[e] for e in order)
+        for j, e in enumerate(order):
+            idx[t, j] = e
+            wts[t, j] = p[e] / s
+    return idx, wts
+
+
+def silu(v: np.ndarray) -> np.ndarray:
+    return v / (1.0 + np.exp(-v))
+
+
+def moe_ref(x: np.ndarray, logits: np.ndarray, gate: np.ndarray, up: np.ndarray, down_t: np.ndarray, top_k: int) -> np.ndarray:
+    """x [T][hidden]; gate, up [E][ffn][hidden]; down_t [E][ffn][hidden] (row-parallel weights are stored transposed,
+    reading L1: down_e(h) = h @ down_t[e]); gate / up / down_t may be arrays or mappings expert -> matrix (only the routed
+    experts are touched); returns y [T][hidden] in fp64."""
+    x = np.asarray(x, dtype=np.float64)
+    idx, wts = moe_route(logits, top_k)
+    y = np.zeros((x.shape[0], x.shape[1]), dtype=np.float64)
+    for t in range(x.shape[0]):
+        for j in range(top_k):
+            e = int(idx[t, j])
+            h = silu(np.asarray(gate[e], dtype=np.float64) @ x[t]) * (np.asarray(up[e], dtype=np.float64) @ x[t])
+            y[t] += wts[t, j] * (h @ np.asarray(down_t[e], dtype=np.float64))
+    return y

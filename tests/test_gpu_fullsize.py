@@ -253,6 +253,40 @@ def check_linear_sampled(ctx, state, step_idx, layer, tokens, n_tok=12, n_feat=2
     return worst
 
 
+def check_moe_layer(ctx, state, step_idx, layer, tokens=16):
+    """Reading G5 at full size (config 4): one MoE layer on the resharded expert slabs, per-expert etp_shard_linear calls on
+    the routed tokens (tests/moe_util.py), against the oracle's fp64 MoE layer on the generator's UNSHARDED expert matrices."""
+    from oracle import linear as OL
+    from tests import moe_util as MU
+    from workloads.gen import as_u8
+    m = state.cfg.model
+    E, F, Hd, dtn = m.n_experts, m.expert_ffn, m.hidden, m.dtype
+    names = {"gate": f"l{layer}.exp_gate", "up": f"l{layer}.exp_up", "down_t": f"l{layer}.exp_down_t"}
+    spec = {k: next(s for s in state.specs if s.name == n) for k, n in names.items()}
+    new = state.steps[step_idx].new["expert"]
+    x = fill_normal16(state.seed, 9300 + layer, 0, tokens * Hd, 1.0, state.dt, device=state.device).view(tokens, Hd)
+    logits = fill_normal16(state.seed, 9400 + layer, 0, tokens * E, 1.0, state.dt, device=state.device).view(tokens, E)
+
+    def locate(kind, e):
+        r = next(rr for (rr, b, en, _) in new if b <= e < en)
+        anchor, cap = state.geom["expert"][r]
+        return state.slabs[names[kind]][r].data_ptr(), anchor, cap, spec[kind].unit_bytes
+
+    y, order, wts, _ = MU.moe_layer_per_expert(ctx, dtn, x, logits, m.top_k, F, locate)
+
+    class Unsharded:
+        """expert -> fp64 [F][Hd] straight from the position-addressable generator (never from a slab)."""
+        def __init__(self, sp):
+            self.sp = sp
+        def __getitem__(self, e):
+            w = fill_normal16(state.seed, self.sp.stream, e * F * Hd, F * Hd, m.init_std, state.dt, device=state.device)
+            return OL.decode16(as_u8(w), dtn).reshape(F, Hd)
+
+    return MU.check_against_oracle(y, order, wts, OL.decode16(as_u8(x), dtn).reshape(tokens, Hd),
+                                   OL.decode16(as_u8(logits), dtn).reshape(tokens, E), Unsharded(spec["gate"]),
+                                   Unsharded(spec["up"]), Unsharded(spec["down_t"]), m.top_k)
+
+
 # ------------------------------------------------------------------------------------------------ the tests
 def run_full_config(ctx, key, image, linear_tokens=(), garbage=True, shrink=None):
     cfg = get_config(key)
@@ -291,6 +325,8 @@ def run_full_config(ctx, key, image, linear_tokens=(), garbage=True, shrink=None
         check_kv_whole_state(state, i + 1, garbage)
         for T in linear_tokens:
             check_linear_sampled(ctx, state, i, layer, T)
+        if m.n_experts and linear_tokens:
+            check_moe_layer(ctx, state, i, layer)
     return state
 
 
@@ -312,7 +348,7 @@ def test_config3_full_state(ctx):
 
 def test_config4_full_state_moe(ctx):
     """configs[3]: Qwen3-30B-A3B shape (24 layers), 4 -> 3, experts repartitioned unequally (42/43/43)."""
-    run_full_config(ctx, "4", "pinned")
+    run_full_config(ctx, "4", "pinned", linear_tokens=(4,))
 
 
 def test_config5a_sequential_failures_full_state(ctx):

@@ -187,6 +187,41 @@ def test_config1_layer_outputs_survive_the_reshard(ctx, mode):
             assert np.array_equal(before[sp.name], after[sp.name]), sp.name
 
 
+def test_moe_layer_on_resharded_experts(ctx):
+    """Reading G5 at a size the oracle finishes in seconds: 12 experts over 4 ranks (3/3/3/3), rank 1 fails, experts are
+    repartitioned 4/4/4; router logits N(0,1), top-4.  Every routed expert's gate / up / down runs through etp_shard_linear on
+    the bytes the reshard left in the slabs; the layer output matches the oracle's unsharded fp64 MoE layer within 5e-3."""
+    import dataclasses
+    from tests import moe_util as MU
+    from tests import test_gpu_reshard as TR
+    from workloads.configs import Config, KVShape, ModelShape, Scenario
+    shape = ModelShape("tiny-moe", 1, 256, 8, 4, 32, n_experts=12, expert_ffn=128, top_k=4)
+    cfg = Config(9, "moe-small", shape, KVShape(2, 64), Scenario(4, (1,)))
+    world = H.build_param_world(cfg, side=LibSide, mode="tight")
+    bufs, images = TR.upload_param_world(world)
+    TR.run_param_step(ctx, world, bufs, images, 0, Streams())
+    expect, _ = H.oracle_reshard_params(world, 0)
+    TR.compare_params(world, bufs, expect, {1})
+    new = world.steps[0].new["expert"]
+    dt = torch_dtype(shape.dtype)
+    T, E, F, Hd = 24, shape.n_experts, shape.expert_ffn, shape.hidden
+    x = fill_normal16(SEED, 740, 0, T * Hd, 1.0, dt).view(T, Hd).cuda()
+    logits = fill_normal16(SEED, 741, 0, T * E, 1.0, dt).view(T, E).cuda()
+    names = {"gate": "l0.exp_gate", "up": "l0.exp_up", "down_t": "l0.exp_down_t"}
+
+    def locate(kind, e):
+        r = next(rr for (rr, b, en, _) in new if b <= e < en)
+        anchor, cap = world.geom[names[kind]][r]
+        return bufs[names[kind]][r].ptr, anchor, cap, F * Hd * 2
+
+    y, order, wts, calls = MU.moe_layer_per_expert(ctx, shape.dtype, x, logits, shape.top_k, F, locate)
+    assert calls == 3 * len(np.unique(order))
+    mats = {k: OL.decode16(world.unsharded[n], shape.dtype).reshape(E, F, Hd) for k, n in names.items()}
+    MU.check_against_oracle(y, order, wts, OL.decode16(as_u8(x.cpu()), shape.dtype).reshape(T, Hd),
+                            OL.decode16(as_u8(logits.cpu()), shape.dtype).reshape(T, E), mats["gate"], mats["up"], mats["down_t"],
+                            shape.top_k)
+
+
 def test_shard_linear_argument_errors(ctx):
     T, K, N = 4, 64, 128
     w = DevBuf(np.zeros(N * K * 2, dtype=np.uint8))

@@ -263,6 +263,49 @@ def test_kv_staged_reload_mode(ctx):
         ctx.set_option(etp.OPT_KV_RELOAD_MODE, 0)
 
 
+# ------------------------------------------------------------------------------------------------ scale-up (a rank joins)
+@pytest.mark.parametrize("tight", [False, True])
+def test_scale_up_a_repaired_rank_joins(ctx, tight):
+    """PAPER.md:168 (scale-up after a GPU is repaired), reading C6: the joining rank is an ALIVE rank with an empty interval.
+    3 -> 4 ranks of 1201 units x 4112 B; nothing is reloaded, every target tiles from transfers and keeps; with tight slabs
+    (cap = the wider of old and new shard) shards wrap and the plan needs hazard phases."""
+    from oracle import planning as OP
+    Hn, ub = 1201, 4112
+    old = [(0, 0, 400, 1), (1, 400, 800, 1), (2, 800, Hn, 1), (3, Hn, Hn, 1)]
+    tasks, new = OP.cmm_plan(old, 4)
+    assert OP.plan_stats(tasks)["reload_units"] == 0 and new[3][2] - new[3][1] > 0
+    geom = {}
+    for (r, b, e, _), (_, nb, ne, _) in zip(old, new):
+        if tight:
+            geom[r] = (b if e > b else nb, max(e - b, ne - nb))
+        else:
+            lo, hi = (min(b, nb), max(e, ne)) if e > b else (nb, ne)
+            geom[r] = (lo, hi - lo)
+    rng = np.random.default_rng(11)
+    w = rng.integers(0, 256, Hn * ub, dtype=np.uint8)
+    slabs = {}
+    for (r, b, e, _) in old:
+        anchor, cap = geom[r]
+        slab = rng.integers(0, 256, cap * ub, dtype=np.uint8)
+        OS.place_units(slab, anchor, cap, ub, b, e, w)
+        slabs[r] = slab
+    expect, stats = OS.apply_params(tasks, slabs, geom, ub, None, 0)
+    for (r, b, e, _) in new:                       # the plain definition: every new shard is the unsharded slice
+        assert np.array_equal(OS.read_units(expect[r], *geom[r], ub, b, e), w[b * ub:e * ub])
+    bufs = {r: DevBuf(a) for r, a in slabs.items()}
+    plan = etp.etp_cmm_plan(old, 4)
+    assert plan.tasks() == [tuple(t) for t in tasks]
+    desc = etp.TensorDesc(Hn, ub, {r: (bufs[r].ptr, geom[r][1], geom[r][0]) for r in bufs}, 4, 0)
+    st = Streams()
+    rep = etp.etp_reshard_params(ctx, [desc], [plan], st.copy.cuda_stream, st.reload.cuda_stream)
+    st.sync()
+    assert rep["d2d_bytes"] == stats["d2d_bytes"] and rep["h2d_bytes"] == 0
+    assert rep["n_phases"] >= 2 if tight else rep["n_phases"] == 1
+    for r, b in bufs.items():
+        assert b.guards_intact()
+        assert np.array_equal(b.payload(), expect[r]), f"rank {r}: slab differs from the oracle image"
+
+
 # ------------------------------------------------------------------------------------------------ interval copy (5b)
 @pytest.mark.parametrize("n,hi", [(0, 1 << 20), (1, 1 << 20), (300, 4 << 20), (20000, 8 << 10)])
 @pytest.mark.parametrize("tma_min", [None, 16, 1 << 62])

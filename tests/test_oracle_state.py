@@ -271,3 +271,55 @@ def test_decode16_exact():
         got = OL.decode16(t.view(torch.uint8).numpy(), name)
         assert np.array_equal(got, t.to(torch.float64).numpy())
     assert OL.max_rel_err(np.array([1.0, 2.0]), np.array([1.0, 2.01])) == pytest.approx(0.01 / 2.01)
+
+
+# ------------------------------------------------------------------------------------------ MoE reference (reading G5)
+def test_moe_route_hand_worked():
+    """softmax / top-k / renormalisation on a case small enough to do by hand: logits (0, ln 2, ln 4, ln 1) -> p = (1, 2, 4, 1)/8;
+    top-2 = experts 2 and 1 with weights 4/6 and 2/6; the tie between experts 0 and 3 goes to the lower index (top-3)."""
+    import math
+    lg = np.array([[0.0, math.log(2.0), math.log(4.0), 0.0]])
+    idx, w = OL.moe_route(lg, 2)
+    assert idx.tolist() == [[2, 1]]
+    np.testing.assert_allclose(w, [[4 / 6, 2 / 6]], rtol=1e-14)
+    idx, w = OL.moe_route(lg, 3)
+    assert idx.tolist() == [[2, 1, 0]]
+    np.testing.assert_allclose(w, [[4 / 7, 2 / 7, 1 / 7]], rtol=1e-14)
+    # shift invariance of softmax and weights summing to one
+    idx2, w2 = OL.moe_route(lg + 123.0, 3)
+    assert idx2.tolist() == idx.tolist()
+    np.testing.assert_allclose(w2, w, rtol=1e-12)
+
+
+def test_moe_ref_special_cases():
+    import math
+    rng = np.random.default_rng(7)
+    T, Hd, F, E = 5, 6, 4, 3
+    x = rng.standard_normal((T, Hd))
+    gate, up, down_t = (rng.standard_normal((E, F, Hd)) for _ in range(3))
+    lg = rng.standard_normal((T, E))
+    # (i) one expert, top-1: the layer is a dense SwiGLU MLP, written out with scalar loops
+    y = OL.moe_ref(x, lg[:, :1], gate[:1], up[:1], down_t[:1], 1)
+    for t in range(T):
+        for o in range(Hd):
+            acc = 0.0
+            for f in range(F):
+                g = sum(gate[0, f, k] * x[t, k] for k in range(Hd))
+                u = sum(up[0, f, k] * x[t, k] for k in range(Hd))
+                acc += g / (1.0 + math.exp(-g)) * u * down_t[0, f, o]
+            assert y[t, o] == pytest.approx(acc, rel=1e-12, abs=1e-12)
+    # (ii) identical experts: the renormalised weights sum to one, so any routing gives the single-expert output
+    same = lambda a: np.repeat(a[:1], E, axis=0)
+    np.testing.assert_allclose(OL.moe_ref(x, lg, same(gate), same(up), same(down_t), 2), y, rtol=1e-12, atol=1e-12)
+    # (iii) renaming the experts (and the logit columns with them) changes nothing
+    perm = np.array([2, 0, 1])
+    np.testing.assert_allclose(OL.moe_ref(x, lg[:, perm], gate[perm], up[perm], down_t[perm], 2),
+                               OL.moe_ref(x, lg, gate, up, down_t, 2), rtol=1e-12, atol=1e-12)
+    # (iv) top_k = E with equal logits: the plain average of all experts
+    avg = sum(OL.moe_ref(x, lg[:, :1], gate[e:e + 1], up[e:e + 1], down_t[e:e + 1], 1) for e in range(E)) / E
+    np.testing.assert_allclose(OL.moe_ref(x, np.zeros((T, E)), gate, up, down_t, E), avg, rtol=1e-12, atol=1e-12)
+    # (v) a hugely dominant logit with top-1 picks exactly that expert
+    big = np.full((T, E), -50.0)
+    big[:, 1] = 50.0
+    np.testing.assert_allclose(OL.moe_ref(x, big, gate, up, down_t, 1),
+                               OL.moe_ref(x, lg[:, :1], gate[1:2], up[1:2], down_t[1:2], 1), rtol=1e-12, atol=1e-12)
