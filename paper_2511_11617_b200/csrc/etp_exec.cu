@@ -56,6 +56,7 @@ extern "C" etp_status etp_ctx_create(int device, int64_t staging_bytes, etp_ctx*
     c->opts[ETP_OPT_KV_RELOAD_MODE] = 0;
     c->opts[ETP_OPT_GRID_CTAS] = 0;
     c->opts[ETP_OPT_GATHER_CTAS] = 16;
+    c->opts[ETP_OPT_LINEAR_CTA_PAIR] = 1;
     c->staging_bytes = staging_bytes ? staging_bytes : (int64_t(256) << 20);
     CtxExtra* x = new (std::nothrow) CtxExtra();
     if (!x) { delete c; ETP_FAIL(ETP_ERR_NOMEM, "etp_ctx_create: out of memory"); }

@@ -348,6 +348,225 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
     }
 }
 
+// ------------------------------------------------------------------------------------------------ CTA-pair kernel
+// Large token counts (BN = 256): two CTAs of a cluster (one TPC) run ONE tcgen05.mma.cta_group::2 of M = 256 out features x
+// N = 256 tokens.  CTA rank c owns out-feature tile 2*pair + c (its own A tile and its own 128 TMEM lanes x 256 columns)
+// and stages HALF of the X tile (tokens t0 + 128*c ..), so every SM reads 16 + 16 KiB of shared memory per K chunk
+// instead of 16 + 32 KiB.  Only the leader (rank 0) issues MMAs; both CTAs issue TMA loads that complete on the
+// LEADER's full barrier; tcgen05.commit multicasts the "stage free" and "accumulator ready" arrivals to both CTAs; the
+// epilogue warps of both CTAs arrive on the leader's "accumulator drained" barrier.
+// PBN = tokens per pair tile (UMMA_N): 256, or 128 when that fills the 74 CTA pairs more evenly (host heuristic).
+template <int PBN>
+struct PairCfg {
+    static constexpr int kBBytes = (PBN / 2) * kBK * 2;   // this CTA's half of the X tile
+    static constexpr int kStageBytes = kABytes + kBBytes;
+    static constexpr int kStages = kSmemBudget / kStageBytes > 8 ? 8 : kSmemBudget / kStageBytes;
+    static constexpr int kTmemCols = 2 * PBN;             // two accumulator stages of PBN fp32 columns
+    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 + 256;
+};
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t mapa_rank0(uint32_t saddr) {   // the same shared-memory offset in CTA 0 of the cluster
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, 0;" : "=r"(r) : "r"(saddr));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tma_load_2d_pair(void* smem_dst, const CUtensorMap* map, uint32_t leader_bar, int32_t c0, int32_t c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+            smem_u32(smem_dst)),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(leader_bar), "r"(c0), "r"(c1)
+        : "memory");
+}
+__device__ __forceinline__ void tc_commit_pair(uint64_t* bar) {   // arrives on `bar` at the same offset in BOTH CTAs
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)),
+                 "h"(uint16_t(3))
+                 : "memory");
+}
+__device__ __forceinline__ void tc_mma_pair(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__host__ __device__ constexpr uint32_t make_idesc_pair(uint32_t fmt, uint32_t a_mn_major, uint32_t n) {
+    return (1u << 4) | (fmt << 7) | (fmt << 10) | (a_mn_major << 15) | ((n >> 3) << 17) | ((uint32_t(2 * kBM) >> 4) << 24);
+}
+
+// Items are (pair of m tiles, token tile); p.n_m_tiles counts PAIRS and runs[].first indexes pairs (column-parallel).
+template <int PBN, typename OutT>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_shard_linear_pair_kernel(const __grid_constant__ LinearParams p) {
+    constexpr int kPairBN = PBN, kPairStages = PairCfg<PBN>::kStages, kPairStageBytes = PairCfg<PBN>::kStageBytes;
+    constexpr int kPairTmemCols = PairCfg<PBN>::kTmemCols;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + kPairStages * kPairStageBytes);
+    uint64_t* empty_bar = full_bar + kPairStages;
+    uint64_t* tmem_full = empty_bar + kPairStages;
+    uint64_t* tmem_empty = tmem_full + 2;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
+    const int n_items = p.n_m_tiles * p.n_n_tiles;
+    const bool row_par = p.mode == ETP_ROW_PARALLEL;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kPairStages; ++s) {
+            mbar_init(&full_bar[s], 1);      // used in the leader only: its own arrive.expect_tx of both CTAs' bytes
+            mbar_init(&empty_bar[s], 1);     // one multicast commit per use
+        }
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&tmem_full[s], 1);     // one multicast commit per item
+            mbar_init(&tmem_empty[s], 8);    // leader only: 4 epilogue warps of each CTA
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {   // one warp of EACH CTA, same warp id, same destination offset
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_ptr)), "r"(uint32_t(kPairTmemCols))
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();      // the peer's barriers exist before anything signals them
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+
+    if (warp == 0) {
+        // ===================================================================== TMA producer (one lane of each CTA)
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int item = cluster_id; item < n_items; item += n_clusters) {
+                const int pn = item % p.n_n_tiles, pm = item / p.n_n_tiles;
+                const int t0 = pn * kPairBN + int(rank) * (kPairBN / 2);
+                int r = row_par ? 0 : find_run(p, pm);
+                const int row = row_par ? 0 : ((pm - p.runs[r].first) * 2 + int(rank)) * kBM;   // may lie past the run: zero-filled
+                const int m0 = (pm * 2 + int(rank)) * kBM;                                      // row-parallel: out features
+                for (int c = 0; c < p.n_chunks; ++c) {
+                    uint8_t* sa = smem + stage * kPairStageBytes;
+                    uint8_t* sb = sa + kABytes;
+                    mbar_wait(&empty_bar[stage], phase ^ 1);
+                    const uint32_t lbar = mapa_rank0(smem_u32(&full_bar[stage]));
+                    if (rank == 0) mbar_expect_tx(&full_bar[stage], 2 * kPairStageBytes);
+                    if (!row_par) {
+                        tma_load_2d_pair(sa, &p.map_w[r], lbar, c * kBK, row);
+                        tma_load_2d_pair(sb, &p.map_x, lbar, c * kBK, t0);
+                    } else {
+                        while (r + 1 < p.n_runs && p.runs[r + 1].first <= c) ++r;
+                        const int feat0 = int(p.runs[r].feat0);
+                        const int xk = (feat0 / kBK + (c - p.runs[r].first)) * kBK;
+                        const int kin = xk - feat0;
+                        tma_load_2d_pair(sa, &p.map_w[r], lbar, m0, kin);
+                        tma_load_2d_pair(sa + kABytes / 2, &p.map_w[r], lbar, m0 + 64, kin);
+                        tma_load_2d_pair(sb, &p.map_x, lbar, xk, t0);
+                    }
+                    if (++stage == kPairStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 1) {
+        // ===================================================================== MMA issuer (one lane of the LEADER)
+        if (lane == 0 && rank == 0) {
+            const bool a_mn = row_par;
+            const uint32_t idesc = make_idesc_pair(p.dtype == ETP_BF16 ? 1u : 0u, a_mn ? 1u : 0u, uint32_t(kPairBN));
+            const uint32_t a_lbo = a_mn ? uint32_t(kABytes / 2) : 16u;
+            const uint32_t a_kstep = a_mn ? (uint32_t(kUmmaK) * 128u) >> 4 : (uint32_t(kUmmaK) * 2u) >> 4;
+            int stage = 0;
+            uint32_t phase = 0;
+            int local = 0;
+            for (int item = cluster_id; item < n_items; item += n_clusters, ++local) {
+                const int as = local & 1;
+                const uint32_t aph = (local >> 1) & 1;
+                mbar_wait(&tmem_empty[as], aph ^ 1);   // both CTAs' epilogues have drained this accumulator stage
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + uint32_t(as * kPairBN);
+                for (int c = 0; c < p.n_chunks; ++c) {
+                    uint8_t* sa = smem + stage * kPairStageBytes;
+                    mbar_wait(&full_bar[stage], phase);
+                    tc_fence_after();
+                    const uint64_t a_desc = make_smem_desc(smem_u32(sa), a_lbo, 1024);
+                    const uint64_t b_desc = make_smem_desc(smem_u32(sa + kABytes), 16, 1024);
+#pragma unroll
+                    for (int k = 0; k < kBK / kUmmaK; ++k)
+                        tc_mma_pair(d_tmem, a_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > 0 || k > 0) ? 1u : 0u);
+                    tc_commit_pair(&empty_bar[stage]);   // frees the stage in BOTH CTAs once these MMAs have read it
+                    if (++stage == kPairStages) { stage = 0; phase ^= 1; }
+                }
+                tc_commit_pair(&tmem_full[as]);
+            }
+        }
+        __syncwarp();
+    } else {
+        // ===================================================================== epilogue warps 2..5 of both CTAs
+        const int q = warp & 3;
+        const int m_local = q * 32 + lane;
+        OutT* y = reinterpret_cast<OutT*>(p.y);
+        const uint32_t drained = mapa_rank0(smem_u32(&tmem_empty[0]));
+        int local = 0;
+        for (int item = cluster_id; item < n_items; item += n_clusters, ++local) {
+            const int pn = item % p.n_n_tiles, pm = item / p.n_n_tiles;
+            const int as = local & 1;
+            const uint32_t aph = (local >> 1) & 1;
+            const int t0 = pn * kPairBN;
+            const int n_tok = min(kPairBN, p.tokens - t0);
+            int64_t gm0;
+            int valid;
+            if (!row_par) {
+                const int r = find_run(p, pm);
+                const int row = ((pm - p.runs[r].first) * 2 + int(rank)) * kBM;
+                gm0 = p.runs[r].feat0 + row;
+                valid = min(kBM, p.runs[r].n_feat - row);
+            } else {
+                gm0 = int64_t(pm * 2 + int(rank)) * kBM;
+                valid = min(int64_t(kBM), int64_t(p.out_features) - gm0);
+            }
+            mbar_wait(&tmem_full[as], aph);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + uint32_t(as * kPairBN) + (uint32_t(q * 32) << 16);
+            for (int c16 = 0; c16 < n_tok; c16 += 16) {
+                uint32_t v[16];
+                tc_ld16(taddr + uint32_t(c16), v);
+                tc_ld_wait();
+                if (m_local < valid) {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j)
+                        if (c16 + j < n_tok) y[size_t(t0 + c16 + j) * p.out_features + gm0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(drained + uint32_t(as) * 8u);
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();      // the leader's MMAs read the peer's shared memory and both CTAs free the paired TMEM
+    if (warp == 1) {
+        __syncwarp();
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(uint32_t(kPairTmemCols)) : "memory");
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ host side
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -414,6 +633,23 @@ etp_status launch_linear(const LinearParams& p, int grid, cudaStream_t stream) {
     }
     e = cudaGetLastError();
     if (e != cudaSuccess) ETP_FAIL(ETP_ERR_CUDA, "etp_shard_linear: launch failed: %s", cudaGetErrorString(e));
+    return ETP_OK;
+}
+
+template <int PBN>
+etp_status launch_linear_pair(const LinearParams& p, int grid, cudaStream_t stream) {
+    constexpr int kPairSmemBytes = PairCfg<PBN>::kSmemBytes;
+    if (p.dtype == ETP_BF16) {
+        auto k = etp_shard_linear_pair_kernel<PBN, __nv_bfloat16>;
+        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmemBytes));
+        k<<<grid, kLinThreads, kPairSmemBytes, stream>>>(p);
+    } else {
+        auto k = etp_shard_linear_pair_kernel<PBN, __half>;
+        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmemBytes));
+        k<<<grid, kLinThreads, kPairSmemBytes, stream>>>(p);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) ETP_FAIL(ETP_ERR_CUDA, "etp_shard_linear: pair launch failed: %s", cudaGetErrorString(e));
     return ETP_OK;
 }
 
@@ -488,23 +724,46 @@ extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_d
 
     // ---- tiling
     const int bn = tokens <= 16 ? 16 : (tokens <= 64 ? 64 : 256);
+    // > 64 tokens: CTA pairs (256 out features x 256 tokens per pair) unless single-CTA 128 x 256 tiles need fewer rounds of
+    // the persistent grid (few, ragged m tiles: e.g. 1024 out features in runs of 384/384/256).  Per item a pair takes ~0.93
+    // of the single-CTA time (it stages 32 KiB instead of 48 KiB per K chunk and SM; measured on the config-2 shapes).
+    const int64_t pair_opt = ctx->opts[ETP_OPT_LINEAR_CTA_PAIR];
+    bool pair = bn == 256 && pair_opt != 0 && ctx->n_sms >= 2;
+    const int pbn = pair_opt == 128 ? 128 : 256;
+    if (pair && pair_opt == 1) {
+        int64_t mt_single = 0, mt_pair = 0;
+        if (row_par) {
+            mt_single = (out_features + kBM - 1) / kBM;
+            mt_pair = (out_features + 2 * kBM - 1) / (2 * kBM);
+        } else {
+            for (int r = 0; r < n_runs; ++r) {
+                mt_single += (p.runs[r].n_feat + kBM - 1) / kBM;
+                mt_pair += (p.runs[r].n_feat + 2 * kBM - 1) / (2 * kBM);
+            }
+        }
+        const int64_t tt = (tokens + 255) / 256, units = ctx->n_sms / 2;
+        const int64_t rounds_single = (mt_single * tt + ctx->n_sms - 1) / ctx->n_sms, rounds_pair = (mt_pair * tt + units - 1) / units;
+        pair = double(rounds_pair) * 0.93 <= double(rounds_single);
+    }
+    const int m_tile = pair ? 2 * kBM : kBM;
+    const int tile_n = pair ? pbn : bn;
     p.n_runs = n_runs;
     p.mode = mode;
     p.dtype = dtype;
     p.tokens = int32_t(tokens);
     p.in_features = int32_t(in_features);
     p.out_features = int32_t(out_features);
-    p.n_n_tiles = int32_t((tokens + bn - 1) / bn);
+    p.n_n_tiles = int32_t((tokens + tile_n - 1) / tile_n);
     p.y = y;
     int32_t acc = 0;
     for (int r = 0; r < n_runs; ++r) {
         p.runs[r].first = acc;
         if (row_par) acc += int32_t((p.runs[r].feat0 + p.runs[r].n_feat + kBK - 1) / kBK - p.runs[r].feat0 / kBK);   // 64-aligned global K chunks it touches
-        else acc += (p.runs[r].n_feat + kBM - 1) / kBM;
+        else acc += (p.runs[r].n_feat + m_tile - 1) / m_tile;
     }
     if (row_par) {
         p.n_chunks = acc;
-        p.n_m_tiles = int32_t((out_features + kBM - 1) / kBM);
+        p.n_m_tiles = int32_t((out_features + m_tile - 1) / m_tile);
     } else {
         p.n_m_tiles = acc;
         p.n_chunks = int32_t((in_features + kBK - 1) / kBK);
@@ -540,15 +799,19 @@ extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_d
     }
 
     // ---- tensor maps: X [tokens][in]; one map per run so that TMA zero-fills everything past a run's end
-    ETP_TRY(encode_2d(&p.map_x, dtype, x, tokens, in_features, in_features, kBK, bn));
+    ETP_TRY(encode_2d(&p.map_x, dtype, x, tokens, in_features, in_features, kBK, pair ? pbn / 2 : bn));
     for (int r = 0; r < n_runs; ++r) {
         if (row_par) ETP_TRY(encode_2d(&p.map_w[r], dtype, run_addr[r], p.runs[r].n_feat, out_features, out_features, 64, kBK));
         else ETP_TRY(encode_2d(&p.map_w[r], dtype, run_addr[r], p.runs[r].n_feat, in_features, in_features, kBK, kBM));
     }
 
-    const int grid = int(std::min<int64_t>(n_items, ctx->n_sms));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     ctx->launches = 1;
+    if (pair) {
+        const int pgrid = 2 * int(std::min<int64_t>(n_items, ctx->n_sms / 2));
+        return pbn == 128 ? launch_linear_pair<128>(p, pgrid, st) : launch_linear_pair<256>(p, pgrid, st);
+    }
+    const int grid = int(std::min<int64_t>(n_items, ctx->n_sms));
     if (bn == 16) return launch_linear<16>(p, grid, st);
     if (bn == 64) return launch_linear<64>(p, grid, st);
     return launch_linear<256>(p, grid, st);

@@ -93,7 +93,20 @@ CASES = [
     ("row", "bf16", 4, 5120, 5120, 640, (3, 3, 2), "tight"),               # Qwen3-14B wo_t
     ("col", "bf16", 512, 2048, 2304, 1, (768, 769, 767), "wrap"),          # several items per CTA (accumulator stages)
     ("row", "bf16", 512, 2307 + 5, 2048, 1, (770, 771, 771), "wrap"),
+    ("col", "bf16", 1000, 1024, 3000, 1, (1000, 1001, 999), "wrap"),       # CTA pairs: odd m-tile counts per run, 4 token tiles
+    ("row", "bf16", 700, 3000, 1000, 1, (1000, 1001, 999), "wrap"),        # CTA pairs: out = 3.9 pair tiles, ragged tokens
 ]
+
+
+@pytest.mark.parametrize("mode,dtype,T,K,N,fpu,widths,gmode", [c for c in CASES if c[2] > 64])
+def test_shard_linear_forced_tile_modes_at_large_T(ctx, mode, dtype, T, K, N, fpu, widths, gmode):
+    """> 64 tokens: CTA pairs (cta_group::2) with 256- and 128-token tiles and the single-CTA 128 x 256 path, each forced."""
+    for forced in (0, 256, 128):            # 1 (default) picks pairs or single tiles by rounds of the persistent grid
+        ctx.set_option(etp.OPT_LINEAR_CTA_PAIR, forced)
+        try:
+            test_shard_linear_matches_unsharded_reference(ctx, mode, dtype, T, K, N, fpu, widths, gmode)
+        finally:
+            ctx.set_option(etp.OPT_LINEAR_CTA_PAIR, 1)
 
 
 @pytest.mark.parametrize("mode,dtype,T,K,N,fpu,widths,gmode", CASES)
