@@ -464,6 +464,17 @@ def run_ours(args):
         d_kms, d_bytes, d_kl = (sum(dacc[k][i] for k in dacc) for i in range(3))
     finally:
         ctx.set_option(etp.OPT_SKIP_RELOAD, 0)
+    # SURVEY.md 8(d) "overlap": the whole step with only the copy kernels (a), with only the reload pipeline (b), and with
+    # both (the e2e leg above); overlap = t_both / max(t_a, t_b), 1.0 = the device copies are fully hidden under the reload
+    alone = {}
+    for name, opt in (("a_only_ms", etp.OPT_SKIP_RELOAD), ("b_only_ms", etp.OPT_SKIP_D2D)):
+        ctx.set_option(opt, 1)
+        try:
+            one_step("pinned")
+            alone[name] = sum(one_step("pinned")[0] for _ in range(K)) / K
+        finally:
+            ctx.set_option(opt, 0)
+    overlap = {"both_ms": e_ms / K, **alone, "ratio": (e_ms / K) / max(alone.values())}
     lin = None
     if state.specs and cfg.model.ffn and not args.no_linear:
         lin = shard_linear_leg(state, ctx, dev, hbm_peak)
@@ -490,7 +501,7 @@ def run_ours(args):
                    "l2": "inputs larger than L2 (every step re-reads and re-writes GBs; plans are hazard-free so a step is idempotent in place)",
                    "replicas": world, "step": "S1 partition + S2 CMM plan + S3 lowering + S4 copy + S5 reload + S6 page table, synchronised per step"},
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": e_h2d // K, "d2h_bytes_per_step": 0,
-                "ms_per_step": e_ms / K, "h2d_GBps": e_h2d / (e_ms * 1e-3) / 1e9,
+                "ms_per_step": e_ms / K, "h2d_GBps": e_h2d / (e_ms * 1e-3) / 1e9, "overlap": overlap,
                 "note": "reload sources in pinned host memory; result stays on the device (the page table is host-side)"},
         "gpu_launches": launches + kl + e_launches + d_kl + (lin["launches"] if lin else 0),
         "shard_linear": lin,
