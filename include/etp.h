@@ -107,7 +107,12 @@ typedef struct { int32_t kind; int32_t src_rank /* -1 for RELOAD */; int32_t dst
                  int64_t begin, end; } etp_task;
 typedef struct { int64_t total_units, keep_units, transfer_units, reload_units,
                  reload_lower_bound /* Eq. 1 */, n_tasks; } etp_plan_stats;
-typedef enum { ETP_PLAN_CMM = 0, ETP_PLAN_GREEDY = 1, ETP_PLAN_FULL_RELOAD = 2 } etp_plan_mode;
+typedef enum { ETP_PLAN_CMM = 0, ETP_PLAN_GREEDY = 1, ETP_PLAN_FULL_RELOAD = 2,
+               ETP_PLAN_MIGRATION_AWARE = 3 /* Algorithm 1 with the owner of every target (and, when target_bounds is NULL,
+                  the placement of the ceil(H/M)-wide shards) chosen to minimise the transferred units at the same minimal
+                  reload volume; ties -> lexicographically smallest (bounds, owner ranks).  An extension (PAPER.md:160, :247:
+                  the paper minimises reload only).  <= 10 alive ranks, else ETP_ERR_UNSUPPORTED.  The new layout is in
+                  target order, not rank order. */ } etp_plan_mode;
 
 /* Host-only.  old_layout: n_old entries (host), distinct rank ids, arbitrary intervals.  target_bounds: M+1 bounds
  * tiling [0,H), H = max end over ALL entries, or NULL for the floor formula.  Target j is owned by the j-th alive
@@ -115,7 +120,8 @@ typedef enum { ETP_PLAN_CMM = 0, ETP_PLAN_GREEDY = 1, ETP_PLAN_FULL_RELOAD = 2 }
  * library: release with etp_plan_free. */
 etp_status etp_cmm_plan(const etp_shard* old_layout, int32_t n_old, const int64_t* target_bounds, int32_t M,
                         etp_plan** out);
-/* same with the comparison planners of PAPER.md:204 / Table II (Greedy: no P2P for gaps; Full Reload: no reuse) */
+/* same with the comparison planners of PAPER.md:204 / Table II (Greedy: no P2P for gaps; Full Reload: no reuse) and the
+ * migration-aware extension */
 etp_status etp_plan_create(etp_plan_mode mode, const etp_shard* old_layout, int32_t n_old,
                            const int64_t* target_bounds, int32_t M, etp_plan** out);
 /* copies up to cap tasks into out (host); *n_out = total number of tasks (call with cap = 0 to size) */

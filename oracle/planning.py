@@ -80,9 +80,11 @@ def _subtract(rest: List[Tuple[int, int]], a: int, b: int) -> List[Tuple[int, in
     return out
 
 
-def cmm_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None
-             ) -> Tuple[List[Task], List[Shard]]:
-    """Algorithm 1 with readings C1-C7.  Returns (tasks sorted by (dst, begin), new layout)."""
+def cmm_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None,
+             owners: Optional[Sequence[int]] = None) -> Tuple[List[Task], List[Shard]]:
+    """Algorithm 1 with readings C1-C7.  Returns (tasks sorted by (dst, begin), new layout).
+    ``owners`` (reading M1, not in the paper): owners[j] = the alive rank that will hold target j, instead of the
+    j-th alive rank of reading C3."""
     old = [tuple(int(v) for v in s) for s in old_layout]
     if not old:
         raise ValueError("empty layout")
@@ -100,6 +102,11 @@ def cmm_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequen
         raise ValueError("duplicate rank id")
     if M > len(G) or M < 1:
         raise ValueError("M must be in 1..#alive (reading C6)")
+    if owners is not None:
+        G = [int(r) for r in owners]
+        alive_ids = {r for (r, _, _, a) in old if a}
+        if len(G) != M or len(set(G)) != M or any(r not in alive_ids for r in G):
+            raise ValueError("owners must be M distinct alive ranks")
     alive_sorted = sorted((s for s in old if s[3]), key=lambda s: s[0])
     tasks: List[Task] = []
     for j in range(M):                                                   # l.6
@@ -118,6 +125,52 @@ def cmm_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequen
     tasks.sort(key=lambda t: (t[2], t[3]))
     new_layout = [(G[j], tb[j], tb[j + 1], 1) for j in range(M)]
     return tasks, new_layout
+
+
+MAX_ALIVE_MIGRATION_AWARE = 10
+
+
+def width_arrangements(H: int, M: int) -> List[List[int]]:
+    """Every bounds vector whose widths are floor(H/M) or ceil(H/M) (PAPER.md:94 fixes the widths, not which ranks are
+    wide), in lexicographic order."""
+    import itertools
+    q, r = divmod(H, M)
+    out = []
+    for wide in itertools.combinations(range(M), r):
+        b = [0]
+        for j in range(M):
+            b.append(b[-1] + q + (1 if j in wide else 0))
+        out.append(b)
+    return sorted(out)
+
+
+def migration_aware_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None):
+    """SURVEY.md 8(f) #2 / DESIGN.md reading M1 (an extension; PAPER.md:160 makes only the reload volume minimal and
+    :247/:257 leave transfer cost to future work).  Plain definition by exhaustion: over every admissible bounds vector
+    (all placements of the wide shards, or the given bounds) and every injective assignment of targets to alive ranks,
+    run Algorithm 1 with those owners and take the lexicographic minimum of
+        (reload units, transfer units, bounds vector, owners vector).
+    Returns (tasks, new layout) like cmm_plan."""
+    import itertools
+    old = [tuple(int(v) for v in s) for s in old_layout]
+    H = max(e for (_, _, e, _) in old)
+    alive = sorted(r for (r, _, _, a) in old if a)
+    if M < 1 or M > len(alive):
+        raise ValueError("M must be in 1..#alive (reading C6)")
+    if len(alive) > MAX_ALIVE_MIGRATION_AWARE:
+        raise ValueError("migration-aware search is limited to 10 alive ranks")
+    if target_bounds is None and H < M:
+        raise ValueError("fewer units than shards")
+    cands = [list(int(x) for x in target_bounds)] if target_bounds is not None else width_arrangements(H, M)
+    best = None
+    for tb in cands:
+        for owners in itertools.permutations(alive, M):
+            tasks, new = cmm_plan(old, M, tb, owners)
+            st = plan_stats(tasks)
+            key = (st["reload_units"], st["transfer_units"], tuple(tb), tuple(owners))
+            if best is None or key < best[0]:
+                best = (key, tasks, new)
+    return best[1], best[2]
 
 
 def greedy_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None):

@@ -16,7 +16,7 @@ STATUS = {0: "OK", 1: "INVALID_ARG", 2: "ALIGNMENT", 3: "CAPACITY", 4: "NO_SOURC
 KEEP, TRANSFER, RELOAD = 0, 1, 2
 SPLIT = {"floor": 0, "ceil_first": 1}
 GRAN = {"head": 0, "ffn": 1, "expert": 2, "vocab": 3}
-PLAN_CMM, PLAN_GREEDY, PLAN_FULL_RELOAD = 0, 1, 2
+PLAN_CMM, PLAN_GREEDY, PLAN_FULL_RELOAD, PLAN_MIGRATION_AWARE = 0, 1, 2, 3
 COL_PARALLEL, ROW_PARALLEL = 0, 1
 DTYPE = {"bf16": 0, "fp16": 1}
 KV_TOKEN_MAJOR, KV_HEAD_MAJOR = 0, 1

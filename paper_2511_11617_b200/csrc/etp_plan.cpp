@@ -100,6 +100,72 @@ void finish_stats(etp_plan* p, const std::vector<int64_t>& tb) {
     st.reload_lower_bound = p->total_units - reuse;
     p->stats = st;
 }
+
+// ETP_PLAN_MIGRATION_AWARE (reading M1; an extension, PAPER.md:160 minimises only the reload volume and :247/:257
+// leave transfer cost to future work).  The reload volume does not depend on who owns what, so minimising the transferred
+// units means maximising the KEPT units  sum_j |target_j  n  old interval of owner(j)|  over injective owner choices and,
+// when the bounds are free, over every placement of the ceil(H/M)-wide shards.  Assignment by dynamic programming over
+// subsets of alive ranks (f[mask] = best keep of targets popcount(mask).. with the ranks in mask taken); ties go to the
+// lexicographically smallest (bounds, owners) - bounds vectors are visited in lexicographic order and an equal score never
+// replaces the incumbent; the owners are rebuilt front to back taking the smallest rank that still reaches f.
+constexpr int kMaxAliveMigrationAware = 10;
+
+int64_t best_owners(const std::vector<etp_shard>& alive, const std::vector<int64_t>& tb, int M, std::vector<int>* owners) {
+    const int n = (int)alive.size();
+    auto keep = [&](int j, int i) {
+        return std::max<int64_t>(0, std::min(tb[j + 1], alive[i].end) - std::max(tb[j], alive[i].begin));
+    };
+    std::vector<int64_t> f(size_t(1) << n, -1);
+    for (int64_t mask = (int64_t(1) << n) - 1; mask >= 0; --mask) {
+        const int j = __builtin_popcountll((unsigned long long)mask);
+        if (j > M) continue;
+        if (j == M) { f[mask] = 0; continue; }
+        int64_t best = -1;
+        for (int i = 0; i < n; ++i)
+            if (!(mask >> i & 1) && f[mask | (int64_t(1) << i)] >= 0) best = std::max(best, keep(j, i) + f[mask | (int64_t(1) << i)]);
+        f[mask] = best;
+    }
+    owners->assign(M, 0);
+    int64_t mask = 0;
+    for (int j = 0; j < M; ++j)
+        for (int i = 0; i < n; ++i)
+            if (!(mask >> i & 1) && f[mask | (int64_t(1) << i)] >= 0 && keep(j, i) + f[mask | (int64_t(1) << i)] == f[mask]) {
+                (*owners)[j] = i;
+                mask |= int64_t(1) << i;
+                break;
+            }
+    return f[0];
+}
+
+etp_status choose_layout(const std::vector<etp_shard>& alive, int64_t H, int M, bool bounds_fixed, std::vector<int64_t>* tb,
+                         std::vector<int>* owner_idx) {
+    if ((int)alive.size() > kMaxAliveMigrationAware)
+        ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_plan_create: the migration-aware search is limited to %d alive ranks", kMaxAliveMigrationAware);
+    if (bounds_fixed) {
+        best_owners(alive, *tb, M, owner_idx);
+        return ETP_OK;
+    }
+    if (H < M) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_plan_create: %lld units over %d shards needs replication", (long long)H, M);
+    const int64_t q = H / M;
+    const int r = int(H % M);
+    // width vectors with exactly r wide shards in lexicographic order (narrow before wide at the first difference)
+    std::vector<int> wide(M, 0);
+    for (int j = M - r; j < M; ++j) wide[j] = 1;   // lexicographically smallest: the wide shards last
+    int64_t best_keep = -1;
+    std::vector<int64_t> cand(M + 1);
+    std::vector<int> own;
+    do {
+        cand[0] = 0;
+        for (int j = 0; j < M; ++j) cand[j + 1] = cand[j] + q + wide[j];
+        const int64_t k = best_owners(alive, cand, M, &own);
+        if (k > best_keep) {
+            best_keep = k;
+            *tb = cand;
+            *owner_idx = own;
+        }
+    } while (std::next_permutation(wide.begin(), wide.end()));
+    return ETP_OK;
+}
 }  // namespace
 
 extern "C" etp_status etp_plan_create(etp_plan_mode mode, const etp_shard* old_layout, int32_t n_old,
@@ -107,7 +173,7 @@ extern "C" etp_status etp_plan_create(etp_plan_mode mode, const etp_shard* old_l
     if (!out) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_create: out is NULL");
     *out = nullptr;
     if (!old_layout || n_old < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_create: empty old layout");
-    if (mode != ETP_PLAN_CMM && mode != ETP_PLAN_GREEDY && mode != ETP_PLAN_FULL_RELOAD)
+    if (mode != ETP_PLAN_CMM && mode != ETP_PLAN_GREEDY && mode != ETP_PLAN_FULL_RELOAD && mode != ETP_PLAN_MIGRATION_AWARE)
         ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_create: unknown mode %d", (int)mode);
     int64_t H = 0;
     std::set<int32_t> seen;
@@ -136,20 +202,26 @@ extern "C" etp_status etp_plan_create(etp_plan_mode mode, const etp_shard* old_l
         for (int32_t j = 0; j <= M; ++j) tb[j] = (int64_t(j) * H) / M;  // Alg. 1 l.2-5
     }
 
+    // owner_idx[j] = index into `alive` of the rank that holds target j.  Reading C3: the j-th alive rank in ascending id.
+    std::vector<int> owner_idx(M);
+    for (int32_t j = 0; j < M; ++j) owner_idx[j] = j;
+    if (mode == ETP_PLAN_MIGRATION_AWARE) ETP_TRY(choose_layout(alive, H, M, target_bounds != nullptr, &tb, &owner_idx));
+
     etp_plan* p = new (std::nothrow) etp_plan();
     if (!p) ETP_FAIL(ETP_ERR_NOMEM, "etp_plan_create: out of memory");
     p->mode = mode;
     p->total_units = H;
     p->old_layout.assign(old_layout, old_layout + n_old);
     for (int32_t j = 0; j < M; ++j) {
-        const int32_t owner = alive[j].rank;  // reading C3: j-th alive rank in ascending id owns target j
+        const etp_shard& own = alive[owner_idx[j]];
+        const int32_t owner = own.rank;
         p->new_layout.push_back({owner, 1, tb[j], tb[j + 1]});
         std::vector<Span> open;
         if (tb[j] < tb[j + 1]) open.push_back({tb[j], tb[j + 1]});
         if (mode != ETP_PLAN_FULL_RELOAD) {
             // sources in the order of reading C7: the owner itself, then ascending rank id
             std::vector<const etp_shard*> order;
-            order.push_back(&alive[j]);
+            order.push_back(&own);
             for (const etp_shard& s : alive)
                 if (s.rank != owner) order.push_back(&s);
             for (const etp_shard* s : order) {

@@ -306,6 +306,68 @@ def test_scale_up_a_repaired_rank_joins(ctx, tight):
         assert np.array_equal(b.payload(), expect[r]), f"rank {r}: slab differs from the oracle image"
 
 
+# ------------------------------------------------------------------------------------------------ migration-aware plan
+@pytest.mark.parametrize("slabs_mode", ["span", "full"])
+def test_migration_aware_plan_reshard_and_linear(ctx, slabs_mode):
+    """Reading M1: config 5a's second failure in miniature - 7 ranks of 200 units, rank 0 dies, 6 targets.
+    The migration-aware plan permutes the owners (the new layout is not in rank order) and transfers fewer units than
+    Algorithm 1's in-order owners; the reshard is bit-exact to the oracle applying the oracle's own migration-aware plan, and
+    the column-parallel linear on the permuted layout still matches the unsharded reference."""
+    from oracle import linear as OL
+    from oracle import planning as OP
+    K = 1032                                             # in-features; unit = one out-feature row
+    Hn, ub = 1400, K * 2
+    ranks = [0, 1, 2, 3, 4, 6, 7]
+    old = [(r, 200 * i, 200 * (i + 1), 0 if r == 0 else 1) for i, r in enumerate(ranks)]
+    tasks, new = OP.migration_aware_plan(old, 6)
+    base = OP.plan_stats(OP.cmm_plan(old, 6)[0])
+    st = OP.plan_stats(tasks)
+    assert st["reload_units"] == base["reload_units"] == 200 and st["transfer_units"] < base["transfer_units"]
+    assert [r for (r, _, _, _) in new] != sorted(r for (r, _, _, _) in new)
+    plan = etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, old, 6)
+    assert plan.tasks() == tasks and plan.new_layout() == new
+    geom = {}
+    for (r, b, e, a) in old:
+        if not a:
+            continue
+        if slabs_mode == "full":
+            geom[r] = (0, Hn)
+        else:
+            first, span = plan.slab_span(r)
+            geom[r] = (first, span)
+    from workloads.gen import as_u8, fill_normal16
+    w = as_u8(fill_normal16(77, 1, 0, Hn * K, 0.02, torch.bfloat16)).copy()
+    rng = np.random.default_rng(3)
+    slabs = {}
+    for (r, b, e, a) in old:
+        if a:
+            slab = np.full(geom[r][1] * ub, 0xFF, dtype=np.uint8)      # NaN patterns outside the shard
+            OS.place_units(slab, *geom[r], ub, b, e, w)
+            slabs[r] = slab
+    expect, stats = OS.apply_params(tasks, slabs, geom, ub, w, 0)
+    for (r, b, e, _) in new:
+        assert np.array_equal(OS.read_units(expect[r], *geom[r], ub, b, e), w[b * ub:e * ub])
+    bufs = {r: DevBuf(a) for r, a in slabs.items()}
+    image = pinned(w)
+    desc = etp.TensorDesc(Hn, ub, {r: (bufs[r].ptr, geom[r][1], geom[r][0]) for r in bufs}, 8, 0, image.data_ptr(), 0, Hn)
+    s = Streams()
+    rep = etp.etp_reshard_params(ctx, [desc], [plan], s.copy.cuda_stream, s.reload.cuda_stream)
+    s.sync()
+    assert rep["d2d_bytes"] == stats["d2d_bytes"] == st["transfer_units"] * ub and rep["h2d_bytes"] == 200 * ub
+    for r, b in bufs.items():
+        assert b.guards_intact()
+        assert np.array_equal(b.payload(), expect[r]), f"rank {r}: slab differs from the oracle image"
+    # S7 on the permuted layout
+    T = 4
+    x = as_u8(fill_normal16(77, 2, 0, T * K, 1.0, torch.bfloat16)).copy()
+    xb, yb = DevBuf(x), DevBuf(np.full(T * Hn * 2, 0xEE, dtype=np.uint8))
+    etp.etp_shard_linear(ctx, etp.COL_PARALLEL, "bf16", xb.ptr, T, K, Hn, desc, new, 1, yb.ptr)
+    torch.cuda.synchronize()
+    y = OL.decode16(yb.payload(), "bf16").reshape(T, Hn)
+    ref = OL.linear_ref(OL.decode16(x, "bf16").reshape(T, K), OL.decode16(w, "bf16").reshape(Hn, K))
+    assert np.isfinite(y).all() and OL.max_rel_err(y, ref) <= 5e-3
+
+
 # ------------------------------------------------------------------------------------------------ interval copy (5b)
 @pytest.mark.parametrize("n,hi", [(0, 1 << 20), (1, 1 << 20), (300, 4 << 20), (20000, 8 << 10)])
 @pytest.mark.parametrize("tma_min", [None, 16, 1 << 62])

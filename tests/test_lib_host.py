@@ -117,6 +117,35 @@ def test_comparison_planners_match_oracle():
         assert pc.stats()["reload_units"] <= pg.stats()["reload_units"] <= pf.stats()["reload_units"]
 
 
+def test_migration_aware_planner_matches_oracle():
+    """Reading M1: the library's subset-DP assignment against the oracle's exhaustive search, task for task (ties included),
+    with free bounds (all placements of the wide shards) and with fixed bounds; never more transfers than Algorithm 1's
+    in-order owners, the same (minimal) reload."""
+    rng = np.random.default_rng(29)
+    gained = 0
+    for it in range(150):
+        old = random_layout(rng)
+        n_alive = sum(a for (_, _, _, a) in old)
+        M = int(rng.integers(1, n_alive + 1))
+        Ht = max(e for (_, _, e, _) in old)
+        if Ht < M or M > 5:
+            continue
+        tb = OP.partition(Ht, M, "ceil_first") if it % 3 == 0 else None
+        tasks, new = OP.migration_aware_plan(old, M, tb)
+        p = etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, old, M, tb)
+        assert p.new_layout() == new
+        assert p.tasks() == tasks
+        base = etp.etp_cmm_plan(old, M, tb).stats()
+        st = p.stats()
+        assert st["reload_units"] == base["reload_units"] == st["reload_lower_bound"]
+        assert st["transfer_units"] <= base["transfer_units"]
+        gained += st["transfer_units"] < base["transfer_units"]
+    assert gained > 10
+    with pytest.raises(etp.EtpError) as e:      # search limited to 10 alive ranks
+        etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, [(r, r, r + 1, 1) for r in range(11)], 11)
+    assert e.value.status == 5
+
+
 def test_replicated_sources_reading_c7():
     old = [(0, 0, 6, 1), (1, 4, 10, 1), (2, 8, 12, 0)]
     tasks, new = OP.cmm_plan(old, 2)

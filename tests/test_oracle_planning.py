@@ -192,6 +192,62 @@ def test_in_order_ownership_is_not_always_transfer_minimal():
     assert all(c[0] == 1 for c in best.values())      # reload minimum is permutation-independent (Eq. 1)
 
 
+def test_migration_aware_plan_against_unit_level_bruteforce():
+    """Reading M1: the search over owners and wide-shard placements reaches exactly the minimum that
+    oracle/bruteforce.py finds by enumerating a source for every single unit under every owner permutation and every
+    bounds vector with widths in {floor, ceil} - no intervals, no Algorithm 1 on that side."""
+    import itertools
+    from oracle.planning import migration_aware_plan, width_arrangements
+    rng = random.Random(17)
+    improved = n_checked = 0
+    for _ in range(60):
+        n = rng.randint(2, 4)
+        H = rng.randint(n, 8)
+        cuts = sorted(rng.sample(range(1, H), n - 1))
+        lay = layout_from_bounds([0] + cuts + [H])
+        dead = set(rng.sample(range(n), 1))
+        old = [(r, s, e, 0 if r in dead else 1) for (r, s, e, _) in lay]
+        M = n - 1
+        if H < M:
+            continue
+        tasks, new = migration_aware_plan(old, M)
+        check_invariants(old, M, tasks, new)
+        st = plan_stats(tasks)
+        got = (st["reload_units"], st["transfer_units"])
+        # every bounds vector the definition admits: q/q+1 widths, sum H
+        arrs = width_arrangements(H, M)
+        q, r = divmod(H, M)
+        assert len(arrs) == len(set(map(tuple, arrs))) == len(list(itertools.combinations(range(M), r)))
+        assert all(b[0] == 0 and b[-1] == H and all(b[j + 1] - b[j] in (q, q + 1) for j in range(M)) for b in arrs)
+        brute = min(min(bruteforce.best_over_owner_permutations(old, tb).values()) for tb in arrs)
+        assert got == brute
+        base = plan_stats(cmm_plan(old, M)[0])
+        assert got[0] == base["reload_units"] and got[1] <= base["transfer_units"]
+        improved += got[1] < base["transfer_units"]
+        n_checked += 1
+    assert n_checked > 40 and improved > 5
+
+
+def test_migration_aware_plan_worked_example_and_ties():
+    from oracle.planning import migration_aware_plan
+    # the C11 example: N=4, H=4, rank 0 dead.  In-order floor bounds 0/1/2/4 transfer 2 units; with the bounds fixed the best
+    # owners transfer 1; letting the wide shard go first (0/2/3/4) every survivor keeps its unit and rank 1 reloads unit 0.
+    old = [(0, 0, 1, 0), (1, 1, 2, 1), (2, 2, 3, 1), (3, 3, 4, 1)]
+    tasks, new = migration_aware_plan(old, 3, partition(4, 3))
+    assert plan_stats(tasks)["transfer_units"] == 1
+    tasks, new = migration_aware_plan(old, 3)
+    assert new == [(1, 0, 2, 1), (2, 2, 3, 1), (3, 3, 4, 1)]
+    assert tasks == [(RELOAD, -1, 1, 0, 1), (KEEP, 1, 1, 1, 2), (KEEP, 2, 2, 2, 3), (KEEP, 3, 3, 3, 4)]
+    # nothing to gain: an intact formula layout keeps everything and the tie goes to the smallest (bounds, owners)
+    lay = layout_from_bounds(partition(10, 3))
+    tasks, new = migration_aware_plan(lay, 3)
+    assert new == lay and all(k == KEEP for (k, _, _, _, _) in tasks)
+    # fixed bounds: only the owners move
+    old = [(0, 0, 4, 1), (1, 4, 8, 0), (2, 8, 12, 1), (3, 12, 16, 1)]
+    tasks, new = migration_aware_plan(old, 3, [0, 5, 11, 16])
+    assert [b for (_, b, _, _) in new] == [0, 5, 11]
+
+
 def test_table2_ordering_in_units():
     """PAPER.md:204 / Table II: reload(Full) >= reload(Greedy) >= reload(CM); P2P only in CM."""
     rng = random.Random(3)
