@@ -226,6 +226,20 @@ etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype,
                             const etp_tensor* w, const etp_shard* layout, int32_t n_shards,
                             int64_t features_per_unit, void* y, void* stream);
 
+/* ------------------------------------------------------------------------------------------------ grouped MoE linear
+ * SURVEY.md 8(f) #3, reading G5; PAPER.md:172-174 (experts are the unit of the expert-granularity plan).  One
+ * launch computes, for every expert e,  Y_perm[r][:] = X_perm[r][:] . W_e^T  for its routed rows r in
+ * [row_offsets[e], row_offsets[e+1]) on the expert matrices where the reshard left them.  w: total_units = n_experts, one
+ * unit = one expert matrix of in_features x out_features 16-bit elements (unit_bytes = in x out x 2):
+ *   ETP_COL_PARALLEL: stored [out][in] (gate, up);  ETP_ROW_PARALLEL: stored transposed [in][out] (down), in % 64 == 0.
+ * x_perm [n_rows][in_features], y_perm [n_rows][out_features]: device, 16-B aligned, row-major, rows grouped by expert in
+ * ascending expert id; row_offsets: HOST array of n_experts + 1 non-decreasing offsets starting at 0.  Routing, activation
+ * and the weighted combine are the caller's.  fp32 accumulation, one rounding to 16 bit.  Asynchronous on `stream`; calls
+ * on one ctx must not overlap in time (ctx-owned work-item table). */
+etp_status etp_moe_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x_perm,
+                          const int64_t* row_offsets, int32_t n_experts, int64_t in_features, int64_t out_features,
+                          const etp_tensor* w, const etp_shard* layout, int32_t n_shards, void* y_perm, void* stream);
+
 /* ------------------------------------------------------------------------------------------------ microbenchmark entry
  * Copies n arbitrary intervals with the same persistent kernel (config 5b).  host_descs: host array; src/dst: device,
  * 16-B aligned; bytes: multiple of 16.  Destinations must be mutually disjoint and disjoint from every source. */

@@ -77,7 +77,7 @@ class etp_interval(C.Structure):
 EXPORTS = ["etp_ctx_create", "etp_ctx_destroy", "etp_last_error", "etp_version", "etp_ctx_set_option", "etp_ctx_get_option",
            "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_tasks", "etp_plan_new_layout",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
-           "etp_copy_intervals"]
+           "etp_moe_linear", "etp_copy_intervals"]
 
 _lib = None
 
@@ -112,6 +112,8 @@ def lib() -> C.CDLL:
                                      vp, vp, C.POINTER(etp_reshard_report)]
         L.etp_shard_linear.argtypes = [vp, C.c_int, C.c_int, vp, i64, i64, i64, C.POINTER(etp_tensor), C.POINTER(etp_shard), i32, i64,
                                        vp, vp]
+        L.etp_moe_linear.argtypes = [vp, C.c_int, C.c_int, vp, C.POINTER(i64), i32, i64, i64, C.POINTER(etp_tensor), C.POINTER(etp_shard),
+                                     i32, vp, vp]
         L.etp_copy_intervals.argtypes = [vp, C.POINTER(etp_interval), i64, vp, C.POINTER(etp_reshard_report)]
         _lib = L
     return _lib
@@ -327,6 +329,17 @@ def etp_shard_linear(ctx: Context, mode: int, dtype: str, x_ptr: int, tokens: in
     arr, keep = _marshal_tensors([w])
     _check(lib().etp_shard_linear(ctx.handle, mode, DTYPE[dtype], x_ptr, tokens, in_features, out_features, arr, _shards(layout),
                                   len(layout), features_per_unit, y_ptr, stream or None))
+    del keep
+
+
+def etp_moe_linear(ctx: Context, mode: int, dtype: str, x_ptr: int, row_offsets: Sequence[int], in_features: int, out_features: int,
+                   w: TensorDesc, layout: Sequence[Shard], y_ptr: int, stream: int = 0) -> None:
+    """row_offsets: n_experts + 1 host offsets into the expert-grouped rows of x / y."""
+    arr, keep = _marshal_tensors([w])
+    n = len(row_offsets) - 1
+    offs = (i64 * (n + 1))(*[int(v) for v in row_offsets])
+    _check(lib().etp_moe_linear(ctx.handle, mode, DTYPE[dtype], x_ptr, offs, n, in_features, out_features, arr, _shards(layout),
+                                len(layout), y_ptr, stream or None))
     del keep
 
 

@@ -99,6 +99,7 @@ extern "C" void etp_ctx_destroy(etp_ctx* c) {
     if (c->d_staging) cudaFree(c->d_staging);
     if (c->lin_ws) cudaFree(c->lin_ws);
     if (c->lin_tickets) cudaFree(c->lin_tickets);
+    if (c->moe_items) cudaFree(c->moe_items);
     cudaGetLastError();
     delete c;
 }

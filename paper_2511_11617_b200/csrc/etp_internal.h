@@ -132,6 +132,8 @@ struct etp_ctx {
     int64_t lin_ws_bytes = 0;
     unsigned int* lin_tickets = nullptr; // per-tile arrival tickets of the split-K reduction (zero between launches)
     int64_t lin_tickets_n = 0;
+    void* moe_items = nullptr;          // work-item table of etp_moe_linear (device), grown on demand
+    int64_t moe_items_bytes = 0;
 };
 
 namespace etp {

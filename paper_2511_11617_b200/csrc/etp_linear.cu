@@ -20,27 +20,17 @@
 // stores, or fp32 split-K partials + ticketed last-arriver reduction in fixed split order, so results are deterministic).
 // Persistent grid, static round-robin over (m tile, token tile, k split) items; two TMEM accumulator stages so the epilogue
 // of item i overlaps the MMAs of item i+1.
-#include <cuda.h>
-#include <cuda_bf16.h>
-#include <cuda_fp16.h>
 
 #include <algorithm>
 #include <cstring>
 #include <vector>
 
-#include "etp_internal.h"
+#include "etp_tc.cuh"
 
 using namespace etp;
+using namespace etp::tc;
 
 namespace {
-
-constexpr int kBM = 128;          // out features per tile = UMMA_M
-constexpr int kBK = 64;           // K elements per pipeline stage: 128 bytes = one 128B-swizzle atom
-constexpr int kUmmaK = 16;        // K per tcgen05.mma for 16-bit inputs
-constexpr int kMaxRuns = 16;      // <= 2 contiguous runs per rank, 8 ranks
-constexpr int kLinThreads = 192;  // 6 warps
-constexpr int kABytes = kBM * kBK * 2;
-constexpr int kSmemBudget = 200 << 10;
 
 struct Run {          // one contiguous slot range of a rank's shard, runs sorted by global feature
     int64_t feat0;    // first global feature of the run (out-feature: column-parallel, in-feature: row-parallel)
@@ -59,74 +49,6 @@ struct alignas(64) LinearParams {
     float* partials;          // split-K workspace [(tile * n_splits + split)][BN][128]
     unsigned int* tickets;    // one per output tile, zero between launches (the last arriver resets its ticket)
 };
-
-// ------------------------------------------------------------------------------------------------ PTX wrappers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\t"
-        "bra WAIT_%=;\n\t"
-        "DONE_%=:\n\t"
-        "}" ::"r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int32_t c0, int32_t c1) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
-            smem_u32(smem_dst)),
-        "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
-        : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint64_t* bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
-        "}" ::"r"(d_tmem),
-        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-__device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&v)[16]) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
-          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-        : "r"(taddr)
-        : "memory");
-}
-__device__ __forceinline__ void tc_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// Shared-memory matrix descriptor (tcgen05 "smem descriptor"): start address, leading / stride byte offsets (all >> 4),
-// descriptor version 1 (Blackwell) at bit 46, layout type SWIZZLE_128B (= 2) at bits 61-63.
-__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-    return uint64_t((saddr & 0x3FFFFu) >> 4) | (uint64_t(lbo_bytes >> 4) << 16) | (uint64_t(sbo_bytes >> 4) << 32) |
-           (uint64_t(1) << 46) | (uint64_t(2) << 61);
-}
-// Instruction descriptor of kind::f16: D = fp32 (bits 4-5 = 1), A/B format (0 = fp16, 1 = bf16) at bits 7-9 / 10-12,
-// A/B major (0 = K, 1 = MN) at bits 15 / 16, N >> 3 at bits 17-22, M >> 4 at bits 24-28.
-__host__ __device__ constexpr uint32_t make_idesc(uint32_t fmt, uint32_t a_mn_major, uint32_t n) {
-    return (1u << 4) | (fmt << 7) | (fmt << 10) | (a_mn_major << 15) | ((n >> 3) << 17) | ((uint32_t(kBM) >> 4) << 24);
-}
 
 template <int BN>
 struct Cfg {
@@ -155,13 +77,6 @@ __device__ __forceinline__ int find_run(const LinearParams& p, int key) {   // l
     while (r + 1 < p.n_runs && p.runs[r + 1].first <= key) ++r;
     return r;
 }
-template <typename T>
-__device__ __forceinline__ T cvt16(float v);
-template <>
-__device__ __forceinline__ __nv_bfloat16 cvt16<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
-template <>
-__device__ __forceinline__ __half cvt16<__half>(float v) { return __float2half_rn(v); }
-
 // ------------------------------------------------------------------------------------------------ the kernel
 template <int BN, typename OutT>
 __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const __grid_constant__ LinearParams p) {
@@ -568,42 +483,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
 }
 
 // ------------------------------------------------------------------------------------------------ host side
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_tiled_fn() {
-    static EncodeTiledFn fn = [] {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) {
-            cudaGetLastError();
-            p = nullptr;
-        }
-        return reinterpret_cast<EncodeTiledFn>(p);
-    }();
-    return fn;
-}
-
-// 2-D row-major 16-bit tensor [rows][cols] at `base`, box {box_cols (= 64 elements = 128 B), box_rows}, 128B swizzle,
-// out-of-bounds elements read as zero.
-etp_status encode_2d(CUtensorMap* map, etp_dtype dtype, const void* base, int64_t rows, int64_t cols, int64_t pitch_elems,
-                     int box_cols, int box_rows) {
-    EncodeTiledFn fn = encode_tiled_fn();
-    if (!fn) ETP_FAIL(ETP_ERR_CUDA, "etp_shard_linear: cuTensorMapEncodeTiled is not available from the driver");
-    cuuint64_t dims[2] = {cuuint64_t(cols), cuuint64_t(rows)};
-    cuuint64_t strides[1] = {cuuint64_t(pitch_elems) * 2};
-    cuuint32_t box[2] = {cuuint32_t(box_cols), cuuint32_t(box_rows)};
-    cuuint32_t estr[2] = {1, 1};
-    CUresult r = fn(map, dtype == ETP_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
-                    const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS)
-        ETP_FAIL(ETP_ERR_CUDA, "etp_shard_linear: cuTensorMapEncodeTiled failed (%d) for [%lld][%lld] pitch %lld box {%d,%d}", int(r),
-                 (long long)rows, (long long)cols, (long long)pitch_elems, box_cols, box_rows);
-    return ETP_OK;
-}
-
 // Number of K splits: a function of the nominal shapes only (never of the shard layout), so a column-parallel output is
 // bit-identical before and after a reshard (G3).  Splitting only pays when few output tiles exist (small T).
 int choose_splits(int64_t nominal_tiles, int nominal_chunks, int n_sms, int bn) {

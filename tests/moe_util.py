@@ -64,3 +64,32 @@ def check_against_oracle(y, order, wts, x_f64, logits_f64, gate, up, down_t, top
     err = OL.max_rel_err(got, ref)
     assert err <= tol, f"MoE layer output: max relative error {err:.3e} > {tol}"
     return err
+
+
+def moe_layer_grouped(ctx, dtype: str, x: torch.Tensor, logits: torch.Tensor, top_k: int, ffn: int, descs, layout):
+    """Same layer through etp_moe_linear: the (token, expert) pairs are sorted by expert, then ONE grouped
+    launch each for gate, up and down on the whole expert tensors.  descs = {"gate"|"up"|"down_t": TensorDesc of the expert
+    tensor (one unit = one expert)}, layout = the expert class's shards.  Returns (y fp32, order, weights, per-expert rows)."""
+    T, hidden = x.shape
+    dt = x.dtype
+    E = logits.shape[1]
+    order, wts = route(logits, top_k)
+    flat_e = order.reshape(-1)
+    perm = torch.argsort(flat_e, stable=True)                     # grouped by expert, token order kept inside a group
+    tok = (perm // top_k)
+    counts = torch.bincount(flat_e, minlength=E).cpu().numpy()
+    offs = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    R = int(offs[-1])
+    xp = x[tok].contiguous()
+    g = torch.full((R, ffn), float("nan"), dtype=dt, device=x.device)
+    u = torch.full((R, ffn), float("nan"), dtype=dt, device=x.device)
+    etp.etp_moe_linear(ctx, etp.COL_PARALLEL, dtype, xp.data_ptr(), offs, hidden, ffn, descs["gate"], layout, g.data_ptr())
+    etp.etp_moe_linear(ctx, etp.COL_PARALLEL, dtype, xp.data_ptr(), offs, hidden, ffn, descs["up"], layout, u.data_ptr())
+    h = (torch.nn.functional.silu(g.float()) * u.float()).to(dt).contiguous()
+    yp = torch.full((R, hidden), float("nan"), dtype=dt, device=x.device)
+    etp.etp_moe_linear(ctx, etp.ROW_PARALLEL, dtype, h.data_ptr(), offs, ffn, hidden, descs["down_t"], layout, yp.data_ptr())
+    torch.cuda.synchronize()
+    w_flat = wts.reshape(-1)[perm].float()
+    y = torch.zeros(T, hidden, dtype=torch.float32, device=x.device)
+    y.index_add_(0, tok, w_flat[:, None] * yp.float())
+    return y, order.cpu().numpy(), wts.cpu().numpy(), counts, (g, u, yp, tok, flat_e[perm])

@@ -282,9 +282,26 @@ def check_moe_layer(ctx, state, step_idx, layer, tokens=16):
             w = fill_normal16(state.seed, self.sp.stream, e * F * Hd, F * Hd, m.init_std, state.dt, device=state.device)
             return OL.decode16(as_u8(w), dtn).reshape(F, Hd)
 
-    return MU.check_against_oracle(y, order, wts, OL.decode16(as_u8(x), dtn).reshape(tokens, Hd),
-                                   OL.decode16(as_u8(logits), dtn).reshape(tokens, E), Unsharded(spec["gate"]),
-                                   Unsharded(spec["up"]), Unsharded(spec["down_t"]), m.top_k)
+    err = MU.check_against_oracle(y, order, wts, OL.decode16(as_u8(x), dtn).reshape(tokens, Hd),
+                                  OL.decode16(as_u8(logits), dtn).reshape(tokens, E), Unsharded(spec["gate"]),
+                                  Unsharded(spec["up"]), Unsharded(spec["down_t"]), m.top_k)
+    # the grouped kernel (etp_moe_linear) at a serving-size batch: 2048 tokens x top-8 = 16384 routed rows over 128 experts,
+    # three launches; 8 sampled tokens against the oracle (a token's output depends on no other token)
+    T2 = 2048
+    x2 = fill_normal16(state.seed, 9500 + layer, 0, T2 * Hd, 1.0, state.dt, device=state.device).view(T2, Hd)
+    lg2 = fill_normal16(state.seed, 9600 + layer, 0, T2 * E, 1.0, state.dt, device=state.device).view(T2, E)
+    descs = {}
+    for kind, sp in spec.items():
+        slabs = {r: (state.slabs[sp.name][r].data_ptr(), state.geom["expert"][r][1], state.geom["expert"][r][0]) for (r, _, _, _) in new}
+        descs[kind] = etp.TensorDesc(E, sp.unit_bytes, slabs, state.n_ranks, 0)
+    y2, order2, wts2, counts, _ = MU.moe_layer_grouped(ctx, dtn, x2, lg2, m.top_k, F, descs, new)
+    assert counts.sum() == T2 * m.top_k and torch.isfinite(y2).all()
+    pick = np.unique(np.concatenate([[0, T2 - 1], np.random.default_rng(layer).integers(0, T2, 6)]))
+    pk = torch.from_numpy(pick).to(state.device)
+    MU.check_against_oracle(y2[pk], order2[pick], wts2[pick], OL.decode16(as_u8(x2[pk]), dtn).reshape(len(pick), Hd),
+                            OL.decode16(as_u8(lg2[pk]), dtn).reshape(len(pick), E), Unsharded(spec["gate"]),
+                            Unsharded(spec["up"]), Unsharded(spec["down_t"]), m.top_k)
+    return err
 
 
 # ------------------------------------------------------------------------------------------------ the tests

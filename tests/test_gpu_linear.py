@@ -230,9 +230,62 @@ def test_moe_layer_on_resharded_experts(ctx):
     y, order, wts, calls = MU.moe_layer_per_expert(ctx, shape.dtype, x, logits, shape.top_k, F, locate)
     assert calls == 3 * len(np.unique(order))
     mats = {k: OL.decode16(world.unsharded[n], shape.dtype).reshape(E, F, Hd) for k, n in names.items()}
-    MU.check_against_oracle(y, order, wts, OL.decode16(as_u8(x.cpu()), shape.dtype).reshape(T, Hd),
-                            OL.decode16(as_u8(logits.cpu()), shape.dtype).reshape(T, E), mats["gate"], mats["up"], mats["down_t"],
-                            shape.top_k)
+    x64 = OL.decode16(as_u8(x.cpu()), shape.dtype).reshape(T, Hd)
+    lg64 = OL.decode16(as_u8(logits.cpu()), shape.dtype).reshape(T, E)
+    MU.check_against_oracle(y, order, wts, x64, lg64, mats["gate"], mats["up"], mats["down_t"], shape.top_k)
+    # the grouped kernel (etp_moe_linear): one launch per projection over all experts, same oracle, and bitwise the same
+    # 16-bit projections as the per-expert calls would give is NOT required - only the tolerance is
+    n_ranks = 4
+    descs = {k: etp.TensorDesc(E, F * Hd * 2, {r: (bufs[n][r].ptr, world.geom[n][r][1], world.geom[n][r][0]) for (r, _, _, _) in new},
+                               n_ranks, 0) for k, n in names.items()}
+    y2, order2, wts2, counts, (g, u, yp, tok, exp_of_row) = MU.moe_layer_grouped(ctx, shape.dtype, x, logits, shape.top_k, F, descs, new)
+    assert counts.sum() == T * shape.top_k and np.array_equal(order2, order)
+    MU.check_against_oracle(y2, order2, wts2, x64, lg64, mats["gate"], mats["up"], mats["down_t"], shape.top_k)
+    # every grouped projection row by row against the unsharded expert matrix (reading G4: each linear on its own)
+    gg = OL.decode16(as_u8(g.cpu()), shape.dtype).reshape(-1, F)
+    tok_h, exp_h = tok.cpu().numpy(), exp_of_row.cpu().numpy()
+    ref_g = np.stack([mats["gate"][e] @ x64[t] for t, e in zip(tok_h, exp_h)])
+    assert np.isfinite(gg).all() and OL.max_rel_err(gg, ref_g) <= TOL
+    assert all(b.guards_intact() for n in names.values() for b in bufs[n].values())
+
+
+@pytest.mark.parametrize("T,E,F,Hd,top_k,widths,gmode", [
+    (4, 8, 128, 256, 2, (3, 3, 2), "tight"),          # a few rows per expert: 16-row tiles, experts without rows
+    (300, 6, 192, 320, 3, (2, 1, 3), "wrap"),         # F not a multiple of 128 (a tile runs into the next expert's rows), wrapped shards
+    (1500, 5, 256, 136, 2, (5,), "tight"),            # > 256 rows per expert: several row tiles; K tail (136 = 2 chunks + 8)
+])
+def test_moe_linear_grouped_vs_reference(ctx, T, E, F, Hd, top_k, widths, gmode):
+    """etp_moe_linear on synthetic expert tensors (NaN-filled slack slots): every row of the column-parallel (gate-like) and
+    row-parallel (down-like) grouped outputs against the fp64 product with ITS expert's unsharded matrix."""
+    dt = torch_dtype("bf16")
+    rng = np.random.default_rng(T + E)
+    layout = widths_to_layout(widths)
+    geom = {}
+    for (r, b, e, _) in layout:
+        if gmode == "tight":
+            geom[r] = (b, e - b)
+        else:
+            cap = (e - b) + 1 + r
+            geom[r] = (b - (cap - (e - b) // 2) % cap, cap)
+    ub = F * Hd * 2
+    assign = np.sort(rng.integers(0, E, T * top_k)) if T > 4 else np.array([1, 1, 1, 4, 4, 6, 6, 6])
+    counts = np.bincount(assign, minlength=E)
+    offs = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    R = int(offs[-1])
+    for mode, (K, N) in ((etp.COL_PARALLEL, (Hd, F)), (etp.ROW_PARALLEL, (F, Hd))):
+        w_u8 = as_u8(fill_normal16(SEED, 760 + mode, 0, E * F * Hd, 0.02, dt)).copy()
+        x_u8 = as_u8(fill_normal16(SEED, 770 + mode, 0, R * K, 1.0, dt)).copy()
+        slabs = shard_into_slabs(w_u8, ub, layout, geom)
+        bufs = {r: DevBuf(a) for r, a in slabs.items()}
+        desc = etp.TensorDesc(E, ub, {r: (bufs[r].ptr, geom[r][1], geom[r][0]) for r in bufs}, len(widths), 0)
+        xb, yb = DevBuf(x_u8), DevBuf(np.full(R * N * 2, 0xEE, dtype=np.uint8))
+        etp.etp_moe_linear(ctx, mode, "bf16", xb.ptr, offs, K, N, desc, layout, yb.ptr)
+        torch.cuda.synchronize()
+        assert xb.guards_intact() and yb.guards_intact() and all(b.guards_intact() for b in bufs.values())
+        x64 = OL.decode16(x_u8, "bf16").reshape(R, K)
+        w64 = OL.decode16(w_u8, "bf16").reshape(E, F, Hd)        # col: [E][out=F][in=Hd]; row: [E][in=F][out=Hd]
+        ref = np.stack([(w64[e] @ x64[r]) if mode == etp.COL_PARALLEL else (x64[r] @ w64[e]) for r, e in enumerate(assign)])
+        check(yb.payload(), ref, "bf16", R, N)
 
 
 def test_shard_linear_argument_errors(ctx):
