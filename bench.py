@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--seqs", type=int, default=0, help="debug: fewer sequences (marks the result as reduced)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--microbench", action="store_true", help="config 5b: copy-kernel microbenchmark over synthetic plans")
+    ap.add_argument("--moe", action="store_true", help="config 4: grouped MoE shard linear (etp_moe_linear) on the resharded experts")
     ap.add_argument("--no-linear", action="store_true", help="skip the S7 (shard linear) leg")
     ap.add_argument("--linear-only", action="store_true", help="only the S7 leg, on parameters alone (for ncu captures of kernel (c))")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0, help="CPU seconds of oracle work in the cpu_baseline leg")
@@ -324,6 +325,78 @@ def run_microbench(args):
     return 0
 
 
+def run_moe(args):
+    """Config 4 (Qwen3-30B-A3B shape, 24 layers): the parameters are resharded 4 -> 3 (experts 42/43/43), then the three
+    expert projections of a layer run through etp_moe_linear (one grouped launch each) on the NEW layout, layers cycling so
+    the expert matrices are never L2-resident.  Routing: seeded N(0,1) logits, top-8 (torch, outside the timed region).
+    T = 64 tokens (512 routed rows: a weight stream over the experts that were hit) and T = 4096 (32768 rows)."""
+    import numpy as np
+    import torch
+    import paper_2511_11617_b200 as etp
+    from paper_2511_11617_b200.state import ModelState
+    from workloads import get_config
+    from workloads.configs import scaled
+    from workloads.gen import fill_normal16
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    hbm_peak, peak_src = load_peaks()
+    cfg = get_config("4")
+    if args.layers:
+        cfg = scaled(cfg, n_layers=args.layers)
+    m = cfg.model
+    ctx = etp.Context(0)
+    state = ModelState(cfg, device=dev, image="device", with_kv=False)
+    cs, rs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+    state.reshard(ctx, 0, "device", cs.cuda_stream, rs.cuda_stream, replan=True)
+    cs.synchronize(), rs.synchronize()
+    new = state.steps[0].new["expert"]
+    E, F, Hd, k = m.n_experts, m.expert_ffn, m.hidden, m.top_k
+    kinds = {"exp_gate": (etp.COL_PARALLEL, Hd, F), "exp_up": (etp.COL_PARALLEL, Hd, F), "exp_down_t": (etp.ROW_PARALLEL, F, Hd)}
+    descs = {}
+    for l in range(m.n_layers):
+        for kind in kinds:
+            sp = next(s for s in state.specs if s.name == f"l{l}.{kind}")
+            slabs = {r: (state.slabs[sp.name][r].data_ptr(), state.geom["expert"][r][1], state.geom["expert"][r][0]) for (r, _, _, _) in new}
+            descs[(l, kind)] = etp.TensorDesc(E, sp.unit_bytes, slabs, state.n_ranks, 0)
+    st = torch.cuda.Stream(dev)
+    flush = torch.zeros(64 << 20, dtype=torch.int32, device=dev)
+    out = {"moe": f"config 4: etp_moe_linear on the resharded experts {[e - b for (_, b, e, _) in new]}", "peak": hbm_peak,
+           "peak_source": peak_src, "launches": 0}
+    for T in (64, 4096):
+        logits = fill_normal16(state.seed, 9700 + T, 0, T * E, 1.0, state.dt, device=dev).view(T, E)
+        order = torch.argsort(-torch.softmax(logits.double(), 1), dim=1, stable=True)[:, :k]
+        counts = torch.bincount(order.reshape(-1), minlength=E).cpu().numpy()
+        offs = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+        R, hit = int(offs[-1]), int((counts > 0).sum())
+        per, tot_ms, tot_flop, tot_bytes = {}, 0.0, 0.0, 0.0
+        for kind, (mode, K, N) in kinds.items():
+            x = fill_normal16(state.seed, 9800 + T, 0, R * K, 1.0, state.dt, device=dev)
+            y = torch.empty(R * N, dtype=state.dt, device=dev)
+            seq = [(l % m.n_layers) for l in range(-3, m.n_layers)]
+            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in seq]
+            with torch.cuda.stream(st):
+                for (e0, e1), l in zip(evs, seq):
+                    for _ in range(3):
+                        flush.sum()
+                    e0.record(st)
+                    etp.etp_moe_linear(ctx, mode, m.dtype, x.data_ptr(), offs, K, N, descs[(l, kind)], new, y.data_ptr(), st.cuda_stream)
+                    e1.record(st)
+            st.synchronize()
+            ms = sorted(a.elapsed_time(b) for a, b in evs[3:])
+            med = ms[len(ms) // 2]
+            flop, byts = 2.0 * R * K * N, 2.0 * hit * K * N + 2.0 * R * (K + N)
+            per[kind] = {"K": K, "N": N, "us": round(med * 1e3, 2), "TFLOPs": round(flop / med / 1e9, 1), "GBps": round(byts / med / 1e6, 1)}
+            tot_ms, tot_flop, tot_bytes = tot_ms + med, tot_flop + flop, tot_bytes + byts
+            out["launches"] += len(evs)
+        out[f"T{T}"] = {"routed_rows": R, "experts_hit": hit, "rows_per_expert_max": int(counts.max()), "layer_us": round(tot_ms * 1e3, 1),
+                        "TFLOPs": round(tot_flop / tot_ms / 1e9, 1), "GBps": round(tot_bytes / tot_ms / 1e6, 1),
+                        "hbm_frac": round(tot_bytes / tot_ms / 1e6 / hbm_peak, 4), "per_projection": per,
+                        "bytes": "2KN per expert hit + 2R(K+N)"}
+    print(json.dumps(out))
+    ctx.close()
+    return 0
+
+
 # ================================================================================================ multi-rank plumbing
 def max_over_ranks(ms: float, world: int, device) -> float:
     """Replicas only: every rank times its own replica; the job's time is the MAX over ranks."""
@@ -530,4 +603,6 @@ if __name__ == "__main__":
     a = parse_args()
     if a.microbench:
         sys.exit(run_microbench(a))
+    if a.moe:
+        sys.exit(run_moe(a))
     sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))

@@ -263,17 +263,16 @@ extern "C" etp_status etp_moe_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dty
     for (const RunInfo& r : runs)
         if (r.n * rows_per_expert >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: run too long");
 
-    // ---- row tile: the candidate that wastes the fewest accumulator columns over the ragged expert sizes (larger on ties)
+    // ---- row tile BN: operand fetch into the SM bounds a tile (measured on kernel (c): 48 KiB per K chunk at BN = 256 is the
+    // limit, the MMA is not), so an item costs (A tile + BN rows of X) bytes per K chunk; take the BN with the least total.
     int bn = 16;
     {
         int64_t best = INT64_MAX;
         for (int cand : {256, 128, 64, 16}) {
-            int64_t cols = 0;
-            for (int32_t e = 0; e < n_experts; ++e) {
-                const int64_t c = row_offsets[e + 1] - row_offsets[e];
-                cols += (c + cand - 1) / cand * std::max(cand, 32);   // an MMA narrower than 32 columns costs as much as 32
-            }
-            if (cols < best) { best = cols; bn = cand; }
+            int64_t tiles = 0;
+            for (int32_t e = 0; e < n_experts; ++e) tiles += (row_offsets[e + 1] - row_offsets[e] + cand - 1) / cand;
+            const int64_t cost = tiles * (kABytes + int64_t(cand) * kBK * 2);
+            if (cost < best) { best = cost; bn = cand; }
         }
     }
 
