@@ -56,7 +56,7 @@ struct Cfg {
     static constexpr int kStageBytes = kABytes + kBBytes;
     static constexpr int kStages = (kSmemBudget / kStageBytes) > 12 ? 12 : (kSmemBudget / kStageBytes);
     static constexpr int kTmemCols = (2 * BN) < 32 ? 32 : 2 * BN;   // two accumulator stages; a power of two >= 32
-    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */ + kStageTileBytes /* epilogue transpose */;
 };
 
 struct Item {
@@ -191,6 +191,8 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
         const int q = warp & 3;                 // a warp may only touch TMEM lanes 32*(warp % 4) .. +31
         const int m_local = q * 32 + lane;
         OutT* y = reinterpret_cast<OutT*>(p.y);
+        OutT* stage_t = reinterpret_cast<OutT*>(smem + C::kStages * C::kStageBytes + 256);
+        const bool vec_out = (p.out_features & 7) == 0;     // 16-byte epilogue stores need 16-byte aligned Y rows
         int local = 0;
         for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++local) {
             const Item it = decode_item(p, item);
@@ -217,7 +219,9 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
                 uint32_t v[16];
                 tc_ld16(taddr + uint32_t(c16), v);
                 tc_ld_wait();
-                if (p.n_splits == 1) {
+                if (p.n_splits == 1 && vec_out) {
+                    store_block16(stage_t, v, m_local, y, size_t(t0 + c16), min(16, n_tok - c16), p.out_features, gm0, valid);
+                } else if (p.n_splits == 1) {
                     if (m_local < valid) {
 #pragma unroll
                         for (int j = 0; j < 16; ++j)
@@ -277,7 +281,7 @@ struct PairCfg {
     static constexpr int kStageBytes = kABytes + kBBytes;
     static constexpr int kStages = kSmemBudget / kStageBytes > 8 ? 8 : kSmemBudget / kStageBytes;
     static constexpr int kTmemCols = 2 * PBN;             // two accumulator stages of PBN fp32 columns
-    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 + 256;
+    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 + 256 + kStageTileBytes;
 };
 
 __device__ __forceinline__ uint32_t cluster_ctarank() {
@@ -436,6 +440,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
         const int m_local = q * 32 + lane;
         OutT* y = reinterpret_cast<OutT*>(p.y);
         const uint32_t drained = mapa_rank0(smem_u32(&tmem_empty[0]));
+        OutT* stage_t = reinterpret_cast<OutT*>(smem + kPairStages * kPairStageBytes + 256);
+        const bool vec_out = (p.out_features & 7) == 0;
         int local = 0;
         for (int item = cluster_id; item < n_items; item += n_clusters, ++local) {
             const int pn = item % p.n_n_tiles, pm = item / p.n_n_tiles;
@@ -461,7 +467,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
                 uint32_t v[16];
                 tc_ld16(taddr + uint32_t(c16), v);
                 tc_ld_wait();
-                if (m_local < valid) {
+                if (vec_out) {
+                    store_block16(stage_t, v, m_local, y, size_t(t0 + c16), min(16, n_tok - c16), p.out_features, gm0, valid);
+                } else if (m_local < valid) {
 #pragma unroll
                     for (int j = 0; j < 16; ++j)
                         if (c16 + j < n_tok) y[size_t(t0 + c16 + j) * p.out_features + gm0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));

@@ -45,7 +45,7 @@ struct MoeCfg {
     static constexpr int kStageBytes = kABytes + kBBytes;
     static constexpr int kStages = (kSmemBudget / kStageBytes) > 12 ? 12 : (kSmemBudget / kStageBytes);
     static constexpr int kTmemCols = (2 * BN) < 32 ? 32 : 2 * BN;
-    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 + 256;
+    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 + 256 + 4096;   // + per-warp epilogue transpose buffers
 };
 
 __device__ __forceinline__ MoeItem load_item(const MoeItem* items, int i) {
@@ -147,8 +147,8 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
         __syncwarp();
     } else {               // ---------------------------------------------------------------------- epilogue warps 2..5
         const int q = warp & 3;
-        const int m_local = q * 32 + lane;
         OutT* y = reinterpret_cast<OutT*>(p.y);
+        OutT* stage_t = reinterpret_cast<OutT*>(smem + C::kStages * C::kStageBytes + 256) + q * 512;   // [16 rows][32 features]
         int local = 0;
         for (int i = blockIdx.x; i < p.n_items; i += gridDim.x, ++local) {
             const MoeItem it = load_item(p.items, i);
@@ -157,15 +157,31 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
             mbar_wait(&tmem_full[as], aph);
             tc_fence_after();
             const uint32_t taddr = tmem_base + uint32_t(as * BN) + (uint32_t(q * 32) << 16);
-            for (int c16 = 0; c16 < it.n_rows; c16 += 16) {
-                uint32_t v[16];
-                tc_ld16(taddr + uint32_t(c16), v);
-                tc_ld_wait();
-                if (m_local < it.valid) {
+            // up to 64 accumulator columns per tcgen05.wait::ld (four loads in flight hide the TMEM read latency); every 16
+            // columns go through a 1-KiB per-warp transpose buffer so that the global stores are 16 bytes per lane (8 routed
+            // rows x 64 contiguous bytes per instruction) instead of 2 - m0 and out_features are multiples of 8 by contract.
+            for (int c64 = 0; c64 < it.n_rows; c64 += 64) {
+                uint32_t v[4][16];
 #pragma unroll
-                    for (int j = 0; j < 16; ++j)
-                        if (c16 + j < it.n_rows)
-                            y[size_t(it.x_row + c16 + j) * p.out_features + it.m0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
+                for (int g = 0; g < 4; ++g)
+                    if (BN >= 16 * (g + 1) && c64 + 16 * g < it.n_rows) tc_ld16(taddr + uint32_t(c64 + 16 * g), v[g]);
+                tc_ld_wait();
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                    if (BN >= 16 * (g + 1) && c64 + 16 * g < it.n_rows) {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) stage_t[j * 32 + lane] = cvt16<OutT>(__uint_as_float(v[g][j]));
+                        __syncwarp();
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const int row = h * 8 + (lane >> 2), chunk = lane & 3;
+                            const int tok = c64 + 16 * g + row;
+                            const uint4 val = *reinterpret_cast<const uint4*>(stage_t + row * 32 + chunk * 8);
+                            if (tok < it.n_rows && q * 32 + chunk * 8 < it.valid)
+                                *reinterpret_cast<uint4*>(y + size_t(it.x_row + tok) * p.out_features + it.m0 + q * 32 + chunk * 8) = val;
+                        }
+                        __syncwarp();
+                    }
                 }
             }
             tc_fence_before();

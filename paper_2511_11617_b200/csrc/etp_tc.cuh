@@ -95,6 +95,39 @@ template <>
 __device__ __forceinline__ __half cvt16<__half>(float v) { return __float2half_rn(v); }
 
 
+// Epilogue store of one [128 out features][16 tokens] fp32 block held by the four epilogue warps (thread = out feature
+// m_local = 32 * (warp % 4) + lane, v[j] = token j) into row-major Y[token][out_features] as 16-BYTE stores.  The block is
+// transposed through a [16][kStagePitch] 16-bit shared buffer written at column (gm0 mod 8) + m_local, so that column c of the
+// buffer is global feature (gm0 - gm0 mod 8) + c and every aligned 8-element chunk of the buffer is an aligned 16-byte chunk
+// of Y (out_features % 8 == 0 required); the <= 2 ragged chunks of a row fall back to 2-byte stores.  128 threads, named
+// barrier 1.  `valid` may be <= 0 (nothing stored).
+constexpr int kStagePitch = kBM + 8;                       // elements
+constexpr int kStageTileBytes = 16 * kStagePitch * 2 + 256;  // rounded up
+template <typename OutT>
+__device__ __forceinline__ void store_block16(OutT* stage, const uint32_t (&v)[16], int m_local, OutT* y, size_t row0, int n_tok,
+                                              int64_t out_features, int64_t gm0, int valid) {
+    const int a = int(gm0 & 7);
+#pragma unroll
+    for (int j = 0; j < 16; ++j) stage[j * kStagePitch + a + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+    constexpr int kChunks = kStagePitch / 8;               // 17
+    for (int id = m_local; id < 16 * kChunks; id += 128) {
+        const int row = id / kChunks, ch = id - row * kChunks;
+        if (row >= n_tok) break;
+        const int c0 = ch * 8 - a;                         // feature of the chunk's first element, relative to gm0
+        OutT* dst = y + (row0 + size_t(row)) * size_t(out_features) + gm0 + c0;
+        const OutT* src = stage + row * kStagePitch + ch * 8;
+        if (c0 >= 0 && c0 + 8 <= valid) {
+            *reinterpret_cast<uint4*>(dst) = *reinterpret_cast<const uint4*>(src);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 8; ++e)
+                if (c0 + e >= 0 && c0 + e < valid) dst[e] = src[e];
+        }
+    }
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
