@@ -71,8 +71,9 @@ typedef enum {
                                     events (on that stream) so that etp_ctx_kernel_time can report device durations   */
     ETP_OPT_LINEAR_CTA_PAIR = 9, /* 1 (default): etp_shard_linear at > 64 tokens runs CTA pairs (tcgen05 cta_group::2,
                                     256 out features x 256 tokens per pair) unless single-CTA tiles need fewer rounds of
-                                    the persistent grid; 256 / 128: always pairs, with that token tile; 0: always
-                                    single-CTA 128 x 256 tiles                                                         */
+                                    the persistent grid, and a partial last round of a row-parallel linear is cut along
+                                    K over the idle pairs (fp32 partials summed in range order); 256 / 128: always
+                                    pairs, with that token tile, no tail split; 0: always single-CTA 128 x 256 tiles  */
     ETP_OPT__COUNT
 } etp_option;
 etp_status etp_ctx_set_option(etp_ctx* ctx, etp_option key, int64_t value);

@@ -48,6 +48,8 @@ struct alignas(64) LinearParams {
     void* y;
     float* partials;          // split-K workspace [(tile * n_splits + split)][BN][128]
     unsigned int* tickets;    // one per output tile, zero between launches (the last arriver resets its ticket)
+    int32_t tail_first, tail_splits;   // CTA-pair kernel: items >= tail_first (the grid's last, partial round) are cut into
+                                       // tail_splits K ranges, one per CTA pair (0 / 1 = no split)
 };
 
 template <int BN>
@@ -327,6 +329,29 @@ __host__ __device__ constexpr uint32_t make_idesc_pair(uint32_t fmt, uint32_t a_
     return (1u << 4) | (fmt << 7) | (fmt << 10) | (a_mn_major << 15) | ((n >> 3) << 17) | ((uint32_t(2 * kBM) >> 4) << 24);
 }
 
+// The k-th piece of work of a CTA pair.  Full rounds: item = cluster + k * n_clusters over all K chunks.  Then, if the last round
+// is partial (tail_splits > 1), ONE K range [c0, c1) of a tail item, so that round costs ~1/tail_splits of a full one; its fp32
+// partial tile goes through the split-K workspace and the last pair to arrive sums the ranges in order 0..S-1 (deterministic).
+struct PairWork {
+    int item, c0, c1, split;   // split < 0: the whole K range, written straight to Y
+};
+__device__ __forceinline__ bool pair_work(const LinearParams& p, int cluster_id, int n_clusters, int k, PairWork* w) {
+    const int n_items = p.n_m_tiles * p.n_n_tiles;
+    const int full = p.tail_splits > 1 ? p.tail_first : n_items;
+    const int item = cluster_id + k * n_clusters;
+    if (item < full) {
+        *w = {item, 0, p.n_chunks, -1};
+        return true;
+    }
+    if (p.tail_splits > 1 && k == full / n_clusters && cluster_id < (n_items - full) * p.tail_splits) {
+        const int split = cluster_id % p.tail_splits;
+        *w = {full + cluster_id / p.tail_splits, int(int64_t(split) * p.n_chunks / p.tail_splits),
+              int(int64_t(split + 1) * p.n_chunks / p.tail_splits), split};
+        return true;
+    }
+    return false;
+}
+
 // Items are (pair of m tiles, token tile); p.n_m_tiles counts PAIRS and runs[].first indexes pairs (column-parallel).
 template <int PBN, typename OutT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_shard_linear_pair_kernel(const __grid_constant__ LinearParams p) {
@@ -339,11 +364,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
     uint64_t* tmem_full = empty_bar + kPairStages;
     uint64_t* tmem_empty = tmem_full + 2;
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+    uint32_t* last_flag = tmem_ptr + 1;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
     const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
-    const int n_items = p.n_m_tiles * p.n_n_tiles;
     const bool row_par = p.mode == ETP_ROW_PARALLEL;
 
     if (threadIdx.x == 0) {
@@ -373,13 +398,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
         if (lane == 0) {
             int stage = 0;
             uint32_t phase = 0;
-            for (int item = cluster_id; item < n_items; item += n_clusters) {
-                const int pn = item % p.n_n_tiles, pm = item / p.n_n_tiles;
+            PairWork w;
+            for (int kk = 0; pair_work(p, cluster_id, n_clusters, kk, &w); ++kk) {
+                const int pn = w.item % p.n_n_tiles, pm = w.item / p.n_n_tiles;
                 const int t0 = pn * kPairBN + int(rank) * (kPairBN / 2);
                 int r = row_par ? 0 : find_run(p, pm);
                 const int row = row_par ? 0 : ((pm - p.runs[r].first) * 2 + int(rank)) * kBM;   // may lie past the run: zero-filled
                 const int m0 = (pm * 2 + int(rank)) * kBM;                                      // row-parallel: out features
-                for (int c = 0; c < p.n_chunks; ++c) {
+                for (int c = w.c0; c < w.c1; ++c) {
                     uint8_t* sa = smem + stage * kPairStageBytes;
                     uint8_t* sb = sa + kABytes;
                     mbar_wait(&empty_bar[stage], phase ^ 1);
@@ -412,13 +438,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
             int stage = 0;
             uint32_t phase = 0;
             int local = 0;
-            for (int item = cluster_id; item < n_items; item += n_clusters, ++local) {
+            PairWork w;
+            for (; pair_work(p, cluster_id, n_clusters, local, &w); ++local) {
                 const int as = local & 1;
                 const uint32_t aph = (local >> 1) & 1;
                 mbar_wait(&tmem_empty[as], aph ^ 1);   // both CTAs' epilogues have drained this accumulator stage
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + uint32_t(as * kPairBN);
-                for (int c = 0; c < p.n_chunks; ++c) {
+                for (int c = w.c0; c < w.c1; ++c) {
                     uint8_t* sa = smem + stage * kPairStageBytes;
                     mbar_wait(&full_bar[stage], phase);
                     tc_fence_after();
@@ -426,7 +453,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
                     const uint64_t b_desc = make_smem_desc(smem_u32(sa + kABytes), 16, 1024);
 #pragma unroll
                     for (int k = 0; k < kBK / kUmmaK; ++k)
-                        tc_mma_pair(d_tmem, a_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > 0 || k > 0) ? 1u : 0u);
+                        tc_mma_pair(d_tmem, a_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > w.c0 || k > 0) ? 1u : 0u);
                     tc_commit_pair(&empty_bar[stage]);   // frees the stage in BOTH CTAs once these MMAs have read it
                     if (++stage == kPairStages) { stage = 0; phase ^= 1; }
                 }
@@ -443,8 +470,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
         OutT* stage_t = reinterpret_cast<OutT*>(smem + kPairStages * kPairStageBytes + 256);
         const bool vec_out = (p.out_features & 7) == 0;
         int local = 0;
-        for (int item = cluster_id; item < n_items; item += n_clusters, ++local) {
-            const int pn = item % p.n_n_tiles, pm = item / p.n_n_tiles;
+        PairWork w;
+        for (; pair_work(p, cluster_id, n_clusters, local, &w); ++local) {
+            const int pn = w.item % p.n_n_tiles, pm = w.item / p.n_n_tiles;
             const int as = local & 1;
             const uint32_t aph = (local >> 1) & 1;
             const int t0 = pn * kPairBN;
@@ -467,7 +495,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
                 uint32_t v[16];
                 tc_ld16(taddr + uint32_t(c16), v);
                 tc_ld_wait();
-                if (vec_out) {
+                if (w.split >= 0) {
+                    float* ws = p.partials + ((size_t(w.item - p.tail_first) * 2 + rank) * p.tail_splits + w.split) * size_t(kPairBN) * kBM;
+#pragma unroll
+                    for (int j = 0; j < 16; ++j)
+                        if (c16 + j < n_tok) ws[(c16 + j) * kBM + m_local] = __uint_as_float(v[j]);
+                } else if (vec_out) {
                     store_block16(stage_t, v, m_local, y, size_t(t0 + c16), min(16, n_tok - c16), p.out_features, gm0, valid);
                 } else if (m_local < valid) {
 #pragma unroll
@@ -478,6 +511,47 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(drained + uint32_t(as) * 8u);
+            if (w.split >= 0) {
+                // the last of the tail_splits pairs to arrive at this (tile, CTA rank) sums the partials in range order
+                unsigned int* ticket = p.tickets + (w.item - p.tail_first) * 2 + rank;
+                __threadfence();
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (threadIdx.x == 64) *last_flag = (atomicAdd(ticket, 1u) == uint32_t(p.tail_splits - 1)) ? 1u : 0u;
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (*last_flag) {
+                    __threadfence();
+                    const float* w0 = p.partials + (size_t(w.item - p.tail_first) * 2 + rank) * p.tail_splits * size_t(kPairBN) * kBM;
+                    // 32 threads x float4 cover the 128 features of one token, the four warps take tokens j, j+1, j+2, j+3; eight
+                    // tokens per thread in flight.  Row-parallel only: gm0 is a multiple of 128 and out_features of 8, so the
+                    // four 16-bit results of a thread are one aligned 8-byte store and `valid` is a multiple of 8.
+                    const int col4 = lane * 4;
+                    for (int j0 = q; j0 < n_tok; j0 += 32) {
+                        float4 acc[8];
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        for (int sp = 0; sp < p.tail_splits; ++sp) {
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) {
+                                const int j = j0 + 4 * u;
+                                if (j < n_tok) {
+                                    const float4 t = __ldcg(reinterpret_cast<const float4*>(w0 + (size_t(sp) * kPairBN + j) * kBM + col4));
+                                    acc[u].x += t.x; acc[u].y += t.y; acc[u].z += t.z; acc[u].w += t.w;
+                                }
+                            }
+                        }
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) {
+                            const int j = j0 + 4 * u;
+                            if (j < n_tok && col4 < valid) {
+                                OutT o[4] = {cvt16<OutT>(acc[u].x), cvt16<OutT>(acc[u].y), cvt16<OutT>(acc[u].z), cvt16<OutT>(acc[u].w)};
+                                *reinterpret_cast<uint2*>(y + size_t(t0 + j) * p.out_features + gm0 + col4) = *reinterpret_cast<const uint2*>(o);
+                            }
+                        }
+                    }
+                    if (threadIdx.x == 64) *ticket = 0;
+                }
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+            }
         }
     }
 
@@ -661,9 +735,27 @@ extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_d
     const int64_t n_items = n_tiles * p.n_splits;
     if (n_items >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: too many work items");
 
+    // CTA pairs, row-parallel: a partial last round of the persistent grid is cut along K over the idle pairs (row-parallel only:
+    // its items depend on the nominal shapes alone, and reading G3 keeps column-parallel outputs independent of the layout)
+    int64_t ws_tiles = n_tiles, ws_splits = p.n_splits, ws_bn = bn;
+    if (pair && row_par && pbn == 256 && pair_opt != 256) {
+        const int64_t units = ctx->n_sms / 2, tail = n_items % units;
+        if (n_items > units && tail > 0) {
+            const int64_t S = std::min<int64_t>({units / tail, 8, int64_t(p.n_chunks)});
+            if (S >= 2) {
+                p.tail_first = int32_t(n_items - tail);
+                p.tail_splits = int32_t(S);
+                ws_tiles = tail * 2;
+                ws_splits = S;
+                ws_bn = pbn;
+            }
+        }
+    }
+
     ETP_CUDA_OK(cudaSetDevice(ctx->device));
-    if (p.n_splits > 1) {   // split-K workspace, owned by the ctx and grown on demand (calls on one ctx must not overlap in time)
-        const int64_t need = n_tiles * p.n_splits * bn * kBM * int64_t(sizeof(float));
+    if (p.n_splits > 1 || p.tail_splits > 1) {   // split-K workspace, owned by the ctx and grown on demand (calls on one ctx must not overlap in time)
+        const int64_t n_tiles = ws_tiles;
+        const int64_t need = n_tiles * ws_splits * ws_bn * kBM * int64_t(sizeof(float));
         if (need > ctx->lin_ws_bytes) {
             if (ctx->lin_ws) ETP_CUDA_OK(cudaFree(ctx->lin_ws));
             ctx->lin_ws = nullptr;

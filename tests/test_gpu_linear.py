@@ -95,6 +95,9 @@ CASES = [
     ("row", "bf16", 512, 2307 + 5, 2048, 1, (770, 771, 771), "wrap"),
     ("col", "bf16", 1000, 1024, 3000, 1, (1000, 1001, 999), "wrap"),       # CTA pairs: odd m-tile counts per run, 4 token tiles
     ("row", "bf16", 700, 3000, 1000, 1, (1000, 1001, 999), "wrap"),        # CTA pairs: out = 3.9 pair tiles, ragged tokens
+    ("row", "bf16", 2560, 1000, 2040, 1, (300, 400, 300), "wrap"),         # 8 x 10 = 80 pair items over 74 pairs: the 6 items of
+                                                                           # the last round are cut into 8 K ranges each (tail split)
+    ("col", "bf16", 2560, 1000, 2040, 1, (680, 680, 680), "tight"),        # same item count, column-parallel: no tail split (G3)
 ]
 
 
