@@ -247,11 +247,30 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
                 if (*last_flag) {
                     __threadfence();
                     const float* w0 = p.partials + size_t(it.tile) * p.n_splits * size_t(BN) * kBM;
-                    if (m_local < valid) {
-                        for (int j = 0; j < n_tok; ++j) {
-                            float acc = 0.f;
-                            for (int s = 0; s < p.n_splits; ++s) acc += __ldcg(w0 + (size_t(s) * BN + j) * kBM + m_local);
-                            y[size_t(t0 + j) * p.out_features + gm0 + m_local] = cvt16<OutT>(acc);
+                    // 32 threads x float4 cover the 128 features of one token, the four warps take tokens q, q+4, ...; the partials
+                    // of four splits are loaded together (independent L2 round trips) and added in split order 0..S-1.
+                    const int col4 = lane * 4;
+                    const bool vec8 = ((gm0 | p.out_features) & 3) == 0;
+                    for (int j = q; j < n_tok; j += 4) {
+                        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                        for (int s0 = 0; s0 < p.n_splits; s0 += 4) {
+                            float4 t[4];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u)
+                                t[u] = s0 + u < p.n_splits ? __ldcg(reinterpret_cast<const float4*>(w0 + (size_t(s0 + u) * BN + j) * kBM + col4))
+                                                           : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                            for (int u = 0; u < 4; ++u)
+                                if (s0 + u < p.n_splits) { acc.x += t[u].x; acc.y += t[u].y; acc.z += t[u].z; acc.w += t[u].w; }
+                        }
+                        OutT o[4] = {cvt16<OutT>(acc.x), cvt16<OutT>(acc.y), cvt16<OutT>(acc.z), cvt16<OutT>(acc.w)};
+                        OutT* dst = y + size_t(t0 + j) * p.out_features + gm0 + col4;
+                        if (vec8 && col4 + 4 <= valid) {
+                            *reinterpret_cast<uint2*>(dst) = *reinterpret_cast<const uint2*>(o);
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < 4; ++e)
+                                if (col4 + e < valid) dst[e] = o[e];
                         }
                     }
                     if (threadIdx.x == 64) p.tickets[it.tile] = 0;
