@@ -315,6 +315,37 @@ def test_shard_linear_argument_errors(ctx):
     assert e.value.status == 3
 
 
+def test_moe_linear_argument_errors(ctx):
+    E, F, Hd = 4, 64, 128
+    w = DevBuf(np.zeros(E * F * Hd * 2, dtype=np.uint8))
+    x = DevBuf(np.zeros(8 * Hd * 2, dtype=np.uint8))
+    y = DevBuf(np.full(8 * F * 2, 0xEE, dtype=np.uint8))
+    desc = etp.TensorDesc(E, F * Hd * 2, {0: (w.ptr, E, 0)}, 1, 0)
+    lay = [(0, 0, E, 1)]
+    etp.etp_moe_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, [0, 3, 3, 8, 8], Hd, F, desc, lay, y.ptr)
+    torch.cuda.synchronize()
+    assert not y.payload().any()                        # zero weights: every routed row written, as zeros
+    etp.etp_moe_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, [0, 0, 0, 0, 0], Hd, F, desc, lay, y.ptr)   # no rows: a no-op
+    for offs, status in (([1, 3, 3, 8, 8], 1), ([0, 3, 2, 8, 8], 1), ([0, 3, 8], 1)):
+        with pytest.raises(etp.EtpError) as e:          # offsets must start at 0, not decrease, and cover every expert
+            etp.etp_moe_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, offs, Hd, F, desc, lay, y.ptr)
+        assert e.value.status == status
+    with pytest.raises(etp.EtpError) as e:              # unit_bytes inconsistent with the shapes
+        etp.etp_moe_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, [0, 3, 3, 8, 8], Hd + 8, F, desc, lay, y.ptr)
+    assert e.value.status == 1
+    with pytest.raises(etp.EtpError) as e:              # row-parallel experts need in_features % 64 == 0
+        d2 = etp.TensorDesc(E, 72 * Hd * 2, {0: (w.ptr, E, 0)}, 1, 0)
+        etp.etp_moe_linear(ctx, etp.ROW_PARALLEL, "bf16", x.ptr, [0, 3, 3, 8, 8], 72, Hd, d2, lay, y.ptr)
+    assert e.value.status == 5
+    with pytest.raises(etp.EtpError) as e:              # layout with a gap
+        etp.etp_moe_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr, [0, 3, 3, 8, 8], Hd, F, desc, [(0, 0, E - 1, 1)], y.ptr)
+    assert e.value.status == 1
+    with pytest.raises(etp.EtpError) as e:              # misaligned x
+        etp.etp_moe_linear(ctx, etp.COL_PARALLEL, "bf16", x.ptr + 2, [0, 3, 3, 8, 8], Hd, F, desc, lay, y.ptr)
+    assert e.value.status == 2
+    assert x.guards_intact() and y.guards_intact() and w.guards_intact()
+
+
 def smoke_shard_linear(ctx):
     """Used by __graft_entry__.smoke(): config 1's layer on the resharded state, 4 tokens, against the oracle reference."""
     from tests import test_gpu_reshard as TR
