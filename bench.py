@@ -581,6 +581,7 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
                      "traffic": None if reduced or cfg.key != "2" else ncu_traffic_per_launch(),
                      "kernel": "etp_interval_copy_kernel", "peak_source": peak_src,
+                     "frac_of_datasheet_8TBps": achieved / 8000.0,   # state both denominators
                      "bytes_per_launch": 2.0 * kbytes / max(kl, 1), "ms_per_launch": kms / max(kl, 1), "launches": kl,
                      "d2d_only": {"moved_bytes": d_bytes // max(K, 1), "ms": d_kms / max(K, 1),
                                   "moved_GBps": d_bytes / (d_kms * 1e-3) / 1e9 if d_kms > 0 else None,
