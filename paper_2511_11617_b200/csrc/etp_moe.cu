@@ -60,6 +60,7 @@ __device__ __forceinline__ MoeItem load_item(const MoeItem* items, int i) {
 template <int BN, typename OutT>
 __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __grid_constant__ MoeParams p) {
     using C = MoeCfg<BN>;
+    constexpr int kXBox = BN < 64 ? BN : 64;   // rows per TMA box of the X tile
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + C::kStages * C::kStageBytes);
@@ -98,18 +99,20 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
             uint32_t phase = 0;
             for (int i = blockIdx.x; i < p.n_items; i += gridDim.x) {
                 const MoeItem it = load_item(p.items, i);
+                const int nb = (it.n_rows + kXBox - 1) / kXBox;
                 for (int c = 0; c < p.n_chunks; ++c) {
                     uint8_t* sa = smem + stage * C::kStageBytes;
                     uint8_t* sb = sa + kABytes;
                     mbar_wait(&empty_bar[stage], phase ^ 1);
-                    mbar_expect_tx(&full_bar[stage], C::kStageBytes);
+                    mbar_expect_tx(&full_bar[stage], uint32_t(kABytes + nb * kXBox * kBK * 2));
                     if (!row_par) {
                         tma_load_2d(sa, &p.map_w[it.run], &full_bar[stage], c * kBK, it.a_row);
                     } else {
                         tma_load_2d(sa, &p.map_w[it.run], &full_bar[stage], it.m0, it.a_row + c * kBK);
                         tma_load_2d(sa + kABytes / 2, &p.map_w[it.run], &full_bar[stage], it.m0 + 64, it.a_row + c * kBK);
                     }
-                    tma_load_2d(sb, &p.map_x, &full_bar[stage], c * kBK, it.x_row);
+                    for (int b = 0; b < nb; ++b)   // the X tile in 64-row boxes: a ragged last tile only fetches the boxes it has rows in
+                        tma_load_2d(sb + b * kXBox * kBK * 2, &p.map_x, &full_bar[stage], c * kBK, it.x_row + b * kXBox);
                     if (++stage == C::kStages) { stage = 0; phase ^= 1; }
                 }
             }
@@ -117,13 +120,15 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
         __syncwarp();
     } else if (warp == 1) {
         if (lane == 0) {   // ------------------------------------------------------------------ MMA issuer
-            const uint32_t idesc = make_idesc(p.dtype == ETP_BF16 ? 1u : 0u, row_par ? 1u : 0u, uint32_t(BN));
+            // UMMA_N per item: only the 64-row boxes of X that were fetched (a ragged last row tile of an expert runs a narrower MMA)
             const uint32_t a_lbo = row_par ? uint32_t(kABytes / 2) : 16u;
             const uint32_t a_kstep = row_par ? (uint32_t(kUmmaK) * 128u) >> 4 : (uint32_t(kUmmaK) * 2u) >> 4;
             int stage = 0;
             uint32_t phase = 0;
             int local = 0;
             for (int i = blockIdx.x; i < p.n_items; i += gridDim.x, ++local) {
+                const int n_rows = __ldg(&p.items[i].n_rows);
+                const uint32_t idesc = make_idesc(p.dtype == ETP_BF16 ? 1u : 0u, row_par ? 1u : 0u, uint32_t((n_rows + kXBox - 1) / kXBox * kXBox));
                 const int as = local & 1;
                 const uint32_t aph = (local >> 1) & 1;
                 mbar_wait(&tmem_empty[as], aph ^ 1);
@@ -285,9 +290,13 @@ extern "C" etp_status etp_moe_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dty
     {
         int64_t best = INT64_MAX;
         for (int cand : {256, 128, 64, 16}) {
-            int64_t tiles = 0;
-            for (int32_t e = 0; e < n_experts; ++e) tiles += (row_offsets[e + 1] - row_offsets[e] + cand - 1) / cand;
-            const int64_t cost = tiles * (kABytes + int64_t(cand) * kBK * 2);
+            int64_t cost = 0;
+            const int box = std::min(cand, 64);
+            for (int32_t e = 0; e < n_experts; ++e) {
+                const int64_t c = row_offsets[e + 1] - row_offsets[e];
+                const int64_t tiles = (c + cand - 1) / cand, boxes = (c + box - 1) / box;   // X is fetched in boxes of <= 64 rows
+                cost += tiles * kABytes + boxes * box * kBK * 2;
+            }
             if (cost < best) { best = cost; bn = cand; }
         }
     }
@@ -336,7 +345,7 @@ extern "C" etp_status etp_moe_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dty
     p.n_chunks = int32_t((in_features + kBK - 1) / kBK);
     p.out_features = int32_t(out_features);
     p.y = y_perm;
-    ETP_TRY(encode_2d(&p.map_x, dtype, x_perm, n_rows, in_features, in_features, kBK, bn));
+    ETP_TRY(encode_2d(&p.map_x, dtype, x_perm, n_rows, in_features, in_features, kBK, std::min(bn, 64)));
     for (size_t ri = 0; ri < runs.size(); ++ri) {
         const void* base = runs[ri].base + runs[ri].slot0 * w->unit_bytes;
         if (row_par) ETP_TRY(encode_2d(&p.map_w[ri], dtype, base, runs[ri].n * rows_per_expert, row_len, row_len, 64, kBK));
