@@ -96,6 +96,10 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
     const int n_items = p.n_m_tiles * p.n_n_tiles * p.n_splits;
     const bool row_par = p.mode == ETP_ROW_PARALLEL;
 
+    if (warp == 0 && lane == 1) {
+        prefetch_tensormap(&p.map_x);
+        for (int r = 0; r < p.n_runs; ++r) prefetch_tensormap(&p.map_w[r]);
+    }
     if (threadIdx.x == 0) {
         for (int s = 0; s < C::kStages; ++s) {
             mbar_init(&full_bar[s], 1);
@@ -390,6 +394,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
     const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
     const bool row_par = p.mode == ETP_ROW_PARALLEL;
 
+    if (warp == 0 && lane == 1) {
+        prefetch_tensormap(&p.map_x);
+        for (int r = 0; r < p.n_runs; ++r) prefetch_tensormap(&p.map_w[r]);
+    }
     if (threadIdx.x == 0) {
         for (int s = 0; s < kPairStages; ++s) {
             mbar_init(&full_bar[s], 1);      // used in the leader only: its own arrive.expect_tx of both CTAs' bytes

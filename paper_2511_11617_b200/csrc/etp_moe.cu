@@ -35,7 +35,7 @@ struct alignas(64) MoeParams {
     CUtensorMap map_w[kMaxRuns];
     const MoeItem* items;
     int32_t n_items, mode, dtype, n_chunks;   // n_chunks: K chunks of kBK per item
-    int32_t out_features;
+    int32_t out_features, n_runs;
     void* y;
 };
 
@@ -72,6 +72,10 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool row_par = p.mode == ETP_ROW_PARALLEL;
 
+    if (warp == 0 && lane == 1) {
+        prefetch_tensormap(&p.map_x);
+        for (int r = 0; r < p.n_runs; ++r) prefetch_tensormap(&p.map_w[r]);
+    }
     if (threadIdx.x == 0) {
         for (int s = 0; s < C::kStages; ++s) {
             mbar_init(&full_bar[s], 1);
@@ -344,6 +348,7 @@ extern "C" etp_status etp_moe_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dty
     p.dtype = dtype;
     p.n_chunks = int32_t((in_features + kBK - 1) / kBK);
     p.out_features = int32_t(out_features);
+    p.n_runs = int32_t(runs.size());
     p.y = y_perm;
     ETP_TRY(encode_2d(&p.map_x, dtype, x_perm, n_rows, in_features, in_features, kBK, std::min(bn, 64)));
     for (size_t ri = 0; ri < runs.size(); ++ri) {
