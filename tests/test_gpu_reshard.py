@@ -185,7 +185,7 @@ def test_param_errors(ctx):
 
 
 # ------------------------------------------------------------------------------------------------ KV
-def run_kv(ctx, world, budget, backup="pinned", head_cap=None):
+def run_kv(ctx, world, budget, backup="pinned", head_cap=None, plan=None):
     st = world.steps[0]
     g = world.g
     new_table, evicted, pairs = OS.page_table_rewrite(world.table, world.seq_lens, world.last_use, g.block_size, budget)
@@ -199,7 +199,7 @@ def run_kv(ctx, world, budget, backup="pinned", head_cap=None):
         img = torch.from_numpy(world.host_backup).cuda()
     else:
         img = None
-    plan = make_plans(st)["head"]
+    plan = plan or make_plans(st)["head"]
     n_ranks = max(world.pools) + 1
     table = world.table.copy()
     s = Streams()
@@ -307,6 +307,39 @@ def test_scale_up_a_repaired_rank_joins(ctx, tight):
 
 
 # ------------------------------------------------------------------------------------------------ migration-aware plan
+class MigSide(LibSide):
+    """plans with the owner of every target chosen to minimise transfers (reading M1); bounds as the scenario gives them"""
+    name = "libetp-migration-aware"
+
+    @staticmethod
+    def plan(old, M, tb=None):
+        p = etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, old, M, tb)
+        return p.tasks(), p.new_layout()
+
+
+@pytest.mark.parametrize("layout", [0, 1])
+@pytest.mark.parametrize("dead", [0, 1, 2])
+def test_kv_with_migration_aware_head_plan(ctx, layout, dead):
+    """Paged KV under a permuted head layout: config 1 (4 heads on 4 ranks), one rank dies, the migration-aware plan keeps
+    more heads in place than the in-order one; a rank may now own a head interval disjoint from its old one, so a reload can
+    land on a slot another rank still has to read (write-after-read phases across the copy and reload streams)."""
+    from oracle import planning as OP
+    cfg = get_config("1")
+    world = H.build_kv_world(cfg, side=MigSide, layout=layout, failed=(dead,))
+    st = world.steps[0]
+    old = [tuple(x) for x in st.old["head"]]
+    tb = [b for (_, b, _, _) in st.new["head"]] + [st.new["head"][-1][2]]
+    tasks, new = OP.migration_aware_plan(old, len(st.new["head"]), tb)
+    assert [tuple(t) for t in st.tasks["head"]] == [tuple(t) for t in tasks] and [tuple(x) for x in st.new["head"]] == new
+    base = OP.plan_stats(OP.cmm_plan(old, len(new), tb)[0])
+    assert OP.plan_stats(tasks)["transfer_units"] <= base["transfer_units"]
+    plan = etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, old, len(new), tb)
+    ev, evicted, rep, stats = run_kv(ctx, world, world.g.n_blocks, plan=plan)
+    assert ev == evicted == []
+    assert rep["d2d_bytes"] == stats["d2d_bytes"] and rep["h2d_bytes"] == stats["h2d_bytes"]
+
+
+# ------------------------------------------------------------------------------------------------ migration-aware plan (parameters)
 @pytest.mark.parametrize("slabs_mode", ["span", "full"])
 def test_migration_aware_plan_reshard_and_linear(ctx, slabs_mode):
     """Reading M1: config 5a's second failure in miniature - 7 ranks of 200 units, rank 0 dies, 6 targets.
