@@ -227,6 +227,17 @@ etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype,
                             const etp_tensor* w, const etp_shard* layout, int32_t n_shards,
                             int64_t features_per_unit, void* y, void* stream);
 
+/* Several COLUMN-parallel linears that share X, in_features and the shard layout of their granularity class (q | k | v of the
+ * attention class, gate | up of the FFN class) in ONE launch: at a few tokens a linear is a weight stream with a fixed cost of
+ * several microseconds per launch, and a serving engine runs these projections as one GEMM anyway.  Every
+ * linear keeps its own slabs and its own output y [tokens][out_features]; results are bitwise those of separate
+ * etp_shard_linear calls only when no K split is chosen (the split count depends on the total width).  n_outs in 1..8, all
+ * w->total_units equal; the rest as etp_shard_linear. */
+typedef struct { const etp_tensor* w; int64_t out_features; int64_t features_per_unit; void* y; } etp_linear_out;
+etp_status etp_shard_linear_multi(etp_ctx* ctx, etp_dtype dtype, const void* x, int64_t tokens, int64_t in_features,
+                                  const etp_linear_out* outs, int32_t n_outs, const etp_shard* layout, int32_t n_shards,
+                                  void* stream);
+
 /* ------------------------------------------------------------------------------------------------ grouped MoE linear
  * SURVEY.md 8(f) #3, reading G5; PAPER.md:172-174 (experts are the unit of the expert-granularity plan).  One
  * launch computes, for every expert e,  Y_perm[r][:] = X_perm[r][:] . W_e^T  for its routed rows r in

@@ -70,6 +70,10 @@ class etp_page_table(C.Structure):
                 ("last_use", C.POINTER(i64))]
 
 
+class etp_linear_out(C.Structure):
+    _fields_ = [("w", C.POINTER(etp_tensor)), ("out_features", i64), ("features_per_unit", i64), ("y", vp)]
+
+
 class etp_interval(C.Structure):
     _fields_ = [("src", vp), ("dst", vp), ("bytes", i64)]
 
@@ -77,7 +81,7 @@ class etp_interval(C.Structure):
 EXPORTS = ["etp_ctx_create", "etp_ctx_destroy", "etp_last_error", "etp_version", "etp_ctx_set_option", "etp_ctx_get_option",
            "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_tasks", "etp_plan_new_layout",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
-           "etp_moe_linear", "etp_copy_intervals"]
+           "etp_shard_linear_multi", "etp_moe_linear", "etp_copy_intervals"]
 
 _lib = None
 
@@ -112,6 +116,7 @@ def lib() -> C.CDLL:
                                      vp, vp, C.POINTER(etp_reshard_report)]
         L.etp_shard_linear.argtypes = [vp, C.c_int, C.c_int, vp, i64, i64, i64, C.POINTER(etp_tensor), C.POINTER(etp_shard), i32, i64,
                                        vp, vp]
+        L.etp_shard_linear_multi.argtypes = [vp, C.c_int, vp, i64, i64, C.POINTER(etp_linear_out), i32, C.POINTER(etp_shard), i32, vp]
         L.etp_moe_linear.argtypes = [vp, C.c_int, C.c_int, vp, C.POINTER(i64), i32, i64, i64, C.POINTER(etp_tensor), C.POINTER(etp_shard),
                                      i32, vp, vp]
         L.etp_copy_intervals.argtypes = [vp, C.POINTER(etp_interval), i64, vp, C.POINTER(etp_reshard_report)]
@@ -330,6 +335,26 @@ def etp_shard_linear(ctx: Context, mode: int, dtype: str, x_ptr: int, tokens: in
     _check(lib().etp_shard_linear(ctx.handle, mode, DTYPE[dtype], x_ptr, tokens, in_features, out_features, arr, _shards(layout),
                                   len(layout), features_per_unit, y_ptr, stream or None))
     del keep
+
+
+class PreparedMultiLinear:
+    """Pre-marshalled arguments of one etp_shard_linear_multi call: column-parallel linears (each a PreparedLinear of the same
+    class and in_features) fused into one launch; run() takes one output pointer per linear."""
+
+    def __init__(self, linears: Sequence["PreparedLinear"]):
+        assert linears and all(l.mode == COL_PARALLEL and l.K == linears[0].K and l.dtype == linears[0].dtype for l in linears)
+        self.lins = list(linears)
+        self.K, self.dtype = linears[0].K, linears[0].dtype
+        self.layout, self.n = linears[0].layout, linears[0].n
+        self.outs = (etp_linear_out * len(linears))()
+        for i, l in enumerate(linears):
+            self.outs[i] = etp_linear_out(C.cast(l.arr, C.POINTER(etp_tensor)), l.N, l.fpu, None)
+
+    def run(self, ctx: Context, x_ptr: int, tokens: int, y_ptrs: Sequence[int], stream: int = 0) -> None:
+        for i, y in enumerate(y_ptrs):
+            self.outs[i].y = y
+        _check(lib().etp_shard_linear_multi(ctx.handle, self.dtype, x_ptr, tokens, self.K, self.outs, len(self.lins), self.layout, self.n,
+                                            stream or None))
 
 
 def etp_moe_linear(ctx: Context, mode: int, dtype: str, x_ptr: int, row_offsets: Sequence[int], in_features: int, out_features: int,

@@ -32,16 +32,20 @@ using namespace etp::tc;
 
 namespace {
 
-struct Run {          // one contiguous slot range of a rank's shard, runs sorted by global feature
+constexpr int kMaxLinRuns = 32;   // <= 2 contiguous runs per rank, 8 ranks, up to 3 fused linears (q|k|v) - capped at 32
+
+struct Run {          // one contiguous slot range of a rank's shard, runs sorted by (linear, global feature)
     int64_t feat0;    // first global feature of the run (out-feature: column-parallel, in-feature: row-parallel)
     int32_t n_feat;   // features in the run
     int32_t first;    // column-parallel: index of the run's first m tile; row-parallel: of its first K chunk entry
+    void* y;          // column-parallel: output of the linear this run belongs to (etp_shard_linear_multi fuses several)
+    int32_t out_features, pad;   // ... and its row pitch
 };
 
 struct alignas(64) LinearParams {
     CUtensorMap map_x;
-    CUtensorMap map_w[kMaxRuns];
-    Run runs[kMaxRuns];
+    CUtensorMap map_w[kMaxLinRuns];
+    Run runs[kMaxLinRuns];
     int32_t n_runs, mode, dtype;
     int32_t tokens, in_features, out_features;
     int32_t n_m_tiles, n_n_tiles, n_splits, n_chunks;   // n_chunks: K chunks of kBK per output tile
@@ -197,8 +201,9 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
         const int q = warp & 3;                 // a warp may only touch TMEM lanes 32*(warp % 4) .. +31
         const int m_local = q * 32 + lane;
         OutT* y = reinterpret_cast<OutT*>(p.y);
+        int64_t outf = p.out_features;          // column-parallel: per run (a fused launch carries several linears)
         OutT* stage_t = reinterpret_cast<OutT*>(smem + C::kStages * C::kStageBytes + 256);
-        const bool vec_out = (p.out_features & 7) == 0;     // 16-byte epilogue stores need 16-byte aligned Y rows
+        bool vec_out = (p.out_features & 7) == 0;     // 16-byte epilogue stores need 16-byte aligned Y rows
         int local = 0;
         for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++local) {
             const Item it = decode_item(p, item);
@@ -213,9 +218,12 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
                 const int row = (it.m - p.runs[r].first) * kBM;
                 gm0 = p.runs[r].feat0 + row;
                 valid = min(kBM, p.runs[r].n_feat - row);
+                y = reinterpret_cast<OutT*>(p.runs[r].y);
+                outf = p.runs[r].out_features;
+                vec_out = (outf & 7) == 0;
             } else {
                 gm0 = int64_t(it.m) * kBM;
-                valid = min(kBM, p.out_features - it.m * kBM);
+                valid = min(kBM, int(outf) - it.m * kBM);
             }
             mbar_wait(&tmem_full[as], aph);
             tc_fence_after();
@@ -226,12 +234,12 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
                 tc_ld16(taddr + uint32_t(c16), v);
                 tc_ld_wait();
                 if (p.n_splits == 1 && vec_out) {
-                    store_block16(stage_t, v, m_local, y, size_t(t0 + c16), min(16, n_tok - c16), p.out_features, gm0, valid);
+                    store_block16(stage_t, v, m_local, y, size_t(t0 + c16), min(16, n_tok - c16), outf, gm0, valid);
                 } else if (p.n_splits == 1) {
                     if (m_local < valid) {
 #pragma unroll
                         for (int j = 0; j < 16; ++j)
-                            if (c16 + j < n_tok) y[size_t(t0 + c16 + j) * p.out_features + gm0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
+                            if (c16 + j < n_tok) y[size_t(t0 + c16 + j) * outf + gm0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
                     }
                 } else {
 #pragma unroll
@@ -254,7 +262,7 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
                     // 32 threads x float4 cover the 128 features of one token, the four warps take tokens q, q+4, ...; the partials
                     // of four splits are loaded together (independent L2 round trips) and added in split order 0..S-1.
                     const int col4 = lane * 4;
-                    const bool vec8 = ((gm0 | p.out_features) & 3) == 0;
+                    const bool vec8 = ((gm0 | outf) & 3) == 0;
                     for (int j = q; j < n_tok; j += 4) {
                         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
                         for (int s0 = 0; s0 < p.n_splits; s0 += 4) {
@@ -268,7 +276,7 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
                                 if (s0 + u < p.n_splits) { acc.x += t[u].x; acc.y += t[u].y; acc.z += t[u].z; acc.w += t[u].w; }
                         }
                         OutT o[4] = {cvt16<OutT>(acc.x), cvt16<OutT>(acc.y), cvt16<OutT>(acc.z), cvt16<OutT>(acc.w)};
-                        OutT* dst = y + size_t(t0 + j) * p.out_features + gm0 + col4;
+                        OutT* dst = y + size_t(t0 + j) * outf + gm0 + col4;
                         if (vec8 && col4 + 4 <= valid) {
                             *reinterpret_cast<uint2*>(dst) = *reinterpret_cast<const uint2*>(o);
                         } else {
@@ -493,9 +501,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
         const int q = warp & 3;
         const int m_local = q * 32 + lane;
         OutT* y = reinterpret_cast<OutT*>(p.y);
+        int64_t outf = p.out_features;          // column-parallel: per run (a fused launch carries several linears)
         const uint32_t drained = mapa_rank0(smem_u32(&tmem_empty[0]));
         OutT* stage_t = reinterpret_cast<OutT*>(smem + kPairStages * kPairStageBytes + 256);
-        const bool vec_out = (p.out_features & 7) == 0;
+        bool vec_out = (p.out_features & 7) == 0;
         int local = 0;
         PairWork w;
         for (; pair_work(p, cluster_id, n_clusters, local, &w); ++local) {
@@ -511,9 +520,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
                 const int row = ((pm - p.runs[r].first) * 2 + int(rank)) * kBM;
                 gm0 = p.runs[r].feat0 + row;
                 valid = min(kBM, p.runs[r].n_feat - row);
+                y = reinterpret_cast<OutT*>(p.runs[r].y);
+                outf = p.runs[r].out_features;
+                vec_out = (outf & 7) == 0;
             } else {
                 gm0 = int64_t(pm * 2 + int(rank)) * kBM;
-                valid = min(int64_t(kBM), int64_t(p.out_features) - gm0);
+                valid = int(min(int64_t(kBM), outf - gm0));
             }
             mbar_wait(&tmem_full[as], aph);
             tc_fence_after();
@@ -528,11 +540,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
                     for (int j = 0; j < 16; ++j)
                         if (c16 + j < n_tok) ws[(c16 + j) * kBM + m_local] = __uint_as_float(v[j]);
                 } else if (vec_out) {
-                    store_block16(stage_t, v, m_local, y, size_t(t0 + c16), min(16, n_tok - c16), p.out_features, gm0, valid);
+                    store_block16(stage_t, v, m_local, y, size_t(t0 + c16), min(16, n_tok - c16), outf, gm0, valid);
                 } else if (m_local < valid) {
 #pragma unroll
                     for (int j = 0; j < 16; ++j)
-                        if (c16 + j < n_tok) y[size_t(t0 + c16 + j) * p.out_features + gm0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
+                        if (c16 + j < n_tok) y[size_t(t0 + c16 + j) * outf + gm0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
                 }
             }
             tc_fence_before();
@@ -571,7 +583,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
                             const int j = j0 + 4 * u;
                             if (j < n_tok && col4 < valid) {
                                 OutT o[4] = {cvt16<OutT>(acc[u].x), cvt16<OutT>(acc[u].y), cvt16<OutT>(acc[u].z), cvt16<OutT>(acc[u].w)};
-                                *reinterpret_cast<uint2*>(y + size_t(t0 + j) * p.out_features + gm0 + col4) = *reinterpret_cast<const uint2*>(o);
+                                *reinterpret_cast<uint2*>(y + size_t(t0 + j) * outf + gm0 + col4) = *reinterpret_cast<const uint2*>(o);
                             }
                         }
                     }
@@ -643,31 +655,59 @@ etp_status launch_linear_pair(const LinearParams& p, int grid, cudaStream_t stre
 
 }  // namespace
 
-extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x, int64_t tokens,
-                                       int64_t in_features, int64_t out_features, const etp_tensor* w, const etp_shard* layout,
-                                       int32_t n_shards, int64_t features_per_unit, void* y, void* stream) {
-    if (!ctx || !w || !layout || !w->slabs) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: NULL argument");
+namespace {
+struct LinOut {   // one linear of a (possibly fused) launch
+    const etp_tensor* w;
+    int64_t out_features, features_per_unit;
+    void* y;
+};
+}  // namespace
+
+// Column-parallel: n_outs >= 1 linears that share X, in_features and the shard layout of their class (q|k|v, gate|up) in ONE
+// launch - the runs of all of them are concatenated and every run carries its own Y.  Row-parallel: n_outs == 1.
+static etp_status shard_linear_impl(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x, int64_t tokens,
+                                    int64_t in_features, const LinOut* outs, int32_t n_outs, const etp_shard* layout,
+                                    int32_t n_shards, void* stream) {
+    if (!ctx || !outs || !layout || n_outs < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: NULL argument");
     if (mode != ETP_COL_PARALLEL && mode != ETP_ROW_PARALLEL) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: bad mode %d", int(mode));
     if (dtype != ETP_BF16 && dtype != ETP_FP16) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: dtype %d is not bf16/fp16", int(dtype));
-    if (tokens < 0 || in_features <= 0 || out_features <= 0 || features_per_unit <= 0 || n_shards <= 0)
-        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: non-positive size");
-    if (tokens >= (int64_t(1) << 31) || in_features >= (int64_t(1) << 31) || out_features >= (int64_t(1) << 31))
-        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: sizes must be below 2^31");
     const bool row_par = mode == ETP_ROW_PARALLEL;
-    const int64_t sharded = row_par ? in_features : out_features;   // the dimension the weight is cut along
-    const int64_t row_len = row_par ? out_features : in_features;   // contiguous elements per feature row of the stored weight
-    if (w->total_units * features_per_unit != sharded)
-        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: total_units %lld x features_per_unit %lld != sharded dimension %lld",
-                 (long long)w->total_units, (long long)features_per_unit, (long long)sharded);
-    if (w->unit_bytes != features_per_unit * row_len * 2)
-        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: unit_bytes %lld != features_per_unit x row length x 2 = %lld",
-                 (long long)w->unit_bytes, (long long)(features_per_unit * row_len * 2));
-    if ((in_features * 2) % 16 || (row_len * 2) % 16)
-        ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: row pitches must be multiples of 16 bytes (in %lld, stored row %lld elements)",
-                 (long long)in_features, (long long)row_len);
+    if (row_par && n_outs != 1) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear_multi: only column-parallel linears can be fused");
+    if (tokens < 0 || in_features <= 0 || n_shards <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: non-positive size");
+    if (tokens >= (int64_t(1) << 31) || in_features >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: sizes must be below 2^31");
+    int64_t out_total = 0;
+    for (int32_t o = 0; o < n_outs; ++o) {
+        const etp_tensor* w = outs[o].w;
+        const int64_t out_features = outs[o].out_features, features_per_unit = outs[o].features_per_unit;
+        if (!w || !w->slabs) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: NULL argument");
+        if (out_features <= 0 || features_per_unit <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: non-positive size");
+        if (out_features >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: sizes must be below 2^31");
+        const int64_t sharded = row_par ? in_features : out_features;   // the dimension the weight is cut along
+        const int64_t row_len = row_par ? out_features : in_features;   // contiguous elements per feature row of the stored weight
+        if (w->total_units * features_per_unit != sharded)
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: total_units %lld x features_per_unit %lld != sharded dimension %lld",
+                     (long long)w->total_units, (long long)features_per_unit, (long long)sharded);
+        if (w->unit_bytes != features_per_unit * row_len * 2)
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: unit_bytes %lld != features_per_unit x row length x 2 = %lld",
+                     (long long)w->unit_bytes, (long long)(features_per_unit * row_len * 2));
+        if ((in_features * 2) % 16 || (row_len * 2) % 16)
+            ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: row pitches must be multiples of 16 bytes (in %lld, stored row %lld elements)",
+                     (long long)in_features, (long long)row_len);
+        if (w->total_units != outs[0].w->total_units)
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear_multi: fused linears must belong to one granularity class (%lld vs %lld units)",
+                     (long long)w->total_units, (long long)outs[0].w->total_units);
+        out_total += out_features;
+    }
     if (tokens == 0) return ETP_OK;
-    if (!x || !y) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: x / y is NULL");
-    if ((reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(y)) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: x / y not 16-byte aligned");
+    if (!x) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: x / y is NULL");
+    if (reinterpret_cast<uintptr_t>(x) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: x / y not 16-byte aligned");
+    for (int32_t o = 0; o < n_outs; ++o) {
+        if (!outs[o].y) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: x / y is NULL");
+        if (reinterpret_cast<uintptr_t>(outs[o].y) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: x / y not 16-byte aligned");
+    }
+    const int64_t out_features = outs[0].out_features;   // row-parallel: the one linear's width
+    void* const y = outs[0].y;
+    const int64_t total_units = outs[0].w->total_units;
 
     // ---- the shards in ascending unit order must tile [0, total_units)
     std::vector<etp_shard> sh;
@@ -676,37 +716,43 @@ extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_d
     std::sort(sh.begin(), sh.end(), [](const etp_shard& a, const etp_shard& b) { return a.begin < b.begin; });
     int64_t cursor = 0;
     for (const etp_shard& s : sh) {
-        if (s.begin != cursor) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: layout does not tile [0,%lld): gap or overlap at unit %lld", (long long)w->total_units, (long long)cursor);
+        if (s.begin != cursor) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: layout does not tile [0,%lld): gap or overlap at unit %lld", (long long)total_units, (long long)cursor);
         cursor = s.end;
     }
-    if (cursor != w->total_units) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: layout covers %lld of %lld units", (long long)cursor, (long long)w->total_units);
+    if (cursor != total_units) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: layout covers %lld of %lld units", (long long)cursor, (long long)total_units);
 
-    // ---- contiguous runs of every shard inside its slot-addressed slab (L3)
+    // ---- contiguous runs of every shard inside its slot-addressed slab (L3), linear by linear
     LinearParams p;
     std::memset(&p, 0, sizeof(p));
-    const void* run_addr[kMaxRuns];
+    const void* run_addr[kMaxLinRuns];
     int n_runs = 0;
-    for (const etp_shard& s : sh) {
-        if (s.rank < 0 || s.rank >= w->n_ranks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d outside the tensor's %d slabs", s.rank, w->n_ranks);
-        const etp_slab& sl = w->slabs[s.rank];
-        if (!sl.base) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d has no slab", s.rank);
-        if (reinterpret_cast<uintptr_t>(sl.base) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: slab of rank %d not 16-byte aligned", s.rank);
-        const int64_t width = s.end - s.begin;
-        if (sl.cap_units <= 0 || width > sl.cap_units) ETP_FAIL(ETP_ERR_CAPACITY, "etp_shard_linear: shard of rank %d (%lld units) exceeds its slab (%lld)", s.rank, (long long)width, (long long)sl.cap_units);
-        int64_t slot0 = (s.begin - sl.anchor_unit) % sl.cap_units;
-        if (slot0 < 0) slot0 += sl.cap_units;
-        const int64_t len1 = std::min(width, sl.cap_units - slot0);
-        const int64_t piece_b[2] = {s.begin, s.begin + len1};
-        const int64_t piece_n[2] = {len1, width - len1};
-        const int64_t piece_slot[2] = {slot0, 0};
-        for (int k = 0; k < 2; ++k) {
-            if (piece_n[k] == 0) continue;
-            if (n_runs == kMaxRuns) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: more than %d contiguous runs", kMaxRuns);
-            if (piece_n[k] * features_per_unit >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: run too long");
-            p.runs[n_runs].feat0 = piece_b[k] * features_per_unit;
-            p.runs[n_runs].n_feat = int32_t(piece_n[k] * features_per_unit);
-            run_addr[n_runs] = static_cast<const char*>(sl.base) + piece_slot[k] * w->unit_bytes;
-            ++n_runs;
+    for (int32_t o = 0; o < n_outs; ++o) {
+        const etp_tensor* w = outs[o].w;
+        const int64_t features_per_unit = outs[o].features_per_unit;
+        for (const etp_shard& s : sh) {
+            if (s.rank < 0 || s.rank >= w->n_ranks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d outside the tensor's %d slabs", s.rank, w->n_ranks);
+            const etp_slab& sl = w->slabs[s.rank];
+            if (!sl.base) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d has no slab", s.rank);
+            if (reinterpret_cast<uintptr_t>(sl.base) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: slab of rank %d not 16-byte aligned", s.rank);
+            const int64_t width = s.end - s.begin;
+            if (sl.cap_units <= 0 || width > sl.cap_units) ETP_FAIL(ETP_ERR_CAPACITY, "etp_shard_linear: shard of rank %d (%lld units) exceeds its slab (%lld)", s.rank, (long long)width, (long long)sl.cap_units);
+            int64_t slot0 = (s.begin - sl.anchor_unit) % sl.cap_units;
+            if (slot0 < 0) slot0 += sl.cap_units;
+            const int64_t len1 = std::min(width, sl.cap_units - slot0);
+            const int64_t piece_b[2] = {s.begin, s.begin + len1};
+            const int64_t piece_n[2] = {len1, width - len1};
+            const int64_t piece_slot[2] = {slot0, 0};
+            for (int k = 0; k < 2; ++k) {
+                if (piece_n[k] == 0) continue;
+                if (n_runs == kMaxLinRuns) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: more than %d contiguous runs", kMaxLinRuns);
+                if (piece_n[k] * features_per_unit >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: run too long");
+                p.runs[n_runs].feat0 = piece_b[k] * features_per_unit;
+                p.runs[n_runs].n_feat = int32_t(piece_n[k] * features_per_unit);
+                p.runs[n_runs].y = outs[o].y;
+                p.runs[n_runs].out_features = int32_t(outs[o].out_features);
+                run_addr[n_runs] = static_cast<const char*>(sl.base) + piece_slot[k] * w->unit_bytes;
+                ++n_runs;
+            }
         }
     }
 
@@ -756,7 +802,9 @@ extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_d
         p.n_m_tiles = acc;
         p.n_chunks = int32_t((in_features + kBK - 1) / kBK);
     }
-    const int64_t nominal_tiles = ((out_features + kBM - 1) / kBM) * p.n_n_tiles;
+    int64_t nominal_m = 0;
+    for (int32_t o = 0; o < n_outs; ++o) nominal_m += (outs[o].out_features + kBM - 1) / kBM;
+    const int64_t nominal_tiles = nominal_m * p.n_n_tiles;
     p.n_splits = std::min(choose_splits(nominal_tiles, int((in_features + kBK - 1) / kBK), ctx->n_sms, bn), p.n_chunks);
     const int64_t n_tiles = int64_t(p.n_m_tiles) * p.n_n_tiles;
     const int64_t n_items = n_tiles * p.n_splits;
@@ -821,4 +869,20 @@ extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_d
     if (bn == 16) return launch_linear<16>(p, grid, st);
     if (bn == 64) return launch_linear<64>(p, grid, st);
     return launch_linear<256>(p, grid, st);
+}
+
+extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x, int64_t tokens,
+                                       int64_t in_features, int64_t out_features, const etp_tensor* w, const etp_shard* layout,
+                                       int32_t n_shards, int64_t features_per_unit, void* y, void* stream) {
+    const LinOut one{w, out_features, features_per_unit, y};
+    return shard_linear_impl(ctx, mode, dtype, x, tokens, in_features, &one, 1, layout, n_shards, stream);
+}
+
+extern "C" etp_status etp_shard_linear_multi(etp_ctx* ctx, etp_dtype dtype, const void* x, int64_t tokens, int64_t in_features,
+                                             const etp_linear_out* outs, int32_t n_outs, const etp_shard* layout, int32_t n_shards,
+                                             void* stream) {
+    if (!outs || n_outs < 1 || n_outs > 8) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear_multi: 1..8 linears");
+    LinOut lo[8];
+    for (int32_t o = 0; o < n_outs; ++o) lo[o] = {outs[o].w, outs[o].out_features, outs[o].features_per_unit, outs[o].y};
+    return shard_linear_impl(ctx, ETP_COL_PARALLEL, dtype, x, tokens, in_features, lo, n_outs, layout, n_shards, stream);
 }

@@ -143,6 +143,52 @@ def test_shard_linear_matches_unsharded_reference(ctx, mode, dtype, T, K, N, fpu
         assert np.array_equal(b.payload(), slabs[r]), "the weight slabs are read-only for the linear"
 
 
+@pytest.mark.parametrize("T", [4, 40, 100, 700])
+def test_shard_linear_multi_fuses_qkv(ctx, T):
+    """etp_shard_linear_multi: q | k | v (one granularity class: 8 KV-head groups, 5 / 1 / 1 rows of 32 per group... here 160 /
+    32 / 32 features per unit) over unequal shards 3/3/2 with wrapped slabs, ONE launch; every output against the unsharded
+    reference, and - where the kernel takes no K split (> 64 tokens) - bitwise equal to three separate etp_shard_linear calls."""
+    dt = torch_dtype("bf16")
+    K, units = 520, 8
+    fpus = (160, 32, 32)
+    layout = widths_to_layout((3, 3, 2))
+    x_u8 = as_u8(fill_normal16(SEED, 780 + T, 0, T * K, 1.0, dt)).copy()
+    xb = DevBuf(x_u8)
+    lins, ybufs, refs, keep = [], [], [], []
+    for i, fpu in enumerate(fpus):
+        N = units * fpu
+        ub = fpu * K * 2
+        w_u8 = as_u8(fill_normal16(SEED, 790 + i, 0, N * K, 0.02, dt)).copy()
+        geom = {}
+        for (r, b, e, _) in layout:
+            cap = (e - b) + 1 + r + i
+            geom[r] = (b - (cap - (e - b) // 2) % cap, cap)
+        slabs = shard_into_slabs(w_u8, ub, layout, geom)
+        bufs = {r: DevBuf(a) for r, a in slabs.items()}
+        keep.append(bufs)
+        desc = etp.TensorDesc(units, ub, {r: (bufs[r].ptr, geom[r][1], geom[r][0]) for r in bufs}, 3, 0)
+        lins.append(etp.PreparedLinear(etp.COL_PARALLEL, "bf16", K, N, desc, layout, fpu))
+        ybufs.append(DevBuf(np.full(T * N * 2, 0xEE, dtype=np.uint8)))
+        refs.append(reference("bf16", x_u8, w_u8, T, K, N, False))
+    multi = etp.PreparedMultiLinear(lins)
+    multi.run(ctx, xb.ptr, T, [y.ptr for y in ybufs])
+    torch.cuda.synchronize()
+    for lin, yb, ref in zip(lins, ybufs, refs):
+        assert yb.guards_intact()
+        check(yb.payload(), ref, "bf16", T, lin.N)
+    if T > 64:
+        for lin, yb in zip(lins, ybufs):
+            y1 = DevBuf(np.full(T * lin.N * 2, 0xEE, dtype=np.uint8))
+            lin.run(ctx, xb.ptr, T, y1.ptr)
+            torch.cuda.synchronize()
+            assert np.array_equal(y1.payload(), yb.payload())
+    with pytest.raises(etp.EtpError) as e:      # different granularity classes cannot be fused
+        other = etp.PreparedLinear(etp.COL_PARALLEL, "bf16", K, 4 * 32, etp.TensorDesc(4, 32 * K * 2, {0: (keep[0][0].ptr, 4, 0)}, 3, 0),
+                                   layout, 32)
+        etp.PreparedMultiLinear([lins[0], other]).run(ctx, xb.ptr, T, [ybufs[0].ptr, ybufs[1].ptr])
+    assert e.value.status == 1
+
+
 def test_column_parallel_is_bitwise_independent_of_the_split(ctx):
     """Reading G3: the K order of a column-parallel output does not depend on how out-features are cut."""
     T, K, N = 4, 1024, 1536
