@@ -243,18 +243,38 @@ __device__ void copy_small_batch(const CopyArgs& a, unsigned int k, int lane) {
         for (uint32_t w0 = 0; w0 < total; w0 += 32 * kUnroll) {   // uniform trip count: every lane joins the shuffles
             uint4 buf[kUnroll];
             uint64_t da[kUnroll];
+            // the interval of the block's first and of its last word (warp-uniform): when they coincide - every interval of
+            // 4 KiB and more, block after block - the whole block takes its addresses from one lane and skips the per-word search
+            const uint32_t w_last = min(w0 + 32 * kUnroll, total) - 1;
+            int j_lo = 0, j_hi = 0;
 #pragma unroll
-            for (int u = 0; u < kUnroll; ++u) {
-                const uint32_t w = w0 + 32 * u + lane;
-                int j = 0;
+            for (int step = 16; step >= 1; step >>= 1) {
+                const uint32_t e_lo = __shfl_sync(0xffffffffu, excl, j_lo + step), e_hi = __shfl_sync(0xffffffffu, excl, j_hi + step);
+                if (e_lo <= w0) j_lo += step;
+                if (e_hi <= w_last) j_hi += step;
+            }
+            if (j_lo == j_hi) {
+                const uint64_t sj = __shfl_sync(0xffffffffu, sb, j_lo), dj = __shfl_sync(0xffffffffu, db, j_lo);
 #pragma unroll
-                for (int step = 16; step >= 1; step >>= 1) {
-                    const uint32_t e = __shfl_sync(0xffffffffu, excl, j + step);
-                    if (e <= w) j += step;
+                for (int u = 0; u < kUnroll; ++u) {
+                    const uint32_t w = w0 + 32 * u + lane;
+                    da[u] = dj + (uint64_t)w * 16;
+                    if (w < total) buf[u] = ld_stream(reinterpret_cast<const char*>(sj + (uint64_t)w * 16));
                 }
-                const uint64_t sj = __shfl_sync(0xffffffffu, sb, j);
-                da[u] = __shfl_sync(0xffffffffu, db, j) + (uint64_t)w * 16;
-                if (w < total) buf[u] = ld_stream(reinterpret_cast<const char*>(sj + (uint64_t)w * 16));
+            } else {
+#pragma unroll
+                for (int u = 0; u < kUnroll; ++u) {
+                    const uint32_t w = w0 + 32 * u + lane;
+                    int j = 0;
+#pragma unroll
+                    for (int step = 16; step >= 1; step >>= 1) {
+                        const uint32_t e = __shfl_sync(0xffffffffu, excl, j + step);
+                        if (e <= w) j += step;
+                    }
+                    const uint64_t sj = __shfl_sync(0xffffffffu, sb, j);
+                    da[u] = __shfl_sync(0xffffffffu, db, j) + (uint64_t)w * 16;
+                    if (w < total) buf[u] = ld_stream(reinterpret_cast<const char*>(sj + (uint64_t)w * 16));
+                }
             }
 #pragma unroll
             for (int u = 0; u < kUnroll; ++u)
