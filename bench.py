@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--seqs", type=int, default=0, help="debug: fewer sequences (marks the result as reduced)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--microbench", action="store_true", help="config 5b: copy-kernel microbenchmark over synthetic plans")
+    ap.add_argument("--planners", action="store_true", help="CMM vs Greedy vs Full Reload (PAPER.md:204) on the config's parameters")
     ap.add_argument("--moe", action="store_true", help="config 4: grouped MoE shard linear (etp_moe_linear) on the resharded experts")
     ap.add_argument("--no-linear", action="store_true", help="skip the S7 (shard linear) leg")
     ap.add_argument("--linear-only", action="store_true", help="only the S7 leg, on parameters alone (for ncu captures of kernel (c))")
@@ -358,6 +359,54 @@ def run_microbench(args):
     return 0
 
 
+def run_planners(args):
+    """PAPER.md:204 / Table II in bytes and milliseconds on one B200: the PARAMETERS of the config resharded with the reload
+    sources in pinned host memory under the three planners - CMM (the paper's), Greedy (keeps the local overlap, reloads every
+    gap from the host, no device-to-device transfer) and Full Reload (no reuse: every target byte comes over the host link)."""
+    import gc
+    import torch
+    import paper_2511_11617_b200 as etp
+    from paper_2511_11617_b200.state import ModelState
+    from workloads import get_config
+    from workloads.configs import scaled
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    cfg = get_config(args.config)
+    if args.layers:
+        cfg = scaled(cfg, n_layers=args.layers)
+    ctx = etp.Context(0)
+    cs, rs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+    rows = []
+    for name, mode in (("cmm", etp.PLAN_CMM), ("greedy", etp.PLAN_GREEDY), ("full_reload", etp.PLAN_FULL_RELOAD)):
+        state = ModelState(cfg, device=dev, image="pinned", with_kv=False, plan_mode=mode)
+        ms = []
+        for it in range(1 + max(args.steps, 1)):
+            e0, e1, er = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event()
+            e0.record(cs)
+            rep = state.reshard(ctx, 0, "pinned", cs.cuda_stream, rs.cuda_stream, replan=True)["params"]
+            er.record(rs)
+            cs.wait_event(er)
+            e1.record(cs)
+            e1.synchronize()
+            if it:
+                ms.append(e0.elapsed_time(e1))
+        ms.sort()
+        med = ms[len(ms) // 2]
+        rows.append({"planner": name, "ms": round(med, 2), "kept_GB": round(rep["kept_bytes"] / 1e9, 3), "d2d_GB": round(rep["d2d_bytes"] / 1e9, 3),
+                     "h2d_GB": round(rep["h2d_bytes"] / 1e9, 3), "h2d_GBps": round(rep["h2d_bytes"] / med / 1e6, 1)})
+        del state
+        gc.collect()
+        torch.cuda.empty_cache()
+    base = rows[0]["ms"]
+    for r in rows:
+        r["vs_cmm"] = round(r["ms"] / base, 2)
+    print(json.dumps({"planners": f"config {cfg.key}: parameters only, reload sources in pinned host memory (PAPER.md:204, Table II)",
+                      "param_GB": round(sum(sp.total_units * sp.unit_bytes for sp in __import__("workloads.configs", fromlist=["x"]).tensor_inventory(cfg)) / 1e9, 2),
+                      "rows": rows}))
+    ctx.close()
+    return 0
+
+
 def run_moe(args):
     """Config 4 (Qwen3-30B-A3B shape, 24 layers): the parameters are resharded 4 -> 3 (experts 42/43/43), then the three
     expert projections of a layer run through etp_moe_linear (one grouped launch each) on the NEW layout, layers cycling so
@@ -639,4 +688,6 @@ if __name__ == "__main__":
         sys.exit(run_microbench(a))
     if a.moe:
         sys.exit(run_moe(a))
+    if a.planners:
+        sys.exit(run_planners(a))
     sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))

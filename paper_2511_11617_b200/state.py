@@ -63,8 +63,10 @@ class ModelState:
     """Slabs, pools, images and page table of one config.  ``image`` in {"pinned", "device", "both"}."""
 
     def __init__(self, cfg: Config, device="cuda:0", image: str = "both", with_kv: bool = True,
-                 with_params: bool = True, slack_garbage: bool = False, seq_lens: Optional[Sequence[int]] = None):
+                 with_params: bool = True, slack_garbage: bool = False, seq_lens: Optional[Sequence[int]] = None,
+                 plan_mode: int = B.PLAN_CMM):
         self.cfg, self.device = cfg, torch.device(device)
+        self.plan_mode = plan_mode        # B.PLAN_CMM (the paper's planner) | PLAN_GREEDY | PLAN_FULL_RELOAD (PAPER.md:204)
         self.seed = SEED0 + 1000 * cfg.index
         self.image_kinds = ("pinned", "device") if image == "both" else (image,)
         self.specs: List[TensorSpec] = tensor_inventory(cfg) if with_params else []
@@ -102,7 +104,7 @@ class ModelState:
             old = [(r, s, e, 0 if r == dead else 1) for (r, s, e, _) in cur[klass]]
             M = len(old) - 1
             tb = B.etp_partition(H, M, sc.new_policy, granularity=klass)
-            plan = B.etp_cmm_plan(old, M, tb)
+            plan = B.etp_plan_create(self.plan_mode, old, M, tb)
             st.old[klass], st.bounds[klass], st.plans[klass] = old, tb, plan
             st.new[klass] = plan.new_layout()
         return st

@@ -65,11 +65,11 @@ class Streams:
         self.reload.synchronize()
 
 
-def make_plans(step) -> Dict[str, "etp.Plan"]:
-    """One plan handle per granularity class, from the step's old layout and new bounds."""
+def make_plans(step, mode: int = 0) -> Dict[str, "etp.Plan"]:
+    """One plan handle per granularity class, from the step's old layout and new bounds (mode: etp.PLAN_*)."""
     plans = {}
     for klass, old in step.old.items():
         new = step.new[klass]
         tb = [b for (_, b, _, _) in new] + [new[-1][2]]
-        plans[klass] = etp.etp_cmm_plan(old, len(new), tb)
+        plans[klass] = etp.etp_plan_create(mode, old, len(new), tb)
     return plans

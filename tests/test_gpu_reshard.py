@@ -56,9 +56,9 @@ def tensor_descs(world, bufs, images, step, class_index):
     return out
 
 
-def run_param_step(ctx, world, bufs, images, step_idx, streams):
+def run_param_step(ctx, world, bufs, images, step_idx, streams, mode=0):
     step = world.steps[step_idx]
-    plans = make_plans(step)
+    plans = make_plans(step, mode)
     klasses = sorted(plans)
     class_index = {k: i for i, k in enumerate(klasses)}
     descs = tensor_descs(world, bufs, images, step, class_index)
@@ -111,6 +111,29 @@ def test_mid_params_bit_exact_every_copy_path(ctx, image, tma_min):
     compare_params(world, bufs, expect, {1})
     assert rep["d2d_bytes"] == stats["d2d_bytes"]
     assert rep["h2d_bytes"] + rep["reload_dev_bytes"] == stats["h2d_bytes"]
+
+
+@pytest.mark.parametrize("planner", ["greedy", "full_reload"])
+def test_comparison_planners_bit_exact(ctx, planner):
+    """PAPER.md:204 / Table II: the Greedy (no P2P for gaps) and Full Reload (no reuse) planners through the same lowering and
+    the same reload pipeline, against the oracle applying the oracle's own plan of that kind; Full Reload moves no byte D2D."""
+    from oracle import planning as OP
+    fn, mode = {"greedy": (OP.greedy_plan, etp.PLAN_GREEDY), "full_reload": (OP.full_reload_plan, etp.PLAN_FULL_RELOAD)}[planner]
+
+    class Side(LibSide):
+        @staticmethod
+        def plan(old, M, tb=None):
+            return fn(old, M, tb)
+
+    world = H.build_param_world(MID, side=Side, mode="span")
+    expect, stats = H.oracle_reshard_params(world, 0)
+    assert stats["d2d_bytes"] == 0
+    bufs, images = upload_param_world(world)
+    rep = run_param_step(ctx, world, bufs, images, 0, Streams(), mode=mode)
+    compare_params(world, bufs, expect, {1})
+    assert rep["d2d_bytes"] == 0 and rep["h2d_bytes"] == stats["h2d_bytes"]
+    if planner == "full_reload":
+        assert rep["kept_bytes"] == 0 and rep["h2d_bytes"] == sum(sp.total_units * sp.unit_bytes for sp in world.specs)
 
 
 @pytest.mark.parametrize("mode", ["span", "tight"])
