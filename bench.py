@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--seqs", type=int, default=0, help="debug: fewer sequences (marks the result as reduced)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--microbench", action="store_true", help="config 5b: copy-kernel microbenchmark over synthetic plans")
+    ap.add_argument("--sweep", action="store_true", help="config 5a: time every reshard of the sequential-failure scenario")
     ap.add_argument("--planners", action="store_true", help="CMM vs Greedy vs Full Reload (PAPER.md:204) on the config's parameters")
     ap.add_argument("--moe", action="store_true", help="config 4: grouped MoE shard linear (etp_moe_linear) on the resharded experts")
     ap.add_argument("--no-linear", action="store_true", help="skip the S7 (shard linear) leg")
@@ -407,6 +408,58 @@ def run_planners(args):
     return 0
 
 
+def run_sweep(args):
+    """Config 5a (Fig. 5's k -> k-1 switches): sequential failures 8 -> 7 -> 6 -> 5 on the Llama-3-8B shape, each
+    reshard planned from the previous layout.  Every step is timed in place (a single-phase plan is idempotent: its sources are
+    never overwritten) with device-resident and with pinned-host reload sources."""
+    import torch
+    import paper_2511_11617_b200 as etp
+    from paper_2511_11617_b200.state import ModelState
+    from workloads import get_config
+    from workloads.configs import scaled
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    hbm_peak, peak_src = load_peaks()
+    cfg = get_config("5a")
+    if args.layers or args.seqs:
+        cfg = scaled(cfg, n_layers=args.layers or None, n_seqs=args.seqs or None)
+    ctx = etp.Context(0)
+    state = ModelState(cfg, device=dev, image="both")
+    cs, rs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+
+    def one(i, image):
+        e0, e1, er = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event()
+        e0.record(cs)
+        rep = state.reshard(ctx, i, image, cs.cuda_stream, rs.cuda_stream, replan=True)
+        er.record(rs)
+        cs.wait_event(er)
+        e1.record(cs)
+        e1.synchronize()
+        return e0.elapsed_time(e1), rep
+
+    rows = []
+    for i, st in enumerate(state.steps):
+        row = {"step": f"{len(st.old['head'])} -> {len(st.new['head'])} ranks, rank {st.dead} fails"}
+        for image in ("device", "pinned"):
+            for _ in range(2):
+                one(i, image)
+            res = [one(i, image) for _ in range(max(args.steps, 3))]
+            ms = sorted(r[0] for r in res)[len(res) // 2]
+            rep = res[-1][1]
+            assert rep["params"]["n_phases"] == 1
+            d2d = sum(r["d2d_bytes"] for r in (rep["params"], rep["kv"]))
+            rel = sum(r["h2d_bytes"] + r["reload_dev_bytes"] for r in (rep["params"], rep["kv"]))
+            row[image] = {"ms": round(ms, 3), "moved_GBps": round((d2d + rel) / ms / 1e6, 1)}
+            row.update({"kept_GB": round(sum(r["kept_bytes"] for r in (rep["params"], rep["kv"])) / 1e9, 2), "d2d_GB": round(d2d / 1e9, 2),
+                        "reload_GB": round(rel / 1e9, 2)})
+        row["device"]["hbm_frac"] = round(2.0 * row["device"]["moved_GBps"] / hbm_peak, 3)
+        rows.append(row)
+    print(json.dumps({"sweep": "config 5a: sequential failures, every reshard planned from the previous layout", "peak": hbm_peak,
+                      "peak_source": peak_src, "state_GB": round(sum(state.state_bytes().values()) / 1e9, 2), "rows": rows}))
+    ctx.close()
+    return 0
+
+
 def run_moe(args):
     """Config 4 (Qwen3-30B-A3B shape, 24 layers): the parameters are resharded 4 -> 3 (experts 42/43/43), then the three
     expert projections of a layer run through etp_moe_linear (one grouped launch each) on the NEW layout, layers cycling so
@@ -690,4 +743,6 @@ if __name__ == "__main__":
         sys.exit(run_moe(a))
     if a.planners:
         sys.exit(run_planners(a))
+    if a.sweep:
+        sys.exit(run_sweep(a))
     sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))
