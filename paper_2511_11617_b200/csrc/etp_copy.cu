@@ -262,18 +262,29 @@ __device__ void copy_small_batch(const CopyArgs& a, unsigned int k, int lane) {
                     if (w < total) buf[u] = ld_stream(reinterpret_cast<const char*>(sj + (uint64_t)w * 16));
                 }
             } else {
+                // the 8 rows' searches are interleaved step by step: 8 independent shuffles per step instead of 8 serial
+                // chains of 5 dependent ones (the warp was stalled on its own shuffle latency, not on memory)
+                int j[kUnroll];
+#pragma unroll
+                for (int u = 0; u < kUnroll; ++u) j[u] = 0;
+#pragma unroll
+                for (int step = 16; step >= 1; step >>= 1) {
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) {
+                        const uint32_t e = __shfl_sync(0xffffffffu, excl, j[u] + step);
+                        if (e <= w0 + 32 * u + lane) j[u] += step;
+                    }
+                }
+                uint64_t sa[kUnroll];
+#pragma unroll
+                for (int u = 0; u < kUnroll; ++u) {
+                    sa[u] = __shfl_sync(0xffffffffu, sb, j[u]);
+                    da[u] = __shfl_sync(0xffffffffu, db, j[u]) + (uint64_t)(w0 + 32 * u + lane) * 16;
+                }
 #pragma unroll
                 for (int u = 0; u < kUnroll; ++u) {
                     const uint32_t w = w0 + 32 * u + lane;
-                    int j = 0;
-#pragma unroll
-                    for (int step = 16; step >= 1; step >>= 1) {
-                        const uint32_t e = __shfl_sync(0xffffffffu, excl, j + step);
-                        if (e <= w) j += step;
-                    }
-                    const uint64_t sj = __shfl_sync(0xffffffffu, sb, j);
-                    da[u] = __shfl_sync(0xffffffffu, db, j) + (uint64_t)w * 16;
-                    if (w < total) buf[u] = ld_stream(reinterpret_cast<const char*>(sj + (uint64_t)w * 16));
+                    if (w < total) buf[u] = ld_stream(reinterpret_cast<const char*>(sa[u] + (uint64_t)w * 16));
                 }
             }
 #pragma unroll
