@@ -346,7 +346,8 @@ def run_microbench(args):
         r = run_plan(so, do, sz, arena)
         r["size_hi"] = MICROBENCH_HI[n]
         sweep.append(r)
-    for size, n in ((256, 1 << 18), (4096, 1 << 18), (65536, 1 << 16), (1 << 20, 1 << 13), (16 << 20, 512)):
+    for size, n in ((256, 1 << 18), (256, 1 << 22), (512, 1 << 21), (1024, 1 << 20), (2048, 1 << 19), (4096, 1 << 18), (65536, 1 << 16),
+                    (1 << 20, 1 << 13), (16 << 20, 512)):
         sz = np.full(n, size, dtype=np.int64)
         so = rng.integers(0, (src_arena - size) // 16, n).astype(np.int64) * 16
         do = np.arange(n, dtype=np.int64) * (size + 16)
