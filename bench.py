@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--seqs", type=int, default=0, help="debug: fewer sequences (marks the result as reduced)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--microbench", action="store_true", help="config 5b: copy-kernel microbenchmark over synthetic plans")
+    ap.add_argument("--plan-mode", default="cmm", choices=["cmm", "migration_aware"],
+                    help="cmm: Algorithm 1's in-order owners (the paper's); migration_aware: DESIGN.md reading M1")
     ap.add_argument("--sweep", action="store_true", help="config 5a: time every reshard of the sequential-failure scenario")
     ap.add_argument("--planners", action="store_true", help="CMM vs Greedy vs Full Reload (PAPER.md:204) on the config's parameters")
     ap.add_argument("--moe", action="store_true", help="config 4: grouped MoE shard linear (etp_moe_linear) on the resharded experts")
@@ -577,7 +579,8 @@ def run_ours(args):
     hbm_peak, peak_src = load_peaks()
 
     t_build = time.perf_counter()
-    state = ModelState(cfg, device=dev, image="device" if args.linear_only else "both", with_kv=not args.linear_only)
+    plan_mode = {"cmm": etp.PLAN_CMM, "migration_aware": etp.PLAN_MIGRATION_AWARE}[args.plan_mode]
+    state = ModelState(cfg, device=dev, image="device" if args.linear_only else "both", with_kv=not args.linear_only, plan_mode=plan_mode)
     t_build = time.perf_counter() - t_build
     ctx = etp.Context(local_rank)
     ctx.set_option(etp.OPT_TIME_KERNELS, 1)
@@ -704,7 +707,8 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": tot_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
         "data": "synthetic",
-        "config": {"workload": f"config {cfg.key}: {cfg.note}" + (" [REDUCED: debug run, not a bench value]" if reduced else ""),
+        "config": {"workload": f"config {cfg.key}: {cfg.note}" + (" [REDUCED: debug run, not a bench value]" if reduced else "")
+                               + (" [migration-aware plan, DESIGN.md reading M1]" if args.plan_mode != "cmm" else ""),
                    "state_GB": round((sb["param_bytes"] + sb["kv_live_bytes"]) / 1e9, 2),
                    "moved_GB_per_step": round(moved / K / 1e9, 3),
                    "l2": "inputs larger than L2 (every step re-reads and re-writes GBs; plans are hazard-free so a step is idempotent in place)",

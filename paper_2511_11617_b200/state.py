@@ -104,9 +104,12 @@ class ModelState:
             old = [(r, s, e, 0 if r == dead else 1) for (r, s, e, _) in cur[klass]]
             M = len(old) - 1
             tb = B.etp_partition(H, M, sc.new_policy, granularity=klass)
-            plan = B.etp_plan_create(self.plan_mode, old, M, tb)
-            st.old[klass], st.bounds[klass], st.plans[klass] = old, tb, plan
+            # migration-aware (reading M1): the planner also places the wide shards, so no bounds are imposed
+            plan = B.etp_plan_create(self.plan_mode, old, M, None if self.plan_mode == B.PLAN_MIGRATION_AWARE else tb)
             st.new[klass] = plan.new_layout()
+            if self.plan_mode == B.PLAN_MIGRATION_AWARE:
+                tb = [b for (_, b, _, _) in st.new[klass]] + [st.new[klass][-1][2]]
+            st.old[klass], st.bounds[klass], st.plans[klass] = old, tb, plan
         return st
 
     def plan_steps(self) -> List[StepPlan]:

@@ -31,6 +31,24 @@ def ctx():
     c.close()
 
 
+_ORACLE_PLANS = {}
+
+
+def oracle_tasks(state, st, klass, total_units):
+    """The ORACLE's plan of one class for this step: Algorithm 1 on the policy's bounds, or - when the state was planned
+    migration-aware (reading M1) - the oracle's own exhaustive search (cached: 5040 owner orders x the wide-shard placements)."""
+    old = tuple(tuple(s) for s in st.old[klass])
+    M = len(st.new[klass])
+    if state.plan_mode == etp.PLAN_MIGRATION_AWARE:
+        key = (old, M)
+        if key not in _ORACLE_PLANS:
+            _ORACLE_PLANS[key] = OP.migration_aware_plan(list(old), M)
+        tasks, new = _ORACLE_PLANS[key]
+        assert [tuple(x) for x in st.new[klass]] == new, "the library's migration-aware layout differs from the oracle's"
+        return tasks
+    return OP.cmm_plan(list(old), M, OP.partition(total_units, M, state.cfg.scenario.new_policy))[0]
+
+
 def slot_runs(begin, end, anchor, cap):
     """[(first unit, n units, first slot)] of units [begin, end) in a slot-addressed slab (test-side restatement of L3)."""
     out, u = [], begin
@@ -102,7 +120,7 @@ def oracle_layer_params(state, step_idx, snap):
         if sp.name not in snap:
             continue
         M = len(st.new[sp.klass])
-        tasks = OP.cmm_plan([tuple(s) for s in st.old[sp.klass]], M, OP.partition(sp.total_units, M, state.cfg.scenario.new_policy))[0]
+        tasks = oracle_tasks(state, st, sp.klass, sp.total_units)
         lo, hi = state.reload_range[sp.klass]
         epu = sp.unit_bytes // state.cfg.model.elem_bytes
         img = None
@@ -202,7 +220,7 @@ def oracle_layer_kv(state, step_idx, layer, snap, image):
     g1 = OS.KVGeom(1, n_blocks, bs, cap, m.head_dim, m.elem_bytes, 0)
     sc = state.cfg.scenario
     H = m.n_kv_heads
-    tasks = OP.cmm_plan([tuple(s) for s in st.old["head"]], len(st.new["head"]), OP.partition(H, len(st.new["head"]), sc.new_policy))[0]
+    tasks = oracle_tasks(state, st, "head", H)
     _, evicted, pairs = OS.page_table_rewrite(kv["table"], kv["seq_lens"], kv["last_use"], bs, n_blocks)
     assert not evicted
     per_kind, hh, ds = kv["backup"][step_idx]
@@ -305,11 +323,11 @@ def check_moe_layer(ctx, state, step_idx, layer, tokens=16):
 
 
 # ------------------------------------------------------------------------------------------------ the tests
-def run_full_config(ctx, key, image, linear_tokens=(), garbage=True, shrink=None):
+def run_full_config(ctx, key, image, linear_tokens=(), garbage=True, shrink=None, plan_mode=etp.PLAN_CMM):
     cfg = get_config(key)
     if shrink:
         cfg = scaled(cfg, **shrink)
-    state = ModelState(cfg, device="cuda:0", image=image, slack_garbage=garbage)
+    state = ModelState(cfg, device="cuda:0", image=image, slack_garbage=garbage, plan_mode=plan_mode)
     cs, rs = torch.cuda.Stream(), torch.cuda.Stream()
     m = cfg.model
     for i, st in enumerate(state.steps):
@@ -332,7 +350,7 @@ def run_full_config(ctx, key, image, linear_tokens=(), garbage=True, shrink=None
         d2d = h2d = 0
         for sp in state.specs:
             M = len(st.new[sp.klass])
-            tasks = OP.cmm_plan([tuple(s) for s in st.old[sp.klass]], M, OP.partition(sp.total_units, M, cfg.scenario.new_policy))[0]
+            tasks = oracle_tasks(state, st, sp.klass, sp.total_units)
             ps = OP.plan_stats(tasks)
             d2d += ps["transfer_units"] * sp.unit_bytes
             h2d += ps["reload_units"] * sp.unit_bytes
@@ -361,6 +379,17 @@ def test_config2b_full_state_floor_policy(ctx):
 def test_config3_full_state(ctx):
     """configs[2]: Llama-3-8B shape, 8 -> 7 after rank 5 fails, unequal old FFN widths."""
     run_full_config(ctx, "3", "pinned", linear_tokens=(4,))
+
+
+def test_config3_full_state_migration_aware(ctx):
+    """configs[2] under the migration-aware planner (reading M1): owners and wide-shard placement chosen by the library, checked
+    against the oracle's exhaustive search; 2.55 GB instead of 5.04 GB move device-to-device; same whole-state and oracle checks."""
+    state = run_full_config(ctx, "3", "pinned", linear_tokens=(4,), plan_mode=etp.PLAN_MIGRATION_AWARE)
+    st = state.steps[0]
+    base = sum(OP.plan_stats(OP.cmm_plan([tuple(s) for s in st.old[k]], len(st.new[k]),
+                                         OP.partition(max(e for (_, _, e, _) in st.old[k]), len(st.new[k]), "floor"))[0])["transfer_units"]
+               for k in ("head",))
+    assert st.plans["head"].stats()["transfer_units"] < base
 
 
 def test_config4_full_state_moe(ctx):
