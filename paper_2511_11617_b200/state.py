@@ -255,7 +255,7 @@ class ModelState:
 
     # ------------------------------------------------------------------ one pass of the hot path (S1-S6)
     def reshard(self, ctx: B.Context, step_idx: int, image: str, copy_stream: int, reload_stream: int,
-                replan: bool = True, table: Optional[np.ndarray] = None) -> Dict[str, object]:
+                replan: bool = True, table: Optional[np.ndarray] = None, block_budget: Optional[int] = None) -> Dict[str, object]:
         """S1 partition + S2 CMM plan (host, inside libetp.so), then S3-S5 on the parameters and S3-S6 on the KV cache.
         Asynchronous: returns after enqueueing; the caller synchronises both streams."""
         st = self.steps[step_idx]
@@ -280,7 +280,8 @@ class ModelState:
                 ctx, n_layers=m.n_layers, n_blocks=kv["n_blocks"], block_size=self.cfg.kv.block_size, head_cap=kv["head_cap"],
                 head_dim=m.head_dim, elem_bytes=m.elem_bytes, layout=B.KV_TOKEN_MAJOR, pools=alive_pools,
                 head_anchor=kv["anchors"], n_ranks=self.n_ranks, table=new_table, seq_lens=kv["seq_lens"],
-                last_use=kv["last_use"], head_plan=plans["head"], new_block_budget=kv["n_blocks"],
+                last_use=kv["last_use"], head_plan=plans["head"],
+                new_block_budget=kv["n_blocks"] if block_budget is None else block_budget,
                 host_backup=per_kind[image].data_ptr() if hh > 0 else 0, host_heads=hh, host_head0=ds,
                 copy_stream=copy_stream, reload_stream=reload_stream)
         return {"params": rep_p, "kv": rep_k, "evicted": evicted, "table": new_table, "plans": plans}

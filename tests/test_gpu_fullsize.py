@@ -213,7 +213,7 @@ def snapshot_layer_kv(state, layer):
     return {r: layer_slice(state, p, layer, cap).cpu().numpy().copy() for r, p in state.kv["pools"].items()}
 
 
-def oracle_layer_kv(state, step_idx, layer, snap, image):
+def oracle_layer_kv(state, step_idx, layer, snap, image, budget=None):
     st = state.steps[step_idx]
     m, kv = state.cfg.model, state.kv
     planes, n_blocks, bs, cap, frag = kv_dims(state)
@@ -221,8 +221,8 @@ def oracle_layer_kv(state, step_idx, layer, snap, image):
     sc = state.cfg.scenario
     H = m.n_kv_heads
     tasks = oracle_tasks(state, st, "head", H)
-    _, evicted, pairs = OS.page_table_rewrite(kv["table"], kv["seq_lens"], kv["last_use"], bs, n_blocks)
-    assert not evicted
+    _, evicted, pairs = OS.page_table_rewrite(kv["table"], kv["seq_lens"], kv["last_use"], bs, n_blocks if budget is None else budget)
+    assert budget is not None or not evicted
     per_kind, hh, ds = kv["backup"][step_idx]
     backup = layer_slice(state, per_kind[image], layer, hh).cpu().numpy() if hh > 0 else None
     alive = {r: a for r, a in snap.items() if r != st.dead and any(rr == r for (rr, _, _, _) in st.old["head"])}
@@ -390,6 +390,37 @@ def test_config3_full_state_migration_aware(ctx):
                                          OP.partition(max(e for (_, _, e, _) in st.old[k]), len(st.new[k]), "floor"))[0])["transfer_units"]
                for k in ("head",))
     assert st.plans["head"].stats()["transfer_units"] < base
+
+
+@pytest.mark.parametrize("budget_kind", ["relocate", "evict"])
+def test_config2_kv_block_budget_shrink_full_size(ctx, budget_kind):
+    """Reading K5 at full size: config 2's KV cache (8 layers of it; 64 x 2048 tokens = 8192 live blocks in a fragmented pool of
+    10240) resharded 4 -> 3 with a block budget below the pool size.  "relocate": budget = 8192 live blocks, every live block
+    with id >= 8192 moves to a free id below it (same-rank copies of kept heads, incoming heads written straight to the new id);
+    "evict": budget = 6000 < live, the coldest sequences are evicted first.  Table, evicted list and byte counts
+    against the oracle's rule; the planes of two layers byte for byte against the oracle."""
+    cfg = scaled(get_config("2"), n_layers=8)
+    state = ModelState(cfg, device="cuda:0", image="pinned", with_params=False, slack_garbage=True)
+    kv, m = state.kv, cfg.model
+    bs = cfg.kv.block_size
+    live = int(((kv["seq_lens"].astype(np.int64) + bs - 1) // bs).sum())
+    budget = live if budget_kind == "relocate" else 6000
+    exp_table, exp_evicted, pairs = OS.page_table_rewrite(kv["table"], kv["seq_lens"], kv["last_use"], bs, budget)
+    assert (len(exp_evicted) > 0) == (budget_kind == "evict")
+    assert sum(1 for p in pairs if p[2] != p[3]) > 500                      # plenty of relocations in a fragmented pool
+    layers = [1, 6]
+    snaps = {L: snapshot_layer_kv(state, L) for L in layers}
+    cs, rs = torch.cuda.Stream(), torch.cuda.Stream()
+    rep = state.reshard(ctx, 0, "pinned", cs.cuda_stream, rs.cuda_stream, replan=True, block_budget=budget)
+    cs.synchronize()
+    rs.synchronize()
+    assert sorted(rep["evicted"]) == sorted(exp_evicted)
+    assert np.array_equal(rep["table"], exp_table)
+    assert rep["table"][rep["table"] >= 0].max() < budget
+    for L in layers:
+        kexp, kstats = oracle_layer_kv(state, 0, L, snaps[L], "pinned", budget=budget)
+        compare_layer_kv(state, L, kexp)
+    assert (rep["kv"]["d2d_bytes"], rep["kv"]["h2d_bytes"]) == (kstats["d2d_bytes"] * m.n_layers, kstats["h2d_bytes"] * m.n_layers)
 
 
 def test_config4_full_state_moe(ctx):
