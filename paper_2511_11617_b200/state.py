@@ -64,8 +64,10 @@ class ModelState:
 
     def __init__(self, cfg: Config, device="cuda:0", image: str = "both", with_kv: bool = True,
                  with_params: bool = True, slack_garbage: bool = False, seq_lens: Optional[Sequence[int]] = None,
-                 plan_mode: int = B.PLAN_CMM):
+                 plan_mode: int = B.PLAN_CMM, cap_mode: str = "span"):
         self.cfg, self.device = cfg, torch.device(device)
+        self.cap_mode = cap_mode          # "span": union span of the rank's intervals (one hazard phase, L5);
+                                          # "tight": the widest shard the rank ever holds (shards wrap, plans need phases)
         self.plan_mode = plan_mode        # B.PLAN_CMM (the paper's planner) | PLAN_GREEDY | PLAN_FULL_RELOAD
         self.seed = SEED0 + 1000 * cfg.index
         self.image_kinds = ("pinned", "device") if image == "both" else (image,)
@@ -137,7 +139,11 @@ class ModelState:
                         a, n = st.plans[klass].slab_span(r)
                         if n > 0:
                             lo, hi = min(lo, a), max(hi, a + n)
-                g[r] = (s, max(hi - lo, 1))
+                if self.cap_mode == "tight":
+                    widest = max([e - s] + [e2 - s2 for st in self.steps for (rr, s2, e2, _) in st.new[klass] if rr == r])
+                    g[r] = (s, max(widest, 1))
+                else:
+                    g[r] = (s, max(hi - lo, 1))
             self.geom[klass] = g
             rl = [(b, e) for st in self.steps for (k, _, _, b, e) in st.plans[klass].tasks() if k == B.RELOAD]
             self.reload_range[klass] = (min(b for b, _ in rl), max(e for _, e in rl)) if rl else (0, 0)
