@@ -61,3 +61,13 @@ def test_ours_fails_loudly_without_a_gpu():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--warmup", "0"], env=env,
                        capture_output=True, text=True, timeout=600)
     assert r.returncode != 0 and "no CPU fallback" in (r.stderr + r.stdout)
+
+
+def test_roofline_traffic_is_read_from_the_committed_ncu_capture():
+    """bench.py's roofline.traffic comes from profiles/r1_copy_kernel_full.csv (one parameter launch + one KV launch of config 2):
+    the file must stay in the layout the parser reads, and the DRAM bytes must stay near the algorithmic 2 B per moved byte."""
+    import bench
+    t = bench.ncu_traffic_per_launch()
+    assert t is not None, "profiles/r1_copy_kernel_full.csv is missing or not in the 'metric,unit,launch1,launch2,...' layout"
+    algorithmic = 2.0 * (9.425e9 + 5.369e9) / 2.0          # config 2, device-resident images: bytes moved by the two launches
+    assert 0.95 < t / algorithmic < 1.10
