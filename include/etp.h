@@ -12,7 +12,7 @@
  *  - the CALLER owns every data buffer (device slabs, KV pools, host image, page table, X/Y); pointers are raw
  *    (torch.Tensor.data_ptr()) and streams are raw cudaStream_t (torch.cuda.Stream.cuda_stream), passed as void*.
  *    "device" / "host" / "pinned host" is stated per argument.
- *  - the LIBRARY owns plan objects, descriptor arenas (pinned + device), the staging ring and its events; they
+ *  - the LIBRARY owns plan objects, descriptor arenas (pinned + device) and its events; they
  *    live in an etp_ctx / etp_plan and are freed by the matching _destroy / _free.
  *  - device calls are ASYNCHRONOUS: work is enqueued on the given streams and is complete when the caller has
  *    synchronised BOTH streams.  Data buffers must stay valid until then.  A ctx may be used from one host
@@ -46,9 +46,10 @@ typedef struct etp_plan etp_plan;
 
 /* ------------------------------------------------------------------------------------------------ context */
 
-/* Create a context on CUDA device `device`.  `staging_bytes` (>= 0; 0 = default 256 MiB) sizes the device staging
- * ring used by the KV reload pipeline (pinned host -> staging by DMA, staging -> head-strided fragments by the
- * copy kernel).  Fails with ETP_ERR_CUDA if the device is missing or is not compute capability 10.x. */
+/* Create a context on CUDA device `device`.  `staging_bytes` must be >= 0 and is otherwise RESERVED: the KV reload
+ * pipeline needs no device staging ring (the copy kernel reads the pinned backup over the host link and writes the
+ * head-strided fragments in place), so nothing is allocated for it.  Fails with ETP_ERR_CUDA if the
+ * device is missing or is not compute capability 10.x. */
 etp_status etp_ctx_create(int device, int64_t staging_bytes, etp_ctx** out);
 void etp_ctx_destroy(etp_ctx* ctx);
 const char* etp_last_error(void);
@@ -62,9 +63,8 @@ typedef enum {
                                     INT64_MAX disables the TMA path, 0 sends everything 16-B aligned to it       */
     ETP_OPT_LDG_STEALS_BULK = 3, /* 1 (default 0): vector-copy warps also drain the bulk queue when theirs is empty */
     ETP_OPT_RELOAD_CHUNK_BYTES = 4, /* max bytes per cudaMemcpyAsync of the reload pipeline (default 64 MiB)     */
-    ETP_OPT_KV_RELOAD_MODE = 5,  /* 0 (default): zero-copy gather - the copy kernel reads the pinned backup over the
-                                    host link and writes the head-strided fragments in place; 1: DMA of whole
-                                    (layer, K|V) planes to the staging ring + scatter by the copy kernel           */
+    ETP_OPT_RESERVED_5 = 5,      /* ignored (round 1 reserved it for a staged KV reload that was never built: the
+                                    zero-copy gather already runs at the speed of the host link)                   */
     ETP_OPT_GRID_CTAS = 6,       /* persistent grid size; 0 (default) = number of SMs                            */
     ETP_OPT_GATHER_CTAS = 7,     /* CTAs of the zero-copy gather launch on the reload stream (default 16)        */
     ETP_OPT_TIME_KERNELS = 8,    /* 1 (default 0): bracket every launch of the copy kernel on the copy stream with CUDA
@@ -74,6 +74,9 @@ typedef enum {
                                     the persistent grid, and a partial last round of a row-parallel linear is cut along
                                     K over the idle pairs (fp32 partials summed in range order); 256 / 128: always
                                     pairs, with that token tile, no tail split; 0: always single-CTA 128 x 256 tiles  */
+    ETP_OPT_VALIDATE_INTERVALS = 10, /* 1 (default): etp_copy_intervals checks on the host that the destinations are mutually
+                                    disjoint and disjoint from every source (two sorts, O(n log n)) and returns
+                                    ETP_ERR_INVALID_ARG before anything is enqueued; 0: trust the caller                   */
     ETP_OPT__COUNT
 } etp_option;
 etp_status etp_ctx_set_option(etp_ctx* ctx, etp_option key, int64_t value);
@@ -254,7 +257,9 @@ etp_status etp_moe_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, c
 
 /* ------------------------------------------------------------------------------------------------ microbenchmark entry
  * Copies n arbitrary intervals with the same persistent kernel (config 5b).  host_descs: host array; src/dst: device,
- * 16-B aligned; bytes: multiple of 16.  Destinations must be mutually disjoint and disjoint from every source. */
+ * 16-B aligned; bytes: multiple of 16.  Destinations must be mutually disjoint and disjoint from every source (the
+ * intervals of one call are unordered); checked unless ETP_OPT_VALIDATE_INTERVALS is 0 -> ETP_ERR_INVALID_ARG, nothing
+ * enqueued.  Sources may overlap each other. */
 typedef struct { const void* src; void* dst; int64_t bytes; } etp_interval;
 etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_descs, int64_t n, void* stream,
                               etp_reshard_report* report);

@@ -25,8 +25,9 @@ Pin status (tests/test_oracle_*.py, all ``-m "not gpu"``):
                  instances; invariants I1-I5; Table II ordering in units (:204)
   apply_params   pinned: plain definition (new shard == slice of the unsharded tensor), untouched bytes,
                  hand-written golden slab image (tests/golden/slab_tiny.txt)
-  apply_kv       pinned: plain definition KV_ref[s][t][l][c][h] readable at its new place; hand-written
-                 golden (tests/golden/kv_tiny.txt)
+  apply_kv       pinned: plain definition KV_ref[s][t][l][c][h] readable at its new place (numpy N-d views, not the
+                 oracle's offset arithmetic); hand-written golden tests/golden/kv_tiny.txt (relocated block, TRANSFER
+                 head, RELOAD head into a wrapped slot, both layouts; tests/test_oracle_state.py::test_golden_kv_image)
   page_table     pinned: hand-worked example (tests/golden/page_table.txt), injectivity / budget properties.
                  The eviction + relocation RULE itself is a DESIGN.md reading (K5) of PAPER.md:86 — the
                  paper fixes only "LRU"; no value in the paper pins the relocation order.

@@ -90,3 +90,59 @@ int64_t oracle_apply_kv_task(int kind, int64_t h_begin, int64_t h_end, int layou
     }
     return written;
 }
+
+/* ---------------------------------------------------------------------------------------------------------------
+ * All-cores leg of the CPU baseline (SURVEY.md 8(d) "Oracle timing": once on 1 core, once with an OpenMP parallel for
+ * over tasks on all cores).  The SAME element-by-element functions above, called from a parallel loop over a job list
+ * (one job = one task, or a sub-range of a task's units / live blocks so that the loop balances); jobs write disjoint
+ * bytes (targets tile the unit space, live blocks are distinct), and sources are read from the snapshot only.
+ * Built twice from this file: libetp_oracle.so (-O2; the pragma is ignored) and libetp_oracle_omp.so (-O2 -fopenmp). */
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int oracle_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+typedef struct {
+    int64_t kind, begin, end, unit_bytes;
+    const uint8_t* snap_src; int64_t src_anchor, src_cap;
+    uint8_t* out_dst; int64_t dst_anchor, dst_cap;
+    const uint8_t* host_image; int64_t host_unit0;
+} oracle_param_job;
+
+int64_t oracle_apply_param_jobs(const oracle_param_job* jobs, int64_t n_jobs) {
+    int64_t written = 0;
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : written)
+    for (int64_t j = 0; j < n_jobs; ++j) {
+        const oracle_param_job* q = &jobs[j];
+        written += oracle_apply_param_task((int)q->kind, q->begin, q->end, q->unit_bytes, q->snap_src, q->src_anchor, q->src_cap,
+                                           q->out_dst, q->dst_anchor, q->dst_cap, q->host_image, q->host_unit0);
+    }
+    return written;
+}
+
+typedef struct {
+    int64_t kind, h_begin, h_end, layout, n_layers, n_blocks, block_size, head_cap, frag_bytes;
+    const uint8_t* snap_src; int64_t src_anchor;
+    uint8_t* out_dst; int64_t dst_anchor;
+    const uint8_t* host_backup; int64_t host_heads, host_head0;
+    const int32_t* old_ids; const int32_t* new_ids; int64_t n_pairs;
+} oracle_kv_job;
+
+int64_t oracle_apply_kv_jobs(const oracle_kv_job* jobs, int64_t n_jobs) {
+    int64_t written = 0;
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : written)
+    for (int64_t j = 0; j < n_jobs; ++j) {
+        const oracle_kv_job* q = &jobs[j];
+        written += oracle_apply_kv_task((int)q->kind, q->h_begin, q->h_end, (int)q->layout, q->n_layers, q->n_blocks, q->block_size,
+                                        q->head_cap, q->frag_bytes, q->snap_src, q->src_anchor, q->out_dst, q->dst_anchor,
+                                        q->host_backup, q->host_heads, q->host_head0, q->old_ids, q->new_ids, q->n_pairs);
+    }
+    return written;
+}

@@ -3,7 +3,8 @@
 PAPER.md:45, :92-94 — ETP shards "attention and linear layers" with unequal widths; a correct resharded
 state must compute the same layer output as the unsharded weight.  This is the textbook definition
 (no sharding, no blocking); numpy's matmul is the library routine, pinned against an explicit triple loop
-in tests/test_oracle_linear.py.
+in tests/test_oracle_state.py::test_linear_ref_is_the_textbook_definition (decode16 against torch in
+::test_decode16_exact, the MoE layer in ::test_moe_route_hand_worked / ::test_moe_ref_special_cases).
 """
 from __future__ import annotations
 

@@ -21,27 +21,53 @@ _SRC = os.path.join(_HERE, "etp_apply.c")
 _lib_handle = None
 
 
-def build(force: bool = False) -> str:
-    """gcc -O2, no intrinsics.  (Building the checker is not using it.)"""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-Wall", "-shared", "-fPIC", "-o", _SO, _SRC])
-    return _SO
+_SO_OMP = os.path.join(_HERE, "libetp_oracle_omp.so")
+_lib_omp_handle = None
+
+
+def build(force: bool = False, omp: bool = False) -> str:
+    """gcc -O2, no intrinsics.  (Building the checker is not using it.)  ``omp``: the same file with -fopenmp, for the
+    all-cores leg of the CPU baseline."""
+    so = _SO_OMP if omp else _SO
+    if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-Wall", "-shared", "-fPIC"] + (["-fopenmp"] if omp else []) + ["-o", so, _SRC])
+    return so
+
+
+def _declare(L):
+    i64, p, i32 = ctypes.c_int64, ctypes.c_void_p, ctypes.c_int
+    L.oracle_slot.restype = i64
+    L.oracle_slot.argtypes = [i64, i64, i64]
+    L.oracle_apply_param_task.restype = i64
+    L.oracle_apply_param_task.argtypes = [i32, i64, i64, i64, p, i64, i64, p, i64, i64, p, i64]
+    L.oracle_apply_kv_task.restype = i64
+    L.oracle_apply_kv_task.argtypes = [i32, i64, i64, i32, i64, i64, i64, i64, i64,
+                                       p, i64, p, i64, p, i64, i64, p, p, i64]
+    L.oracle_threads.restype = i32
+    L.oracle_apply_param_jobs.restype = i64
+    L.oracle_apply_param_jobs.argtypes = [p, i64]
+    L.oracle_apply_kv_jobs.restype = i64
+    L.oracle_apply_kv_jobs.argtypes = [p, i64]
+    return L
 
 
 def _lib():
     global _lib_handle
     if _lib_handle is None:
-        L = ctypes.CDLL(build())
-        i64, p, i32 = ctypes.c_int64, ctypes.c_void_p, ctypes.c_int
-        L.oracle_slot.restype = i64
-        L.oracle_slot.argtypes = [i64, i64, i64]
-        L.oracle_apply_param_task.restype = i64
-        L.oracle_apply_param_task.argtypes = [i32, i64, i64, i64, p, i64, i64, p, i64, i64, p, i64]
-        L.oracle_apply_kv_task.restype = i64
-        L.oracle_apply_kv_task.argtypes = [i32, i64, i64, i32, i64, i64, i64, i64, i64,
-                                           p, i64, p, i64, p, i64, i64, p, p, i64]
-        _lib_handle = L
+        _lib_handle = _declare(ctypes.CDLL(build()))
     return _lib_handle
+
+
+def _lib_omp():
+    global _lib_omp_handle
+    if _lib_omp_handle is None:
+        _lib_omp_handle = _declare(ctypes.CDLL(build(omp=True)))
+    return _lib_omp_handle
+
+
+def omp_threads() -> int:
+    """Threads the all-cores leg runs on (omp_get_max_threads of the -fopenmp build)."""
+    return int(_lib_omp().oracle_threads())
 
 
 def _ptr(a: Optional[np.ndarray]):
@@ -214,3 +240,93 @@ def kv_fragment(pool: np.ndarray, g: KVGeom, anchor: int, l: int, c: int, block:
     sl = slot(head, anchor, g.head_cap if heads is None else heads)
     o = g.frag_off(l, c, block, t, sl, heads)
     return pool[o:o + g.frag_bytes]
+
+
+# ----------------------------------------------------------------------------- all-cores leg (SURVEY.md 8(d) "Oracle timing")
+_PARAM_JOB = np.dtype([(n, np.int64) for n in ("kind", "begin", "end", "unit_bytes", "snap_src", "src_anchor", "src_cap",
+                                                "out_dst", "dst_anchor", "dst_cap", "host_image", "host_unit0")])
+_KV_JOB = np.dtype([(n, np.int64) for n in ("kind", "h_begin", "h_end", "layout", "n_layers", "n_blocks", "block_size", "head_cap",
+                                             "frag_bytes", "snap_src", "src_anchor", "out_dst", "dst_anchor", "host_backup",
+                                             "host_heads", "host_head0", "old_ids", "new_ids", "n_pairs")])
+
+
+def _addr(a: Optional[np.ndarray]) -> int:
+    if a is None:
+        return 0
+    assert a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data
+
+
+def apply_params_parallel(items, job_bytes: int = 4 << 20):
+    """The same plan application as ``apply_params`` for a LIST of tensors at once, with the element-by-element loops of
+    etp_apply.c run from an OpenMP ``parallel for`` over jobs (one job = a task, cut into unit sub-ranges of about
+    ``job_bytes`` so the loop balances).  items: [(tasks, snap, geom, unit_bytes, host_image, host_unit0)].
+    Returns ([out slabs per item], byte counters)."""
+    L = _lib_omp()
+    outs, jobs = [], []
+    stats = {"d2d_bytes": 0, "h2d_bytes": 0, "kept_bytes": 0}
+    for (tasks, snap, geom, unit_bytes, host_image, host_unit0) in items:
+        out = {r: a.copy() for r, a in snap.items()}
+        outs.append(out)
+        step = max(1, job_bytes // unit_bytes)
+        for (kind, src, dst, b, e) in tasks:
+            if kind == KEEP:
+                stats["kept_bytes"] += (e - b) * unit_bytes
+                continue
+            da, dc = geom[dst]
+            assert e - b <= dc
+            if kind == TRANSFER:
+                sa, sc = geom[src]
+                row = (TRANSFER, 0, 0, unit_bytes, _addr(snap[src]), sa, sc, _addr(out[dst]), da, dc, 0, 0)
+                stats["d2d_bytes"] += (e - b) * unit_bytes
+            else:
+                assert host_image is not None and host_unit0 <= b and (e - host_unit0) * unit_bytes <= host_image.size
+                row = (RELOAD, 0, 0, unit_bytes, 0, 0, 1, _addr(out[dst]), da, dc, _addr(host_image), host_unit0)
+                stats["h2d_bytes"] += (e - b) * unit_bytes
+            for u in range(b, e, step):
+                jobs.append(row[:1] + (u, min(e, u + step)) + row[3:])
+    arr = np.array(jobs, dtype=_PARAM_JOB) if jobs else np.zeros(0, dtype=_PARAM_JOB)
+    n = L.oracle_apply_param_jobs(arr.ctypes.data_as(ctypes.c_void_p), len(jobs))
+    assert n == stats["d2d_bytes"] + stats["h2d_bytes"]
+    return outs, stats
+
+
+def apply_kv_parallel(head_tasks: Sequence[Task], snap: Dict[int, np.ndarray], anchors: Dict[int, int], g: KVGeom,
+                      host_backup: Optional[np.ndarray], host_heads: int, host_head0: int,
+                      pairs: Sequence[Tuple[int, int, int, int]], pairs_per_job: int = 64):
+    """``apply_kv`` with the live blocks of every head task cut into jobs of ``pairs_per_job`` blocks, run from the
+    OpenMP parallel for of etp_apply.c (distinct live blocks have distinct new ids, so jobs write disjoint bytes)."""
+    L = _lib_omp()
+    out = {r: a.copy() for r, a in snap.items()}
+    old_ids = np.ascontiguousarray([p[2] for p in pairs], dtype=np.int32)
+    new_ids = np.ascontiguousarray([p[3] for p in pairs], dtype=np.int32)
+    stats = {"d2d_bytes": 0, "h2d_bytes": 0, "kept_bytes": 0}
+    per_head_live = len(pairs) * g.n_layers * 2 * g.block_size * g.frag_bytes
+    jobs, kinds = [], []
+    for (kind, src, dst, b, e) in head_tasks:
+        if kind == RELOAD and host_backup is None:
+            continue
+        if kind == RELOAD:
+            assert host_head0 <= b and e <= host_head0 + host_heads
+            s_ptr, s_anchor, hb = 0, 0, _addr(host_backup)
+        else:
+            s_ptr, s_anchor, hb = _addr(snap[dst if kind == KEEP else src]), anchors[dst if kind == KEEP else src], 0
+        if kind == KEEP:
+            stats["kept_bytes"] += per_head_live * (e - b)
+        for p0 in range(0, len(pairs), pairs_per_job):
+            n = min(pairs_per_job, len(pairs) - p0)
+            jobs.append((kind, b, e, g.layout, g.n_layers, g.n_blocks, g.block_size, g.head_cap, g.frag_bytes, s_ptr, s_anchor,
+                         _addr(out[dst]), anchors[dst], hb, host_heads, host_head0, old_ids.ctypes.data + 4 * p0,
+                         new_ids.ctypes.data + 4 * p0, n))
+            kinds.append(kind)
+    # per-kind byte counters need per-kind totals: run the kinds one after the other (three parallel loops)
+    for kind, key in ((KEEP, "d2d_bytes"), (TRANSFER, "d2d_bytes"), (RELOAD, "h2d_bytes")):
+        sel = [j for j, k in zip(jobs, kinds) if k == kind]
+        if not sel:
+            continue
+        arr = np.array(sel, dtype=_KV_JOB)
+        n = L.oracle_apply_kv_jobs(arr.ctypes.data_as(ctypes.c_void_p), len(sel))
+        stats[key] += n
+        if kind == KEEP:
+            stats["kept_bytes"] -= n
+    return out, stats

@@ -44,6 +44,32 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return SO
 
 
+def kernel_sass_sha(pattern: str = "etp_interval_copy_kernel", so: str = SO) -> str:
+    """sha256 (first 16 hex digits) of the SASS instruction text of every function of the built library whose mangled name
+    contains ``pattern`` (cuobjdump -sass; addresses and encodings stripped).  It stamps an ncu capture with the exact
+    kernel it profiled: bench.py reports it beside ``roofline.traffic`` and a CPU test fails when the built kernel no longer
+    matches the capture under profiles/."""
+    import hashlib
+    import re
+    cuobjdump = os.path.join(os.path.dirname(NVCC), "cuobjdump")
+    out = subprocess.run([cuobjdump, "-sass", so], stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True, check=True).stdout
+    h = hashlib.sha256()
+    take, n = False, 0
+    ins = re.compile(r"^\s*/\*[0-9a-f]{4,}\*/\s+(.*?;)")
+    for line in out.splitlines():
+        if "Function :" in line:
+            take = pattern in line
+            continue
+        if take:
+            m = ins.match(line)
+            if m:
+                h.update(" ".join(m.group(1).split()).encode() + b"\n")
+                n += 1
+    if n == 0:
+        raise RuntimeError(f"no SASS found for a function matching {pattern!r} in {so}")
+    return h.hexdigest()[:16]
+
+
 if __name__ == "__main__":
     import sys
     print(build(force=True, verbose="-v" in sys.argv))

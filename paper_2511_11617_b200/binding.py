@@ -20,8 +20,8 @@ PLAN_CMM, PLAN_GREEDY, PLAN_FULL_RELOAD, PLAN_MIGRATION_AWARE = 0, 1, 2, 3
 COL_PARALLEL, ROW_PARALLEL = 0, 1
 DTYPE = {"bf16": 0, "fp16": 1}
 KV_TOKEN_MAJOR, KV_HEAD_MAJOR = 0, 1
-(OPT_SKIP_D2D, OPT_SKIP_RELOAD, OPT_TMA_MIN_BYTES, OPT_LDG_STEALS_BULK, OPT_RELOAD_CHUNK_BYTES, OPT_KV_RELOAD_MODE,
- OPT_GRID_CTAS, OPT_GATHER_CTAS, OPT_TIME_KERNELS, OPT_LINEAR_CTA_PAIR) = range(10)
+(OPT_SKIP_D2D, OPT_SKIP_RELOAD, OPT_TMA_MIN_BYTES, OPT_LDG_STEALS_BULK, OPT_RELOAD_CHUNK_BYTES, OPT_RESERVED_5,
+ OPT_GRID_CTAS, OPT_GATHER_CTAS, OPT_TIME_KERNELS, OPT_LINEAR_CTA_PAIR, OPT_VALIDATE_INTERVALS) = range(11)
 
 
 class EtpError(RuntimeError):
@@ -225,7 +225,7 @@ def etp_page_table_rewrite(table, seq_lens, last_use, block_size: int, budget: i
 
 # ------------------------------------------------------------------------------------------------ device calls
 class Context:
-    """Owns an etp_ctx (descriptor arenas, staging ring, events) on one CUDA device."""
+    """Owns an etp_ctx (descriptor arenas, events) on one CUDA device."""
 
     def __init__(self, device: int = 0, staging_bytes: int = 0):
         h = vp()

@@ -11,7 +11,7 @@ using namespace etp;
 
 namespace {
 constexpr int kArenaSlots = 2;
-constexpr int kCounterSlots = 256;   // pairs of work-queue heads available to one call
+constexpr int kCounterSlots = 256;   // pairs of work-queue heads available to one call (they live in the call's arena slot)
 
 struct ArenaSlot {
     void* h = nullptr;
@@ -53,16 +53,14 @@ extern "C" etp_status etp_ctx_create(int device, int64_t staging_bytes, etp_ctx*
     c->opts[ETP_OPT_TMA_MIN_BYTES] = 32768;
     c->opts[ETP_OPT_LDG_STEALS_BULK] = 0;
     c->opts[ETP_OPT_RELOAD_CHUNK_BYTES] = 64 << 20;
-    c->opts[ETP_OPT_KV_RELOAD_MODE] = 0;
     c->opts[ETP_OPT_GRID_CTAS] = 0;
     c->opts[ETP_OPT_GATHER_CTAS] = 16;
     c->opts[ETP_OPT_LINEAR_CTA_PAIR] = 1;
-    c->staging_bytes = staging_bytes ? staging_bytes : (int64_t(256) << 20);
+    c->opts[ETP_OPT_VALIDATE_INTERVALS] = 1;
     CtxExtra* x = new (std::nothrow) CtxExtra();
     if (!x) { delete c; ETP_FAIL(ETP_ERR_NOMEM, "etp_ctx_create: out of memory"); }
     c->impl = x;
-    cudaError_t e = cudaMalloc(&c->d_counters, sizeof(unsigned int) * 2 * kCounterSlots);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&x->uploaded, cudaEventDisableTiming);
+    cudaError_t e = cudaEventCreateWithFlags(&x->uploaded, cudaEventDisableTiming);
     for (int i = 0; i < kArenaSlots && e == cudaSuccess; ++i) {
         e = cudaEventCreateWithFlags(&x->slot[i].done_copy, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&x->slot[i].done_reload, cudaEventDisableTiming);
@@ -73,7 +71,6 @@ extern "C" etp_status etp_ctx_create(int device, int64_t staging_bytes, etp_ctx*
         etp_ctx_destroy(c);
         return ETP_ERR_CUDA;
     }
-    c->n_counter_slots = kCounterSlots;
     *out = c;
     return ETP_OK;
 }
@@ -95,8 +92,6 @@ extern "C" void etp_ctx_destroy(etp_ctx* c) {
     }
     for (cudaEvent_t e : c->events) cudaEventDestroy(e);
     for (cudaEvent_t e : c->tev) cudaEventDestroy(e);
-    if (c->d_counters) cudaFree(c->d_counters);
-    if (c->d_staging) cudaFree(c->d_staging);
     if (c->lin_ws) cudaFree(c->lin_ws);
     if (c->lin_tickets) cudaFree(c->lin_tickets);
     if (c->moe_items) cudaFree(c->moe_items);
@@ -155,15 +150,20 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
     w->phases.resize(n_ph);
     w->host_gather.resize(n_ph);
 
-    // ---- descriptor arena layout: pairs | per phase: bulk segs, bulk items, vec segs, vec items, small segs, batch starts,
-    //      gather segs, gather items
+    // ---- descriptor arena layout: work-queue heads (zero) | pairs | per phase: bulk segs, bulk items, vec segs, vec items,
+    //      small segs, batch starts, gather segs, gather items.  The queue heads travel with the descriptors, so the
+    //      done_copy / done_reload events that guard an arena slot also guard its counters: a call whose zero-copy gather is
+    //      still queued behind GBs of DMA on the reload stream cannot have its heads reset by the next call.
     int64_t total = 0, n_jobs = 0, n_items = 0;
     auto pad = [](int64_t b) { return (b + 255) & ~int64_t(255); };
     struct Off { int64_t bulk, bulk_items, vec, vec_items, small, small_first, gat, gat_items; };
     std::vector<Off> off(n_ph);
-    const int64_t off_pairs = 0;
-    total += pad((int64_t)w->pairs.size() * sizeof(int32_t));
     int launches_needed = 0;
+    for (size_t p = 0; p < n_ph; ++p) launches_needed += (!w->phases[p].empty()) + (!w->host_gather[p].vec.empty());
+    const int64_t off_counters = 0;
+    total += pad((int64_t)launches_needed * 2 * sizeof(unsigned int));
+    const int64_t off_pairs = total;
+    total += pad((int64_t)w->pairs.size() * sizeof(int32_t));
     for (size_t p = 0; p < n_ph; ++p) {
         const JobList &jl = w->phases[p], &gl = w->host_gather[p];
         off[p].bulk = total;        total += pad((int64_t)jl.bulk.size() * sizeof(BulkSeg));
@@ -176,12 +176,11 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
         off[p].gat_items = total;   total += pad((int64_t)gl.n_vec_items * sizeof(uint32_t));
         n_jobs += (int64_t)(jl.bulk.size() + jl.vec.size() + jl.small.size() + gl.vec.size());
         n_items += (int64_t)jl.n_bulk_items + jl.n_vec_items + (int64_t)jl.small_first.size() + gl.n_vec_items;
-        launches_needed += (!jl.empty()) + (!gl.vec.empty());
         if (jl.bulk.size() >= 0xFFFFFFF0ull || jl.vec.size() >= 0xFFFFFFF0ull || jl.small.size() >= 0xFFFFFFF0ull ||
             gl.vec.size() >= 0xFFFFFFF0ull || (uint64_t)jl.n_vec_items + jl.small_first.size() >= 0xFFFFFFF0ull)
             ETP_FAIL(ETP_ERR_CAPACITY, "too many segments in one phase");
     }
-    if (launches_needed > c->n_counter_slots) ETP_FAIL(ETP_ERR_CAPACITY, "plan needs %d launches > %d", launches_needed, c->n_counter_slots);
+    if (launches_needed > kCounterSlots) ETP_FAIL(ETP_ERR_CAPACITY, "plan needs %d launches > %d", launches_needed, kCounterSlots);
 
     // item table: the segment index of every work item, one fill per segment
     auto fill_items = [](uint32_t* items, uint32_t n_items_total, const uint32_t* firsts, size_t n_segs, size_t stride) {
@@ -213,6 +212,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
             slot->bytes = want;
         }
         char* h = (char*)slot->h;
+        std::memset(h + off_counters, 0, (size_t)launches_needed * 2 * sizeof(unsigned int));
         if (!w->pairs.empty()) std::memcpy(h + off_pairs, w->pairs.data(), w->pairs.size() * sizeof(int32_t));
         for (size_t p = 0; p < n_ph; ++p) {
             const JobList &jl = w->phases[p], &gl = w->host_gather[p];
@@ -236,7 +236,6 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
             }
         }
         d_base = (char*)slot->d;
-        ETP_CUDA_OK(cudaMemsetAsync(c->d_counters, 0, sizeof(unsigned int) * 2 * launches_needed, cs));
         ETP_CUDA_OK(cudaMemcpyAsync(d_base, h, total, cudaMemcpyHostToDevice, cs));
         ETP_CUDA_OK(cudaEventRecord(x->uploaded, cs));
     }
@@ -269,7 +268,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
             a.small = (const SmallSeg*)(d_base + off[p].small);
             a.small_first = (const uint32_t*)(d_base + off[p].small_first);
             a.n_small_batches = (unsigned int)jl.small_first.size();
-            a.counters = c->d_counters + 2 * counter_slot;
+            a.counters = (unsigned int*)(d_base + off_counters) + 2 * counter_slot;
             a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
             if (timed) {
                 while ((int)c->tev.size() < 2 * (c->n_timed + 1)) {
@@ -331,7 +330,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
                 a.small_first = nullptr;
                 a.n_small_batches = 0;
                 a.n_vec_items = gl.n_vec_items;
-                a.counters = c->d_counters + 2 * counter_slot;
+                a.counters = (unsigned int*)(d_base + off_counters) + 2 * counter_slot;
                 a.flags = 0;
                 const int ggrid = (int)std::max<int64_t>(1, std::min<int64_t>(c->opts[ETP_OPT_GATHER_CTAS], c->n_sms));
                 launch_copy_kernel(a, ggrid, rs);
@@ -381,38 +380,51 @@ extern "C" etp_status etp_reshard_kv(etp_ctx* ctx, const etp_kv_geometry* geom, 
     if (new_block_budget < 0 || new_block_budget > geom->n_blocks)
         ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: budget %d outside [0, n_blocks=%d]", new_block_budget, geom->n_blocks);
     if (head_plan->total_units < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: empty head plan");
-    // validate before touching the caller's table
+    if (geom->block_size < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: block_size %d < 1", geom->block_size);
+    if (pt->n_seqs < 0 || pt->max_blocks < 0 || (pt->n_seqs > 0 && (!pt->block_table || !pt->seq_lens || !pt->last_use)))
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: bad page table");
+    // Nothing of the caller's is written before the whole call is known to succeed: the page-table rule runs on a PRIVATE
+    // copy of the table, the plan is lowered (geometry, capacity, backup range, alignment, hazard analysis) against it, and
+    // only then are the new table and the eviction list copied out and the work enqueued.
     int64_t max_pairs = 0;
     for (int32_t s = 0; s < pt->n_seqs; ++s) {
-        if (!pt->seq_lens) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: seq_lens is NULL");
-        max_pairs += (pt->seq_lens[s] + geom->block_size - 1) / std::max(geom->block_size, 1);
-    }
-    for (int32_t s = 0; s < pt->n_seqs; ++s)
-        for (int32_t i = 0; i < (pt->seq_lens[s] + geom->block_size - 1) / geom->block_size && i < pt->max_blocks; ++i) {
+        if (pt->seq_lens[s] < 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: negative seq_len");
+        const int32_t need = (pt->seq_lens[s] + geom->block_size - 1) / geom->block_size;
+        max_pairs += need;
+        for (int32_t i = 0; i < need && i < pt->max_blocks; ++i) {
             const int32_t b = pt->block_table[(int64_t)s * pt->max_blocks + i];
             if (b >= geom->n_blocks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_kv: block id %d >= n_blocks %d", b, geom->n_blocks);
         }
+    }
+    const size_t table_n = (size_t)pt->n_seqs * (size_t)pt->max_blocks;
+    std::vector<int32_t> table(pt->block_table, pt->block_table + table_n);
+    etp_page_table priv = *pt;
+    priv.block_table = table.data();
     std::vector<int32_t> pairs((size_t)std::max<int64_t>(max_pairs, 1) * 2);
     std::vector<int32_t> ev((size_t)std::max(pt->n_seqs, 1));
     int64_t n_pairs = 0;
     int32_t n_ev = 0;
-    ETP_TRY(etp_page_table_rewrite(pt, geom->block_size, new_block_budget, ev.data(), &n_ev, pairs.data(), max_pairs, &n_pairs));
+    ETP_TRY(etp_page_table_rewrite(&priv, geom->block_size, new_block_budget, ev.data(), &n_ev, pairs.data(), max_pairs, &n_pairs));
     bool needs_backup = false;
     for (const etp_task& t : head_plan->tasks) needs_backup = needs_backup || (t.kind == ETP_RELOAD && t.begin < t.end);
     if (needs_backup && !geom->host_backup) {
-        // reading K4: without a backup the reloaded heads stay missing; every surviving sequence is reported too
+        // reading K4: without a backup the reloaded heads stay missing, so every surviving sequence is reported too.  Their
+        // rows stay mapped and their TRANSFER / relocated heads are still moved: the surviving heads are valid where the new
+        // table says, and a replay (out of scope) would only have to refill the missing heads.
         std::vector<char> gone((size_t)std::max(pt->n_seqs, 1), 0);
         for (int32_t i = 0; i < n_ev; ++i) gone[ev[i]] = 1;
         for (int32_t s = 0; s < pt->n_seqs; ++s)
             if (!gone[s] && pt->seq_lens[s] > 0) ev[n_ev++] = s;
     }
-    *n_evicted = n_ev;
-    if (evicted_seqs_out)
-        for (int32_t i = 0; i < n_ev; ++i) evicted_seqs_out[i] = ev[i];
     LoweredWork w;
     ETP_TRY(lower_kv(ctx, geom, head_plan, pairs.data(), n_pairs, &w));
     w.rep.lower_ms = now_ms() - t0;
-    return execute(ctx, &w, copy_stream, reload_stream, report);
+    ETP_TRY(execute(ctx, &w, copy_stream, reload_stream, report));   // capacity checks come before its first enqueue
+    if (table_n) std::memcpy(pt->block_table, table.data(), table_n * sizeof(int32_t));
+    *n_evicted = n_ev;
+    if (evicted_seqs_out)
+        for (int32_t i = 0; i < n_ev; ++i) evicted_seqs_out[i] = ev[i];
+    return ETP_OK;
 }
 
 extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_descs, int64_t n, void* stream,
@@ -431,6 +443,37 @@ extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_
             ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_copy_intervals: interval %lld is not 16-byte aligned", (long long)i);
         push_contiguous(ctx, &w.phases[0], d.src, d.dst, d.bytes);
         w.rep.d2d_bytes += d.bytes;
+    }
+    if (ctx->opts[ETP_OPT_VALIDATE_INTERVALS]) {
+        // the contract of include/etp.h: destinations mutually disjoint and disjoint from every source (one launch, no order
+        // between intervals).  Sort both sides by start address, then one sweep each.
+        struct Iv { uint64_t b, e; int64_t i; };
+        std::vector<Iv> dst, src;
+        dst.reserve((size_t)n);
+        src.reserve((size_t)n);
+        for (int64_t i = 0; i < n; ++i) {
+            const etp_interval& d = host_descs[i];
+            if (d.bytes == 0) continue;
+            dst.push_back({(uint64_t)(uintptr_t)d.dst, (uint64_t)(uintptr_t)d.dst + (uint64_t)d.bytes, i});
+            src.push_back({(uint64_t)(uintptr_t)d.src, (uint64_t)(uintptr_t)d.src + (uint64_t)d.bytes, i});
+        }
+        auto by_start = [](const Iv& a, const Iv& b) { return a.b < b.b; };
+        std::sort(dst.begin(), dst.end(), by_start);
+        std::sort(src.begin(), src.end(), by_start);
+        for (size_t k = 1; k < dst.size(); ++k)
+            if (dst[k].b < dst[k - 1].e)
+                ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: destinations of intervals %lld and %lld overlap", (long long)dst[k - 1].i, (long long)dst[k].i);
+        size_t si = 0;
+        uint64_t src_reach = 0;   // largest end among the sources that start below the current destination's end
+        int64_t src_reach_i = -1;
+        for (const Iv& d : dst) {   // destinations are disjoint and ascending, so one forward pass over the sources suffices
+            while (si < src.size() && src[si].b < d.e) {
+                if (src[si].e > src_reach) { src_reach = src[si].e; src_reach_i = src[si].i; }
+                ++si;
+            }
+            if (src_reach > d.b)
+                ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: destination of interval %lld overlaps the source of interval %lld", (long long)d.i, (long long)src_reach_i);
+        }
     }
     w.rep.n_phases = 1;
     w.rep.lower_ms = now_ms() - t0;

@@ -120,10 +120,6 @@ struct etp_ctx {
     int n_sms = 0;
     int64_t opts[ETP_OPT__COUNT];
     void* impl = nullptr;               // executor state (descriptor arenas, events), etp_exec.cu
-    unsigned int* d_counters = nullptr; // work-queue heads (device), one pair per kernel launch of a call
-    int n_counter_slots = 0;
-    void* d_staging = nullptr;          // staging ring of the KV reload pipeline (allocated on first use)
-    int64_t staging_bytes = 0;
     std::vector<cudaEvent_t> events;    // hazard-phase events
     int32_t launches = 0;               // kernels launched by the last call
     std::vector<cudaEvent_t> tev;       // timing events (pairs) around copy-stream launches, ETP_OPT_TIME_KERNELS

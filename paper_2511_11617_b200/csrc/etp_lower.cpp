@@ -4,6 +4,7 @@
 // boundaries, range reads of only the needed byte intervals); layout contract: DESIGN.md readings L1-L7, K1-K6.
 #include <algorithm>
 #include <cstring>
+#include <map>
 
 #include "etp_internal.h"
 
@@ -84,30 +85,63 @@ struct Range {
     int32_t rank;
     int64_t b, e;  // slots
 };
-inline bool hits(const Range& a, const Range& b) { return a.rank == b.rank && a.b < b.e && b.b < a.e; }
 
 // Hazard phases (reading L4): task k must run after every task j that READS bytes k OVERWRITES.
 // phase(k) = 0 if nothing reads what k writes, else 1 + max phase of those readers.  A cycle is unsupported.
+// Cost: the read ranges are sorted per rank with a running maximum of their ends, every write range finds its readers
+// with one binary search and a backward scan that stops as soon as no earlier read can reach it (reads of one plan are
+// disjoint, so that is the readers themselves), then one longest-path sweep in topological order:
+// O((R + W) log R + edges) for R read and W write ranges, instead of testing every pair of tasks in every round.
 etp_status assign_phases(const std::vector<std::vector<Range>>& reads, const std::vector<std::vector<Range>>& writes,
                          std::vector<int32_t>* phase) {
     const size_t n = reads.size();
     phase->assign(n, 0);
-    for (size_t round = 0; round <= n; ++round) {
-        bool changed = false;
-        for (size_t k = 0; k < n; ++k)
-            for (size_t j = 0; j < n; ++j) {
-                if (j == k) continue;
-                bool dep = false;
-                for (const Range& w : writes[k])
-                    for (const Range& r : reads[j]) dep = dep || hits(w, r);
-                if (dep && (*phase)[k] < (*phase)[j] + 1) {
-                    (*phase)[k] = (*phase)[j] + 1;
-                    changed = true;
-                }
+    struct Rd { int32_t rank; int64_t b, e; uint32_t task; int64_t max_e; };
+    std::vector<Rd> rd;
+    for (size_t j = 0; j < n; ++j)
+        for (const Range& r : reads[j])
+            if (r.b < r.e) rd.push_back({r.rank, r.b, r.e, (uint32_t)j, 0});
+    if (rd.empty()) return ETP_OK;
+    std::sort(rd.begin(), rd.end(), [](const Rd& a, const Rd& b) { return a.rank != b.rank ? a.rank < b.rank : a.b < b.b; });
+    for (size_t i = 0; i < rd.size(); ++i)
+        rd[i].max_e = (i > 0 && rd[i - 1].rank == rd[i].rank) ? std::max(rd[i - 1].max_e, rd[i].e) : rd[i].e;
+    // edges reader j -> writer k
+    std::vector<std::pair<uint32_t, uint32_t>> edges;
+    for (size_t k = 0; k < n; ++k)
+        for (const Range& w : writes[k]) {
+            if (w.b >= w.e) continue;
+            // first read (rank, begin) >= (w.rank, w.e): everything before it on this rank begins below w.e
+            size_t hi = std::lower_bound(rd.begin(), rd.end(), w, [](const Rd& a, const Range& w) {
+                            return a.rank != w.rank ? a.rank < w.rank : a.b < w.e;
+                        }) - rd.begin();
+            while (hi > 0 && rd[hi - 1].rank == w.rank && rd[hi - 1].max_e > w.b) {
+                const Rd& r = rd[hi - 1];
+                if (r.e > w.b && r.task != k) edges.push_back({r.task, (uint32_t)k});
+                --hi;
             }
-        if (!changed) return ETP_OK;
+        }
+    if (edges.empty()) return ETP_OK;
+    std::sort(edges.begin(), edges.end());
+    edges.erase(std::unique(edges.begin(), edges.end()), edges.end());
+    std::vector<uint32_t> first(n + 1, 0), indeg(n, 0);
+    for (const auto& e : edges) { ++first[e.first + 1]; ++indeg[e.second]; }
+    for (size_t i = 0; i < n; ++i) first[i + 1] += first[i];
+    std::vector<uint32_t> ready;
+    for (size_t i = 0; i < n; ++i)
+        if (!indeg[i]) ready.push_back((uint32_t)i);
+    size_t done = 0;
+    while (!ready.empty()) {
+        const uint32_t j = ready.back();
+        ready.pop_back();
+        ++done;
+        for (uint32_t x = first[j]; x < first[j + 1]; ++x) {
+            const uint32_t k = edges[x].second;
+            (*phase)[k] = std::max((*phase)[k], (*phase)[j] + 1);
+            if (--indeg[k] == 0) ready.push_back(k);
+        }
     }
-    ETP_FAIL(ETP_ERR_UNSUPPORTED, "cyclic write-after-read hazard between tasks (needs a bounce buffer)");
+    if (done != n) ETP_FAIL(ETP_ERR_UNSUPPORTED, "cyclic write-after-read hazard between tasks (needs a bounce buffer)");
+    return ETP_OK;
 }
 
 JobList& phase_list(std::vector<JobList>& v, int32_t p) {
@@ -122,6 +156,7 @@ etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n
     if (n_tensors < 0 || n_plans < 0 || (n_tensors > 0 && (!tensors || !plans)))
         ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_reshard_params: NULL tensors/plans");
     std::vector<SlotRun> runs;
+    std::map<std::vector<int64_t>, std::vector<int32_t>> phase_cache;
     int32_t max_phase = 0;
     for (int32_t t = 0; t < n_tensors; ++t) {
         const etp_tensor& T = tensors[t];
@@ -148,27 +183,44 @@ etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n
         MemKind image_kind = MEM_HOST_PAGEABLE;
         bool image_checked = false;
 
-        // read / write slot ranges per task for the hazard analysis
+        // read / write slot ranges per task for the hazard analysis.  Slot ranges are in UNITS, so every tensor of a
+        // granularity class with the same per-rank (anchor, cap) shares one phase vector (config 2: 4 analyses, not 282).
         const size_t nt = P.tasks.size();
-        std::vector<std::vector<Range>> reads(nt), writes(nt);
+        std::vector<int64_t> key;
+        key.reserve(2 + 2 * (size_t)T.n_ranks);
+        key.push_back(T.plan_index);
+        key.push_back(T.n_ranks);
+        for (int32_t r = 0; r < T.n_ranks; ++r) {
+            key.push_back(T.slabs[r].base ? T.slabs[r].anchor_unit : 0);
+            key.push_back(T.slabs[r].base ? T.slabs[r].cap_units : 0);
+        }
         for (size_t k = 0; k < nt; ++k) {
             const etp_task& K = P.tasks[k];
-            if (K.kind == ETP_KEEP || K.begin >= K.end) continue;
-            const etp_slab* D = slab_of(K.dst_rank);
-            const etp_slab* S = K.kind == ETP_TRANSFER ? slab_of(K.src_rank) : nullptr;
-            if (K.kind == ETP_TRANSFER) {
-                if (!S || !S->base || S->cap_units < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "tensor %d: no slab for source rank %d", t, K.src_rank);
-                if ((uintptr_t)S->base % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "tensor %d rank %d: slab base not 16-byte aligned", t, K.src_rank);
-                if (K.end - K.begin > S->cap_units) ETP_FAIL(ETP_ERR_CAPACITY, "tensor %d: transfer wider than the source slab", t);
-            }
-            slot_runs(K.begin, K.end, S ? S->anchor_unit : 0, S ? S->cap_units : 0, D->anchor_unit, D->cap_units, &runs);
-            for (const SlotRun& r : runs) {
-                writes[k].push_back({K.dst_rank, r.dst_slot, r.dst_slot + r.count});
-                if (S) reads[k].push_back({K.src_rank, r.src_slot, r.src_slot + r.count});
-            }
+            if (K.kind != ETP_TRANSFER || K.begin >= K.end) continue;
+            const etp_slab* S = slab_of(K.src_rank);
+            if (!S || !S->base || S->cap_units < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "tensor %d: no slab for source rank %d", t, K.src_rank);
+            if ((uintptr_t)S->base % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "tensor %d rank %d: slab base not 16-byte aligned", t, K.src_rank);
+            if (K.end - K.begin > S->cap_units) ETP_FAIL(ETP_ERR_CAPACITY, "tensor %d: transfer wider than the source slab", t);
         }
-        std::vector<int32_t> phase;
-        ETP_TRY(assign_phases(reads, writes, &phase));
+        auto hit = phase_cache.find(key);
+        if (hit == phase_cache.end()) {
+            std::vector<std::vector<Range>> reads(nt), writes(nt);
+            for (size_t k = 0; k < nt; ++k) {
+                const etp_task& K = P.tasks[k];
+                if (K.kind == ETP_KEEP || K.begin >= K.end) continue;
+                const etp_slab* D = slab_of(K.dst_rank);
+                const etp_slab* S = K.kind == ETP_TRANSFER ? slab_of(K.src_rank) : nullptr;
+                slot_runs(K.begin, K.end, S ? S->anchor_unit : 0, S ? S->cap_units : 0, D->anchor_unit, D->cap_units, &runs);
+                for (const SlotRun& r : runs) {
+                    writes[k].push_back({K.dst_rank, r.dst_slot, r.dst_slot + r.count});
+                    if (S) reads[k].push_back({K.src_rank, r.src_slot, r.src_slot + r.count});
+                }
+            }
+            std::vector<int32_t> ph;
+            ETP_TRY(assign_phases(reads, writes, &ph));
+            hit = phase_cache.emplace(std::move(key), std::move(ph)).first;
+        }
+        const std::vector<int32_t>& phase = hit->second;
 
         for (size_t k = 0; k < nt; ++k) {
             const etp_task& K = P.tasks[k];

@@ -64,11 +64,12 @@ class ModelState:
 
     def __init__(self, cfg: Config, device="cuda:0", image: str = "both", with_kv: bool = True,
                  with_params: bool = True, slack_garbage: bool = False, seq_lens: Optional[Sequence[int]] = None,
-                 plan_mode: int = B.PLAN_CMM, cap_mode: str = "span"):
+                 plan_mode: int = B.PLAN_CMM, cap_mode: str = "span", kv_layout: int = B.KV_TOKEN_MAJOR):
         self.cfg, self.device = cfg, torch.device(device)
         self.cap_mode = cap_mode          # "span": union span of the rank's intervals (one hazard phase, L5);
                                           # "tight": the widest shard the rank ever holds (shards wrap, plans need phases)
         self.plan_mode = plan_mode        # B.PLAN_CMM (the paper's planner) | PLAN_GREEDY | PLAN_FULL_RELOAD
+        self.kv_layout = kv_layout        # B.KV_TOKEN_MAJOR (reading K1) | B.KV_HEAD_MAJOR (its optional second layout)
         self.seed = SEED0 + 1000 * cfg.index
         self.image_kinds = ("pinned", "device") if image == "both" else (image,)
         self.specs: List[TensorSpec] = tensor_inventory(cfg) if with_params else []
@@ -206,7 +207,9 @@ class ModelState:
         frag = m.head_dim * m.elem_bytes
         rows = m.n_layers * 2 * n_blocks * kvs.block_size
         kv = {"table": table, "seq_lens": seq_lens, "last_use": last_use, "n_blocks": n_blocks, "head_cap": head_cap,
-              "frag": frag, "rows": rows, "anchors": {r: s for (r, s, e, _) in first}, "pools": {}, "backup": {}}
+              "frag": frag, "rows": rows, "anchors": {r: s for (r, s, e, _) in first}, "pools": {}, "backup": {},
+              "layout": self.kv_layout}
+        lay = dict(layout=self.kv_layout, block_size=kvs.block_size)
         for (r, s, e, _) in first:
             nb = rows * head_cap * frag
             if slack_garbage:
@@ -214,7 +217,7 @@ class ModelState:
             else:
                 pool = torch.zeros(nb, dtype=torch.uint8, device=self.device)
             if e > s:
-                fill_kv_pool(pool, rows, head_cap, m.head_dim, 0, s, e - s, m.n_kv_heads, seed, 1, self.dt)
+                fill_kv_pool(pool, rows, head_cap, m.head_dim, 0, s, e - s, m.n_kv_heads, seed, 1, self.dt, **lay)
             kv["pools"][r] = pool
         # the backup of each rank that dies: its pool at the time of death compacted to its own heads (reading K4)
         for i, st in enumerate(self.steps):
@@ -223,7 +226,7 @@ class ModelState:
             per_kind = {}
             if hh > 0:
                 dev = torch.empty(rows * hh * frag, dtype=torch.uint8, device=self.device)
-                fill_kv_pool(dev, rows, hh, m.head_dim, 0, ds, hh, m.n_kv_heads, seed, 1, self.dt)
+                fill_kv_pool(dev, rows, hh, m.head_dim, 0, ds, hh, m.n_kv_heads, seed, 1, self.dt, **lay)
                 for k in self.image_kinds:
                     if k == "device":
                         per_kind[k] = dev
@@ -284,7 +287,7 @@ class ModelState:
                            if r != st.dead and any(rr == r for (rr, _, _, _) in st.old["head"])}
             evicted, rep_k = B.etp_reshard_kv(
                 ctx, n_layers=m.n_layers, n_blocks=kv["n_blocks"], block_size=self.cfg.kv.block_size, head_cap=kv["head_cap"],
-                head_dim=m.head_dim, elem_bytes=m.elem_bytes, layout=B.KV_TOKEN_MAJOR, pools=alive_pools,
+                head_dim=m.head_dim, elem_bytes=m.elem_bytes, layout=kv["layout"], pools=alive_pools,
                 head_anchor=kv["anchors"], n_ranks=self.n_ranks, table=new_table, seq_lens=kv["seq_lens"],
                 last_use=kv["last_use"], head_plan=plans["head"],
                 new_block_budget=kv["n_blocks"] if block_budget is None else block_budget,

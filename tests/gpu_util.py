@@ -14,17 +14,27 @@ GUARD_BYTE = 0xA5
 
 
 class LibSide:
-    """partition / plan through the C ABI (same interface as harness.OracleSide)."""
+    """partition / plan through the C ABI (same interface as harness.OracleSide).  Every answer of the library is compared
+    with the oracle's on the spot, so a world built with this side proves S1 / S2 on the GPU box too (`-m gpu` deselects the
+    host-only parity tests of tests/test_lib_host.py): a wrong library plan fails here, not silently in the expected image."""
     name = "libetp"
 
     @staticmethod
     def partition(H, M, policy="floor", align=1):
-        return etp.etp_partition(H, M, policy, align)
+        from oracle import planning as OP
+        got = etp.etp_partition(H, M, policy, align)
+        assert got == OP.partition(H, M, policy, align), f"etp_partition({H}, {M}, {policy}) differs from the oracle"
+        return got
 
     @staticmethod
     def plan(old, M, tb=None):
+        from oracle import planning as OP
         p = etp.etp_cmm_plan(old, M, tb)
-        return p.tasks(), p.new_layout()
+        tasks, new = p.tasks(), p.new_layout()
+        o_tasks, o_new = OP.cmm_plan(old, M, tb)
+        assert [tuple(t) for t in tasks] == [tuple(t) for t in o_tasks], "etp_cmm_plan: task list differs from oracle.planning.cmm_plan"
+        assert [tuple(s) for s in new] == [tuple(s) for s in o_new], "etp_cmm_plan: new layout differs from oracle.planning.cmm_plan"
+        return tasks, new
 
 
 class DevBuf:

@@ -167,10 +167,11 @@ def expected_pool(state, r, upto_step, garbage):
     else:
         exp = torch.zeros(nb, dtype=torch.uint8, device=state.device)
     s, e = first[r]
+    layout = state.kv["layout"]
     if e > s:
-        fill_kv_pool(exp, rows, cap, m.head_dim, 0, s, e - s, m.n_kv_heads, seed, 1, state.dt)
+        fill_kv_pool(exp, rows, cap, m.head_dim, 0, s, e - s, m.n_kv_heads, seed, 1, state.dt, layout=layout, block_size=bs)
     live = live_block_ids(state)
-    ev = exp.view(planes, n_blocks, bs, cap, frag)
+    ev = exp.view(planes, n_blocks, bs, cap, frag) if layout == 0 else exp.view(planes, n_blocks, cap, bs, frag)
     held = set(range(s, e))
     for i in range(upto_step):
         new = [(b, e2) for (rr, b, e2, _) in state.steps[i].new["head"] if rr == r]
@@ -181,7 +182,10 @@ def expected_pool(state, r, upto_step, garbage):
                 one = torch.empty(rows * frag, dtype=torch.uint8, device=state.device)
                 fill_kv_pool(one, rows, 1, m.head_dim, 0, h, 1, m.n_kv_heads, seed, 1, state.dt)
                 ov = one.view(planes, n_blocks, bs, frag)
-                ev[:, live, :, (h - anchor) % cap, :] = ov[:, live]
+                if layout == 0:
+                    ev[:, live, :, (h - anchor) % cap, :] = ov[:, live]
+                else:
+                    ev[:, live, (h - anchor) % cap, :, :] = ov[:, live]
                 del one, ov
             held = set(range(b, e2))
     return exp
@@ -217,7 +221,7 @@ def oracle_layer_kv(state, step_idx, layer, snap, image, budget=None):
     st = state.steps[step_idx]
     m, kv = state.cfg.model, state.kv
     planes, n_blocks, bs, cap, frag = kv_dims(state)
-    g1 = OS.KVGeom(1, n_blocks, bs, cap, m.head_dim, m.elem_bytes, 0)
+    g1 = OS.KVGeom(1, n_blocks, bs, cap, m.head_dim, m.elem_bytes, kv["layout"])
     sc = state.cfg.scenario
     H = m.n_kv_heads
     tasks = oracle_tasks(state, st, "head", H)
@@ -442,3 +446,58 @@ def test_config4_full_state_moe(ctx):
 def test_config5a_sequential_failures_full_state(ctx):
     """configs[4] (a): Llama-3-8B shape, 8 -> 7 -> 6 -> 5, each reshard planned from the previous layout."""
     run_full_config(ctx, "5a", "pinned", linear_tokens=(4,))
+
+
+# ------------------------------------------------------------------------------------------------ config 5b at its own sizes
+@pytest.mark.parametrize("n", [100_000, 1_000_000])
+def test_config5b_copy_intervals_full_size_every_byte(ctx, n):
+    """configs[4] (b) at the sizes bench.py --microbench times (recipe of workloads/gen.py::microbench_intervals, DESIGN.md R-5b):
+    10^5 intervals up to 2 MiB (21.7 GiB) and 10^6 intervals up to 128 KiB (19.5 GiB), random 16-byte aligned sources in a
+    32-GiB arena, disjoint destinations in random order with random gaps.  EVERY destination byte is checked: the expected
+    arena is built on the device from the plain definition - one `dst[b:b+m] = src[a:a+m]` per interval, nothing else - and
+    compared whole, gaps and guard bands included (a gap keeps the seeded garbage it held)."""
+    from workloads.configs import MICROBENCH_HI, MICROBENCH_LO
+    from workloads.gen import SEED0, microbench_intervals
+    dev = torch.device("cuda:0")
+    src_arena = 32 << 30
+    G = 4096
+    so, do, sz, dst_arena = microbench_intervals(n, MICROBENCH_LO, MICROBENCH_HI[n], SEED0 + 5000 + n, src_arena)
+    src = fill_bytes(SEED0 + 5000, 1, 0, src_arena, device=dev)
+    nb = (dst_arena + 2 * G + 7) // 8 * 8
+    got = fill_bytes(SEED0 + 5001, 2, 0, nb, device=dev)          # destination arena between two guard bands, all garbage
+    exp = got.clone()
+    torch.cuda.synchronize()
+    st = torch.cuda.Stream()
+    rep = etp.etp_copy_intervals(ctx, so + src.data_ptr(), do + got.data_ptr() + G, sz, st.cuda_stream)
+    so_l, do_l, sz_l = so.tolist(), (do + G).tolist(), sz.tolist()
+    for a, b, m in zip(so_l, do_l, sz_l):                         # the plain definition, interval by interval
+        exp[b:b + m] = src[a:a + m]
+    st.synchronize()
+    torch.cuda.synchronize()
+    assert rep["d2d_bytes"] == int(sz.sum()) and rep["n_phases"] == 1
+    if not torch.equal(got, exp):
+        bad = torch.nonzero(got != exp)[:4].flatten().tolist()
+        raise AssertionError(f"n = {n}: destination arena differs from the plain definition at bytes {bad}")
+    del got, exp, src
+    torch.cuda.empty_cache()
+
+
+def test_config2_kv_head_major_full_size(ctx):
+    """Reading K1's second layout at config-2 size (8 layers of the KV cache): pool[r] = [layer][K|V][block][slot][token][dim],
+    so a head of a block is one 4-KiB contiguous run instead of 16 strided 256-byte fragments.  Whole-state plain definition
+    on the device, two layers against the oracle's element-by-element applier, pinned backup (zero-copy gather)."""
+    cfg = scaled(get_config("2"), n_layers=8)
+    state = ModelState(cfg, device="cuda:0", image="pinned", with_params=False, slack_garbage=True, kv_layout=etp.KV_HEAD_MAJOR)
+    m = cfg.model
+    layers = [0, 5]
+    snaps = {L: snapshot_layer_kv(state, L) for L in layers}
+    cs, rs = torch.cuda.Stream(), torch.cuda.Stream()
+    rep = state.reshard(ctx, 0, "pinned", cs.cuda_stream, rs.cuda_stream, replan=True)
+    cs.synchronize()
+    rs.synchronize()
+    assert not rep["evicted"]
+    for L in layers:
+        kexp, kstats = oracle_layer_kv(state, 0, L, snaps[L], "pinned")
+        compare_layer_kv(state, L, kexp)
+    assert (rep["kv"]["d2d_bytes"], rep["kv"]["h2d_bytes"]) == (kstats["d2d_bytes"] * m.n_layers, kstats["h2d_bytes"] * m.n_layers)
+    check_kv_whole_state(state, 1, True)

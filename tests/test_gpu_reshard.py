@@ -96,8 +96,10 @@ def test_config1_params_bit_exact(ctx, mode, policy, dead):
 
 @pytest.mark.parametrize("image", ["pinned", "device"])
 @pytest.mark.parametrize("tma_min", [None, 16, 1 << 62])
-def test_mid_params_bit_exact_every_copy_path(ctx, image, tma_min):
-    """Multi-tile sizes with ragged tails; TMA-only, vector-only and mixed routing of the same plan."""
+@pytest.mark.parametrize("steal", [0, 1])
+def test_mid_params_bit_exact_every_copy_path(ctx, image, tma_min, steal):
+    """Multi-tile sizes with ragged tails; TMA-only, vector-only and mixed routing of the same plan; with
+    ETP_OPT_LDG_STEALS_BULK the vector warps also drain the bulk queue (both engines race for the same items)."""
     world = H.build_param_world(MID, side=LibSide, mode="span")
     expect, stats = H.oracle_reshard_params(world, 0)
     bufs, images = upload_param_world(world, image)
@@ -105,9 +107,11 @@ def test_mid_params_bit_exact_every_copy_path(ctx, image, tma_min):
     try:
         if tma_min is not None:
             ctx.set_option(etp.OPT_TMA_MIN_BYTES, tma_min)
+        ctx.set_option(etp.OPT_LDG_STEALS_BULK, steal)
         rep = run_param_step(ctx, world, bufs, images, 0, Streams())
     finally:
         ctx.set_option(etp.OPT_TMA_MIN_BYTES, default)
+        ctx.set_option(etp.OPT_LDG_STEALS_BULK, 0)
     compare_params(world, bufs, expect, {1})
     assert rep["d2d_bytes"] == stats["d2d_bytes"]
     assert rep["h2d_bytes"] + rep["reload_dev_bytes"] == stats["h2d_bytes"]
@@ -274,16 +278,6 @@ def test_kv_budget_shrink_and_no_backup(ctx):
     # reading K4: no backup -> reload heads untouched, every live sequence reported
     ev, evicted, rep, stats = run_kv(ctx, world, world.g.n_blocks, backup=None)
     assert sorted(ev) == [0, 1, 2] and rep["h2d_bytes"] == 0
-
-
-def test_kv_staged_reload_mode(ctx):
-    cfg = dataclasses.replace(MID, model=dataclasses.replace(MID.model, n_layers=2))
-    world = H.build_kv_world(cfg, side=LibSide, layout=0, seq_lens=[300, 7, 1000], head_cap=4)
-    ctx.set_option(etp.OPT_KV_RELOAD_MODE, 1)
-    try:
-        run_kv(ctx, world, world.g.n_blocks, "pinned")
-    finally:
-        ctx.set_option(etp.OPT_KV_RELOAD_MODE, 0)
 
 
 # ------------------------------------------------------------------------------------------------ scale-up (a rank joins)
@@ -484,8 +478,101 @@ def test_copy_intervals_small_batches(ctx, size, n):
 
 
 def test_copy_intervals_errors(ctx):
-    S, D = DevBuf(np.zeros(4096, np.uint8)), DevBuf(np.zeros(4096, np.uint8))
+    S, D = DevBuf(np.zeros(4096, np.uint8)), DevBuf(np.full(4096, 7, np.uint8))
     for so, do, sz, status in [(8, 0, 16, 2), (0, 0, 24, 2), (0, 0, -16, 1)]:
         with pytest.raises(etp.EtpError) as e:
             etp.etp_copy_intervals(ctx, np.array([S.ptr + so]), np.array([D.ptr + do]), np.array([sz]))
         assert e.value.status == status
+    # the contract of include/etp.h: destinations mutually disjoint and disjoint from every source -> INVALID_ARG, nothing enqueued
+    a = np.array
+    cases = [
+        (a([S.ptr, S.ptr + 512]), a([D.ptr, D.ptr + 48]), a([64, 64])),                  # two destinations overlap by 16 bytes
+        (a([S.ptr, S.ptr + 512, S.ptr + 64]), a([D.ptr + 1024, D.ptr, D.ptr + 1040]), a([32, 64, 16])),   # ... out of order in the list
+        (a([S.ptr, D.ptr + 96]), a([D.ptr + 64, D.ptr + 2048]), a([64, 64])),          # a destination overlaps another interval's source
+        (a([D.ptr + 16]), a([D.ptr]), a([64])),                                           # ... its own source (a shifting copy)
+    ]
+    for sp, dp, sz in cases:
+        with pytest.raises(etp.EtpError) as e:
+            etp.etp_copy_intervals(ctx, sp, dp, sz)
+        assert e.value.status == 1
+    torch.cuda.synchronize()
+    assert (D.payload() == 7).all() and D.guards_intact()
+    # touching but not overlapping is fine; with validation off the caller is trusted
+    etp.etp_copy_intervals(ctx, a([S.ptr, S.ptr + 64]), a([D.ptr, D.ptr + 64]), a([64, 64]))
+    ctx.set_option(etp.OPT_VALIDATE_INTERVALS, 0)
+    try:
+        etp.etp_copy_intervals(ctx, a([S.ptr]), a([D.ptr + 128]), a([64]))
+    finally:
+        ctx.set_option(etp.OPT_VALIDATE_INTERVALS, 1)
+    torch.cuda.synchronize()
+    assert (D.payload()[:192] == 0).all() and (D.payload()[192:] == 7).all()
+
+
+def test_back_to_back_calls_without_a_sync(ctx):
+    """Two calls in flight on one ctx (the descriptor arena is double-buffered): a KV reshard whose zero-copy gather sits on
+    the reload stream behind a large pinned-host copy, then - without any synchronisation - a multi-phase parameter reshard
+    (tight slabs: several launches on the copy stream).  The work-queue heads of the first call's gather must not be reset
+    or shared by the second call's launches (they live in the call's own arena slot)."""
+    cfg = dataclasses.replace(MID, model=dataclasses.replace(MID.model, n_layers=2))
+    kvw = H.build_kv_world(cfg, side=LibSide, layout=0, seq_lens=[300, 7, 1000], head_cap=4)
+    st = kvw.steps[0]
+    g = kvw.g
+    new_table, evicted, pairs = OS.page_table_rewrite(kvw.table, kvw.seq_lens, kvw.last_use, g.block_size, g.n_blocks)
+    snap = {r: p for r, p in kvw.pools.items() if r != st.dead}
+    kexpect, _ = OS.apply_kv(st.tasks["head"], snap, kvw.anchors, g, kvw.host_backup, kvw.host_heads, kvw.host_head0, pairs)
+    kbufs = {r: DevBuf(p) for r, p in snap.items()}
+    img = pinned(kvw.host_backup)
+    world = H.build_param_world(MID, side=LibSide, mode="tight", failed=(2,))
+    pexpect, _ = H.oracle_reshard_params(world, 0)
+    pbufs, pimages = upload_param_world(world)
+    plans = make_plans(world.steps[0])
+    klasses = sorted(plans)
+    descs = tensor_descs(world, pbufs, pimages, world.steps[0], {k: i for i, k in enumerate(klasses)})
+    s = Streams()
+    big = torch.empty(1 << 30, dtype=torch.uint8).pin_memory()
+    sink = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    table = kvw.table.copy()
+    with torch.cuda.stream(s.reload):
+        sink.copy_(big, non_blocking=True)              # ~20 ms of DMA ahead of the gather on the reload stream
+    ev, _ = etp.etp_reshard_kv(ctx, n_layers=g.n_layers, n_blocks=g.n_blocks, block_size=g.block_size, head_cap=g.head_cap,
+                               head_dim=g.head_dim, elem_bytes=g.elem_bytes, layout=g.layout, pools={r: b.ptr for r, b in kbufs.items()},
+                               head_anchor=kvw.anchors, n_ranks=max(kvw.pools) + 1, table=table, seq_lens=kvw.seq_lens,
+                               last_use=kvw.last_use, head_plan=make_plans(st)["head"], new_block_budget=g.n_blocks,
+                               host_backup=img.data_ptr(), host_heads=kvw.host_heads, host_head0=kvw.host_head0,
+                               copy_stream=s.copy.cuda_stream, reload_stream=s.reload.cuda_stream)
+    rep = etp.etp_reshard_params(ctx, descs, [plans[k] for k in klasses], s.copy.cuda_stream, s.reload.cuda_stream)
+    assert rep["n_phases"] >= 2 and rep["n_kernel_launches"] >= 2
+    s.sync()
+    assert ev == evicted and np.array_equal(table, new_table)
+    for r, b in kbufs.items():
+        assert b.guards_intact() and b.payload().tobytes() == kexpect[r].tobytes(), f"pool of rank {r} differs from the oracle image"
+    compare_params(world, pbufs, pexpect, {2})
+
+
+def test_failed_kv_call_leaves_the_table_alone(ctx):
+    """A call that fails in lowering (head_cap too small for the new shard; backup that does not cover the reloaded heads) must
+    not have rewritten the caller's page table or reported evictions, and must not have moved a byte."""
+    cfg = dataclasses.replace(MID, model=dataclasses.replace(MID.model, n_layers=1))
+    world = H.build_kv_world(cfg, side=LibSide, layout=0, seq_lens=[300, 7, 1000], head_cap=4)
+    st, g = world.steps[0], world.g
+    live = int(((world.seq_lens + 15) // 16).sum())
+    snap = {r: p for r, p in world.pools.items() if r != st.dead}
+    bufs = {r: DevBuf(p) for r, p in snap.items()}
+    img = pinned(world.host_backup)
+    s = Streams()
+    for kw, status in ((dict(head_cap=2), 3), (dict(host_head0=world.host_head0 + 1), 4), (dict(block_size=0), 1)):
+        table = world.table.copy()
+        args = dict(n_layers=g.n_layers, n_blocks=g.n_blocks, block_size=g.block_size, head_cap=g.head_cap, head_dim=g.head_dim,
+                    elem_bytes=g.elem_bytes, layout=g.layout, pools={r: b.ptr for r, b in bufs.items()}, head_anchor=world.anchors,
+                    n_ranks=max(world.pools) + 1, table=table, seq_lens=world.seq_lens, last_use=world.last_use,
+                    head_plan=make_plans(st)["head"], new_block_budget=live - 10, host_backup=img.data_ptr(),
+                    host_heads=world.host_heads, host_head0=world.host_head0, copy_stream=s.copy.cuda_stream,
+                    reload_stream=s.reload.cuda_stream)
+        args.update(kw)
+        with pytest.raises(etp.EtpError) as e:
+            etp.etp_reshard_kv(ctx, **args)
+        assert e.value.status == status, (kw, e.value)
+        assert np.array_equal(table, world.table), f"{kw}: the failed call rewrote the page table"
+    s.sync()
+    for r, b in bufs.items():
+        assert b.guards_intact() and b.payload().tobytes() == snap[r].tobytes()

@@ -240,6 +240,75 @@ def test_config1_kv_plain_definition(layout, dead, budget):
                 assert np.array_equal(v0[:, :, b], v1[:, :, b])
 
 
+def load_kv_golden(golden_dir):
+    g = {"plan": [], "anchor": {}, "before": {}, "after": {}, "backup": {}}
+    kinds = {"K": OP.KEEP, "T": OP.TRANSFER, "R": OP.RELOAD}
+    for line in open(f"{golden_dir}/kv_tiny.txt"):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = line.split()
+        if w[0] == "plan":
+            g["plan"].append((kinds[w[1]], int(w[2]), int(w[3]), int(w[4]), int(w[5])))
+        elif w[0] == "anchor":
+            g["anchor"][int(w[1])] = int(w[2])
+        elif w[0] in ("before", "after"):
+            g[w[0]][(int(w[1]), int(w[2]), int(w[3]))] = w[5:]
+        elif w[0] == "backup":
+            g["backup"][(int(w[1]), int(w[2]))] = w[4:]
+        elif w[0] in ("table", "new_table", "stats"):
+            g[w[0]] = [int(x) for x in w[1:]]
+        else:
+            g[w[0]] = int(w[1])
+    return g
+
+
+def kv_golden_pool(g, rows, heads, layout, frag):
+    """Expand the golden's per-plane picture {(block, token): [fragment per slot]} into a pool image through a numpy N-d
+    view (never through the oracle's offset arithmetic): fragment "c4" in plane p -> bytes 1 + 4 + 8*2 + 32*p."""
+    L, nb, bs = g["n_layers"], g["n_blocks"], g["block_size"]
+    shape = (L, 2, nb, bs, heads, frag) if layout == 0 else (L, 2, nb, heads, bs, frag)
+    pool = np.zeros(shape, dtype=np.uint8)
+    for (b, t), slots in rows.items():
+        for sl, name in enumerate(slots):
+            for l in range(L):
+                for c in range(2):
+                    p = 2 * l + c
+                    val = 200 + int(name[1:]) + 10 * p if name[0] == "g" else 1 + int(name[1]) + 8 * (ord(name[0]) - ord("a")) + 32 * p
+                    if layout == 0:
+                        pool[l, c, b, t, sl, :] = val
+                    else:
+                        pool[l, c, b, sl, t, :] = val
+    return pool.reshape(-1)
+
+
+@pytest.mark.parametrize("layout", [0, 1])
+@pytest.mark.parametrize("frag", [1, 16])
+def test_golden_kv_image(golden_dir, layout, frag):
+    """tests/golden/kv_tiny.txt: a relocated block, a TRANSFER head, a RELOAD head into a wrapped slot, kept heads, a free
+    block, both block layouts - the hand-worked picture against page_table_rewrite + apply_kv."""
+    g = load_kv_golden(golden_dir)
+    old = [(0, 0, 3, 1), (1, 3, 4, 0), (2, 4, 5, 1)]
+    tasks, new = OP.cmm_plan(old, 2)
+    assert tasks == g["plan"] and new == [(0, 0, 2, 1), (2, 2, 5, 1)]
+    table = np.array([g["table"]], dtype=np.int32)
+    new_table, evicted, pairs = OS.page_table_rewrite(table, [4], [0], g["block_size"], g["budget"])
+    assert new_table.tolist() == [g["new_table"]] and evicted == [] and pairs == [(0, 0, 2, 1), (0, 1, 0, 0)]
+    geom = OS.KVGeom(g["n_layers"], g["n_blocks"], g["block_size"], g["head_cap"], frag, 1, layout)
+    per_rank = lambda which, r: {(b, t): v for (rr, b, t), v in g[which].items() if rr == r}
+    snap = {r: kv_golden_pool(g, per_rank("before", r), g["head_cap"], layout, frag) for r in (0, 2)}
+    before = {r: a.copy() for r, a in snap.items()}
+    backup = kv_golden_pool(g, g["backup"], 1, layout, frag)
+    out, stats = OS.apply_kv(tasks, snap, g["anchor"], geom, backup, 1, 3, pairs)
+    for r in (0, 2):
+        exp = kv_golden_pool(g, per_rank("after", r), g["head_cap"], layout, frag)
+        assert out[r].tobytes() == exp.tobytes(), f"rank {r}, layout {layout}"
+        assert snap[r].tobytes() == before[r].tobytes()          # snapshot semantics: the inputs were not modified
+    d2d, h2d, kept = g["stats"]
+    assert stats == {"d2d_bytes": d2d * frag, "h2d_bytes": h2d * frag, "kept_bytes": kept * frag}
+    # a single fragment through the oracle's own accessor: token b (block 1 after the move), head 3 at r2's wrapped slot 2
+    assert OS.kv_fragment(out[2], geom, g["anchor"][2], 1, 1, 1, 1, 3)[0] == 1 + 3 + 8 * 1 + 32 * 3
+
+
 def test_kv_ragged_lengths_and_head_major():
     cfg = get_config("1")
     world = H.build_kv_world(cfg, layout=1, seq_lens=[37, 128])
@@ -323,3 +392,33 @@ def test_moe_ref_special_cases():
     big[:, 1] = 50.0
     np.testing.assert_allclose(OL.moe_ref(x, big, gate, up, down_t, 1),
                                OL.moe_ref(x, lg[:, :1], gate[1:2], up[1:2], down_t[1:2], 1), rtol=1e-12, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------------------ all-cores leg == 1-core oracle
+def test_parallel_appliers_equal_the_plain_ones():
+    """oracle.state.apply_params_parallel / apply_kv_parallel (the OpenMP loop over jobs that bench.py times as the all-cores
+    baseline) must produce exactly the images and counters of apply_params / apply_kv, task by task and byte by byte."""
+    cfg = get_config("1")
+    for mode, dead in (("tight", 2), ("span", 0), ("full", 3)):
+        world = H.build_param_world(cfg, mode=mode, failed=(dead,))
+        expect, stats = H.oracle_reshard_params(world, 0)
+        st = world.steps[0]
+        items = [(st.tasks[sp.klass], {r: a for r, a in world.slabs[sp.name].items() if r != st.dead}, world.geom[sp.name],
+                  sp.unit_bytes, world.unsharded[sp.name], 0) for sp in world.specs]
+        outs, pstats = OS.apply_params_parallel(items, job_bytes=4096)
+        assert pstats == stats
+        for sp, out in zip(world.specs, outs):
+            for r, a in out.items():
+                assert a.tobytes() == expect[sp.name][r].tobytes(), (mode, sp.name, r)
+    for layout in (0, 1):
+        kw = H.build_kv_world(cfg, layout=layout, failed=(1,))
+        st, g = kw.steps[0], kw.g
+        _, evicted, pairs = OS.page_table_rewrite(kw.table, kw.seq_lens, kw.last_use, g.block_size, 12)
+        snap = {r: p for r, p in kw.pools.items() if r != st.dead}
+        exp, stats = OS.apply_kv(st.tasks["head"], snap, kw.anchors, g, kw.host_backup, kw.host_heads, kw.host_head0, pairs)
+        got, pstats = OS.apply_kv_parallel(st.tasks["head"], snap, kw.anchors, g, kw.host_backup, kw.host_heads, kw.host_head0, pairs,
+                                           pairs_per_job=3)
+        assert pstats == stats
+        for r in exp:
+            assert got[r].tobytes() == exp[r].tobytes()
+    assert OS.omp_threads() >= 1

@@ -87,19 +87,30 @@ def fill_normal16(seed: int, stream: int, elem_offset: int, n: int, std: float, 
 
 
 def fill_kv_pool(pool: torch.Tensor, rows: int, heads_in_pool: int, dim: int, slot0: int, head0: int, n: int,
-                 n_kv_heads: int, seed: int, stream: int, dtype: torch.dtype, row_chunk: int = 1 << 16) -> None:
+                 n_kv_heads: int, seed: int, stream: int, dtype: torch.dtype, row_chunk: int = 1 << 16,
+                 layout: int = 0, block_size: int = 1) -> None:
     """Paged-KV content that is a pure function of (row, head, d): element d of KV head ``h`` at pool row ``row``
     (row = flattened (layer, K|V, block, token)) has the value of stream index (row * n_kv_heads + h) * dim + d,
-    N(0,1).  Writes heads head0..head0+n-1 into slots slot0..slot0+n-1 of ``pool`` viewed as
-    [rows][heads_in_pool][dim] (token-major layout); every other slot is left as it is."""
-    v = pool.view(dtype).view(rows, heads_in_pool, dim)
+    N(0,1).  Writes heads head0..head0+n-1 into slots slot0..slot0+n-1 of ``pool``; every other slot is left as it is.
+    ``layout`` 0: pool viewed as [rows][heads_in_pool][dim] (token-major); ``layout`` 1: [rows / block_size][heads_in_pool]
+    [block_size][dim] (head-major: the tokens of a block are contiguous per head).  Same values either way."""
     d = torch.arange(dim, dtype=torch.int64, device=pool.device)
     hh = torch.arange(head0, head0 + n, dtype=torch.int64, device=pool.device)
+    if layout == 0:
+        v = pool.view(dtype).view(rows, heads_in_pool, dim)
+    else:
+        assert rows % block_size == 0
+        row_chunk = max(row_chunk // block_size, 1) * block_size
+        v = pool.view(dtype).view(rows // block_size, heads_in_pool, block_size, dim)
     for a in range(0, rows, row_chunk):
         b = min(rows, a + row_chunk)
         r = torch.arange(a, b, dtype=torch.int64, device=pool.device)
         idx = ((r[:, None, None] * n_kv_heads + hh[None, :, None]) * dim) + d[None, None, :]
-        v[a:b, slot0:slot0 + n, :] = normal16_at(idx, seed, stream, 1.0, dtype)
+        val = normal16_at(idx, seed, stream, 1.0, dtype)                     # [rows of the chunk][n heads][dim]
+        if layout == 0:
+            v[a:b, slot0:slot0 + n, :] = val
+        else:
+            v[a // block_size:b // block_size, slot0:slot0 + n] = val.view((b - a) // block_size, block_size, n, dim).permute(0, 2, 1, 3)
 
 
 def torch_dtype(name: str) -> torch.dtype:
