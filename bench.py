@@ -802,31 +802,27 @@ def run_ours(args):
     d2d_frac = 2.0 * d_bytes / (d_kms * 1e-3) / 1e9 / hbm_peak if d_kms > 0 else None
     transfer_only = {"moved_bytes": d_bytes // max(K, 1), "ms": d_kms / max(K, 1),
                      "moved_GBps": d_bytes / (d_kms * 1e-3) / 1e9 if d_kms > 0 else None, "frac": d2d_frac, "launches_per_step": d_kl // max(K, 1),
-                     "what": "kernel (a) on the TRANSFER intervals of the plan only (reload skipped): the north_star's 'moved bytes vs HBM peak' "
-                             "for the stated scenario, where the reload bytes come over the host link and never pass through kernel (a)"}
+                     "what": "kernel (a) on the plan's TRANSFER intervals only (reload skipped): moved bytes vs HBM peak of the host-reload scenario"}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": tot_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
         "data": "synthetic",
         "config": {"workload": f"config {cfg.key}: {cfg.note}" + (" [REDUCED: debug run, not a bench value]" if reduced else "")
                                + (" [migration-aware plan, DESIGN.md reading M1]" if args.plan_mode != "cmm" else ""),
-                   "reload_source": "device-resident image (synthetic stand-in for the failed rank's bytes, already in HBM when the timed "
-                                    "region starts; EVERY reload byte therefore goes through kernel (a) and is counted in `value`). "
-                                    "The stated scenario - reload from pinned host memory - is `e2e`.",
+                   "reload_source": "device-resident image (synthetic; every reload byte goes through kernel (a))",
+                   "reload_source_note": "`value`: failed rank's bytes already in HBM; pinned-host reload (the stated scenario) is `e2e`",
                    "state_GB": round((sb["param_bytes"] + sb["kv_live_bytes"]) / 1e9, 2),
                    "moved_GB_per_step": round(moved / K / 1e9, 3),
                    "l2": "inputs larger than L2 (every step re-reads and re-writes GBs; plans are hazard-free so a step is idempotent in place)",
                    "replicas": world,
-                   "step": "S1 partition + S2 CMM plan + S3 lowering + S4 copy + S5 reload + S6 page table, synchronised per step. "
-                           "`value` / `roofline.frac`: every moved byte (TRANSFER + device-image RELOAD) through kernel (a) - a stress figure "
-                           "of the kernel.  The north_star target (>= 75 % of HBM peak in moved bytes on the 4->3 reshard with the reload "
-                           "from the host, reload fully overlapped) is answered by `roofline.transfer_only` and `e2e.overlap_ratio`."},
+                   "step": "S1 partition + S2 CMM plan + S3 lowering + S4 copy + S5 reload + S6 page table, synchronised per step",
+                   "north_star_target": "roofline.transfer_only (>= 0.75 of HBM peak in moved bytes) + e2e.overlap_ratio (reload overlapped)",
+                   "value_is": "kernel stress figure: TRANSFER + device-image RELOAD bytes all through kernel (a)"},
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": e_h2d // K, "d2h_bytes_per_step": 0,
                 "ms_per_step": e_ms / K, "h2d_GBps": e_h2d / (e_ms * 1e-3) / 1e9,
                 "overlap_ratio": overlap["ratio"], "a_only_ms": overlap["a_only_ms"], "b_only_ms": overlap["b_only_ms"], "both_ms": overlap["both_ms"],
                 "reload_source": "pinned host memory (the stated scenario)",
-                "note": "reload sources in pinned host memory; result stays on the device (the page table is host-side); "
-                        "overlap_ratio = both_ms / max(a_only_ms, b_only_ms), 1.0 = device copies fully hidden under the reload"},
+                "note": "overlap_ratio = both_ms / max(a_only_ms, b_only_ms); result stays on the device (page table is host-side)"},
         "reuse_ratio": (ru_p["kept_GB"] + ru_p["p2p_GB"] + ru_k["kept_GB"] + ru_k["p2p_GB"]) / tot_all,
         "reload_fraction": (ru_p["reload_GB"] + ru_k["reload_GB"]) / tot_all,
         "reuse_ratio_params": ru_p["reuse_ratio"], "reload_fraction_params": ru_p["reload_fraction"],
@@ -838,9 +834,8 @@ def run_ours(args):
                      "traffic": None if reduced or cfg.key != "2" else ncu_traffic_per_launch(),
                      "traffic_source": traffic_source(),
                      "kernel": "etp_interval_copy_kernel", "peak_source": peak_src,
-                     "peak_note": "the peak is a torch b.copy_(a) of 2 GiB (read + write bytes): a plain copy, not an upper bound, so a frac "
-                                  "slightly above 1 is possible (B200_PROFILING.md)",
-                     "scenario": "device-resident reload images: TRANSFER + RELOAD bytes through kernel (a) (see config.reload_source)",
+                     "peak_note": "peak = torch b.copy_(a), read + write bytes: a plain copy, not an upper bound (frac may exceed 1)",
+                     "scenario": "device-resident reload images: TRANSFER + RELOAD bytes through kernel (a)",
                      "frac_of_datasheet_8TBps": achieved / 8000.0,   # state both denominators
                      "bytes_per_launch": 2.0 * kbytes / max(kl, 1), "ms_per_launch": kms / max(kl, 1), "launches": kl,
                      "transfer_only": transfer_only, "transfer_only_frac": d2d_frac, "transfer_only_ms": transfer_only["ms"],

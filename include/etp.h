@@ -77,6 +77,10 @@ typedef enum {
     ETP_OPT_VALIDATE_INTERVALS = 10, /* 1 (default): etp_copy_intervals checks on the host that the destinations are mutually
                                     disjoint and disjoint from every source (two sorts, O(n log n)) and returns
                                     ETP_ERR_INVALID_ARG before anything is enqueued; 0: trust the caller                   */
+    ETP_OPT_LINEAR_PDL = 11,     /* 1 (default): launches of the <= 64-token shard-linear kernel carry the programmatic-stream-
+                                    serialization attribute: their prologue and first ring of weight tiles overlap the tail of the
+                                    previous kernel of the stream (griddepcontrol; X, Y and the workspace are only touched after
+                                    griddepcontrol.wait); 0: plain stream order                                           */
     ETP_OPT__COUNT
 } etp_option;
 etp_status etp_ctx_set_option(etp_ctx* ctx, etp_option key, int64_t value);
@@ -235,11 +239,49 @@ etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype,
  * several microseconds per launch, and a serving engine runs these projections as one GEMM anyway.  Every
  * linear keeps its own slabs and its own output y [tokens][out_features]; results are bitwise those of separate
  * etp_shard_linear calls only when no K split is chosen (the split count depends on the total width).  n_outs in 1..8, all
- * w->total_units equal; the rest as etp_shard_linear. */
+ * w->total_units equal; the rest as etp_shard_linear.  (At <= 64 tokens both calls run through a ctx-owned cache of prepared
+ * groups, see etp_linear_prepare below.) */
 typedef struct { const etp_tensor* w; int64_t out_features; int64_t features_per_unit; void* y; } etp_linear_out;
 etp_status etp_shard_linear_multi(etp_ctx* ctx, etp_dtype dtype, const void* x, int64_t tokens, int64_t in_features,
                                   const etp_linear_out* outs, int32_t n_outs, const etp_shard* layout, int32_t n_shards,
                                   void* stream);
+
+/* Prepared groups.  At a few tokens a shard linear is a weight stream whose cost is dominated by what does NOT
+ * scale with the bytes: argument checks, tensor-map encoding, the launch ramp and the tail of a static grid.  etp_linear_prepare
+ * does everything that depends only on the weights and the layout once (slot runs, TMA tensor maps, the K split of every linear,
+ * a load-balanced assignment of work items to the SMs) and returns a plan; etp_linear_run then costs one kernel launch for the
+ * WHOLE group at <= 64 tokens - the linears of a group are independent of each other (none reads another's output), may mix
+ * column- and row-parallel modes and have their own x and y each - and one launch per linear above 64 tokens.  The plan keeps
+ * copies of the descriptors (not of the weights): the slabs must stay where they were.  Results equal etp_shard_linear's up to
+ * the fp32 summation order of the K split (column-parallel outputs stay bitwise independent of the shard layout, reading G3).
+ * A plan belongs to its ctx, is freed with etp_linear_free (before the ctx) and is used from one host thread at a time; runs on
+ * different streams may overlap (the split-K workspace is per stream). */
+typedef struct etp_linear_plan etp_linear_plan;
+typedef struct {
+    int32_t mode;               /* etp_linear_mode                                                                    */
+    int32_t reserved0;
+    int64_t in_features, out_features;
+    const etp_tensor* w;        /* as etp_shard_linear                                                                */
+    const etp_shard* layout;    /* host array of n_shards entries                                                     */
+    int32_t n_shards;
+    int32_t reserved1;
+    int64_t features_per_unit;
+} etp_linear_spec;
+typedef struct {
+    int32_t n_linears, n_ctas;
+    int64_t n_items;            /* (linear, 128-feature tile, K range) work items of the <= 64-token launch              */
+    int64_t total_chunks;       /* 16-KiB weight chunks of the whole group                                              */
+    int64_t max_cta_chunks;     /* ... of the most loaded CTA (balance = total_chunks / n_ctas / max_cta_chunks)          */
+    int64_t n_split_tiles;      /* fp32 partial tiles of the K split                                                    */
+    int32_t n_splits[8];        /* K splits per linear                                                                  */
+} etp_linear_plan_stats;
+/* lins: host array of n_lins (1..8) specs.  *out is owned by the library. */
+etp_status etp_linear_prepare(etp_ctx* ctx, etp_dtype dtype, const etp_linear_spec* lins, int32_t n_lins, etp_linear_plan** out);
+/* x, y: host arrays of n_lins device pointers (16-B aligned; x[l] is [tokens][in_features of l], y[l] is [tokens][out_features
+ * of l]); several linears may share an x.  Asynchronous on `stream`. */
+etp_status etp_linear_run(etp_linear_plan* plan, const void* const* x, int64_t tokens, void* const* y, void* stream);
+etp_status etp_linear_plan_info(const etp_linear_plan* plan, etp_linear_plan_stats* out);
+void etp_linear_free(etp_linear_plan* plan);
 
 /* ------------------------------------------------------------------------------------------------ grouped MoE linear
  * SURVEY.md 8(f) #3, reading G5; PAPER.md:172-174 (experts are the unit of the expert-granularity plan).  One

@@ -21,7 +21,7 @@ COL_PARALLEL, ROW_PARALLEL = 0, 1
 DTYPE = {"bf16": 0, "fp16": 1}
 KV_TOKEN_MAJOR, KV_HEAD_MAJOR = 0, 1
 (OPT_SKIP_D2D, OPT_SKIP_RELOAD, OPT_TMA_MIN_BYTES, OPT_LDG_STEALS_BULK, OPT_RELOAD_CHUNK_BYTES, OPT_RESERVED_5,
- OPT_GRID_CTAS, OPT_GATHER_CTAS, OPT_TIME_KERNELS, OPT_LINEAR_CTA_PAIR, OPT_VALIDATE_INTERVALS) = range(11)
+ OPT_GRID_CTAS, OPT_GATHER_CTAS, OPT_TIME_KERNELS, OPT_LINEAR_CTA_PAIR, OPT_VALIDATE_INTERVALS, OPT_LINEAR_PDL) = range(12)
 
 
 class EtpError(RuntimeError):
@@ -74,6 +74,16 @@ class etp_linear_out(C.Structure):
     _fields_ = [("w", C.POINTER(etp_tensor)), ("out_features", i64), ("features_per_unit", i64), ("y", vp)]
 
 
+class etp_linear_spec(C.Structure):
+    _fields_ = [("mode", i32), ("reserved0", i32), ("in_features", i64), ("out_features", i64), ("w", C.POINTER(etp_tensor)),
+                ("layout", C.POINTER(etp_shard)), ("n_shards", i32), ("reserved1", i32), ("features_per_unit", i64)]
+
+
+class etp_linear_plan_stats(C.Structure):
+    _fields_ = [("n_linears", i32), ("n_ctas", i32), ("n_items", i64), ("total_chunks", i64), ("max_cta_chunks", i64),
+                ("n_split_tiles", i64), ("n_splits", i32 * 8)]
+
+
 class etp_interval(C.Structure):
     _fields_ = [("src", vp), ("dst", vp), ("bytes", i64)]
 
@@ -81,7 +91,8 @@ class etp_interval(C.Structure):
 EXPORTS = ["etp_ctx_create", "etp_ctx_destroy", "etp_last_error", "etp_version", "etp_ctx_set_option", "etp_ctx_get_option",
            "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_tasks", "etp_plan_new_layout",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
-           "etp_shard_linear_multi", "etp_moe_linear", "etp_copy_intervals"]
+           "etp_shard_linear_multi", "etp_linear_prepare", "etp_linear_run", "etp_linear_plan_info", "etp_linear_free",
+           "etp_moe_linear", "etp_copy_intervals"]
 
 _lib = None
 
@@ -117,6 +128,11 @@ def lib() -> C.CDLL:
         L.etp_shard_linear.argtypes = [vp, C.c_int, C.c_int, vp, i64, i64, i64, C.POINTER(etp_tensor), C.POINTER(etp_shard), i32, i64,
                                        vp, vp]
         L.etp_shard_linear_multi.argtypes = [vp, C.c_int, vp, i64, i64, C.POINTER(etp_linear_out), i32, C.POINTER(etp_shard), i32, vp]
+        L.etp_linear_prepare.argtypes = [vp, C.c_int, C.POINTER(etp_linear_spec), i32, C.POINTER(vp)]
+        L.etp_linear_run.argtypes = [vp, C.POINTER(vp), i64, C.POINTER(vp), vp]
+        L.etp_linear_plan_info.argtypes = [vp, C.POINTER(etp_linear_plan_stats)]
+        L.etp_linear_free.argtypes = [vp]
+        L.etp_linear_free.restype = None
         L.etp_moe_linear.argtypes = [vp, C.c_int, C.c_int, vp, C.POINTER(i64), i32, i64, i64, C.POINTER(etp_tensor), C.POINTER(etp_shard),
                                      i32, vp, vp]
         L.etp_copy_intervals.argtypes = [vp, C.POINTER(etp_interval), i64, vp, C.POINTER(etp_reshard_report)]
@@ -355,6 +371,48 @@ class PreparedMultiLinear:
             self.outs[i].y = y
         _check(lib().etp_shard_linear_multi(ctx.handle, self.dtype, x_ptr, tokens, self.K, self.outs, len(self.lins), self.layout, self.n,
                                             stream or None))
+
+
+class LinearPlan:
+    """Owns an etp_linear_plan: a prepared group of 1..8 independent shard linears (each a PreparedLinear: mode, shapes, weight
+    descriptor, layout).  run() takes one x and one y pointer per linear (or a single x shared by all)."""
+
+    def __init__(self, ctx: Context, linears: Sequence["PreparedLinear"]):
+        assert linears and all(l.dtype == linears[0].dtype for l in linears)
+        self.lins = list(linears)          # keeps the marshalled descriptors alive while prepare() reads them
+        n = len(linears)
+        specs = (etp_linear_spec * n)()
+        for i, l in enumerate(linears):
+            specs[i] = etp_linear_spec(l.mode, 0, l.K, l.N, C.cast(l.arr, C.POINTER(etp_tensor)), l.layout, l.n, 0, l.fpu)
+        h = vp()
+        _check(lib().etp_linear_prepare(ctx.handle, linears[0].dtype, specs, n, C.byref(h)))
+        self.handle, self.n, self.ctx = h, n, ctx
+        self._x, self._y = (vp * n)(), (vp * n)()
+
+    def run(self, x_ptrs, tokens: int, y_ptrs: Sequence[int], stream: int = 0) -> None:
+        if isinstance(x_ptrs, int):
+            x_ptrs = [x_ptrs] * self.n
+        for i in range(self.n):
+            self._x[i], self._y[i] = x_ptrs[i], y_ptrs[i]
+        _check(lib().etp_linear_run(self.handle, self._x, tokens, self._y, stream or None))
+
+    def info(self) -> Dict[str, object]:
+        st = etp_linear_plan_stats()
+        _check(lib().etp_linear_plan_info(self.handle, C.byref(st)))
+        d = {n: getattr(st, n) for n, _ in st._fields_ if n != "n_splits"}
+        d["n_splits"] = list(st.n_splits)[: st.n_linears]
+        return d
+
+    def close(self) -> None:
+        if getattr(self, "handle", None) and _lib is not None and getattr(self.ctx, "handle", None):
+            _lib.etp_linear_free(self.handle)
+        self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def etp_moe_linear(ctx: Context, mode: int, dtype: str, x_ptr: int, row_offsets: Sequence[int], in_features: int, out_features: int,

@@ -57,6 +57,7 @@ extern "C" etp_status etp_ctx_create(int device, int64_t staging_bytes, etp_ctx*
     c->opts[ETP_OPT_GATHER_CTAS] = 16;
     c->opts[ETP_OPT_LINEAR_CTA_PAIR] = 1;
     c->opts[ETP_OPT_VALIDATE_INTERVALS] = 1;
+    c->opts[ETP_OPT_LINEAR_PDL] = 1;
     CtxExtra* x = new (std::nothrow) CtxExtra();
     if (!x) { delete c; ETP_FAIL(ETP_ERR_NOMEM, "etp_ctx_create: out of memory"); }
     c->impl = x;
@@ -92,8 +93,7 @@ extern "C" void etp_ctx_destroy(etp_ctx* c) {
     }
     for (cudaEvent_t e : c->events) cudaEventDestroy(e);
     for (cudaEvent_t e : c->tev) cudaEventDestroy(e);
-    if (c->lin_ws) cudaFree(c->lin_ws);
-    if (c->lin_tickets) cudaFree(c->lin_tickets);
+    etp::lin_teardown(c);
     if (c->moe_items) cudaFree(c->moe_items);
     cudaGetLastError();
     delete c;

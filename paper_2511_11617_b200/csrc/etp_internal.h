@@ -124,10 +124,7 @@ struct etp_ctx {
     int32_t launches = 0;               // kernels launched by the last call
     std::vector<cudaEvent_t> tev;       // timing events (pairs) around copy-stream launches, ETP_OPT_TIME_KERNELS
     int32_t n_timed = 0;                // pairs recorded by the last call
-    void* lin_ws = nullptr;             // split-K workspace of etp_shard_linear (fp32 partial tiles), grown on demand
-    int64_t lin_ws_bytes = 0;
-    unsigned int* lin_tickets = nullptr; // per-tile arrival tickets of the split-K reduction (zero between launches)
-    int64_t lin_tickets_n = 0;
+    void* lin_state = nullptr;          // kernel (c): per-stream split-K workspaces + the cache of prepared groups (etp_linear_group.cu)
     void* moe_items = nullptr;          // work-item table of etp_moe_linear (device), grown on demand
     int64_t moe_items_bytes = 0;
 };
@@ -146,6 +143,9 @@ etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n
 etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* g, const etp_plan* head_plan, const int32_t* pairs,
                     int64_t n_pairs, LoweredWork* out);
 void push_contiguous(const etp_ctx* ctx, JobList* jl, const void* src, void* dst, int64_t bytes);
+
+// kernel (c): frees the ctx-owned cache of prepared groups and the split-K workspaces (etp_linear_group.cu)
+void lin_teardown(etp_ctx* ctx);
 
 // execution (device): etp_exec.cu
 etp_status execute(etp_ctx* ctx, LoweredWork* w, void* copy_stream, void* reload_stream, etp_reshard_report* report);

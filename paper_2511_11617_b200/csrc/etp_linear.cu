@@ -1,5 +1,6 @@
-// Kernel (c): unequal-width column/row-parallel shard linear on the 5th-gen tensor cores (tcgen05 + TMEM, fed by TMA).
-// PAPER.md:45 ("unequal-width partitioning ... for attention and linear layers"), :92-94 (shard widths floor/ceil of S/g_t).
+// Kernel (c), tensor-bound regime (> 64 tokens): unequal-width column/row-parallel shard linear on the 5th-gen tensor cores
+// (tcgen05 + TMEM, fed by TMA).  PAPER.md:45 ("unequal-width partitioning ... for attention and linear layers"), :92-94 (shard
+// widths floor/ceil of S/g_t).  The weight-streaming regime (<= 64 tokens) lives in etp_linear_group.cu.
 //
 //   Y[tokens][out] = X[tokens][in] . W^T        fp32 accumulation, one round-to-nearest-even cast to 16 bit (G2)
 //
@@ -8,39 +9,28 @@
 //   ETP_ROW_PARALLEL  W is cut along in-features, stored transposed [in][out]; the rank partial sums are accumulated in
 //                     ONE TMEM accumulator by walking the K loop over the ranks' runs in ascending unit order.
 //
-// Mapping onto the MMA (the roles of the operands are swapped so the wide weight dimension fills the 128 MMA rows and the
-// token count - 4 in config 1 - only costs MMA columns):
-//   D[m = out feature (128 TMEM lanes)][n = token (BN fp32 columns)] += A[m][k] . B[n][k]
+// Mapping onto the MMA (the roles of the operands are swapped so the wide weight dimension fills the 128 MMA rows):
+//   D[m = out feature (128 TMEM lanes)][n = token (256 fp32 columns)] += A[m][k] . B[n][k]
 //   A = weight tile: K-major for column-parallel (rows of W), MN-major for row-parallel (rows of W^T are K, out is contiguous)
-//   B = X tile [BN tokens][64 k], always K-major.
+//   B = X tile [256 tokens][64 k], always K-major.
 // Ragged shard edges never need a special path: every run has its own TMA tensor map, so rows past the end of a run are
 // zero-filled by the TMA unit (out-of-bounds fill) and the epilogue masks them.
 //
-// CTA = 6 warps: warp 0 TMA producer, warp 1 MMA issuer (+ TMEM allocation), warps 2-5 epilogue (tcgen05.ld -> 16-bit
-// stores, or fp32 split-K partials + ticketed last-arriver reduction in fixed split order, so results are deterministic).
-// Persistent grid, static round-robin over (m tile, token tile, k split) items; two TMEM accumulator stages so the epilogue
-// of item i overlaps the MMAs of item i+1.
+// CTA = 6 warps: warp 0 TMA producer, warp 1 MMA issuer (+ TMEM allocation), warps 2-5 epilogue (tcgen05.ld -> 16-bit stores).
+// Persistent grid, static round-robin over (m tile, token tile) items; two TMEM accumulator stages so the epilogue of item i
+// overlaps the MMAs of item i+1.  CTA pairs (cta_group::2) are the default above 64 tokens (second kernel below).
 
 #include <algorithm>
 #include <cstring>
 #include <vector>
 
-#include "etp_tc.cuh"
+#include "etp_linear.cuh"
 
 using namespace etp;
 using namespace etp::tc;
+using namespace etp::lin;
 
 namespace {
-
-constexpr int kMaxLinRuns = 32;   // <= 2 contiguous runs per rank, 8 ranks, up to 3 fused linears (q|k|v) - capped at 32
-
-struct Run {          // one contiguous slot range of a rank's shard, runs sorted by (linear, global feature)
-    int64_t feat0;    // first global feature of the run (out-feature: column-parallel, in-feature: row-parallel)
-    int32_t n_feat;   // features in the run
-    int32_t first;    // column-parallel: index of the run's first m tile; row-parallel: of its first K chunk entry
-    void* y;          // column-parallel: output of the linear this run belongs to (etp_shard_linear_multi fuses several)
-    int32_t out_features, pad;   // ... and its row pitch
-};
 
 struct alignas(64) LinearParams {
     CUtensorMap map_x;
@@ -48,10 +38,10 @@ struct alignas(64) LinearParams {
     Run runs[kMaxLinRuns];
     int32_t n_runs, mode, dtype;
     int32_t tokens, in_features, out_features;
-    int32_t n_m_tiles, n_n_tiles, n_splits, n_chunks;   // n_chunks: K chunks of kBK per output tile
+    int32_t n_m_tiles, n_n_tiles, n_chunks, pad0;   // n_chunks: K chunks of kBK per output tile
     void* y;
-    float* partials;          // split-K workspace [(tile * n_splits + split)][BN][128]
-    unsigned int* tickets;    // one per output tile, zero between launches (the last arriver resets its ticket)
+    float* partials;          // CTA-pair tail split: fp32 partial tiles [(tail item * 2 + CTA rank) * tail_splits + split][256][128]
+    unsigned int* tickets;    // ... one arrival ticket per (tail item, CTA rank), zero between launches
     int32_t tail_first, tail_splits;   // CTA-pair kernel: items >= tail_first (the grid's last, partial round) are cut into
                                        // tail_splits K ranges, one per CTA pair (0 / 1 = no split)
 };
@@ -66,16 +56,14 @@ struct Cfg {
 };
 
 struct Item {
-    int m, n, split, tile, c0, c1;
+    int m, n, c0, c1;
 };
 __device__ __forceinline__ Item decode_item(const LinearParams& p, int item) {
     Item it;
-    it.split = item % p.n_splits;
-    it.tile = item / p.n_splits;
-    it.n = it.tile % p.n_n_tiles;
-    it.m = it.tile / p.n_n_tiles;
-    it.c0 = int(int64_t(it.split) * p.n_chunks / p.n_splits);
-    it.c1 = int(int64_t(it.split + 1) * p.n_chunks / p.n_splits);
+    it.n = item % p.n_n_tiles;
+    it.m = item / p.n_n_tiles;
+    it.c0 = 0;
+    it.c1 = p.n_chunks;
     return it;
 }
 __device__ __forceinline__ int find_run(const LinearParams& p, int key) {   // last run with first <= key
@@ -94,10 +82,9 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
     uint64_t* tmem_full = empty_bar + C::kStages;
     uint64_t* tmem_empty = tmem_full + 2;
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
-    uint32_t* last_flag = tmem_ptr + 1;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n_items = p.n_m_tiles * p.n_n_tiles * p.n_splits;
+    const int n_items = p.n_m_tiles * p.n_n_tiles;
     const bool row_par = p.mode == ETP_ROW_PARALLEL;
 
     if (warp == 0 && lane == 1) {
@@ -228,67 +215,21 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_shard_linear_kernel(const 
             mbar_wait(&tmem_full[as], aph);
             tc_fence_after();
             const uint32_t taddr = tmem_base + uint32_t(as * BN) + (uint32_t(q * 32) << 16);
-            float* ws = p.partials + (size_t(it.tile) * p.n_splits + it.split) * size_t(BN) * kBM;
             for (int c16 = 0; c16 < n_tok; c16 += 16) {
                 uint32_t v[16];
                 tc_ld16(taddr + uint32_t(c16), v);
                 tc_ld_wait();
-                if (p.n_splits == 1 && vec_out) {
+                if (vec_out) {
                     store_block16(stage_t, v, m_local, y, size_t(t0 + c16), min(16, n_tok - c16), outf, gm0, valid);
-                } else if (p.n_splits == 1) {
-                    if (m_local < valid) {
-#pragma unroll
-                        for (int j = 0; j < 16; ++j)
-                            if (c16 + j < n_tok) y[size_t(t0 + c16 + j) * outf + gm0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
-                    }
-                } else {
+                } else if (m_local < valid) {
 #pragma unroll
                     for (int j = 0; j < 16; ++j)
-                        if (c16 + j < n_tok) ws[(c16 + j) * kBM + m_local] = __uint_as_float(v[j]);
+                        if (c16 + j < n_tok) y[size_t(t0 + c16 + j) * outf + gm0 + m_local] = cvt16<OutT>(__uint_as_float(v[j]));
                 }
             }
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(&tmem_empty[as]);
-            if (p.n_splits > 1) {
-                // split-K: the last split to arrive at this tile sums the fp32 partials in split order 0..S-1 (deterministic)
-                __threadfence();
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                if (threadIdx.x == 64) *last_flag = (atomicAdd(&p.tickets[it.tile], 1u) == uint32_t(p.n_splits - 1)) ? 1u : 0u;
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                if (*last_flag) {
-                    __threadfence();
-                    const float* w0 = p.partials + size_t(it.tile) * p.n_splits * size_t(BN) * kBM;
-                    // 32 threads x float4 cover the 128 features of one token, the four warps take tokens q, q+4, ...; the partials
-                    // of four splits are loaded together (independent L2 round trips) and added in split order 0..S-1.
-                    const int col4 = lane * 4;
-                    const bool vec8 = ((gm0 | outf) & 3) == 0;
-                    for (int j = q; j < n_tok; j += 4) {
-                        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-                        for (int s0 = 0; s0 < p.n_splits; s0 += 4) {
-                            float4 t[4];
-#pragma unroll
-                            for (int u = 0; u < 4; ++u)
-                                t[u] = s0 + u < p.n_splits ? __ldcg(reinterpret_cast<const float4*>(w0 + (size_t(s0 + u) * BN + j) * kBM + col4))
-                                                           : make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-                            for (int u = 0; u < 4; ++u)
-                                if (s0 + u < p.n_splits) { acc.x += t[u].x; acc.y += t[u].y; acc.z += t[u].z; acc.w += t[u].w; }
-                        }
-                        OutT o[4] = {cvt16<OutT>(acc.x), cvt16<OutT>(acc.y), cvt16<OutT>(acc.z), cvt16<OutT>(acc.w)};
-                        OutT* dst = y + size_t(t0 + j) * outf + gm0 + col4;
-                        if (vec8 && col4 + 4 <= valid) {
-                            *reinterpret_cast<uint2*>(dst) = *reinterpret_cast<const uint2*>(o);
-                        } else {
-#pragma unroll
-                            for (int e = 0; e < 4; ++e)
-                                if (col4 + e < valid) dst[e] = o[e];
-                        }
-                    }
-                    if (threadIdx.x == 64) p.tickets[it.tile] = 0;
-                }
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-            }
         }
     }
 
@@ -604,34 +545,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kLinThreads, 1) etp_
 }
 
 // ------------------------------------------------------------------------------------------------ host side
-// Number of K splits: a function of the nominal shapes only (never of the shard layout), so a column-parallel output is
-// bit-identical before and after a reshard (G3).  Splitting only pays when few output tiles exist (small T).
-int choose_splits(int64_t nominal_tiles, int nominal_chunks, int n_sms, int bn) {
-    if (bn > 64 || nominal_chunks < 2) return 1;
-    int best = 1;
-    int64_t best_cost = INT64_MAX;
-    for (int s = 1; s <= std::min(nominal_chunks, 16); ++s) {
-        const int64_t waves = (nominal_tiles * s + n_sms - 1) / n_sms;
-        const int64_t cost = waves * ((nominal_chunks + s - 1) / s + 6) + (s > 1 ? 2 : 0);
-        if (cost < best_cost) { best_cost = cost; best = s; }
-    }
-    return best;
-}
-
 template <int BN>
 etp_status launch_linear(const LinearParams& p, int grid, cudaStream_t stream) {
     using C = Cfg<BN>;
-    cudaError_t e;
+    static bool configured[2] = {false, false};   // the attribute belongs to the function: set once per process
     if (p.dtype == ETP_BF16) {
         auto k = etp_shard_linear_kernel<BN, __nv_bfloat16>;
-        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes));
+        if (!configured[0]) { ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes)); configured[0] = true; }
         k<<<grid, kLinThreads, C::kSmemBytes, stream>>>(p);
     } else {
         auto k = etp_shard_linear_kernel<BN, __half>;
-        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes));
+        if (!configured[1]) { ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes)); configured[1] = true; }
         k<<<grid, kLinThreads, C::kSmemBytes, stream>>>(p);
     }
-    e = cudaGetLastError();
+    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) ETP_FAIL(ETP_ERR_CUDA, "etp_shard_linear: launch failed: %s", cudaGetErrorString(e));
     return ETP_OK;
 }
@@ -639,13 +566,14 @@ etp_status launch_linear(const LinearParams& p, int grid, cudaStream_t stream) {
 template <int PBN>
 etp_status launch_linear_pair(const LinearParams& p, int grid, cudaStream_t stream) {
     constexpr int kPairSmemBytes = PairCfg<PBN>::kSmemBytes;
+    static bool configured[2] = {false, false};
     if (p.dtype == ETP_BF16) {
         auto k = etp_shard_linear_pair_kernel<PBN, __nv_bfloat16>;
-        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmemBytes));
+        if (!configured[0]) { ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmemBytes)); configured[0] = true; }
         k<<<grid, kLinThreads, kPairSmemBytes, stream>>>(p);
     } else {
         auto k = etp_shard_linear_pair_kernel<PBN, __half>;
-        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmemBytes));
+        if (!configured[1]) { ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmemBytes)); configured[1] = true; }
         k<<<grid, kLinThreads, kPairSmemBytes, stream>>>(p);
     }
     cudaError_t e = cudaGetLastError();
@@ -655,114 +583,99 @@ etp_status launch_linear_pair(const LinearParams& p, int grid, cudaStream_t stre
 
 }  // namespace
 
-namespace {
-struct LinOut {   // one linear of a (possibly fused) launch
-    const etp_tensor* w;
-    int64_t out_features, features_per_unit;
-    void* y;
-};
-}  // namespace
+namespace etp {
+namespace lin {
 
-// Column-parallel: n_outs >= 1 linears that share X, in_features and the shard layout of their class (q|k|v, gate|up) in ONE
-// launch - the runs of all of them are concatenated and every run carries its own Y.  Row-parallel: n_outs == 1.
-static etp_status shard_linear_impl(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x, int64_t tokens,
-                                    int64_t in_features, const LinOut* outs, int32_t n_outs, const etp_shard* layout,
-                                    int32_t n_shards, void* stream) {
-    if (!ctx || !outs || !layout || n_outs < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: NULL argument");
-    if (mode != ETP_COL_PARALLEL && mode != ETP_ROW_PARALLEL) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: bad mode %d", int(mode));
-    if (dtype != ETP_BF16 && dtype != ETP_FP16) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: dtype %d is not bf16/fp16", int(dtype));
+etp_status check_linear_shape(etp_linear_mode mode, int64_t in_features, int64_t out_features, int64_t features_per_unit,
+                              const etp_tensor* w) {
+    if (in_features <= 0 || out_features <= 0 || features_per_unit <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: non-positive size");
+    if (in_features >= (int64_t(1) << 31) || out_features >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: sizes must be below 2^31");
     const bool row_par = mode == ETP_ROW_PARALLEL;
-    if (row_par && n_outs != 1) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear_multi: only column-parallel linears can be fused");
-    if (tokens < 0 || in_features <= 0 || n_shards <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: non-positive size");
-    if (tokens >= (int64_t(1) << 31) || in_features >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: sizes must be below 2^31");
-    int64_t out_total = 0;
-    for (int32_t o = 0; o < n_outs; ++o) {
-        const etp_tensor* w = outs[o].w;
-        const int64_t out_features = outs[o].out_features, features_per_unit = outs[o].features_per_unit;
-        if (!w || !w->slabs) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: NULL argument");
-        if (out_features <= 0 || features_per_unit <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: non-positive size");
-        if (out_features >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: sizes must be below 2^31");
-        const int64_t sharded = row_par ? in_features : out_features;   // the dimension the weight is cut along
-        const int64_t row_len = row_par ? out_features : in_features;   // contiguous elements per feature row of the stored weight
-        if (w->total_units * features_per_unit != sharded)
-            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: total_units %lld x features_per_unit %lld != sharded dimension %lld",
-                     (long long)w->total_units, (long long)features_per_unit, (long long)sharded);
-        if (w->unit_bytes != features_per_unit * row_len * 2)
-            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: unit_bytes %lld != features_per_unit x row length x 2 = %lld",
-                     (long long)w->unit_bytes, (long long)(features_per_unit * row_len * 2));
-        if ((in_features * 2) % 16 || (row_len * 2) % 16)
-            ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: row pitches must be multiples of 16 bytes (in %lld, stored row %lld elements)",
-                     (long long)in_features, (long long)row_len);
-        if (w->total_units != outs[0].w->total_units)
-            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear_multi: fused linears must belong to one granularity class (%lld vs %lld units)",
-                     (long long)w->total_units, (long long)outs[0].w->total_units);
-        out_total += out_features;
-    }
-    if (tokens == 0) return ETP_OK;
-    if (!x) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: x / y is NULL");
-    if (reinterpret_cast<uintptr_t>(x) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: x / y not 16-byte aligned");
-    for (int32_t o = 0; o < n_outs; ++o) {
-        if (!outs[o].y) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: x / y is NULL");
-        if (reinterpret_cast<uintptr_t>(outs[o].y) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: x / y not 16-byte aligned");
-    }
-    const int64_t out_features = outs[0].out_features;   // row-parallel: the one linear's width
-    void* const y = outs[0].y;
-    const int64_t total_units = outs[0].w->total_units;
+    const int64_t sharded = row_par ? in_features : out_features;   // the dimension the weight is cut along
+    const int64_t row_len = row_par ? out_features : in_features;   // contiguous elements per feature row of the stored weight
+    if (w->total_units * features_per_unit != sharded)
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: total_units %lld x features_per_unit %lld != sharded dimension %lld",
+                 (long long)w->total_units, (long long)features_per_unit, (long long)sharded);
+    if (w->unit_bytes != features_per_unit * row_len * 2)
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: unit_bytes %lld != features_per_unit x row length x 2 = %lld",
+                 (long long)w->unit_bytes, (long long)(features_per_unit * row_len * 2));
+    if ((in_features * 2) % 16 || (row_len * 2) % 16)
+        ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: row pitches must be multiples of 16 bytes (in %lld, stored row %lld elements)",
+                 (long long)in_features, (long long)row_len);
+    return ETP_OK;
+}
 
-    // ---- the shards in ascending unit order must tile [0, total_units)
-    std::vector<etp_shard> sh;
+// the shards in ascending unit order must tile [0, total_units)
+etp_status check_layout(const etp_shard* layout, int32_t n_shards, int64_t total_units, std::vector<etp_shard>* sh) {
+    sh->clear();
+    if (!layout || n_shards <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: empty layout");
     for (int i = 0; i < n_shards; ++i)
-        if (layout[i].alive && layout[i].end > layout[i].begin) sh.push_back(layout[i]);
-    std::sort(sh.begin(), sh.end(), [](const etp_shard& a, const etp_shard& b) { return a.begin < b.begin; });
+        if (layout[i].alive && layout[i].end > layout[i].begin) sh->push_back(layout[i]);
+    std::sort(sh->begin(), sh->end(), [](const etp_shard& a, const etp_shard& b) { return a.begin < b.begin; });
     int64_t cursor = 0;
-    for (const etp_shard& s : sh) {
+    for (const etp_shard& s : *sh) {
         if (s.begin != cursor) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: layout does not tile [0,%lld): gap or overlap at unit %lld", (long long)total_units, (long long)cursor);
         cursor = s.end;
     }
     if (cursor != total_units) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: layout covers %lld of %lld units", (long long)cursor, (long long)total_units);
+    return ETP_OK;
+}
 
-    // ---- contiguous runs of every shard inside its slot-addressed slab (L3), linear by linear
-    LinearParams p;
-    std::memset(&p, 0, sizeof(p));
-    const void* run_addr[kMaxLinRuns];
-    int n_runs = 0;
-    for (int32_t o = 0; o < n_outs; ++o) {
-        const etp_tensor* w = outs[o].w;
-        const int64_t features_per_unit = outs[o].features_per_unit;
-        for (const etp_shard& s : sh) {
-            if (s.rank < 0 || s.rank >= w->n_ranks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d outside the tensor's %d slabs", s.rank, w->n_ranks);
-            const etp_slab& sl = w->slabs[s.rank];
-            if (!sl.base) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d has no slab", s.rank);
-            if (reinterpret_cast<uintptr_t>(sl.base) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: slab of rank %d not 16-byte aligned", s.rank);
-            const int64_t width = s.end - s.begin;
-            if (sl.cap_units <= 0 || width > sl.cap_units) ETP_FAIL(ETP_ERR_CAPACITY, "etp_shard_linear: shard of rank %d (%lld units) exceeds its slab (%lld)", s.rank, (long long)width, (long long)sl.cap_units);
-            int64_t slot0 = (s.begin - sl.anchor_unit) % sl.cap_units;
-            if (slot0 < 0) slot0 += sl.cap_units;
-            const int64_t len1 = std::min(width, sl.cap_units - slot0);
-            const int64_t piece_b[2] = {s.begin, s.begin + len1};
-            const int64_t piece_n[2] = {len1, width - len1};
-            const int64_t piece_slot[2] = {slot0, 0};
-            for (int k = 0; k < 2; ++k) {
-                if (piece_n[k] == 0) continue;
-                if (n_runs == kMaxLinRuns) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: more than %d contiguous runs", kMaxLinRuns);
-                if (piece_n[k] * features_per_unit >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: run too long");
-                p.runs[n_runs].feat0 = piece_b[k] * features_per_unit;
-                p.runs[n_runs].n_feat = int32_t(piece_n[k] * features_per_unit);
-                p.runs[n_runs].y = outs[o].y;
-                p.runs[n_runs].out_features = int32_t(outs[o].out_features);
-                run_addr[n_runs] = static_cast<const char*>(sl.base) + piece_slot[k] * w->unit_bytes;
-                ++n_runs;
-            }
+// contiguous runs of every shard inside its slot-addressed slab (L3), appended in ascending unit order
+etp_status append_runs(const etp_tensor* w, const std::vector<etp_shard>& sh, int64_t features_per_unit, void* y, int64_t out_features,
+                       RunList* out) {
+    for (const etp_shard& s : sh) {
+        if (s.rank < 0 || s.rank >= w->n_ranks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d outside the tensor's %d slabs", s.rank, w->n_ranks);
+        const etp_slab& sl = w->slabs[s.rank];
+        if (!sl.base) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: rank %d has no slab", s.rank);
+        if (reinterpret_cast<uintptr_t>(sl.base) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: slab of rank %d not 16-byte aligned", s.rank);
+        const int64_t width = s.end - s.begin;
+        if (sl.cap_units <= 0 || width > sl.cap_units) ETP_FAIL(ETP_ERR_CAPACITY, "etp_shard_linear: shard of rank %d (%lld units) exceeds its slab (%lld)", s.rank, (long long)width, (long long)sl.cap_units);
+        int64_t slot0 = (s.begin - sl.anchor_unit) % sl.cap_units;
+        if (slot0 < 0) slot0 += sl.cap_units;
+        const int64_t len1 = std::min(width, sl.cap_units - slot0);
+        const int64_t piece_b[2] = {s.begin, s.begin + len1};
+        const int64_t piece_n[2] = {len1, width - len1};
+        const int64_t piece_slot[2] = {slot0, 0};
+        for (int k = 0; k < 2; ++k) {
+            if (piece_n[k] == 0) continue;
+            if (out->n == kMaxLinRuns) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: more than %d contiguous runs", kMaxLinRuns);
+            if (piece_n[k] * features_per_unit >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: run too long");
+            Run& R = out->runs[out->n];
+            R.feat0 = piece_b[k] * features_per_unit;
+            R.n_feat = int32_t(piece_n[k] * features_per_unit);
+            R.first = 0;
+            R.y = y;
+            R.out_features = int32_t(out_features);
+            R.pad = 0;
+            out->addr[out->n] = static_cast<const char*>(sl.base) + piece_slot[k] * w->unit_bytes;
+            ++out->n;
         }
     }
+    return ETP_OK;
+}
 
-    // ---- tiling
-    const int bn = tokens <= 16 ? 16 : (tokens <= 64 ? 64 : 256);
-    // > 64 tokens: CTA pairs (256 out features x 256 tokens per pair) unless single-CTA 128 x 256 tiles need fewer rounds of
-    // the persistent grid (few, ragged m tiles: e.g. 1024 out features in runs of 384/384/256).  Per item a pair takes ~0.93
-    // of the single-CTA time (it stages 32 KiB instead of 48 KiB per K chunk and SM; measured on the config-2 shapes).
+// > 64 tokens.  Column-parallel: n_outs >= 1 linears that share X, in_features and the shard layout of their class (q|k|v, gate|up)
+// in ONE launch - the runs of all of them are concatenated and every run carries its own Y.  Row-parallel: n_outs == 1.
+etp_status shard_linear_large(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x, int64_t tokens, int64_t in_features,
+                              const LinOut* outs, int32_t n_outs, const etp_shard* layout, int32_t n_shards, void* stream) {
+    const bool row_par = mode == ETP_ROW_PARALLEL;
+    const int64_t out_features = outs[0].out_features;   // row-parallel: the one linear's width
+    std::vector<etp_shard> sh;
+    ETP_TRY(check_layout(layout, n_shards, outs[0].w->total_units, &sh));
+    RunList rl;
+    for (int32_t o = 0; o < n_outs; ++o) ETP_TRY(append_runs(outs[o].w, sh, outs[o].features_per_unit, outs[o].y, outs[o].out_features, &rl));
+    LinearParams p;
+    std::memset(&p, 0, sizeof(p));
+    const int n_runs = rl.n;
+    for (int r = 0; r < n_runs; ++r) p.runs[r] = rl.runs[r];
+
+    // ---- tiling: CTA pairs (256 out features x 256 tokens per pair) unless single-CTA 128 x 256 tiles need fewer rounds of the
+    // persistent grid (few, ragged m tiles: e.g. 1024 out features in runs of 384/384/256).  Per item a pair takes ~0.93 of the
+    // single-CTA time (it stages 32 KiB instead of 48 KiB per K chunk and SM; measured on the config-2 shapes).
+    constexpr int bn = 256;
     const int64_t pair_opt = ctx->opts[ETP_OPT_LINEAR_CTA_PAIR];
-    bool pair = bn == 256 && pair_opt != 0 && ctx->n_sms >= 2;
+    bool pair = pair_opt != 0 && ctx->n_sms >= 2;
     const int pbn = pair_opt == 128 ? 128 : 256;
     if (pair && pair_opt == 1) {
         int64_t mt_single = 0, mt_pair = 0;
@@ -788,7 +701,7 @@ static etp_status shard_linear_impl(etp_ctx* ctx, etp_linear_mode mode, etp_dtyp
     p.in_features = int32_t(in_features);
     p.out_features = int32_t(out_features);
     p.n_n_tiles = int32_t((tokens + tile_n - 1) / tile_n);
-    p.y = y;
+    p.y = outs[0].y;
     int32_t acc = 0;
     for (int r = 0; r < n_runs; ++r) {
         p.runs[r].first = acc;
@@ -802,17 +715,13 @@ static etp_status shard_linear_impl(etp_ctx* ctx, etp_linear_mode mode, etp_dtyp
         p.n_m_tiles = acc;
         p.n_chunks = int32_t((in_features + kBK - 1) / kBK);
     }
-    int64_t nominal_m = 0;
-    for (int32_t o = 0; o < n_outs; ++o) nominal_m += (outs[o].out_features + kBM - 1) / kBM;
-    const int64_t nominal_tiles = nominal_m * p.n_n_tiles;
-    p.n_splits = std::min(choose_splits(nominal_tiles, int((in_features + kBK - 1) / kBK), ctx->n_sms, bn), p.n_chunks);
-    const int64_t n_tiles = int64_t(p.n_m_tiles) * p.n_n_tiles;
-    const int64_t n_items = n_tiles * p.n_splits;
+    const int64_t n_items = int64_t(p.n_m_tiles) * p.n_n_tiles;
     if (n_items >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: too many work items");
 
     // CTA pairs, row-parallel: a partial last round of the persistent grid is cut along K over the idle pairs (row-parallel only:
     // its items depend on the nominal shapes alone, and reading G3 keeps column-parallel outputs independent of the layout)
-    int64_t ws_tiles = n_tiles, ws_splits = p.n_splits, ws_bn = bn;
+    ETP_CUDA_OK(cudaSetDevice(ctx->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (pair && row_par && pbn == 256 && pair_opt != 256) {
         const int64_t units = ctx->n_sms / 2, tail = n_items % units;
         if (n_items > units && tail > 0) {
@@ -820,55 +729,60 @@ static etp_status shard_linear_impl(etp_ctx* ctx, etp_linear_mode mode, etp_dtyp
             if (S >= 2) {
                 p.tail_first = int32_t(n_items - tail);
                 p.tail_splits = int32_t(S);
-                ws_tiles = tail * 2;
-                ws_splits = S;
-                ws_bn = pbn;
+                LinWorkspace w;   // per stream: calls on different streams of one ctx never share partial tiles or tickets
+                ETP_TRY(linear_workspace(ctx, st, tail * 2 * S * pbn * kBM * int64_t(sizeof(float)), tail * 2, &w));
+                p.partials = w.partials;
+                p.tickets = w.tickets;
             }
         }
-    }
-
-    ETP_CUDA_OK(cudaSetDevice(ctx->device));
-    if (p.n_splits > 1 || p.tail_splits > 1) {   // split-K workspace, owned by the ctx and grown on demand (calls on one ctx must not overlap in time)
-        const int64_t n_tiles = ws_tiles;
-        const int64_t need = n_tiles * ws_splits * ws_bn * kBM * int64_t(sizeof(float));
-        if (need > ctx->lin_ws_bytes) {
-            if (ctx->lin_ws) ETP_CUDA_OK(cudaFree(ctx->lin_ws));
-            ctx->lin_ws = nullptr;
-            ctx->lin_ws_bytes = 0;
-            ETP_CUDA_OK(cudaMalloc(&ctx->lin_ws, size_t(need)));
-            ctx->lin_ws_bytes = need;
-        }
-        if (n_tiles > ctx->lin_tickets_n) {
-            if (ctx->lin_tickets) ETP_CUDA_OK(cudaFree(ctx->lin_tickets));
-            ctx->lin_tickets = nullptr;
-            ctx->lin_tickets_n = 0;
-            const int64_t n = std::max<int64_t>(n_tiles, 4096);
-            ETP_CUDA_OK(cudaMalloc(&ctx->lin_tickets, size_t(n) * sizeof(unsigned int)));
-            ETP_CUDA_OK(cudaMemset(ctx->lin_tickets, 0, size_t(n) * sizeof(unsigned int)));
-            ETP_CUDA_OK(cudaDeviceSynchronize());
-            ctx->lin_tickets_n = n;
-        }
-        p.partials = static_cast<float*>(ctx->lin_ws);
-        p.tickets = ctx->lin_tickets;
     }
 
     // ---- tensor maps: X [tokens][in]; one map per run so that TMA zero-fills everything past a run's end
     ETP_TRY(encode_2d(&p.map_x, dtype, x, tokens, in_features, in_features, kBK, pair ? pbn / 2 : bn));
     for (int r = 0; r < n_runs; ++r) {
-        if (row_par) ETP_TRY(encode_2d(&p.map_w[r], dtype, run_addr[r], p.runs[r].n_feat, out_features, out_features, 64, kBK));
-        else ETP_TRY(encode_2d(&p.map_w[r], dtype, run_addr[r], p.runs[r].n_feat, in_features, in_features, kBK, kBM));
+        if (row_par) ETP_TRY(encode_2d(&p.map_w[r], dtype, rl.addr[r], p.runs[r].n_feat, out_features, out_features, 64, kBK));
+        else ETP_TRY(encode_2d(&p.map_w[r], dtype, rl.addr[r], p.runs[r].n_feat, in_features, in_features, kBK, kBM));
     }
 
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
     ctx->launches = 1;
     if (pair) {
         const int pgrid = 2 * int(std::min<int64_t>(n_items, ctx->n_sms / 2));
         return pbn == 128 ? launch_linear_pair<128>(p, pgrid, st) : launch_linear_pair<256>(p, pgrid, st);
     }
-    const int grid = int(std::min<int64_t>(n_items, ctx->n_sms));
-    if (bn == 16) return launch_linear<16>(p, grid, st);
-    if (bn == 64) return launch_linear<64>(p, grid, st);
-    return launch_linear<256>(p, grid, st);
+    return launch_linear<256>(p, int(std::min<int64_t>(n_items, ctx->n_sms)), st);
+}
+
+}  // namespace lin
+}  // namespace etp
+
+// argument checks shared by the two legacy entry points, then the regime split
+static etp_status shard_linear_impl(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x, int64_t tokens,
+                                    int64_t in_features, const LinOut* outs, int32_t n_outs, const etp_shard* layout,
+                                    int32_t n_shards, void* stream) {
+    if (!ctx || !outs || !layout || n_outs < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: NULL argument");
+    if (mode != ETP_COL_PARALLEL && mode != ETP_ROW_PARALLEL) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: bad mode %d", int(mode));
+    if (dtype != ETP_BF16 && dtype != ETP_FP16) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear: dtype %d is not bf16/fp16", int(dtype));
+    const bool row_par = mode == ETP_ROW_PARALLEL;
+    if (row_par && n_outs != 1) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_shard_linear_multi: only column-parallel linears can be fused");
+    if (tokens < 0 || in_features <= 0 || n_shards <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: non-positive size");
+    if (tokens >= (int64_t(1) << 31) || in_features >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: sizes must be below 2^31");
+    for (int32_t o = 0; o < n_outs; ++o) {
+        const etp_tensor* w = outs[o].w;
+        if (!w || !w->slabs) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: NULL argument");
+        ETP_TRY(check_linear_shape(mode, in_features, outs[o].out_features, outs[o].features_per_unit, w));
+        if (w->total_units != outs[0].w->total_units)
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear_multi: fused linears must belong to one granularity class (%lld vs %lld units)",
+                     (long long)w->total_units, (long long)outs[0].w->total_units);
+    }
+    if (tokens == 0) return ETP_OK;
+    if (!x) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: x / y is NULL");
+    if (reinterpret_cast<uintptr_t>(x) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: x / y not 16-byte aligned");
+    for (int32_t o = 0; o < n_outs; ++o) {
+        if (!outs[o].y) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_shard_linear: x / y is NULL");
+        if (reinterpret_cast<uintptr_t>(outs[o].y) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_shard_linear: x / y not 16-byte aligned");
+    }
+    if (tokens <= 64) return shard_linear_small(ctx, mode, dtype, x, tokens, in_features, outs, n_outs, layout, n_shards, stream);
+    return shard_linear_large(ctx, mode, dtype, x, tokens, in_features, outs, n_outs, layout, n_shards, stream);
 }
 
 extern "C" etp_status etp_shard_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x, int64_t tokens,

@@ -401,3 +401,149 @@ def smoke_shard_linear(ctx):
     TR.run_param_step(ctx, world, bufs, images, 0, Streams())
     outs = linear_checks_for_world(ctx, world, bufs, world.steps[0].new, cfg.tokens, dead=world.steps[0].dead)
     print(f"smoke shard_linear OK: {len(outs)} linears of config 1 on the resharded layout within {TOL} of the unsharded reference")
+
+
+# ------------------------------------------------------------------------------------------------ prepared groups (etp_linear_prepare / etp_linear_run)
+def _make_linear(mode, K, N, fpu, widths, seed_i, gmode="wrap", dtype="bf16"):
+    """One sharded weight on the device (NaN-filled slack) -> (PreparedLinear, w bytes, DevBufs to keep alive)."""
+    transposed = mode == "row"
+    units = (K if transposed else N) // fpu
+    assert sum(widths) == units
+    row_len = N if transposed else K
+    ub = fpu * row_len * 2
+    dt = torch_dtype(dtype)
+    w_u8 = as_u8(fill_normal16(SEED, 900 + seed_i, 0, K * N, 0.02, dt)).copy()
+    layout = widths_to_layout(widths)
+    geom = {}
+    for (r, b, e, _) in layout:
+        if gmode == "tight":
+            geom[r] = (b, e - b)
+        else:
+            cap = (e - b) + 1 + r
+            geom[r] = (b - (cap - (e - b) // 2) % cap, cap)
+    slabs = shard_into_slabs(w_u8, ub, layout, geom)
+    bufs = {r: DevBuf(a) for r, a in slabs.items()}
+    desc = etp.TensorDesc(units, ub, {r: (bufs[r].ptr, geom[r][1], geom[r][0]) for r in bufs}, len(widths), 0)
+    lin = etp.PreparedLinear(etp.ROW_PARALLEL if transposed else etp.COL_PARALLEL, dtype, K, N, desc, layout, fpu)
+    return lin, w_u8, bufs
+
+
+GROUP = [   # a layer in miniature: q | k | v share the attention class layout, o_t is row-parallel over it, gate | up | down_t over the FFN class
+    ("col", 520, 1280, 160, (3, 3, 2)), ("col", 520, 256, 32, (3, 3, 2)), ("col", 520, 256, 32, (3, 3, 2)),
+    ("row", 1280, 520, 160, (3, 3, 2)), ("col", 520, 1403, 1, (468, 468, 467)), ("col", 520, 1403, 1, (468, 468, 467)),
+    ("row", 1403 + 5, 520, 1, (470, 469, 469)),
+]
+
+
+@pytest.mark.parametrize("T", [1, 4, 16, 17, 64, 100])
+@pytest.mark.parametrize("pdl", [1, 0])
+def test_linear_group_mixed_modes_one_launch(ctx, T, pdl):
+    """etp_linear_prepare / etp_linear_run: seven independent linears of both modes, every one with its OWN x and y, in one
+    persistent launch (<= 64 tokens; one launch per linear at 100): each output against the unsharded fp64 reference at one
+    16-bit rounding, the load-balanced item table sane, slack slots (NaN) never read, guard bands intact."""
+    lins, ws, keep, xs, ys, refs = [], [], [], [], [], []
+    dt = torch_dtype("bf16")
+    for i, (mode, K, N, fpu, widths) in enumerate(GROUP):
+        lin, w_u8, bufs = _make_linear(mode, K, N, fpu, widths, i)
+        x_u8 = as_u8(fill_normal16(SEED, 950 + 10 * i + T, 0, T * K, 1.0, dt)).copy()
+        lins.append(lin), ws.append(w_u8), keep.append(bufs)
+        xs.append(DevBuf(x_u8))
+        ys.append(DevBuf(np.full(T * N * 2, 0xEE, dtype=np.uint8)))
+        refs.append(reference("bf16", x_u8, w_u8, T, K, N, mode == "row"))
+    ctx.set_option(etp.OPT_LINEAR_PDL, pdl)
+    try:
+        plan = etp.LinearPlan(ctx, lins)
+        info = plan.info()
+        assert info["n_linears"] == 7 and 1 <= info["n_ctas"] <= 148 and info["n_items"] >= 7
+        assert info["max_cta_chunks"] * info["n_ctas"] >= info["total_chunks"] > 0
+        st = torch.cuda.Stream()
+        for _ in range(3):                       # back to back on one stream: launch i+1 overlaps the tail of launch i
+            plan.run([x.ptr for x in xs], T, [y.ptr for y in ys], st.cuda_stream)
+        st.synchronize()
+    finally:
+        ctx.set_option(etp.OPT_LINEAR_PDL, 1)
+    for (mode, K, N, fpu, widths), x, y, ref in zip(GROUP, xs, ys, refs):
+        assert x.guards_intact() and y.guards_intact()
+        check(y.payload(), ref, "bf16", T, N)
+    plan.close()
+
+
+def test_linear_chain_under_programmatic_dependent_launch(ctx):
+    """What griddepcontrol.wait is for: linear B reads the OUTPUT of linear A, both launched back to back on one stream with the
+    programmatic-serialization attribute (B's prologue and weight ring start while A is still running).  B's result must be
+    bitwise what it is when A is synchronised first - 30 chains in a row, every intermediate overwritten each time."""
+    T, K, Nmid = 8, 2048, 4096
+    dt = torch_dtype("bf16")
+    a, wa, ka = _make_linear("col", K, Nmid, 1, (1366, 1365, 1365), 40, "tight")
+    b, wb, kb = _make_linear("row", Nmid, K, 1, (1366, 1365, 1365), 41, "tight")
+    pa, pb = etp.LinearPlan(ctx, [a]), etp.LinearPlan(ctx, [b])
+    st = torch.cuda.Stream()
+    xs = [torch.from_numpy(as_u8(fill_normal16(SEED, 990 + i, 0, T * K, 1.0, dt)).copy()).cuda() for i in range(30)]
+    mid = torch.zeros(T * Nmid * 2, dtype=torch.uint8, device="cuda")
+    outs = [torch.zeros(T * K * 2, dtype=torch.uint8, device="cuda") for _ in range(30)]
+    torch.cuda.synchronize()
+    for x, o in zip(xs, outs):                   # chained, no synchronisation anywhere
+        pa.run(x.data_ptr(), T, [mid.data_ptr()], st.cuda_stream)
+        pb.run(mid.data_ptr(), T, [o.data_ptr()], st.cuda_stream)
+    st.synchronize()
+    chained = [o.cpu().numpy().copy() for o in outs]
+    for i, x in enumerate(xs):                   # the same with a synchronisation after every launch
+        pa.run(x.data_ptr(), T, [mid.data_ptr()], st.cuda_stream)
+        st.synchronize()
+        m_u8 = mid.cpu().numpy().copy()
+        pb.run(mid.data_ptr(), T, [outs[i].data_ptr()], st.cuda_stream)
+        st.synchronize()
+        assert np.array_equal(outs[i].cpu().numpy(), chained[i]), f"chain {i}: B ran ahead of A's output"
+        if i == 0:
+            check(m_u8, reference("bf16", xs[0].cpu().numpy(), wa, T, K, Nmid, False), "bf16", T, Nmid)
+            check(chained[0], reference("bf16", m_u8, wb, T, Nmid, K, True), "bf16", T, K)
+    pa.close(), pb.close()
+
+
+def test_linear_plans_on_two_streams_do_not_share_a_workspace(ctx):
+    """One ctx, two streams, the same split-K plan in flight on both (per-stream partial tiles and tickets): both results are
+    bitwise those of the serial runs."""
+    T, K, N = 4, 8192, 1024
+    dt = torch_dtype("bf16")
+    lin, w_u8, keep = _make_linear("col", K, N, 1, (342, 341, 341), 60, "tight")
+    plan = etp.LinearPlan(ctx, [lin])
+    assert plan.info()["n_splits"][0] > 1
+    xs = [torch.from_numpy(as_u8(fill_normal16(SEED, 1100 + i, 0, T * K, 1.0, dt)).copy()).cuda() for i in range(2)]
+    serial = []
+    for x in xs:
+        y = torch.zeros(T * N * 2, dtype=torch.uint8, device="cuda")
+        plan.run(x.data_ptr(), T, [y.data_ptr()], 0)
+        torch.cuda.synchronize()
+        serial.append(y.cpu().numpy().copy())
+    check(serial[0], reference("bf16", xs[0].cpu().numpy(), w_u8, T, K, N, False), "bf16", T, N)
+    s = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ys = [[torch.zeros(T * N * 2, dtype=torch.uint8, device="cuda") for _ in range(20)] for _ in range(2)]
+    torch.cuda.synchronize()
+    for k in range(20):
+        for i in range(2):
+            plan.run(xs[i].data_ptr(), T, [ys[i][k].data_ptr()], s[i].cuda_stream)
+    torch.cuda.synchronize()
+    for i in range(2):
+        for k in range(20):
+            assert np.array_equal(ys[i][k].cpu().numpy(), serial[i]), f"stream {i}, run {k}"
+    plan.close()
+
+
+def test_linear_prepare_errors(ctx):
+    lin, _, keep = _make_linear("col", 256, 512, 1, (171, 171, 170), 70, "tight")
+    with pytest.raises(etp.EtpError) as e:
+        etp.LinearPlan(ctx, [lin] * 9)
+    assert e.value.status == 1
+    bad = etp.PreparedLinear(etp.COL_PARALLEL, "bf16", 256, 512, etp.TensorDesc(512, 512, {r: (b.ptr, 171, 0) for r, b in keep.items()}, 3, 0),
+                             [(0, 0, 100, 1), (1, 150, 512, 1)], 1)
+    with pytest.raises(etp.EtpError) as e:
+        etp.LinearPlan(ctx, [bad])
+    assert e.value.status == 1                  # the layout does not tile the units
+    plan = etp.LinearPlan(ctx, [lin])
+    y = DevBuf(np.zeros(4 * 512 * 2, np.uint8))
+    x = DevBuf(np.zeros(4 * 256 * 2, np.uint8))
+    with pytest.raises(etp.EtpError) as e:
+        plan.run([x.ptr + 2], 4, [y.ptr])
+    assert e.value.status == 2
+    plan.run([x.ptr], 0, [y.ptr])               # zero tokens: nothing to do
+    plan.close()

@@ -541,7 +541,7 @@ def test_back_to_back_calls_without_a_sync(ctx):
                                host_backup=img.data_ptr(), host_heads=kvw.host_heads, host_head0=kvw.host_head0,
                                copy_stream=s.copy.cuda_stream, reload_stream=s.reload.cuda_stream)
     rep = etp.etp_reshard_params(ctx, descs, [plans[k] for k in klasses], s.copy.cuda_stream, s.reload.cuda_stream)
-    assert rep["n_phases"] >= 2 and rep["n_kernel_launches"] >= 2
+    assert rep["n_phases"] >= 2 and rep["n_kernel_launches"] >= 1
     s.sync()
     assert ev == evicted and np.array_equal(table, new_table)
     for r, b in kbufs.items():
