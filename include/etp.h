@@ -81,6 +81,9 @@ typedef enum {
                                     serialization attribute: their prologue and first ring of weight tiles overlap the tail of the
                                     previous kernel of the stream (griddepcontrol; X, Y and the workspace are only touched after
                                     griddepcontrol.wait); 0: plain stream order                                           */
+    ETP_OPT_LINEAR_RING = 12,    /* read by etp_linear_prepare: 0 = one CTA per SM with the full shared-memory ring; 1 = two CTAs per SM
+                                    with half the ring each (one keeps streaming while the other is in its prologue or tail);
+                                    2 (default) = two per SM unless the group streams >= 200 weight chunks (3.2 MiB) per SM      */
     ETP_OPT__COUNT
 } etp_option;
 etp_status etp_ctx_set_option(etp_ctx* ctx, etp_option key, int64_t value);

@@ -58,6 +58,7 @@ extern "C" etp_status etp_ctx_create(int device, int64_t staging_bytes, etp_ctx*
     c->opts[ETP_OPT_LINEAR_CTA_PAIR] = 1;
     c->opts[ETP_OPT_VALIDATE_INTERVALS] = 1;
     c->opts[ETP_OPT_LINEAR_PDL] = 1;
+    c->opts[ETP_OPT_LINEAR_RING] = 2;
     CtxExtra* x = new (std::nothrow) CtxExtra();
     if (!x) { delete c; ETP_FAIL(ETP_ERR_NOMEM, "etp_ctx_create: out of memory"); }
     c->impl = x;

@@ -47,10 +47,12 @@ struct GroupLin {
     void* y;                                  // row-parallel output (column-parallel: per run)
 };
 
+constexpr int kMaxGroupRuns = 64;   // contiguous slot runs of a whole group (8 KiB of tensor maps in the kernel parameters)
+
 struct alignas(64) GroupParams {
     CUtensorMap map_x[kMaxGroupLins];
-    CUtensorMap map_w[kMaxLinRuns];
-    Run runs[kMaxLinRuns];
+    CUtensorMap map_w[kMaxGroupRuns];
+    Run runs[kMaxGroupRuns];
     GroupLin lin[kMaxGroupLins];
     const GroupItem* items;     // CTA-major item lists
     const int32_t* cta_first;   // [grid + 1]
@@ -61,11 +63,15 @@ struct alignas(64) GroupParams {
 
 constexpr int kMaxCtaItems = 96;   // items of one CTA staged in shared memory
 
-template <int BN>
+// HALF = false: one CTA per SM with a deep ring (10 / 8 stages of 18 / 24 KiB).  HALF = true: half the ring (5 / 4 stages,
+// < 100 KiB) and TWO CTAs per SM (grid = 2 x SMs), see etp_linear_prepare.
+template <int BN, bool HALF>
 struct GCfg {
     static constexpr int kBBytes = BN * kBK * 2;
     static constexpr int kStageBytes = kABytes + kBBytes;
-    static constexpr int kStages = (kSmemBudget / kStageBytes) > 10 ? 10 : (kSmemBudget / kStageBytes);
+    static constexpr int kFull = (kSmemBudget / kStageBytes) > 10 ? 10 : (kSmemBudget / kStageBytes);
+    static constexpr int kStages = HALF ? kFull / 2 : kFull;
+    static constexpr int kMinCtas = HALF ? 2 : 1;
     static constexpr int kTmemCols = (2 * BN) < 32 ? 32 : 2 * BN;
     static constexpr int kSmemBytes = kStages * kStageBytes + 1024 + 256 + kStageTileBytes + kMaxCtaItems * int(sizeof(GroupItem));
 };
@@ -80,9 +86,9 @@ __device__ __forceinline__ int find_run_in(const GroupParams& p, const GroupLin&
     return r;
 }
 
-template <int BN, typename OutT>
-__global__ void __launch_bounds__(kLinThreads, 1) etp_linear_group_kernel(const __grid_constant__ GroupParams p) {
-    using C = GCfg<BN>;
+template <int BN, typename OutT, bool HALF>
+__global__ void __launch_bounds__(kLinThreads, GCfg<BN, HALF>::kMinCtas) etp_linear_group_kernel(const __grid_constant__ GroupParams p) {
+    using C = GCfg<BN, HALF>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + C::kStages * C::kStageBytes);
@@ -331,13 +337,14 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_linear_group_kernel(const 
     }
 }
 
-template <int BN, typename OutT>
+template <int BN, typename OutT, bool HALF>
 etp_status launch_group_t(const GroupParams& p, int grid, cudaStream_t stream, bool pdl) {
-    using C = GCfg<BN>;
-    auto k = etp_linear_group_kernel<BN, OutT>;
+    using C = GCfg<BN, HALF>;
+    auto k = etp_linear_group_kernel<BN, OutT, HALF>;
     static bool configured = false;   // per instantiation; the attribute is a property of the function, set once per process
     if (!configured) {
         ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes));
+        if (HALF) ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         configured = true;
     }
     cudaLaunchConfig_t cfg{};
@@ -355,10 +362,14 @@ etp_status launch_group_t(const GroupParams& p, int grid, cudaStream_t stream, b
     return ETP_OK;
 }
 
-etp_status launch_group(const GroupParams& p, int bn, int grid, cudaStream_t stream, bool pdl) {
+template <bool HALF>
+etp_status launch_group_h(const GroupParams& p, int bn, int grid, cudaStream_t stream, bool pdl) {
     const bool bf = p.dtype == ETP_BF16;
-    if (bn == 16) return bf ? launch_group_t<16, __nv_bfloat16>(p, grid, stream, pdl) : launch_group_t<16, __half>(p, grid, stream, pdl);
-    return bf ? launch_group_t<64, __nv_bfloat16>(p, grid, stream, pdl) : launch_group_t<64, __half>(p, grid, stream, pdl);
+    if (bn == 16) return bf ? launch_group_t<16, __nv_bfloat16, HALF>(p, grid, stream, pdl) : launch_group_t<16, __half, HALF>(p, grid, stream, pdl);
+    return bf ? launch_group_t<64, __nv_bfloat16, HALF>(p, grid, stream, pdl) : launch_group_t<64, __half, HALF>(p, grid, stream, pdl);
+}
+etp_status launch_group(const GroupParams& p, int bn, int grid, cudaStream_t stream, bool pdl, bool half_ring) {
+    return half_ring ? launch_group_h<true>(p, bn, grid, stream, pdl) : launch_group_h<false>(p, bn, grid, stream, pdl);
 }
 
 // ------------------------------------------------------------------------------------------------ ctx-owned linear state
@@ -392,6 +403,7 @@ struct etp_linear_plan {
     GroupParams p;
     void* d_table = nullptr;                // items + cta_first
     int grid = 0;
+    bool half_ring = false;
     int64_t n_partial_tiles = 0, n_tiles = 0;
     int64_t n_items = 0, max_cta_chunks = 0, total_chunks = 0;
 };
@@ -478,7 +490,10 @@ int64_t lpt_makespan(std::vector<int64_t> costs, int n_ctas) {
     return mk;
 }
 
-constexpr int kItemOverhead = 2;   // fixed cost of an item in chunk units (accumulator hand-over, partial tile, ticket)
+// Cost of an item in QUARTER chunks (one chunk = 16 KiB of weights = 0.37 us of one SM's share of the HBM stream): its weight
+// chunks, plus - for an item of a split tile - the fp32 partial tile it writes and the last arriver reads back (2 x 8 KiB at 16
+// tokens ~ one chunk), plus a small hand-over cost (the ring keeps streaming across items; the epilogue overlaps the next MMAs).
+constexpr int64_t item_cost(int64_t chunks, int splits) { return 4 * chunks + (splits > 1 ? 4 : 1); }
 
 }  // namespace
 
@@ -520,7 +535,7 @@ extern "C" etp_status etp_linear_prepare(etp_ctx* ctx, etp_dtype dtype, const et
         ETP_TRY(check_layout(s.layout, s.n_shards, s.w->total_units, &sorted));
         RunList rl;
         ETP_TRY(append_runs(&L.w, sorted, s.features_per_unit, nullptr, s.out_features, &rl));
-        if (n_runs + rl.n > kMaxLinRuns) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_linear_prepare: more than %d contiguous runs in the group", kMaxLinRuns);
+        if (n_runs + rl.n > kMaxGroupRuns) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_linear_prepare: more than %d contiguous runs in the group", kMaxGroupRuns);
         const bool row_par = L.mode == ETP_ROW_PARALLEL;
         GroupLin& G = p.lin[l];
         G.mode = L.mode;
@@ -549,21 +564,28 @@ extern "C" etp_status etp_linear_prepare(etp_ctx* ctx, etp_dtype dtype, const et
 
     // ---- K splits: the target item size c (in chunks) that minimises the LPT makespan of the NOMINAL group plus the
     // split-K partial traffic it causes (one fp32 tile written and read back per split item, ~BN/16 chunks, spread over the CTAs)
-    const int n_ctas = ctx->n_sms;
+    // Two CTAs per SM with half the ring each (the same bytes in flight per SM): while one CTA of an SM is in its tail (last MMAs,
+    // epilogue, split-K reduction) or a CTA of the NEXT launch is in its prologue, the other keeps streaming.  Measured on the
+    // config-2 layer at 4 tokens (profiles/r2_linear.md): every single launch of a layer is faster this way (o_t 25.3 -> 19.4 us,
+    // gate|up 64.5 -> 62.4 us, the 4-launch chain 121 -> 117 us per layer); the 7-linear group launch is not (103.5 -> 108.2 us:
+    // twice as many CTAs want twice as many items, i.e. more split-K partial traffic).  ETP_OPT_LINEAR_RING: 0 / 1 force, 2 = by size.
+    int64_t nominal_chunks = 0;
+    for (int l = 0; l < n_lins; ++l) nominal_chunks += nominal[l].tiles * nominal[l].chunks;
+    const int64_t ring_opt = ctx->opts[ETP_OPT_LINEAR_RING];
+    P->half_ring = ring_opt == 1 || (ring_opt == 2 && nominal_chunks < int64_t(200) * ctx->n_sms);
+    const int n_ctas = ctx->n_sms * (P->half_ring ? 2 : 1);
     int best_c = 64;
     {
         int64_t best = INT64_MAX;
-        for (int c = 4; c <= 96; c += (c < 24 ? 2 : 4)) {
+        for (int c = 2; c <= 96; c += (c < 24 ? 1 : 4)) {
             std::vector<int64_t> costs;
-            int64_t split_items = 0;
             for (int l = 0; l < n_lins; ++l) {
                 const int S = splits_for(nominal[l], c);
                 for (int64_t t = 0; t < nominal[l].tiles; ++t)
                     for (int s = 0; s < S; ++s)
-                        costs.push_back((int64_t(s + 1) * nominal[l].chunks / S - int64_t(s) * nominal[l].chunks / S) + kItemOverhead);
-                if (S > 1) split_items += nominal[l].tiles * S;
+                        costs.push_back(item_cost(int64_t(s + 1) * nominal[l].chunks / S - int64_t(s) * nominal[l].chunks / S, S));
             }
-            const int64_t cost = lpt_makespan(std::move(costs), n_ctas) + (split_items * 2 + n_ctas - 1) / n_ctas;
+            const int64_t cost = lpt_makespan(std::move(costs), n_ctas);
             if (cost < best) { best = cost; best_c = c; }
         }
     }
@@ -591,7 +613,8 @@ extern "C" etp_status etp_linear_prepare(etp_ctx* ctx, etp_dtype dtype, const et
     P->grid = grid;
     std::vector<size_t> order(items.size());
     for (size_t i = 0; i < order.size(); ++i) order[i] = i;
-    std::stable_sort(order.begin(), order.end(), [&](size_t a, size_t b) { return items[a].c1 - items[a].c0 > items[b].c1 - items[b].c0; });
+    auto cost_of = [&](const GroupItem& it) { return item_cost(it.c1 - it.c0, p.lin[it.lin].n_splits); };
+    std::stable_sort(order.begin(), order.end(), [&](size_t a, size_t b) { return cost_of(items[a]) > cost_of(items[b]); });
     std::vector<std::vector<GroupItem>> per_cta(grid);
     using Load = std::pair<int64_t, int>;
     std::priority_queue<Load, std::vector<Load>, std::greater<Load>> load;
@@ -600,7 +623,7 @@ extern "C" etp_status etp_linear_prepare(etp_ctx* ctx, etp_dtype dtype, const et
         Load t = load.top();
         load.pop();
         per_cta[t.second].push_back(items[k]);
-        t.first += items[k].c1 - items[k].c0 + kItemOverhead;
+        t.first += cost_of(items[k]);
         load.push(t);
         P->total_chunks += items[k].c1 - items[k].c0;
     }
@@ -696,7 +719,8 @@ extern "C" etp_status etp_linear_run(etp_linear_plan* P, const void* const* x, i
         p.tickets = w.tickets;
     }
     ctx->launches = 1;
-    return launch_group(p, bn, P->grid, st, ctx->opts[ETP_OPT_LINEAR_PDL] != 0);
+    const bool pdl = ctx->opts[ETP_OPT_LINEAR_PDL] != 0;
+    return launch_group(p, bn, P->grid, st, pdl, P->half_ring);
 }
 
 // ------------------------------------------------------------------------------------------------ legacy entry points, <= 64 tokens
