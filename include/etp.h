@@ -52,6 +52,26 @@ typedef struct etp_plan etp_plan;
  * device is missing or is not compute capability 10.x. */
 etp_status etp_ctx_create(int device, int64_t staging_bytes, etp_ctx** out);
 void etp_ctx_destroy(etp_ctx* ctx);
+
+/* Multi-device (SURVEY.md 8(e), 8(f) #1; PAPER.md:64 "P2P direct access over high-speed interconnects", :162-166 execution
+ * scheduler).  A ctx over n_devices LOGICAL devices: devices[i] is the CUDA device of logical device i; several logical
+ * devices may name the same CUDA device (that is how the partitioned path is exercised on a one-GPU box).  Peer access is
+ * enabled between every pair of distinct CUDA devices (ETP_ERR_UNSUPPORTED if the hardware cannot).  etp_reshard_params and
+ * etp_reshard_kv then PARTITION THEIR WORK BY DESTINATION: logical device d runs, on its own library-owned streams, one launch
+ * of the copy kernel per hazard phase that writes only memory of the ranks mapped to d and pulls its incoming intervals
+ * through peer-mapped source pointers, plus the reloads of those ranks over its own host link; hazard phases are ordered
+ * across devices with events; the caller's copy / reload streams (streams of devices[0]) are forked from and joined back
+ * to, so "complete when both streams are synchronised" still holds.  No collective is involved.
+ *
+ * etp_ctx_set_rank_devices: device_of_rank[r] = the logical device whose memory holds rank r's slabs and KV pool, or -1 for
+ * a rank that ANOTHER PROCESS writes (one process per GPU: its slabs are still valid SOURCES here if the caller passes
+ * pointers this process can read, e.g. CUDA-IPC mappings, but no byte of it is written by this ctx; those bytes are counted
+ * in etp_reshard_report.remote_bytes).  Every process lowers the same plan and therefore sees the same hazard phases; with
+ * more than one phase in a multi-process job the caller runs the phases one by one (ETP_OPT_ONLY_PHASE) with a barrier of
+ * its own in between.  Default (never called, or n_ranks = 0): every rank on logical device 0.
+ * etp_ctx_device_report: what the last call enqueued on one logical device (bytes by destination, launches, memcpys). */
+etp_status etp_ctx_create_multi(const int32_t* devices, int32_t n_devices, etp_ctx** out);
+etp_status etp_ctx_set_rank_devices(etp_ctx* ctx, const int32_t* device_of_rank, int32_t n_ranks);
 const char* etp_last_error(void);
 /* library version string, e.g. "etp 0.1 sm_100a" (static storage) */
 const char* etp_version(void);
@@ -84,6 +104,8 @@ typedef enum {
     ETP_OPT_LINEAR_RING = 12,    /* read by etp_linear_prepare: 0 = one CTA per SM with the full shared-memory ring; 1 = two CTAs per SM
                                     with half the ring each (one keeps streaming while the other is in its prologue or tail);
                                     2 (default) = two per SM unless the group streams >= 200 weight chunks (3.2 MiB) per SM      */
+    ETP_OPT_ONLY_PHASE = 13,     /* 0 (default): a call runs every hazard phase, ordered by events; k > 0: only phase k - 1 is
+                                    enqueued (multi-process jobs: the caller puts its own barrier between the phases)         */
     ETP_OPT__COUNT
 } etp_option;
 etp_status etp_ctx_set_option(etp_ctx* ctx, etp_option key, int64_t value);
@@ -176,7 +198,9 @@ typedef struct {
     int32_t n_phases;           /* hazard phases (1 = hazard-free)                                                 */
     int32_t n_kernel_launches;  /* launches of this library's kernels                                              */
     double lower_ms;            /* host time spent lowering + enqueueing                                           */
+    int64_t remote_bytes;       /* TRANSFER + RELOAD bytes whose destination rank another process writes (rank map -1) */
 } etp_reshard_report;
+etp_status etp_ctx_device_report(etp_ctx* ctx, int32_t logical_device, etp_reshard_report* out);
 
 /* tensors: host array.  plans: host array of n_plans plan handles.  copy_stream / reload_stream: cudaStream_t of the
  * ctx device (may be the same stream; NULL = legacy default stream).  report: host, may be NULL. */

@@ -21,7 +21,7 @@ COL_PARALLEL, ROW_PARALLEL = 0, 1
 DTYPE = {"bf16": 0, "fp16": 1}
 KV_TOKEN_MAJOR, KV_HEAD_MAJOR = 0, 1
 (OPT_SKIP_D2D, OPT_SKIP_RELOAD, OPT_TMA_MIN_BYTES, OPT_LDG_STEALS_BULK, OPT_RELOAD_CHUNK_BYTES, OPT_RESERVED_5,
- OPT_GRID_CTAS, OPT_GATHER_CTAS, OPT_TIME_KERNELS, OPT_LINEAR_CTA_PAIR, OPT_VALIDATE_INTERVALS, OPT_LINEAR_PDL, OPT_LINEAR_RING) = range(13)
+ OPT_GRID_CTAS, OPT_GATHER_CTAS, OPT_TIME_KERNELS, OPT_LINEAR_CTA_PAIR, OPT_VALIDATE_INTERVALS, OPT_LINEAR_PDL, OPT_LINEAR_RING, OPT_ONLY_PHASE) = range(14)
 
 
 class EtpError(RuntimeError):
@@ -53,7 +53,7 @@ class etp_tensor(C.Structure):
 
 class etp_reshard_report(C.Structure):
     _fields_ = [("d2d_bytes", i64), ("h2d_bytes", i64), ("reload_dev_bytes", i64), ("kept_bytes", i64), ("n_jobs", i64), ("n_units", i64),
-                ("n_memcpys", i64), ("n_phases", i32), ("n_kernel_launches", i32), ("lower_ms", C.c_double)]
+                ("n_memcpys", i64), ("n_phases", i32), ("n_kernel_launches", i32), ("lower_ms", C.c_double), ("remote_bytes", i64)]
 
     def as_dict(self) -> Dict[str, float]:
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -88,7 +88,7 @@ class etp_interval(C.Structure):
     _fields_ = [("src", vp), ("dst", vp), ("bytes", i64)]
 
 
-EXPORTS = ["etp_ctx_create", "etp_ctx_destroy", "etp_last_error", "etp_version", "etp_ctx_set_option", "etp_ctx_get_option",
+EXPORTS = ["etp_ctx_create", "etp_ctx_create_multi", "etp_ctx_set_rank_devices", "etp_ctx_device_report", "etp_ctx_destroy", "etp_last_error", "etp_version", "etp_ctx_set_option", "etp_ctx_get_option",
            "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_tasks", "etp_plan_new_layout",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
            "etp_shard_linear_multi", "etp_linear_prepare", "etp_linear_run", "etp_linear_plan_info", "etp_linear_free",
@@ -106,6 +106,9 @@ def lib() -> C.CDLL:
         L.etp_last_error.restype = C.c_char_p
         L.etp_version.restype = C.c_char_p
         L.etp_ctx_create.argtypes = [C.c_int, i64, C.POINTER(vp)]
+        L.etp_ctx_create_multi.argtypes = [C.POINTER(i32), i32, C.POINTER(vp)]
+        L.etp_ctx_set_rank_devices.argtypes = [vp, C.POINTER(i32), i32]
+        L.etp_ctx_device_report.argtypes = [vp, i32, C.POINTER(etp_reshard_report)]
         L.etp_ctx_destroy.argtypes = [vp]
         L.etp_ctx_destroy.restype = None
         L.etp_ctx_set_option.argtypes = [vp, C.c_int, i64]
@@ -243,10 +246,27 @@ def etp_page_table_rewrite(table, seq_lens, last_use, block_size: int, budget: i
 class Context:
     """Owns an etp_ctx (descriptor arenas, events) on one CUDA device."""
 
-    def __init__(self, device: int = 0, staging_bytes: int = 0):
+    def __init__(self, device: int = 0, staging_bytes: int = 0, devices: Optional[Sequence[int]] = None):
+        """``devices``: CUDA device of every LOGICAL device (etp_ctx_create_multi; entries may repeat); default one device."""
         h = vp()
-        _check(lib().etp_ctx_create(device, staging_bytes, C.byref(h)))
+        if devices is None:
+            _check(lib().etp_ctx_create(device, staging_bytes, C.byref(h)))
+            self.n_devices = 1
+        else:
+            arr = (i32 * len(devices))(*[int(d) for d in devices])
+            _check(lib().etp_ctx_create_multi(arr, len(devices), C.byref(h)))
+            self.n_devices = len(devices)
         self.handle = h
+
+    def set_rank_devices(self, device_of_rank: Sequence[int]) -> None:
+        """rank -> logical device that holds (and writes) its memory; -1 = a rank another process writes."""
+        arr = (i32 * max(len(device_of_rank), 1))(*[int(d) for d in device_of_rank])
+        _check(lib().etp_ctx_set_rank_devices(self.handle, arr, len(device_of_rank)))
+
+    def device_report(self, logical_device: int) -> Dict[str, float]:
+        rep = etp_reshard_report()
+        _check(lib().etp_ctx_device_report(self.handle, logical_device, C.byref(rep)))
+        return rep.as_dict()
 
     def close(self):
         if getattr(self, "handle", None):

@@ -116,14 +116,11 @@ struct etp_plan {
 };
 
 struct etp_ctx {
-    int device = 0;
+    int device = 0;                     // physical CUDA device of logical device 0 (the caller's streams live there)
     int n_sms = 0;
     int64_t opts[ETP_OPT__COUNT];
-    void* impl = nullptr;               // executor state (descriptor arenas, events), etp_exec.cu
-    std::vector<cudaEvent_t> events;    // hazard-phase events
+    void* impl = nullptr;               // executor state (per logical device: streams, descriptor arenas, events), etp_exec.cu
     int32_t launches = 0;               // kernels launched by the last call
-    std::vector<cudaEvent_t> tev;       // timing events (pairs) around copy-stream launches, ETP_OPT_TIME_KERNELS
-    int32_t n_timed = 0;                // pairs recorded by the last call
     void* lin_state = nullptr;          // kernel (c): per-stream split-K workspaces + the cache of prepared groups (etp_linear_group.cu)
     void* moe_items = nullptr;          // work-item table of etp_moe_linear (device), grown on demand
     int64_t moe_items_bytes = 0;
@@ -131,13 +128,20 @@ struct etp_ctx {
 
 namespace etp {
 // lowering (host): etp_lower.cpp
-struct LoweredWork {
+// The work of one call, partitioned by DESTINATION device ("each GPU pulls its own incoming intervals").
+struct DeviceWork {
     std::vector<JobList> phases;       // device-copy segments per hazard phase (copy stream)
     std::vector<JobList> host_gather;  // segments whose source is pinned host memory (zero-copy gather, reload stream), per phase
     std::vector<DmaCopy> dma;          // pinned host -> device DMAs (reload stream)
-    std::vector<int32_t> pairs;        // {old block id, new block id} lists referenced by VEC_PAGED segments
-    etp_reshard_report rep{};
+    etp_reshard_report rep{};          // bytes this device writes
 };
+struct LoweredWork {
+    std::vector<DeviceWork> dev;       // indexed by logical device of the ctx
+    std::vector<int32_t> pairs;        // {old block id, new block id} lists referenced by VEC_PAGED segments (uploaded to every device)
+    etp_reshard_report rep{};          // totals
+};
+int n_logical_devices(const etp_ctx* ctx);
+int device_of_rank(const etp_ctx* ctx, int32_t rank);   // logical device that WRITES the rank's memory; -1 = another process does
 etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n_tensors, const etp_plan* const* plans,
                         int32_t n_plans, LoweredWork* out);
 etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* g, const etp_plan* head_plan, const int32_t* pairs,

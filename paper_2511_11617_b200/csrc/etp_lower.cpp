@@ -158,6 +158,7 @@ etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n
     std::vector<SlotRun> runs;
     std::map<std::vector<int64_t>, std::vector<int32_t>> phase_cache;
     int32_t max_phase = 0;
+    out->dev.resize((size_t)n_logical_devices(ctx));
     for (int32_t t = 0; t < n_tensors; ++t) {
         const etp_tensor& T = tensors[t];
         if (T.plan_index < 0 || T.plan_index >= n_plans || !plans[T.plan_index])
@@ -230,16 +231,23 @@ etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n
                 continue;
             }
             if (K.begin >= K.end) continue;
-            max_phase = std::max(max_phase, phase[k]);
+            max_phase = std::max(max_phase, phase[k]);   // the phase structure is global: every process agrees on it
             const etp_slab* D = slab_of(K.dst_rank);
+            const int dv = device_of_rank(ctx, K.dst_rank);
+            if (dv < 0) {   // a rank whose memory another process writes (its own executor pulls these bytes)
+                out->rep.remote_bytes += bytes;
+                continue;
+            }
+            DeviceWork& W = out->dev[(size_t)dv];
             if (K.kind == ETP_TRANSFER) {
                 const etp_slab* S = slab_of(K.src_rank);
                 slot_runs(K.begin, K.end, S->anchor_unit, S->cap_units, D->anchor_unit, D->cap_units, &runs);
                 for (const SlotRun& r : runs) {
-                    push_contiguous(ctx, &phase_list(out->phases, phase[k]), (const char*)S->base + r.src_slot * T.unit_bytes,
+                    push_contiguous(ctx, &phase_list(W.phases, phase[k]), (const char*)S->base + r.src_slot * T.unit_bytes,
                                     (char*)D->base + r.dst_slot * T.unit_bytes, r.count * T.unit_bytes);
                 }
                 out->rep.d2d_bytes += bytes;
+                W.rep.d2d_bytes += bytes;
             } else {  // RELOAD
                 if (!T.host_image || K.begin < T.host_unit0 || K.end > T.host_unit0 + T.host_units)
                     ETP_FAIL(ETP_ERR_NO_SOURCE, "tensor %d: RELOAD [%lld,%lld) not covered by the host image", t,
@@ -254,13 +262,13 @@ etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n
                     const char* src = (const char*)T.host_image + (r.first_unit - T.host_unit0) * T.unit_bytes;
                     char* dst = (char*)D->base + r.dst_slot * T.unit_bytes;
                     if (image_kind == MEM_DEVICE) {
-                        push_contiguous(ctx, &phase_list(out->phases, phase[k]), src, dst, r.count * T.unit_bytes);
+                        push_contiguous(ctx, &phase_list(W.phases, phase[k]), src, dst, r.count * T.unit_bytes);
                     } else {
-                        out->dma.push_back({src, dst, r.count * T.unit_bytes, phase[k]});
+                        W.dma.push_back({src, dst, r.count * T.unit_bytes, phase[k]});
                     }
                 }
-                if (image_kind == MEM_DEVICE) out->rep.reload_dev_bytes += bytes;
-                else out->rep.h2d_bytes += bytes;
+                if (image_kind == MEM_DEVICE) { out->rep.reload_dev_bytes += bytes; W.rep.reload_dev_bytes += bytes; }
+                else { out->rep.h2d_bytes += bytes; W.rep.h2d_bytes += bytes; }
             }
         }
     }
@@ -332,6 +340,7 @@ etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* gp, const etp_pla
     std::vector<int32_t> phase;
     ETP_TRY(assign_phases(reads, writes, &phase));
     int32_t max_phase = 0;
+    out->dev.resize((size_t)n_logical_devices(ctx));
 
     // pair lists on the device: [0, n_pairs) every surviving live block, [n_pairs, n_pairs + n_reloc) the relocated ones
     out->pairs.assign(pairs, pairs + 2 * n_pairs);
@@ -349,18 +358,26 @@ etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* gp, const etp_pla
         const int64_t live_bytes = (K.end - K.begin) * frag * g.block_size * n_planes * n_pairs;
         const char* src_base;
         const PoolShape* ss;
-        std::vector<JobList>* dest = &out->phases;
-        int64_t* counter;
+        const int dv = device_of_rank(ctx, K.dst_rank);   // KV heads are written by the device that holds the destination pool
+        if (dv < 0) {
+            if (K.kind != ETP_KEEP) out->rep.remote_bytes += live_bytes;
+            continue;
+        }
+        DeviceWork& W = out->dev[(size_t)dv];
+        std::vector<JobList>* dest = &W.phases;
+        int64_t *counter, *dev_counter;
         if (K.kind == ETP_KEEP) {
             src_base = (const char*)g.pools[K.dst_rank];
             ss = &dev;
             slot_runs(K.begin, K.end, g.head_anchor[K.dst_rank], g.head_cap, g.head_anchor[K.dst_rank], g.head_cap, &runs);
             counter = &out->rep.d2d_bytes;
+            dev_counter = &W.rep.d2d_bytes;
         } else if (K.kind == ETP_TRANSFER) {
             src_base = (const char*)g.pools[K.src_rank];
             ss = &dev;
             slot_runs(K.begin, K.end, g.head_anchor[K.src_rank], g.head_cap, g.head_anchor[K.dst_rank], g.head_cap, &runs);
             counter = &out->rep.d2d_bytes;
+            dev_counter = &W.rep.d2d_bytes;
         } else {
             if (!g.host_backup) continue;  // reading K4: fragments left untouched; the caller reports the sequences
             if (K.begin < g.host_head0 || K.end > g.host_head0 + g.host_heads)
@@ -372,9 +389,11 @@ etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* gp, const etp_pla
             for (SlotRun& r : runs) r.src_slot = r.first_unit - g.host_head0;
             if (backup_kind == MEM_DEVICE) {
                 counter = &out->rep.reload_dev_bytes;
+                dev_counter = &W.rep.reload_dev_bytes;
             } else {
                 counter = &out->rep.h2d_bytes;
-                dest = &out->host_gather;
+                dev_counter = &W.rep.h2d_bytes;
+                dest = &W.host_gather;
             }
         }
         const int32_t ph = K.kind == ETP_KEEP ? 0 : phase[k];
@@ -420,11 +439,11 @@ etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* gp, const etp_pla
             moved += np_task * n_planes * plane_bytes;
         }
         *counter += moved;
+        *dev_counter += moved;
         if (K.kind == ETP_KEEP) out->rep.kept_bytes += live_bytes - moved;
         if (moved) max_phase = std::max(max_phase, ph);
     }
     out->rep.n_phases = std::max<int32_t>(out->rep.n_phases, max_phase + 1);
-    (void)ctx;
     return ETP_OK;
 }
 
