@@ -12,7 +12,8 @@ Metric (BASELINE.json): moved-bytes GB/s of the reshard (+ full-state reshard ms
   roofline   interval-copy kernel: 2 * bytes it moved / its device time (CUDA events recorded by the library on the
              launching stream), against MEASURED_PEAKS.json hbm_gbs.
   cpu_baseline / --impl reference: the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
-Multi-GPU: "replicas only" — every rank reshards its own replica, no collective on the data path.
+Multi-GPU: `--gpus N` = N independent replicas (north_star: "replicas only"); `--gpus N --sharded` = ONE reshard
+partitioned by destination rank over N processes / GPUs (peers through CUDA IPC, no collective) - the real multi-GPU form.
 """
 from __future__ import annotations
 
@@ -49,6 +50,9 @@ def parse_args():
     ap.add_argument("--moe", action="store_true", help="config 4: grouped MoE shard linear (etp_moe_linear) on the resharded experts")
     ap.add_argument("--no-linear", action="store_true", help="skip the S7 (shard linear) leg")
     ap.add_argument("--linear-only", action="store_true", help="only the S7 leg, on parameters alone (for ncu captures of kernel (c))")
+    ap.add_argument("--sharded", action="store_true",
+                    help="--gpus N > 1: ONE reshard sharded by destination rank over N processes / GPUs (simulated rank r on GPU r mod N, "
+                         "peers' memory through CUDA IPC, no collective) instead of N independent replicas")
     ap.add_argument("--lin-pdl", type=int, default=-1, help="A/B: ETP_OPT_LINEAR_PDL for the S7 leg (default: the library's)")
     ap.add_argument("--lin-ring", type=int, default=-1, help="A/B: ETP_OPT_LINEAR_RING for the S7 leg (default: the library's)")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0, help="CPU seconds of oracle work in the cpu_baseline leg")
@@ -694,6 +698,125 @@ def whole_job_gbps(bytes_per_rank: float, world: int, ms: float) -> float:
     return bytes_per_rank * world / (ms * 1e-3) / 1e9
 
 
+# ================================================================================================ sharded multi-GPU reshard
+def split_ranks(n_ranks: int, world: int):
+    """Simulated TP rank r lives on process / GPU r mod world (partition by destination rank)."""
+    return [[r for r in range(n_ranks) if r % world == p] for p in range(world)]
+
+
+def run_sharded(args):
+    """`--gpus N --sharded` under torchrun: the real multi-GPU form of the path.  Every process owns one
+    GPU and the slabs + KV pools of the simulated ranks r with r mod N == its rank, maps its peers' memory through CUDA IPC,
+    lowers the SAME plan and executes only the tasks whose DESTINATION it owns - each GPU pulls its incoming intervals over
+    NVLink and reloads over its own host link.  No data-path collective; barriers and the max-over-ranks of the timing only.
+    value = bytes moved by all processes / the slowest process' time (strong scaling: the state is fixed, N splits it).
+    ETP_BENCH_ALIAS_GPU0=1 puts every process on cuda:0 (gloo plumbing) - how the path is exercised on a one-GPU box."""
+    import torch
+    import torch.distributed as dist
+    rank, local_rank, world = (int(os.environ.get(k, d)) for k, d in (("RANK", "0"), ("LOCAL_RANK", "0"), ("WORLD_SIZE", "1")))
+    alias = os.environ.get("ETP_BENCH_ALIAS_GPU0") == "1"
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dev_index = 0 if alias else local_rank
+    torch.cuda.set_device(dev_index)
+    dev = torch.device("cuda", dev_index)
+    if world > 1:
+        dist.init_process_group("gloo" if alias else "nccl", **({} if alias else {"device_id": dev}))
+    import paper_2511_11617_b200 as etp
+    from paper_2511_11617_b200.state import ModelState
+    from workloads import get_config
+    from workloads.configs import scaled
+    cfg = get_config(args.config)
+    reduced = bool(args.layers or args.seqs)
+    if reduced:
+        cfg = scaled(cfg, n_layers=args.layers or None, n_seqs=args.seqs or None)
+    hbm_peak, peak_src = load_peaks()
+
+    def exchange(mine):
+        if world == 1:
+            return [mine]
+        out = [None] * world
+        dist.all_gather_object(out, mine)      # picklable IPC handles: plumbing, not the data path
+        return out
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def reduce(v, op):
+        if world == 1:
+            return v
+        t = torch.tensor([float(v)], dtype=torch.float64, device=("cpu" if alias else dev))
+        dist.all_reduce(t, op=op)
+        return float(t.item())
+
+    state = ModelState(cfg, device=dev, image="both", shard=(rank, world), exchange=exchange)
+    barrier()                                   # every owner has filled its slabs before anybody reads them
+    ctx = etp.Context(dev_index)
+    ctx.set_rank_devices(state.rank_devices())
+    cs, rs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+
+    def one_step(image):
+        e0, e1, er = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event()
+        e0.record(cs)
+        rep = state.reshard(ctx, 0, image, cs.cuda_stream, rs.cuda_stream, replan=True)
+        er.record(rs)
+        cs.wait_event(er)
+        e1.record(cs)
+        e1.synchronize()
+        return e0.elapsed_time(e1), rep
+
+    def timed(image):
+        for _ in range(max(args.warmup, 0)):
+            one_step(image)
+            barrier()
+        barrier()
+        tot, moved, h2d, launches = 0.0, 0, 0, 0
+        for _ in range(args.steps):
+            ms, rep = one_step(image)
+            barrier()                           # a step of the JOB ends when its slowest process has finished
+            tot += reduce(ms, dist.ReduceOp.MAX) if world > 1 else ms
+            for r in (rep["params"], rep["kv"]):
+                if r:
+                    assert r["n_phases"] == 1, "the sharded bench runs hazard-free plans (span slabs)"
+                    moved += r["d2d_bytes"] + r["h2d_bytes"] + r["reload_dev_bytes"]
+                    h2d += r["h2d_bytes"]
+                    launches += r["n_kernel_launches"]
+        return tot, reduce(moved, dist.ReduceOp.SUM) if world > 1 else moved, reduce(h2d, dist.ReduceOp.SUM) if world > 1 else h2d, launches
+
+    sampler = ClockSampler(dev_index)
+    if rank == 0:
+        sampler.start()
+    tot_ms, moved, _, launches = timed("device")
+    e_ms, e_moved, e_h2d, e_launches = timed("pinned")
+    clocks = sampler.stop() if rank == 0 else None
+    owners = split_ranks(state.n_ranks, world)
+    if rank == 0:
+        K = args.steps
+        sb = state.state_bytes()
+        print(json.dumps({
+            "metric": METRIC, "value": moved / (tot_ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": tot_ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+            "config": {"workload": f"config {cfg.key}: {cfg.note}" + (" [REDUCED: debug run, not a bench value]" if reduced else ""),
+                       "parallelism": f"sharded by destination rank over {world} processes: simulated ranks {owners}; peers through CUDA IPC; no collective",
+                       "reload_source": "device-resident image (synthetic; every reload byte goes through kernel (a))",
+                       "state_GB": round((sb["param_bytes"] + sb["kv_live_bytes"]) / 1e9, 2), "moved_GB_per_step": round(moved / K / 1e9, 3),
+                       "aliased_to_gpu0": alias, "l2": "inputs larger than L2", "unmeasured_on_multi_gpu_hardware": True},
+            "e2e": {"value": e_moved / (e_ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(e_h2d // K), "d2h_bytes_per_step": 0,
+                    "ms_per_step": e_ms / K, "h2d_GBps": e_h2d / (e_ms * 1e-3) / 1e9},
+            "gpu_launches": launches + e_launches, "clocks": clocks,
+            "roofline": {"bound": "hbm", "achieved": 2.0 * moved / (tot_ms * 1e-3) / 1e9, "peak": hbm_peak * world, "unit": "GB/s",
+                         "frac": 2.0 * moved / (tot_ms * 1e-3) / 1e9 / (hbm_peak * world), "traffic": None, "peak_source": peak_src,
+                         "note": "whole step (host lowering included), all GPUs; local pulls are HBM-bound, peer pulls NVLink-bound"}}))
+    ctx.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
 # ================================================================================================ the CUDA path
 def run_ours(args):
     import torch
@@ -924,4 +1047,6 @@ if __name__ == "__main__":
         sys.exit(run_planners(a))
     if a.sweep:
         sys.exit(run_sweep(a))
-    sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))
+    if a.impl == "reference":
+        sys.exit(run_reference(a))
+    sys.exit(run_sharded(a) if a.sharded else run_ours(a))

@@ -43,6 +43,13 @@ class Arena:
         assert self.t.data_ptr() % ALIGN == 0
         self.off = 0
 
+    @classmethod
+    def wrap(cls, t: torch.Tensor) -> "Arena":
+        """An arena over memory somebody else allocated (a CUDA-IPC mapping of a peer process' arena)."""
+        a = cls.__new__(cls)
+        a.t, a.off = t, 0
+        return a
+
     def take(self, n_bytes: int) -> torch.Tensor:
         a = self.off
         self.off = a + _round_up(n_bytes)
@@ -64,12 +71,17 @@ class ModelState:
 
     def __init__(self, cfg: Config, device="cuda:0", image: str = "both", with_kv: bool = True,
                  with_params: bool = True, slack_garbage: bool = False, seq_lens: Optional[Sequence[int]] = None,
-                 plan_mode: int = B.PLAN_CMM, cap_mode: str = "span", kv_layout: int = B.KV_TOKEN_MAJOR):
+                 plan_mode: int = B.PLAN_CMM, cap_mode: str = "span", kv_layout: int = B.KV_TOKEN_MAJOR,
+                 shard: Optional[Tuple[int, int]] = None, exchange=None):
         self.cfg, self.device = cfg, torch.device(device)
         self.cap_mode = cap_mode          # "span": union span of the rank's intervals (one hazard phase, L5);
                                           # "tight": the widest shard the rank ever holds (shards wrap, plans need phases)
         self.plan_mode = plan_mode        # B.PLAN_CMM (the paper's planner) | PLAN_GREEDY | PLAN_FULL_RELOAD
         self.kv_layout = kv_layout        # B.KV_TOKEN_MAJOR (reading K1) | B.KV_HEAD_MAJOR (its optional second layout)
+        # One process per GPU: shard = (this process, number of processes); simulated rank r lives in the
+        # memory of process r mod n.  This process allocates and fills only ITS ranks; the others' arenas / pools are opened as
+        # CUDA-IPC mappings (`exchange`: an all-gather of picklable handles, e.g. torch.distributed.all_gather_object).
+        self.shard, self.exchange = shard, exchange
         self.seed = SEED0 + 1000 * cfg.index
         self.image_kinds = ("pinned", "device") if image == "both" else (image,)
         self.specs: List[TensorSpec] = tensor_inventory(cfg) if with_params else []
@@ -85,6 +97,27 @@ class ModelState:
         if with_kv:
             self._alloc_kv(slack_garbage, seq_lens)
         self._prepared: Dict[Tuple[int, str], object] = {}
+
+    def is_local(self, rank: int) -> bool:
+        return self.shard is None or rank % self.shard[1] == self.shard[0]
+
+    def rank_devices(self) -> List[int]:
+        """etp_ctx_set_rank_devices map of this process: its own ranks on logical device 0, everybody else's -1."""
+        return [0 if self.is_local(r) else -1 for r in range(self.n_ranks)]
+
+    def _open_remote(self, local: Dict[int, torch.Tensor]) -> Dict[int, torch.Tensor]:
+        """rank -> uint8 tensor for EVERY rank: the local ones as they are, the others through CUDA IPC."""
+        if self.shard is None:
+            return dict(local)
+        mine = {r: t.untyped_storage()._share_cuda_() + (t.storage_offset(), t.numel()) for r, t in local.items()}
+        out = dict(local)
+        for handles in self.exchange(mine):
+            for r, h in handles.items():
+                if r in out:
+                    continue
+                st = torch.UntypedStorage._new_shared_cuda(*h[:-2])
+                out[r] = torch.empty(0, dtype=torch.uint8, device=st.device).set_(st, h[-2], (h[-1],))
+        return out
 
     # ------------------------------------------------------------------ S1 + S2 through the C ABI
     def initial_layouts(self) -> Dict[str, List[B.Shard]]:
@@ -158,7 +191,9 @@ class ModelState:
                 need[r] += _round_up(cap * sp.unit_bytes)
             lo, hi = self.reload_range[sp.klass]
             img_bytes += _round_up((hi - lo) * sp.unit_bytes)
-        self.rank_arena = {r: Arena(need[r], self.device) for r in range(self.n_ranks)}
+        local = {r: Arena(need[r], self.device) for r in range(self.n_ranks) if self.is_local(r)}
+        opened = self._open_remote({r: a.t for r, a in local.items()})
+        self.rank_arena = {r: local[r] if r in local else Arena.wrap(opened[r]) for r in range(self.n_ranks)}
         self.image_arena = {k: Arena(img_bytes, self.device, pinned=(k == "pinned"), zero=False) for k in self.image_kinds}
         self.slabs: Dict[str, Dict[int, torch.Tensor]] = {}
         self.images: Dict[str, Dict[str, torch.Tensor]] = {k: {} for k in self.image_kinds}
@@ -169,13 +204,15 @@ class ModelState:
             for (r, s, e, _) in first[sp.klass]:
                 _, cap = self.geom[sp.klass][r]
                 slab = self.rank_arena[r].take(cap * sp.unit_bytes)
+                self.slabs[sp.name][r] = slab
+                if not self.is_local(r):
+                    continue                   # its owner fills it
                 if slack_garbage:
                     nb8 = (slab.numel() + 7) // 8 * 8
                     slab.copy_(fill_bytes(self.seed, 10_000 + sp.stream * 16 + r, 0, nb8, device=self.device)[: slab.numel()])
                 if e > s:   # anchor = s, so the old shard sits at slots [0, e - s)
                     fill_normal16(self.seed, sp.stream, s * epu, (e - s) * epu, self.cfg.model.init_std, self.dt,
                                   out=slab[: (e - s) * sp.unit_bytes].view(self.dt))
-                self.slabs[sp.name][r] = slab
             lo, hi = self.reload_range[sp.klass]
             dev_img = None
             for k in self.image_kinds:
@@ -211,6 +248,8 @@ class ModelState:
               "layout": self.kv_layout}
         lay = dict(layout=self.kv_layout, block_size=kvs.block_size)
         for (r, s, e, _) in first:
+            if not self.is_local(r):
+                continue
             nb = rows * head_cap * frag
             if slack_garbage:
                 pool = fill_bytes(seed, 100 + r, 0, (nb + 7) // 8 * 8, device=self.device)[:nb]
@@ -219,6 +258,8 @@ class ModelState:
             if e > s:
                 fill_kv_pool(pool, rows, head_cap, m.head_dim, 0, s, e - s, m.n_kv_heads, seed, 1, self.dt, **lay)
             kv["pools"][r] = pool
+        torch.cuda.synchronize(self.device)
+        kv["pools"] = self._open_remote(kv["pools"])
         # the backup of each rank that dies: its pool at the time of death compacted to its own heads (reading K4)
         for i, st in enumerate(self.steps):
             ds, de = [(s, e) for (r, s, e, _) in st.old["head"] if r == st.dead][0]

@@ -120,19 +120,19 @@ def test_one_context_per_rank_group_pulls_only_its_own_destinations(mode):
         for c, m in zip(ctxs, maps):
             c.set_rank_devices(m)
         streams = [Streams(), Streams()]
-        reps = [run_params(c, world, bufs, images, 0, s) if mode == "span" else None for c, s in zip(ctxs, streams)]
-        if mode == "tight":
-            n_phases = None
-            for c in ctxs:
-                c.set_option(etp.OPT_ONLY_PHASE, 1)
-            phase = 0
-            while n_phases is None or phase < n_phases:
+        reps = [None, None]
+        if mode == "span":
+            reps = [run_params(c, world, bufs, images, 0, s) for c, s in zip(ctxs, streams)]
+            assert all(r["n_phases"] == 1 for r in reps)
+        else:
+            phase, n_phases = 0, 1
+            while phase < n_phases:
                 for i, (c, s) in enumerate(zip(ctxs, streams)):
                     c.set_option(etp.OPT_ONLY_PHASE, phase + 1)
-                    reps[i] = run_params(c, world, bufs, images, 0, s)
+                    reps[i] = run_params(c, world, bufs, images, 0, s)      # lowers the whole plan, enqueues this phase only
                     n_phases = reps[i]["n_phases"]
                 for s in streams:
-                    s.sync()                      # the barrier between hazard phases
+                    s.sync()                                                # the barrier between hazard phases
                 phase += 1
             assert n_phases >= 2
         for s in streams:
@@ -199,3 +199,39 @@ def test_two_processes_pull_through_cuda_ipc_mappings():
                 assert t.cpu().numpy().tobytes() == expect[sp.name][r].tobytes(), f"{sp.name} rank {r}: slab differs from the oracle image"
     assert sum(g[1] for g in got) == stats["d2d_bytes"] and sum(g[2] for g in got) == stats["h2d_bytes"]
     assert all(g[3] > 0 for g in got)
+
+
+def _torchrun(script_args, n=2, timeout=900):
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, ETP_BENCH_ALIAS_GPU0="1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", "29617"] + script_args
+    return subprocess.run(cmd, cwd=root, env=env, capture_output=True, text=True, timeout=timeout)
+
+
+@pytest.mark.parametrize("n", [2, 3])
+def test_sharded_state_one_process_per_rank_group(n):
+    """tests/sharded_check.py under torchrun: the sharded ModelState (CUDA-IPC mapped peers) resharded by N processes, whole state
+    against the plain definition in every process."""
+    r = _torchrun(["tests/sharded_check.py", "2", "2", "8"], n=n)
+    assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-3000:]
+    assert r.stdout.count("SHARDED_OK") == n
+
+
+def test_bench_sharded_moves_the_same_bytes_as_one_process():
+    """`bench.py --gpus 2 --sharded` (two processes aliased to cuda:0) prints the contract line, strong scaling, and moves exactly
+    the bytes the single-process run of the same reduced workload moves."""
+    import json
+    common = ["bench.py", "--sharded", "--config", "2", "--layers", "2", "--seqs", "4", "--steps", "2", "--warmup", "1"]
+    two = _torchrun(common + ["--gpus", "2"], n=2)
+    assert two.returncode == 0, two.stdout[-3000:] + two.stderr[-3000:]
+    one = _torchrun(common + ["--gpus", "1"], n=1)
+    assert one.returncode == 0, one.stdout[-3000:] + one.stderr[-3000:]
+    l2 = json.loads([l for l in two.stdout.splitlines() if l.startswith("{")][-1])
+    l1 = json.loads([l for l in one.stdout.splitlines() if l.startswith("{")][-1])
+    assert l2["n_gpus"] == 2 and l2["scaling"] == "strong" and l2["config"]["aliased_to_gpu0"] is True
+    assert l2["config"]["moved_GB_per_step"] == l1["config"]["moved_GB_per_step"] > 0
+    assert l2["e2e"]["h2d_bytes_per_step"] == l1["e2e"]["h2d_bytes_per_step"] > 0

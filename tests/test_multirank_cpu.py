@@ -39,6 +39,42 @@ def test_max_over_ranks_and_whole_job_value_gloo_world2():
     assert gbps == pytest.approx(2 * 3e9 / 15e-3 / 1e9)      # bytes of all ranks / max time
 
 
+def _shard_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch
+    import torch.distributed as dist
+    import bench
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    owners = bench.split_ranks(8, world)
+    mine = {r: ("handle-of", rank, r) for r in owners[rank]}        # what ModelState._open_remote exchanges (picklable handles)
+    got = [None] * world
+    dist.all_gather_object(got, mine)
+    seen = sorted(r for h in got for r in h)
+    moved = torch.tensor([float(100 * (rank + 1))], dtype=torch.float64)
+    dist.all_reduce(moved, op=dist.ReduceOp.SUM)
+    ms = torch.tensor([float(3 + rank)], dtype=torch.float64)
+    dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    out.put((rank, owners, seen, moved.item(), ms.item(), [got[p][r][1] for p in range(world) for r in got[p]]))
+    dist.destroy_process_group()
+
+
+def test_sharded_partition_by_destination_rank_gloo_world2():
+    """--sharded bookkeeping on CPU: simulated rank r belongs to process r mod N, every rank has exactly one owner, the handle
+    exchange reaches everybody, the job's bytes are the SUM and its time the MAX over processes."""
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_shard_worker, args=(r, 2, 29713, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(out.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+    for rank, owners, seen, moved, ms, owner_of_handle in res:
+        assert owners == [[0, 2, 4, 6], [1, 3, 5, 7]] and seen == list(range(8))
+        assert moved == 300.0 and ms == 4.0
+        assert owner_of_handle == [0, 0, 0, 0, 1, 1, 1, 1]
+
+
 def _run_reference(rank):
     env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", LOCAL_RANK=str(rank), CUDA_VISIBLE_DEVICES="")
     return subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1", "--gpus", "2",
