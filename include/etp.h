@@ -157,6 +157,15 @@ etp_status etp_cmm_plan(const etp_shard* old_layout, int32_t n_old, const int64_
  * migration-aware extension */
 etp_status etp_plan_create(etp_plan_mode mode, const etp_shard* old_layout, int32_t n_old,
                            const int64_t* target_bounds, int32_t M, etp_plan** out);
+/* ETP_PLAN_MIGRATION_AWARE with a price per link (reading M2; "requires incorporating link
+ * reachability and cost weighting into planning", :257): link_cost is a host array [n_cost_ranks][n_cost_ranks] of integers
+ * in [0, 2^20], link_cost[src * n_cost_ranks + dst] = cost of moving ONE unit from rank src to rank dst (indexed by rank id).
+ * The planner minimises sum(transferred units x link cost) at the same minimal reload volume; a unit held by several alive
+ * ranks is taken from the cheapest link (tie: lower rank id).  link_cost = NULL is etp_plan_create (every link costs 1; on one
+ * NVSwitch node the matrix is uniform and the plan is the unweighted one). */
+etp_status etp_plan_create_weighted(etp_plan_mode mode, const etp_shard* old_layout, int32_t n_old,
+                                    const int64_t* target_bounds, int32_t M, const int64_t* link_cost,
+                                    int32_t n_cost_ranks, etp_plan** out);
 /* copies up to cap tasks into out (host); *n_out = total number of tasks (call with cap = 0 to size) */
 etp_status etp_plan_tasks(const etp_plan* plan, etp_task* out, int64_t cap, int64_t* n_out);
 /* writes the M new shards (host, M entries), alive = 1 */

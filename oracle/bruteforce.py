@@ -33,6 +33,22 @@ def min_cost_given_owners(old_layout, target_bounds: Sequence[int], owners: Sequ
     return best
 
 
+def min_weighted_cost_given_owners(old_layout, target_bounds: Sequence[int], owners: Sequence[int], link_cost) -> Tuple[int, int]:
+    """Same enumeration with a per-link price (reading M2): minimum of (reloaded units, sum over transferred units of
+    link_cost[source][owner]).  No intervals, no Algorithm 1."""
+    units = []
+    for j in range(len(target_bounds) - 1):
+        for u in range(target_bounds[j], target_bounds[j + 1]):
+            units.append((owners[j], _holders(old_layout, u) + [HOST]))
+    best = None
+    for choice in itertools.product(*[srcs for (_, srcs) in units]):
+        reload_units = sum(1 for c in choice if c == HOST)
+        cost = sum(link_cost[c][own] for (own, _), c in zip(units, choice) if c != HOST and c != own)
+        if best is None or (reload_units, cost) < best:
+            best = (reload_units, cost)
+    return best
+
+
 def best_over_owner_permutations(old_layout, target_bounds: Sequence[int]) -> Dict[Tuple[int, ...], Tuple[int, int]]:
     """Same, for every injective choice of owners among the alive ranks (reading C11: reported, not required)."""
     alive = sorted(r for (r, _, _, a) in old_layout if a)

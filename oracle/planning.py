@@ -81,10 +81,11 @@ def _subtract(rest: List[Tuple[int, int]], a: int, b: int) -> List[Tuple[int, in
 
 
 def cmm_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None,
-             owners: Optional[Sequence[int]] = None) -> Tuple[List[Task], List[Shard]]:
+             owners: Optional[Sequence[int]] = None, link_cost=None) -> Tuple[List[Task], List[Shard]]:
     """Algorithm 1 with readings C1-C7.  Returns (tasks sorted by (dst, begin), new layout).
     ``owners`` (reading M1, not in the paper): owners[j] = the alive rank that will hold target j, instead of the
-    j-th alive rank of reading C3."""
+    j-th alive rank of reading C3.  ``link_cost`` (reading M2): link_cost[src][dst] = integer cost of moving one unit from
+    rank src to rank dst; replicated sources are then tried in ascending (cost to the owner, rank id) instead of rank id."""
     old = [tuple(int(v) for v in s) for s in old_layout]
     if not old:
         raise ValueError("empty layout")
@@ -112,7 +113,10 @@ def cmm_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequen
     for j in range(M):                                                   # l.6
         dst = G[j]
         rest = [(tb[j], tb[j + 1])] if tb[j] < tb[j + 1] else []         # l.7 tar_range
-        order = [s for s in alive_sorted if s[0] == dst] + [s for s in alive_sorted if s[0] != dst]   # C7
+        others = [s for s in alive_sorted if s[0] != dst]
+        if link_cost is not None:
+            others.sort(key=lambda s: (link_cost[s[0]][dst], s[0]))                                  # M2
+        order = [s for s in alive_sorted if s[0] == dst] + others                                    # C7
         for (rank_i, s_i, e_i, _) in order:                              # l.8-9, alive only
             for (x, y) in list(rest):
                 a, b = max(x, s_i), min(y, e_i)                          # l.10 inter
@@ -144,12 +148,19 @@ def width_arrangements(H: int, M: int) -> List[List[int]]:
     return sorted(out)
 
 
-def migration_aware_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None):
+def weighted_transfer_cost(tasks: Sequence[Task], link_cost) -> int:
+    """Sum over TRANSFER tasks of units x link_cost[src][dst] (reading M2; "link reachability and cost weighting")."""
+    return sum((e - b) * (1 if link_cost is None else link_cost[s][d]) for (k, s, d, b, e) in tasks if k == TRANSFER)
+
+
+def migration_aware_plan(old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None, link_cost=None):
     """SURVEY.md 8(f) #2 / DESIGN.md reading M1 (an extension; PAPER.md:160 makes only the reload volume minimal and
     :247/:257 leave transfer cost to future work).  Plain definition by exhaustion: over every admissible bounds vector
     (all placements of the wide shards, or the given bounds) and every injective assignment of targets to alive ranks,
     run Algorithm 1 with those owners and take the lexicographic minimum of
         (reload units, transfer units, bounds vector, owners vector).
+    With ``link_cost`` (reading M2: PAPER.md:247, :257 leave "link reachability and cost weighting" of the planner to future
+    work) the second component is the WEIGHTED transfer cost sum(units x link_cost[src][dst]); uniform costs change nothing.
     Returns (tasks, new layout) like cmm_plan."""
     import itertools
     old = [tuple(int(v) for v in s) for s in old_layout]
@@ -165,9 +176,9 @@ def migration_aware_plan(old_layout: Sequence[Shard], M: int, target_bounds: Opt
     best = None
     for tb in cands:
         for owners in itertools.permutations(alive, M):
-            tasks, new = cmm_plan(old, M, tb, owners)
+            tasks, new = cmm_plan(old, M, tb, owners, link_cost)
             st = plan_stats(tasks)
-            key = (st["reload_units"], st["transfer_units"], tuple(tb), tuple(owners))
+            key = (st["reload_units"], weighted_transfer_cost(tasks, link_cost), tuple(tb), tuple(owners))
             if best is None or key < best[0]:
                 best = (key, tasks, new)
     return best[1], best[2]

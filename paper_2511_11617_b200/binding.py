@@ -89,7 +89,7 @@ class etp_interval(C.Structure):
 
 
 EXPORTS = ["etp_ctx_create", "etp_ctx_create_multi", "etp_ctx_set_rank_devices", "etp_ctx_device_report", "etp_ctx_destroy", "etp_last_error", "etp_version", "etp_ctx_set_option", "etp_ctx_get_option",
-           "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_tasks", "etp_plan_new_layout",
+           "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_create_weighted", "etp_plan_tasks", "etp_plan_new_layout",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
            "etp_shard_linear_multi", "etp_linear_prepare", "etp_linear_run", "etp_linear_plan_info", "etp_linear_free",
            "etp_moe_linear", "etp_copy_intervals"]
@@ -118,6 +118,7 @@ def lib() -> C.CDLL:
         L.etp_partition.argtypes = [C.c_int, i64, i32, C.c_int, i64, C.POINTER(i64)]
         L.etp_cmm_plan.argtypes = [C.POINTER(etp_shard), i32, C.POINTER(i64), i32, C.POINTER(vp)]
         L.etp_plan_create.argtypes = [C.c_int, C.POINTER(etp_shard), i32, C.POINTER(i64), i32, C.POINTER(vp)]
+        L.etp_plan_create_weighted.argtypes = [C.c_int, C.POINTER(etp_shard), i32, C.POINTER(i64), i32, C.POINTER(i64), i32, C.POINTER(vp)]
         L.etp_plan_tasks.argtypes = [vp, C.POINTER(etp_task), i64, C.POINTER(i64)]
         L.etp_plan_new_layout.argtypes = [vp, C.POINTER(etp_shard), i32, C.POINTER(i32)]
         L.etp_plan_get_stats.argtypes = [vp, C.POINTER(etp_plan_stats)]
@@ -206,12 +207,19 @@ class Plan:
         return {n: getattr(st, n) for n, _ in st._fields_}
 
 
-def etp_plan_create(mode: int, old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None) -> Plan:
+def etp_plan_create(mode: int, old_layout: Sequence[Shard], M: int, target_bounds: Optional[Sequence[int]] = None,
+                    link_cost: Optional[Sequence[Sequence[int]]] = None) -> Plan:
+    """link_cost: square matrix [src][dst] of per-unit link prices (etp_plan_create_weighted), migration-aware mode only."""
     h = vp()
     tb = None
     if target_bounds is not None:
         tb = (i64 * len(target_bounds))(*[int(x) for x in target_bounds])
-    _check(lib().etp_plan_create(mode, _shards(old_layout), len(old_layout), tb, M, C.byref(h)))
+    if link_cost is None:
+        _check(lib().etp_plan_create(mode, _shards(old_layout), len(old_layout), tb, M, C.byref(h)))
+    else:
+        n = len(link_cost)
+        flat = (i64 * (n * n))(*[int(v) for row in link_cost for v in row])
+        _check(lib().etp_plan_create_weighted(mode, _shards(old_layout), len(old_layout), tb, M, flat, n, C.byref(h)))
     return Plan(h.value)
 
 

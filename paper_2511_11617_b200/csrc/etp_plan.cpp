@@ -101,35 +101,79 @@ void finish_stats(etp_plan* p, const std::vector<int64_t>& tb) {
     p->stats = st;
 }
 
-// ETP_PLAN_MIGRATION_AWARE (reading M1; an extension, PAPER.md:160 minimises only the reload volume and :247/:257
-// leave transfer cost to future work).  The reload volume does not depend on who owns what, so minimising the transferred
-// units means maximising the KEPT units  sum_j |target_j  n  old interval of owner(j)|  over injective owner choices and,
-// when the bounds are free, over every placement of the ceil(H/M)-wide shards.  Assignment by dynamic programming over
-// subsets of alive ranks (f[mask] = best keep of targets popcount(mask).. with the ranks in mask taken); ties go to the
-// lexicographically smallest (bounds, owners) - bounds vectors are visited in lexicographic order and an equal score never
-// replaces the incumbent; the owners are rebuilt front to back taking the smallest rank that still reaches f.
-constexpr int kMaxAliveMigrationAware = 10;
+// One target of Algorithm 1 for a given owner: intersect with the sources in the order of reading C7 (the owner itself, then
+// ascending rank id) - or, with link costs (reading M2), ascending (cost of the link to the owner, rank id) - and subtract;
+// what stays open is reloaded.  Appends the tasks when `tasks` is given; returns the weighted transfer cost of the target.
+struct LinkCost {
+    const int64_t* m = nullptr;   // [n][n], m[src * n + dst] per unit; NULL = every link costs 1
+    int32_t n = 0;
+    int64_t at(int32_t src, int32_t dst) const { return m ? m[(int64_t)src * n + dst] : 1; }
+};
 
-int64_t best_owners(const std::vector<etp_shard>& alive, const std::vector<int64_t>& tb, int M, std::vector<int>* owners) {
+int64_t plan_target(etp_plan_mode mode, const std::vector<etp_shard>& alive, const etp_shard& own, int64_t tb0, int64_t tb1,
+                    const LinkCost& lc, std::vector<etp_task>* tasks) {
+    const int32_t owner = own.rank;
+    std::vector<Span> open;
+    if (tb0 < tb1) open.push_back({tb0, tb1});
+    int64_t cost = 0;
+    if (mode != ETP_PLAN_FULL_RELOAD) {
+        std::vector<const etp_shard*> order;
+        for (const etp_shard& s : alive)
+            if (s.rank != owner) order.push_back(&s);
+        if (lc.m)
+            std::stable_sort(order.begin(), order.end(), [&](const etp_shard* a, const etp_shard* b) { return lc.at(a->rank, owner) < lc.at(b->rank, owner); });
+        order.insert(order.begin(), &own);
+        for (const etp_shard* s : order) {
+            const bool self = s->rank == owner;
+            if (mode == ETP_PLAN_GREEDY && !self) continue;  // no cross-device transfer for gaps
+            std::vector<Span> hits;
+            for (const Span& o : open) {
+                const int64_t b = std::max(o.b, s->begin), e = std::min(o.e, s->end);  // Alg. 1 l.10
+                if (b < e) hits.push_back({b, e});
+            }
+            for (const Span& h : hits) {
+                if (tasks) tasks->push_back({self ? ETP_KEEP : ETP_TRANSFER, s->rank, owner, 0, h.b, h.e});  // l.11-12, C1, C4
+                if (!self) cost += (h.e - h.b) * lc.at(s->rank, owner);
+                carve(open, h.b, h.e);                                                                     // l.13
+            }
+        }
+    }
+    if (tasks)
+        for (const Span& o : open) tasks->push_back({ETP_RELOAD, -1, owner, 0, o.b, o.e});  // l.17-18, C2, C5
+    return cost;
+}
+
+// ETP_PLAN_MIGRATION_AWARE (readings M1, M2; an extension, PAPER.md:160 minimises only the reload volume and
+// :247/:257 leave transfer cost and "link reachability and cost weighting" to future work).  The reload volume does not depend
+// on who owns what, so the search minimises the (link-weighted) TRANSFER cost  sum_j cost(target j owned by owner(j))  over
+// injective owner choices and, when the bounds are free, over every placement of the ceil(H/M)-wide shards.  Assignment by
+// dynamic programming over subsets of alive ranks (f[mask] = least cost of targets popcount(mask).. with the ranks in mask
+// taken); ties go to the lexicographically smallest (bounds, owners) - bounds vectors are visited in lexicographic order and
+// an equal score never replaces the incumbent; the owners are rebuilt front to back taking the smallest rank that still reaches f.
+constexpr int kMaxAliveMigrationAware = 10;
+constexpr int64_t kNoAssignment = INT64_MAX;
+
+int64_t best_owners(const std::vector<etp_shard>& alive, const std::vector<int64_t>& tb, int M, const LinkCost& lc, std::vector<int>* owners) {
     const int n = (int)alive.size();
-    auto keep = [&](int j, int i) {
-        return std::max<int64_t>(0, std::min(tb[j + 1], alive[i].end) - std::max(tb[j], alive[i].begin));
-    };
-    std::vector<int64_t> f(size_t(1) << n, -1);
+    std::vector<int64_t> cost((size_t)M * n);
+    for (int j = 0; j < M; ++j)
+        for (int i = 0; i < n; ++i) cost[(size_t)j * n + i] = plan_target(ETP_PLAN_CMM, alive, alive[i], tb[j], tb[j + 1], lc, nullptr);
+    std::vector<int64_t> f(size_t(1) << n, kNoAssignment);
     for (int64_t mask = (int64_t(1) << n) - 1; mask >= 0; --mask) {
         const int j = __builtin_popcountll((unsigned long long)mask);
         if (j > M) continue;
         if (j == M) { f[mask] = 0; continue; }
-        int64_t best = -1;
+        int64_t best = kNoAssignment;
         for (int i = 0; i < n; ++i)
-            if (!(mask >> i & 1) && f[mask | (int64_t(1) << i)] >= 0) best = std::max(best, keep(j, i) + f[mask | (int64_t(1) << i)]);
+            if (!(mask >> i & 1) && f[mask | (int64_t(1) << i)] != kNoAssignment)
+                best = std::min(best, cost[(size_t)j * n + i] + f[mask | (int64_t(1) << i)]);
         f[mask] = best;
     }
     owners->assign(M, 0);
     int64_t mask = 0;
     for (int j = 0; j < M; ++j)
         for (int i = 0; i < n; ++i)
-            if (!(mask >> i & 1) && f[mask | (int64_t(1) << i)] >= 0 && keep(j, i) + f[mask | (int64_t(1) << i)] == f[mask]) {
+            if (!(mask >> i & 1) && f[mask | (int64_t(1) << i)] != kNoAssignment && cost[(size_t)j * n + i] + f[mask | (int64_t(1) << i)] == f[mask]) {
                 (*owners)[j] = i;
                 mask |= int64_t(1) << i;
                 break;
@@ -137,12 +181,12 @@ int64_t best_owners(const std::vector<etp_shard>& alive, const std::vector<int64
     return f[0];
 }
 
-etp_status choose_layout(const std::vector<etp_shard>& alive, int64_t H, int M, bool bounds_fixed, std::vector<int64_t>* tb,
-                         std::vector<int>* owner_idx) {
+etp_status choose_layout(const std::vector<etp_shard>& alive, int64_t H, int M, bool bounds_fixed, const LinkCost& lc,
+                         std::vector<int64_t>* tb, std::vector<int>* owner_idx) {
     if ((int)alive.size() > kMaxAliveMigrationAware)
         ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_plan_create: the migration-aware search is limited to %d alive ranks", kMaxAliveMigrationAware);
     if (bounds_fixed) {
-        best_owners(alive, *tb, M, owner_idx);
+        best_owners(alive, *tb, M, lc, owner_idx);
         return ETP_OK;
     }
     if (H < M) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_plan_create: %lld units over %d shards needs replication", (long long)H, M);
@@ -151,15 +195,15 @@ etp_status choose_layout(const std::vector<etp_shard>& alive, int64_t H, int M, 
     // width vectors with exactly r wide shards in lexicographic order (narrow before wide at the first difference)
     std::vector<int> wide(M, 0);
     for (int j = M - r; j < M; ++j) wide[j] = 1;   // lexicographically smallest: the wide shards last
-    int64_t best_keep = -1;
+    int64_t best_cost = kNoAssignment;
     std::vector<int64_t> cand(M + 1);
     std::vector<int> own;
     do {
         cand[0] = 0;
         for (int j = 0; j < M; ++j) cand[j + 1] = cand[j] + q + wide[j];
-        const int64_t k = best_owners(alive, cand, M, &own);
-        if (k > best_keep) {
-            best_keep = k;
+        const int64_t k = best_owners(alive, cand, M, lc, &own);
+        if (k < best_cost) {
+            best_cost = k;
             *tb = cand;
             *owner_idx = own;
         }
@@ -170,6 +214,12 @@ etp_status choose_layout(const std::vector<etp_shard>& alive, int64_t H, int M, 
 
 extern "C" etp_status etp_plan_create(etp_plan_mode mode, const etp_shard* old_layout, int32_t n_old,
                                       const int64_t* target_bounds, int32_t M, etp_plan** out) {
+    return etp_plan_create_weighted(mode, old_layout, n_old, target_bounds, M, nullptr, 0, out);
+}
+
+extern "C" etp_status etp_plan_create_weighted(etp_plan_mode mode, const etp_shard* old_layout, int32_t n_old,
+                                               const int64_t* target_bounds, int32_t M, const int64_t* link_cost,
+                                               int32_t n_cost_ranks, etp_plan** out) {
     if (!out) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_create: out is NULL");
     *out = nullptr;
     if (!old_layout || n_old < 1) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_create: empty old layout");
@@ -205,7 +255,17 @@ extern "C" etp_status etp_plan_create(etp_plan_mode mode, const etp_shard* old_l
     // owner_idx[j] = index into `alive` of the rank that holds target j.  Reading C3: the j-th alive rank in ascending id.
     std::vector<int> owner_idx(M);
     for (int32_t j = 0; j < M; ++j) owner_idx[j] = j;
-    if (mode == ETP_PLAN_MIGRATION_AWARE) ETP_TRY(choose_layout(alive, H, M, target_bounds != nullptr, &tb, &owner_idx));
+    LinkCost lc;
+    if (link_cost) {
+        if (mode != ETP_PLAN_MIGRATION_AWARE) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_create_weighted: link costs belong to ETP_PLAN_MIGRATION_AWARE");
+        for (const etp_shard& s : alive)
+            if (s.rank >= n_cost_ranks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_create_weighted: rank %d outside the %d x %d cost matrix", s.rank, n_cost_ranks, n_cost_ranks);
+        for (int64_t k = 0; k < (int64_t)n_cost_ranks * n_cost_ranks; ++k)
+            if (link_cost[k] < 0 || link_cost[k] > (int64_t(1) << 20)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_plan_create_weighted: link costs must be in [0, 2^20]");
+        lc.m = link_cost;
+        lc.n = n_cost_ranks;
+    }
+    if (mode == ETP_PLAN_MIGRATION_AWARE) ETP_TRY(choose_layout(alive, H, M, target_bounds != nullptr, lc, &tb, &owner_idx));
 
     etp_plan* p = new (std::nothrow) etp_plan();
     if (!p) ETP_FAIL(ETP_ERR_NOMEM, "etp_plan_create: out of memory");
@@ -214,31 +274,8 @@ extern "C" etp_status etp_plan_create(etp_plan_mode mode, const etp_shard* old_l
     p->old_layout.assign(old_layout, old_layout + n_old);
     for (int32_t j = 0; j < M; ++j) {
         const etp_shard& own = alive[owner_idx[j]];
-        const int32_t owner = own.rank;
-        p->new_layout.push_back({owner, 1, tb[j], tb[j + 1]});
-        std::vector<Span> open;
-        if (tb[j] < tb[j + 1]) open.push_back({tb[j], tb[j + 1]});
-        if (mode != ETP_PLAN_FULL_RELOAD) {
-            // sources in the order of reading C7: the owner itself, then ascending rank id
-            std::vector<const etp_shard*> order;
-            order.push_back(&own);
-            for (const etp_shard& s : alive)
-                if (s.rank != owner) order.push_back(&s);
-            for (const etp_shard* s : order) {
-                const bool self = s->rank == owner;
-                if (mode == ETP_PLAN_GREEDY && !self) continue;  // no cross-device transfer for gaps
-                std::vector<Span> hits;
-                for (const Span& o : open) {
-                    const int64_t b = std::max(o.b, s->begin), e = std::min(o.e, s->end);  // Alg. 1 l.10
-                    if (b < e) hits.push_back({b, e});
-                }
-                for (const Span& h : hits) {
-                    p->tasks.push_back({self ? ETP_KEEP : ETP_TRANSFER, s->rank, owner, 0, h.b, h.e});  // l.11-12, C1, C4
-                    carve(open, h.b, h.e);                                                              // l.13
-                }
-            }
-        }
-        for (const Span& o : open) p->tasks.push_back({ETP_RELOAD, -1, owner, 0, o.b, o.e});  // l.17-18, C2, C5
+        p->new_layout.push_back({own.rank, 1, tb[j], tb[j + 1]});
+        plan_target(mode, alive, own, tb[j], tb[j + 1], lc, &p->tasks);
     }
     std::stable_sort(p->tasks.begin(), p->tasks.end(), [](const etp_task& a, const etp_task& b) {
         return a.dst_rank != b.dst_rank ? a.dst_rank < b.dst_rank : a.begin < b.begin;

@@ -238,3 +238,42 @@ def test_no_cpu_fallback_without_a_device():
     with pytest.raises(etp.EtpError) as e:
         etp.Context(0)
     assert e.value.status == 6                      # ETP_ERR_CUDA
+
+
+def test_weighted_migration_aware_planner_matches_oracle():
+    """etp_plan_create_weighted (reading M2) against oracle.planning.migration_aware_plan(link_cost=...): random layouts (rank
+    ids with gaps, several dead ranks), random integer link prices, free and fixed bounds; task for task and layout for
+    layout.  Uniform prices give the unweighted plan; link costs with another planner mode are rejected."""
+    rng = np.random.default_rng(77)
+    done = 0
+    while done < 150:
+        old = random_layout(rng, max_n=6, max_h=60)
+        alive = [s for s in old if s[3]]
+        M = int(rng.integers(1, len(alive) + 1))
+        Hn = max(e for (_, _, e, _) in old)
+        if Hn < M:
+            continue
+        n_cost = max(r for (r, _, _, _) in old) + 1
+        cost = [[0 if a == b else int(rng.integers(1, 10)) for b in range(n_cost)] for a in range(n_cost)]
+        tb = OP.partition(Hn, M, ["floor", "ceil_first"][int(rng.integers(0, 2))]) if rng.random() < 0.4 else None
+        p = etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, old, M, tb, link_cost=cost)
+        tasks, new = OP.migration_aware_plan(old, M, tb, cost)
+        assert p.tasks() == tasks and p.new_layout() == new, (old, M, tb, cost)
+        done += 1
+    # replicated sources: the cheaper link supplies the unit (C7 -> M2)
+    rep = [(0, 0, 4, 1), (1, 0, 4, 1), (2, 4, 8, 1), (3, 8, 8, 1)]
+    cost = [[0, 9, 9, 9], [9, 0, 9, 1], [9, 9, 0, 9], [9, 9, 9, 0]]
+    p = etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, rep, 4, [0, 2, 4, 6, 8], link_cost=cost)
+    tasks, new = OP.migration_aware_plan(rep, 4, [0, 2, 4, 6, 8], cost)
+    assert p.tasks() == tasks and p.new_layout() == new
+    old = [(r, 7 * r, 7 * r + 7, 0 if r == 3 else 1) for r in range(8)]
+    ones = [[0 if a == b else 1 for b in range(8)] for a in range(8)]
+    base = etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, old, 7)
+    same = etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, old, 7, link_cost=ones)
+    assert same.tasks() == base.tasks() and same.new_layout() == base.new_layout()
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_plan_create(etp.PLAN_CMM, old, 7, link_cost=ones)
+    assert e.value.status == 1
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, old, 7, link_cost=[[0, 1], [1, 0]])
+    assert e.value.status == 1

@@ -8,8 +8,8 @@ import pytest
 
 from oracle import bruteforce
 from oracle.planning import (CEIL_FIRST, FLOOR, KEEP, RELOAD, TRANSFER, cmm_plan, eq1_reload_lower_bound,
-                             full_reload_plan, greedy_plan, layout_from_bounds, layout_from_widths, partition,
-                             plan_stats)
+                             full_reload_plan, greedy_plan, layout_from_bounds, layout_from_widths, migration_aware_plan,
+                             partition, plan_stats, weighted_transfer_cost, width_arrangements)
 
 KIND = {"KEEP": KEEP, "TRANSFER": TRANSFER, "RELOAD": RELOAD}
 
@@ -312,3 +312,55 @@ def test_errors_and_edge_cases():
     old = [(0, 0, 2, 0), (1, 2, 4, 1), (2, 4, 6, 0), (3, 6, 8, 1)]
     tasks, _ = cmm_plan(old, 1)
     assert [(k, b, e) for (k, _, _, b, e) in tasks] == [(RELOAD, 0, 2), (KEEP, 2, 4), (RELOAD, 4, 6), (TRANSFER, 6, 8)]
+
+
+# ------------------------------------------------------------------------------------------ link-cost weights (reading M2)
+def two_island_cost(n, island, far):
+    """link_cost[src][dst]: 1 inside an island of `island` consecutive ranks, `far` across islands."""
+    return [[0 if a == b else (1 if a // island == b // island else far) for b in range(n)] for a in range(n)]
+
+
+def test_weighted_migration_aware_plan_against_unit_level_bruteforce():
+    """Reading M2 ("incorporating link reachability and cost weighting into planning"): the weighted planner's
+    (reload, weighted transfer cost) equals the minimum, over every owner permutation and every {floor, ceil} bounds vector, of
+    the UNIT-LEVEL brute force that prices every unit's source by its link - no intervals, no Algorithm 1."""
+    import itertools
+    from oracle import bruteforce as BF
+    rng = random.Random(20)
+    checked = 0
+    while checked < 25:
+        n = rng.randint(3, 4)
+        Hn = rng.randint(n, 8)
+        cuts = sorted(rng.sample(range(1, Hn), n - 1)) if Hn > n else list(range(1, n))
+        b = [0] + cuts + [Hn]
+        dead = rng.randrange(n)
+        old = [(r, b[r], b[r + 1], 0 if r == dead else 1) for r in range(n)]
+        M = n - 1
+        if Hn < M:
+            continue
+        cost = [[0 if a == c else rng.randint(1, 5) for c in range(n)] for a in range(n)]
+        tasks, new = migration_aware_plan(old, M, None, cost)
+        st = plan_stats(tasks)
+        got = (st["reload_units"], weighted_transfer_cost(tasks, cost))
+        alive = [r for (r, _, _, a) in old if a]
+        best = min(BF.min_weighted_cost_given_owners(old, tb, owners, cost)
+                   for tb in width_arrangements(Hn, M) for owners in itertools.permutations(alive, M))
+        assert got == best, (old, cost, got, best)
+        checked += 1
+
+
+def test_weighted_plan_prefers_cheap_links_and_uniform_costs_change_nothing():
+    # two NVLink islands {0,1,2,3} and {4,5,6,7}; rank 3 dies; 7 targets over 56 units
+    old = [(r, 7 * r, 7 * r + 7, 0 if r == 3 else 1) for r in range(8)]
+    uniform = two_island_cost(8, 8, 1)
+    islands = two_island_cost(8, 4, 16)
+    base = migration_aware_plan(old, 7)
+    assert migration_aware_plan(old, 7, None, uniform) == base                      # one NVSwitch node: the result to state
+    tasks, new = migration_aware_plan(old, 7, None, islands)
+    assert plan_stats(tasks)["reload_units"] == plan_stats(base[0])["reload_units"] == 7
+    assert weighted_transfer_cost(tasks, islands) <= weighted_transfer_cost(base[0], islands)
+    # replicated sources (C7 -> M2): the cheaper holder supplies the unit
+    rep = [(0, 0, 4, 1), (1, 0, 4, 1), (2, 4, 8, 1), (3, 8, 8, 1)]
+    cost = [[0, 9, 9, 9], [9, 0, 9, 1], [9, 9, 0, 9], [9, 9, 9, 0]]
+    t, _ = cmm_plan(rep, 4, [0, 2, 4, 6, 8], owners=[0, 3, 2, 1], link_cost=cost)
+    assert (TRANSFER, 1, 3, 2, 4) in t                                              # rank 3 pulls [2,4) from rank 1 (cost 1), not rank 0 (9)
