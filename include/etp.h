@@ -333,6 +333,24 @@ etp_status etp_moe_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, c
                           const int64_t* row_offsets, int32_t n_experts, int64_t in_features, int64_t out_features,
                           const etp_tensor* w, const etp_shard* layout, int32_t n_shards, void* y_perm, void* stream);
 
+/* ------------------------------------------------------------------------------------------------ EPLB-style placement
+ * PAPER.md:172-174, Fig. 4, :235, :249 - "replicating hot-spot experts and adjusting routing"; after an unequal-width reshard
+ * one GPU holds a smaller shard and "more idle compute capacity", and the planner "schedules more expert replicas to the
+ * under-utilized GPU".  The rule is DESIGN.md reading E1 (the paper gives none).  Host-only, exact integer arithmetic.
+ *   expert_load[e]   tokens routed to expert e (0 .. 2^40);  home_rank[e]: the rank that holds e (the expert plan), or -1 for
+ *                    an expert without a holder (Fig. 4's recovered expert);
+ *   rank_capacity[r] compute available for expert work on rank r (0 = dead rank, <= 2^30);  spare_slots[r]: free expert slots.
+ * An expert with k instances (<= 8) serves load / k on each; L(r) = (sum of the shares on r) / capacity[r].  Step 1: holderless
+ * experts, hottest first, go to the usable rank with a spare slot that is least loaded after taking them.  Step 2: while it
+ * strictly lowers max L, add the instance (expert on the hottest rank -> rank with a spare slot) that minimises the new max L
+ * (ties: lower expert id, then lower rank id).  replicas_out receives the new instances in creation order (call with cap = 0
+ * to size).  Routing convention for etp_moe_linear_instances: instance j of k gets rows [floor(j n / k), floor((j+1) n / k))
+ * of the expert's n routed rows, instances ordered home first, then replicas in creation order. */
+typedef struct { int32_t expert, rank; } etp_replica;
+etp_status etp_eplb_place(const int64_t* expert_load, const int32_t* home_rank, int32_t n_experts,
+                          const int64_t* rank_capacity, const int32_t* spare_slots, int32_t n_ranks,
+                          etp_replica* replicas_out, int32_t cap, int32_t* n_replicas);
+
 /* ------------------------------------------------------------------------------------------------ microbenchmark entry
  * Copies n arbitrary intervals with the same persistent kernel (config 5b).  host_descs: host array; src/dst: device,
  * 16-B aligned; bytes: multiple of 16.  Destinations must be mutually disjoint and disjoint from every source (the

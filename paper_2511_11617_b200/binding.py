@@ -84,6 +84,10 @@ class etp_linear_plan_stats(C.Structure):
                 ("n_split_tiles", i64), ("n_splits", i32 * 8)]
 
 
+class etp_replica(C.Structure):
+    _fields_ = [("expert", i32), ("rank", i32)]
+
+
 class etp_interval(C.Structure):
     _fields_ = [("src", vp), ("dst", vp), ("bytes", i64)]
 
@@ -92,7 +96,7 @@ EXPORTS = ["etp_ctx_create", "etp_ctx_create_multi", "etp_ctx_set_rank_devices",
            "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_create_weighted", "etp_plan_tasks", "etp_plan_new_layout",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
            "etp_shard_linear_multi", "etp_linear_prepare", "etp_linear_run", "etp_linear_plan_info", "etp_linear_free",
-           "etp_moe_linear", "etp_copy_intervals"]
+           "etp_moe_linear", "etp_eplb_place", "etp_copy_intervals"]
 
 _lib = None
 
@@ -139,6 +143,8 @@ def lib() -> C.CDLL:
         L.etp_linear_free.restype = None
         L.etp_moe_linear.argtypes = [vp, C.c_int, C.c_int, vp, C.POINTER(i64), i32, i64, i64, C.POINTER(etp_tensor), C.POINTER(etp_shard),
                                      i32, vp, vp]
+        L.etp_eplb_place.argtypes = [C.POINTER(i64), C.POINTER(i32), i32, C.POINTER(i64), C.POINTER(i32), i32, C.POINTER(etp_replica), i32,
+                                     C.POINTER(i32)]
         L.etp_copy_intervals.argtypes = [vp, C.POINTER(etp_interval), i64, vp, C.POINTER(etp_reshard_report)]
         _lib = L
     return _lib
@@ -248,6 +254,21 @@ def etp_page_table_rewrite(table, seq_lens, last_use, block_size: int, budget: i
     _check(lib().etp_page_table_rewrite(C.byref(pt), block_size, budget, ev.ctypes.data_as(C.POINTER(i32)), C.byref(n_ev),
                                         pairs.ctypes.data_as(C.POINTER(i32)), cap, C.byref(n_pairs)))
     return [int(v) for v in ev[: n_ev.value]], [(int(a), int(b)) for a, b in pairs[: n_pairs.value]]
+
+
+def etp_eplb_place(expert_load: Sequence[int], home_rank: Sequence[int], rank_capacity: Sequence[int],
+                   spare_slots: Sequence[int]) -> List[Tuple[int, int]]:
+    """EPLB-style replica placement (host-only): [(expert, rank)] of the new instances in creation order."""
+    E, R = len(expert_load), len(rank_capacity)
+    ld = (i64 * max(E, 1))(*[int(v) for v in expert_load])
+    hm = (i32 * max(E, 1))(*[int(v) for v in home_rank])
+    cp = (i64 * R)(*[int(v) for v in rank_capacity])
+    sl = (i32 * R)(*[int(v) for v in spare_slots])
+    n = i32()
+    _check(lib().etp_eplb_place(ld, hm, E, cp, sl, R, None, 0, C.byref(n)))
+    out = (etp_replica * max(n.value, 1))()
+    _check(lib().etp_eplb_place(ld, hm, E, cp, sl, R, out, n.value, C.byref(n)))
+    return [(r.expert, r.rank) for r in out[: n.value]]
 
 
 # ------------------------------------------------------------------------------------------------ device calls

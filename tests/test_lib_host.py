@@ -277,3 +277,31 @@ def test_weighted_migration_aware_planner_matches_oracle():
     with pytest.raises(etp.EtpError) as e:
         etp.etp_plan_create(etp.PLAN_MIGRATION_AWARE, old, 7, link_cost=[[0, 1], [1, 0]])
     assert e.value.status == 1
+
+
+def test_eplb_place_matches_oracle():
+    """etp_eplb_place (incremental integer loads, 128-bit cross-multiplication) against oracle/eplb.py (Fractions, recomputed
+    from scratch every step): Fig. 4's hand-worked instance and 300 random ones incl. dead ranks, homeless experts, zero loads."""
+    from oracle import eplb
+    assert etp.etp_eplb_place([60, 20, 20, 10], [0, -1, 2, 3], [2, 0, 2, 3], [2, 0, 2, 2]) == [(1, 3), (0, 3), (1, 2)]
+    rng = np.random.default_rng(5)
+    for _ in range(300):
+        R = int(rng.integers(2, 7))
+        E = int(rng.integers(1, 14))
+        load = [int(v) for v in rng.integers(0, 2000, E)]
+        cap = [int(v) for v in rng.integers(0, 6, R)]
+        if not any(cap):
+            cap[0] = 1
+        usable = [r for r in range(R) if cap[r] > 0]
+        home = [int(rng.choice(usable)) if rng.random() > 0.15 else -1 for _ in range(E)]
+        slots = [int(v) for v in rng.integers(0, 4, R)]
+        if sum(slots[r] for r in usable) < sum(1 for h in home if h < 0):
+            with pytest.raises(etp.EtpError) as e:
+                etp.etp_eplb_place(load, home, cap, slots)
+            assert e.value.status == 3
+            continue
+        replicas, _ = eplb.place(load, home, cap, slots)
+        assert etp.etp_eplb_place(load, home, cap, slots) == replicas, (load, home, cap, slots)
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_eplb_place([1], [0], [0], [1])
+    assert e.value.status == 1
