@@ -327,11 +327,30 @@ void etp_linear_free(etp_linear_plan* plan);
  *   ETP_COL_PARALLEL: stored [out][in] (gate, up);  ETP_ROW_PARALLEL: stored transposed [in][out] (down), in % 64 == 0.
  * x_perm [n_rows][in_features], y_perm [n_rows][out_features]: device, 16-B aligned, row-major, rows grouped by expert in
  * ascending expert id; row_offsets: HOST array of n_experts + 1 non-decreasing offsets starting at 0.  Routing, activation
- * and the weighted combine are the caller's.  fp32 accumulation, one rounding to 16 bit.  Asynchronous on `stream`; calls
- * on one ctx must not overlap in time (ctx-owned work-item table). */
+ * and the weighted combine are the caller's.  fp32 accumulation, one rounding to 16 bit.  Asynchronous on `stream`; the work-item
+ * table lives in a stream-ordered allocation, so calls on different streams of one ctx may overlap. */
 etp_status etp_moe_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x_perm,
                           const int64_t* row_offsets, int32_t n_experts, int64_t in_features, int64_t out_features,
                           const etp_tensor* w, const etp_shard* layout, int32_t n_shards, void* y_perm, void* stream);
+
+/* The same with explicit expert INSTANCES (reading E1): after etp_eplb_place / etp_eplb_apply an expert may exist on
+ * several ranks, each instance serving a slice of the expert's routed rows.  instances: host array; instance i multiplies rows
+ * [row_begin, row_end) of x_perm by the expert matrix that sits in slot `slot` of rank `rank`'s slab (for the home instance
+ * slot = (expert - anchor_unit) mod cap_units, for a replica the slot etp_eplb_apply returned).  Row ranges must be disjoint
+ * and inside [0, n_rows); rows no instance covers are left untouched.  `expert` is informational. */
+typedef struct { int32_t expert, rank; int64_t slot; int64_t row_begin, row_end; } etp_moe_instance;
+etp_status etp_moe_linear_instances(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x_perm,
+                                    const etp_moe_instance* instances, int32_t n_instances, int64_t n_rows, int32_t n_experts,
+                                    int64_t in_features, int64_t out_features, const etp_tensor* w, void* y_perm, void* stream);
+/* gate | up of a SwiGLU expert layer in ONE launch (reading G5): h_perm[r][:] = silu(W_gate,e x_perm[r]) * (W_up,e x_perm[r]),
+ * fp32 accumulation, the activation in fp32, ONE rounding to 16 bit; X is read once and the two [rows][ffn] intermediates of
+ * the separate launches never exist.  Both tensors column-parallel [ffn][in] per expert, slabs of the same geometry rank by
+ * rank.  Either instances != NULL (as etp_moe_linear_instances; row_offsets / layout ignored) or row_offsets + layout (as
+ * etp_moe_linear; n_rows ignored). */
+etp_status etp_moe_gate_up(etp_ctx* ctx, etp_dtype dtype, const void* x_perm, const int64_t* row_offsets,
+                           const etp_moe_instance* instances, int32_t n_instances, int64_t n_rows, int32_t n_experts,
+                           int64_t in_features, int64_t ffn, const etp_tensor* w_gate, const etp_tensor* w_up,
+                           const etp_shard* layout, int32_t n_shards, void* h_perm, void* stream);
 
 /* ------------------------------------------------------------------------------------------------ EPLB-style placement
  * PAPER.md:172-174, Fig. 4, :235, :249 - "replicating hot-spot experts and adjusting routing"; after an unequal-width reshard
@@ -350,6 +369,14 @@ typedef struct { int32_t expert, rank; } etp_replica;
 etp_status etp_eplb_place(const int64_t* expert_load, const int32_t* home_rank, int32_t n_experts,
                           const int64_t* rank_capacity, const int32_t* spare_slots, int32_t n_ranks,
                           etp_replica* replicas_out, int32_t cap, int32_t* n_replicas);
+
+/* Materialises replicas: for every replica (expert e -> rank d) the lowest spare slot of rank d's slab (a slot that holds no
+ * unit of d's shard under `layout` and was not given to an earlier replica of this call) receives a copy of e's unit from its
+ * home rank, in EVERY tensor of the class (e.g. gate, up, down of a layer; all must share total_units and, rank by rank, the
+ * slab geometry, so a replica has ONE slot).  One launch of the interval-copy kernel on `stream`; slots_out[i] (host) = the
+ * slot of replica i.  ETP_ERR_CAPACITY if a rank has no spare slot. */
+etp_status etp_eplb_apply(etp_ctx* ctx, const etp_tensor* tensors, int32_t n_tensors, const etp_shard* layout, int32_t n_shards,
+                          const etp_replica* replicas, int32_t n_replicas, int64_t* slots_out, void* stream);
 
 /* ------------------------------------------------------------------------------------------------ microbenchmark entry
  * Copies n arbitrary intervals with the same persistent kernel (config 5b).  host_descs: host array; src/dst: device,

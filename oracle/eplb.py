@@ -102,3 +102,20 @@ def place(load: Sequence[int], home: Sequence[int], capacity: Sequence[int], slo
 def split_rows(n_rows: int, k: int) -> List[Tuple[int, int]]:
     """Rows of one expert's block over its k instances (even routing): instance j gets [floor(j n / k), floor((j+1) n / k))."""
     return [((j * n_rows) // k, ((j + 1) * n_rows) // k) for j in range(k)]
+
+
+def replica_slots(shards: Sequence[Tuple[int, int, int, int]], geom: Dict[int, Tuple[int, int]], replicas: Sequence[Tuple[int, int]]) -> List[int]:
+    """Where a replica lives (reading E1, memory side): rank d keeps unit u of its shard at slot (u - anchor) mod cap (reading
+    L3); a replica takes the LOWEST slot of d's slab that holds no unit of d's current shard and no earlier replica.
+    shards: [(rank, begin, end, alive)] of the expert class; geom[rank] = (anchor, cap)."""
+    taken = {r: set() for r in geom}
+    for (r, b, e, alive) in shards:
+        if alive:
+            for u in range(b, e):
+                taken[r].add((u - geom[r][0]) % geom[r][1])
+    out = []
+    for (e, d) in replicas:
+        s = next(s for s in range(geom[d][1]) if s not in taken[d])
+        taken[d].add(s)
+        out.append(s)
+    return out

@@ -71,6 +71,16 @@ def silu(v: np.ndarray) -> np.ndarray:
     return v / (1.0 + np.exp(-v))
 
 
+def swiglu_ref(x: np.ndarray, gate_e: np.ndarray, up_e: np.ndarray) -> np.ndarray:
+    """The intermediate of one expert, row by row: h[r] = silu(gate_e x[r]) * (up_e x[r]) in fp64 (x [R][hidden]; gate_e, up_e
+    [ffn][hidden]).  It is the inner term of moe_ref written for a block of rows; pins the fused gate|up kernel."""
+    x = np.asarray(x, dtype=np.float64)
+    out = np.zeros((x.shape[0], gate_e.shape[0]), dtype=np.float64)
+    for r in range(x.shape[0]):
+        out[r] = silu(np.asarray(gate_e, dtype=np.float64) @ x[r]) * (np.asarray(up_e, dtype=np.float64) @ x[r])
+    return out
+
+
 def moe_ref(x: np.ndarray, logits: np.ndarray, gate: np.ndarray, up: np.ndarray, down_t: np.ndarray, top_k: int) -> np.ndarray:
     """x [T][hidden]; gate, up [E][ffn][hidden]; down_t [E][ffn][hidden] (row-parallel weights are stored transposed,
     reading L1: down_e(h) = h @ down_t[e]); gate / up / down_t may be arrays or mappings expert -> matrix (only the routed

@@ -84,6 +84,10 @@ class etp_linear_plan_stats(C.Structure):
                 ("n_split_tiles", i64), ("n_splits", i32 * 8)]
 
 
+class etp_moe_instance(C.Structure):
+    _fields_ = [("expert", i32), ("rank", i32), ("slot", i64), ("row_begin", i64), ("row_end", i64)]
+
+
 class etp_replica(C.Structure):
     _fields_ = [("expert", i32), ("rank", i32)]
 
@@ -96,7 +100,7 @@ EXPORTS = ["etp_ctx_create", "etp_ctx_create_multi", "etp_ctx_set_rank_devices",
            "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_create_weighted", "etp_plan_tasks", "etp_plan_new_layout",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
            "etp_shard_linear_multi", "etp_linear_prepare", "etp_linear_run", "etp_linear_plan_info", "etp_linear_free",
-           "etp_moe_linear", "etp_eplb_place", "etp_copy_intervals"]
+           "etp_moe_linear", "etp_moe_linear_instances", "etp_moe_gate_up", "etp_eplb_place", "etp_eplb_apply", "etp_copy_intervals"]
 
 _lib = None
 
@@ -143,6 +147,11 @@ def lib() -> C.CDLL:
         L.etp_linear_free.restype = None
         L.etp_moe_linear.argtypes = [vp, C.c_int, C.c_int, vp, C.POINTER(i64), i32, i64, i64, C.POINTER(etp_tensor), C.POINTER(etp_shard),
                                      i32, vp, vp]
+        L.etp_moe_linear_instances.argtypes = [vp, C.c_int, C.c_int, vp, C.POINTER(etp_moe_instance), i32, i64, i32, i64, i64,
+                                               C.POINTER(etp_tensor), vp, vp]
+        L.etp_moe_gate_up.argtypes = [vp, C.c_int, vp, C.POINTER(i64), C.POINTER(etp_moe_instance), i32, i64, i32, i64, i64,
+                                      C.POINTER(etp_tensor), C.POINTER(etp_tensor), C.POINTER(etp_shard), i32, vp, vp]
+        L.etp_eplb_apply.argtypes = [vp, C.POINTER(etp_tensor), i32, C.POINTER(etp_shard), i32, C.POINTER(etp_replica), i32, C.POINTER(i64), vp]
         L.etp_eplb_place.argtypes = [C.POINTER(i64), C.POINTER(i32), i32, C.POINTER(i64), C.POINTER(i32), i32, C.POINTER(etp_replica), i32,
                                      C.POINTER(i32)]
         L.etp_copy_intervals.argtypes = [vp, C.POINTER(etp_interval), i64, vp, C.POINTER(etp_reshard_report)]
@@ -473,6 +482,50 @@ def etp_moe_linear(ctx: Context, mode: int, dtype: str, x_ptr: int, row_offsets:
     _check(lib().etp_moe_linear(ctx.handle, mode, DTYPE[dtype], x_ptr, offs, n, in_features, out_features, arr, _shards(layout),
                                 len(layout), y_ptr, stream or None))
     del keep
+
+
+def _instances(instances):
+    """[(expert, rank, slot, row_begin, row_end)] -> ctypes array"""
+    arr = (etp_moe_instance * max(len(instances), 1))()
+    for i, (e, r, s, b, en) in enumerate(instances):
+        arr[i] = etp_moe_instance(int(e), int(r), int(s), int(b), int(en))
+    return arr
+
+
+def etp_moe_linear_instances(ctx: Context, mode: int, dtype: str, x_ptr: int, instances, n_rows: int, n_experts: int, in_features: int,
+                             out_features: int, w: TensorDesc, y_ptr: int, stream: int = 0) -> None:
+    arr, keep = _marshal_tensors([w])
+    _check(lib().etp_moe_linear_instances(ctx.handle, mode, DTYPE[dtype], x_ptr, _instances(instances), len(instances), n_rows, n_experts,
+                                          in_features, out_features, arr, y_ptr, stream or None))
+    del keep
+
+
+def etp_moe_gate_up(ctx: Context, dtype: str, x_ptr: int, in_features: int, ffn: int, w_gate: TensorDesc, w_up: TensorDesc, h_ptr: int,
+                    row_offsets: Optional[Sequence[int]] = None, layout: Optional[Sequence[Shard]] = None, instances=None,
+                    n_rows: int = 0, stream: int = 0) -> None:
+    """Fused gate | up + SwiGLU.  Either (row_offsets, layout) or (instances, n_rows)."""
+    ag, kg = _marshal_tensors([w_gate])
+    au, ku = _marshal_tensors([w_up])
+    n_experts = w_gate.total_units
+    if instances is not None:
+        _check(lib().etp_moe_gate_up(ctx.handle, DTYPE[dtype], x_ptr, None, _instances(instances), len(instances), n_rows, n_experts,
+                                     in_features, ffn, ag, au, None, 0, h_ptr, stream or None))
+    else:
+        offs = (i64 * len(row_offsets))(*[int(v) for v in row_offsets])
+        _check(lib().etp_moe_gate_up(ctx.handle, DTYPE[dtype], x_ptr, offs, None, 0, 0, n_experts, in_features, ffn, ag, au,
+                                     _shards(layout), len(layout), h_ptr, stream or None))
+    del kg, ku
+
+
+def etp_eplb_apply(ctx: Context, tensors: Sequence[TensorDesc], layout: Sequence[Shard], replicas: Sequence[Tuple[int, int]],
+                   stream: int = 0) -> List[int]:
+    """Copies every replica's expert into the lowest spare slot of its rank, in every tensor; returns the slots."""
+    arr, keep = _marshal_tensors(tensors)
+    reps = (etp_replica * max(len(replicas), 1))(*[etp_replica(int(e), int(r)) for (e, r) in replicas])
+    slots = (i64 * max(len(replicas), 1))()
+    _check(lib().etp_eplb_apply(ctx.handle, arr, len(tensors), _shards(layout), len(layout), reps, len(replicas), slots, stream or None))
+    del keep
+    return [int(s) for s in slots[: len(replicas)]]
 
 
 class PreparedLinear:

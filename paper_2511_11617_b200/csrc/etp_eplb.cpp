@@ -19,7 +19,6 @@ struct Frac {   // S / c with c > 0
     int64_t s, c;
 };
 inline bool less(const Frac& a, const Frac& b) { return (i128)a.s * b.c < (i128)b.s * a.c; }
-inline bool equal(const Frac& a, const Frac& b) { return (i128)a.s * b.c == (i128)b.s * a.c; }
 
 struct State {
     int32_t E, R;

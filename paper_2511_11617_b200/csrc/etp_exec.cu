@@ -189,7 +189,6 @@ extern "C" void etp_ctx_destroy(etp_ctx* c) {
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
     etp::lin_teardown(c);
-    if (c->moe_items) cudaFree(c->moe_items);
     cudaGetLastError();
     delete x;
     delete c;

@@ -122,8 +122,6 @@ struct etp_ctx {
     void* impl = nullptr;               // executor state (per logical device: streams, descriptor arenas, events), etp_exec.cu
     int32_t launches = 0;               // kernels launched by the last call
     void* lin_state = nullptr;          // kernel (c): per-stream split-K workspaces + the cache of prepared groups (etp_linear_group.cu)
-    void* moe_items = nullptr;          // work-item table of etp_moe_linear (device), grown on demand
-    int64_t moe_items_bytes = 0;
 };
 
 namespace etp {

@@ -1,13 +1,18 @@
-// Grouped shard linear for MoE experts (reading G5): one launch computes, for every expert e
-// with routed rows,  Y_perm[rows of e][out] = X_perm[rows of e][in] . W_e^T  on the expert matrices exactly where the
-// expert-granularity reshard left them (the expert is the unit of the plan; slot-addressed slabs, L3).
+// Grouped shard linear for MoE experts (readings G5, E1): one launch computes, for every expert
+// INSTANCE with routed rows,  Y_perm[rows][out] = X_perm[rows][in] . W_e^T  on the expert matrices exactly where the
+// expert-granularity reshard (the expert is the unit of the plan; slot-addressed slabs, L3) or the EPLB-style
+// replication (Fig. 4) left them.
 //   ETP_COL_PARALLEL  W_e stored [out][in]  (gate, up):   A = K-major rows of W_e
 //   ETP_ROW_PARALLEL  W_e stored [in][out]  (down_t):     A = MN-major, K loop over the expert's own in-features
-// Same tcgen05 / TMEM / TMA pipeline as etp_shard_linear (etp_linear.cu): D[m = out feature][n = routed row] in TMEM,
-// 128 x BN tiles, warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 epilogue, two accumulator stages.  What differs is the
-// work list: the host expands (expert, m tile, row tile) into 32-byte ITEM descriptors (the experts' row counts are ragged),
-// uploaded with the call; a tile may over-read rows of the next expert (X) or of the next expert's matrix (W, column-parallel)
-// - both only feed accumulator rows / columns that the epilogue masks.
+//   FUSED gate | up   (etp_moe_gate_up): both projections of an item share the X tile; two TMEM accumulators per stage;
+//                     the epilogue writes silu(gate x) . (up x) once, in 16 bit - X is read once and the two [rows][ffn]
+//                     intermediates of the three-launch layer never exist.
+// Same tcgen05 / TMEM / TMA pipeline as etp_shard_linear: D[m = out feature][n = routed row] in TMEM, 128 x BN tiles, warp 0
+// TMA producer, warp 1 MMA issuer, warps 2-5 epilogue, two accumulator stages.  The work list is a table of 32-byte ITEM
+// descriptors (instance, m tile, row tile) built on the host per call (the experts' row counts are ragged) and uploaded into a
+// stream-ordered allocation, so calls on different streams of one ctx share nothing.  One tensor map per rank covers the whole
+// slab; a tile may over-read rows of the next slot (W, column-parallel) or of the next expert (X) - both only feed accumulator
+// rows / columns that the epilogue masks.
 #include <algorithm>
 #include <cstring>
 #include <vector>
@@ -20,46 +25,52 @@ using namespace etp::tc;
 namespace {
 
 struct MoeItem {       // 32 bytes
-    int32_t run;       // tensor map of the contiguous slot run that holds the expert
-    int32_t a_row;     // column-parallel: first weight row of the tile inside the run; row-parallel: the expert's first k row
+    int32_t map;       // tensor map of the rank whose slab holds the instance
+    int32_t a_row;     // column-parallel: first weight row of the tile inside the slab; row-parallel: the instance's first k row
     int32_t m0;        // first out feature of the tile (column offset in Y_perm)
     int32_t valid;     // out features of the tile that exist (<= 128)
     int32_t x_row;     // first routed row of the tile in X_perm / Y_perm
-    int32_t n_rows;    // rows of the tile that belong to the expert (<= BN)
+    int32_t n_rows;    // rows of the tile that belong to the instance (<= BN)
     int32_t pad[2];
 };
 static_assert(sizeof(MoeItem) == 32, "MoeItem layout");
 
 struct alignas(64) MoeParams {
     CUtensorMap map_x;
-    CUtensorMap map_w[kMaxRuns];
+    CUtensorMap map_w[kMaxRuns];    // per rank (gate, in the fused kernel)
+    CUtensorMap map_w2[kMaxRuns];   // fused kernel: up
     const MoeItem* items;
     int32_t n_items, mode, dtype, n_chunks;   // n_chunks: K chunks of kBK per item
-    int32_t out_features, n_runs;
+    int32_t out_features, n_maps;
     void* y;
 };
 
-template <int BN>
+template <int BN, bool FUSED>
 struct MoeCfg {
+    static constexpr int kAStage = FUSED ? 2 * kABytes : kABytes;
     static constexpr int kBBytes = BN * kBK * 2;
-    static constexpr int kStageBytes = kABytes + kBBytes;
+    static constexpr int kStageBytes = kAStage + kBBytes;
     static constexpr int kStages = (kSmemBudget / kStageBytes) > 12 ? 12 : (kSmemBudget / kStageBytes);
-    static constexpr int kTmemCols = (2 * BN) < 32 ? 32 : 2 * BN;
+    static constexpr int kAccCols = FUSED ? 2 * BN : BN;                          // TMEM columns of one accumulator stage
+    static constexpr int kTmemCols = (2 * kAccCols) < 32 ? 32 : 2 * kAccCols;      // two stages; a power of two >= 32
     static constexpr int kSmemBytes = kStages * kStageBytes + 1024 + 256 + 4096;   // + per-warp epilogue transpose buffers
+    static_assert(kTmemCols <= 512, "TMEM has 512 columns");
 };
 
 __device__ __forceinline__ MoeItem load_item(const MoeItem* items, int i) {
     const int4 a = __ldg(reinterpret_cast<const int4*>(items + i));
     const int4 b = __ldg(reinterpret_cast<const int4*>(items + i) + 1);
     MoeItem it;
-    it.run = a.x; it.a_row = a.y; it.m0 = a.z; it.valid = a.w;
+    it.map = a.x; it.a_row = a.y; it.m0 = a.z; it.valid = a.w;
     it.x_row = b.x; it.n_rows = b.y;
     return it;
 }
 
-template <int BN, typename OutT>
+__device__ __forceinline__ float silu_mul(float g, float u) { return __fdividef(g, 1.f + __expf(-g)) * u; }
+
+template <int BN, typename OutT, bool FUSED>
 __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __grid_constant__ MoeParams p) {
-    using C = MoeCfg<BN>;
+    using C = MoeCfg<BN, FUSED>;
     constexpr int kXBox = BN < 64 ? BN : 64;   // rows per TMA box of the X tile
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -70,11 +81,14 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const bool row_par = p.mode == ETP_ROW_PARALLEL;
+    const bool row_par = !FUSED && p.mode == ETP_ROW_PARALLEL;
 
     if (warp == 0 && lane == 1) {
         prefetch_tensormap(&p.map_x);
-        for (int r = 0; r < p.n_runs; ++r) prefetch_tensormap(&p.map_w[r]);
+        for (int r = 0; r < p.n_maps; ++r) {
+            prefetch_tensormap(&p.map_w[r]);
+            if (FUSED) prefetch_tensormap(&p.map_w2[r]);
+        }
     }
     if (threadIdx.x == 0) {
         for (int s = 0; s < C::kStages; ++s) {
@@ -106,14 +120,15 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
                 const int nb = (it.n_rows + kXBox - 1) / kXBox;
                 for (int c = 0; c < p.n_chunks; ++c) {
                     uint8_t* sa = smem + stage * C::kStageBytes;
-                    uint8_t* sb = sa + kABytes;
+                    uint8_t* sb = sa + C::kAStage;
                     mbar_wait(&empty_bar[stage], phase ^ 1);
-                    mbar_expect_tx(&full_bar[stage], uint32_t(kABytes + nb * kXBox * kBK * 2));
+                    mbar_expect_tx(&full_bar[stage], uint32_t(C::kAStage + nb * kXBox * kBK * 2));
                     if (!row_par) {
-                        tma_load_2d(sa, &p.map_w[it.run], &full_bar[stage], c * kBK, it.a_row);
+                        tma_load_2d(sa, &p.map_w[it.map], &full_bar[stage], c * kBK, it.a_row);
+                        if (FUSED) tma_load_2d(sa + kABytes, &p.map_w2[it.map], &full_bar[stage], c * kBK, it.a_row);
                     } else {
-                        tma_load_2d(sa, &p.map_w[it.run], &full_bar[stage], it.m0, it.a_row + c * kBK);
-                        tma_load_2d(sa + kABytes / 2, &p.map_w[it.run], &full_bar[stage], it.m0 + 64, it.a_row + c * kBK);
+                        tma_load_2d(sa, &p.map_w[it.map], &full_bar[stage], it.m0, it.a_row + c * kBK);
+                        tma_load_2d(sa + kABytes / 2, &p.map_w[it.map], &full_bar[stage], it.m0 + 64, it.a_row + c * kBK);
                     }
                     for (int b = 0; b < nb; ++b)   // the X tile in 64-row boxes: a ragged last tile only fetches the boxes it has rows in
                         tma_load_2d(sb + b * kXBox * kBK * 2, &p.map_x, &full_bar[stage], c * kBK, it.x_row + b * kXBox);
@@ -137,16 +152,22 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
                 const uint32_t aph = (local >> 1) & 1;
                 mbar_wait(&tmem_empty[as], aph ^ 1);
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + uint32_t(as * BN);
+                const uint32_t d_tmem = tmem_base + uint32_t(as * C::kAccCols);
                 for (int c = 0; c < p.n_chunks; ++c) {
                     uint8_t* sa = smem + stage * C::kStageBytes;
                     mbar_wait(&full_bar[stage], phase);
                     tc_fence_after();
                     const uint64_t a_desc = make_smem_desc(smem_u32(sa), a_lbo, 1024);
-                    const uint64_t b_desc = make_smem_desc(smem_u32(sa + kABytes), 16, 1024);
+                    const uint64_t b_desc = make_smem_desc(smem_u32(sa + C::kAStage), 16, 1024);
 #pragma unroll
                     for (int k = 0; k < kBK / kUmmaK; ++k)
                         tc_mma(d_tmem, a_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > 0 || k > 0) ? 1u : 0u);
+                    if (FUSED) {   // the up projection of the same rows into the second accumulator of the stage
+                        const uint64_t a2_desc = make_smem_desc(smem_u32(sa + kABytes), a_lbo, 1024);
+#pragma unroll
+                        for (int k = 0; k < kBK / kUmmaK; ++k)
+                            tc_mma(d_tmem + uint32_t(BN), a2_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > 0 || k > 0) ? 1u : 0u);
+                    }
                     tc_commit(&empty_bar[stage]);
                     if (++stage == C::kStages) { stage = 0; phase ^= 1; }
                 }
@@ -165,26 +186,34 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
             const uint32_t aph = (local >> 1) & 1;
             mbar_wait(&tmem_full[as], aph);
             tc_fence_after();
-            const uint32_t taddr = tmem_base + uint32_t(as * BN) + (uint32_t(q * 32) << 16);
-            // up to 64 accumulator columns per tcgen05.wait::ld (four loads in flight hide the TMEM read latency); every 16
-            // columns go through a 1-KiB per-warp transpose buffer so that the global stores are 16 bytes per lane (8 routed
-            // rows x 64 contiguous bytes per instruction) instead of 2 - m0 and out_features are multiples of 8 by contract.
-            for (int c64 = 0; c64 < it.n_rows; c64 += 64) {
+            const uint32_t taddr = tmem_base + uint32_t(as * C::kAccCols) + (uint32_t(q * 32) << 16);
+            // up to 64 accumulator columns per tcgen05.wait::ld (four loads in flight hide the TMEM read latency; the fused kernel
+            // reads 32 columns of each of its two accumulators); every 16 columns go through a 1-KiB per-warp transpose buffer so
+            // that the global stores are 16 bytes per lane (8 routed rows x 64 contiguous bytes per instruction) instead of 2 - m0
+            // and out_features are multiples of 8 by contract.
+            constexpr int kStep = FUSED ? 32 : 64;
+            for (int c0 = 0; c0 < it.n_rows; c0 += kStep) {
                 uint32_t v[4][16];
 #pragma unroll
-                for (int g = 0; g < 4; ++g)
-                    if (BN >= 16 * (g + 1) && c64 + 16 * g < it.n_rows) tc_ld16(taddr + uint32_t(c64 + 16 * g), v[g]);
+                for (int g = 0; g < 4; ++g) {
+                    const int col = FUSED ? c0 + 16 * (g & 1) : c0 + 16 * g;   // fused: g = 0, 1 gate columns, g = 2, 3 the same columns of up
+                    if (BN >= 16 * ((FUSED ? (g & 1) : g) + 1) && col < it.n_rows) tc_ld16(taddr + uint32_t(col) + (FUSED && g >= 2 ? uint32_t(BN) : 0u), v[g]);
+                }
                 tc_ld_wait();
 #pragma unroll
-                for (int g = 0; g < 4; ++g) {
-                    if (BN >= 16 * (g + 1) && c64 + 16 * g < it.n_rows) {
+                for (int g = 0; g < (FUSED ? 2 : 4); ++g) {
+                    const int col = c0 + 16 * g;
+                    if (BN >= 16 * (g + 1) && col < it.n_rows) {
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) stage_t[j * 32 + lane] = cvt16<OutT>(__uint_as_float(v[g][j]));
+                        for (int j = 0; j < 16; ++j) {
+                            const float r = FUSED ? silu_mul(__uint_as_float(v[g][j]), __uint_as_float(v[g + 2][j])) : __uint_as_float(v[g][j]);
+                            stage_t[j * 32 + lane] = cvt16<OutT>(r);
+                        }
                         __syncwarp();
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
                             const int row = h * 8 + (lane >> 2), chunk = lane & 3;
-                            const int tok = c64 + 16 * g + row;
+                            const int tok = col + row;
                             const uint4 val = *reinterpret_cast<const uint4*>(stage_t + row * 32 + chunk * 8);
                             if (tok < it.n_rows && q * 32 + chunk * 8 < it.valid)
                                 *reinterpret_cast<uint4*>(y + size_t(it.x_row + tok) * p.out_features + it.m0 + q * 32 + chunk * 8) = val;
@@ -207,20 +236,220 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
     }
 }
 
-template <int BN>
-etp_status launch_moe(const MoeParams& p, int grid, cudaStream_t stream) {
-    using C = MoeCfg<BN>;
-    if (p.dtype == ETP_BF16) {
-        auto k = etp_moe_linear_kernel<BN, __nv_bfloat16>;
+template <int BN, typename OutT, bool FUSED>
+etp_status launch_moe_t(const MoeParams& p, int grid, cudaStream_t stream) {
+    using C = MoeCfg<BN, FUSED>;
+    auto k = etp_moe_linear_kernel<BN, OutT, FUSED>;
+    static bool configured = false;
+    if (!configured) {
         ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes));
-        k<<<grid, kLinThreads, C::kSmemBytes, stream>>>(p);
-    } else {
-        auto k = etp_moe_linear_kernel<BN, __half>;
-        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes));
-        k<<<grid, kLinThreads, C::kSmemBytes, stream>>>(p);
+        configured = true;
     }
+    k<<<grid, kLinThreads, C::kSmemBytes, stream>>>(p);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) ETP_FAIL(ETP_ERR_CUDA, "etp_moe_linear: launch failed: %s", cudaGetErrorString(e));
+    return ETP_OK;
+}
+
+template <bool FUSED>
+etp_status launch_moe(const MoeParams& p, int bn, int grid, cudaStream_t st) {
+    const bool bf = p.dtype == ETP_BF16;
+    if (bn == 16) return bf ? launch_moe_t<16, __nv_bfloat16, FUSED>(p, grid, st) : launch_moe_t<16, __half, FUSED>(p, grid, st);
+    if (bn == 64) return bf ? launch_moe_t<64, __nv_bfloat16, FUSED>(p, grid, st) : launch_moe_t<64, __half, FUSED>(p, grid, st);
+    if (bn == 128) return bf ? launch_moe_t<128, __nv_bfloat16, FUSED>(p, grid, st) : launch_moe_t<128, __half, FUSED>(p, grid, st);
+    if constexpr (FUSED) {   // two accumulators of 256 columns x two stages would exceed the 512 TMEM columns
+        ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_moe_gate_up: no 256-row tile");
+    } else {
+        return bf ? launch_moe_t<256, __nv_bfloat16, false>(p, grid, st) : launch_moe_t<256, __half, false>(p, grid, st);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+struct Inst {   // one expert instance with routed rows
+    int32_t rank;
+    int64_t slot, row_b, row_e;
+};
+
+// Slot of unit u in rank r's slab (L3) if the layout says r holds u, else -1.
+etp_status home_of(const etp_tensor* w, const std::vector<etp_shard>& sh, int64_t u, int32_t* rank, int64_t* slot) {
+    for (const etp_shard& s : sh)
+        if (s.begin <= u && u < s.end) {
+            if (s.rank < 0 || s.rank >= w->n_ranks || !w->slabs[s.rank].base) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: rank %d has no slab", s.rank);
+            const etp_slab& sl = w->slabs[s.rank];
+            if (sl.cap_units <= 0 || s.end - s.begin > sl.cap_units)
+                ETP_FAIL(ETP_ERR_CAPACITY, "etp_moe_linear: shard of rank %d (%lld experts) exceeds its slab (%lld)", s.rank, (long long)(s.end - s.begin), (long long)sl.cap_units);
+            int64_t v = (u - sl.anchor_unit) % sl.cap_units;
+            *slot = v < 0 ? v + sl.cap_units : v;
+            *rank = s.rank;
+            return ETP_OK;
+        }
+    ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: expert %lld is in no shard of the layout", (long long)u);
+}
+
+etp_status sorted_layout(const etp_shard* layout, int32_t n_shards, int64_t n_units, std::vector<etp_shard>* sh) {
+    sh->clear();
+    if (!layout || n_shards <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: empty layout");
+    for (int i = 0; i < n_shards; ++i)
+        if (layout[i].alive && layout[i].end > layout[i].begin) sh->push_back(layout[i]);
+    std::sort(sh->begin(), sh->end(), [](const etp_shard& a, const etp_shard& b) { return a.begin < b.begin; });
+    int64_t cursor = 0;
+    for (const etp_shard& s : *sh) {
+        if (s.begin != cursor) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: layout does not tile [0,%lld): gap or overlap at expert %lld", (long long)n_units, (long long)cursor);
+        cursor = s.end;
+    }
+    if (cursor != n_units) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: layout covers %lld of %lld experts", (long long)cursor, (long long)n_units);
+    return ETP_OK;
+}
+
+// w2 != NULL: fused gate | up (column-parallel, silu(w x) . (w2 x)); its slabs must mirror w's geometry rank by rank.
+etp_status moe_run(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x_perm, int64_t n_rows, const std::vector<Inst>& insts,
+                   int64_t in_features, int64_t out_features, const etp_tensor* w, const etp_tensor* w2, void* y_perm, void* stream) {
+    const bool fused = w2 != nullptr;
+    const bool row_par = mode == ETP_ROW_PARALLEL;
+    const int64_t rows_per_expert = row_par ? in_features : out_features;   // rows of the stored expert matrix
+    const int64_t row_len = row_par ? out_features : in_features;
+    if (n_rows == 0 || insts.empty()) return ETP_OK;
+    if (!x_perm || !y_perm) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: x / y is NULL");
+    if ((reinterpret_cast<uintptr_t>(x_perm) | reinterpret_cast<uintptr_t>(y_perm)) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_moe_linear: x / y not 16-byte aligned");
+
+    MoeParams p;
+    std::memset(&p, 0, sizeof(p));
+    // ---- one tensor map per rank over its whole slab
+    std::vector<int32_t> map_of(size_t(w->n_ranks), -1);
+    int n_maps = 0;
+    for (const Inst& in : insts) {
+        if (in.rank < 0 || in.rank >= w->n_ranks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: instance on rank %d, the tensor has %d slabs", in.rank, w->n_ranks);
+        const etp_slab& sl = w->slabs[in.rank];
+        if (!sl.base) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: rank %d has no slab", in.rank);
+        if (in.slot < 0 || in.slot >= sl.cap_units) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: slot %lld outside the slab of rank %d (%lld slots)", (long long)in.slot, in.rank, (long long)sl.cap_units);
+        if (map_of[in.rank] >= 0) continue;
+        if (reinterpret_cast<uintptr_t>(sl.base) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_moe_linear: slab of rank %d not 16-byte aligned", in.rank);
+        if (n_maps == kMaxRuns) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_moe_linear: more than %d ranks", kMaxRuns);
+        if (sl.cap_units * rows_per_expert >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: slab too long");
+        const int bc = row_par ? 64 : kBK, br = row_par ? kBK : kBM;
+        ETP_TRY(encode_2d(&p.map_w[n_maps], dtype, sl.base, sl.cap_units * rows_per_expert, row_len, row_len, bc, br));
+        if (fused) {
+            if (in.rank >= w2->n_ranks || !w2->slabs[in.rank].base || w2->slabs[in.rank].cap_units != sl.cap_units || w2->slabs[in.rank].anchor_unit != sl.anchor_unit)
+                ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_gate_up: the slabs of gate and up must have the same geometry (rank %d)", in.rank);
+            if (reinterpret_cast<uintptr_t>(w2->slabs[in.rank].base) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_moe_gate_up: slab of rank %d not 16-byte aligned", in.rank);
+            ETP_TRY(encode_2d(&p.map_w2[n_maps], dtype, w2->slabs[in.rank].base, sl.cap_units * rows_per_expert, row_len, row_len, bc, br));
+        }
+        map_of[in.rank] = n_maps++;
+    }
+
+    // ---- row tile BN: operand fetch into the SM bounds a tile (measured on kernel (c): 48 KiB per K chunk at BN = 256 is the
+    // limit, the MMA is not), so an item costs (A tile(s) + BN rows of X) bytes per K chunk; take the BN with the least total.
+    int bn = 16;
+    {
+        int64_t best = INT64_MAX;
+        const int64_t a_bytes = fused ? 2 * kABytes : kABytes;
+        for (int cand : {256, 128, 64, 16}) {
+            if (fused && cand == 256) continue;
+            int64_t cost = 0;
+            const int box = std::min(cand, 64);
+            for (const Inst& in : insts) {
+                const int64_t c = in.row_e - in.row_b;
+                const int64_t tiles = (c + cand - 1) / cand, boxes = (c + box - 1) / box;   // X is fetched in boxes of <= 64 rows
+                cost += tiles * a_bytes + boxes * box * kBK * 2;
+            }
+            if (cost < best) { best = cost; bn = cand; }
+        }
+    }
+
+    // ---- items: (instance, row tile, m tile), m tiles of one row tile adjacent so that its X tile stays in L2
+    const int64_t m_tiles = (out_features + kBM - 1) / kBM;
+    std::vector<MoeItem> items;
+    for (const Inst& in : insts) {
+        for (int64_t t = in.row_b; t < in.row_e; t += bn)
+            for (int64_t mt = 0; mt < m_tiles; ++mt) {
+                MoeItem it{};
+                it.map = map_of[in.rank];
+                it.m0 = int32_t(mt * kBM);
+                it.valid = int32_t(std::min<int64_t>(kBM, out_features - mt * kBM));
+                it.a_row = int32_t(row_par ? in.slot * rows_per_expert : in.slot * rows_per_expert + mt * kBM);
+                it.x_row = int32_t(t);
+                it.n_rows = int32_t(std::min<int64_t>(bn, in.row_e - t));
+                items.push_back(it);
+            }
+    }
+    if (items.empty()) return ETP_OK;
+    if (items.size() >= (size_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: too many work items");
+
+    ETP_CUDA_OK(cudaSetDevice(ctx->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t need = items.size() * sizeof(MoeItem);
+    void* d_items = nullptr;
+    ETP_CUDA_OK(cudaMallocAsync(&d_items, need, st));   // stream-ordered: nothing is shared between calls or streams
+    cudaError_t e = cudaMemcpyAsync(d_items, items.data(), need, cudaMemcpyHostToDevice, st);   // pageable source: staged before return
+    if (e != cudaSuccess) {
+        cudaFreeAsync(d_items, st);
+        ETP_FAIL(ETP_ERR_CUDA, "etp_moe_linear: uploading the item table failed: %s", cudaGetErrorString(e));
+    }
+    p.items = static_cast<const MoeItem*>(d_items);
+    p.n_items = int32_t(items.size());
+    p.mode = mode;
+    p.dtype = dtype;
+    p.n_chunks = int32_t((in_features + kBK - 1) / kBK);
+    p.out_features = int32_t(out_features);
+    p.n_maps = n_maps;
+    p.y = y_perm;
+    etp_status s = encode_2d(&p.map_x, dtype, x_perm, n_rows, in_features, in_features, kBK, std::min(bn, 64));
+    const int grid = int(std::min<int64_t>(p.n_items, ctx->n_sms));
+    ctx->launches = 1;
+    if (s == ETP_OK) s = fused ? launch_moe<true>(p, bn, grid, st) : launch_moe<false>(p, bn, grid, st);
+    cudaFreeAsync(d_items, st);
+    return s;
+}
+
+etp_status check_moe_shapes(const char* who, etp_ctx* ctx, int mode, etp_dtype dtype, int32_t n_experts, int64_t in_features,
+                            int64_t out_features, const etp_tensor* w) {
+    if (!ctx || !w || !w->slabs) ETP_FAIL(ETP_ERR_INVALID_ARG, "%s: NULL argument", who);
+    if (mode != ETP_COL_PARALLEL && mode != ETP_ROW_PARALLEL) ETP_FAIL(ETP_ERR_INVALID_ARG, "%s: bad mode %d", who, mode);
+    if (dtype != ETP_BF16 && dtype != ETP_FP16) ETP_FAIL(ETP_ERR_UNSUPPORTED, "%s: dtype %d is not bf16/fp16", who, int(dtype));
+    if (n_experts <= 0 || in_features <= 0 || out_features <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "%s: non-positive size", who);
+    if (w->total_units != n_experts) ETP_FAIL(ETP_ERR_INVALID_ARG, "%s: the tensor has %lld units, n_experts = %d (one unit = one expert)", who, (long long)w->total_units, n_experts);
+    if (w->unit_bytes != in_features * out_features * 2)
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "%s: unit_bytes %lld != in x out x 2 = %lld", who, (long long)w->unit_bytes, (long long)(in_features * out_features * 2));
+    if ((in_features * 2) % 16 || (out_features * 2) % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "%s: feature counts must be multiples of 8", who);
+    if (mode == ETP_ROW_PARALLEL && in_features % kBK)
+        ETP_FAIL(ETP_ERR_UNSUPPORTED, "%s: row-parallel experts need in_features %% %d == 0 (a K chunk must not run into the next expert)", who, kBK);
+    if (in_features >= (int64_t(1) << 31) || out_features >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "%s: sizes must be below 2^31", who);
+    return ETP_OK;
+}
+
+// rows [row_offsets[e], row_offsets[e+1]) of every expert on the rank / slot where the layout holds it
+etp_status instances_from_layout(const int64_t* row_offsets, int32_t n_experts, const etp_tensor* w, const etp_shard* layout,
+                                 int32_t n_shards, std::vector<Inst>* out, int64_t* n_rows) {
+    if (!row_offsets || !layout) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: NULL argument");
+    if (row_offsets[0] != 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: row_offsets[0] != 0");
+    for (int32_t e = 0; e < n_experts; ++e)
+        if (row_offsets[e + 1] < row_offsets[e]) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: row_offsets decrease at expert %d", e);
+    *n_rows = row_offsets[n_experts];
+    if (*n_rows >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: sizes must be below 2^31");
+    std::vector<etp_shard> sh;
+    ETP_TRY(sorted_layout(layout, n_shards, n_experts, &sh));
+    for (int32_t e = 0; e < n_experts; ++e) {
+        int32_t r;
+        int64_t slot;
+        ETP_TRY(home_of(w, sh, e, &r, &slot));   // also validates every shard's slab, routed rows or not
+        if (row_offsets[e + 1] > row_offsets[e]) out->push_back({r, slot, row_offsets[e], row_offsets[e + 1]});
+    }
+    return ETP_OK;
+}
+
+etp_status instances_from_list(const etp_moe_instance* inst, int32_t n_inst, int64_t n_rows, std::vector<Inst>* out) {
+    if (n_inst < 0 || (n_inst > 0 && !inst) || n_rows < 0 || n_rows >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear_instances: bad arguments");
+    std::vector<std::pair<int64_t, int64_t>> ranges;
+    for (int32_t i = 0; i < n_inst; ++i) {
+        if (inst[i].row_begin < 0 || inst[i].row_end < inst[i].row_begin || inst[i].row_end > n_rows)
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear_instances: instance %d has rows [%lld,%lld) outside [0,%lld)", i, (long long)inst[i].row_begin, (long long)inst[i].row_end, (long long)n_rows);
+        if (inst[i].row_end == inst[i].row_begin) continue;
+        out->push_back({inst[i].rank, inst[i].slot, inst[i].row_begin, inst[i].row_end});
+        ranges.push_back({inst[i].row_begin, inst[i].row_end});
+    }
+    std::sort(ranges.begin(), ranges.end());
+    for (size_t k = 1; k < ranges.size(); ++k)
+        if (ranges[k].first < ranges[k - 1].second) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear_instances: two instances share row %lld", (long long)ranges[k].first);
     return ETP_OK;
 }
 
@@ -229,137 +458,95 @@ etp_status launch_moe(const MoeParams& p, int grid, cudaStream_t stream) {
 extern "C" etp_status etp_moe_linear(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x_perm,
                                      const int64_t* row_offsets, int32_t n_experts, int64_t in_features, int64_t out_features,
                                      const etp_tensor* w, const etp_shard* layout, int32_t n_shards, void* y_perm, void* stream) {
-    if (!ctx || !w || !layout || !w->slabs || !row_offsets) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: NULL argument");
-    if (mode != ETP_COL_PARALLEL && mode != ETP_ROW_PARALLEL) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: bad mode %d", int(mode));
-    if (dtype != ETP_BF16 && dtype != ETP_FP16) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_moe_linear: dtype %d is not bf16/fp16", int(dtype));
-    if (n_experts <= 0 || in_features <= 0 || out_features <= 0 || n_shards <= 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: non-positive size");
-    if (w->total_units != n_experts) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: the tensor has %lld units, n_experts = %d (one unit = one expert)", (long long)w->total_units, n_experts);
-    if (w->unit_bytes != in_features * out_features * 2)
-        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: unit_bytes %lld != in x out x 2 = %lld", (long long)w->unit_bytes, (long long)(in_features * out_features * 2));
-    const bool row_par = mode == ETP_ROW_PARALLEL;
-    const int64_t rows_per_expert = row_par ? in_features : out_features;   // rows of the stored expert matrix
-    const int64_t row_len = row_par ? out_features : in_features;
-    if ((in_features * 2) % 16 || (out_features * 2) % 16) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_moe_linear: feature counts must be multiples of 8");
-    if (row_par && in_features % kBK)
-        ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_moe_linear: row-parallel experts need in_features %% %d == 0 (a K chunk must not run into the next expert)", kBK);
-    if (row_offsets[0] != 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: row_offsets[0] != 0");
-    int64_t max_rows = 0;
-    for (int32_t e = 0; e < n_experts; ++e) {
-        if (row_offsets[e + 1] < row_offsets[e]) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: row_offsets decrease at expert %d", e);
-        max_rows = std::max(max_rows, row_offsets[e + 1] - row_offsets[e]);
-    }
-    const int64_t n_rows = row_offsets[n_experts];
-    if (n_rows >= (int64_t(1) << 31) || in_features >= (int64_t(1) << 31) || out_features >= (int64_t(1) << 31))
-        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: sizes must be below 2^31");
-    if (n_rows == 0) return ETP_OK;
-    if (!x_perm || !y_perm) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: x / y is NULL");
-    if ((reinterpret_cast<uintptr_t>(x_perm) | reinterpret_cast<uintptr_t>(y_perm)) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_moe_linear: x / y not 16-byte aligned");
+    ETP_TRY(check_moe_shapes("etp_moe_linear", ctx, mode, dtype, n_experts, in_features, out_features, w));
+    std::vector<Inst> insts;
+    int64_t n_rows = 0;
+    ETP_TRY(instances_from_layout(row_offsets, n_experts, w, layout, n_shards, &insts, &n_rows));
+    return moe_run(ctx, mode, dtype, x_perm, n_rows, insts, in_features, out_features, w, nullptr, y_perm, stream);
+}
 
-    // ---- shards must tile [0, n_experts); every shard is <= 2 contiguous slot runs of its slab (L3)
+extern "C" etp_status etp_moe_linear_instances(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const void* x_perm,
+                                               const etp_moe_instance* instances, int32_t n_instances, int64_t n_rows,
+                                               int32_t n_experts, int64_t in_features, int64_t out_features, const etp_tensor* w,
+                                               void* y_perm, void* stream) {
+    ETP_TRY(check_moe_shapes("etp_moe_linear_instances", ctx, mode, dtype, n_experts, in_features, out_features, w));
+    std::vector<Inst> insts;
+    ETP_TRY(instances_from_list(instances, n_instances, n_rows, &insts));
+    return moe_run(ctx, mode, dtype, x_perm, n_rows, insts, in_features, out_features, w, nullptr, y_perm, stream);
+}
+
+extern "C" etp_status etp_moe_gate_up(etp_ctx* ctx, etp_dtype dtype, const void* x_perm, const int64_t* row_offsets,
+                                      const etp_moe_instance* instances, int32_t n_instances, int64_t n_rows, int32_t n_experts,
+                                      int64_t in_features, int64_t ffn, const etp_tensor* w_gate, const etp_tensor* w_up,
+                                      const etp_shard* layout, int32_t n_shards, void* h_perm, void* stream) {
+    ETP_TRY(check_moe_shapes("etp_moe_gate_up", ctx, ETP_COL_PARALLEL, dtype, n_experts, in_features, ffn, w_gate));
+    ETP_TRY(check_moe_shapes("etp_moe_gate_up", ctx, ETP_COL_PARALLEL, dtype, n_experts, in_features, ffn, w_up));
+    if (w_gate->n_ranks != w_up->n_ranks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_gate_up: gate and up have different rank counts");
+    std::vector<Inst> insts;
+    if (instances) {
+        ETP_TRY(instances_from_list(instances, n_instances, n_rows, &insts));
+    } else {
+        ETP_TRY(instances_from_layout(row_offsets, n_experts, w_gate, layout, n_shards, &insts, &n_rows));
+    }
+    return moe_run(ctx, ETP_COL_PARALLEL, dtype, x_perm, n_rows, insts, in_features, ffn, w_gate, w_up, h_perm, stream);
+}
+
+// ------------------------------------------------------------------------------------------------ EPLB: materialise replicas
+extern "C" etp_status etp_eplb_apply(etp_ctx* ctx, const etp_tensor* tensors, int32_t n_tensors, const etp_shard* layout,
+                                     int32_t n_shards, const etp_replica* replicas, int32_t n_replicas, int64_t* slots_out,
+                                     void* stream) {
+    if (!ctx || !tensors || n_tensors < 1 || !layout || n_replicas < 0 || (n_replicas > 0 && (!replicas || !slots_out)))
+        ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_eplb_apply: bad arguments");
+    const etp_tensor& T0 = tensors[0];
     std::vector<etp_shard> sh;
-    for (int i = 0; i < n_shards; ++i)
-        if (layout[i].alive && layout[i].end > layout[i].begin) sh.push_back(layout[i]);
-    std::sort(sh.begin(), sh.end(), [](const etp_shard& a, const etp_shard& b) { return a.begin < b.begin; });
-    int64_t cursor = 0;
-    for (const etp_shard& s : sh) {
-        if (s.begin != cursor) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: layout does not tile [0,%d): gap or overlap at expert %lld", n_experts, (long long)cursor);
-        cursor = s.end;
+    ETP_TRY(sorted_layout(layout, n_shards, T0.total_units, &sh));
+    for (int32_t t = 0; t < n_tensors; ++t) {
+        const etp_tensor& T = tensors[t];
+        if (!T.slabs || T.n_ranks != T0.n_ranks || T.total_units != T0.total_units || T.unit_bytes <= 0 || T.unit_bytes % 16)
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_eplb_apply: tensor %d does not belong to the class of tensor 0 (or unit_bytes not a multiple of 16)", t);
+        for (int32_t r = 0; r < T.n_ranks; ++r)
+            if ((T.slabs[r].base != nullptr) != (T0.slabs[r].base != nullptr) ||
+                (T.slabs[r].base && (T.slabs[r].cap_units != T0.slabs[r].cap_units || T.slabs[r].anchor_unit != T0.slabs[r].anchor_unit)))
+                ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_eplb_apply: tensor %d, rank %d: slab geometry differs from tensor 0 (a replica takes the same slot in every tensor)", t, r);
     }
-    if (cursor != n_experts) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: layout covers %lld of %d experts", (long long)cursor, n_experts);
-
-    MoeParams p;
-    std::memset(&p, 0, sizeof(p));
-    struct RunInfo { int64_t first_expert, n, slot0; const char* base; };
-    std::vector<RunInfo> runs;
-    for (const etp_shard& s : sh) {
-        if (s.rank < 0 || s.rank >= w->n_ranks) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: rank %d outside the tensor's %d slabs", s.rank, w->n_ranks);
-        const etp_slab& sl = w->slabs[s.rank];
-        if (!sl.base) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: rank %d has no slab", s.rank);
-        if (reinterpret_cast<uintptr_t>(sl.base) & 15) ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_moe_linear: slab of rank %d not 16-byte aligned", s.rank);
-        const int64_t width = s.end - s.begin;
-        if (sl.cap_units <= 0 || width > sl.cap_units) ETP_FAIL(ETP_ERR_CAPACITY, "etp_moe_linear: shard of rank %d (%lld experts) exceeds its slab (%lld)", s.rank, (long long)width, (long long)sl.cap_units);
-        int64_t slot0 = (s.begin - sl.anchor_unit) % sl.cap_units;
-        if (slot0 < 0) slot0 += sl.cap_units;
-        const int64_t len1 = std::min(width, sl.cap_units - slot0);
-        runs.push_back({s.begin, len1, slot0, static_cast<const char*>(sl.base)});
-        if (width > len1) runs.push_back({s.begin + len1, width - len1, 0, static_cast<const char*>(sl.base)});
-    }
-    if ((int)runs.size() > kMaxRuns) ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_moe_linear: more than %d contiguous runs", kMaxRuns);
-    for (const RunInfo& r : runs)
-        if (r.n * rows_per_expert >= (int64_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: run too long");
-
-    // ---- row tile BN: operand fetch into the SM bounds a tile (measured on kernel (c): 48 KiB per K chunk at BN = 256 is the
-    // limit, the MMA is not), so an item costs (A tile + BN rows of X) bytes per K chunk; take the BN with the least total.
-    int bn = 16;
-    {
-        int64_t best = INT64_MAX;
-        for (int cand : {256, 128, 64, 16}) {
-            int64_t cost = 0;
-            const int box = std::min(cand, 64);
-            for (int32_t e = 0; e < n_experts; ++e) {
-                const int64_t c = row_offsets[e + 1] - row_offsets[e];
-                const int64_t tiles = (c + cand - 1) / cand, boxes = (c + box - 1) / box;   // X is fetched in boxes of <= 64 rows
-                cost += tiles * kABytes + boxes * box * kBK * 2;
-            }
-            if (cost < best) { best = cost; bn = cand; }
+    // free slots of every rank: not holding a unit of its current shard, not given to an earlier replica; lowest slot first
+    std::vector<std::vector<char>> taken((size_t)T0.n_ranks);
+    for (int32_t r = 0; r < T0.n_ranks; ++r)
+        if (T0.slabs[r].base && T0.slabs[r].cap_units > 0) taken[r].assign((size_t)T0.slabs[r].cap_units, 0);
+    for (const etp_shard& s : sh)
+        for (int64_t u = s.begin; u < s.end; ++u) {
+            int32_t r;
+            int64_t slot;
+            ETP_TRY(home_of(&T0, sh, u, &r, &slot));
+            taken[r][(size_t)slot] = 1;
+        }
+    LoweredWork w;
+    w.dev.resize((size_t)n_logical_devices(ctx));
+    for (int32_t i = 0; i < n_replicas; ++i) {
+        const int32_t e = replicas[i].expert, d = replicas[i].rank;
+        if (e < 0 || e >= T0.total_units || d < 0 || d >= T0.n_ranks || taken[d].empty())
+            ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_eplb_apply: replica %d: expert %d / rank %d out of range", i, e, d);
+        int32_t hr;
+        int64_t hslot;
+        ETP_TRY(home_of(&T0, sh, e, &hr, &hslot));
+        if (hr == d) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_eplb_apply: replica %d: rank %d already holds expert %d", i, d, e);
+        int64_t slot = -1;
+        for (size_t s = 0; s < taken[d].size(); ++s)
+            if (!taken[d][s]) { slot = (int64_t)s; break; }
+        if (slot < 0) ETP_FAIL(ETP_ERR_CAPACITY, "etp_eplb_apply: replica %d: rank %d has no spare slot", i, d);
+        taken[d][(size_t)slot] = 1;
+        slots_out[i] = slot;
+        const int dv = device_of_rank(ctx, d);
+        if (dv < 0) continue;   // another process materialises it
+        DeviceWork& W = w.dev[(size_t)dv];
+        if (W.phases.empty()) W.phases.resize(1);
+        for (int32_t t = 0; t < n_tensors; ++t) {
+            const etp_tensor& T = tensors[t];
+            push_contiguous(ctx, &W.phases[0], (const char*)T.slabs[hr].base + hslot * T.unit_bytes, (char*)T.slabs[d].base + slot * T.unit_bytes, T.unit_bytes);
+            w.rep.d2d_bytes += T.unit_bytes;
+            W.rep.d2d_bytes += T.unit_bytes;
         }
     }
-
-    // ---- items: (expert, m tile, row tile), m tiles of one expert adjacent so that its X tile stays in L2
-    const int64_t m_extent = out_features;
-    const int64_t m_tiles = (m_extent + kBM - 1) / kBM;
-    std::vector<MoeItem> items;
-    for (size_t ri = 0; ri < runs.size(); ++ri) {
-        const RunInfo& r = runs[ri];
-        for (int64_t k = 0; k < r.n; ++k) {
-            const int64_t e = r.first_expert + k;
-            const int64_t cnt = row_offsets[e + 1] - row_offsets[e];
-            for (int64_t t = 0; t < cnt; t += bn)
-                for (int64_t mt = 0; mt < m_tiles; ++mt) {
-                    MoeItem it{};
-                    it.run = int32_t(ri);
-                    it.m0 = int32_t(mt * kBM);
-                    it.valid = int32_t(std::min<int64_t>(kBM, m_extent - mt * kBM));
-                    it.a_row = int32_t(row_par ? k * rows_per_expert : k * rows_per_expert + mt * kBM);
-                    it.x_row = int32_t(row_offsets[e] + t);
-                    it.n_rows = int32_t(std::min<int64_t>(bn, cnt - t));
-                    items.push_back(it);
-                }
-        }
-    }
-    if (items.size() >= (size_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: too many work items");
-
-    ETP_CUDA_OK(cudaSetDevice(ctx->device));
-    const int64_t need = int64_t(items.size()) * int64_t(sizeof(MoeItem));
-    if (need > ctx->moe_items_bytes) {   // ctx-owned, grown on demand (calls on one ctx must not overlap in time)
-        if (ctx->moe_items) ETP_CUDA_OK(cudaFree(ctx->moe_items));
-        ctx->moe_items = nullptr;
-        ctx->moe_items_bytes = 0;
-        const int64_t want = std::max<int64_t>(need + need / 2, 1 << 16);
-        ETP_CUDA_OK(cudaMalloc(&ctx->moe_items, size_t(want)));
-        ctx->moe_items_bytes = want;
-    }
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    ETP_CUDA_OK(cudaMemcpyAsync(ctx->moe_items, items.data(), size_t(need), cudaMemcpyHostToDevice, st));   // pageable source: staged before return
-
-    p.items = static_cast<const MoeItem*>(ctx->moe_items);
-    p.n_items = int32_t(items.size());
-    p.mode = mode;
-    p.dtype = dtype;
-    p.n_chunks = int32_t((in_features + kBK - 1) / kBK);
-    p.out_features = int32_t(out_features);
-    p.n_runs = int32_t(runs.size());
-    p.y = y_perm;
-    ETP_TRY(encode_2d(&p.map_x, dtype, x_perm, n_rows, in_features, in_features, kBK, std::min(bn, 64)));
-    for (size_t ri = 0; ri < runs.size(); ++ri) {
-        const void* base = runs[ri].base + runs[ri].slot0 * w->unit_bytes;
-        if (row_par) ETP_TRY(encode_2d(&p.map_w[ri], dtype, base, runs[ri].n * rows_per_expert, row_len, row_len, 64, kBK));
-        else ETP_TRY(encode_2d(&p.map_w[ri], dtype, base, runs[ri].n * rows_per_expert, row_len, row_len, kBK, kBM));
-    }
-    const int grid = int(std::min<int64_t>(p.n_items, ctx->n_sms));
-    ctx->launches = 1;
-    if (bn == 16) return launch_moe<16>(p, grid, st);
-    if (bn == 64) return launch_moe<64>(p, grid, st);
-    if (bn == 128) return launch_moe<128>(p, grid, st);
-    return launch_moe<256>(p, grid, st);
+    w.rep.n_phases = 1;
+    return execute(ctx, &w, stream, stream, nullptr);
 }

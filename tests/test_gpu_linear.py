@@ -547,3 +547,122 @@ def test_linear_prepare_errors(ctx):
     assert e.value.status == 2
     plan.run([x.ptr], 0, [y.ptr])               # zero tokens: nothing to do
     plan.close()
+
+
+# ------------------------------------------------------------------------------------------------ fused gate|up, EPLB replicas
+def _moe_world(E, F, Hd, widths, slack, seed_i):
+    """gate / up / down_t expert tensors of one layer sharded over len(widths) ranks with `slack` spare slots per rank (NaN-filled):
+    returns (w bytes per kind, TensorDescs per kind, layout, geom, DevBufs per kind)."""
+    dt = torch_dtype("bf16")
+    layout = widths_to_layout(widths)
+    geom = {r: (b, (e - b) + slack) for (r, b, e, _) in layout}
+    ub = F * Hd * 2
+    ws, descs, bufs = {}, {}, {}
+    for i, kind in enumerate(("gate", "up", "down_t")):
+        ws[kind] = as_u8(fill_normal16(SEED, 1200 + 10 * seed_i + i, 0, E * F * Hd, 0.02 if kind != "down_t" else 0.05, dt)).copy()
+        slabs = shard_into_slabs(ws[kind], ub, layout, geom)
+        bufs[kind] = {r: DevBuf(a) for r, a in slabs.items()}
+        descs[kind] = etp.TensorDesc(E, ub, {r: (bufs[kind][r].ptr, geom[r][1], geom[r][0]) for r in bufs[kind]}, len(widths), 0)
+    return ws, descs, layout, geom, bufs
+
+
+@pytest.mark.parametrize("rows_per_expert,E,F,Hd,widths", [
+    ((0, 3, 17, 0, 1, 40), 6, 128, 256, (2, 2, 2)),           # 16-row tiles, experts without rows
+    ((130, 64, 257, 5), 4, 192, 320, (1, 3)),                 # F not a multiple of 128: tiles run into the next slot; 128-row tiles
+    ((300, 900), 2, 256, 136, (2,)),                          # several row tiles per expert; K tail
+])
+def test_moe_gate_up_fused_matches_fp64_swiglu(ctx, rows_per_expert, E, F, Hd, widths):
+    """etp_moe_gate_up: h = silu(gate x) * (up x) in one launch (two TMEM accumulators, activation in the epilogue), every row
+    against oracle.linear.swiglu_ref in fp64 - fp32 accumulation and ONE 16-bit rounding, so the error is at most one rounding
+    (tighter than the three-launch layer, which rounds gate and up to 16 bit first)."""
+    ws, descs, layout, geom, bufs = _moe_world(E, F, Hd, widths, 1, E)
+    offs = np.concatenate([[0], np.cumsum(rows_per_expert)]).astype(np.int64)
+    R = int(offs[-1])
+    dt = torch_dtype("bf16")
+    x_u8 = as_u8(fill_normal16(SEED, 1300 + E, 0, R * Hd, 1.0, dt)).copy()
+    xb, hb = DevBuf(x_u8), DevBuf(np.full(R * F * 2, 0xEE, dtype=np.uint8))
+    etp.etp_moe_gate_up(ctx, "bf16", xb.ptr, Hd, F, descs["gate"], descs["up"], hb.ptr, row_offsets=offs, layout=layout)
+    torch.cuda.synchronize()
+    assert xb.guards_intact() and hb.guards_intact()
+    x64 = OL.decode16(x_u8, "bf16").reshape(R, Hd)
+    g64, u64 = (OL.decode16(ws[k], "bf16").reshape(E, F, Hd) for k in ("gate", "up"))
+    ref = np.concatenate([OL.swiglu_ref(x64[offs[e]:offs[e + 1]], g64[e], u64[e]) for e in range(E)])
+    check(hb.payload(), ref, "bf16", R, F)
+
+
+def test_moe_layer_with_eplb_replicas_is_bitwise_the_unreplicated_layer(ctx):
+    """Reading E1 end to end: seeded Zipf loads -> etp_eplb_place (== oracle) -> etp_eplb_apply copies the hot experts into
+    spare slots (slot choice == oracle.eplb.replica_slots; the replica's bytes are the expert's, nothing else changes) ->
+    the layer through etp_moe_gate_up + etp_moe_linear_instances with every expert's rows split over its instances.  A row is
+    computed by exactly one instance from identical weights, so the output must be BITWISE the unreplicated layer's, and it
+    matches the oracle's fp64 MoE layer within 5e-3."""
+    from oracle import eplb
+    from tests import moe_util as MU
+    E, F, Hd, top_k, T = 12, 128, 256, 2, 96
+    widths = (4, 4, 4)
+    ws, descs, layout, geom, bufs = _moe_world(E, F, Hd, widths, 2, 77)
+    dt = torch_dtype("bf16")
+    x = fill_normal16(SEED, 1400, 0, T * Hd, 1.0, dt).view(T, Hd).cuda()
+    logits = fill_normal16(SEED, 1401, 0, T * E, 1.0, dt).view(T, E).cuda()
+    logits[:, 1] += 3.0                                            # a hot expert on rank 0, a warm one on rank 2
+    logits[:, 9] += 1.5
+    order, wts = MU.route(logits, top_k)
+    flat_e = order.reshape(-1)
+    perm = torch.argsort(flat_e, stable=True)
+    tok = perm // top_k
+    counts = torch.bincount(flat_e, minlength=E).cpu().numpy()
+    offs = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    R = int(offs[-1])
+    home = [next(r for (r, b, e, _) in layout if b <= ex < e) for ex in range(E)]
+    capacity, spare = [2, 3, 2], [2, 2, 2]                         # rank 1 got the smaller dense shard: more idle compute
+    replicas = etp.etp_eplb_place([int(c) for c in counts], home, capacity, spare)
+    o_rep, o_inst = eplb.place([int(c) for c in counts], home, capacity, spare)
+    assert replicas == o_rep and len(replicas) >= 1
+    before = {k: {r: b.payload().copy() for r, b in bufs[k].items()} for k in bufs}
+    slots = etp.etp_eplb_apply(ctx, [descs["gate"], descs["up"], descs["down_t"]], layout, replicas)
+    torch.cuda.synchronize()
+    assert slots == eplb.replica_slots(layout, geom, replicas)
+    ub = F * Hd * 2
+    for k in bufs:                                                  # the replica slots hold the expert's bytes, everything else is untouched
+        for r, b in bufs[k].items():
+            exp = before[k][r].copy()
+            for (ex, d), s in zip(replicas, slots):
+                if d == r:
+                    exp[s * ub:(s + 1) * ub] = ws[k][ex * ub:(ex + 1) * ub]
+            assert b.guards_intact() and np.array_equal(b.payload(), exp), f"{k} rank {r}"
+    # instances: home first, then replicas in creation order; rows split evenly (oracle.eplb.split_rows)
+    slot_of = {(ex, d): s for (ex, d), s in zip(replicas, slots)}
+    inst = []
+    for ex in range(E):
+        ranks = o_inst[ex]
+        for (b, e), r in zip(eplb.split_rows(int(counts[ex]), len(ranks)), ranks):
+            s = slot_of.get((ex, r), (ex - geom[r][0]) % geom[r][1] if r == home[ex] else None)
+            inst.append((ex, r, s, int(offs[ex]) + b, int(offs[ex]) + e))
+    assert max(len(r) for r in o_inst) >= 2
+    xp = x[tok].contiguous()
+
+    def layer(use_instances):
+        h = torch.full((R, F), float("nan"), dtype=dt, device="cuda")
+        yp = torch.full((R, Hd), float("nan"), dtype=dt, device="cuda")
+        if use_instances:
+            etp.etp_moe_gate_up(ctx, "bf16", xp.data_ptr(), Hd, F, descs["gate"], descs["up"], h.data_ptr(), instances=inst, n_rows=R)
+            etp.etp_moe_linear_instances(ctx, etp.ROW_PARALLEL, "bf16", h.data_ptr(), inst, R, E, F, Hd, descs["down_t"], yp.data_ptr())
+        else:
+            etp.etp_moe_gate_up(ctx, "bf16", xp.data_ptr(), Hd, F, descs["gate"], descs["up"], h.data_ptr(), row_offsets=offs, layout=layout)
+            etp.etp_moe_linear(ctx, etp.ROW_PARALLEL, "bf16", h.data_ptr(), offs, F, Hd, descs["down_t"], layout, yp.data_ptr())
+        torch.cuda.synchronize()
+        return h, yp
+
+    h0, y0 = layer(False)
+    h1, y1 = layer(True)
+    assert torch.equal(h0.view(torch.int16), h1.view(torch.int16)) and torch.equal(y0.view(torch.int16), y1.view(torch.int16))
+    w_flat = wts.reshape(-1)[perm].float()
+    y = torch.zeros(T, Hd, dtype=torch.float32, device="cuda")
+    y.index_add_(0, tok, w_flat[:, None] * y1.float())
+    mats = {k: OL.decode16(ws[k], "bf16").reshape(E, F, Hd) for k in ws}
+    MU.check_against_oracle(y, order.cpu().numpy(), wts.cpu().numpy(), OL.decode16(as_u8(x.cpu()), "bf16").reshape(T, Hd),
+                            OL.decode16(as_u8(logits.cpu()), "bf16").reshape(T, E), mats["gate"], mats["up"], mats["down_t"], top_k)
+    with pytest.raises(etp.EtpError) as e:                          # two instances may not share a row
+        etp.etp_moe_linear_instances(ctx, etp.ROW_PARALLEL, "bf16", h1.data_ptr(), [(0, 0, 0, 0, 5), (1, 0, 1, 4, 8)], R, E, F, Hd,
+                                     descs["down_t"], y1.data_ptr())
+    assert e.value.status == 1

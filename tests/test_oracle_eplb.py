@@ -103,3 +103,12 @@ def test_split_rows_and_errors():
     with pytest.raises(ValueError):
         eplb.place([1], [-1], [1], [0])           # homeless expert, no slot
     assert eplb.place([5, 5], [0, 1], [1, 1], [4, 4]) == ([], [[0], [1]])      # balanced: nothing to do
+
+
+def test_replica_slots_hand_worked():
+    # rank 0: anchor 0, cap 5, shard [0,3) -> slots 0 1 2 taken; rank 1: anchor 3, cap 4, shard [2,5): slots (2-3)%4=3, 0, 1 taken
+    geom = {0: (0, 5), 1: (3, 4)}
+    shards = [(0, 0, 3, 1), (1, 2, 5, 1)]
+    assert eplb.replica_slots(shards, geom, [(4, 0), (0, 1), (3, 0)]) == [3, 2, 4]
+    with pytest.raises(StopIteration):
+        eplb.replica_slots(shards, geom, [(0, 1), (1, 1)])            # rank 1 has one spare slot only

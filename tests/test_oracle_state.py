@@ -422,3 +422,20 @@ def test_parallel_appliers_equal_the_plain_ones():
         for r in exp:
             assert got[r].tobytes() == exp[r].tobytes()
     assert OS.omp_threads() >= 1
+
+
+def test_swiglu_ref_is_the_inner_term_of_moe_ref():
+    """oracle.linear.swiglu_ref (pins the fused gate|up kernel) against scalar loops, and moe_ref with one expert and an
+    identity down projection returns exactly it."""
+    import math
+    rng = np.random.default_rng(9)
+    R, Hd, F = 3, 5, 5                       # F = hidden so that an identity down projection exists
+    x, g, u = rng.normal(size=(R, Hd)), rng.normal(size=(F, Hd)), rng.normal(size=(F, Hd))
+    h = OL.swiglu_ref(x, g, u)
+    for r in range(R):
+        for f in range(F):
+            a = sum(g[f, k] * x[r, k] for k in range(Hd))
+            b = sum(u[f, k] * x[r, k] for k in range(Hd))
+            assert abs(h[r, f] - a / (1.0 + math.exp(-a)) * b) < 1e-12
+    y = OL.moe_ref(x, np.zeros((R, 1)), g[None], u[None], np.eye(F)[None], 1)
+    np.testing.assert_allclose(y, h, rtol=1e-13)
