@@ -672,10 +672,49 @@ def run_moe(args):
             per[kind] = {"K": K, "N": N, "us": round(med * 1e3, 2), "TFLOPs": round(flop / med / 1e9, 1), "GBps": round(byts / med / 1e6, 1)}
             tot_ms, tot_flop, tot_bytes = tot_ms + med, tot_flop + flop, tot_bytes + byts
             out["launches"] += len(evs)
+        # the layer as etp_moe_gate_up + etp_moe_linear(down): X read once, SwiGLU in the epilogue, no [R][F] gate / up intermediates
+        xg = fill_normal16(state.seed, 9800 + T, 0, R * Hd, 1.0, state.dt, device=dev)
+        hbuf = torch.empty(R * F, dtype=state.dt, device=dev)
+        ybuf = torch.empty(R * Hd, dtype=state.dt, device=dev)
+        fus = {}
+        for name in ("gate_up", "down"):
+            seq = [(l % m.n_layers) for l in range(-3, m.n_layers)]
+            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in seq]
+            with torch.cuda.stream(st):
+                for (e0, e1), l in zip(evs, seq):
+                    for _ in range(3):
+                        flush.sum()
+                    e0.record(st)
+                    if name == "gate_up":
+                        etp.etp_moe_gate_up(ctx, m.dtype, xg.data_ptr(), Hd, F, descs[(l, "exp_gate")], descs[(l, "exp_up")], hbuf.data_ptr(),
+                                            row_offsets=offs, layout=new, stream=st.cuda_stream)
+                    else:
+                        etp.etp_moe_linear(ctx, etp.ROW_PARALLEL, m.dtype, hbuf.data_ptr(), offs, F, Hd, descs[(l, "exp_down_t")], new,
+                                           ybuf.data_ptr(), st.cuda_stream)
+                    e1.record(st)
+            st.synchronize()
+            ms = sorted(a.elapsed_time(b) for a, b in evs[3:])
+            fus[name] = ms[len(ms) // 2]
+            out["launches"] += len(evs)
+        f_ms = fus["gate_up"] + fus["down"]
+        f_bytes = 3 * 2.0 * hit * Hd * F + 2.0 * R * Hd + 2 * 2.0 * R * F + 2.0 * R * Hd
+        tf_burst = None
+        pp = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(pp):
+            with open(pp) as f:
+                tf_burst = json.load(f).get("bf16_tflops")
+        t_hbm, t_tc = f_bytes / hbm_peak / 1e3, (tot_flop / tf_burst / 1e6 if tf_burst else 0.0)     # us
         out[f"T{T}"] = {"routed_rows": R, "experts_hit": hit, "rows_per_expert_max": int(counts.max()), "layer_us": round(tot_ms * 1e3, 1),
                         "TFLOPs": round(tot_flop / tot_ms / 1e9, 1), "GBps": round(tot_bytes / tot_ms / 1e6, 1),
                         "hbm_frac": round(tot_bytes / tot_ms / 1e6 / hbm_peak, 4), "per_projection": per,
-                        "bytes": "2KN per expert hit + 2R(K+N)"}
+                        "bytes": "2KN per expert hit + 2R(K+N)",
+                        "fused": {"launches_per_layer": 2, "layer_us": round(f_ms * 1e3, 1), "gate_up_us": round(fus["gate_up"] * 1e3, 2),
+                                  "down_us": round(fus["down"] * 1e3, 2), "TFLOPs": round(tot_flop / f_ms / 1e9, 1),
+                                  "GBps": round(f_bytes / f_ms / 1e6, 1), "hbm_frac": round(f_bytes / f_ms / 1e6 / hbm_peak, 4),
+                                  "tensor_frac": round(tot_flop / f_ms / 1e9 / tf_burst, 4) if tf_burst else None,
+                                  "bound_us": {"hbm": round(t_hbm, 1), "tensor": round(t_tc, 1)},
+                                  "frac_of_bound": round(max(t_hbm, t_tc) / (f_ms * 1e3), 4),
+                                  "bytes": "6KN per expert hit + 2RK (x once) + 4RF (h written and read) + 2RK (y)"}}
     print(json.dumps(out))
     ctx.close()
     return 0

@@ -454,7 +454,7 @@ def test_linear_group_mixed_modes_one_launch(ctx, T, pdl):
     try:
         plan = etp.LinearPlan(ctx, lins)
         info = plan.info()
-        assert info["n_linears"] == 7 and 1 <= info["n_ctas"] <= 148 and info["n_items"] >= 7
+        assert info["n_linears"] == 7 and 1 <= info["n_ctas"] <= 2 * 148 and info["n_items"] >= 7    # up to two CTAs per SM
         assert info["max_cta_chunks"] * info["n_ctas"] >= info["total_chunks"] > 0
         st = torch.cuda.Stream()
         for _ in range(3):                       # back to back on one stream: launch i+1 overlaps the tail of launch i
