@@ -220,15 +220,25 @@ __device__ void copy_vec_item(const CopyArgs& a, unsigned int idx, int lane) {
 // addresses come from lane j (pre-biased by -excl[j]*16 so that address = base + w*16).
 __device__ void copy_small_batch(const CopyArgs& a, unsigned int k, int lane) {
     const uint32_t s0 = __ldg(a.small_first + k), s1 = __ldg(a.small_first + k + 1);
+    // the descriptors of round r + 1 are requested before round r is walked, so their latency hides under the round's copies
+    uint4 n0 = make_uint4(0, 0, 0, 0), n1 = make_uint4(0, 0, 0, 0);
+    if (s0 + lane < s1) {
+        const uint4* p = reinterpret_cast<const uint4*>(a.small + s0 + lane);
+        n0 = __ldg(p);
+        n1 = __ldg(p + 1);
+    }
     for (uint32_t s = s0; s < s1; s += 32) {
         uint64_t sb = 0, db = 0;
         uint32_t nv = 0;
         if (s + lane < s1) {
-            const uint4* p = reinterpret_cast<const uint4*>(a.small + s + lane);
-            const uint4 q0 = __ldg(p), q1 = __ldg(p + 1);
-            sb = u64_of(q0.x, q0.y);
-            db = u64_of(q0.z, q0.w);
-            nv = q1.x >> 4;
+            sb = u64_of(n0.x, n0.y);
+            db = u64_of(n0.z, n0.w);
+            nv = n1.x >> 4;
+        }
+        if (s + 32 + lane < s1) {
+            const uint4* p = reinterpret_cast<const uint4*>(a.small + s + 32 + lane);
+            n0 = __ldg(p);
+            n1 = __ldg(p + 1);
         }
         uint32_t incl = nv;
 #pragma unroll
@@ -320,8 +330,14 @@ __device__ void vector_warp(const CopyArgs& a, int lane) {
     }
 }
 
-__global__ void __launch_bounds__(kCopyThreads, 1) etp_interval_copy_kernel(const CopyArgs a) {
+__global__ void __launch_bounds__(kCopyThreads, 1) etp_interval_copy_kernel(const CopyArgs args) {
     extern __shared__ __align__(1024) uint8_t smem[];
+    CopyArgs a = args;
+    if (args.dev_counts) {   // queue lengths computed on the device by the classifier kernels that ran before this launch
+        a.n_bulk_items = __ldg(args.dev_counts);
+        a.n_vec_items = __ldg(args.dev_counts + 1);
+        a.n_small_batches = __ldg(args.dev_counts + 2);
+    }
     uint8_t* ring = smem;
     uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + (size_t)kStages * kStageBytes);
     uint64_t* s_dst = full_bar + kStages;

@@ -30,6 +30,8 @@ struct CopyArgs {
     const SmallSeg* small;        // small contiguous intervals, batched: vector-queue items n_vec_items .. + n_small_batches
     const uint32_t* small_first;  // n_small_batches + 1 entries
     unsigned int n_bulk_items, n_vec_items, n_small_batches;
+    const unsigned int* dev_counts;   // != NULL: {n_bulk_items, n_vec_items, n_small_batches} live on the device (descriptors
+                                      // lowered by the device-side classifier, etp_lower_dev.cu) and override the three above
     unsigned int* counters;       // [0] bulk head, [1] vec head (zeroed before launch)
     unsigned int flags;           // bit 0: vector warps also drain the bulk queue when theirs is empty
 };

@@ -188,6 +188,7 @@ extern "C" void etp_ctx_destroy(etp_ctx* c) {
     }
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
+    etp::free_interval_state(c);
     etp::lin_teardown(c);
     cudaGetLastError();
     delete x;
@@ -222,7 +223,9 @@ extern "C" etp_status etp_ctx_kernel_time(etp_ctx* c, double* ms_out, int32_t* n
         }
         n += D.n_timed;
     }
-    *ms_out = ms;
+    double iv_ms = 0;
+    n += interval_timed_launches(c, &iv_ms);   // chunked launches of a device-lowered etp_copy_intervals
+    *ms_out = ms + iv_ms;
     *n_out = n;
     return ETP_OK;
 }
@@ -264,6 +267,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
     const double t0 = now_ms();
     cudaStream_t caller_cs = (cudaStream_t)copy_stream_v, caller_rs = (cudaStream_t)reload_stream_v;
     CtxExtra* x = extra(c);
+    reset_interval_timing(c);
     const size_t n_dev = x->dev.size();
     const bool multi = n_dev > 1;
     const bool skip_d2d = c->opts[ETP_OPT_SKIP_D2D] != 0, skip_reload = c->opts[ETP_OPT_SKIP_RELOAD] != 0;
@@ -414,6 +418,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
                 a.small = (const SmallSeg*)(P.d_base + o.small);
                 a.small_first = (const uint32_t*)(P.d_base + o.small_first);
                 a.n_small_batches = (unsigned int)jl.small_first.size();
+                a.dev_counts = nullptr;
                 a.counters = (unsigned int*)(P.d_base + P.off_counters) + 2 * P.counter_slot;
                 a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
                 if (timed) {
@@ -490,6 +495,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
                         a.small_first = nullptr;
                         a.n_small_batches = 0;
                         a.n_vec_items = gl.n_vec_items;
+                        a.dev_counts = nullptr;
                         a.counters = (unsigned int*)(P.d_base + P.off_counters) + 2 * P.counter_slot;
                         a.flags = 0;
                         const int ggrid = (int)std::max<int64_t>(1, std::min<int64_t>(c->opts[ETP_OPT_GATHER_CTAS], c->n_sms));
@@ -625,20 +631,16 @@ extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_
                                          etp_reshard_report* report) {
     if (!ctx || n < 0 || (n > 0 && !host_descs)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: bad arguments");
     const double t0 = now_ms();
-    LoweredWork w;
-    w.dev.resize(1);   // the intervals are raw addresses: everything runs on the ctx's first logical device
-    w.dev[0].phases.resize(1);
-    w.dev[0].phases[0].small.reserve((size_t)n);
-    for (int64_t i = 0; i < n; ++i) {
-        const etp_interval& d = host_descs[i];
-        if (d.bytes < 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has negative size", (long long)i);
-        if (d.bytes == 0) continue;
-        if (!d.src || !d.dst) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has a NULL pointer", (long long)i);
-        if (((uintptr_t)d.src | (uintptr_t)d.dst | (uint64_t)d.bytes) & 15)
-            ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_copy_intervals: interval %lld is not 16-byte aligned", (long long)i);
-        push_contiguous(ctx, &w.dev[0].phases[0], d.src, d.dst, d.bytes);
-        w.rep.d2d_bytes += d.bytes;
-        w.dev[0].rep.d2d_bytes += d.bytes;
+    const bool device_path = n >= kDeviceLoweringMin;
+    if (ctx->opts[ETP_OPT_VALIDATE_INTERVALS] || !device_path) {
+        for (int64_t i = 0; i < n; ++i) {
+            const etp_interval& d = host_descs[i];
+            if (d.bytes < 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has negative size", (long long)i);
+            if (d.bytes == 0) continue;
+            if (!d.src || !d.dst) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has a NULL pointer", (long long)i);
+            if (((uintptr_t)d.src | (uintptr_t)d.dst | (uint64_t)d.bytes) & 15)
+                ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_copy_intervals: interval %lld is not 16-byte aligned", (long long)i);
+        }
     }
     if (ctx->opts[ETP_OPT_VALIDATE_INTERVALS]) {
         // the contract of include/etp.h: destinations mutually disjoint and disjoint from every source (one launch, no order
@@ -670,6 +672,24 @@ extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_
             if (src_reach > d.b)
                 ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: destination of interval %lld overlaps the source of interval %lld", (long long)d.i, (long long)src_reach_i);
         }
+    }
+    if (device_path) {
+        // 10^5 .. 10^6 intervals: the raw records are uploaded in chunks and lowered by kernels while the previous chunk is being
+        // copied (without the validation above, argument errors of a later chunk surface after earlier chunks were enqueued)
+        ETP_TRY(copy_intervals_device(ctx, host_descs, n, stream, report));
+        if (report) report->lower_ms = now_ms() - t0;
+        return ETP_OK;
+    }
+    LoweredWork w;
+    w.dev.resize(1);   // the intervals are raw addresses: everything runs on the ctx's first logical device
+    w.dev[0].phases.resize(1);
+    w.dev[0].phases[0].small.reserve((size_t)n);
+    for (int64_t i = 0; i < n; ++i) {
+        const etp_interval& d = host_descs[i];
+        if (d.bytes == 0) continue;
+        push_contiguous(ctx, &w.dev[0].phases[0], d.src, d.dst, d.bytes);
+        w.rep.d2d_bytes += d.bytes;
+        w.dev[0].rep.d2d_bytes += d.bytes;
     }
     w.rep.n_phases = 1;
     w.rep.lower_ms = now_ms() - t0;

@@ -121,6 +121,7 @@ struct etp_ctx {
     int64_t opts[ETP_OPT__COUNT];
     void* impl = nullptr;               // executor state (per logical device: streams, descriptor arenas, events), etp_exec.cu
     int32_t launches = 0;               // kernels launched by the last call
+    void* iv_state = nullptr;           // device-side lowering of etp_copy_intervals (etp_lower_dev.cu)
     void* lin_state = nullptr;          // kernel (c): per-stream split-K workspaces + the cache of prepared groups (etp_linear_group.cu)
 };
 
@@ -145,6 +146,13 @@ etp_status lower_params(const etp_ctx* ctx, const etp_tensor* tensors, int32_t n
 etp_status lower_kv(const etp_ctx* ctx, const etp_kv_geometry* g, const etp_plan* head_plan, const int32_t* pairs,
                     int64_t n_pairs, LoweredWork* out);
 void push_contiguous(const etp_ctx* ctx, JobList* jl, const void* src, void* dst, int64_t bytes);
+
+// etp_copy_intervals above kDeviceLoweringMin intervals: descriptors are built by kernels from the raw records (etp_lower_dev.cu)
+constexpr int64_t kDeviceLoweringMin = 32768;
+etp_status copy_intervals_device(etp_ctx* ctx, const etp_interval* host_descs, int64_t n, void* stream, etp_reshard_report* report);
+void free_interval_state(etp_ctx* ctx);
+int interval_timed_launches(etp_ctx* ctx, double* ms);
+void reset_interval_timing(etp_ctx* ctx);
 
 // kernel (c): frees the ctx-owned cache of prepared groups and the split-K workspaces (etp_linear_group.cu)
 void lin_teardown(etp_ctx* ctx);

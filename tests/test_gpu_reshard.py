@@ -419,14 +419,17 @@ def test_migration_aware_plan_reshard_and_linear(ctx, slabs_mode):
 
 
 # ------------------------------------------------------------------------------------------------ interval copy (5b)
-@pytest.mark.parametrize("n,hi", [(0, 1 << 20), (1, 1 << 20), (300, 4 << 20), (20000, 8 << 10)])
+@pytest.mark.parametrize("n,hi", [(0, 1 << 20), (1, 1 << 20), (300, 4 << 20), (20000, 8 << 10),
+                                  (40000, 8 << 10), (70000, 96 << 10)])    # >= 32768 intervals: device-side lowering, 1 and 2 chunks
 @pytest.mark.parametrize("tma_min", [None, 16, 1 << 62])
 def test_copy_intervals_bit_exact(ctx, n, hi, tma_min):
     """Config 5b recipe at a size the host reproduces in seconds: log-uniform sizes from 16 B, random 16-B aligned
-    offsets, overlapping sources, disjoint destinations with random gaps (gaps must keep their old bytes)."""
+    offsets, overlapping sources, disjoint destinations with random gaps (gaps must keep their old bytes).  From 32768
+    intervals on the descriptors are built on the device (etp_lower_dev.cu); tma_min routes the same plan through the bulk
+    queue only, the vector queue only (linear + small segments), or both."""
     src_arena = 64 << 20
     if n:
-        so, do, sz, dst_arena = microbench_intervals(n, 16, hi, 1234 + n, src_arena, max_total=256 << 20)
+        so, do, sz, dst_arena = microbench_intervals(n, 16, hi, 1234 + n, src_arena, max_total=(1 << 30) if n > 30000 else (256 << 20))
     else:
         so = do = sz = np.zeros(0, dtype=np.int64)
         dst_arena = 1024
