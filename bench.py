@@ -465,17 +465,21 @@ def run_microbench(args):
     def run_plan(so, do, sz, dst_arena, iters=5):
         dst = torch.empty(dst_arena + 256, dtype=torch.uint8, device=dev)
         sp, dp = so + src.data_ptr(), do + dst.data_ptr()
-        kms, cms = [], []
-        for it in range(2 + iters):
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(st)
-            rep = etp.etp_copy_intervals(ctx, sp, dp, sz, st.cuda_stream)
-            e1.record(st)
-            e1.synchronize()
-            ms, _ = ctx.kernel_time()
-            if it >= 2:
-                kms.append(ms)
-                cms.append(e0.elapsed_time(e1))
+        kms, cms, pms = [], [], []
+        lists = {"pageable": etp.IntervalList(sp, dp, sz), "pinned": etp.IntervalList(sp, dp, sz, pin=True)}   # marshalled once: the loop pays the C call
+        for kind, cm in (("pageable", cms), ("pinned", pms)):
+            for it in range(2 + iters):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(st)
+                rep = lists[kind].run(ctx, st.cuda_stream)
+                e1.record(st)
+                e1.synchronize()
+                ms, _ = ctx.kernel_time()
+                if it >= 2:
+                    if kind == "pageable":
+                        kms.append(ms)
+                    cm.append(e0.elapsed_time(e1))
+        pms.sort()
         n = len(sz)
         pick = np.unique(np.concatenate([[int(np.argmax(sz)), int(np.argmin(sz))], rng.integers(0, n, 62)]))
         for i in pick:
@@ -499,6 +503,7 @@ def run_microbench(args):
             ctx.set_option(etp.OPT_VALIDATE_INTERVALS, 0)
         return {"n": n, "total_GiB": round(tot / 2 ** 30, 3), "kernel_ms": round(k, 4), "moved_GBps": round(tot / k / 1e6, 1),
                 "hbm_frac": round(2.0 * tot / k / 1e6 / hbm_peak, 4), "call_ms": round(c, 3), "call_over_kernel": round(c / k, 3),
+                "call_ms_pinned_records": round(pms[len(pms) // 2], 3), "descriptor_MB": round(24e-6 * n, 2),
                 "call_GBps": round(tot / c / 1e6, 1), "call_ms_validated": round(cv, 3),
                 "segments": rep["n_jobs"], "work_items": rep["n_units"], "lower_ms": round(rep["lower_ms"], 3),
                 "lowering": "device (chunks of 65536 intervals, upload + classify overlapped with the copies)" if n >= 32768 else "host"}

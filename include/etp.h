@@ -379,8 +379,10 @@ etp_status etp_eplb_apply(etp_ctx* ctx, const etp_tensor* tensors, int32_t n_ten
                           const etp_replica* replicas, int32_t n_replicas, int64_t* slots_out, void* stream);
 
 /* ------------------------------------------------------------------------------------------------ microbenchmark entry
- * Copies n arbitrary intervals with the same persistent kernel (config 5b).  host_descs: host array; src/dst: device,
- * 16-B aligned; bytes: multiple of 16.  Destinations must be mutually disjoint and disjoint from every source (the
+ * Copies n arbitrary intervals with the same persistent kernel (config 5b).  host_descs: host array (pageable: consumed before
+ * the call returns; page-locked: read by DMA, must stay valid until `stream` is synchronised); src/dst: device, 16-B aligned;
+ * bytes: multiple of 16.  From 32768 intervals on, the raw records are uploaded in chunks and lowered to work descriptors by
+ * kernels on a library-owned stream while earlier chunks are being copied (one kernel launch per 262144 intervals).  Destinations must be mutually disjoint and disjoint from every source (the
  * intervals of one call are unordered); checked unless ETP_OPT_VALIDATE_INTERVALS is 0 -> ETP_ERR_INVALID_ARG, nothing
  * enqueued.  Sources may overlap each other. */
 typedef struct { const void* src; void* dst; int64_t bytes; } etp_interval;

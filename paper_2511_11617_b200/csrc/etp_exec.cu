@@ -52,6 +52,9 @@ double now_ms() {
 }  // namespace
 
 namespace etp {
+void reset_device_timing(etp_ctx* c) {
+    for (DevState& D : extra(c)->dev) D.n_timed = 0;
+}
 int n_logical_devices(const etp_ctx* c) { return (int)extra(c)->dev.size(); }
 int device_of_rank(const etp_ctx* c, int32_t rank) {
     const CtxExtra* x = extra(c);

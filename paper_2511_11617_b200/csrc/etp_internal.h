@@ -153,6 +153,7 @@ etp_status copy_intervals_device(etp_ctx* ctx, const etp_interval* host_descs, i
 void free_interval_state(etp_ctx* ctx);
 int interval_timed_launches(etp_ctx* ctx, double* ms);
 void reset_interval_timing(etp_ctx* ctx);
+void reset_device_timing(etp_ctx* ctx);   // forgets the timing events of the last executor call (etp_exec.cu)
 
 // kernel (c): frees the ctx-owned cache of prepared groups and the split-K workspaces (etp_linear_group.cu)
 void lin_teardown(etp_ctx* ctx);

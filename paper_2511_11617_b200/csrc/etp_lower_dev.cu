@@ -11,10 +11,11 @@
 //            entries; small intervals also record the byte offset at which they start in the concatenation of all small ones
 //   batches  small intervals are batched by 32-KiB windows of that concatenation (an interval is <= 32 KiB, so no window is
 //            empty and the window index IS the batch index): the first interval of every window writes the batch start
-// Chunks are double-buffered: the upload and the lowering of chunk k+1 run on a library-owned stream while the copy kernel of
-// chunk k runs on the caller's stream, so the call costs about the copy kernels plus the first chunk's upload.
+// Chunks are triple-buffered: the upload and the lowering of chunks k+1 and k+2 run on a library-owned stream while the copy
+// kernel of chunk k runs on the caller's stream, so the call costs about the copy kernels plus the first chunk's upload.
 #include <algorithm>
 #include <chrono>
+#include <cstring>
 #include <vector>
 
 #include "etp_copy.cuh"
@@ -23,9 +24,9 @@ using namespace etp;
 
 namespace {
 
-constexpr int kChunk = 1 << 16;       // intervals per chunk
+constexpr int kChunk = 1 << 18;       // intervals per chunk (a launch of the copy kernel per chunk: 64 MiB even at 256 B per interval)
 constexpr int kBlock = 1024;
-constexpr int kSlots = 2;
+constexpr int kSlots = 3;         // descriptors of chunk k are copied while chunks k+1 and k+2 are uploaded and counted
 enum { C_BULK_SEGS = 0, C_BULK_ITEMS, C_VEC_SEGS, C_VEC_ITEMS, C_SMALL_SEGS, C_SMALL_BYTES, C_ALL_BYTES, C_N };
 
 struct Totals {            // written by the scan kernel, copied to pinned host memory
@@ -110,18 +111,19 @@ __global__ void __launch_bounds__(kBlock) etp_iv_count_kernel(const etp_interval
         for (int k = 0; k < C_N; ++k) block_sums[(size_t)blockIdx.x * C_N + k] = tot.v[k];
 }
 
-// one block: exclusive scan over the (<= 64) block sums; also zeroes the copy kernel's work-queue heads for this chunk
+// one block: exclusive scan over the (<= 256) block sums; also zeroes the copy kernel's work-queue heads for this chunk
 __global__ void etp_iv_scan_kernel(unsigned long long* block_sums, int n_blocks, Totals* totals, const unsigned int* bad, unsigned int* counters) {
-    if (threadIdx.x == 0) {
-        unsigned long long run[C_N];
-        for (int k = 0; k < C_N; ++k) run[k] = 0;
-        for (int b = 0; b < n_blocks; ++b)
-            for (int k = 0; k < C_N; ++k) {
-                const unsigned long long s = block_sums[(size_t)b * C_N + k];
-                block_sums[(size_t)b * C_N + k] = run[k];
-                run[k] += s;
-            }
-        for (int k = 0; k < C_N; ++k) totals->v[k] = run[k];
+    const int k = threadIdx.x;   // one thread per counter
+    if (k < C_N) {
+        unsigned long long run = 0;
+        for (int b = 0; b < n_blocks; ++b) {
+            const unsigned long long s = block_sums[(size_t)b * C_N + k];
+            block_sums[(size_t)b * C_N + k] = run;
+            run += s;
+        }
+        totals->v[k] = run;
+    }
+    if (k == 0) {
         totals->bad_align = bad[0] == 0xffffffffu ? 0u : bad[0] + 1u;
         totals->bad_size = bad[1] == 0xffffffffu ? 0u : bad[1] + 1u;
         counters[0] = 0;
@@ -189,6 +191,7 @@ __global__ void etp_iv_batches_kernel(const SmallSeg* small, const Totals* total
 }
 
 struct Slot {
+    etp_interval* h_raw = nullptr;   // pinned staging: the host copies the caller's (pageable) records here, the DMA is then truly asynchronous
     etp_interval* d_raw = nullptr;
     unsigned long long* d_block_sums = nullptr;
     Totals* d_totals = nullptr;
@@ -202,7 +205,7 @@ struct Slot {
     uint32_t *d_bulk_items = nullptr, *d_vec_items = nullptr;
     int64_t bulk_items_cap = 0, vec_items_cap = 0;
     cudaEvent_t uploaded = nullptr, totals_ready = nullptr, lowered = nullptr, copied = nullptr;
-    bool busy = false;
+    bool busy = false, staged = false;
 };
 struct IvState {
     cudaStream_t side = nullptr;     // upload + lowering stream
@@ -226,6 +229,7 @@ etp_status ensure_state(etp_ctx* c, IvState** out) {
     ETP_CUDA_OK(cudaStreamCreateWithFlags(&S->side, cudaStreamNonBlocking));
     const int n_blocks = kChunk / kBlock;
     for (Slot& s : S->slot) {
+        ETP_CUDA_OK(cudaMallocHost(&s.h_raw, sizeof(etp_interval) * kChunk));
         ETP_CUDA_OK(cudaMalloc(&s.d_raw, sizeof(etp_interval) * kChunk));
         ETP_CUDA_OK(cudaMalloc(&s.d_block_sums, sizeof(unsigned long long) * C_N * n_blocks));
         ETP_CUDA_OK(cudaMalloc(&s.d_totals, sizeof(Totals)));
@@ -254,6 +258,7 @@ void free_interval_state(etp_ctx* c) {
                         (void*)s.d_small, (void*)s.d_small_first, (void*)s.d_bulk_items, (void*)s.d_vec_items})
             if (p) cudaFree(p);
         if (s.h_totals) cudaFreeHost(s.h_totals);
+        if (s.h_raw) cudaFreeHost(s.h_raw);
         for (cudaEvent_t e : {s.uploaded, s.totals_ready, s.lowered, s.copied})
             if (e) cudaEventDestroy(e);
     }
@@ -292,6 +297,7 @@ etp_status copy_intervals_device(etp_ctx* c, const etp_interval* host_descs, int
     etp_reshard_report rep{};
     rep.n_phases = 1;
     const int64_t n_chunks = (n + kChunk - 1) / kChunk;
+    const bool pinned_input = classify_pointer(host_descs) == MEM_HOST_PINNED;
 
     // stage A of chunk k (side stream): upload the raw records, count, scan, totals -> pinned host
     auto stage_a = [&](int64_t k) -> etp_status {
@@ -301,7 +307,18 @@ etp_status copy_intervals_device(etp_ctx* c, const etp_interval* host_descs, int
             ETP_CUDA_OK(cudaStreamWaitEvent(S->side, s.copied, 0));
             s.busy = false;
         }
-        ETP_CUDA_OK(cudaMemcpyAsync(s.d_raw, host_descs + b, sizeof(etp_interval) * (size_t)m, cudaMemcpyHostToDevice, S->side));
+        if (pinned_input) {   // the caller's array is page-locked: the DMA reads it directly (it must stay valid until the stream is synchronised)
+            ETP_CUDA_OK(cudaMemcpyAsync(s.d_raw, host_descs + b, sizeof(etp_interval) * (size_t)m, cudaMemcpyHostToDevice, S->side));
+        } else {
+            if (s.staged) {   // the DMA that last read this slot's staging buffer
+                ETP_CUDA_OK(cudaEventSynchronize(s.uploaded));
+                s.staged = false;
+            }
+            std::memcpy(s.h_raw, host_descs + b, sizeof(etp_interval) * (size_t)m);
+            ETP_CUDA_OK(cudaMemcpyAsync(s.d_raw, s.h_raw, sizeof(etp_interval) * (size_t)m, cudaMemcpyHostToDevice, S->side));
+            ETP_CUDA_OK(cudaEventRecord(s.uploaded, S->side));
+            s.staged = true;
+        }
         ETP_CUDA_OK(cudaMemsetAsync(s.d_bad, 0xff, 2 * sizeof(unsigned int), S->side));
         const int nb = int((m + kBlock - 1) / kBlock);
         etp_iv_count_kernel<<<nb, kBlock, 0, S->side>>>(s.d_raw, (int)m, tma_min, s.d_block_sums, s.d_bad);
@@ -312,7 +329,8 @@ etp_status copy_intervals_device(etp_ctx* c, const etp_interval* host_descs, int
         return ETP_OK;
     };
 
-    if (n_chunks > 0) ETP_TRY(stage_a(0));
+    reset_device_timing(c);
+    for (int64_t k = 0; k < std::min<int64_t>(n_chunks, kSlots - 1); ++k) ETP_TRY(stage_a(k));
     for (int64_t k = 0; k < n_chunks; ++k) {
         Slot& s = S->slot[k % kSlots];
         const int64_t b = k * kChunk, m = std::min<int64_t>(kChunk, n - b);
@@ -340,7 +358,6 @@ etp_status copy_intervals_device(etp_ctx* c, const etp_interval* host_descs, int
         etp_iv_batches_kernel<<<(unsigned)std::max<unsigned long long>(1, (n_small + 255) / 256), 256, 0, S->side>>>(s.d_small, s.d_totals, s.d_small_first, s.d_counts);
         ETP_CUDA_OK(cudaGetLastError());
         ETP_CUDA_OK(cudaEventRecord(s.lowered, S->side));
-        if (k + 1 < n_chunks) ETP_TRY(stage_a(k + 1));   // upload + count of the next chunk overlap this chunk's copy
         // stage C (caller's stream): the copy kernel on the device-built descriptors
         const unsigned long long moved_items = T.v[C_BULK_ITEMS] + T.v[C_VEC_ITEMS] + n_small;
         if (moved_items > 0) {
@@ -376,6 +393,9 @@ etp_status copy_intervals_device(etp_ctx* c, const etp_interval* host_descs, int
         }
         ETP_CUDA_OK(cudaEventRecord(s.copied, user));
         s.busy = true;
+        // upload + count of chunk k + 2 (the slot chunk k - 1 used) while chunks k and k + 1 are copied / lowered; issued AFTER this
+        // chunk's copy launch because the upload from pageable memory blocks the host
+        if (k + kSlots - 1 < n_chunks) ETP_TRY(stage_a(k + kSlots - 1));
         rep.n_jobs += (int64_t)(T.v[C_BULK_SEGS] + T.v[C_VEC_SEGS] + T.v[C_SMALL_SEGS]);
         rep.n_units += (int64_t)moved_items;
         rep.d2d_bytes += (int64_t)T.v[C_ALL_BYTES];
