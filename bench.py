@@ -53,6 +53,7 @@ def parse_args():
     ap.add_argument("--sharded", action="store_true",
                     help="--gpus N > 1: ONE reshard sharded by destination rank over N processes / GPUs (simulated rank r on GPU r mod N, "
                          "peers' memory through CUDA IPC, no collective) instead of N independent replicas")
+    ap.add_argument("--small-staged", type=int, default=-1, help="A/B: ETP_OPT_SMALL_STAGED for --microbench (default: the library's)")
     ap.add_argument("--lin-pdl", type=int, default=-1, help="A/B: ETP_OPT_LINEAR_PDL for the S7 leg (default: the library's)")
     ap.add_argument("--lin-ring", type=int, default=-1, help="A/B: ETP_OPT_LINEAR_RING for the S7 leg (default: the library's)")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0, help="CPU seconds of oracle work in the cpu_baseline leg")
@@ -456,6 +457,8 @@ def run_microbench(args):
     ctx = etp.Context(0)
     ctx.set_option(etp.OPT_TIME_KERNELS, 1)
     ctx.set_option(etp.OPT_VALIDATE_INTERVALS, 0)      # the timed calls trust the plan; the validated call is timed beside them
+    if args.small_staged >= 0:
+        ctx.set_option(etp.OPT_SMALL_STAGED, args.small_staged)
     st = torch.cuda.Stream(dev)
     src_arena = 32 << 30
     src = fill_bytes(SEED0 + 5000, 1, 0, src_arena, device=dev)

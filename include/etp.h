@@ -106,6 +106,12 @@ typedef enum {
                                     2 (default) = two per SM unless the group streams >= 200 weight chunks (3.2 MiB) per SM      */
     ETP_OPT_ONLY_PHASE = 13,     /* 0 (default): a call runs every hazard phase, ordered by events; k > 0: only phase k - 1 is
                                     enqueued (multi-process jobs: the caller puts its own barrier between the phases)         */
+    ETP_OPT_MOE_CTA_PAIR = 14,   /* 1 (default): the grouped MoE kernels run CTA pairs (tcgen05 cta_group::2, 256 out features x up to
+                                    256 routed rows per pair, each CTA staging half of the rows) when the instances carry enough rows
+                                    for >= 128-row tiles; 2: always; 0: never (single-CTA 128-feature tiles)                  */
+    ETP_OPT_SMALL_STAGED = 15,   /* 1 (default): in a launch of the copy kernel without bulk (>= TMA_MIN_BYTES) intervals, batches of small
+                                    intervals are staged through the idle shared-memory ring with per-lane cp.async.bulk copies (more
+                                    bytes in flight than the register path allows); 0: always the register path                    */
     ETP_OPT__COUNT
 } etp_option;
 etp_status etp_ctx_set_option(etp_ctx* ctx, etp_option key, int64_t value);

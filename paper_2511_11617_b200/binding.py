@@ -21,7 +21,8 @@ COL_PARALLEL, ROW_PARALLEL = 0, 1
 DTYPE = {"bf16": 0, "fp16": 1}
 KV_TOKEN_MAJOR, KV_HEAD_MAJOR = 0, 1
 (OPT_SKIP_D2D, OPT_SKIP_RELOAD, OPT_TMA_MIN_BYTES, OPT_LDG_STEALS_BULK, OPT_RELOAD_CHUNK_BYTES, OPT_RESERVED_5,
- OPT_GRID_CTAS, OPT_GATHER_CTAS, OPT_TIME_KERNELS, OPT_LINEAR_CTA_PAIR, OPT_VALIDATE_INTERVALS, OPT_LINEAR_PDL, OPT_LINEAR_RING, OPT_ONLY_PHASE) = range(14)
+ OPT_GRID_CTAS, OPT_GATHER_CTAS, OPT_TIME_KERNELS, OPT_LINEAR_CTA_PAIR, OPT_VALIDATE_INTERVALS, OPT_LINEAR_PDL, OPT_LINEAR_RING, OPT_ONLY_PHASE,
+ OPT_MOE_CTA_PAIR, OPT_SMALL_STAGED) = range(16)
 
 
 class EtpError(RuntimeError):

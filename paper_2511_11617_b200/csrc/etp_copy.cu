@@ -304,8 +304,116 @@ __device__ void copy_small_batch(const CopyArgs& a, unsigned int k, int lane) {
     }
 }
 
-__device__ void vector_warp(const CopyArgs& a, int lane) {
+// ---------------------------------------------------------------------------------------------- small batches, staged
+// The register path above keeps one block (8 x 32 words = 4 KiB) per warp in flight: a block's stores wait for its loads, the next
+// block's loads are issued after them, and 126 registers per thread leave no room for a second buffer - at 256 B per interval the
+// walk runs at 0.4-0.5 of the copy peak, latency-bound.  When a launch has NO bulk items the 192-KiB ring is idle, and every vector
+// warp takes 12 KiB of it as kSmStages stages of 2 KiB.  A batch is then a sequence of BLOCKS of 128 words (rounds of 32 descriptors,
+// prefix-summed as above); for every block each lane intersects ITS OWN interval with the block's word range and issues at most one
+// cp.async.bulk global -> shared for that piece (completion in bytes on the stage's mbarrier) and, kSmLag blocks later, at most one
+// cp.async.bulk shared -> global for the same piece.  No per-word search, no data in registers: the bytes in flight are bounded by
+// shared memory (kSmLag blocks per warp), and 32 lanes issue the tensor-less bulk copies in parallel.
+constexpr int kSmBlockWords = 128;
+constexpr int kSmStages = 6;
+constexpr int kSmLag = 4;
+constexpr int kSmWarpBytes = kSmStages * kSmBlockWords * 16;
+static_assert(15 * kSmWarpBytes <= kStages * kStageBytes, "staged small path must fit the ring");
+
+struct SmallGen {        // walks the blocks of one batch; every lane runs it (it shuffles)
+    uint32_t s, s1;      // next round's first descriptor, batch end
+    uint64_t base;       // this lane's src (or dst) address, pre-biased by -excl * 16
+    uint32_t excl, nv, total, w0;
+    bool valid;
+};
+
+__device__ __forceinline__ void gen_advance(SmallGen& g, const SmallSeg* small, int lane, bool use_dst) {
+    g.w0 += kSmBlockWords;
+    while (g.w0 >= g.total) {
+        if (g.s >= g.s1) {
+            g.valid = false;
+            return;
+        }
+        uint64_t b = 0;
+        uint32_t nv = 0;
+        if (g.s + lane < g.s1) {
+            const uint4* p = reinterpret_cast<const uint4*>(small + g.s + lane);
+            const uint4 q0 = __ldg(p), q1 = __ldg(p + 1);
+            b = use_dst ? u64_of(q0.z, q0.w) : u64_of(q0.x, q0.y);
+            nv = q1.x >> 4;
+        }
+        uint32_t incl = nv;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        g.nv = nv;
+        g.excl = incl - nv;
+        g.total = __shfl_sync(0xffffffffu, incl, 31);
+        g.base = b - (uint64_t)g.excl * 16;
+        g.s += 32;
+        g.w0 = 0;
+    }
+    g.valid = true;
+}
+
+__device__ void copy_small_batch_staged(const CopyArgs& a, unsigned int k, int lane, uint8_t* stage_mem, uint64_t* bars, uint32_t& gb) {
+    SmallGen lead, lag;
+    lead.s = lag.s = __ldg(a.small_first + k);
+    lead.s1 = lag.s1 = __ldg(a.small_first + k + 1);
+    lead.total = lag.total = 0;
+    lead.w0 = lag.w0 = 0;
+    lead.nv = lag.nv = lead.excl = lag.excl = 0;
+    lead.base = lag.base = 0;
+    gen_advance(lead, a.small, lane, false);
+    gen_advance(lag, a.small, lane, true);
+    uint32_t issued = 0, stored = 0;
+    for (;;) {
+        bool did = false;
+        if (lead.valid && issued - stored < (uint32_t)kSmLag) {
+            const uint32_t g = gb + issued, st = g % kSmStages;
+            // the stage's previous block (g - kSmStages) was stored at least kSmStages - kSmLag store groups ago
+            bulk_wait_read<kSmStages - kSmLag>();
+            __syncwarp();
+            const uint32_t bar = smem_u32(&bars[st]);
+            const uint32_t blk = min((uint32_t)kSmBlockWords, lead.total - lead.w0);
+            if (lane == 0) mbar_arrive_expect_tx(bar, blk * 16);
+            const uint32_t lo = max(lead.excl, lead.w0), hi = min(lead.excl + lead.nv, lead.w0 + blk);
+            if (lo < hi)
+                bulk_g2s(smem_u32(stage_mem + (size_t)st * (kSmBlockWords * 16) + (size_t)(lo - lead.w0) * 16), lead.base + (uint64_t)lo * 16, (hi - lo) * 16, bar);
+            ++issued;
+            gen_advance(lead, a.small, lane, false);
+            did = true;
+        }
+        if (stored < issued && (issued - stored == (uint32_t)kSmLag || !lead.valid)) {
+            const uint32_t g = gb + stored, st = g % kSmStages;
+            mbar_wait(smem_u32(&bars[st]), (g / kSmStages) & 1u);
+            const uint32_t blk = min((uint32_t)kSmBlockWords, lag.total - lag.w0);
+            const uint32_t lo = max(lag.excl, lag.w0), hi = min(lag.excl + lag.nv, lag.w0 + blk);
+            if (lo < hi)
+                bulk_s2g(lag.base + (uint64_t)lo * 16, smem_u32(stage_mem + (size_t)st * (kSmBlockWords * 16) + (size_t)(lo - lag.w0) * 16), (hi - lo) * 16);
+            bulk_commit();
+            ++stored;
+            gen_advance(lag, a.small, lane, true);
+            did = true;
+        }
+        if (!did) break;
+    }
+    gb += issued;
+}
+
+__device__ void vector_warp(const CopyArgs& a, int lane, uint8_t* stage_mem, uint64_t* bars) {
     const unsigned int n_items = a.n_vec_items + a.n_small_batches;
+    const bool staged = stage_mem != nullptr;   // warp-uniform: the ring is idle (no bulk items) and the option is on
+    uint32_t gb = 0;                            // blocks this warp has pushed through its stages (stage = gb % kSmStages)
+    if (staged) {
+        if (lane == 0) {
+            for (int s = 0; s < kSmStages; ++s) mbar_init(smem_u32(&bars[s]), 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        }
+        __syncwarp();
+    }
     for (;;) {
         unsigned int idx = 0;
         if (lane == 0) idx = atomicAdd(&a.counters[1], 1u);
@@ -313,9 +421,12 @@ __device__ void vector_warp(const CopyArgs& a, int lane) {
         if (idx >= n_items) break;
         if (idx < a.n_vec_items)
             copy_vec_item(a, idx, lane);
+        else if (staged)
+            copy_small_batch_staged(a, idx - a.n_vec_items, lane, stage_mem, bars, gb);
         else
             copy_small_batch(a, idx - a.n_vec_items, lane);
     }
+    if (staged) bulk_wait_all();
     if (a.flags & 1u) {
         // drain the bulk queue too (one item per warp at a time)
         for (;;) {
@@ -351,7 +462,9 @@ __global__ void __launch_bounds__(kCopyThreads, 1) etp_interval_copy_kernel(cons
             tma_driver(a, ring, full_bar, s_dst, s_bytes);
         }
     } else {
-        vector_warp(a, lane);
+        const bool staged = (a.flags & 2u) && a.n_bulk_items == 0 && a.n_small_batches != 0;
+        uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)kStages * kStageBytes + 128) + (warp - 1) * kSmStages;
+        vector_warp(a, lane, staged ? ring + (size_t)(warp - 1) * kSmWarpBytes : nullptr, bars);
     }
 }
 

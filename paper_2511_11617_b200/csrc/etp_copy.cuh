@@ -33,7 +33,8 @@ struct CopyArgs {
     const unsigned int* dev_counts;   // != NULL: {n_bulk_items, n_vec_items, n_small_batches} live on the device (descriptors
                                       // lowered by the device-side classifier, etp_lower_dev.cu) and override the three above
     unsigned int* counters;       // [0] bulk head, [1] vec head (zeroed before launch)
-    unsigned int flags;           // bit 0: vector warps also drain the bulk queue when theirs is empty
+    unsigned int flags;           // bit 0: vector warps also drain the bulk queue when theirs is empty; bit 1: small batches may be
+                                  // staged through the ring when the launch has no bulk items (ETP_OPT_SMALL_STAGED)
 };
 
 void launch_copy_kernel(const CopyArgs& a, int grid, cudaStream_t stream);

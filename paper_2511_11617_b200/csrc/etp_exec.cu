@@ -109,6 +109,8 @@ extern "C" etp_status etp_ctx_create_multi(const int32_t* devices, int32_t n_dev
     c->opts[ETP_OPT_LINEAR_PDL] = 1;
     c->opts[ETP_OPT_LINEAR_RING] = 2;
     c->opts[ETP_OPT_ONLY_PHASE] = 0;
+    c->opts[ETP_OPT_MOE_CTA_PAIR] = 1;
+    c->opts[ETP_OPT_SMALL_STAGED] = 0;
     CtxExtra* x = new (std::nothrow) CtxExtra();
     if (!x) { delete c; ETP_FAIL(ETP_ERR_NOMEM, "etp_ctx_create: out of memory"); }
     c->impl = x;
@@ -423,7 +425,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
                 a.n_small_batches = (unsigned int)jl.small_first.size();
                 a.dev_counts = nullptr;
                 a.counters = (unsigned int*)(P.d_base + P.off_counters) + 2 * P.counter_slot;
-                a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
+                a.flags = (c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u) | (c->opts[ETP_OPT_SMALL_STAGED] ? 2u : 0u);
                 if (timed) {
                     while ((int)D.tev.size() < 2 * (D.n_timed + 1)) {
                         cudaEvent_t e;

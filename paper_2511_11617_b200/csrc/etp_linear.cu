@@ -258,49 +258,6 @@ struct PairCfg {
     static constexpr int kSmemBytes = kStages * kStageBytes + 1024 + 256 + kStageTileBytes;
 };
 
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ uint32_t mapa_rank0(uint32_t saddr) {   // the same shared-memory offset in CTA 0 of the cluster
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, 0;" : "=r"(r) : "r"(saddr));
-    return r;
-}
-__device__ __forceinline__ void cluster_sync_all() {
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tma_load_2d_pair(void* smem_dst, const CUtensorMap* map, uint32_t leader_bar, int32_t c0, int32_t c1) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
-            smem_u32(smem_dst)),
-        "l"(reinterpret_cast<uint64_t>(map)), "r"(leader_bar), "r"(c0), "r"(c1)
-        : "memory");
-}
-__device__ __forceinline__ void tc_commit_pair(uint64_t* bar) {   // arrives on `bar` at the same offset in BOTH CTAs
-    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)),
-                 "h"(uint16_t(3))
-                 : "memory");
-}
-__device__ __forceinline__ void tc_mma_pair(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
-        "}" ::"r"(d_tmem),
-        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
-}
-__host__ __device__ constexpr uint32_t make_idesc_pair(uint32_t fmt, uint32_t a_mn_major, uint32_t n) {
-    return (1u << 4) | (fmt << 7) | (fmt << 10) | (a_mn_major << 15) | ((n >> 3) << 17) | ((uint32_t(2 * kBM) >> 4) << 24);
-}
-
 // The k-th piece of work of a CTA pair.  Full rounds: item = cluster + k * n_clusters over all K chunks.  Then, if the last round
 // is partial (tail_splits > 1), ONE K range [c0, c1) of a tail item, so that round costs ~1/tail_splits of a full one; its fp32
 // partial tile goes through the split-K workspace and the last pair to arrive sums the ranges in order 0..S-1 (deterministic).

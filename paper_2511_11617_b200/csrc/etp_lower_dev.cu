@@ -372,7 +372,7 @@ etp_status copy_intervals_device(etp_ctx* c, const etp_interval* host_descs, int
             a.small_first = s.d_small_first;
             a.dev_counts = s.d_counts;
             a.counters = s.d_counts + 3;
-            a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
+            a.flags = (c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u) | (c->opts[ETP_OPT_SMALL_STAGED] ? 2u : 0u);
             if (timed) {
                 while ((int)S->timing.size() < 2 * (S->n_timed + 1)) {
                     cudaEvent_t e;

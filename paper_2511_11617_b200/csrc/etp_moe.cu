@@ -37,9 +37,11 @@ static_assert(sizeof(MoeItem) == 32, "MoeItem layout");
 
 struct alignas(64) MoeParams {
     CUtensorMap map_x;
+    CUtensorMap map_xh[8];          // CTA-pair kernel: the same X with boxes of 16, 32, .. 128 rows (one TMA per half tile)
     CUtensorMap map_w[kMaxRuns];    // per rank (gate, in the fused kernel)
     CUtensorMap map_w2[kMaxRuns];   // fused kernel: up
     const MoeItem* items;
+    const int32_t* first;                     // CTA-pair kernel: cluster c runs items [first[c], first[c + 1]) of `items`
     int32_t n_items, mode, dtype, n_chunks;   // n_chunks: K chunks of kBK per item
     int32_t out_features, n_maps;
     void* y;
@@ -236,6 +238,272 @@ __global__ void __launch_bounds__(kLinThreads, 1) etp_moe_linear_kernel(const __
     }
 }
 
+// ------------------------------------------------------------------------------------------------ CTA-pair kernel
+// Many routed rows per expert: the single-CTA kernel above is bound by what an SM can pull from L2 (the chip-wide L2 output of
+// ~6300 B/clk is ~42 B/clk per SM; a fused item stages 32 KiB of weights + 16 KiB of X per K chunk for 2 x 128 x 128 x 64 MACs).
+// Two CTAs of a cluster run ONE tcgen05.mma.cta_group::2 of M = 256 out features x N <= 256 routed rows: CTA rank c owns out
+// feature tile 2 * pm + c (its A tile(s), its 128 TMEM lanes) and stages HALF of the X rows, so the same MACs need 48 KiB per CTA
+// for twice the rows (fused: 171 flop per staged byte instead of 85).  N is the item's row count rounded up to 32; each CTA
+// loads its N / 2 rows with ONE TMA (eight X maps with boxes of 16 .. 128 rows).  Protocol as etp_shard_linear_pair_kernel: both CTAs' TMA loads complete on the LEADER's full
+// barrier, only the leader issues MMAs, tcgen05.commit multicasts "stage free" / "accumulator ready" to both CTAs, the epilogue
+// warps of both arrive on the leader's "accumulator drained" barrier.  The fused kernel holds gate and up for 256 rows in all
+// 512 TMEM columns (one accumulator stage: its epilogue is not overlapped with the next item's MMAs); the plain kernel keeps two
+// stages of 256 columns.  Work: cluster c runs items [first[c], first[c + 1]) - a list schedule computed on the host from a cost
+// model, in instance order so that the items sharing an X tile or an expert's weights run at about the same time (L2 hits).
+template <bool FUSED>
+struct MoePairCfg {
+    static constexpr int kBN = 256;
+    static constexpr int kAStage = FUSED ? 2 * kABytes : kABytes;
+    static constexpr int kBBytes = (kBN / 2) * kBK * 2;
+    static constexpr int kStageBytes = kAStage + kBBytes;
+    static constexpr int kStages = (kSmemBudget / kStageBytes) > 8 ? 8 : (kSmemBudget / kStageBytes);
+    static constexpr int kAccCols = FUSED ? 2 * kBN : kBN;
+    static constexpr int kAccStages = FUSED ? 1 : 2;
+    static constexpr int kTmemCols = 512;
+    static constexpr int kThreads = 320;                             // TMA warp, MMA warp, 8 epilogue warps
+    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 + 256 + 8192;
+};
+
+#ifdef ETP_MOE_TIMING
+// bring-up instrumentation (never in the product build): per cluster, sums of SM clocks
+__device__ unsigned long long g_moe_t[128][8];
+#define MOE_T(slot, expr) do { if (rank == 0) atomicAdd(&g_moe_t[cluster_id][slot], (unsigned long long)(expr)); } while (0)
+#define MOE_CLK() clock64()
+#else
+#define MOE_T(slot, expr) do { } while (0)
+#define MOE_CLK() 0ll
+#endif
+
+template <typename OutT, bool FUSED>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(MoePairCfg<FUSED>::kThreads, 1) etp_moe_pair_kernel(const __grid_constant__ MoeParams p) {
+    using C = MoePairCfg<FUSED>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + C::kStages * C::kStageBytes);
+    uint64_t* empty_bar = full_bar + C::kStages;
+    uint64_t* tmem_full = empty_bar + C::kStages;
+    uint64_t* tmem_empty = tmem_full + 2;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int cluster_id = blockIdx.x >> 1;
+    const bool row_par = !FUSED && p.mode == ETP_ROW_PARALLEL;
+    const int i_begin = __ldg(&p.first[cluster_id]), i_end = __ldg(&p.first[cluster_id + 1]);
+    const long long t_kernel0 = MOE_CLK();
+    (void)t_kernel0;
+
+    if (warp == 0 && lane == 1) {
+        for (int r = 0; r < 8; ++r) prefetch_tensormap(&p.map_xh[r]);
+        for (int r = 0; r < p.n_maps; ++r) {
+            prefetch_tensormap(&p.map_w[r]);
+            if (FUSED) prefetch_tensormap(&p.map_w2[r]);
+        }
+    }
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < C::kStages; ++s) {
+            mbar_init(&full_bar[s], 1);      // used in the leader only: its own arrive.expect_tx of both CTAs' bytes
+            mbar_init(&empty_bar[s], 1);     // one multicast commit per use
+        }
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&tmem_full[s], 1);     // one multicast commit per item
+            mbar_init(&tmem_empty[s], 16);   // leader only: 8 epilogue warps of each CTA
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_ptr)), "r"(uint32_t(C::kTmemCols))
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();      // the peer's barriers exist before anything signals them
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+
+    if (warp == 0) {
+        if (lane == 0) {   // ------------------------------------------------------------------ TMA producer (one lane of each CTA)
+            int stage = 0;
+            uint32_t phase = 0;
+            MoeItem nxt = i_begin < i_end ? load_item(p.items, i_begin) : MoeItem{};
+            for (int i = i_begin; i < i_end; ++i) {
+                const MoeItem it = nxt;
+                if (i + 1 < i_end) nxt = load_item(p.items, i + 1);         // in flight while this item's tiles are requested
+                const int h = ((it.n_rows + 31) >> 5) << 4;                 // N = 2 h (a multiple of 32); this CTA stages rows [x0, x0 + h)
+                const int x0 = it.x_row + int(rank) * h;
+                const CUtensorMap* mx = &p.map_xh[(h >> 4) - 1];
+                const int a_row = row_par ? it.a_row : it.a_row + int(rank) * kBM;
+                const int m0 = it.m0 + int(rank) * kBM;
+                for (int c = 0; c < p.n_chunks; ++c) {
+                    uint8_t* sa = smem + stage * C::kStageBytes;
+                    uint8_t* sb = sa + C::kAStage;
+                    const long long tp0 = MOE_CLK();
+                    mbar_wait(&empty_bar[stage], phase ^ 1);
+                    MOE_T(0, MOE_CLK() - tp0);
+                    const uint32_t lbar = mapa_rank0(smem_u32(&full_bar[stage]));
+                    if (rank == 0) mbar_expect_tx(&full_bar[stage], 2u * uint32_t(C::kAStage + h * kBK * 2));
+                    if (!row_par) {
+                        tma_load_2d_pair(sa, &p.map_w[it.map], lbar, c * kBK, a_row);
+                        if (FUSED) tma_load_2d_pair(sa + kABytes, &p.map_w2[it.map], lbar, c * kBK, a_row);
+                    } else {
+                        tma_load_2d_pair(sa, &p.map_w[it.map], lbar, m0, a_row + c * kBK);
+                        tma_load_2d_pair(sa + kABytes / 2, &p.map_w[it.map], lbar, m0 + 64, a_row + c * kBK);
+                    }
+                    tma_load_2d_pair(sb, mx, lbar, c * kBK, x0);
+                    if (++stage == C::kStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 1) {
+        if (lane == 0 && rank == 0) {   // ------------------------------------------------------ MMA issuer (one lane of the LEADER)
+            const uint32_t a_lbo = row_par ? uint32_t(kABytes / 2) : 16u;
+            const uint32_t a_kstep = row_par ? (uint32_t(kUmmaK) * 128u) >> 4 : (uint32_t(kUmmaK) * 2u) >> 4;
+            int stage = 0;
+            uint32_t phase = 0;
+            int local = 0;
+            int n_rows_next = i_begin < i_end ? __ldg(&p.items[i_begin].n_rows) : 0;
+            for (int i = i_begin; i < i_end; ++i, ++local) {
+                const int n_rows = n_rows_next;
+                if (i + 1 < i_end) n_rows_next = __ldg(&p.items[i + 1].n_rows);   // in flight while this item's MMAs are issued
+                const uint32_t idesc = make_idesc_pair(p.dtype == ETP_BF16 ? 1u : 0u, row_par ? 1u : 0u, uint32_t(((n_rows + 31) >> 5) << 5));
+                const int as = local % C::kAccStages;
+                const uint32_t aph = uint32_t(local / C::kAccStages) & 1u;
+                const long long tm0 = MOE_CLK();
+                mbar_wait(&tmem_empty[as], aph ^ 1);   // both CTAs' epilogues have drained this accumulator stage
+                MOE_T(1, MOE_CLK() - tm0);
+                MOE_T(4, 1);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + uint32_t(as * C::kAccCols);
+                for (int c = 0; c < p.n_chunks; ++c) {
+                    uint8_t* sa = smem + stage * C::kStageBytes;
+                    const long long tm1 = MOE_CLK();
+                    mbar_wait(&full_bar[stage], phase);
+                    MOE_T(c < C::kStages ? 2 : 3, MOE_CLK() - tm1);
+                    tc_fence_after();
+                    const uint64_t a_desc = make_smem_desc(smem_u32(sa), a_lbo, 1024);
+                    const uint64_t b_desc = make_smem_desc(smem_u32(sa + C::kAStage), 16, 1024);
+#pragma unroll
+                    for (int k = 0; k < kBK / kUmmaK; ++k)
+                        tc_mma_pair(d_tmem, a_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > 0 || k > 0) ? 1u : 0u);
+                    if (FUSED) {
+                        const uint64_t a2_desc = make_smem_desc(smem_u32(sa + kABytes), a_lbo, 1024);
+#pragma unroll
+                        for (int k = 0; k < kBK / kUmmaK; ++k)
+                            tc_mma_pair(d_tmem + uint32_t(C::kBN), a2_desc + uint64_t(k) * a_kstep, b_desc + uint64_t(k) * 2u, idesc, (c > 0 || k > 0) ? 1u : 0u);
+                    }
+                    tc_commit_pair(&empty_bar[stage]);   // frees the stage in BOTH CTAs once these MMAs have read it
+                    if (++stage == C::kStages) { stage = 0; phase ^= 1; }
+                }
+                tc_commit_pair(&tmem_full[as]);
+            }
+        }
+        __syncwarp();
+    } else {               // ---------------------------------------------------------------------- epilogue warps 2..9 of both CTAs
+        // Two warps per TMEM lane quarter (a warp may only read lanes 32 * (warp % 4) ..): warp `half` of a quarter takes the column
+        // blocks half, half + 2, ... of kStep routed rows.  The tcgen05.ld of the next block are in flight while the current one
+        // goes through the activation, the transpose buffer and the 16-byte stores.
+        const int q = warp & 3, half = (warp - 2) >> 2;
+        OutT* y = reinterpret_cast<OutT*>(p.y);
+        OutT* stage_t = reinterpret_cast<OutT*>(smem + C::kStages * C::kStageBytes + 256) + (warp - 2) * 512;   // [16 rows][32 features]
+        const uint32_t drained = mapa_rank0(smem_u32(&tmem_empty[0]));
+        constexpr int kStep = FUSED ? 32 : 64;
+        int local = 0;
+        for (int i = i_begin; i < i_end; ++i, ++local) {
+            const MoeItem it = load_item(p.items, i);
+            const int as = local % C::kAccStages;
+            const uint32_t aph = uint32_t(local / C::kAccStages) & 1u;
+            const int m0 = it.m0 + int(rank) * kBM;
+            const int valid = it.valid - int(rank) * kBM;   // <= 0: this CTA's tile lies past the last out feature
+            mbar_wait(&tmem_full[as], aph);
+            const long long te0 = MOE_CLK();
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + uint32_t(as * C::kAccCols) + (uint32_t(q * 32) << 16);
+            auto load_blk = [&](int c0, uint32_t (&v)[4][16]) {
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                    const int col = FUSED ? c0 + 16 * (g & 1) : c0 + 16 * g;   // fused: g = 0, 1 gate columns, g = 2, 3 the same columns of up
+                    if (col < it.n_rows) tc_ld16(taddr + uint32_t(col) + (FUSED && g >= 2 ? uint32_t(C::kBN) : 0u), v[g]);
+                }
+            };
+            auto emit_blk = [&](int c0, const uint32_t (&v)[4][16]) {
+#pragma unroll
+                for (int g = 0; g < (FUSED ? 2 : 4); ++g) {
+                    const int col = c0 + 16 * g;
+                    if (col < it.n_rows) {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const float r = FUSED ? silu_mul(__uint_as_float(v[g][j]), __uint_as_float(v[g + 2][j])) : __uint_as_float(v[g][j]);
+                            stage_t[j * 32 + lane] = cvt16<OutT>(r);
+                        }
+                        __syncwarp();
+#pragma unroll
+                        for (int hh = 0; hh < 2; ++hh) {
+                            const int row = hh * 8 + (lane >> 2), chunk = lane & 3;
+                            const int tok = col + row;
+                            const uint4 val = *reinterpret_cast<const uint4*>(stage_t + row * 32 + chunk * 8);
+                            if (tok < it.n_rows && q * 32 + chunk * 8 < valid)
+                                *reinterpret_cast<uint4*>(y + size_t(it.x_row + tok) * p.out_features + m0 + q * 32 + chunk * 8) = val;
+                        }
+                        __syncwarp();
+                    }
+                }
+            };
+            int c0 = half * kStep;
+            if (q * 32 < valid && c0 < it.n_rows) {
+                uint32_t va[4][16], vb[4][16];
+                load_blk(c0, va);
+                tc_ld_wait();
+                for (;;) {
+                    const int c1 = c0 + 2 * kStep;
+                    if (c1 < it.n_rows) load_blk(c1, vb);
+                    emit_blk(c0, va);
+                    if (c1 >= it.n_rows) break;
+                    tc_ld_wait();
+                    c0 = c1 + 2 * kStep;
+                    if (c0 < it.n_rows) load_blk(c0, va);
+                    emit_blk(c1, vb);
+                    if (c0 >= it.n_rows) break;
+                    tc_ld_wait();
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(drained + uint32_t(as) * 8u);
+            if (warp == 2 && lane == 0) MOE_T(5, MOE_CLK() - te0);
+        }
+    }
+    if (threadIdx.x == 0) MOE_T(6, MOE_CLK() - t_kernel0);
+
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();      // the leader's MMAs read the peer's shared memory and both CTAs free the paired TMEM
+    if (warp == 1) {
+        __syncwarp();
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(uint32_t(C::kTmemCols)) : "memory");
+    }
+}
+
+template <typename OutT, bool FUSED>
+etp_status launch_moe_pair_t(const MoeParams& p, int grid, cudaStream_t stream) {
+    using C = MoePairCfg<FUSED>;
+    auto k = etp_moe_pair_kernel<OutT, FUSED>;
+    static bool configured = false;
+    if (!configured) {
+        ETP_CUDA_OK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes));
+        configured = true;
+    }
+    k<<<grid, C::kThreads, C::kSmemBytes, stream>>>(p);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) ETP_FAIL(ETP_ERR_CUDA, "etp_moe_linear: pair launch failed: %s", cudaGetErrorString(e));
+    return ETP_OK;
+}
+template <bool FUSED>
+etp_status launch_moe_pair(const MoeParams& p, int grid, cudaStream_t st) {
+    return p.dtype == ETP_BF16 ? launch_moe_pair_t<__nv_bfloat16, FUSED>(p, grid, st) : launch_moe_pair_t<__half, FUSED>(p, grid, st);
+}
+
 template <int BN, typename OutT, bool FUSED>
 etp_status launch_moe_t(const MoeParams& p, int grid, cudaStream_t stream) {
     using C = MoeCfg<BN, FUSED>;
@@ -356,47 +624,113 @@ etp_status moe_run(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtype, const vo
         }
     }
 
+    // ---- CTA pairs when the row tiles are large (ETP_OPT_MOE_CTA_PAIR: 1 = when the cost model above picked >= 128 rows,
+    // 2 = always, 0 = never)
+    const int64_t pair_opt = ctx->opts[ETP_OPT_MOE_CTA_PAIR];
+    const bool pair = ctx->n_sms >= 2 && (pair_opt == 2 || (pair_opt == 1 && bn >= 128));
+
     // ---- items: (instance, row tile, m tile), m tiles of one row tile adjacent so that its X tile stays in L2
-    const int64_t m_tiles = (out_features + kBM - 1) / kBM;
+    // Pair kernel: an instance with c rows gets ceil(c / 256) row tiles of EQUAL size (rounded up to 32 rows) - a 296-row expert
+    // runs 160 + 136 rows, not 256 + 40: every tile re-streams the expert's weights, and a 40-row tile would do so for a quarter of
+    // the MMA work of a full one (it is bound by the weight fetch, not by the MMA).
+    const int m_step = pair ? 2 * kBM : kBM;
+    const int64_t m_tiles = (out_features + m_step - 1) / m_step;
     std::vector<MoeItem> items;
     for (const Inst& in : insts) {
-        for (int64_t t = in.row_b; t < in.row_e; t += bn)
+        const int64_t c_rows = in.row_e - in.row_b;
+        int64_t row_step = bn;
+        if (pair) {
+            const int64_t tiles = (c_rows + 255) / 256;
+            row_step = ((c_rows + tiles - 1) / tiles + 31) / 32 * 32;
+        }
+        for (int64_t t = in.row_b; t < in.row_e; t += row_step)
             for (int64_t mt = 0; mt < m_tiles; ++mt) {
                 MoeItem it{};
                 it.map = map_of[in.rank];
-                it.m0 = int32_t(mt * kBM);
-                it.valid = int32_t(std::min<int64_t>(kBM, out_features - mt * kBM));
-                it.a_row = int32_t(row_par ? in.slot * rows_per_expert : in.slot * rows_per_expert + mt * kBM);
+                it.m0 = int32_t(mt * m_step);
+                it.valid = int32_t(std::min<int64_t>(m_step, out_features - mt * m_step));
+                it.a_row = int32_t(row_par ? in.slot * rows_per_expert : in.slot * rows_per_expert + mt * m_step);
                 it.x_row = int32_t(t);
-                it.n_rows = int32_t(std::min<int64_t>(bn, in.row_e - t));
+                it.n_rows = int32_t(std::min<int64_t>(row_step, in.row_e - t));
                 items.push_back(it);
             }
     }
     if (items.empty()) return ETP_OK;
     if (items.size() >= (size_t(1) << 31)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_moe_linear: too many work items");
+    const int32_t n_chunks = int32_t((in_features + kBK - 1) / kBK);
+
+    // ---- pair kernel: list schedule.  Items are dealt in order to the cluster with the least accumulated cost (what a work queue
+    // would do, decided here so that the two CTAs of a cluster need no exchange); cost of an item in SM clocks = the larger of its
+    // operand fetch (~55 B/clk per SM sustained from L2, measured on kernel (c)'s pair kernel) and its MMA time (N / 2 clk per
+    // UMMA_K step), plus the epilogue where it is not overlapped (fused: one accumulator stage; ~22 clk per row, from ncu's
+    // tensor-pipe-active share), plus a fixed per-item cost (pipeline refill, descriptor fetch).
+    std::vector<int32_t> first;
+    int n_clusters = 0;
+    if (pair) {
+        n_clusters = int(std::min<int64_t>(int64_t(items.size()), ctx->n_sms / 2));
+        std::vector<int64_t> load(size_t(n_clusters), 0);
+        std::vector<int32_t> owner(items.size());
+        const int64_t a_stage = fused ? 2 * kABytes : kABytes;
+        for (size_t i = 0; i < items.size(); ++i) {
+            const int64_t h = (items[i].n_rows + 31) / 32 * 16;   // rows staged per CTA; UMMA_N = 2 h
+            const int64_t fetch = (a_stage + h * kBK * 2) * n_chunks / 55;
+            const int64_t mma = int64_t(n_chunks) * (kBK / kUmmaK) * (fused ? 2 : 1) * h;
+            const int64_t epi = int64_t(items[i].n_rows) * (fused ? 22 : 11);
+            const int64_t cost = (fused ? std::max(fetch, mma) + epi : std::max(std::max(fetch, mma), epi)) + 1000;
+            int best = 0;
+            for (int c = 1; c < n_clusters; ++c)
+                if (load[size_t(c)] < load[size_t(best)]) best = c;
+            owner[i] = best;
+            load[size_t(best)] += cost;
+        }
+        first.assign(size_t(n_clusters) + 1, 0);
+        for (size_t i = 0; i < items.size(); ++i) ++first[size_t(owner[i]) + 1];
+        for (int c = 0; c < n_clusters; ++c) first[size_t(c) + 1] += first[size_t(c)];
+        std::vector<int32_t> cursor(first.begin(), first.end() - 1);
+        std::vector<MoeItem> sorted(items.size());
+        for (size_t i = 0; i < items.size(); ++i) sorted[size_t(cursor[size_t(owner[i])]++)] = items[i];
+        items.swap(sorted);
+    }
 
     ETP_CUDA_OK(cudaSetDevice(ctx->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t need = items.size() * sizeof(MoeItem);
+    // table = [first[] padded to 32 bytes][items]; one stream-ordered allocation, one upload
+    const size_t head = (first.size() * sizeof(int32_t) + 31) / 32 * 32;
+    const size_t need = head + items.size() * sizeof(MoeItem);
+    std::vector<uint8_t> table(need, 0);
+    if (!first.empty()) std::memcpy(table.data(), first.data(), first.size() * sizeof(int32_t));
+    std::memcpy(table.data() + head, items.data(), items.size() * sizeof(MoeItem));
     void* d_items = nullptr;
     ETP_CUDA_OK(cudaMallocAsync(&d_items, need, st));   // stream-ordered: nothing is shared between calls or streams
-    cudaError_t e = cudaMemcpyAsync(d_items, items.data(), need, cudaMemcpyHostToDevice, st);   // pageable source: staged before return
+    cudaError_t e = cudaMemcpyAsync(d_items, table.data(), need, cudaMemcpyHostToDevice, st);   // pageable source: staged before return
     if (e != cudaSuccess) {
         cudaFreeAsync(d_items, st);
         ETP_FAIL(ETP_ERR_CUDA, "etp_moe_linear: uploading the item table failed: %s", cudaGetErrorString(e));
     }
-    p.items = static_cast<const MoeItem*>(d_items);
+    p.first = static_cast<const int32_t*>(d_items);
+    p.items = reinterpret_cast<const MoeItem*>(static_cast<const uint8_t*>(d_items) + head);
     p.n_items = int32_t(items.size());
     p.mode = mode;
     p.dtype = dtype;
-    p.n_chunks = int32_t((in_features + kBK - 1) / kBK);
+    p.n_chunks = n_chunks;
     p.out_features = int32_t(out_features);
     p.n_maps = n_maps;
     p.y = y_perm;
-    etp_status s = encode_2d(&p.map_x, dtype, x_perm, n_rows, in_features, in_features, kBK, std::min(bn, 64));
-    const int grid = int(std::min<int64_t>(p.n_items, ctx->n_sms));
+    etp_status s = ETP_OK;
+    if (pair) {
+        for (int r = 0; r < 8 && s == ETP_OK; ++r) s = encode_2d(&p.map_xh[r], dtype, x_perm, n_rows, in_features, in_features, kBK, 16 * (r + 1));
+    } else {
+        s = encode_2d(&p.map_x, dtype, x_perm, n_rows, in_features, in_features, kBK, std::min(bn, 64));
+    }
     ctx->launches = 1;
-    if (s == ETP_OK) s = fused ? launch_moe<true>(p, bn, grid, st) : launch_moe<false>(p, bn, grid, st);
+    if (s == ETP_OK) {
+        if (pair) {
+            s = fused ? launch_moe_pair<true>(p, 2 * n_clusters, st) : launch_moe_pair<false>(p, 2 * n_clusters, st);
+        } else {
+            const int grid = int(std::min<int64_t>(p.n_items, ctx->n_sms));
+            s = fused ? launch_moe<true>(p, bn, grid, st) : launch_moe<false>(p, bn, grid, st);
+        }
+    }
     cudaFreeAsync(d_items, st);
     return s;
 }
@@ -550,3 +884,14 @@ extern "C" etp_status etp_eplb_apply(etp_ctx* ctx, const etp_tensor* tensors, in
     w.rep.n_phases = 1;
     return execute(ctx, &w, stream, stream, nullptr);
 }
+
+#ifdef ETP_MOE_TIMING
+extern "C" void etp_moe_timing_dump(unsigned long long* out, int reset) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out, g_moe_t, sizeof(unsigned long long) * 128 * 8);
+    if (reset) {
+        static unsigned long long z[128 * 8];
+        cudaMemcpyToSymbol(g_moe_t, z, sizeof(z));
+    }
+}
+#endif

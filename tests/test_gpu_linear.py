@@ -302,10 +302,21 @@ def test_moe_layer_on_resharded_experts(ctx):
     (4, 8, 128, 256, 2, (3, 3, 2), "tight"),          # a few rows per expert: 16-row tiles, experts without rows
     (300, 6, 192, 320, 3, (2, 1, 3), "wrap"),         # F not a multiple of 128 (a tile runs into the next expert's rows), wrapped shards
     (1500, 5, 256, 136, 2, (5,), "tight"),            # > 256 rows per expert: several row tiles; K tail (136 = 2 chunks + 8)
+    (900, 4, 384, 192, 2, (1, 2, 1), "wrap"),         # 3 feature tiles: the second CTA pair has one tile past the last feature
 ])
-def test_moe_linear_grouped_vs_reference(ctx, T, E, F, Hd, top_k, widths, gmode):
+@pytest.mark.parametrize("moe_pair", [0, 1, 2])
+def test_moe_linear_grouped_vs_reference(ctx, T, E, F, Hd, top_k, widths, gmode, moe_pair):
     """etp_moe_linear on synthetic expert tensors (NaN-filled slack slots): every row of the column-parallel (gate-like) and
-    row-parallel (down-like) grouped outputs against the fp64 product with ITS expert's unsharded matrix."""
+    row-parallel (down-like) grouped outputs against the fp64 product with ITS expert's unsharded matrix.  moe_pair: single-CTA
+    tiles only / the library's choice / CTA pairs (cta_group::2) forced even for a few rows."""
+    ctx.set_option(etp.OPT_MOE_CTA_PAIR, moe_pair)
+    try:
+        _moe_linear_grouped(ctx, T, E, F, Hd, top_k, widths, gmode)
+    finally:
+        ctx.set_option(etp.OPT_MOE_CTA_PAIR, 1)
+
+
+def _moe_linear_grouped(ctx, T, E, F, Hd, top_k, widths, gmode):
     dt = torch_dtype("bf16")
     rng = np.random.default_rng(T + E)
     layout = widths_to_layout(widths)
@@ -570,11 +581,21 @@ def _moe_world(E, F, Hd, widths, slack, seed_i):
     ((0, 3, 17, 0, 1, 40), 6, 128, 256, (2, 2, 2)),           # 16-row tiles, experts without rows
     ((130, 64, 257, 5), 4, 192, 320, (1, 3)),                 # F not a multiple of 128: tiles run into the next slot; 128-row tiles
     ((300, 900), 2, 256, 136, (2,)),                          # several row tiles per expert; K tail
+    ((256, 257, 0, 64, 321), 5, 384, 192, (2, 3)),            # 3 feature tiles (odd: half a CTA pair is idle), rows around the 256 / 64 edges
 ])
-def test_moe_gate_up_fused_matches_fp64_swiglu(ctx, rows_per_expert, E, F, Hd, widths):
+@pytest.mark.parametrize("moe_pair", [0, 1, 2])
+def test_moe_gate_up_fused_matches_fp64_swiglu(ctx, rows_per_expert, E, F, Hd, widths, moe_pair):
     """etp_moe_gate_up: h = silu(gate x) * (up x) in one launch (two TMEM accumulators, activation in the epilogue), every row
     against oracle.linear.swiglu_ref in fp64 - fp32 accumulation and ONE 16-bit rounding, so the error is at most one rounding
-    (tighter than the three-launch layer, which rounds gate and up to 16 bit first)."""
+    (tighter than the three-launch layer, which rounds gate and up to 16 bit first).  moe_pair as in the test above."""
+    ctx.set_option(etp.OPT_MOE_CTA_PAIR, moe_pair)
+    try:
+        _moe_gate_up_fused(ctx, rows_per_expert, E, F, Hd, widths)
+    finally:
+        ctx.set_option(etp.OPT_MOE_CTA_PAIR, 1)
+
+
+def _moe_gate_up_fused(ctx, rows_per_expert, E, F, Hd, widths):
     ws, descs, layout, geom, bufs = _moe_world(E, F, Hd, widths, 1, E)
     offs = np.concatenate([[0], np.cumsum(rows_per_expert)]).astype(np.int64)
     R = int(offs[-1])

@@ -456,9 +456,19 @@ def test_copy_intervals_bit_exact(ctx, n, hi, tma_min):
 
 
 @pytest.mark.parametrize("size,n", [(16, 5000), (256, 4099), (4096, 777), (32768, 65)])
-def test_copy_intervals_small_batches(ctx, size, n):
+@pytest.mark.parametrize("staged", [1, 0])
+def test_copy_intervals_small_batches(ctx, size, n, staged):
     """The descriptor-bound corner of config 5b: every interval the same small size, so every vector work item is a
-    batch of up to 128 intervals (or 32 KiB) walked with the shuffle search; ragged last batch, last round and last word."""
+    batch of up to 128 intervals (or 32 KiB): staged through the idle ring with per-lane bulk copies (ETP_OPT_SMALL_STAGED, the
+    default when a launch has no bulk intervals) or walked with the shuffle search; ragged last batch, last round and last word."""
+    ctx.set_option(etp.OPT_SMALL_STAGED, staged)
+    try:
+        _small_batches(ctx, size, n)
+    finally:
+        ctx.set_option(etp.OPT_SMALL_STAGED, 1)
+
+
+def _small_batches(ctx, size, n):
     rng = np.random.default_rng(size + n)
     src_arena = 8 << 20
     src = rng.integers(0, 256, src_arena, dtype=np.uint8)
