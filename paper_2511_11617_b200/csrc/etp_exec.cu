@@ -110,7 +110,7 @@ extern "C" etp_status etp_ctx_create_multi(const int32_t* devices, int32_t n_dev
     c->opts[ETP_OPT_LINEAR_RING] = 2;
     c->opts[ETP_OPT_ONLY_PHASE] = 0;
     c->opts[ETP_OPT_MOE_CTA_PAIR] = 1;
-    c->opts[ETP_OPT_SMALL_STAGED] = 0;
+    c->opts[ETP_OPT_SMALL_STAGED] = 1;
     CtxExtra* x = new (std::nothrow) CtxExtra();
     if (!x) { delete c; ETP_FAIL(ETP_ERR_NOMEM, "etp_ctx_create: out of memory"); }
     c->impl = x;
