@@ -367,7 +367,7 @@ __device__ __forceinline__ void gen_advance(SmallGen& g, const SmallSeg* small, 
     g.valid = true;
 }
 
-__device__ void copy_small_batch_staged(const CopyArgs& a, unsigned int k, int lane, uint8_t* stage_mem, uint64_t* bars, uint32_t& gb) {
+__device__ uint32_t copy_small_batch_staged(const CopyArgs& a, unsigned int k, int lane, uint8_t* stage_mem, uint64_t* bars, uint32_t gb) {
     SmallGen lead, lag;
     lead.s = lag.s = __ldg(a.small_first + k);
     lead.s1 = lag.s1 = __ldg(a.small_first + k + 1);
@@ -411,12 +411,13 @@ __device__ void copy_small_batch_staged(const CopyArgs& a, unsigned int k, int l
         }
         if (!did) break;
     }
-    gb += issued;
+    return gb + issued;
 }
 
+template <bool STAGED>
 __device__ void vector_warp(const CopyArgs& a, int lane, uint8_t* stage_mem, uint64_t* bars) {
     const unsigned int n_items = a.n_vec_items + a.n_small_batches;
-    const bool staged = stage_mem != nullptr;   // warp-uniform: the ring is idle (no bulk items) and the option is on
+    constexpr bool staged = STAGED;             // the host launches this instantiation only when the ring is idle (no bulk items)
     uint32_t gb = 0;                            // blocks this warp has pushed through its stages (stage = gb % kSmStages)
     if (staged) {
         if (lane == 0) {
@@ -433,8 +434,8 @@ __device__ void vector_warp(const CopyArgs& a, int lane, uint8_t* stage_mem, uin
         if (idx >= n_items) break;
         if (idx < a.n_vec_items)
             copy_vec_item(a, idx, lane);
-        else if (staged)
-            copy_small_batch_staged(a, idx - a.n_vec_items, lane, stage_mem, bars, gb);
+        else if constexpr (staged)
+            gb = copy_small_batch_staged(a, idx - a.n_vec_items, lane, stage_mem, bars, gb);
         else
             copy_small_batch(a, idx - a.n_vec_items, lane);
     }
@@ -453,6 +454,10 @@ __device__ void vector_warp(const CopyArgs& a, int lane, uint8_t* stage_mem, uin
     }
 }
 
+// STAGED = false is the kernel of the reshard path (and of every launch with bulk intervals); STAGED = true is launched by the host when
+// a launch has small batches and NO bulk items: the ring belongs to the vector warps (copy_small_batch_staged).  Two instantiations, so
+// that the staged code does not perturb the register allocation of the head-strided KV path (it cost that launch 5 % when inlined).
+template <bool STAGED>
 __global__ void __launch_bounds__(kCopyThreads, 1) etp_interval_copy_kernel(const CopyArgs args) {
     extern __shared__ __align__(1024) uint8_t smem[];
     CopyArgs a = args;
@@ -467,27 +472,31 @@ __global__ void __launch_bounds__(kCopyThreads, 1) etp_interval_copy_kernel(cons
     uint32_t* s_bytes = reinterpret_cast<uint32_t*>(s_dst + kStages);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp == 0) {
-        if (lane == 0) {
+        if (!STAGED && lane == 0) {
             for (int s = 0; s < kStages; ++s) mbar_init(smem_u32(&full_bar[s]), 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             tma_driver(a, ring, full_bar, s_dst, s_bytes);
         }
     } else {
-        const bool staged = (a.flags & 2u) && a.n_bulk_items == 0 && a.n_small_batches != 0;
         uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)kStages * kStageBytes + 128) + (warp - 1) * kSmStages;
-        vector_warp(a, lane, staged ? ring + (size_t)(warp - 1) * kSmWarpBytes : nullptr, bars);
+        vector_warp<STAGED>(a, lane, STAGED ? ring + (size_t)(warp - 1) * kSmWarpBytes : nullptr, bars);
     }
 }
 
 }  // namespace
 
 cudaError_t configure_copy_kernel() {
-    return cudaFuncSetAttribute(etp_interval_copy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCopySmemBytes);
+    cudaError_t e = cudaFuncSetAttribute(etp_interval_copy_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCopySmemBytes);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(etp_interval_copy_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCopySmemBytes);
 }
 
-void launch_copy_kernel(const CopyArgs& a, int grid, cudaStream_t stream) {
-    etp_interval_copy_kernel<<<grid, kCopyThreads, kCopySmemBytes, stream>>>(a);
+void launch_copy_kernel(const CopyArgs& a, int grid, cudaStream_t stream, bool staged_small) {
+    if (staged_small)
+        etp_interval_copy_kernel<true><<<grid, kCopyThreads, kCopySmemBytes, stream>>>(a);
+    else
+        etp_interval_copy_kernel<false><<<grid, kCopyThreads, kCopySmemBytes, stream>>>(a);
 }
 
 }  // namespace etp

@@ -33,11 +33,12 @@ struct CopyArgs {
     const unsigned int* dev_counts;   // != NULL: {n_bulk_items, n_vec_items, n_small_batches} live on the device (descriptors
                                       // lowered by the device-side classifier, etp_lower_dev.cu) and override the three above
     unsigned int* counters;       // [0] bulk head, [1] vec head (zeroed before launch)
-    unsigned int flags;           // bit 0: vector warps also drain the bulk queue when theirs is empty; bit 1: small batches may be
-                                  // staged through the ring when the launch has no bulk items (ETP_OPT_SMALL_STAGED)
+    unsigned int flags;           // bit 0: vector warps also drain the bulk queue when theirs is empty
 };
 
-void launch_copy_kernel(const CopyArgs& a, int grid, cudaStream_t stream);
+// staged_small: the launch has small batches and NO bulk items and ETP_OPT_SMALL_STAGED is on -> the instantiation whose vector warps
+// stage small batches through the (idle) ring
+void launch_copy_kernel(const CopyArgs& a, int grid, cudaStream_t stream, bool staged_small = false);
 cudaError_t configure_copy_kernel();
 
 }  // namespace etp

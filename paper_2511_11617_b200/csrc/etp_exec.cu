@@ -425,7 +425,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
                 a.n_small_batches = (unsigned int)jl.small_first.size();
                 a.dev_counts = nullptr;
                 a.counters = (unsigned int*)(P.d_base + P.off_counters) + 2 * P.counter_slot;
-                a.flags = (c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u) | (c->opts[ETP_OPT_SMALL_STAGED] ? 2u : 0u);
+                a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
                 if (timed) {
                     while ((int)D.tev.size() < 2 * (D.n_timed + 1)) {
                         cudaEvent_t e;
@@ -434,7 +434,7 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
                     }
                     ETP_CUDA_OK(cudaEventRecord(D.tev[2 * D.n_timed], cs));
                 }
-                launch_copy_kernel(a, grid, cs);
+                launch_copy_kernel(a, grid, cs, c->opts[ETP_OPT_SMALL_STAGED] && jl.n_bulk_items == 0 && !jl.small_first.empty());
                 ETP_CUDA_OK(cudaGetLastError());
                 if (timed) {
                     ETP_CUDA_OK(cudaEventRecord(D.tev[2 * D.n_timed + 1], cs));

@@ -372,7 +372,7 @@ etp_status copy_intervals_device(etp_ctx* c, const etp_interval* host_descs, int
             a.small_first = s.d_small_first;
             a.dev_counts = s.d_counts;
             a.counters = s.d_counts + 3;
-            a.flags = (c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u) | (c->opts[ETP_OPT_SMALL_STAGED] ? 2u : 0u);
+            a.flags = c->opts[ETP_OPT_LDG_STEALS_BULK] ? 1u : 0u;
             if (timed) {
                 while ((int)S->timing.size() < 2 * (S->n_timed + 1)) {
                     cudaEvent_t e;
@@ -382,7 +382,7 @@ etp_status copy_intervals_device(etp_ctx* c, const etp_interval* host_descs, int
                 ETP_CUDA_OK(cudaEventRecord(S->timing[2 * S->n_timed], user));
             }
             if (!c->opts[ETP_OPT_SKIP_D2D]) {
-                launch_copy_kernel(a, grid, user);
+                launch_copy_kernel(a, grid, user, c->opts[ETP_OPT_SMALL_STAGED] && T.v[C_BULK_ITEMS] == 0 && n_small > 0);
                 ETP_CUDA_OK(cudaGetLastError());
                 ++rep.n_kernel_launches;
             }
