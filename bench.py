@@ -53,6 +53,9 @@ def parse_args():
     ap.add_argument("--sharded", action="store_true",
                     help="--gpus N > 1: ONE reshard sharded by destination rank over N processes / GPUs (simulated rank r on GPU r mod N, "
                          "peers' memory through CUDA IPC, no collective) instead of N independent replicas")
+    ap.add_argument("--gather-ctas", type=int, default=-1, help="A/B: ETP_OPT_GATHER_CTAS (CTAs of the zero-copy KV gather; default: the library's 16)")
+    ap.add_argument("--pcie-probe", action="store_true",
+                    help="zero-copy reads of pinned host memory through kernel (a) (bulk and vector paths, by fragment size and grid) vs cudaMemcpyAsync")
     ap.add_argument("--small-staged", type=int, default=-1, help="A/B: ETP_OPT_SMALL_STAGED for --microbench (default: the library's)")
     ap.add_argument("--lin-pdl", type=int, default=-1, help="A/B: ETP_OPT_LINEAR_PDL for the S7 leg (default: the library's)")
     ap.add_argument("--lin-ring", type=int, default=-1, help="A/B: ETP_OPT_LINEAR_RING for the S7 leg (default: the library's)")
@@ -743,6 +746,56 @@ def run_moe(args):
     return 0
 
 
+# ================================================================================================ host-link probe
+def run_pcie_probe(args):
+    """What bounds pipeline (b)'s zero-copy KV gather: kernel (a) reading PINNED HOST memory directly, through
+    its cp.async.bulk path and through its 16-byte vector path, for contiguous fragments of several sizes at 16 and 148 CTAs,
+    beside a plain cudaMemcpyAsync of the same 2 GiB.  One JSON line."""
+    import numpy as np
+    import torch
+    import paper_2511_11617_b200 as etp
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    ctx = etp.Context(0)
+    ctx.set_option(etp.OPT_VALIDATE_INTERVALS, 0)
+    N = 2 << 30
+    host = torch.empty(N, dtype=torch.uint8).pin_memory()
+    host.random_(0, 255)
+    dst = torch.empty(N, dtype=torch.uint8, device=dev)
+    st = torch.cuda.Stream(dev)
+
+    def timed(fn):
+        fn()
+        st.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        fn()
+        e1.record(st)
+        st.synchronize()
+        return e0.elapsed_time(e1)
+
+    def dma():
+        with torch.cuda.stream(st):
+            dst.copy_(host, non_blocking=True)
+    out = {"pcie_probe": "kernel (a) reading pinned host memory (zero-copy) vs the copy engines", "bytes": N,
+           "cudaMemcpyAsync_GBps": round(N / timed(dma) / 1e6, 2), "rows": []}
+    for frag in (1 << 20, 65536, 4096, 1024, 256):
+        n = N // frag
+        offs = np.arange(n, dtype=np.int64) * frag
+        il = etp.IntervalList(host.data_ptr() + offs, dst.data_ptr() + offs, np.full(n, frag, dtype=np.int64))
+        for grid in (16, 148):
+            row = {"fragment_bytes": frag, "ctas": grid}
+            for name, tma_min in (("vector_path_GBps", 1 << 62), ("bulk_path_GBps", 16)):
+                ctx.set_option(etp.OPT_TMA_MIN_BYTES, tma_min)
+                ctx.set_option(etp.OPT_GRID_CTAS, grid)
+                row[name] = round(n * frag / timed(lambda: il.run(ctx, st.cuda_stream)) / 1e6, 2)
+            out["rows"].append(row)
+        assert torch.equal(dst[:1 << 20].cpu(), host[:1 << 20]), "zero-copy read differs from the host buffer"
+    print(json.dumps(out))
+    ctx.close()
+    return 0
+
+
 # ================================================================================================ multi-rank plumbing
 def max_over_ranks(ms: float, world: int, device) -> float:
     """Replicas only: every rank times its own replica; the job's time is the MAX over ranks."""
@@ -911,6 +964,8 @@ def run_ours(args):
     t_build = time.perf_counter() - t_build
     ctx = etp.Context(local_rank)
     ctx.set_option(etp.OPT_TIME_KERNELS, 1)
+    if args.gather_ctas > 0:
+        ctx.set_option(etp.OPT_GATHER_CTAS, args.gather_ctas)
     if args.lin_pdl >= 0:
         ctx.set_option(etp.OPT_LINEAR_PDL, args.lin_pdl)
     if args.lin_ring >= 0:
@@ -1101,6 +1156,8 @@ def run_ours(args):
 
 if __name__ == "__main__":
     a = parse_args()
+    if a.pcie_probe:
+        sys.exit(run_pcie_probe(a))
     if a.microbench:
         sys.exit(run_microbench(a))
     if a.moe:
