@@ -521,6 +521,46 @@ def test_copy_intervals_errors(ctx):
     assert (D.payload()[:192] == 0).all() and (D.payload()[192:] == 7).all()
 
 
+@pytest.mark.parametrize("n", [5000, 100_000])
+def test_copy_intervals_validation_at_scale(ctx, n):
+    """The disjointness check on many intervals (radix sort of (start, index) pairs, two threads from 65536): a valid random plan
+    passes and is copied exactly; ONE planted overlap - a destination moved 16 bytes into its neighbour, or a source pointed into
+    some destination - is reported with the right interval, and nothing is enqueued."""
+    rng = np.random.default_rng(n)
+    sz = rng.integers(1, 9, n).astype(np.int64) * 16
+    do_sorted = np.cumsum(sz + rng.integers(0, 3, n) * 16) - sz
+    perm = rng.permutation(n)
+    do = do_sorted[perm]
+    sz_p = sz[perm]
+    src_arena = 1 << 20
+    so = rng.integers(0, (src_arena - 256) // 16, n).astype(np.int64) * 16
+    src = rng.integers(0, 256, src_arena, dtype=np.uint8)
+    dst0 = np.full(int(do_sorted[-1] + sz[-1] + 64), 9, dtype=np.uint8)
+    S, D = DevBuf(src), DevBuf(dst0)
+    etp.etp_copy_intervals(ctx, so + S.ptr, do + D.ptr, sz_p)
+    torch.cuda.synchronize()
+    expect = dst0.copy()
+    for a, b, m in zip(so, do, sz_p):
+        expect[b:b + m] = src[a:a + m]
+    assert D.payload().tobytes() == expect.tobytes() and D.guards_intact()
+    D2 = DevBuf(dst0)
+    k = int(np.argmax(do == do_sorted[n // 2]))                   # the interval whose destination is the (n/2)-th in address order
+    bad_d = do.copy()
+    bad_d[k] -= 16                                                # now overlaps the end of its predecessor (gap 0 or more: force it)
+    pred = int(np.argmax(do == do_sorted[n // 2 - 1]))
+    bad_d[k] = do[pred] + sz_p[pred] - 16
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_copy_intervals(ctx, so + S.ptr, bad_d + D2.ptr, sz_p)
+    assert e.value.status == 1 and str(pred) in str(e.value) and str(k) in str(e.value)
+    bad_s = so + S.ptr
+    bad_s[7] = D2.ptr + do[k]                                     # a source inside another interval's destination
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_copy_intervals(ctx, bad_s, do + D2.ptr, sz_p)
+    assert e.value.status == 1
+    torch.cuda.synchronize()
+    assert (D2.payload() == 9).all() and D2.guards_intact()
+
+
 def test_back_to_back_calls_without_a_sync(ctx):
     """Two calls in flight on one ctx (the descriptor arena is double-buffered): a KV reshard whose zero-copy gather sits on
     the reload stream behind a large pinned-host copy, then - without any synchronisation - a multi-phase parameter reshard
