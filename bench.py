@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--sharded", action="store_true",
                     help="--gpus N > 1: ONE reshard sharded by destination rank over N processes / GPUs (simulated rank r on GPU r mod N, "
                          "peers' memory through CUDA IPC, no collective) instead of N independent replicas")
+    ap.add_argument("--kv-own-stream", action="store_true",
+                    help="A/B: the KV reload (zero-copy gather) on a reload stream of its own, sharing the host link with the parameter DMAs")
     ap.add_argument("--gather-ctas", type=int, default=-1, help="A/B: ETP_OPT_GATHER_CTAS (CTAs of the zero-copy KV gather; default: the library's 16)")
     ap.add_argument("--pcie-probe", action="store_true",
                     help="zero-copy reads of pinned host memory through kernel (a) (bulk and vector paths, by fragment size and grid) vs cudaMemcpyAsync")
@@ -970,7 +972,7 @@ def run_ours(args):
         ctx.set_option(etp.OPT_LINEAR_PDL, args.lin_pdl)
     if args.lin_ring >= 0:
         ctx.set_option(etp.OPT_LINEAR_RING, args.lin_ring)
-    cs, rs = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+    cs, rs, rs2 = torch.cuda.Stream(dev), torch.cuda.Stream(dev), torch.cuda.Stream(dev)
 
     if args.linear_only:
         state.reshard(ctx, 0, "device", cs.cuda_stream, rs.cuda_stream, replan=True)   # the linears run on the NEW layout
@@ -990,7 +992,14 @@ def run_ours(args):
         """One pass S1-S6.  Returns (device ms from first enqueue to both streams done, reports)."""
         e0, e1, er = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event()
         e0.record(cs)
-        rep = state.reshard(ctx, 0, image, cs.cuda_stream, rs.cuda_stream, replan=True)
+        if args.kv_own_stream:
+            rs2.wait_event(e0)
+            rep = state.reshard(ctx, 0, image, cs.cuda_stream, rs.cuda_stream, replan=True, kv_reload_stream=rs2.cuda_stream)
+            er2 = torch.cuda.Event()
+            er2.record(rs2)
+            cs.wait_event(er2)
+        else:
+            rep = state.reshard(ctx, 0, image, cs.cuda_stream, rs.cuda_stream, replan=True)
         er.record(rs)
         cs.wait_event(er)
         e1.record(cs)

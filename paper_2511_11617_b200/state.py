@@ -305,9 +305,12 @@ class ModelState:
 
     # ------------------------------------------------------------------ one pass of the hot path (S1-S6)
     def reshard(self, ctx: B.Context, step_idx: int, image: str, copy_stream: int, reload_stream: int,
-                replan: bool = True, table: Optional[np.ndarray] = None, block_budget: Optional[int] = None) -> Dict[str, object]:
+                replan: bool = True, table: Optional[np.ndarray] = None, block_budget: Optional[int] = None,
+                kv_reload_stream: Optional[int] = None) -> Dict[str, object]:
         """S1 partition + S2 CMM plan (host, inside libetp.so), then S3-S5 on the parameters and S3-S6 on the KV cache.
-        Asynchronous: returns after enqueueing; the caller synchronises both streams."""
+        Asynchronous: returns after enqueueing; the caller synchronises both streams (and ``kv_reload_stream`` when the KV reload is
+        given a stream of its own, so that its zero-copy gather shares the host link with the parameter DMAs instead of queueing
+        behind them)."""
         st = self.steps[step_idx]
         if replan:
             cur = {k: [(r, s, e, 1) for (r, s, e, _) in st.old[k]] for k in st.old}
@@ -333,7 +336,7 @@ class ModelState:
                 last_use=kv["last_use"], head_plan=plans["head"],
                 new_block_budget=kv["n_blocks"] if block_budget is None else block_budget,
                 host_backup=per_kind[image].data_ptr() if hh > 0 else 0, host_heads=hh, host_head0=ds,
-                copy_stream=copy_stream, reload_stream=reload_stream)
+                copy_stream=copy_stream, reload_stream=reload_stream if kv_reload_stream is None else kv_reload_stream)
         return {"params": rep_p, "kv": rep_k, "evicted": evicted, "table": new_table, "plans": plans}
 
     # ------------------------------------------------------------------ S7: the layer outputs on the sharded state
