@@ -95,7 +95,7 @@ typedef enum {
                                     K over the idle pairs (fp32 partials summed in range order); 256 / 128: always
                                     pairs, with that token tile, no tail split; 0: always single-CTA 128 x 256 tiles  */
     ETP_OPT_VALIDATE_INTERVALS = 10, /* 1 (default): etp_copy_intervals checks on the host that the destinations are mutually
-                                    disjoint and disjoint from every source (two sorts, O(n log n)) and returns
+                                    disjoint and disjoint from every source (radix sorts of both sides, O(n)) and returns
                                     ETP_ERR_INVALID_ARG before anything is enqueued; 0: trust the caller                   */
     ETP_OPT_LINEAR_PDL = 11,     /* 1 (default): launches of the <= 64-token shard-linear kernel carry the programmatic-stream-
                                     serialization attribute: their prologue and first ring of weight tiles overlap the tail of the

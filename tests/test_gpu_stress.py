@@ -5,6 +5,8 @@ with a disturbing kernel in between so that SM residency and timing differ from 
 the first one bit for bit (all of these paths are deterministic by construction: fixed summation orders, disjoint writes).
 The first run of each case is checked against the oracle, so "all equal" cannot mean "all equally wrong".  Outputs are
 pre-filled with NaN patterns: an element a run failed to write differs from the first run's."""
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -19,7 +21,7 @@ from workloads import get_config
 from workloads.gen import as_u8, fill_normal16, torch_dtype
 
 pytestmark = pytest.mark.gpu
-REPEATS = 25
+REPEATS = int(os.environ.get("ETP_STRESS_REPEATS", "25"))   # the soak run of profiles/r2_sanitizer.md sets 400
 
 
 @pytest.fixture(scope="module")
