@@ -394,6 +394,11 @@ etp_status etp_eplb_apply(etp_ctx* ctx, const etp_tensor* tensors, int32_t n_ten
 typedef struct { const void* src; void* dst; int64_t bytes; } etp_interval;
 etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_descs, int64_t n, void* stream,
                               etp_reshard_report* report);
+/* Host-only, no context: the check etp_copy_intervals runs first (unless ETP_OPT_VALIDATE_INTERVALS is 0).  ETP_ERR_INVALID_ARG for a
+ * negative size, a NULL pointer, two overlapping destinations or a destination that overlaps any source (the message names the two
+ * intervals); ETP_ERR_ALIGNMENT for an address or size that is not a multiple of 16.  Zero-byte intervals are ignored.  O(n) plus
+ * small sorts, on up to 16 threads from 65536 intervals. */
+etp_status etp_intervals_validate(const etp_interval* host_descs, int64_t n);
 
 #ifdef __cplusplus
 }

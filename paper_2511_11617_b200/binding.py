@@ -101,7 +101,7 @@ EXPORTS = ["etp_ctx_create", "etp_ctx_create_multi", "etp_ctx_set_rank_devices",
            "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_create_weighted", "etp_plan_tasks", "etp_plan_new_layout",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
            "etp_shard_linear_multi", "etp_linear_prepare", "etp_linear_run", "etp_linear_plan_info", "etp_linear_free",
-           "etp_moe_linear", "etp_moe_linear_instances", "etp_moe_gate_up", "etp_eplb_place", "etp_eplb_apply", "etp_copy_intervals"]
+           "etp_moe_linear", "etp_moe_linear_instances", "etp_moe_gate_up", "etp_eplb_place", "etp_eplb_apply", "etp_copy_intervals", "etp_intervals_validate"]
 
 _lib = None
 
@@ -156,6 +156,7 @@ def lib() -> C.CDLL:
         L.etp_eplb_place.argtypes = [C.POINTER(i64), C.POINTER(i32), i32, C.POINTER(i64), C.POINTER(i32), i32, C.POINTER(etp_replica), i32,
                                      C.POINTER(i32)]
         L.etp_copy_intervals.argtypes = [vp, C.POINTER(etp_interval), i64, vp, C.POINTER(etp_reshard_report)]
+        L.etp_intervals_validate.argtypes = [C.POINTER(etp_interval), i64]
         _lib = L
     return _lib
 
@@ -563,6 +564,14 @@ class IntervalList:
         rep = etp_reshard_report()
         _check(lib().etp_copy_intervals(ctx.handle, self.rec.ctypes.data_as(C.POINTER(etp_interval)), self.n, stream or None, C.byref(rep)))
         return rep.as_dict()
+
+    def validate(self) -> None:
+        """etp_intervals_validate (host-only, no context): raises EtpError as etp_copy_intervals would."""
+        _check(lib().etp_intervals_validate(self.rec.ctypes.data_as(C.POINTER(etp_interval)), self.n))
+
+
+def etp_intervals_validate(src_ptrs, dst_ptrs, sizes) -> None:
+    IntervalList(src_ptrs, dst_ptrs, sizes).validate()
 
 
 def etp_copy_intervals(ctx: Context, src_ptrs, dst_ptrs, sizes, stream: int = 0) -> Dict[str, float]:

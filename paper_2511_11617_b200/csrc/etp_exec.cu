@@ -12,9 +12,6 @@
 #include <algorithm>
 #include <chrono>
 #include <cstring>
-#include <functional>
-#include <memory>
-#include <thread>
 
 #include "etp_copy.cuh"
 
@@ -640,79 +637,12 @@ extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_
     if (!ctx || n < 0 || (n > 0 && !host_descs)) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: bad arguments");
     const double t0 = now_ms();
     const bool device_path = n >= kDeviceLoweringMin;
-    if (ctx->opts[ETP_OPT_VALIDATE_INTERVALS] || !device_path) {
-        for (int64_t i = 0; i < n; ++i) {
-            const etp_interval& d = host_descs[i];
-            if (d.bytes < 0) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has negative size", (long long)i);
-            if (d.bytes == 0) continue;
-            if (!d.src || !d.dst) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: interval %lld has a NULL pointer", (long long)i);
-            if (((uintptr_t)d.src | (uintptr_t)d.dst | (uint64_t)d.bytes) & 15)
-                ETP_FAIL(ETP_ERR_ALIGNMENT, "etp_copy_intervals: interval %lld is not 16-byte aligned", (long long)i);
-        }
-    }
+    // the contract of include/etp.h (etp_validate.cpp): argument checks always on the host-lowered path, the disjointness check
+    // unless the caller switched it off
     if (ctx->opts[ETP_OPT_VALIDATE_INTERVALS]) {
-        // the contract of include/etp.h: destinations mutually disjoint and disjoint from every source (one launch, no order
-        // between intervals).  Sort both sides by start address, then one sweep each.
-        // (start, end, index) records, LSD radix sort on the significant bits of (start - min start) >> 4 (11 bits per pass: 3 passes
-        // for a 32-GiB arena), the two sides on two threads.
-        struct Key { uint64_t k, e; uint64_t i; };
-        std::vector<Key> dst, src;
-        dst.reserve((size_t)n);
-        src.reserve((size_t)n);
-        for (int64_t i = 0; i < n; ++i) {
-            const etp_interval& d = host_descs[i];
-            if (d.bytes == 0) continue;
-            dst.push_back({(uint64_t)(uintptr_t)d.dst, (uint64_t)(uintptr_t)d.dst + (uint64_t)d.bytes, (uint64_t)i});
-            src.push_back({(uint64_t)(uintptr_t)d.src, (uint64_t)(uintptr_t)d.src + (uint64_t)d.bytes, (uint64_t)i});
-        }
-        auto radix = [](std::vector<Key>& v) {
-            if (v.size() < 2) return;
-            uint64_t lo = UINT64_MAX, hi = 0;
-            for (const Key& x : v) { lo = std::min(lo, x.k); hi = std::max(hi, x.k); }
-            if (v.size() < 4096) {
-                std::sort(v.begin(), v.end(), [](const Key& a, const Key& b) { return a.k < b.k; });
-                return;
-            }
-            int bits = 0;
-            while (bits < 60 && ((hi - lo) >> 4 >> bits) != 0) ++bits;
-            std::unique_ptr<Key[]> tmp(new Key[v.size()]);   // uninitialised: every pass writes all of it
-            Key* in = v.data();
-            Key* out = tmp.get();
-            constexpr int kDigit = 11;
-            for (int shift = 0; shift < bits; shift += kDigit) {
-                size_t count[(1 << kDigit) + 1] = {0};
-                for (size_t j = 0; j < v.size(); ++j) ++count[((((in[j].k - lo) >> 4) >> shift) & ((1u << kDigit) - 1)) + 1];
-                for (int d = 0; d < (1 << kDigit); ++d) count[d + 1] += count[d];
-                for (size_t j = 0; j < v.size(); ++j) out[count[(((in[j].k - lo) >> 4) >> shift) & ((1u << kDigit) - 1)]++] = in[j];
-                std::swap(in, out);
-            }
-            if (in != v.data()) std::memcpy(v.data(), in, v.size() * sizeof(Key));
-        };
-        if (dst.size() >= 65536) {
-            std::thread t(radix, std::ref(src));
-            radix(dst);
-            t.join();
-        } else {
-            radix(dst);
-            radix(src);
-        }
-        auto end_of = [](const Key& x) { return x.e; };
-        for (size_t k = 1; k < dst.size(); ++k)
-            if (dst[k].k < end_of(dst[k - 1]))
-                ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: destinations of intervals %lld and %lld overlap", (long long)dst[k - 1].i, (long long)dst[k].i);
-        size_t si = 0;
-        uint64_t src_reach = 0;   // largest end among the sources that start below the current destination's end
-        int64_t src_reach_i = -1;
-        for (const Key& d : dst) {   // destinations are disjoint and ascending, so one forward pass over the sources suffices
-            const uint64_t d_end = end_of(d);
-            while (si < src.size() && src[si].k < d_end) {
-                const uint64_t s_end = end_of(src[si]);
-                if (s_end > src_reach) { src_reach = s_end; src_reach_i = (int64_t)src[si].i; }
-                ++si;
-            }
-            if (src_reach > d.k)
-                ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_copy_intervals: destination of interval %lld overlaps the source of interval %lld", (long long)d.i, (long long)src_reach_i);
-        }
+        ETP_TRY(validate_intervals(host_descs, n, true));
+    } else if (!device_path) {
+        ETP_TRY(validate_intervals(host_descs, n, false));
     }
     if (device_path) {
         // 10^5 .. 10^6 intervals: the raw records are uploaded in chunks and lowered by kernels while the previous chunk is being

@@ -149,6 +149,8 @@ void push_contiguous(const etp_ctx* ctx, JobList* jl, const void* src, void* dst
 
 // etp_copy_intervals above kDeviceLoweringMin intervals: descriptors are built by kernels from the raw records (etp_lower_dev.cu)
 constexpr int64_t kDeviceLoweringMin = 32768;
+// etp_validate.cpp: argument checks of every interval; with check_overlap also "destinations mutually disjoint and disjoint from every source"
+etp_status validate_intervals(const etp_interval* descs, int64_t n, bool check_overlap);
 etp_status copy_intervals_device(etp_ctx* ctx, const etp_interval* host_descs, int64_t n, void* stream, etp_reshard_report* report);
 void free_interval_state(etp_ctx* ctx);
 int interval_timed_launches(etp_ctx* ctx, double* ms);

@@ -305,3 +305,91 @@ def test_eplb_place_matches_oracle():
     with pytest.raises(etp.EtpError) as e:
         etp.etp_eplb_place([1], [0], [0], [1])
     assert e.value.status == 1
+
+
+# ------------------------------------------------------------------------------------------------ interval contract check (host-only)
+def _brute_force_verdict(src, dst, sz):
+    """The contract of include/etp.h by its plain definition, O(n^2): 'align', 'arg' or None."""
+    n = len(sz)
+    for i in range(n):
+        if sz[i] == 0:
+            continue
+        if sz[i] < 0 or src[i] == 0 or dst[i] == 0:
+            return "arg"
+        if (src[i] | dst[i] | sz[i]) & 15:
+            return "align"
+    live = [i for i in range(n) if sz[i] > 0]
+    for a in live:
+        for b in live:
+            if a < b and dst[a] < dst[b] + sz[b] and dst[b] < dst[a] + sz[a]:
+                return "arg"
+            if dst[a] < src[b] + sz[b] and src[b] < dst[a] + sz[a]:
+                return "arg"
+    return None
+
+
+def _lib_verdict(src, dst, sz):
+    try:
+        etp.etp_intervals_validate(np.asarray(src, np.int64), np.asarray(dst, np.int64), np.asarray(sz, np.int64))
+        return None
+    except etp.EtpError as e:
+        return {1: "arg", 2: "align"}[e.status]
+
+
+def test_intervals_validate_against_the_plain_definition():
+    """etp_intervals_validate (no device, no context) on 3000 random small plans with planted faults of every kind (overlapping
+    destinations, a destination inside a source, its own shifted source, misalignment, negative and zero sizes) against the
+    O(n^2) definition of the contract; touching intervals and overlapping SOURCES are legal."""
+    rng = np.random.default_rng(11617)
+    n_bad = n_ok = 0
+    for case in range(3000):
+        n = int(rng.integers(1, 12))
+        sz = rng.integers(1, 6, n).astype(np.int64) * 16
+        dst = 0x10000 + (np.cumsum(sz + rng.integers(0, 2, n) * 16) - sz)           # disjoint, some touching
+        dst = dst[rng.permutation(n)]
+        src = 0x40000 + rng.integers(0, 64, n).astype(np.int64) * 16                # sources may overlap each other
+        kind = int(rng.integers(0, 8))
+        k, j = int(rng.integers(0, n)), int(rng.integers(0, n))
+        if kind == 1 and n > 1 and k != j:
+            dst[k] = dst[j] + 16 * int(rng.integers(-2, 3))                          # destinations overlap (or touch / miss)
+        elif kind == 2:
+            src[k] = dst[j] + 16 * int(rng.integers(-3, 4))                          # a source on / next to a destination
+        elif kind == 3:
+            src[k] += 8                                                              # misaligned
+        elif kind == 4:
+            sz[k] = -16
+        elif kind == 5:
+            sz[k] = 0                                                                # ignored, whatever its addresses
+            dst[k] = dst[j]
+        elif kind == 6:
+            src[k] = dst[k] + 16                                                     # a shifting copy onto itself
+        want, got = _brute_force_verdict(src, dst, sz), _lib_verdict(src, dst, sz)
+        assert want == got, (case, kind, src.tolist(), dst.tolist(), sz.tolist(), want, got)
+        n_bad += want is not None
+        n_ok += want is None
+    assert n_bad > 500 and n_ok > 500
+
+
+@pytest.mark.parametrize("n", [70_000, 300_000])
+def test_intervals_validate_threaded_path_finds_one_planted_overlap(n):
+    """From 65536 intervals the check runs on several threads (address buckets sorted independently): a valid random plan passes; one
+    destination moved 16 bytes into its neighbour, or one source pointed at some destination, is reported with both indices."""
+    rng = np.random.default_rng(n)
+    sz = rng.integers(1, 9, n).astype(np.int64) * 16
+    dst_sorted = 0x1000000 + (np.cumsum(sz + rng.integers(0, 3, n) * 16) - sz)
+    perm = rng.permutation(n)
+    dst, szp = dst_sorted[perm], sz[perm]
+    src = 0x7f0000000000 + rng.integers(0, 1 << 24, n).astype(np.int64) * 16
+    etp.etp_intervals_validate(src, dst, szp)
+    k = int(np.argmax(dst == dst_sorted[n // 3]))
+    pred = int(np.argmax(dst == dst_sorted[n // 3 - 1]))
+    bad = dst.copy()
+    bad[k] = dst[pred] + szp[pred] - 16
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_intervals_validate(src, bad, szp)
+    assert e.value.status == 1 and str(pred) in str(e.value) and str(k) in str(e.value)
+    bad_s = src.copy()
+    bad_s[5] = dst[k] + 16 if szp[k] > 16 else dst[k]
+    with pytest.raises(etp.EtpError) as e:
+        etp.etp_intervals_validate(bad_s, dst, szp)
+    assert e.value.status == 1 and " 5" in str(e.value) and str(k) in str(e.value)
