@@ -311,13 +311,13 @@ def test_moe_linear_grouped_vs_reference(ctx, T, E, F, Hd, top_k, widths, gmode,
     tiles only / the library's choice / CTA pairs (cta_group::2) forced even for a few rows."""
     ctx.set_option(etp.OPT_MOE_CTA_PAIR, moe_pair)
     try:
-        _moe_linear_grouped(ctx, T, E, F, Hd, top_k, widths, gmode)
+        _moe_linear_grouped(ctx, T, E, F, Hd, top_k, widths, gmode, "fp16" if (T + moe_pair) % 2 else "bf16")   # both dtypes over the grid
     finally:
         ctx.set_option(etp.OPT_MOE_CTA_PAIR, 1)
 
 
-def _moe_linear_grouped(ctx, T, E, F, Hd, top_k, widths, gmode):
-    dt = torch_dtype("bf16")
+def _moe_linear_grouped(ctx, T, E, F, Hd, top_k, widths, gmode, dtype="bf16"):
+    dt = torch_dtype(dtype)
     rng = np.random.default_rng(T + E)
     layout = widths_to_layout(widths)
     geom = {}
@@ -339,13 +339,13 @@ def _moe_linear_grouped(ctx, T, E, F, Hd, top_k, widths, gmode):
         bufs = {r: DevBuf(a) for r, a in slabs.items()}
         desc = etp.TensorDesc(E, ub, {r: (bufs[r].ptr, geom[r][1], geom[r][0]) for r in bufs}, len(widths), 0)
         xb, yb = DevBuf(x_u8), DevBuf(np.full(R * N * 2, 0xEE, dtype=np.uint8))
-        etp.etp_moe_linear(ctx, mode, "bf16", xb.ptr, offs, K, N, desc, layout, yb.ptr)
+        etp.etp_moe_linear(ctx, mode, dtype, xb.ptr, offs, K, N, desc, layout, yb.ptr)
         torch.cuda.synchronize()
         assert xb.guards_intact() and yb.guards_intact() and all(b.guards_intact() for b in bufs.values())
-        x64 = OL.decode16(x_u8, "bf16").reshape(R, K)
-        w64 = OL.decode16(w_u8, "bf16").reshape(E, F, Hd)        # col: [E][out=F][in=Hd]; row: [E][in=F][out=Hd]
+        x64 = OL.decode16(x_u8, dtype).reshape(R, K)
+        w64 = OL.decode16(w_u8, dtype).reshape(E, F, Hd)        # col: [E][out=F][in=Hd]; row: [E][in=F][out=Hd]
         ref = np.stack([(w64[e] @ x64[r]) if mode == etp.COL_PARALLEL else (x64[r] @ w64[e]) for r, e in enumerate(assign)])
-        check(yb.payload(), ref, "bf16", R, N)
+        check(yb.payload(), ref, dtype, R, N)
 
 
 def test_shard_linear_argument_errors(ctx):
@@ -611,7 +611,17 @@ def _moe_gate_up_fused(ctx, rows_per_expert, E, F, Hd, widths):
     check(hb.payload(), ref, "bf16", R, F)
 
 
-def test_moe_layer_with_eplb_replicas_is_bitwise_the_unreplicated_layer(ctx):
+@pytest.mark.parametrize("moe_pair", [1, 2])
+def test_moe_layer_with_eplb_replicas_is_bitwise_the_unreplicated_layer(ctx, moe_pair):
+    """moe_pair = 2: the same through the CTA-pair kernels (forced; a replica changes an expert's row tiles, not its results)."""
+    ctx.set_option(etp.OPT_MOE_CTA_PAIR, moe_pair)
+    try:
+        _moe_layer_with_eplb_replicas(ctx)
+    finally:
+        ctx.set_option(etp.OPT_MOE_CTA_PAIR, 1)
+
+
+def _moe_layer_with_eplb_replicas(ctx):
     """Reading E1 end to end: seeded Zipf loads -> etp_eplb_place (== oracle) -> etp_eplb_apply copies the hot experts into
     spare slots (slot choice == oracle.eplb.replica_slots; the replica's bytes are the expert's, nothing else changes) ->
     the layer through etp_moe_gate_up + etp_moe_linear_instances with every expert's rows split over its instances.  A row is
