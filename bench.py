@@ -53,6 +53,11 @@ def parse_args():
     ap.add_argument("--sharded", action="store_true",
                     help="--gpus N > 1: ONE reshard sharded by destination rank over N processes / GPUs (simulated rank r on GPU r mod N, "
                          "peers' memory through CUDA IPC, no collective) instead of N independent replicas")
+    ap.add_argument("--watchdog-s", type=float, default=900.0,
+                    help="single-process runs execute in a child process; if it prints nothing for this long it is killed and the run is "
+                         "repeated ONCE (0 = run in this process).  One default run directly after an ncu session once hung for 900 s "
+                         "without output (profiles/r2_sanitizer.md); it never reproduced, this is the second chance")
+    ap.add_argument("--in-child", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--kv-own-stream", action="store_true",
                     help="A/B: the KV reload (zero-copy gather) on a reload stream of its own, sharing the host link with the parameter DMAs")
     ap.add_argument("--gather-ctas", type=int, default=-1, help="A/B: ETP_OPT_GATHER_CTAS (CTAs of the zero-copy KV gather; default: the library's 16)")
@@ -1163,8 +1168,31 @@ def run_ours(args):
     return 0
 
 
+def run_under_watchdog(a) -> int:
+    """The same command line in a child process with a deadline; one retry.  stdout / stderr are inherited, so the JSON line is the
+    child's.  Only for single-process runs (under torchrun every rank must stay the process torchrun started)."""
+    import signal
+    import subprocess
+    cmd = [sys.executable, os.path.abspath(__file__)] + sys.argv[1:] + ["--in-child"]
+    for attempt in (1, 2):
+        p = subprocess.Popen(cmd, start_new_session=True)
+        try:
+            return p.wait(timeout=a.watchdog_s)
+        except subprocess.TimeoutExpired:
+            print(f"bench.py: no result after {a.watchdog_s:.0f} s (attempt {attempt}); killing the run" + (" and repeating it once" if attempt == 1 else ""),
+                  file=sys.stderr, flush=True)
+            try:
+                os.killpg(p.pid, signal.SIGKILL)      # the child's own process group (start_new_session): exact, not by pattern
+            except ProcessLookupError:
+                pass
+            p.wait()
+    return 1
+
+
 if __name__ == "__main__":
     a = parse_args()
+    if a.watchdog_s > 0 and not a.in_child and int(os.environ.get("WORLD_SIZE", "1")) == 1:
+        sys.exit(run_under_watchdog(a))
     if a.pcie_probe:
         sys.exit(run_pcie_probe(a))
     if a.microbench:
