@@ -412,6 +412,16 @@ def smoke_shard_linear(ctx):
     TR.run_param_step(ctx, world, bufs, images, 0, Streams())
     outs = linear_checks_for_world(ctx, world, bufs, world.steps[0].new, cfg.tokens, dead=world.steps[0].dead)
     print(f"smoke shard_linear OK: {len(outs)} linears of config 1 on the resharded layout within {TOL} of the unsharded reference")
+    # the other tcgen05 kernels, one small case each against the fp64 references: CTA pairs of kernel (c) (> 64 tokens, row-parallel with
+    # ragged widths), the grouped MoE kernels (fused gate|up through CTA pairs, plain single-CTA tiles)
+    test_shard_linear_matches_unsharded_reference(ctx, "row", "bf16", 300, 1000, 776, 1, (111, 222, 333, 334), "wrap")
+    ctx.set_option(etp.OPT_MOE_CTA_PAIR, 2)
+    try:
+        _moe_gate_up_fused(ctx, (130, 64, 257, 5), 4, 192, 320, (1, 3))
+    finally:
+        ctx.set_option(etp.OPT_MOE_CTA_PAIR, 1)
+    _moe_linear_grouped(ctx, 4, 8, 128, 256, 2, (3, 3, 2), "tight")
+    print("smoke tcgen05 OK: CTA-pair shard linear at 300 tokens, fused MoE gate|up (CTA pairs), grouped MoE linear at a few rows per expert")
 
 
 # ------------------------------------------------------------------------------------------------ prepared groups (etp_linear_prepare / etp_linear_run)
