@@ -400,6 +400,37 @@ etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_descs, int6
  * small sorts, on up to 16 threads from 65536 intervals. */
 etp_status etp_intervals_validate(const etp_interval* host_descs, int64_t n);
 
+/* ------------------------------------------------------------------------------------------------ no-allocation entry
+ * etp_copy_intervals for a caller that cannot allocate device memory.  Such callers are the normal case on the recovery path this
+ * library serves ("a single pass pre-allocates all destination buffers"): when a rank dies the survivors' HBM is already
+ * committed to weights and KV blocks and the serving engine's pool owns the remainder, so a cudaMalloc issued from inside a library
+ * may fail, or shrink what the engine promised its KV cache; cudaMalloc / cudaFree also stall every stream of the device, which hurts
+ * a recovery that overlaps with decode steps; and code that runs inside another component's CUDA context (a plugin, a fault handler)
+ * is often not allowed to create memory at all.  Every other device call here needs an etp_ctx, and etp_ctx_create allocates
+ * (descriptor arenas, events, streams).  This call needs no ctx: it calls no cudaMalloc / cudaFree / cudaHostAlloc, creates no
+ * stream or event, and uses no allocating library routine.
+ *
+ * It launches the same persistent copy kernel; the kernel's scratch (segment descriptors, item table, the two work-queue heads) lives
+ * in a fixed array inside the library's device image: 410,112 bytes (0.4 MiB) that every GPU which loads libetp.so holds until the
+ * process exits, whether or not this call is ever made.
+ *
+ *  - host_descs: host array (pageable is fine; consumed before the call returns); src / dst: device memory of the CURRENT device,
+ *    16-B aligned; bytes: multiple of 16.  Same disjointness contract as etp_copy_intervals, always checked (ETP_ERR_INVALID_ARG /
+ *    ETP_ERR_ALIGNMENT, nothing enqueued).  Runs on the current CUDA device, asynchronously on `stream` (a stream of that device; NULL
+ *    = legacy default stream): the data is in place once the caller has synchronised `stream`.  Intervals of >= 32 KiB take the
+ *    cp.async.bulk ring, smaller ones are batched, as in etp_copy_intervals with default options; there are no options here.
+ *  - Limits, both per call: n <= 4096 intervals, and the intervals of >= 32 KiB together at most 32768 pieces of 256 KiB (8 GiB when
+ *    they are multiples of 256 KiB).  Beyond either -> ETP_ERR_CAPACITY with a message that names the limit; nothing is enqueued.
+ *    Split a larger job into several calls on one stream.
+ *  - The FIRST call on each device does a one-time set-up (looks up the array's device address, raises the kernel's shared-memory
+ *    limit).  Make that first call before any stream capture is begun.
+ *  - All calls on a device share the one array, and it keeps the previous call's contents.  The queue heads are rewritten to zero by
+ *    every call and stale descriptors are never read, so back-to-back calls ON ONE STREAM are safe.  Two calls whose GPU work can
+ *    overlap (different streams without an event between them, or two host threads on different streams) RACE on the array and
+ *    copy wrong bytes: order them yourself.  The host side is serialised by a library mutex. */
+etp_status etp_copy_intervals_static(const etp_interval* host_descs, int64_t n, void* stream);
+
+
 #ifdef __cplusplus
 }
 #endif

@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libetp.so")
-SOURCES = ["etp_plan.cpp", "etp_eplb.cpp", "etp_lower.cpp", "etp_validate.cpp", "etp_lower_dev.cu", "etp_copy.cu", "etp_exec.cu", "etp_linear.cu", "etp_linear_group.cu", "etp_moe.cu"]
+SOURCES = ["etp_plan.cpp", "etp_eplb.cpp", "etp_lower.cpp", "etp_validate.cpp", "etp_lower_dev.cu", "etp_copy.cu", "etp_copy_static.cu", "etp_exec.cu", "etp_linear.cu", "etp_linear_group.cu", "etp_moe.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC,-Wall",
          "-I", os.path.join(ROOT, "include"), "-I", CSRC]

@@ -101,7 +101,8 @@ EXPORTS = ["etp_ctx_create", "etp_ctx_create_multi", "etp_ctx_set_rank_devices",
            "etp_ctx_kernel_time", "etp_partition", "etp_cmm_plan", "etp_plan_create", "etp_plan_create_weighted", "etp_plan_tasks", "etp_plan_new_layout",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
            "etp_shard_linear_multi", "etp_linear_prepare", "etp_linear_run", "etp_linear_plan_info", "etp_linear_free",
-           "etp_moe_linear", "etp_moe_linear_instances", "etp_moe_gate_up", "etp_eplb_place", "etp_eplb_apply", "etp_copy_intervals", "etp_intervals_validate"]
+           "etp_moe_linear", "etp_moe_linear_instances", "etp_moe_gate_up", "etp_eplb_place", "etp_eplb_apply", "etp_copy_intervals", "etp_intervals_validate",
+           "etp_copy_intervals_static"]
 
 _lib = None
 
@@ -157,6 +158,7 @@ def lib() -> C.CDLL:
                                      C.POINTER(i32)]
         L.etp_copy_intervals.argtypes = [vp, C.POINTER(etp_interval), i64, vp, C.POINTER(etp_reshard_report)]
         L.etp_intervals_validate.argtypes = [C.POINTER(etp_interval), i64]
+        L.etp_copy_intervals_static.argtypes = [C.POINTER(etp_interval), i64, vp]
         _lib = L
     return _lib
 
@@ -565,6 +567,10 @@ class IntervalList:
         _check(lib().etp_copy_intervals(ctx.handle, self.rec.ctypes.data_as(C.POINTER(etp_interval)), self.n, stream or None, C.byref(rep)))
         return rep.as_dict()
 
+    def run_static(self, stream: int = 0) -> None:
+        """etp_copy_intervals_static: no Context, nothing allocated (scratch in the library's static device array)."""
+        _check(lib().etp_copy_intervals_static(self.rec.ctypes.data_as(C.POINTER(etp_interval)), self.n, stream or None))
+
     def validate(self) -> None:
         """etp_intervals_validate (host-only, no context): raises EtpError as etp_copy_intervals would."""
         _check(lib().etp_intervals_validate(self.rec.ctypes.data_as(C.POINTER(etp_interval)), self.n))
@@ -577,3 +583,10 @@ def etp_intervals_validate(src_ptrs, dst_ptrs, sizes) -> None:
 def etp_copy_intervals(ctx: Context, src_ptrs, dst_ptrs, sizes, stream: int = 0) -> Dict[str, float]:
     """src_ptrs / dst_ptrs / sizes: numpy int64 arrays of absolute device addresses and byte counts."""
     return IntervalList(src_ptrs, dst_ptrs, sizes).run(ctx, stream)
+
+
+def etp_copy_intervals_static(src_ptrs, dst_ptrs, sizes, stream: int = 0) -> None:
+    """The copy of etp_copy_intervals for callers that must not allocate device memory (a recovery path running while the serving
+    engine's pool owns all free HBM, code inside somebody else's CUDA context): no Context, at most 4096 intervals per call, runs on
+    the current CUDA device.  Calls share one static scratch array: keep them on one stream or order them yourself (include/etp.h)."""
+    IntervalList(src_ptrs, dst_ptrs, sizes).run_static(stream)
