@@ -54,10 +54,11 @@ def parse_args():
                     help="--gpus N > 1: ONE reshard sharded by destination rank over N processes / GPUs (simulated rank r on GPU r mod N, "
                          "peers' memory through CUDA IPC, no collective) instead of N independent replicas")
     ap.add_argument("--watchdog-s", type=float, default=900.0,
-                    help="single-process runs execute in a child process; if it prints nothing for this long it is killed and the run is "
-                         "repeated ONCE (0 = run in this process).  One default run directly after an ncu session once hung for 900 s "
-                         "without output (profiles/r2_sanitizer.md); it never reproduced, this is the second chance")
+                    help="single-process runs execute in a child process; if it has not finished after this long it is killed and the run is "
+                         "repeated ONCE (0 = run in this process); the result line says so in its \"watchdog\" key.  One default run directly "
+                         "after an ncu session once hung for 900 s without output (profiles/r2_sanitizer.md); it never reproduced")
     ap.add_argument("--in-child", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--watchdog-selftest", default="", choices=["", "ok", "hang", "hang_after_result", "hang_once"], help=argparse.SUPPRESS)
     ap.add_argument("--kv-own-stream", action="store_true",
                     help="A/B: the KV reload (zero-copy gather) on a reload stream of its own, sharing the host link with the parameter DMAs")
     ap.add_argument("--gather-ctas", type=int, default=-1, help="A/B: ETP_OPT_GATHER_CTAS (CTAs of the zero-copy KV gather; default: the library's 16)")
@@ -1169,23 +1170,53 @@ def run_ours(args):
 
 
 def run_under_watchdog(a) -> int:
-    """The same command line in a child process with a deadline; one retry.  stdout / stderr are inherited, so the JSON line is the
-    child's.  Only for single-process runs (under torchrun every rank must stay the process torchrun started)."""
+    """The same command line in a child process with a deadline; one retry.  The child's stdout is captured and forwarded, and the
+    LAST JSON object line gets a "watchdog" key ({"attempts", "killed", "deadline_s"}), so a run that needed the retry says so in
+    its result line and a hang can never hide behind a green exit code.  A child that printed its result and then hung (teardown)
+    is killed and NOT repeated: exactly one result line comes out.  stderr is inherited.  Only for single-process runs (under
+    torchrun every rank must stay the process torchrun started)."""
     import signal
     import subprocess
     cmd = [sys.executable, os.path.abspath(__file__)] + sys.argv[1:] + ["--in-child"]
+    killed = 0
+
+    def forward(out: str, attempts: int) -> bool:
+        lines = out.splitlines()
+        last = -1
+        for i, ln in enumerate(lines):
+            if ln.startswith("{"):
+                try:
+                    if isinstance(json.loads(ln), dict):
+                        last = i
+                except ValueError:
+                    pass
+        for i, ln in enumerate(lines):
+            if i == last:
+                d = json.loads(ln)
+                d["watchdog"] = {"attempts": attempts, "killed": killed, "deadline_s": a.watchdog_s}
+                ln = json.dumps(d)
+            print(ln, flush=True)
+        return last >= 0
+
     for attempt in (1, 2):
-        p = subprocess.Popen(cmd, start_new_session=True)
+        p = subprocess.Popen(cmd, start_new_session=True, stdout=subprocess.PIPE, text=True)
         try:
-            return p.wait(timeout=a.watchdog_s)
+            out, _ = p.communicate(timeout=a.watchdog_s)
+            forward(out, attempt)
+            return p.returncode
         except subprocess.TimeoutExpired:
-            print(f"bench.py: no result after {a.watchdog_s:.0f} s (attempt {attempt}); killing the run" + (" and repeating it once" if attempt == 1 else ""),
-                  file=sys.stderr, flush=True)
+            killed += 1
             try:
                 os.killpg(p.pid, signal.SIGKILL)      # the child's own process group (start_new_session): exact, not by pattern
             except ProcessLookupError:
                 pass
-            p.wait()
+            out, _ = p.communicate()
+            had_result = forward(out, attempt) if out else False
+            print(f"bench.py: child still running after {a.watchdog_s:.0f} s (attempt {attempt}); killed"
+                  + (" after it had printed its result: not repeated" if had_result else (" and repeated once" if attempt == 1 else "")),
+                  file=sys.stderr, flush=True)
+            if had_result:
+                return 0
     return 1
 
 
@@ -1193,6 +1224,18 @@ if __name__ == "__main__":
     a = parse_args()
     if a.watchdog_s > 0 and not a.in_child and int(os.environ.get("WORLD_SIZE", "1")) == 1:
         sys.exit(run_under_watchdog(a))
+    if a.watchdog_selftest:      # tests/test_lib_host.py: the watchdog itself, without a GPU
+        mark = os.environ.get("ETP_WATCHDOG_SELFTEST_MARK", "")
+        first = bool(mark) and not os.path.exists(mark)
+        if mark:
+            open(mark, "a").close()
+        if a.watchdog_selftest == "hang" or (a.watchdog_selftest == "hang_once" and first):
+            time.sleep(3600)
+        print("a line that is not the result", flush=True)
+        print(json.dumps({"metric": "selftest", "value": 1.0}), flush=True)
+        if a.watchdog_selftest == "hang_after_result":
+            time.sleep(3600)
+        sys.exit(0)
     if a.pcie_probe:
         sys.exit(run_pcie_probe(a))
     if a.microbench:

@@ -100,12 +100,19 @@ typedef enum {
     ETP_OPT_LINEAR_PDL = 11,     /* 1 (default): launches of the <= 64-token shard-linear kernel carry the programmatic-stream-
                                     serialization attribute: their prologue and first ring of weight tiles overlap the tail of the
                                     previous kernel of the stream (griddepcontrol; X, Y and the workspace are only touched after
-                                    griddepcontrol.wait); 0: plain stream order                                           */
+                                    griddepcontrol.wait, the WEIGHT tiles before it); 0: plain stream order.  The first such launch
+                                    after a call of this library that writes slabs on the same stream (etp_reshard_params / _kv,
+                                    etp_eplb_apply, etp_copy_intervals) is sent without the attribute, so it sees the new weights.
+                                    A caller that writes slabs by other means (its own kernels, cudaMemcpyAsync) directly before a
+                                    <= 64-token linear on the same stream must set this option to 0 for that launch or put an
+                                    event / another kernel in between                                                      */
     ETP_OPT_LINEAR_RING = 12,    /* read by etp_linear_prepare: 0 = one CTA per SM with the full shared-memory ring; 1 = two CTAs per SM
                                     with half the ring each (one keeps streaming while the other is in its prologue or tail);
                                     2 (default) = two per SM unless the group streams >= 200 weight chunks (3.2 MiB) per SM      */
     ETP_OPT_ONLY_PHASE = 13,     /* 0 (default): a call runs every hazard phase, ordered by events; k > 0: only phase k - 1 is
-                                    enqueued (multi-process jobs: the caller puts its own barrier between the phases)         */
+                                    enqueued (multi-process jobs: the caller puts its own barrier between the phases).  Every
+                                    phase call must be given the same arguments; etp_reshard_kv therefore does NOT rewrite
+                                    pt->block_table when k > 0 (see there)                                                    */
     ETP_OPT_MOE_CTA_PAIR = 14,   /* 1 (default): the grouped MoE kernels run CTA pairs (tcgen05 cta_group::2, 256 out features x up to
                                     256 routed rows per pair, each CTA staging half of the rows) when the instances carry enough rows
                                     for >= 128-row tiles; 2: always; 0: never (single-CTA 128-feature tiles)                  */
@@ -257,7 +264,11 @@ etp_status etp_page_table_rewrite(etp_page_table* pt, int32_t block_size, int32_
 
 /* Rewrites the page table (above), then moves KV-head slices of every surviving live block according to head_plan
  * (unit = KV head): TRANSFER heads between pools, RELOAD heads from the backup, KEEP heads only when their block was
- * relocated.  Free blocks are never copied. */
+ * relocated.  Free blocks are never copied.
+ * With ETP_OPT_ONLY_PHASE = k > 0 (phase-by-phase runs of a multi-process job) the call reports the evicted sequences but
+ * leaves pt->block_table as it was: every phase call has to lower the plan from the ORIGINAL table (the {old, new} block
+ * pairs come from it), and n_phases of the report tells how many calls there are.  After the last phase the caller obtains
+ * the new table with etp_page_table_rewrite(pt, block_size, new_block_budget, ...), the same host-only rule this call applies. */
 etp_status etp_reshard_kv(etp_ctx* ctx, const etp_kv_geometry* geom, etp_page_table* pt, const etp_plan* head_plan,
                           int32_t new_block_budget, int32_t* evicted_seqs_out, int32_t* n_evicted,
                           void* copy_stream, void* reload_stream, etp_reshard_report* report);
@@ -296,8 +307,9 @@ etp_status etp_shard_linear_multi(etp_ctx* ctx, etp_dtype dtype, const void* x, 
  * column- and row-parallel modes and have their own x and y each - and one launch per linear above 64 tokens.  The plan keeps
  * copies of the descriptors (not of the weights): the slabs must stay where they were.  Results equal etp_shard_linear's up to
  * the fp32 summation order of the K split (column-parallel outputs stay bitwise independent of the shard layout, reading G3).
- * A plan belongs to its ctx, is freed with etp_linear_free (before the ctx) and is used from one host thread at a time; runs on
- * different streams may overlap (the split-K workspace is per stream). */
+ * A plan belongs to its ctx and is used from one host thread at a time; runs on different streams may overlap (the split-K
+ * workspace is per stream).  etp_linear_run needs the ctx alive; etp_linear_free is also safe after etp_ctx_destroy (it touches
+ * only the plan's own device table). */
 typedef struct etp_linear_plan etp_linear_plan;
 typedef struct {
     int32_t mode;               /* etp_linear_mode                                                                    */
@@ -380,7 +392,9 @@ etp_status etp_eplb_place(const int64_t* expert_load, const int32_t* home_rank, 
  * unit of d's shard under `layout` and was not given to an earlier replica of this call) receives a copy of e's unit from its
  * home rank, in EVERY tensor of the class (e.g. gate, up, down of a layer; all must share total_units and, rank by rank, the
  * slab geometry, so a replica has ONE slot).  One launch of the interval-copy kernel on `stream`; slots_out[i] (host) = the
- * slot of replica i.  ETP_ERR_CAPACITY if a rank has no spare slot. */
+ * slot of replica i.  ETP_ERR_CAPACITY if a rank has no spare slot; ETP_ERR_INVALID_ARG if an (expert, rank) pair is listed twice or
+ * the rank is the expert's home.  The spare slots are derived from `layout` alone: the call does not know what an EARLIER call put
+ * into them, so pass ALL replicas of a layout in ONE call (a second call on the same layout reuses, i.e. overwrites, the same slots). */
 etp_status etp_eplb_apply(etp_ctx* ctx, const etp_tensor* tensors, int32_t n_tensors, const etp_shard* layout, int32_t n_shards,
                           const etp_replica* replicas, int32_t n_replicas, int64_t* slots_out, void* stream);
 

@@ -466,7 +466,7 @@ class LinearPlan:
         return d
 
     def close(self) -> None:
-        if getattr(self, "handle", None) and _lib is not None and getattr(self.ctx, "handle", None):
+        if getattr(self, "handle", None) and _lib is not None:      # also after the ctx was closed: the free needs only the plan
             _lib.etp_linear_free(self.handle)
         self.handle = None
 

@@ -273,6 +273,8 @@ etp_status execute(etp_ctx* c, LoweredWork* w, void* copy_stream_v, void* reload
     cudaStream_t caller_cs = (cudaStream_t)copy_stream_v, caller_rs = (cudaStream_t)reload_stream_v;
     CtxExtra* x = extra(c);
     reset_interval_timing(c);
+    note_slab_write(c, copy_stream_v);     // the next small-token linear launch on these streams must not prefetch weights early
+    note_slab_write(c, reload_stream_v);
     const size_t n_dev = x->dev.size();
     const bool multi = n_dev > 1;
     const bool skip_d2d = c->opts[ETP_OPT_SKIP_D2D] != 0, skip_reload = c->opts[ETP_OPT_SKIP_RELOAD] != 0;
@@ -625,7 +627,11 @@ extern "C" etp_status etp_reshard_kv(etp_ctx* ctx, const etp_kv_geometry* geom, 
     ETP_TRY(lower_kv(ctx, geom, head_plan, pairs.data(), n_pairs, &w));
     w.rep.lower_ms = now_ms() - t0;
     ETP_TRY(execute(ctx, &w, copy_stream, reload_stream, report));   // capacity checks come before its first enqueue
-    if (table_n) std::memcpy(pt->block_table, table.data(), table_n * sizeof(int32_t));
+    // Phase-by-phase runs (ETP_OPT_ONLY_PHASE = k > 0): every phase call must lower the SAME plan, i.e. see the ORIGINAL table - a
+    // rewritten one would give identity {old, new} pairs and the later phases would read the source pools at the new block ids.  So
+    // such a call leaves the caller's table alone (the eviction list, a pure function of the inputs, is still reported); the caller
+    // applies etp_page_table_rewrite itself after the last phase (include/etp.h).
+    if (table_n && ctx->opts[ETP_OPT_ONLY_PHASE] == 0) std::memcpy(pt->block_table, table.data(), table_n * sizeof(int32_t));
     *n_evicted = n_ev;
     if (evicted_seqs_out)
         for (int32_t i = 0; i < n_ev; ++i) evicted_seqs_out[i] = ev[i];

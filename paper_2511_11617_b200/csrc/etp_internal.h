@@ -123,6 +123,11 @@ struct etp_ctx {
     int32_t launches = 0;               // kernels launched by the last call
     void* iv_state = nullptr;           // device-side lowering of etp_copy_intervals (etp_lower_dev.cu)
     void* lin_state = nullptr;          // kernel (c): per-stream split-K workspaces + the cache of prepared groups (etp_linear_group.cu)
+    // Streams on which a call of this library that WRITES slabs (reshard, EPLB replicas, interval copies) was enqueued since the last
+    // <= 64-token shard-linear launch on that stream.  Such a launch prefetches weight tiles before griddepcontrol.wait when it carries
+    // the programmatic-serialization attribute, and CUDA makes the previous kernel's writes visible only after that wait: the first
+    // linear launch behind a slab write therefore goes out WITHOUT the attribute (plain stream order), see etp::take_slab_write.
+    std::vector<void*> slab_write_streams;
 };
 
 namespace etp {
@@ -156,6 +161,26 @@ void free_interval_state(etp_ctx* ctx);
 int interval_timed_launches(etp_ctx* ctx, double* ms);
 void reset_interval_timing(etp_ctx* ctx);
 void reset_device_timing(etp_ctx* ctx);   // forgets the timing events of the last executor call (etp_exec.cu)
+
+inline void note_slab_write(etp_ctx* c, void* stream) {
+    for (void* s : c->slab_write_streams)
+        if (s == stream) return;
+    c->slab_write_streams.push_back(stream);
+}
+// true (and forgets it) if a slab write is pending on `stream`, or on the legacy default stream (NULL), which orders against every
+// blocking stream
+inline bool take_slab_write(etp_ctx* c, void* stream) {
+    bool hit = false;
+    for (size_t i = 0; i < c->slab_write_streams.size();) {
+        if (c->slab_write_streams[i] == stream || c->slab_write_streams[i] == nullptr) {
+            hit = true;
+            c->slab_write_streams.erase(c->slab_write_streams.begin() + (long)i);
+        } else {
+            ++i;
+        }
+    }
+    return hit;
+}
 
 // kernel (c): frees the ctx-owned cache of prepared groups and the split-K workspaces (etp_linear_group.cu)
 void lin_teardown(etp_ctx* ctx);

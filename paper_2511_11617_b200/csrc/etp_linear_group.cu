@@ -388,6 +388,7 @@ LinState* lin_state(etp_ctx* c) {
 // ------------------------------------------------------------------------------------------------ the plan object
 struct etp_linear_plan {
     etp_ctx* ctx = nullptr;
+    int device = 0;                         // CUDA device of d_table (kept here so that etp_linear_free never dereferences ctx)
     etp_dtype dtype = ETP_BF16;
     int n_lins = 0;
     struct Lin {
@@ -507,6 +508,7 @@ extern "C" etp_status etp_linear_prepare(etp_ctx* ctx, etp_dtype dtype, const et
     std::unique_ptr<etp_linear_plan> P(new (std::nothrow) etp_linear_plan());
     if (!P) ETP_FAIL(ETP_ERR_NOMEM, "etp_linear_prepare: out of memory");
     P->ctx = ctx;
+    P->device = ctx->device;
     P->dtype = dtype;
     P->n_lins = n_lins;
     std::memset(&P->p, 0, sizeof(P->p));
@@ -659,7 +661,7 @@ extern "C" etp_status etp_linear_prepare(etp_ctx* ctx, etp_dtype dtype, const et
 extern "C" void etp_linear_free(etp_linear_plan* plan) {
     if (!plan) return;
     if (plan->d_table) {
-        cudaSetDevice(plan->ctx->device);
+        cudaSetDevice(plan->device);   // not plan->ctx->device: a plan may outlive its ctx up to this call
         cudaFree(plan->d_table);   // synchronises with the kernels that may still read the table
     }
     delete plan;
@@ -719,7 +721,8 @@ extern "C" etp_status etp_linear_run(etp_linear_plan* P, const void* const* x, i
         p.tickets = w.tickets;
     }
     ctx->launches = 1;
-    const bool pdl = ctx->opts[ETP_OPT_LINEAR_PDL] != 0;
+    // behind a slab write of this library on the same stream the launch keeps plain stream order once (etp_internal.h)
+    const bool pdl = !etp::take_slab_write(ctx, stream) && ctx->opts[ETP_OPT_LINEAR_PDL] != 0;
     return launch_group(p, bn, P->grid, st, pdl, P->half_ring);
 }
 

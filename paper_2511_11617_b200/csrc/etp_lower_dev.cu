@@ -290,6 +290,7 @@ etp_status copy_intervals_device(etp_ctx* c, const etp_interval* host_descs, int
     ETP_CUDA_OK(cudaSetDevice(c->device));
     IvState* S = nullptr;
     ETP_TRY(ensure_state(c, &S));
+    note_slab_write(c, stream_v);
     S->n_timed = 0;
     const long long tma_min = c->opts[ETP_OPT_TMA_MIN_BYTES];
     const int grid = c->opts[ETP_OPT_GRID_CTAS] > 0 ? (int)c->opts[ETP_OPT_GRID_CTAS] : c->n_sms;

@@ -859,6 +859,15 @@ extern "C" etp_status etp_eplb_apply(etp_ctx* ctx, const etp_tensor* tensors, in
             ETP_TRY(home_of(&T0, sh, u, &r, &slot));
             taken[r][(size_t)slot] = 1;
         }
+    // the same (expert, rank) twice would burn a second slot for a copy no routing convention can address
+    {
+        std::vector<std::pair<int32_t, int32_t>> seen((size_t)n_replicas);
+        for (int32_t i = 0; i < n_replicas; ++i) seen[(size_t)i] = {replicas[i].expert, replicas[i].rank};
+        std::sort(seen.begin(), seen.end());
+        for (int32_t i = 1; i < n_replicas; ++i)
+            if (seen[(size_t)i] == seen[(size_t)i - 1])
+                ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_eplb_apply: replica (expert %d, rank %d) is listed twice", seen[(size_t)i].first, seen[(size_t)i].second);
+    }
     LoweredWork w;
     w.dev.resize((size_t)n_logical_devices(ctx));
     for (int32_t i = 0; i < n_replicas; ++i) {

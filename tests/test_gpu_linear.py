@@ -550,6 +550,60 @@ def test_linear_plans_on_two_streams_do_not_share_a_workspace(ctx):
     plan.close()
 
 
+@pytest.mark.parametrize("mode,K,N", [("col", 2048, 1536), ("row", 2048, 1536)])
+def test_linear_right_behind_a_slab_write_on_the_same_stream(ctx, mode, K, N):
+    """The <= 64-token kernel prefetches its first ring of weight tiles before griddepcontrol.wait when it is launched with the
+    programmatic-serialization attribute, and the previous kernel's writes are only guaranteed visible after that wait.  The
+    library therefore sends the first linear launch behind one of its own slab writes on that stream in plain stream order
+    (ETP_OPT_LINEAR_PDL in include/etp.h).  Here the whole weight is REWRITTEN in place by etp_copy_intervals and the linear is
+    enqueued right behind it, no sync, eight times with fresh weights: every output must follow the weights of its round."""
+    T = 4
+    dt = torch_dtype("bf16")
+    widths = (K // 4, K // 2, K // 4) if mode == "row" else (N // 4, N // 2, N // 4)
+    lin, w_u8, bufs = _make_linear(mode, K, N, 1, widths, 80, "tight")
+    plan = etp.LinearPlan(ctx, [lin])
+    x = torch.from_numpy(as_u8(fill_normal16(SEED, 1300, 0, T * K, 1.0, dt)).copy()).cuda()
+    stream = torch.cuda.Stream()
+    layout = widths_to_layout(widths)
+    ub = (N if mode == "row" else K) * 2
+    rounds = []
+    for i in range(8):
+        w_i = as_u8(fill_normal16(SEED, 1310 + i, 0, K * N, 0.02, dt)).copy()
+        staged = torch.from_numpy(w_i).cuda()
+        y = torch.zeros(T * N * 2, dtype=torch.uint8, device="cuda")
+        rounds.append((w_i, staged, y))
+    torch.cuda.synchronize()
+    for w_i, staged, y in rounds:
+        src = np.array([staged.data_ptr() + b * ub for (r, b, e, _) in layout], dtype=np.int64)
+        dst = np.array([bufs[r].ptr for (r, b, e, _) in layout], dtype=np.int64)
+        sz = np.array([(e - b) * ub for (r, b, e, _) in layout], dtype=np.int64)
+        etp.etp_copy_intervals(ctx, src, dst, sz, stream.cuda_stream)
+        plan.run(x.data_ptr(), T, [y.data_ptr()], stream.cuda_stream)
+    stream.synchronize()
+    for i, (w_i, staged, y) in enumerate(rounds):
+        check(y.cpu().numpy(), reference("bf16", x.cpu().numpy(), w_i, T, K, N, mode == "row"), "bf16", T, N)
+    plan.close()
+
+
+def test_linear_plan_may_be_freed_after_its_ctx():
+    """etp_linear_free touches only the plan's own device table (the device id is kept in the plan), so freeing a plan after
+    etp_ctx_destroy is safe; the wrapper no longer leaks such plans."""
+    own = etp.Context(0)
+    lin, w_u8, keep = _make_linear("col", 256, 512, 1, (171, 171, 170), 70, "tight")
+    plan = etp.LinearPlan(own, [lin])
+    x = torch.from_numpy(as_u8(fill_normal16(SEED, 1200, 0, 4 * 256, 1.0, torch_dtype("bf16"))).copy()).cuda()
+    y = torch.zeros(4 * 512 * 2, dtype=torch.uint8, device="cuda")
+    plan.run(x.data_ptr(), 4, [y.data_ptr()], 0)
+    torch.cuda.synchronize()
+    check(y.cpu().numpy(), reference("bf16", x.cpu().numpy(), w_u8, 4, 256, 512, False), "bf16", 4, 512)
+    own.close()
+    assert plan.handle
+    plan.close()
+    assert plan.handle is None
+    free0 = torch.cuda.mem_get_info()[0]
+    assert free0 > 0                       # the device is still usable
+
+
 def test_linear_prepare_errors(ctx):
     lin, _, keep = _make_linear("col", 256, 512, 1, (171, 171, 170), 70, "tight")
     with pytest.raises(etp.EtpError) as e:
@@ -671,6 +725,9 @@ def _moe_layer_with_eplb_replicas(ctx):
                 if d == r:
                     exp[s * ub:(s + 1) * ub] = ws[k][ex * ub:(ex + 1) * ub]
             assert b.guards_intact() and np.array_equal(b.payload(), exp), f"{k} rank {r}"
+    with pytest.raises(etp.EtpError) as err:                        # the same (expert, rank) twice: refused, nothing enqueued
+        etp.etp_eplb_apply(ctx, [descs["gate"], descs["up"], descs["down_t"]], layout, list(replicas) + [replicas[0]])
+    assert err.value.status == 1 and "twice" in str(err.value)
     # instances: home first, then replicas in creation order; rows split evenly (oracle.eplb.split_rows)
     slot_of = {(ex, d): s for (ex, d), s in zip(replicas, slots)}
     inst = []

@@ -106,6 +106,63 @@ def test_kv_partitioned_by_destination_device(layout):
         ctx.close()
 
 
+@pytest.mark.parametrize("form", ["two_contexts", "three_devices"])
+@pytest.mark.parametrize("budget_delta", [3, -10])
+def test_kv_phase_by_phase_keeps_the_original_table(form, budget_delta):
+    """ETP_OPT_ONLY_PHASE on a KV reshard that needs several hazard phases AND relocates blocks (tight head_cap = the wider shard,
+    so a reloaded head lands in the slot another rank still has to read; a block budget that moves live blocks, and with -10 also
+    evicts).  Every phase call must lower the plan from the ORIGINAL page table: the call therefore leaves the caller's table
+    alone (include/etp.h) - were it rewritten by the phase-1 call, phase 2 would see identity {old, new} pairs and read the
+    source pools at the new block ids.  Run as two contexts that each write their own ranks, and as one ctx over three logical
+    devices; after the last phase the caller's etp_page_table_rewrite gives the table, and pools / evictions match the oracle."""
+    cfg = dataclasses.replace(MID, model=dataclasses.replace(MID.model, n_layers=2))
+    world = H.build_kv_world(cfg, side=LibSide, layout=0, seq_lens=[300, 7, 1000])      # head_cap = max shard width (3): tight
+    st, g = world.steps[0], world.g
+    assert g.head_cap == 3
+    live = int(((world.seq_lens + 15) // 16).sum())
+    budget = live + budget_delta
+    new_table, evicted, pairs = OS.page_table_rewrite(world.table, world.seq_lens, world.last_use, g.block_size, budget)
+    assert any(p[2] != p[3] for p in pairs) and (budget_delta > 0 or evicted)          # (seq, index, old id, new id)
+    snap = {r: p for r, p in world.pools.items() if r != st.dead}
+    expect, stats = OS.apply_kv(st.tasks["head"], snap, world.anchors, g, world.host_backup, world.host_heads, world.host_head0, pairs)
+    bufs = {r: DevBuf(p) for r, p in snap.items()}
+    img = pinned(world.host_backup)
+    if form == "two_contexts":
+        ctxs, maps = [etp.Context(0), etp.Context(0)], ([0, -1, -1, 0], [-1, 0, 0, -1])
+    else:
+        ctxs, maps = [etp.Context(devices=[0, 0, 0])], ([0, 1, 2, 0],)
+    try:
+        for c, m in zip(ctxs, maps):
+            c.set_rank_devices(m)
+        streams = [Streams() for _ in ctxs]
+        table = world.table.copy()
+        phase, n_phases, reps = 0, 1, [None] * len(ctxs)
+        while phase < n_phases:
+            for i, (c, s) in enumerate(zip(ctxs, streams)):
+                c.set_option(etp.OPT_ONLY_PHASE, phase + 1)
+                ev, reps[i] = etp.etp_reshard_kv(c, n_layers=g.n_layers, n_blocks=g.n_blocks, block_size=g.block_size, head_cap=g.head_cap,
+                                                 head_dim=g.head_dim, elem_bytes=g.elem_bytes, layout=g.layout,
+                                                 pools={r: b.ptr for r, b in bufs.items()}, head_anchor=world.anchors, n_ranks=4, table=table,
+                                                 seq_lens=world.seq_lens, last_use=world.last_use, head_plan=make_plans(st)["head"],
+                                                 new_block_budget=budget, host_backup=img.data_ptr(), host_heads=world.host_heads,
+                                                 host_head0=world.host_head0, copy_stream=s.copy.cuda_stream, reload_stream=s.reload.cuda_stream)
+                n_phases = reps[i]["n_phases"]
+                assert ev == evicted                                    # reported by every phase call
+                assert np.array_equal(table, world.table)               # ... and the table is still the original one
+            for s in streams:
+                s.sync()                                                # the barrier between hazard phases
+            phase += 1
+        assert n_phases >= 2
+        ev2, pairs2 = etp.etp_page_table_rewrite(table, world.seq_lens, world.last_use, g.block_size, budget)
+        assert ev2 == evicted and np.array_equal(table, new_table)
+        for r, b in bufs.items():
+            assert b.guards_intact() and b.payload().tobytes() == expect[r].tobytes(), f"pool of rank {r} differs from the oracle image"
+        assert sum(r["d2d_bytes"] for r in reps) == stats["d2d_bytes"] and sum(r["h2d_bytes"] for r in reps) == stats["h2d_bytes"]
+    finally:
+        for c in ctxs:
+            c.close()
+
+
 @pytest.mark.parametrize("mode", ["span", "tight"])
 def test_one_context_per_rank_group_pulls_only_its_own_destinations(mode):
     """The one-process-per-GPU form in one process: context A writes ranks {0, 3}, context B ranks {1, 2} (the others are -1

@@ -393,3 +393,25 @@ def test_intervals_validate_threaded_path_finds_one_planted_overlap(n):
     with pytest.raises(etp.EtpError) as e:
         etp.etp_intervals_validate(bad_s, dst, szp)
     assert e.value.status == 1 and " 5" in str(e.value) and str(k) in str(e.value)
+
+
+# ------------------------------------------------------------------------------------------------ bench.py's watchdog
+@pytest.mark.parametrize("mode,attempts,killed,rc", [("ok", 1, 0, 0), ("hang_once", 2, 1, 0), ("hang_after_result", 1, 1, 0), ("hang", None, 2, 1)])
+def test_bench_watchdog_reports_its_retries(tmp_path, mode, attempts, killed, rc):
+    """A hang must be visible in the result line: the child's stdout is forwarded, the last JSON object gets
+    {"watchdog": {"attempts", "killed"}}; a child that printed its result and then hung is not repeated (exactly one result
+    line); two hangs in a row give a non-zero exit code and no result line."""
+    import json
+    import subprocess
+    import sys
+    env = dict(os.environ, ETP_WATCHDOG_SELFTEST_MARK=str(tmp_path / "mark"))
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--watchdog-selftest", mode, "--watchdog-s", "6"],
+                       stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, env=env, timeout=120)
+    assert p.returncode == rc, p.stderr
+    results = [json.loads(ln) for ln in p.stdout.splitlines() if ln.startswith("{")]
+    if attempts is None:
+        assert results == [] and "killed" in p.stderr
+        return
+    assert len(results) == 1 and results[0]["metric"] == "selftest"
+    assert results[0]["watchdog"] == {"attempts": attempts, "killed": killed, "deadline_s": 6.0}
+    assert p.stdout.count("a line that is not the result") == 1
