@@ -81,13 +81,13 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-CAPTURE_CSV = os.path.join("profiles", "r2_copy_kernel_full.csv")
-CAPTURE_MD = os.path.join("profiles", "r2_copy_kernel_full.md")
+CAPTURE_CSV = os.path.join("profiles", "r3_copy_kernel_full.csv")
+CAPTURE_MD = os.path.join("profiles", "r3_copy_kernel_full.md")
 
 
 def ncu_capture_stamp():
     """{commit, kernel_sass_sha} the committed `ncu --set full` capture of kernel (a) was taken at (two `key: value` lines
-    of profiles/r2_copy_kernel_full.md), or None."""
+    of profiles/r3_copy_kernel_full.md), or None."""
     try:
         out = {}
         with open(os.path.join(ROOT, CAPTURE_MD)) as f:
@@ -102,7 +102,7 @@ def ncu_capture_stamp():
 
 def ncu_traffic_per_launch():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel (a), from the committed `ncu --set full` capture
-    (profiles/r2_copy_kernel_full.csv: one parameter launch + one KV launch of this workload), or None."""
+    (profiles/r3_copy_kernel_full.csv: one parameter launch + one KV launch of this workload), or None."""
     p = os.path.join(ROOT, CAPTURE_CSV)
     try:
         rows = {}
@@ -120,7 +120,7 @@ def ncu_traffic_per_launch():
 
 def traffic_source():
     """Where roofline.traffic comes from and whether it still describes the kernel that was just timed: the capture's commit
-    and SASS hash (profiles/r2_copy_kernel_full.md) beside the SASS hash of etp_interval_copy_kernel in the loaded libetp.so."""
+    and SASS hash (profiles/r3_copy_kernel_full.md) beside the SASS hash of etp_interval_copy_kernel in the loaded libetp.so."""
     stamp = ncu_capture_stamp() or {}
     try:
         from paper_2511_11617_b200 import _build

@@ -414,6 +414,17 @@ etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_descs, int6
  * small sorts, on up to 16 threads from 65536 intervals. */
 etp_status etp_intervals_validate(const etp_interval* host_descs, int64_t n);
 
+/* ------------------------------------------------------------------------------------------------ liveness (debug entry)
+ * Every spin wait inside the kernels of this library is an mbarrier wait with a deadline: a wait that is still unsatisfied after
+ * 10 s (a lost arrival, a wrong byte count: a bug, not a load condition) writes {kernel family, block, thread, barrier, parity, time
+ * waited} to host memory and traps.  The launch fails with a sticky CUDA error, so the next synchronising call of the caller and every
+ * later call of this library fail (ETP_ERR_CUDA) instead of hanging, and etp_last_error() carries the record.  The CUDA context is
+ * lost after a trap: the process has to be restarted, as after any device-side fault.
+ * etp_debug_starved_wait proves the mechanism: it launches a kernel that waits, with the very wait routine the copy kernel uses, on a
+ * barrier nobody arrives on, and synchronises `stream`.  Expected result: ETP_ERR_CUDA after about 10 s with the record in
+ * etp_last_error().  It POISONS THE PROCESS'S CUDA CONTEXT: call it from a throw-away process only (tests/test_gpu_stress.py). */
+etp_status etp_debug_starved_wait(etp_ctx* ctx, void* stream);
+
 /* ------------------------------------------------------------------------------------------------ no-allocation entry
  * etp_copy_intervals for a caller that cannot allocate device memory.  Such callers are the normal case on the recovery path this
  * library serves ("a single pass pre-allocates all destination buffers"): when a rank dies the survivors' HBM is already

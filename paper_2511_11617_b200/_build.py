@@ -14,6 +14,11 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std
          "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 
 
+# debug build: ETP_BOUNDED_WAITS=1 in the environment also bounds the mbarrier waits of the tcgen05 kernels (csrc/etp_wait.cuh; kernel (a)'s are always bounded)
+if os.environ.get("ETP_BOUNDED_WAITS"):
+    FLAGS = FLAGS + ["-DETP_BOUNDED_WAITS=" + os.environ["ETP_BOUNDED_WAITS"]]
+
+
 def _stale() -> bool:
     if not os.path.exists(SO):
         return True

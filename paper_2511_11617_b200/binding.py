@@ -102,7 +102,7 @@ EXPORTS = ["etp_ctx_create", "etp_ctx_create_multi", "etp_ctx_set_rank_devices",
            "etp_plan_get_stats", "etp_plan_slab_span", "etp_plan_free", "etp_reshard_params", "etp_page_table_rewrite", "etp_reshard_kv", "etp_shard_linear",
            "etp_shard_linear_multi", "etp_linear_prepare", "etp_linear_run", "etp_linear_plan_info", "etp_linear_free",
            "etp_moe_linear", "etp_moe_linear_instances", "etp_moe_gate_up", "etp_eplb_place", "etp_eplb_apply", "etp_copy_intervals", "etp_intervals_validate",
-           "etp_copy_intervals_static"]
+           "etp_copy_intervals_static", "etp_debug_starved_wait"]
 
 _lib = None
 
@@ -159,6 +159,7 @@ def lib() -> C.CDLL:
         L.etp_copy_intervals.argtypes = [vp, C.POINTER(etp_interval), i64, vp, C.POINTER(etp_reshard_report)]
         L.etp_intervals_validate.argtypes = [C.POINTER(etp_interval), i64]
         L.etp_copy_intervals_static.argtypes = [C.POINTER(etp_interval), i64, vp]
+        L.etp_debug_starved_wait.argtypes = [vp, vp]
         _lib = L
     return _lib
 
@@ -590,3 +591,9 @@ def etp_copy_intervals_static(src_ptrs, dst_ptrs, sizes, stream: int = 0) -> Non
     engine's pool owns all free HBM, code inside somebody else's CUDA context): no Context, at most 4096 intervals per call, runs on
     the current CUDA device.  Calls share one static scratch array: keep them on one stream or order them yourself (include/etp.h)."""
     IntervalList(src_ptrs, dst_ptrs, sizes).run_static(stream)
+
+
+def etp_debug_starved_wait(ctx: Context, stream: int = 0) -> None:
+    """Launches a kernel that waits on a barrier nobody arrives on: raises EtpError(ETP_ERR_CUDA) with the fault record after about
+    10 s.  The CUDA context of the process is lost afterwards: throw-away processes only."""
+    _check(lib().etp_debug_starved_wait(ctx.handle, stream or None))

@@ -1,4 +1,6 @@
+#define ETP_WAIT_TU 1
 #include "etp_copy.cuh"
+#include "etp_wait.cuh"
 
 namespace etp {
 namespace {
@@ -11,18 +13,8 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\t"
-        "bra WAIT_%=;\n\t"
-        "DONE_%=:\n\t"
-        "}" ::"r"(bar), "r"(parity)
-        : "memory");
-}
+// bounded (etp_wait.cuh): 65536 inline tries, then a slow path that records and traps after kWaitBudgetNs instead of spinning forever
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) { mbar_wait_bounded(bar, parity); }
 // global -> shared, completion counted in bytes on an mbarrier
 __device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, uint64_t src_gmem, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem),
@@ -484,7 +476,19 @@ __global__ void __launch_bounds__(kCopyThreads, 1) etp_interval_copy_kernel(cons
     }
 }
 
+// debug: a barrier nobody arrives on, waited for with the same mbar_wait as the kernels (etp_debug_starved_wait)
+__global__ void etp_starved_wait_kernel() {
+    __shared__ uint64_t bar;
+    if (threadIdx.x == 0) {
+        mbar_init(smem_u32(&bar), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_wait(smem_u32(&bar), 0);
+    }
+}
 }  // namespace
+
+cudaError_t install_wait_fault_copy(unsigned long long* rec) { return wait_fault_install(rec); }
+void launch_starved_wait_kernel(cudaStream_t stream) { etp_starved_wait_kernel<<<3, 64, 0, stream>>>(); }
 
 cudaError_t configure_copy_kernel() {
     cudaError_t e = cudaFuncSetAttribute(etp_interval_copy_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCopySmemBytes);

@@ -131,6 +131,19 @@ extern "C" etp_status etp_ctx_create_multi(const int32_t* devices, int32_t n_dev
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&D.slot[k].done_reload, cudaEventDisableTiming);
         }
         if (e == cudaSuccess) e = configure_copy_kernel();   // a per-device function attribute
+        if (e == cudaSuccess && !g_wait_fault_host) {          // once per process: the fault record of the bounded waits (etp_wait.cuh)
+            void* rec = nullptr;
+            e = cudaHostAlloc(&rec, 64, cudaHostAllocPortable | cudaHostAllocMapped);
+            if (e == cudaSuccess) {
+                std::memset(rec, 0, 64);
+                g_wait_fault_host = static_cast<volatile unsigned long long*>(rec);
+            }
+        }
+        unsigned long long* rec = const_cast<unsigned long long*>(g_wait_fault_host);   // UVA: the host address is the device address
+        if (e == cudaSuccess) e = install_wait_fault_copy(rec);
+        if (e == cudaSuccess) e = install_wait_fault_linear(rec);
+        if (e == cudaSuccess) e = install_wait_fault_group(rec);
+        if (e == cudaSuccess) e = install_wait_fault_moe(rec);
     }
     cudaSetDevice(devices[0]);
     if (e != cudaSuccess) {
@@ -636,6 +649,15 @@ extern "C" etp_status etp_reshard_kv(etp_ctx* ctx, const etp_kv_geometry* geom, 
     if (evicted_seqs_out)
         for (int32_t i = 0; i < n_ev; ++i) evicted_seqs_out[i] = ev[i];
     return ETP_OK;
+}
+
+extern "C" etp_status etp_debug_starved_wait(etp_ctx* ctx, void* stream) {
+    if (!ctx) ETP_FAIL(ETP_ERR_INVALID_ARG, "etp_debug_starved_wait: ctx is NULL");
+    ETP_CUDA_OK(cudaSetDevice(ctx->device));
+    launch_starved_wait_kernel((cudaStream_t)stream);
+    ETP_CUDA_OK(cudaGetLastError());
+    ETP_CUDA_OK(cudaStreamSynchronize((cudaStream_t)stream));   // returns the trap as a sticky error -> ETP_ERR_CUDA + the record
+    ETP_FAIL(ETP_ERR_UNSUPPORTED, "etp_debug_starved_wait: the starved kernel returned without an error");
 }
 
 extern "C" etp_status etp_copy_intervals(etp_ctx* ctx, const etp_interval* host_descs, int64_t n, void* stream,

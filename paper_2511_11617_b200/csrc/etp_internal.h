@@ -182,6 +182,15 @@ inline bool take_slab_write(etp_ctx* c, void* stream) {
     return hit;
 }
 
+// Bounded waits (etp_wait.cuh): the fault record is 8 x u64 of host-mapped pinned memory, allocated once per process by the first
+// etp_ctx_create and installed into every kernel translation unit on every device of a ctx.  set_error appends it to the message.
+extern volatile unsigned long long* g_wait_fault_host;   // etp_plan.cpp; NULL until a ctx exists
+cudaError_t install_wait_fault_copy(unsigned long long* rec);
+cudaError_t install_wait_fault_linear(unsigned long long* rec);
+cudaError_t install_wait_fault_group(unsigned long long* rec);
+cudaError_t install_wait_fault_moe(unsigned long long* rec);
+void launch_starved_wait_kernel(cudaStream_t stream);
+
 // kernel (c): frees the ctx-owned cache of prepared groups and the split-K workspaces (etp_linear_group.cu)
 void lin_teardown(etp_ctx* ctx);
 

@@ -24,6 +24,7 @@
 #include <cstring>
 #include <vector>
 
+#define ETP_WAIT_TU 2
 #include "etp_linear.cuh"
 
 using namespace etp;
@@ -757,3 +758,7 @@ extern "C" etp_status etp_shard_linear_multi(etp_ctx* ctx, etp_dtype dtype, cons
     for (int32_t o = 0; o < n_outs; ++o) lo[o] = {outs[o].w, outs[o].out_features, outs[o].features_per_unit, outs[o].y};
     return shard_linear_impl(ctx, ETP_COL_PARALLEL, dtype, x, tokens, in_features, lo, n_outs, layout, n_shards, stream);
 }
+
+namespace etp {
+cudaError_t install_wait_fault_linear(unsigned long long* rec) { return wait_fault_install(rec); }
+}  // namespace etp

@@ -26,6 +26,7 @@
 #include <unordered_map>
 #include <vector>
 
+#define ETP_WAIT_TU 3
 #include "etp_linear.cuh"
 
 using namespace etp;
@@ -776,4 +777,8 @@ etp_status shard_linear_small(etp_ctx* ctx, etp_linear_mode mode, etp_dtype dtyp
 }
 
 }  // namespace lin
+}  // namespace etp
+
+namespace etp {
+cudaError_t install_wait_fault_group(unsigned long long* rec) { return wait_fault_install(rec); }
 }  // namespace etp

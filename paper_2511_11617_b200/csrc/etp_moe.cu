@@ -17,6 +17,7 @@
 #include <cstring>
 #include <vector>
 
+#define ETP_WAIT_TU 4
 #include "etp_tc.cuh"
 
 using namespace etp;
@@ -909,3 +910,7 @@ extern "C" void etp_moe_timing_dump(unsigned long long* out, int reset) {
     }
 }
 #endif
+
+namespace etp {
+cudaError_t install_wait_fault_moe(unsigned long long* rec) { return wait_fault_install(rec); }
+}  // namespace etp

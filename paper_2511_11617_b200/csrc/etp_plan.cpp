@@ -12,11 +12,22 @@
 
 namespace etp {
 static thread_local char g_err[512] = "";
+volatile unsigned long long* g_wait_fault_host = nullptr;
 void set_error(const char* fmt, ...) {
     va_list ap;
     va_start(ap, fmt);
-    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    int n = vsnprintf(g_err, sizeof(g_err), fmt, ap);
     va_end(ap);
+    // a kernel that gave up on a starved barrier left a record in host memory (etp_wait.cuh): every error after it says so
+    volatile unsigned long long* r = g_wait_fault_host;
+    if (r && r[0] == 0x4554504641554c54ull && n >= 0 && n < (int)sizeof(g_err) - 1) {
+        static const char* const family[] = {"?", "interval copy (etp_copy.cu)", "shard linear (etp_linear.cu)", "grouped linear (etp_linear_group.cu)",
+                                             "MoE (etp_moe.cu)"};
+        snprintf(g_err + n, sizeof(g_err) - (size_t)n,
+                 " [device wait starved: %s kernel, block %llu thread %llu gave up on mbarrier 0x%llx parity %llu after %.1f s and trapped; the "
+                 "CUDA context is lost]",
+                 family[r[1] <= 4 ? r[1] : 0], r[2], r[3], r[4], r[5], (double)r[6] * 1e-9);
+    }
 }
 }  // namespace etp
 

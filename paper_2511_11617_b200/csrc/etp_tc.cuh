@@ -6,6 +6,7 @@
 #include <cuda_fp16.h>
 
 #include "etp_internal.h"
+#include "etp_wait.cuh"
 
 namespace etp {
 namespace tc {
@@ -31,18 +32,8 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\t"
-        "bra WAIT_%=;\n\t"
-        "DONE_%=:\n\t"
-        "}" ::"r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-}
+// etp_wait.cuh: the plain try_wait loop, or (builds with ETP_BOUNDED_WAITS=1) the bounded wait that records and traps after kWaitBudgetNs
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) { etp::mbar_wait_bounded(smem_u32(bar), parity); }
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int32_t c0, int32_t c1) {
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(

@@ -118,3 +118,44 @@ def test_multi_phase_reshard_repeats_bit_for_bit(ctx, image):
         rep = TR.run_param_step(ctx, world, bufs, images, 0, streams)
         TR.compare_params(world, bufs, expect, {world.steps[0].dead})
         assert rep["d2d_bytes"] == stats["d2d_bytes"] and rep["n_phases"] >= 2
+
+
+# ------------------------------------------------------------------------------------------------ liveness of the hand-rolled waits
+def test_starved_barrier_fails_loudly_within_seconds():
+    """Every spin wait of the kernels is an mbarrier wait with a 10-s deadline (csrc/etp_wait.cuh).  etp_debug_starved_wait launches a
+    kernel that waits - with the copy kernel's own wait routine - on a barrier nobody arrives on: the call must come back with
+    ETP_ERR_CUDA and a record naming the kernel family, block, thread and barrier within seconds (not hang until the pool is reset),
+    and every later call must fail as well.  The CUDA context is lost afterwards, so the whole thing runs in a throw-away process."""
+    import json
+    import subprocess
+    import sys
+    code = r'''
+import json, os, sys, time
+import paper_2511_11617_b200 as etp
+c = etp.Context(0)
+out = {}
+t0 = time.time()
+try:
+    etp.etp_debug_starved_wait(c)
+    out["first"] = "no error"
+except etp.EtpError as e:
+    out["first"] = [e.status, str(e)]
+out["seconds"] = time.time() - t0
+try:
+    etp.Context(0)
+    out["later"] = "no error"
+except etp.EtpError as e:
+    out["later"] = [e.status, str(e)]
+print("RESULT " + json.dumps(out), flush=True)
+os._exit(0)          # no teardown on a dead context
+'''
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    p = subprocess.run([sys.executable, "-c", code], cwd=root, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, timeout=120)
+    lines = [ln for ln in p.stdout.splitlines() if ln.startswith("RESULT ")]
+    assert lines, (p.stdout, p.stderr)
+    out = json.loads(lines[-1][7:])
+    status, msg = out["first"]
+    assert status == 6, out                                         # ETP_ERR_CUDA
+    assert "device wait starved" in msg and "interval copy" in msg and "thread 0 " in msg and "parity 0" in msg, msg
+    assert 9.0 <= out["seconds"] <= 40.0, out
+    assert out["later"] != "no error" and out["later"][0] == 6, out   # the error is sticky: nothing hangs, nothing pretends to work

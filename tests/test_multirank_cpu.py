@@ -100,23 +100,23 @@ def test_ours_fails_loudly_without_a_gpu():
 
 
 def test_roofline_traffic_is_read_from_the_committed_ncu_capture():
-    """bench.py's roofline.traffic comes from profiles/r2_copy_kernel_full.csv (one parameter launch + one KV launch of config 2):
+    """bench.py's roofline.traffic comes from profiles/r3_copy_kernel_full.csv (one parameter launch + one KV launch of config 2):
     the file must stay in the layout the parser reads, and the DRAM bytes must stay near the algorithmic 2 B per moved byte."""
     import bench
     t = bench.ncu_traffic_per_launch()
-    assert t is not None, "profiles/r2_copy_kernel_full.csv is missing or not in the 'metric,unit,launch1,launch2,...' layout"
+    assert t is not None, "profiles/r3_copy_kernel_full.csv is missing or not in the 'metric,unit,launch1,launch2,...' layout"
     algorithmic = 2.0 * (9.425e9 + 5.369e9) / 2.0          # config 2, device-resident images: bytes moved by the two launches
     assert 0.95 < t / algorithmic < 1.10
 
 
 def test_ncu_capture_describes_the_kernel_that_is_built():
-    """A stale capture must not be quoted: profiles/r2_copy_kernel_full.md records the commit and the SASS hash of
+    """A stale capture must not be quoted: profiles/r3_copy_kernel_full.md records the commit and the SASS hash of
     etp_interval_copy_kernel it profiled; the hash is recomputed here from the built libetp.so (cuobjdump -sass).  After any
     change to the copy kernel this test fails until the capture is taken again."""
     import bench
     from paper_2511_11617_b200 import _build
     stamp = bench.ncu_capture_stamp()
-    assert stamp is not None, "profiles/r2_copy_kernel_full.md must carry 'commit: <sha>' and 'kernel_sass_sha: <hash>' lines"
+    assert stamp is not None, "profiles/r3_copy_kernel_full.md must carry 'commit: <sha>' and 'kernel_sass_sha: <hash>' lines"
     _build.build()
     built = _build.kernel_sass_sha("etp_interval_copy_kernel")
     assert stamp["kernel_sass_sha"] == built, (
